@@ -1,0 +1,128 @@
+"""BASELINE.json `configs` as seeded synthetic workloads.
+
+Everything here is input preparation: lattice sites, linear interpolation in
+(fractional coordinates, cell matrix) and additive seeded noise.  Potential
+parameters are plain numbers copied from BASELINE.json; no potential is
+evaluated here.
+"""
+import json
+import os
+from dataclasses import dataclass, field
+
+import numpy as np
+
+from .lattices import fcc_supercell, bcc_supercell, bain_final_cell
+from .noise import splitmix64_normals
+
+POT_LJ_SF = 0
+POT_FS_MORSE = 1
+
+
+def lj_params(eps=1.0, sigma=1.0, rc=2.5):
+    """Lennard-Jones shifted-force parameters: pot[0..2] = eps, sigma, r_c (BASELINE.json configs[0])."""
+    p = np.zeros(12)
+    p[0], p[1], p[2] = eps, sigma, rc
+    return p
+
+
+def fs_params(D=0.3, alpha=1.5, r0=2.5, beta=3.0, rho_r0=2.5, A=0.8, r_on=4.5, r_cut=5.0):
+    """Finnis-Sinclair-type parameters (BASELINE.json configs[2]).
+
+    pot[0..7] = D, alpha, r0 (Morse pair), beta, rho_r0 (density exp(-beta (r - rho_r0))),
+    A (embedding F = -A sqrt(rho)), r_on, r_cut (cosine taper).
+    """
+    p = np.zeros(12)
+    p[:8] = [D, alpha, r0, beta, rho_r0, A, r_on, r_cut]
+    return p
+
+
+@dataclass
+class WorkloadSpec:
+    name: str
+    potential: int
+    pot: np.ndarray
+    lattice: str  # "fcc_vacancy" | "bcc_bain"
+    dims: tuple
+    n_atoms: int
+    n_images: int
+    seed: int
+    noise_sigma: float = 1e-3
+    k_spring: float = 1.0
+    climb: bool = True
+    n_steps: int = 200
+    max_images: int = 0
+    # FIRE (SURVEY.md §8c O7 defaults; dt's are per-config inputs)
+    fire: dict = field(default_factory=dict)
+    skin: float = 0.3
+    max_neighbors: int = 128
+
+    @property
+    def r_cut(self):
+        return float(self.pot[2] if self.potential == POT_LJ_SF else self.pot[7])
+
+
+_FIRE_LJ = dict(dt0=0.01, dtmax=0.05, maxstep=0.1, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+_FIRE_EV = dict(dt0=0.1, dtmax=1.0, maxstep=0.2, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+
+CONFIGS = [
+    WorkloadSpec("c0_lj_vacancy_2x2x2", POT_LJ_SF, lj_params(), "fcc_vacancy", (2, 2, 2), 31, 7, 0,
+                 fire=_FIRE_LJ, n_steps=200, max_images=7, skin=0.3, max_neighbors=128),
+    WorkloadSpec("c1_lj_vacancy_4x4x4", POT_LJ_SF, lj_params(), "fcc_vacancy", (4, 4, 4), 255, 9, 1,
+                 fire=_FIRE_LJ, n_steps=2000, max_images=9, skin=0.3, max_neighbors=128),
+    WorkloadSpec("c2_fs_bain_2048", POT_FS_MORSE, fs_params(), "bcc_bain", (8, 8, 16), 2048, 16, 2,
+                 fire=_FIRE_EV, n_steps=200, max_images=16, skin=0.3, max_neighbors=192),
+    WorkloadSpec("c3_fs_bain_9826_adaptive", POT_FS_MORSE, fs_params(), "bcc_bain", (17, 17, 17), 9826, 12, 3,
+                 fire=_FIRE_EV, n_steps=200, max_images=32, skin=0.3, max_neighbors=192),
+    WorkloadSpec("c4_fs_bain_101306", POT_FS_MORSE, fs_params(), "bcc_bain", (37, 37, 37), 101306, 100, 4,
+                 fire=_FIRE_EV, n_steps=500, max_images=100, skin=0.3, max_neighbors=192),
+]
+
+
+def load_lattice_constants():
+    """Relaxed lattice constants written by `oracle/make_lattice_constants.py` (calls only oracle/).
+
+    Keys: lj_fcc_a (sigma), fs_bcc_a (Angstrom), fs_fcc_volume_ratio (Omega_fcc / Omega_bcc per atom).
+    """
+    path = os.path.join(os.path.dirname(__file__), "lattice_constants.json")
+    with open(path) as fh:
+        return json.load(fh)
+
+
+def vacancy_endpoints_unrelaxed(n, a):
+    """fcc n^3 conventional cells minus atom 0; final = the atom at (1/2,1/2,0)a of cell 0 moved to the origin.
+
+    Returns (frac_init, cell, frac_final, cell) with N = 4 n^3 - 1 atoms, unrelaxed.
+    """
+    frac, cell = fcc_supercell(n, n, n, a)
+    frac_init = frac[1:].copy()  # remove atom 0 (origin site)
+    frac_final = frac_init.copy()
+    frac_final[0] = frac[0]  # former atom 1 = (1/2,1/2,0)a of cell 0 hops into the vacancy
+    return frac_init, cell, frac_final, cell.copy()
+
+
+def bain_endpoints(dims, a_bcc, volume_ratio=1.0):
+    """bcc supercell and its Bain-strained (c/a = sqrt 2) image; fractional coordinates are identical."""
+    frac, cell = bcc_supercell(dims[0], dims[1], dims[2], a_bcc)
+    return frac, cell, frac.copy(), bain_final_cell(cell, volume_ratio)
+
+
+def linear_path(frac0, cell0, frac1, cell1, n_images, seed, sigma):
+    """Images linear in (fractional coordinates, cell matrix) + Gaussian noise on interior images.
+
+    Returns Cartesian positions pos[P,N,3] = s_p h_p (+ noise, interior only) and cells[P,3,3].
+    Positions are never wrapped.
+    """
+    P = int(n_images)
+    N = frac0.shape[0]
+    pos = np.empty((P, N, 3))
+    cells = np.empty((P, 3, 3))
+    noise = splitmix64_normals(seed, (P - 2) * N * 3).reshape(P - 2, N, 3) * sigma if P > 2 else None
+    for p in range(P):
+        t = p / (P - 1)
+        s = frac0 + t * (frac1 - frac0)
+        h = cell0 + t * (cell1 - cell0)
+        pos[p] = s @ h
+        cells[p] = h
+        if 0 < p < P - 1:
+            pos[p] += noise[p - 1]
+    return pos, cells

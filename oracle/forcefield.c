@@ -1,0 +1,415 @@
+/*
+ * oracle/forcefield.c -- CPU ORACLE, TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, fp64 C restatement of what the CFNEB hot path computes per image:
+ * neighbours under PBC, per-atom energies (Eq. 4),
+ * pair forces f^ij (Eq. 5), total forces and the virial
+ * V = -1/2 sum_ij r^ij (x) f^ij (Eq. 7-8).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+ * legs may load this.  It shares no code with paper_2510_16721_b200/ (the CUDA path).
+ * Compile with -O2 -ffp-contract=off: no FMA contraction, so the
+ * arithmetic below is exactly what is written.
+ *
+ * Conventions: row vectors; h rows = lattice vectors, R = s h
+ * (PAPER.md:41); Rt = R~ = s h0 (Eq. 10); all 3x3 matrices
+ * row-major double[9].  r^ij = r^j - r^i (+ periodic shift), f^ij = force on i due to j.
+ *
+ * Potentials (BASELINE.json configs[0], configs[2]; readings SURVEY.md §8c O3, A21):
+ *   kind 0, LJ shifted-force:  phi(r) = 4 eps [(sig/r)^12 - (sig/r)^6],
+ *       phi_SF(r) = phi(r) - phi(rc) - (r - rc) phi'(rc) for r < rc, else 0.
+ *       pot = {eps, sig, rc}
+ *   kind 1, Finnis-Sinclair type: v(r) = D[e^{-2a(r-r0)} - 2e^{-a(r-r0)}] t(r),
+ *       psi(r) = e^{-beta (r - rho_r0)} t(r), rho_i = sum_j psi, U_i = 1/2 sum_j v + F(rho_i),
+ *       F(rho) = -A sqrt(rho); t(r) = 1 (r <= r_on), 1/2[1 + cos(pi (r-r_on)/(r_cut-r_on))], 0 (r >= r_cut),
+ *       applied to BOTH pair and density terms.
+ *       pot = {D, a, r0, beta, rho_r0, A, r_on, r_cut}
+ */
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#define ORACLE_OK 0
+#define ORACLE_EINVAL (-1)
+#define ORACLE_ENEIGH_OVERFLOW (-4)
+#define ORACLE_ECELL (-5)
+
+static const double PI = 3.14159265358979323846;
+
+/* ---------- small 3x3 helpers (row-major) ---------- */
+static double det3(const double *m) {
+    return m[0] * (m[4] * m[8] - m[5] * m[7]) - m[1] * (m[3] * m[8] - m[5] * m[6]) +
+           m[2] * (m[3] * m[7] - m[4] * m[6]);
+}
+
+static int inv3(const double *m, double *out) {
+    double d = det3(m);
+    if (d == 0.0 || !isfinite(d)) return ORACLE_ECELL;
+    out[0] = (m[4] * m[8] - m[5] * m[7]) / d;
+    out[1] = (m[2] * m[7] - m[1] * m[8]) / d;
+    out[2] = (m[1] * m[5] - m[2] * m[4]) / d;
+    out[3] = (m[5] * m[6] - m[3] * m[8]) / d;
+    out[4] = (m[0] * m[8] - m[2] * m[6]) / d;
+    out[5] = (m[2] * m[3] - m[0] * m[5]) / d;
+    out[6] = (m[3] * m[7] - m[4] * m[6]) / d;
+    out[7] = (m[1] * m[6] - m[0] * m[7]) / d;
+    out[8] = (m[0] * m[4] - m[1] * m[3]) / d;
+    return ORACLE_OK;
+}
+
+/* row vector times matrix: out_k = sum_l v_l m[l][k] */
+static void vecmat(const double *v, const double *m, double *out) {
+    for (int k = 0; k < 3; ++k) out[k] = v[0] * m[k] + v[1] * m[3 + k] + v[2] * m[6 + k];
+}
+
+/* perpendicular widths w_a = Omega / |h_b x h_c| of the cell h */
+static void perp_widths(const double *h, double *w) {
+    double vol = fabs(det3(h));
+    for (int a = 0; a < 3; ++a) {
+        const double *b = h + 3 * ((a + 1) % 3), *c = h + 3 * ((a + 2) % 3);
+        double cx = b[1] * c[2] - b[2] * c[1], cy = b[2] * c[0] - b[0] * c[2], cz = b[0] * c[1] - b[1] * c[0];
+        w[a] = vol / sqrt(cx * cx + cy * cy + cz * cz);
+    }
+}
+
+/* fractional coordinates s = Rt h0^{-1}, unwrapped */
+static int fractional(int N, const double *Rt, const double *h0, double *s) {
+    double h0inv[9];
+    int rc = inv3(h0, h0inv);
+    if (rc) return rc;
+    for (int i = 0; i < N; ++i) vecmat(Rt + 3 * i, h0inv, s + 3 * i);
+    return ORACLE_OK;
+}
+
+/* ---------- O2: neighbours ---------- */
+
+/*
+ * Brute force over all ordered pairs and all periodic images: THE DEFINITION.
+ * Entry (i; j, n) is accepted iff |(s_j - s_i + n) h| < r_list strictly and not (j == i and n == 0).
+ * count[N]; list[i*cap + k] = j; shift[(i*cap + k)*3 + a] = n_a.
+ */
+int oracle_neighbors_brute(int N, const double *Rt, const double *h0, const double *h, double r_list, int cap,
+                           int *count, int *list, int *shift) {
+    double *s = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double w[3];
+    int M[3];
+    int rc = fractional(N, Rt, h0, s);
+    if (rc) { free(s); return rc; }
+    if (det3(h) == 0.0) { free(s); return ORACLE_ECELL; }
+    perp_widths(h, w);
+    for (int a = 0; a < 3; ++a) M[a] = (int)ceil(r_list / w[a]);
+    double rl2 = r_list * r_list;
+    int status = ORACLE_OK;
+    for (int i = 0; i < N; ++i) {
+        int c = 0;
+        for (int j = 0; j < N; ++j) {
+            double d[3], d0[3], rnd[3];
+            for (int a = 0; a < 3; ++a) {
+                d[a] = s[3 * j + a] - s[3 * i + a];
+                rnd[a] = round(d[a]);
+                d0[a] = d[a] - rnd[a];
+            }
+            for (int ma = -M[0]; ma <= M[0]; ++ma)
+                for (int mb = -M[1]; mb <= M[1]; ++mb)
+                    for (int mc = -M[2]; mc <= M[2]; ++mc) {
+                        int n[3] = {ma - (int)rnd[0], mb - (int)rnd[1], mc - (int)rnd[2]};
+                        if (j == i && n[0] == 0 && n[1] == 0 && n[2] == 0) continue;
+                        double ds[3] = {d0[0] + ma, d0[1] + mb, d0[2] + mc}, r[3];
+                        vecmat(ds, h, r);
+                        double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+                        if (r2 < rl2) {
+                            if (c < cap) {
+                                list[(size_t)i * cap + c] = j;
+                                shift[((size_t)i * cap + c) * 3 + 0] = n[0];
+                                shift[((size_t)i * cap + c) * 3 + 1] = n[1];
+                                shift[((size_t)i * cap + c) * 3 + 2] = n[2];
+                            } else
+                                status = ORACLE_ENEIGH_OVERFLOW;
+                            ++c;
+                        }
+                    }
+        }
+        count[i] = c;
+    }
+    free(s);
+    return status;
+}
+
+/*
+ * Cell list in fractional space (validated against the brute force in tests, then used for the
+ * larger configs).  Axis a gets nb_a = floor(w_a / r_list) bins; if nb_a >= 3 the stencil is the
+ * three adjacent bins with periodic wrap, otherwise the axis uses a single bin and explicit
+ * periodic shifts m_a in [-ceil(r_list/w_a), +ceil(r_list/w_a)].
+ */
+int oracle_neighbors_cells(int N, const double *Rt, const double *h0, const double *h, double r_list, int cap,
+                           int *count, int *list, int *shift) {
+    double *s = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    double *sw = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    int *fl = (int *)malloc(sizeof(int) * 3 * (size_t)N);
+    int *bin = (int *)malloc(sizeof(int) * (size_t)N);
+    double w[3];
+    int nb[3], lo[3], hi[3];
+    int rc = fractional(N, Rt, h0, s);
+    if (rc || det3(h) == 0.0) { free(s); free(sw); free(fl); free(bin); return rc ? rc : ORACLE_ECELL; }
+    perp_widths(h, w);
+    for (int a = 0; a < 3; ++a) {
+        nb[a] = (int)floor(w[a] / r_list);
+        if (nb[a] >= 3) { lo[a] = -1; hi[a] = 1; }
+        else { nb[a] = 1; hi[a] = (int)ceil(r_list / w[a]); lo[a] = -hi[a]; }
+    }
+    int nbins = nb[0] * nb[1] * nb[2];
+    int *start = (int *)calloc((size_t)nbins + 1, sizeof(int));
+    int *members = (int *)malloc(sizeof(int) * (size_t)N);
+    for (int i = 0; i < N; ++i) {
+        int b[3];
+        for (int a = 0; a < 3; ++a) {
+            double f = floor(s[3 * i + a]);
+            fl[3 * i + a] = (int)f;
+            sw[3 * i + a] = s[3 * i + a] - f;
+            b[a] = (int)(sw[3 * i + a] * nb[a]);
+            if (b[a] >= nb[a]) b[a] = nb[a] - 1;
+        }
+        bin[i] = (b[0] * nb[1] + b[1]) * nb[2] + b[2];
+        start[bin[i] + 1]++;
+    }
+    for (int b = 0; b < nbins; ++b) start[b + 1] += start[b];
+    int *cursor = (int *)malloc(sizeof(int) * (size_t)nbins);
+    memcpy(cursor, start, sizeof(int) * (size_t)nbins);
+    for (int i = 0; i < N; ++i) members[cursor[bin[i]]++] = i; /* ascending atom index inside a bin */
+    double rl2 = r_list * r_list;
+    int status = ORACLE_OK;
+    for (int i = 0; i < N; ++i) {
+        int c = 0;
+        int bi[3] = {bin[i] / (nb[1] * nb[2]), (bin[i] / nb[2]) % nb[1], bin[i] % nb[2]};
+        for (int da = lo[0]; da <= hi[0]; ++da)
+            for (int db = lo[1]; db <= hi[1]; ++db)
+                for (int dc = lo[2]; dc <= hi[2]; ++dc) {
+                    int d[3] = {da, db, dc}, bj[3], m[3];
+                    for (int a = 0; a < 3; ++a) {
+                        if (nb[a] >= 3) {
+                            int t = bi[a] + d[a];
+                            m[a] = (t < 0) ? -1 : (t >= nb[a] ? 1 : 0);
+                            bj[a] = t - m[a] * nb[a];
+                        } else { bj[a] = 0; m[a] = d[a]; }
+                    }
+                    int b = (bj[0] * nb[1] + bj[1]) * nb[2] + bj[2];
+                    for (int q = start[b]; q < start[b + 1]; ++q) {
+                        int j = members[q];
+                        int n[3];
+                        double ds[3], r[3];
+                        for (int a = 0; a < 3; ++a) {
+                            ds[a] = sw[3 * j + a] - sw[3 * i + a] + m[a];
+                            n[a] = m[a] - fl[3 * j + a] + fl[3 * i + a];
+                        }
+                        if (j == i && n[0] == 0 && n[1] == 0 && n[2] == 0) continue;
+                        vecmat(ds, h, r);
+                        double r2 = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+                        if (r2 < rl2) {
+                            if (c < cap) {
+                                list[(size_t)i * cap + c] = j;
+                                for (int a = 0; a < 3; ++a) shift[((size_t)i * cap + c) * 3 + a] = n[a];
+                            } else
+                                status = ORACLE_ENEIGH_OVERFLOW;
+                            ++c;
+                        }
+                    }
+                }
+        count[i] = c;
+    }
+    free(s); free(sw); free(fl); free(bin); free(start); free(members); free(cursor);
+    return status;
+}
+
+/* ---------- O3: pair functions ---------- */
+
+/* LJ shifted-force: value and derivative of phi_SF at r < rc */
+static void lj_sf(const double *p, double r, double *phi, double *dphi) {
+    double eps = p[0], sig = p[1], rc = p[2];
+    double sr = sig / r, sr6 = sr * sr * sr * sr * sr * sr, sr12 = sr6 * sr6;
+    double src = sig / rc, src6 = src * src * src * src * src * src, src12 = src6 * src6;
+    double phi_r = 4.0 * eps * (sr12 - sr6);
+    double dphi_r = 4.0 * eps * (-12.0 * sr12 + 6.0 * sr6) / r;
+    double phi_c = 4.0 * eps * (src12 - src6);
+    double dphi_c = 4.0 * eps * (-12.0 * src12 + 6.0 * src6) / rc;
+    *phi = phi_r - phi_c - (r - rc) * dphi_c;
+    *dphi = dphi_r - dphi_c;
+}
+
+/* cosine taper t(r) and t'(r) */
+static void taper(double r, double r_on, double r_cut, double *t, double *dt) {
+    if (r <= r_on) { *t = 1.0; *dt = 0.0; }
+    else if (r >= r_cut) { *t = 0.0; *dt = 0.0; }
+    else {
+        double x = PI * (r - r_on) / (r_cut - r_on);
+        *t = 0.5 * (1.0 + cos(x));
+        *dt = -0.5 * sin(x) * PI / (r_cut - r_on);
+    }
+}
+
+/* FS pair term v(r), v'(r) */
+static void fs_pair(const double *p, double r, double *v, double *dv) {
+    double D = p[0], a = p[1], r0 = p[2], t, dt;
+    taper(r, p[6], p[7], &t, &dt);
+    double e1 = exp(-a * (r - r0)), e2 = exp(-2.0 * a * (r - r0));
+    double m = D * (e2 - 2.0 * e1);
+    double dm = D * (-2.0 * a * e2 + 2.0 * a * e1);
+    *v = m * t;
+    *dv = dm * t + m * dt;
+}
+
+/* FS density term psi(r), psi'(r) */
+static void fs_density(const double *p, double r, double *psi, double *dpsi) {
+    double beta = p[3], rr0 = p[4], t, dt;
+    taper(r, p[6], p[7], &t, &dt);
+    double e = exp(-beta * (r - rr0));
+    *psi = e * t;
+    *dpsi = -beta * e * t + e * dt;
+}
+
+/* embedding F(rho) = -A sqrt(rho), F'(rho) = -A / (2 sqrt(rho)); rho = 0 => F = F' = 0 */
+static void fs_embed(const double *p, double rho, double *F, double *dF) {
+    if (rho <= 0.0) { *F = 0.0; *dF = 0.0; return; }
+    double sq = sqrt(rho);
+    *F = -p[5] * sq;
+    *dF = -p[5] / (2.0 * sq);
+}
+
+/* r^ij = (s_j - s_i + n) h for list entry k of atom i */
+static double pair_vector(const double *s, const double *h, int i, int j, const int *n, double *r) {
+    double ds[3] = {s[3 * j] - s[3 * i] + n[0], s[3 * j + 1] - s[3 * i + 1] + n[1], s[3 * j + 2] - s[3 * i + 2] + n[2]};
+    vecmat(ds, h, r);
+    return r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+}
+
+/*
+ * Energy, forces, virial of one image from its neighbour list (Eq. 4, 5, 8).
+ * Outputs: *E total energy; F[N*3] Cartesian forces; V[9] virial, V_mn = -1/2 sum r_m f_n;
+ * Ui[N] per-atom energies (may be NULL); rho_out[N] FS densities (may be NULL).
+ */
+int oracle_energy_force_virial(int N, const double *Rt, const double *h0, const double *h, int kind,
+                               const double *pot, int cap, const int *count, const int *list, const int *shift,
+                               double *E, double *F, double *V, double *Ui, double *rho_out) {
+    if (kind != 0 && kind != 1) return ORACLE_EINVAL;
+    double *s = (double *)malloc(sizeof(double) * 3 * (size_t)N);
+    int rc = fractional(N, Rt, h0, s);
+    if (rc) { free(s); return rc; }
+    double rcut = (kind == 0) ? pot[2] : pot[7];
+    double rc2 = rcut * rcut;
+    double *dF = NULL;
+    double *rho = NULL;
+    double Etot = 0.0;
+    for (int k = 0; k < 9; ++k) V[k] = 0.0;
+    for (int i = 0; i < 3 * N; ++i) F[i] = 0.0;
+
+    if (kind == 1) { /* pass 1: densities rho_i = sum_j psi(r_ij), then F'(rho_i) */
+        rho = (double *)calloc((size_t)N, sizeof(double));
+        dF = (double *)calloc((size_t)N, sizeof(double));
+        for (int i = 0; i < N; ++i) {
+            int c = count[i] < cap ? count[i] : cap;
+            for (int k = 0; k < c; ++k) {
+                double r[3];
+                size_t e = (size_t)i * cap + k;
+                double r2 = pair_vector(s, h, i, list[e], shift + 3 * e, r);
+                if (r2 < rc2) {
+                    double psi, dpsi;
+                    fs_density(pot, sqrt(r2), &psi, &dpsi);
+                    rho[i] += psi;
+                }
+            }
+        }
+        for (int i = 0; i < N; ++i) {
+            double Fe;
+            fs_embed(pot, rho[i], &Fe, &dF[i]);
+        }
+    }
+
+    for (int i = 0; i < N; ++i) {
+        double ui = 0.0;
+        int c = count[i] < cap ? count[i] : cap;
+        for (int k = 0; k < c; ++k) {
+            double r[3];
+            size_t e = (size_t)i * cap + k;
+            int j = list[e];
+            double r2 = pair_vector(s, h, i, j, shift + 3 * e, r);
+            if (!(r2 < rc2)) continue;
+            double rr = sqrt(r2), fmag; /* fmag = scalar with f^ij = fmag * r_hat */
+            if (kind == 0) {
+                double phi, dphi;
+                lj_sf(pot, rr, &phi, &dphi);
+                ui += 0.5 * phi;
+                fmag = dphi;
+            } else {
+                double v, dv, psi, dpsi;
+                fs_pair(pot, rr, &v, &dv);
+                fs_density(pot, rr, &psi, &dpsi);
+                ui += 0.5 * v;
+                fmag = dv + (dF[i] + dF[j]) * dpsi; /* Eq. 5 applied to U_i = 1/2 sum v + F(rho_i) */
+            }
+            double f[3] = {fmag * r[0] / rr, fmag * r[1] / rr, fmag * r[2] / rr};
+            for (int m = 0; m < 3; ++m) {
+                F[3 * i + m] += f[m];
+                for (int n = 0; n < 3; ++n) V[3 * m + n] += -0.5 * r[m] * f[n];
+            }
+        }
+        if (kind == 1) {
+            double Fe, dFe;
+            fs_embed(pot, rho[i], &Fe, &dFe);
+            ui += Fe;
+        }
+        if (Ui) Ui[i] = ui;
+        Etot += ui;
+    }
+    *E = Etot;
+    if (rho_out && rho) memcpy(rho_out, rho, sizeof(double) * (size_t)N);
+    free(s); free(rho); free(dF);
+    return ORACLE_OK;
+}
+
+/*
+ * Batch over images: neighbours (cell list, or brute force if use_brute) + energy/force/virial.
+ * Rt[P][N*3], h[P][9]; outputs E[P], F[P][N*3], V[P][9].  Images are independent; the loop is the
+ * only place the oracle uses more than one thread (OpenMP, if compiled with -fopenmp).
+ */
+int oracle_eval_images(int P, int N, const double *Rt, const double *h0, const double *h, int kind,
+                       const double *pot, double r_list, int cap, int use_brute, double *E, double *F, double *V) {
+    int status = ORACLE_OK;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int p = 0; p < P; ++p) {
+        int *count = (int *)malloc(sizeof(int) * (size_t)N);
+        int *list = (int *)malloc(sizeof(int) * (size_t)N * cap);
+        int *shift = (int *)malloc(sizeof(int) * (size_t)N * cap * 3);
+        const double *Rp = Rt + (size_t)p * 3 * N;
+        int rc = use_brute ? oracle_neighbors_brute(N, Rp, h0, h + 9 * p, r_list, cap, count, list, shift)
+                           : oracle_neighbors_cells(N, Rp, h0, h + 9 * p, r_list, cap, count, list, shift);
+        if (!rc)
+            rc = oracle_energy_force_virial(N, Rp, h0, h + 9 * p, kind, pot, cap, count, list, shift, E + p,
+                                            F + (size_t)p * 3 * N, V + 9 * p, NULL, NULL);
+        if (rc) {
+#pragma omp critical
+            status = rc;
+        }
+        free(count); free(list); free(shift);
+    }
+    return status;
+}
+
+#ifdef _OPENMP
+extern int omp_get_max_threads(void);
+extern void omp_set_num_threads(int);
+#endif
+
+int oracle_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}

@@ -1,0 +1,169 @@
+"""Pins for oracle/cfneb.py (the crystal band): the vacancy-hop barrier of BASELINE.json configs[0] against
+an independent constrained relaxation, rotation-freeness of the band, the stored lattice
+constants, structural invariants of the adaptive control (O9, "parity unpinned": the paper gives no rule),
+and the one-pass reduction algebra of SURVEY.md §8(d)."""
+import numpy as np
+import pytest
+
+from cfneb_workloads import (CONFIGS, bain_endpoints, bcc_supercell, fcc_supercell, linear_path,
+                             load_lattice_constants, vacancy_endpoints_unrelaxed)
+from oracle import cellfilter as cf
+from oracle import cfneb as oc
+from oracle import forcefield as ff
+from oracle.neb import Fire, improved_tangent, neb_force
+
+
+@pytest.fixture(scope="module")
+def c0():
+    spec = CONFIGS[0]
+    a = load_lattice_constants()["lj_fcc_a"]
+    fi, cell, ffin, _ = vacancy_endpoints_unrelaxed(2, a)
+    R0, h0, E0, fm0, _ = oc.relax_endpoint(fi @ cell, cell, 0, spec.pot, 2.5, fmax_tol=1e-7, fire=spec.fire)
+    R1, h1, E1, fm1, _ = oc.relax_endpoint(ffin @ cell, cell, 0, spec.pot, 2.5, fmax_tol=1e-7, fire=spec.fire)
+    assert fm0 < 1e-7 and fm1 < 1e-7
+    pos, cells = linear_path(R0 @ np.linalg.inv(h0), h0, R1 @ np.linalg.inv(h1), h1, spec.n_images, spec.seed,
+                             spec.noise_sigma)
+    return dict(spec=spec, R0=R0, h0=h0, E0=E0, R1=R1, h1=h1, E1=E1, pos=pos, cells=cells)
+
+
+def test_stored_lattice_constants_are_stress_free():
+    lc = load_lattice_constants()
+    frac, cell = fcc_supercell(2, 2, 2, lc["lj_fcc_a"])
+    nb = ff.neighbors(frac @ cell, cell, cell, 2.5, 128)
+    E, F, V = ff.energy_force_virial(frac @ cell, cell, cell, 0, CONFIGS[0].pot, nb)
+    assert abs(np.trace(V)) < 1e-9 * 32 and abs(E / 32 - lc["lj_fcc_e_coh"]) < 1e-12
+    fr, c0_, fr1, c1_ = bain_endpoints((3, 3, 3), lc["fs_bcc_a"], lc["fs_fcc_volume_ratio"])
+    for frac, cell, nn in ((fr, c0_, 112), (fr1, c1_, 86)):
+        nb = ff.neighbors(frac @ cell, cell, cell, 5.0, 256)
+        E, F, V = ff.energy_force_virial(frac @ cell, cell, cell, 1, CONFIGS[2].pot, nb)
+        assert np.all(nb[0] == nn)
+        assert np.abs(V).max() < 1e-8 * len(frac) and np.abs(F).max() < 1e-10
+    assert abs(np.linalg.det(c1_) / np.linalg.det(c0_) - lc["fs_fcc_volume_ratio"]) < 1e-12
+    assert abs(c1_[2, 2] / c1_[0, 0] - np.sqrt(2.0)) < 1e-12  # c/a = sqrt 2
+
+
+def test_c0_endpoints_equivalent_and_barrier_equals_constrained_saddle(c0):
+    spec = c0["spec"]
+    assert abs(c0["E0"] - c0["E1"]) < 1e-10  # symmetric hop
+    neb = oc.CFNEB(c0["pos"], c0["cells"], 0, spec.pot, 2.5, k_spring=spec.k_spring, climb=True, cell_factor=0.0,
+                   fire=spec.fire)
+    neb.run(1e-5, 5000)
+    assert neb.band.fmax < 1e-5 and neb.band.pstar == 3
+    # independent route: symmetric path => saddle at the midpoint; minimise E with the hop coordinate of the
+    # hopping atom fixed at the midpoint and the centre of mass of the others fixed; rest + cell relaxed.
+    href = c0["h0"]
+    lam = oc.auto_cell_factor(href, 31)
+    ev = oc.CrystalEvaluator(href, 0, spec.pot, 2.8, 128, lam)
+    Rt0, B0, _ = cf.input_mapping(c0["R0"], c0["h0"], href)
+    Rt1, B1, _ = cf.input_mapping(c0["R1"], c0["h1"], href)
+    X = cf.pack(0.5 * (Rt0 + Rt1), 0.5 * (B0 + B1), lam)
+    u = Rt1[0] - Rt0[0]
+    u /= np.linalg.norm(u)
+    fire = Fire((1,) + X.shape, **spec.fire)
+    for _ in range(5000):
+        Es, Gs = ev([X])
+        G = Gs[0].copy()
+        G[0] -= np.dot(G[0], u) * u
+        G[1:-3] -= G[1:-3].mean(axis=0)
+        if np.max(np.sqrt((G * G).sum(axis=1))) < 1e-7:
+            break
+        X = X + fire.step(G[None], X.shape[0])[0]
+        X[-3:] = 0.5 * (X[-3:] + X[-3:].T)
+    assert np.abs(Gs[0]).max() < 1e-6  # the constrained minimum is a true stationary point
+    saddle = Es[0] - c0["E0"]
+    assert abs(neb.band.barrier - saddle) < 1e-6
+    assert 4.9 < saddle < 5.1
+    # paper-literal lam = 1 reaches the same barrier (a constant on the cell block only rescales its mass, A9/A13)
+    neb1 = oc.CFNEB(c0["pos"], c0["cells"], 0, spec.pot, 2.5, k_spring=spec.k_spring, climb=True, cell_factor=1.0,
+                    fire=spec.fire)
+    neb1.run(2e-3, 3000)
+    assert abs(neb1.band.barrier - saddle) < 1e-6
+
+
+def test_band_is_rotation_free(c0):
+    # a final endpoint supplied with a rigid rotation gives the same path, energies and barrier
+    spec = c0["spec"]
+    rng = np.random.default_rng(1)
+    Q, _ = np.linalg.qr(rng.standard_normal((3, 3)))
+    if np.linalg.det(Q) < 0:
+        Q[:, 0] *= -1
+    pos, cells = c0["pos"].copy(), c0["cells"].copy()
+    pos[-1], cells[-1] = pos[-1] @ Q, cells[-1] @ Q
+    pos[2], cells[2] = pos[2] @ Q.T, cells[2] @ Q.T
+    a = oc.CFNEB(c0["pos"], c0["cells"], 0, spec.pot, 2.5, cell_factor=1.0, fire=spec.fire)
+    b = oc.CFNEB(pos, cells, 0, spec.pot, 2.5, cell_factor=1.0, fire=spec.fire)
+    a.step(5)
+    b.step(5)
+    pa, ca, Ea = a.get_path()
+    pb, cb, Eb = b.get_path()
+    assert np.abs(pa - pb).max() < 1e-10 and np.abs(ca - cb).max() < 1e-10 and np.abs(Ea - Eb).max() < 1e-9
+    assert np.allclose(cb[-1], c0["cells"][-1], atol=1e-10)  # get_path returns the un-rotated cell h0 sqrt(B)
+
+
+def test_one_pass_reduction_algebra_matches_direct_evaluation(c0):
+    # f = G + c1 tau+ + c2 tau-, so f.v, f.f follow from ten dot products.
+    spec = c0["spec"]
+    neb = oc.CFNEB(c0["pos"], c0["cells"], 0, spec.pot, 2.5, cell_factor=1.0, fire=spec.fire)
+    neb.step(3)
+    b = neb.band
+    b.forces()
+    v = b.fire.v
+    for p in range(1, b.P - 1):
+        X0, X1, X2 = b.X[p - 1], b.X[p], b.X[p + 1]
+        G, vv_ = b.G[p], v[p - 1]
+        tp, tm = X2 - X1, X1 - X0
+        d = lambda x, y: float(np.sum(x * y))
+        pp, mm, pm, Gp, Gm, GG, Gv, pv, mv = d(tp, tp), d(tm, tm), d(tp, tm), d(G, tp), d(G, tm), d(G, G), d(G, vv_), d(tp, vv_), d(tm, vv_)
+        # tangent weights (a, b) from the energies, O5
+        tau = improved_tangent(X0, X1, X2, b.E[p - 1], b.E[p], b.E[p + 1])[0]
+        A = np.linalg.lstsq(np.stack([tp.ravel(), tm.ravel()], axis=1), tau.ravel(), rcond=None)[0]
+        a_, b_ = A
+        tt = a_ * a_ * pp + 2 * a_ * b_ * pm + b_ * b_ * mm
+        Gt = a_ * Gp + b_ * Gm
+        if p == b.pstar:
+            gam = -2 * Gt / tt
+        else:
+            gam = -Gt / tt + spec.k_spring * (np.sqrt(pp) - np.sqrt(mm)) / np.sqrt(tt)
+        c1, c2 = gam * a_, gam * b_
+        f = b.f[p]
+        assert np.abs(f - (G + c1 * tp + c2 * tm)).max() < 1e-12 * np.abs(f).max() + 1e-13
+        ff_ = GG + 2 * c1 * Gp + 2 * c2 * Gm + c1 * c1 * pp + 2 * c1 * c2 * pm + c2 * c2 * mm
+        fv = Gv + c1 * pv + c2 * mv
+        assert abs(ff_ - d(f, f)) < 1e-10 * d(f, f) and abs(fv - d(f, vv_)) < 1e-10 * max(abs(d(f, vv_)), 1e-3)
+
+
+def test_get_path_round_trip_and_state(c0):
+    spec = c0["spec"]
+    neb = oc.CFNEB(c0["pos"], c0["cells"], 0, spec.pot, 2.5, cell_factor=1.0, fire=spec.fire)
+    pos, cells, E = neb.get_path()
+    assert np.abs(pos - c0["pos"]).max() < 1e-12 and np.abs(cells - c0["cells"]).max() < 1e-12
+    X, v = neb.get_state()
+    assert X.shape == (7, 34, 3) and np.all(v == 0)
+    assert np.allclose(X[0, -3:], np.eye(3))  # B = I at the reference image
+
+
+def test_adaptive_control_structural_invariants(c0):
+    spec = c0["spec"]
+    neb = oc.CFNEB(c0["pos"], c0["cells"], 0, spec.pot, 2.5, cell_factor=1.0, fire=spec.fire)
+    neb.max_images = 9
+    neb.step(3)
+    d = neb.band.segment_lengths()
+    Xold = [x.copy() for x in neb.band.X]
+    q = int(np.argmax(d))
+    n_ins, n_del = neb.adapt(d_insert=0.9 * d.max(), d_delete=0.0)
+    assert (n_ins, n_del) == (1, 0) and neb.P == 8
+    assert np.array_equal(neb.band.X[q + 1], 0.5 * (Xold[q] + Xold[q + 1]))  # exact midpoint
+    assert np.all(neb.band.fire.v == 0) and neb.band.fire.first and neb.band.fire.dt == spec.fire["dt0"]
+    neb.step(2)  # new image gets evaluated
+    assert np.all(np.isfinite(neb.band.E))
+    # deletion: never an endpoint, never the climbing image; P changes by -1
+    ps = neb.band.pstar
+    Xc = neb.band.X[ps].copy()
+    n_ins, n_del = neb.adapt(d_insert=1e9, d_delete=1e9)
+    assert (n_ins, n_del) == (0, 1) and neb.P == 7
+    assert np.array_equal(neb.band.X[neb.band.pstar], Xc)
+    assert np.array_equal(neb.band.X[0], Xold[0]) and np.array_equal(neb.band.X[-1], Xold[-1])
+    # thresholds respected: nothing happens between them; max_images respected
+    assert neb.adapt(d_insert=1e9, d_delete=0.0) == (0, 0)
+    neb.max_images = 7
+    assert neb.adapt(d_insert=0.0, d_delete=0.0) == (0, 0)
