@@ -22,6 +22,8 @@ from .configs import (
     bain_endpoints,
     linear_path,
     load_lattice_constants,
+    load_vacancy_endpoints,
+    build_workload,
 )
 
 __all__ = [
@@ -37,4 +39,6 @@ __all__ = [
     "bain_endpoints",
     "linear_path",
     "load_lattice_constants",
+    "load_vacancy_endpoints",
+    "build_workload",
 ]

@@ -126,3 +126,31 @@ def linear_path(frac0, cell0, frac1, cell1, n_images, seed, sigma):
         if 0 < p < P - 1:
             pos[p] += noise[p - 1]
     return pos, cells
+
+
+def load_vacancy_endpoints(k):
+    """Relaxed vacancy-hop endpoints of configs[k], k in (0, 1), written by `oracle/make_relaxed_endpoints.py`."""
+    path = os.path.join(os.path.dirname(__file__), "vacancy_endpoints_c%d.json" % k)
+    with open(path) as fh:
+        d = json.load(fh)
+    return (np.array(d["pos_init"]), np.array(d["cell_init"]), np.array(d["pos_final"]), np.array(d["cell_final"]))
+
+
+def build_workload(k, n_images=None):
+    """Seeded inputs of BASELINE.json configs[k]: (spec, pos[P,N,3] Cartesian, cells[P,3,3]).
+
+    Vacancy configs: stored relaxed endpoints, 7 / 9 images linear in (fractional coordinates, cell) + noise.
+    Bain configs: perfect bcc at the stress-free lattice constant and its c/a = sqrt(2) image at the stress-free
+    volume (both exact cell-relaxed endpoints of a perfect crystal), linear in the cell matrix (= linear in the
+    deformation gradient D, since h = h0 D) + noise on interior images.
+    """
+    spec = CONFIGS[k]
+    P = int(n_images or spec.n_images)
+    if spec.lattice == "fcc_vacancy":
+        R0, h0, R1, h1 = load_vacancy_endpoints(k)
+        pos, cells = linear_path(R0 @ np.linalg.inv(h0), h0, R1 @ np.linalg.inv(h1), h1, P, spec.seed, spec.noise_sigma)
+    else:
+        lc = load_lattice_constants()
+        f0, c0, f1, c1 = bain_endpoints(spec.dims, lc["fs_bcc_a"], lc["fs_fcc_volume_ratio"])
+        pos, cells = linear_path(f0, c0, f1, c1, P, spec.seed, spec.noise_sigma)
+    return spec, pos, cells

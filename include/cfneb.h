@@ -1,0 +1,205 @@
+/*
+ * cfneb.h -- C ABI of the B200-native CFNEB hot path (arXiv:2510.16721).
+ *
+ * One handle = one nudged-elastic-band chain of P images of N atoms in a variable periodic cell,
+ * resident in GPU memory.  `cfneb_step` runs the whole iteration of the paper's workflow
+ * (PAPER.md "IMPLEMENTATION": cell filter -> force evaluation -> NEB iteration) for all
+ * images at once, in fp64, as hand-written CUDA kernels for sm_100a captured in a CUDA graph;
+ * `cfneb_adapt` / `cfneb_insert_image` / `cfneb_delete_image` are the image-distribution
+ * adjustment of P:128.  Citations `P:n` are lines of the paper text, `O*`/`A*` are the
+ * step definitions and readings of SURVEY.md §8(c) restated in DESIGN.md.
+ *
+ * Conventions (all arrays are plain row-major double / int32, HOST pointers unless stated):
+ *   - row vectors; a cell is double[9], rows = lattice vectors h1,h2,h3, R = s h;
+ *   - positions are Cartesian, double[N*3], never wrapped into the cell (A17);
+ *   - generalized coordinates of an image: X = [R~ ; lam*B], (N+3) x 3, with R~ = R D^-1 (Eq. 10),
+ *     D = h0^-1 h, B = D D^T (Eq. 15), h0 = cell of image 0 (A7), lam = cell_factor (A13);
+ *   - generalized forces: [F D^T ; D^-T V D^-1 / lam] (Eq. 17, as printed, A9), V the virial of Eq. 8.
+ *
+ * Ownership: the caller owns every host buffer (the library copies in/out and never retains host
+ * pointers) and owns the device workspace, which must stay alive and untouched until
+ * cfneb_destroy.  The library allocates no device memory of its own after cfneb_create returns.
+ *
+ * Errors: every call returns 0 (CFNEB_OK) or a negative code; nothing throws or aborts across
+ * the ABI.  Failures detected on the device (neighbour-list overflow, non-positive-definite B,
+ * NaN) set a sticky error word that the next synchronising call returns and cfneb_get_status
+ * reports; once set, further steps leave the state undefined.
+ *
+ * Threading: a handle must be used from one host thread at a time.  All device work is enqueued
+ * on the CUDA stream given to cfneb_create.
+ */
+#ifndef CFNEB_H
+#define CFNEB_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define CFNEB_API __attribute__((visibility("default")))
+#else
+#define CFNEB_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct cfneb cfneb_t; /* opaque */
+
+enum {
+    CFNEB_OK = 0,
+    CFNEB_EINVAL = -1,          /* bad argument (null pointer, n_images < 3, unknown enum, zero tangent ...) */
+    CFNEB_ENOMEM = -2,          /* workspace too small */
+    CFNEB_ECUDA = -3,           /* a CUDA runtime call failed; cfneb_last_cuda_error() has the text */
+    CFNEB_ENEIGH_OVERFLOW = -4, /* an atom has more than max_neighbors neighbours within r_cut + skin */
+    CFNEB_ECELL = -5,           /* B not positive definite / singular cell / periodic shift out of range */
+    CFNEB_ENAN = -6,            /* NaN or Inf in energies or reductions */
+    CFNEB_ERANGE = -7           /* bad image index, endpoint / climbing-image delete, more than max_images */
+};
+
+enum { CFNEB_POT_LJ_SF = 0, CFNEB_POT_FS_MORSE = 1 };
+enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default) */, CFNEB_CELL_D = 2 /* Eq. 14 */ };
+
+/*
+ * Parameters (plain data, copied by cfneb_create).
+ *   potential = CFNEB_POT_LJ_SF:   pot = {eps, sigma, r_c}: phi_SF(r) = phi(r) - phi(r_c) - (r - r_c) phi'(r_c)
+ *   potential = CFNEB_POT_FS_MORSE: pot = {D, alpha, r0, beta, rho_r0, A, r_on, r_cut}:
+ *       v(r) = D[e^{-2 alpha (r-r0)} - 2 e^{-alpha (r-r0)}] t(r), rho_i = sum_j e^{-beta (r - rho_r0)} t(r),
+ *       U_i = 1/2 sum_j v + F(rho_i), F = -A sqrt(rho), t = cosine taper from r_on to r_cut (O3, A21).
+ *   k_spring: uniform spring constant of Eq. 1 (A14).  climb: 1 = climbing image (ref [12]).
+ *   cell_factor: lam of A13; 0 = auto (Omega0^(1/3) N^(1/6)); 1 = the paper's equations literally.
+ *   fire_*: FIRE constants of O7 (one state for the whole band).
+ *   skin: neighbour-list skin; lists hold pairs with r < r_cut + skin and are rebuilt on the device
+ *         when the accumulated displacement bound exceeds skin, or every rebuild_every steps (0 = never
+ *         by count).  max_neighbors: list capacity per atom.  max_images: capacity of the band.
+ */
+typedef struct cfneb_params {
+    int32_t potential;
+    int32_t cell_mode;
+    int32_t climb;
+    int32_t fire_nmin;
+    int32_t max_neighbors;
+    int32_t max_images;
+    int32_t rebuild_every;
+    int32_t reserved0;
+    double pot[12];
+    double k_spring;
+    double cell_factor;
+    double fire_dt0, fire_dtmax, fire_maxstep, fire_finc, fire_fdec, fire_astart, fire_fa;
+    double skin;
+} cfneb_params;
+
+/* Snapshot written by cfneb_get_status (synchronises the stream). */
+typedef struct cfneb_status {
+    int64_t steps;          /* NEB iterations done since create */
+    int64_t rebuilds;       /* per-image neighbour-list rebuilds done on the device */
+    int32_t n_images;       /* current P */
+    int32_t climb_index;    /* p* of the last step (path position), -1 if none */
+    int32_t error;          /* sticky device error (0 or a negative CFNEB_E* code) */
+    int32_t n_pos;          /* FIRE counter of consecutive power > 0 steps */
+    int32_t max_neighbors_seen;
+    int32_t reserved0;
+    double fmax;            /* O8: max row norm of the NEB force of the last step (cell rows count as rows) */
+    double barrier;         /* O8: E_{p*} - E_0 at the last evaluation */
+    double dt, alpha;       /* FIRE state after the last step */
+    double cell_factor;     /* lam actually used */
+    double path_length;     /* sum_p |X_{p+1} - X_p| at the last evaluation */
+} cfneb_status;
+
+/* Kernel classes timed by cfneb_step_timed. */
+enum {
+    CFNEB_K_CELLPREP = 0,  /* K0  cell map D = sqrt(B), Cartesian positions */
+    CFNEB_K_NEIGHBOR = 1,  /* K1  cell-list neighbour build (when it runs) */
+    CFNEB_K_FORCE = 2,     /* K2  batched force / energy / virial (both passes for FS) */
+    CFNEB_K_REDUCE = 3,    /* K4  ten segmented dot products per image */
+    CFNEB_K_SCALAR = 4,    /* K5  tangent weights, climbing image, FIRE scalars, cell rows */
+    CFNEB_K_UPDATE = 5,    /* K6  fused NEB force + cell-filter transform + FIRE update */
+    CFNEB_NKERNELS = 6
+};
+
+/* Fill *prm with the defaults of O7 (FIRE: nmin 5, finc 1.1, fdec 0.5, astart 0.1, fa 0.99, dt0 0.1,
+ * dtmax 1.0, maxstep 0.2), k_spring 1, climb 1, CELL_B, lam 1, skin 0.3, max_neighbors 160,
+ * rebuild_every 0, LJ eps = sigma = 1, r_c = 2.5. */
+CFNEB_API void cfneb_default_params(cfneb_params *prm);
+
+/* Bytes of device workspace cfneb_create needs for n_atoms atoms and prm->max_images images
+ * (0 on invalid arguments).  c4 (101306 atoms x 100 images, 160 neighbours): about 9 GB. */
+CFNEB_API size_t cfneb_workspace_bytes(int32_t n_atoms, const cfneb_params *prm);
+
+/*
+ * Create a band (two known endpoints; positions + lattice per image).
+ *   pos_init/cell_init, pos_final/cell_final: HOST, N*3 and 9 doubles, Cartesian / rows = lattice vectors.
+ *   n_images: P >= 3 including both endpoints, <= prm->max_images.
+ *   path_or_null: HOST, optional explicit interior images, (P-2) blocks of (N*3 + 9) doubles
+ *       (Cartesian positions then cell); if NULL the interior is linear in (R~, B) (or (R~, D) for CELL_D).
+ *   dev_workspace: DEVICE pointer, 256-byte aligned, ws_bytes >= cfneb_workspace_bytes().
+ *   cuda_stream: a cudaStream_t (may be NULL = legacy default stream; must not be capturing).
+ * Maps inputs to generalized coordinates (O0) on the device, evaluates all P images once
+ * (endpoint energies), builds neighbour lists and captures the step graph.  Synchronises.
+ */
+CFNEB_API int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const double *cell_init,
+                 const double *pos_final, const double *cell_final, int32_t n_images, const double *path_or_null,
+                 const cfneb_params *prm, void *dev_workspace, size_t ws_bytes, void *cuda_stream);
+
+/* Enqueue n_steps CFNEB iterations (K0-K6 of DESIGN.md; one force evaluation of every movable image
+ * + one FIRE update each) as CUDA-graph launches on the stream.  Asynchronous: no host
+ * synchronisation, no host<->device traffic. */
+CFNEB_API int cfneb_step(cfneb_t *h, int32_t n_steps);
+
+/* Same iterations launched kernel by kernel with CUDA events between kernel classes; adds the
+ * elapsed milliseconds per class, summed over the n_steps, to kernel_ms[CFNEB_NKERNELS] (HOST).
+ * Synchronises.  For measurement only (bench.py roofline). */
+CFNEB_API int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms);
+
+/* Insert the midpoint of images (after_index, after_index+1) in generalized coordinates (O9);
+ * resets the FIRE state (v = 0, dt = dt0).  The new image's energy is evaluated on the next step. */
+CFNEB_API int cfneb_insert_image(cfneb_t *h, int32_t after_index);
+
+/* Remove an interior image (not an endpoint, not the current climbing image); resets the FIRE state. */
+CFNEB_API int cfneb_delete_image(cfneb_t *h, int32_t index);
+
+/* Host-side control step of O9 (reading A16): at most one deletion (interior non-climbing image
+ * minimising d_{q-1}+d_q, if below d_delete and P > 3) and one insertion (longest segment, if above
+ * d_insert and P < max_images) with d_p = |X_{p+1} - X_p|.  Synchronises.  n_ins/n_del may be NULL. */
+CFNEB_API int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, int32_t *n_del);
+
+/* Segment lengths d_p = |X_{p+1} - X_p|, p = 0..P-2, at the current X (HOST, P-1 doubles). Synchronises. */
+CFNEB_API int cfneb_get_segment_lengths(cfneb_t *h, double *d);
+
+/* Current path: *n_images = P; pos P*N*3 Cartesian (R = R~ D), cells P*9 (h = h0 D, D = sqrt(B):
+ * rotation-free), energies P (of the last evaluation; NaN for an image inserted since).
+ * Any of pos/cells/energies may be NULL.  Synchronises. */
+CFNEB_API int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, double *energies);
+
+/* Replace all P images from HOST Cartesian data (pos P*N*3, cells P*9; image 0's cell must equal h0);
+ * resets the FIRE state and rebuilds neighbour lists; endpoint energies are re-evaluated.  Synchronises. */
+CFNEB_API int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells);
+
+/* Generalized coordinates X and FIRE velocities v, each P*(N+3)*3 (checkpoint; either may be NULL). */
+CFNEB_API int cfneb_get_state(cfneb_t *h, double *X, double *v);
+
+/* Parity hook: evaluate forces at the CURRENT X without updating anything.  F: P*N*3 Cartesian forces
+ * (Eq. 5), virial: P*9 (Eq. 8), f_neb: P*(N+3)*3 NEB force of Eq. 1 in generalized coordinates (zero rows
+ * for endpoints), energies: P.  Any may be NULL.  Synchronises. */
+CFNEB_API int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, double *energies);
+
+/* Parity hook: neighbour list of one image as built on the device for the current X:
+ * count[N], list[N*cap] (entry k of atom i at list[i*cap + k]), shift[N*cap*3]; r^ij = (s_j - s_i + n) h.
+ * cap = prm->max_neighbors.  Forces a fresh build of that image.  Synchronises. */
+CFNEB_API int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int32_t *list, int32_t *shift);
+
+/* Synchronise and report. */
+CFNEB_API int cfneb_get_status(cfneb_t *h, cfneb_status *out);
+
+CFNEB_API void cfneb_destroy(cfneb_t *h);
+CFNEB_API const char *cfneb_strerror(int code);
+CFNEB_API const char *cfneb_last_cuda_error(void);
+
+/* Measurement utility: sustained fp64 FMA throughput of this GPU (TFLOP/s, 2 flops per DFMA) from a
+ * register-resident DFMA chain kernel; the denominator of the force kernel's "alu" roofline. */
+CFNEB_API int cfneb_util_fp64_peak(void *cuda_stream, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CFNEB_H */

@@ -1,0 +1,302 @@
+"""ctypes binding of libcfneb.so -- argument marshalling only; every step of the path runs in the CUDA kernels.
+
+Same names as include/cfneb.h.  PyTorch is used for the device workspace and the stream, nothing else.
+There is no CPU fallback: if the library is missing or no CUDA device is present, calls raise.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libcfneb.so")
+
+OK, EINVAL, ENOMEM, ECUDA, ENEIGH_OVERFLOW, ECELL, ENAN, ERANGE = 0, -1, -2, -3, -4, -5, -6, -7
+POT_LJ_SF, POT_FS_MORSE = 0, 1
+CELL_FIXED, CELL_B, CELL_D = 0, 1, 2
+K_CELLPREP, K_NEIGHBOR, K_FORCE, K_REDUCE, K_SCALAR, K_UPDATE, NKERNELS = 0, 1, 2, 3, 4, 5, 6
+KERNEL_CLASSES = ("cell_prep", "neighbor", "force", "reduce", "scalar", "update")
+
+EXPORTS = (
+    "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_timed",
+    "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_get_segment_lengths", "cfneb_get_path",
+    "cfneb_set_path", "cfneb_get_state", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
+    "cfneb_destroy", "cfneb_strerror", "cfneb_last_cuda_error", "cfneb_util_fp64_peak",
+)
+
+
+class Params(ctypes.Structure):
+    """cfneb_params (include/cfneb.h)."""
+    _fields_ = [
+        ("potential", ctypes.c_int32), ("cell_mode", ctypes.c_int32), ("climb", ctypes.c_int32),
+        ("fire_nmin", ctypes.c_int32), ("max_neighbors", ctypes.c_int32), ("max_images", ctypes.c_int32),
+        ("rebuild_every", ctypes.c_int32), ("reserved0", ctypes.c_int32),
+        ("pot", ctypes.c_double * 12), ("k_spring", ctypes.c_double), ("cell_factor", ctypes.c_double),
+        ("fire_dt0", ctypes.c_double), ("fire_dtmax", ctypes.c_double), ("fire_maxstep", ctypes.c_double),
+        ("fire_finc", ctypes.c_double), ("fire_fdec", ctypes.c_double), ("fire_astart", ctypes.c_double),
+        ("fire_fa", ctypes.c_double), ("skin", ctypes.c_double),
+    ]
+
+
+class Status(ctypes.Structure):
+    """cfneb_status (include/cfneb.h)."""
+    _fields_ = [
+        ("steps", ctypes.c_int64), ("rebuilds", ctypes.c_int64), ("n_images", ctypes.c_int32),
+        ("climb_index", ctypes.c_int32), ("error", ctypes.c_int32), ("n_pos", ctypes.c_int32),
+        ("max_neighbors_seen", ctypes.c_int32), ("reserved0", ctypes.c_int32), ("fmax", ctypes.c_double),
+        ("barrier", ctypes.c_double), ("dt", ctypes.c_double), ("alpha", ctypes.c_double),
+        ("cell_factor", ctypes.c_double), ("path_length", ctypes.c_double),
+    ]
+
+    def as_dict(self):
+        return {k: getattr(self, k) for k, _ in self._fields_ if not k.startswith("reserved")}
+
+
+class CfnebError(RuntimeError):
+    def __init__(self, code, what=""):
+        msg = lib().cfneb_strerror(code).decode()
+        if code == ECUDA:
+            msg += ": " + lib().cfneb_last_cuda_error().decode()
+        super().__init__("%s failed: %s (%d)" % (what, msg, code))
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libcfneb.so (built by `python -m paper_2510_16721_b200.build`).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("libcfneb.so not built: run `python -m paper_2510_16721_b200.build` (no CPU fallback exists)")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, dp, ip = ctypes.c_void_p, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_int32)
+    i32, f64 = ctypes.c_int32, ctypes.c_double
+    pp = ctypes.POINTER(Params)
+    L.cfneb_default_params.restype = None
+    L.cfneb_default_params.argtypes = [pp]
+    L.cfneb_workspace_bytes.restype = ctypes.c_size_t
+    L.cfneb_workspace_bytes.argtypes = [i32, pp]
+    L.cfneb_create.restype = ctypes.c_int
+    L.cfneb_create.argtypes = [ctypes.POINTER(vp), i32, dp, dp, dp, dp, i32, dp, pp, vp, ctypes.c_size_t, vp]
+    for name, args in (
+        ("cfneb_step", [vp, i32]), ("cfneb_step_timed", [vp, i32, dp]), ("cfneb_insert_image", [vp, i32]),
+        ("cfneb_delete_image", [vp, i32]), ("cfneb_adapt", [vp, f64, f64, ip, ip]),
+        ("cfneb_get_segment_lengths", [vp, dp]), ("cfneb_get_path", [vp, ip, dp, dp, dp]),
+        ("cfneb_set_path", [vp, dp, dp]), ("cfneb_get_state", [vp, dp, dp]),
+        ("cfneb_get_forces", [vp, dp, dp, dp, dp]), ("cfneb_get_neighbors", [vp, i32, ip, ip, ip]),
+        ("cfneb_get_status", [vp, ctypes.POINTER(Status)]), ("cfneb_util_fp64_peak", [vp, dp]),
+    ):
+        fn = getattr(L, name)
+        fn.restype = ctypes.c_int
+        fn.argtypes = args
+    L.cfneb_destroy.restype = None
+    L.cfneb_destroy.argtypes = [vp]
+    L.cfneb_strerror.restype = ctypes.c_char_p
+    L.cfneb_strerror.argtypes = [ctypes.c_int]
+    L.cfneb_last_cuda_error.restype = ctypes.c_char_p
+    L.cfneb_last_cuda_error.argtypes = []
+    _lib = L
+    return L
+
+
+def _dptr(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_double)) if a is not None else None
+
+
+def _iptr(a):
+    return a.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)) if a is not None else None
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def default_params(**kw):
+    """cfneb_default_params, then overrides.  `pot` may be any sequence of <= 12 numbers; `fire` a dict with the
+    keys dt0, dtmax, maxstep, nmin, finc, fdec, astart, fa."""
+    p = Params()
+    lib().cfneb_default_params(ctypes.byref(p))
+    fire = kw.pop("fire", None) or {}
+    for k, v in fire.items():
+        setattr(p, "fire_" + k, v)
+    pot = kw.pop("pot", None)
+    if pot is not None:
+        for k in range(12):
+            p.pot[k] = float(pot[k]) if k < len(pot) else 0.0
+    for k, v in kw.items():
+        if not hasattr(p, k):
+            raise KeyError(k)
+        setattr(p, k, v)
+    return p
+
+
+def workspace_bytes(n_atoms, params):
+    return int(lib().cfneb_workspace_bytes(int(n_atoms), ctypes.byref(params)))
+
+
+def fp64_peak_tflops():
+    import torch
+    out = ctypes.c_double(0.0)
+    rc = lib().cfneb_util_fp64_peak(ctypes.c_void_p(torch.cuda.current_stream().cuda_stream), ctypes.byref(out))
+    if rc:
+        raise CfnebError(rc, "cfneb_util_fp64_peak")
+    return out.value
+
+
+class CFNEB:
+    """One band on the GPU.  pos[P,N,3] Cartesian, cells[P,3,3] rows = lattice vectors (or endpoints only with
+    n_images).  Methods mirror the C ABI: step, step_timed, insert_image, delete_image, adapt, get_path, ..."""
+
+    def __init__(self, pos, cells, params, n_images=None, device="cuda:0", stream=None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("CFNEB needs a CUDA device (sm_100a); there is no CPU fallback")
+        pos, cells = _f64(pos), _f64(cells).reshape(-1, 9)
+        self.N = int(pos.shape[1])
+        if n_images is None:
+            n_images = pos.shape[0]
+        explicit = pos.shape[0] == n_images and n_images > 2
+        if not explicit and pos.shape[0] != 2:
+            raise ValueError("give either all n_images images or the two endpoints")
+        self.params = params
+        self.device = torch.device(device)
+        nbytes = workspace_bytes(self.N, params)
+        if nbytes == 0:
+            raise CfnebError(EINVAL, "cfneb_workspace_bytes")
+        with torch.cuda.device(self.device):
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=self.device)
+            base = (self._ws.data_ptr() + 255) // 256 * 256
+            self._stream = stream if stream is not None else torch.cuda.Stream(device=self.device)
+            path = None
+            if explicit:
+                path = np.concatenate([pos[1:-1].reshape(n_images - 2, -1), cells[1:-1]], axis=1)
+                path = np.ascontiguousarray(path)
+            h = ctypes.c_void_p()
+            rc = lib().cfneb_create(ctypes.byref(h), self.N, _dptr(np.ascontiguousarray(pos[0])), _dptr(np.ascontiguousarray(cells[0])),
+                                    _dptr(np.ascontiguousarray(pos[-1])), _dptr(np.ascontiguousarray(cells[-1])), int(n_images), _dptr(path),
+                                    ctypes.byref(params), ctypes.c_void_p(base), nbytes,
+                                    ctypes.c_void_p(self._stream.cuda_stream))
+        if rc:
+            raise CfnebError(rc, "cfneb_create")
+        self._h = h
+        self.workspace_bytes = nbytes
+
+    # -- hot path ----------------------------------------------------------------------------------
+    def step(self, n=1):
+        rc = lib().cfneb_step(self._h, int(n))
+        if rc:
+            raise CfnebError(rc, "cfneb_step")
+
+    def step_timed(self, n=1):
+        ms = np.zeros(NKERNELS)
+        rc = lib().cfneb_step_timed(self._h, int(n), _dptr(ms))
+        if rc:
+            raise CfnebError(rc, "cfneb_step_timed")
+        return ms
+
+    def synchronize(self):
+        self._stream.synchronize()
+
+    @property
+    def stream(self):
+        return self._stream
+
+    # -- image control -------------------------------------------------------------------------------
+    def insert_image(self, after_index):
+        rc = lib().cfneb_insert_image(self._h, int(after_index))
+        if rc:
+            raise CfnebError(rc, "cfneb_insert_image")
+
+    def delete_image(self, index):
+        rc = lib().cfneb_delete_image(self._h, int(index))
+        if rc:
+            raise CfnebError(rc, "cfneb_delete_image")
+
+    def adapt(self, d_insert, d_delete):
+        ni, nd = ctypes.c_int32(0), ctypes.c_int32(0)
+        rc = lib().cfneb_adapt(self._h, float(d_insert), float(d_delete), ctypes.byref(ni), ctypes.byref(nd))
+        if rc:
+            raise CfnebError(rc, "cfneb_adapt")
+        return ni.value, nd.value
+
+    # -- views -----------------------------------------------------------------------------------------
+    def get_status(self):
+        s = Status()
+        rc = lib().cfneb_get_status(self._h, ctypes.byref(s))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_status")
+        return s
+
+    @property
+    def P(self):
+        return int(self.get_status().n_images)
+
+    def get_segment_lengths(self):
+        P = self.P
+        d = np.zeros(P - 1)
+        rc = lib().cfneb_get_segment_lengths(self._h, _dptr(d))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_segment_lengths")
+        return d
+
+    def get_path(self, positions=True):
+        P = self.P
+        pos = np.zeros((P, self.N, 3)) if positions else None
+        cells = np.zeros((P, 3, 3))
+        E = np.zeros(P)
+        n = ctypes.c_int32(0)
+        rc = lib().cfneb_get_path(self._h, ctypes.byref(n), _dptr(pos), _dptr(cells), _dptr(E))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_path")
+        return pos, cells, E
+
+    def set_path(self, pos, cells):
+        pos, cells = _f64(pos), _f64(cells)
+        rc = lib().cfneb_set_path(self._h, _dptr(pos), _dptr(cells))
+        if rc:
+            raise CfnebError(rc, "cfneb_set_path")
+
+    def get_state(self):
+        P = self.P
+        X = np.zeros((P, self.N + 3, 3))
+        v = np.zeros((P, self.N + 3, 3))
+        rc = lib().cfneb_get_state(self._h, _dptr(X), _dptr(v))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_state")
+        return X, v
+
+    def get_forces(self, forces=True, f_neb=True):
+        P = self.P
+        F = np.zeros((P, self.N, 3)) if forces else None
+        V = np.zeros((P, 3, 3))
+        fn = np.zeros((P, self.N + 3, 3)) if f_neb else None
+        E = np.zeros(P)
+        rc = lib().cfneb_get_forces(self._h, _dptr(F), _dptr(V), _dptr(fn), _dptr(E))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_forces")
+        return F, V, fn, E
+
+    def get_neighbors(self, image):
+        cap = int(self.params.max_neighbors)
+        count = np.zeros(self.N, dtype=np.int32)
+        lst = np.zeros((self.N, cap), dtype=np.int32)
+        shift = np.zeros((self.N, cap, 3), dtype=np.int32)
+        rc = lib().cfneb_get_neighbors(self._h, int(image), _iptr(count), _iptr(lst), _iptr(shift))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_neighbors")
+        return count, lst, shift
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().cfneb_destroy(self._h)
+            self._h = None
+            self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,611 @@
+// api.cu -- the C ABI of include/cfneb.h: handle, workspace carving, CUDA-graph capture of one CFNEB
+// iteration (K0-K6), host-side image control (O9) and the parity / checkpoint hooks.
+// All arithmetic of the method runs in the kernels; this file only marshals, launches and copies.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#include "cfneb_internal.cuh"
+
+using namespace cfn;
+
+static thread_local char g_cuda_err[512] = "";
+
+#define CK(call)                                                                                       \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess) {                                                                       \
+            snprintf(g_cuda_err, sizeof g_cuda_err, "%s at %s:%d: %s", #call, __FILE__, __LINE__,     \
+                     cudaGetErrorString(e_));                                                          \
+            return CFNEB_ECUDA;                                                                        \
+        }                                                                                              \
+    } while (0)
+
+struct cfneb {
+    Dev d;
+    cfneb_params prm;
+    cudaStream_t st;
+    bool own_stream;
+    int P;
+    std::vector<int> order;  // host mirror of the order table (only the host edits it)
+    std::vector<int> free_slots;
+    cudaGraph_t graph;
+    cudaGraphExec_t exec;
+    cudaEvent_t ev[CFNEB_NKERNELS + 1];
+    bool have_events;
+};
+
+// ---- workspace carving (one function serves the size query and create) ----
+namespace {
+struct Carver {
+    char *base;
+    size_t off;
+    template <typename T>
+    T *take(size_t n) {
+        off = (off + 255) & ~(size_t)255;
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += n * sizeof(T);
+        return p;
+    }
+};
+
+bool valid_params(int32_t n_atoms, const cfneb_params *prm) {
+    if (!prm || n_atoms < 1 || n_atoms >= kMaxAtoms) return false;
+    if (prm->potential != CFNEB_POT_LJ_SF && prm->potential != CFNEB_POT_FS_MORSE) return false;
+    if (prm->cell_mode < CFNEB_CELL_FIXED || prm->cell_mode > CFNEB_CELL_D) return false;
+    if (prm->max_images < 3 || prm->max_neighbors < 1 || prm->max_neighbors > 4096) return false;
+    if (!(prm->skin >= 0.0) || !(prm->cell_factor >= 0.0)) return false;
+    const double rc = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
+    if (!(rc > 0.0)) return false;
+    if (prm->potential == CFNEB_POT_FS_MORSE && !(prm->pot[7] > prm->pot[6])) return false;
+    if (!(prm->fire_dt0 > 0.0) || !(prm->fire_dtmax > 0.0) || !(prm->fire_maxstep > 0.0)) return false;
+    return true;
+}
+
+size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
+    Dev d;
+    memset(&d, 0, sizeof d);
+    d.N = N;
+    d.Npad = (N + 31) / 32 * 32;
+    d.S = prm->max_images;
+    d.cap = prm->max_neighbors;
+    d.nblk_atom = (N + kThreadsAtom - 1) / kThreadsAtom;
+    d.nblk_stream = (d.Npad + kAtomsPerStreamBlock - 1) / kAtomsPerStreamBlock;
+    d.nbins_max = N > 64 ? N : 64;
+    const size_t S = d.S, Npad = d.Npad, img = 3 * Npad;
+    Carver c{static_cast<char *>(base), 0};
+    d.ctl = c.take<Ctl>(1);
+    d.order = c.take<int>(S);
+    d.geom = c.take<Geom>(S);
+    d.X = c.take<double>(2 * S * img);
+    d.v = c.take<double>(S * img);
+    d.F = c.take<double>(S * img);
+    d.Rc = c.take<double4>(S * Npad);
+    d.Sw = c.take<double4>(S * Npad);
+    d.binned = c.take<double4>(S * Npad);
+    d.Xc = c.take<double>(2 * S * 9);
+    d.vc = c.take<double>(S * 9);
+    d.E = c.take<double>(S);
+    d.V = c.take<double>(S * 9);
+    d.Gc = c.take<double>(S * 9);
+    d.dots = c.take<double>(S * kNDots);
+    d.coef = c.take<double>(S * 4);
+    d.part_force = c.take<double>(S * d.nblk_atom * kNForcePart);
+    d.part_dots = c.take<double>(S * d.nblk_stream * kNDots);
+    d.dispmax = c.take<unsigned long long>(S);
+    d.nbr_count = c.take<int>(S * Npad);
+    d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad);
+    d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
+    d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
+    d.bin_members = c.take<int>(S * Npad);
+    d.atom_bin = c.take<int>(S * Npad);
+    const size_t half = S * (size_t)(N + 3) * 3 * sizeof(double);
+    size_t sb = 2 * half + S * 16 * sizeof(double) + 1024;
+    const size_t nb = (size_t)N * d.cap * 4 * sizeof(int) + (size_t)N * sizeof(int) + 1024;
+    if (nb > sb) sb = nb;
+    d.scratch = c.take<char>(sb);
+    d.scratch_bytes = sb;
+    d.fneb = base ? reinterpret_cast<double *>(static_cast<char *>(d.scratch) + half) : nullptr;
+    if (out) *out = d;
+    return (c.off + 255) & ~(size_t)255;
+}
+
+void perp_widths(const double *h, double *w) {
+    const double vol = fabs(det3(h));
+    for (int a = 0; a < 3; ++a) {
+        const double *b = h + 3 * ((a + 1) % 3), *c = h + 3 * ((a + 2) % 3);
+        const double cx = b[1] * c[2] - b[2] * c[1], cy = b[2] * c[0] - b[0] * c[2], cz = b[0] * c[1] - b[1] * c[0];
+        w[a] = vol / sqrt(cx * cx + cy * cy + cz * cz);
+    }
+}
+
+int device_error(cfneb *h, int *code) {
+    CK(cudaMemcpyAsync(code, &h->d.ctl->error, sizeof(int), cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    return CFNEB_OK;
+}
+
+int sync_status(cfneb *h) {  // synchronise; surface launch errors and the sticky device error
+    int code = 0;
+    int rc = device_error(h, &code);
+    if (rc) return rc;
+    CK(cudaGetLastError());
+    return code;
+}
+
+void enqueue_step(cfneb *h, cudaEvent_t *ev) {
+    const Dev &d = h->d;
+    cudaStream_t st = h->st;
+    if (ev) cudaEventRecord(ev[0], st);
+    launch_cell_prep(d, 1, MODE_STEP, st);
+    if (ev) cudaEventRecord(ev[1], st);
+    launch_neighbor_build(d, 1, st);
+    if (ev) cudaEventRecord(ev[2], st);
+    launch_force(d, 1, st);
+    if (ev) cudaEventRecord(ev[3], st);
+    launch_reduce(d, st);
+    launch_finalize(d, 1, st);
+    if (ev) cudaEventRecord(ev[4], st);
+    launch_scalar(d, 0, st);
+    if (ev) cudaEventRecord(ev[5], st);
+    launch_update(d, st);
+    if (ev) cudaEventRecord(ev[6], st);
+}
+
+// Evaluate every image once at the current X (endpoint energies; fresh neighbour lists).
+void enqueue_evaluate_all(cfneb *h) {
+    const Dev &d = h->d;
+    launch_cell_prep(d, 0, MODE_STEP, h->st);
+    launch_neighbor_build(d, 0, h->st);
+    launch_force(d, 0, h->st);
+    launch_finalize(d, 0, h->st);
+}
+
+int force_rebuild_all(cfneb *h) {
+    std::vector<Geom> g(h->d.S);
+    CK(cudaMemcpyAsync(g.data(), h->d.geom, sizeof(Geom) * h->d.S, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    for (auto &x : g) { x.force_rebuild = 1; x.acc = 0.0; x.since = 0; }
+    CK(cudaMemcpyAsync(h->d.geom, g.data(), sizeof(Geom) * h->d.S, cudaMemcpyHostToDevice, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    return CFNEB_OK;
+}
+
+int upload_order(cfneb *h) {
+    std::vector<int> full(h->d.S, 0);
+    for (int p = 0; p < h->P; ++p) full[p] = h->order[p];
+    CK(cudaMemcpyAsync(h->d.order, full.data(), sizeof(int) * h->d.S, cudaMemcpyHostToDevice, h->st));
+    CK(cudaMemcpyAsync(&h->d.ctl->P, &h->P, sizeof(int), cudaMemcpyHostToDevice, h->st));
+    CK(cudaStreamSynchronize(h->st));  // the host vectors above are temporaries
+    return CFNEB_OK;
+}
+
+int capture_graph(cfneb *h) {
+    CK(cudaStreamBeginCapture(h->st, cudaStreamCaptureModeRelaxed));
+    enqueue_step(h, nullptr);
+    cudaGraph_t g = nullptr;
+    CK(cudaStreamEndCapture(h->st, &g));
+    h->graph = g;
+    CK(cudaGraphInstantiate(&h->exec, g, 0));
+    return CFNEB_OK;
+}
+}  // namespace
+
+extern "C" {
+
+void cfneb_default_params(cfneb_params *prm) {
+    if (!prm) return;
+    memset(prm, 0, sizeof *prm);
+    prm->potential = CFNEB_POT_LJ_SF;
+    prm->cell_mode = CFNEB_CELL_B;
+    prm->climb = 1;
+    prm->fire_nmin = 5;
+    prm->max_neighbors = 160;
+    prm->max_images = 16;
+    prm->rebuild_every = 0;
+    prm->pot[0] = 1.0; prm->pot[1] = 1.0; prm->pot[2] = 2.5;
+    prm->k_spring = 1.0;
+    prm->cell_factor = 1.0;
+    prm->fire_dt0 = 0.1; prm->fire_dtmax = 1.0; prm->fire_maxstep = 0.2;
+    prm->fire_finc = 1.1; prm->fire_fdec = 0.5; prm->fire_astart = 0.1; prm->fire_fa = 0.99;
+    prm->skin = 0.3;
+}
+
+size_t cfneb_workspace_bytes(int32_t n_atoms, const cfneb_params *prm) {
+    if (!valid_params(n_atoms, prm)) return 0;
+    return carve(n_atoms, prm, nullptr, nullptr);
+}
+
+int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const double *cell_init,
+                 const double *pos_final, const double *cell_final, int32_t n_images, const double *path_or_null,
+                 const cfneb_params *prm, void *dev_workspace, size_t ws_bytes, void *cuda_stream) {
+    if (!out) return CFNEB_EINVAL;
+    *out = nullptr;
+    if (!valid_params(n_atoms, prm) || !pos_init || !cell_init || !pos_final || !cell_final || !dev_workspace)
+        return CFNEB_EINVAL;
+    if (n_images < 3) return CFNEB_EINVAL;
+    if (n_images > prm->max_images) return CFNEB_ERANGE;
+    if (reinterpret_cast<uintptr_t>(dev_workspace) & 255u) return CFNEB_EINVAL;
+    if (ws_bytes < carve(n_atoms, prm, nullptr, nullptr)) return CFNEB_ENOMEM;
+    const double vol0 = det3(cell_init), vol1 = det3(cell_final);
+    if (!(fabs(vol0) > 0.0) || !(fabs(vol1) > 0.0) || !std::isfinite(vol0) || !std::isfinite(vol1)) return CFNEB_ECELL;
+
+    cfneb *h = new (std::nothrow) cfneb();
+    if (!h) return CFNEB_ENOMEM;
+    h->prm = *prm;
+    h->graph = nullptr;
+    h->exec = nullptr;
+    h->have_events = false;
+    h->own_stream = false;
+    h->st = static_cast<cudaStream_t>(cuda_stream);
+#define CKH(call)                                  \
+    do {                                           \
+        int rc_ = (call);                          \
+        if (rc_ != CFNEB_OK) { cfneb_destroy(h); return rc_; } \
+    } while (0)
+#define CKC(call)                                                                                      \
+    do {                                                                                               \
+        cudaError_t e_ = (call);                                                                       \
+        if (e_ != cudaSuccess) {                                                                       \
+            snprintf(g_cuda_err, sizeof g_cuda_err, "%s at %s:%d: %s", #call, __FILE__, __LINE__,     \
+                     cudaGetErrorString(e_));                                                          \
+            cfneb_destroy(h);                                                                          \
+            return CFNEB_ECUDA;                                                                        \
+        }                                                                                              \
+    } while (0)
+    if (!h->st) {
+        CKC(cudaStreamCreate(&h->st));
+        h->own_stream = true;
+    }
+    Dev &d = h->d;
+    carve(n_atoms, prm, dev_workspace, &d);
+    d.potential = prm->potential;
+    d.cell_mode = prm->cell_mode;
+    d.climb = prm->climb ? 1 : 0;
+    d.fire_nmin = prm->fire_nmin;
+    d.rebuild_every = prm->rebuild_every;
+    memcpy(d.pot, prm->pot, sizeof d.pot);
+    d.k_spring = prm->k_spring;
+    d.dt0 = prm->fire_dt0; d.dtmax = prm->fire_dtmax; d.maxstep = prm->fire_maxstep;
+    d.finc = prm->fire_finc; d.fdec = prm->fire_fdec; d.astart = prm->fire_astart; d.fa = prm->fire_fa;
+    d.skin = prm->skin;
+    d.r_cut = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
+    d.r_list = d.r_cut + d.skin;
+    memcpy(d.h0, cell_init, sizeof d.h0);  // A7: reference cell = cell of the initial endpoint
+    inv3(d.h0, d.h0inv);
+    // A13: lam = 0 selects Omega0^(1/3) N^(1/6); lam = 1 is the paper's equations literally
+    d.lam = prm->cell_factor > 0.0 ? prm->cell_factor : cbrt(fabs(vol0)) * pow((double)n_atoms, 1.0 / 6.0);
+    {  // per-axis bin caps from the larger endpoint cell, with headroom; product <= nbins_max
+        double w0[3], w1[3];
+        perp_widths(cell_init, w0);
+        perp_widths(cell_final, w1);
+        for (int a = 0; a < 3; ++a) {
+            const double w = fmax(w0[a], w1[a]) * 1.5;
+            d.nb_cap[a] = (int)floor(w / d.r_list);
+            if (d.nb_cap[a] < 3) d.nb_cap[a] = 3;
+        }
+        while ((long long)d.nb_cap[0] * d.nb_cap[1] * d.nb_cap[2] > d.nbins_max) {
+            int a = 0;
+            if (d.nb_cap[1] > d.nb_cap[a]) a = 1;
+            if (d.nb_cap[2] > d.nb_cap[a]) a = 2;
+            if (d.nb_cap[a] <= 3) break;
+            d.nb_cap[a] -= 1;
+        }
+        if ((long long)d.nb_cap[0] * d.nb_cap[1] * d.nb_cap[2] > d.nbins_max) { cfneb_destroy(h); return CFNEB_EINVAL; }
+    }
+    h->P = n_images;
+    h->order.resize(n_images);
+    for (int p = 0; p < n_images; ++p) h->order[p] = p;
+    for (int s = d.S - 1; s >= n_images; --s) h->free_slots.push_back(s);
+
+    CKC(cudaMemsetAsync(dev_workspace, 0, carve(n_atoms, prm, nullptr, nullptr), h->st));
+    Ctl c0;
+    memset(&c0, 0, sizeof c0);
+    c0.P = n_images;
+    c0.first = 1;
+    c0.pstar = -1;
+    c0.dt = d.dt0;
+    c0.alpha = d.astart;
+    CKC(cudaMemcpyAsync(d.ctl, &c0, sizeof c0, cudaMemcpyHostToDevice, h->st));
+    CKH(upload_order(h));
+
+    // stage the host inputs: pos [n][N][3] then cells [n][9]
+    const size_t N3 = (size_t)n_atoms * 3;
+    const int n_in = path_or_null ? n_images : 2;
+    std::vector<double> stage((size_t)n_in * (N3 + 9));
+    double *spos = stage.data(), *scell = stage.data() + (size_t)n_in * N3;
+    memcpy(spos, pos_init, N3 * sizeof(double));
+    memcpy(scell, cell_init, 9 * sizeof(double));
+    memcpy(spos + (size_t)(n_in - 1) * N3, pos_final, N3 * sizeof(double));
+    memcpy(scell + (size_t)(n_in - 1) * 9, cell_final, 9 * sizeof(double));
+    if (path_or_null)
+        for (int q = 0; q < n_images - 2; ++q) {
+            const double *blk = path_or_null + (size_t)q * (N3 + 9);
+            memcpy(spos + (size_t)(q + 1) * N3, blk, N3 * sizeof(double));
+            memcpy(scell + (size_t)(q + 1) * 9, blk + N3, 9 * sizeof(double));
+            const double v = det3(blk + N3);
+            if (!(fabs(v) > 0.0) || !std::isfinite(v)) { cfneb_destroy(h); return CFNEB_ECELL; }
+        }
+    double *dstage = static_cast<double *>(d.scratch);
+    CKC(cudaMemcpyAsync(dstage, stage.data(), stage.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
+    const double *dpos = dstage, *dcell = dstage + (size_t)n_in * N3;
+    if (path_or_null) {
+        launch_input_map(d, dpos, dcell, 0, n_images, h->st);
+    } else {
+        launch_input_map(d, dpos, dcell, 0, 1, h->st);
+        launch_input_map(d, dpos + N3, dcell + 9, n_images - 1, 1, h->st);
+        launch_interpolate(d, n_images, h->st);
+    }
+    CKC(cudaStreamSynchronize(h->st));  // `stage` is a temporary
+    CKH(force_rebuild_all(h));
+    enqueue_evaluate_all(h);
+    int rc = sync_status(h);
+    if (rc) { cfneb_destroy(h); return rc; }
+    CKH(capture_graph(h));
+    for (int k = 0; k <= CFNEB_NKERNELS; ++k) CKC(cudaEventCreate(&h->ev[k]));
+    h->have_events = true;
+    *out = h;
+    return CFNEB_OK;
+#undef CKH
+#undef CKC
+}
+
+int cfneb_step(cfneb_t *h, int32_t n_steps) {
+    if (!h || n_steps < 0) return CFNEB_EINVAL;
+    for (int k = 0; k < n_steps; ++k) CK(cudaGraphLaunch(h->exec, h->st));
+    return CFNEB_OK;
+}
+
+int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms) {
+    if (!h || n_steps < 0 || !kernel_ms) return CFNEB_EINVAL;
+    for (int k = 0; k < n_steps; ++k) {
+        enqueue_step(h, h->ev);
+        CK(cudaEventSynchronize(h->ev[CFNEB_NKERNELS]));
+        for (int c = 0; c < CFNEB_NKERNELS; ++c) {
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, h->ev[c], h->ev[c + 1]));
+            kernel_ms[c] += (double)ms;
+        }
+    }
+    return sync_status(h);
+}
+
+int cfneb_insert_image(cfneb_t *h, int32_t after) {
+    if (!h) return CFNEB_EINVAL;
+    if (after < 0 || after > h->P - 2) return CFNEB_ERANGE;
+    if (h->P >= h->d.S || h->free_slots.empty()) return CFNEB_ERANGE;
+    int pstar = -1;
+    CK(cudaMemcpyAsync(&pstar, &h->d.ctl->pstar, sizeof(int), cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    if (pstar > after) {  // keep the reported climbing index on the same image until the next step
+        pstar += 1;
+        CK(cudaMemcpyAsync(&h->d.ctl->pstar, &pstar, sizeof(int), cudaMemcpyHostToDevice, h->st));
+        CK(cudaStreamSynchronize(h->st));
+    }
+    const int sn = h->free_slots.back();
+    h->free_slots.pop_back();
+    launch_midpoint(h->d, h->order[after], h->order[after + 1], sn, h->st);
+    h->order.insert(h->order.begin() + after + 1, sn);
+    h->P += 1;
+    int rc = upload_order(h);
+    if (rc) return rc;
+    launch_reset_fire(h->d, h->st);
+    CK(cudaGetLastError());
+    return CFNEB_OK;
+}
+
+int cfneb_delete_image(cfneb_t *h, int32_t index) {
+    if (!h) return CFNEB_EINVAL;
+    if (index < 1 || index > h->P - 2 || h->P <= 3) return CFNEB_ERANGE;
+    int pstar = -1;
+    CK(cudaMemcpyAsync(&pstar, &h->d.ctl->pstar, sizeof(int), cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    if (index == pstar) return CFNEB_ERANGE;
+    h->free_slots.push_back(h->order[index]);
+    h->order.erase(h->order.begin() + index);
+    h->P -= 1;
+    if (pstar > index) {  // keep the reported climbing index on the same image until the next step
+        pstar -= 1;
+        CK(cudaMemcpyAsync(&h->d.ctl->pstar, &pstar, sizeof(int), cudaMemcpyHostToDevice, h->st));
+        CK(cudaStreamSynchronize(h->st));
+    }
+    int rc = upload_order(h);
+    if (rc) return rc;
+    launch_reset_fire(h->d, h->st);
+    CK(cudaGetLastError());
+    return CFNEB_OK;
+}
+
+int cfneb_get_segment_lengths(cfneb_t *h, double *dl) {
+    if (!h || !dl) return CFNEB_EINVAL;
+    double *dev = static_cast<double *>(h->d.scratch);
+    launch_segment_lengths(h->d, dev, h->st);
+    CK(cudaMemcpyAsync(dl, dev, sizeof(double) * (h->P - 1), cudaMemcpyDeviceToHost, h->st));
+    return sync_status(h);
+}
+
+int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, int32_t *n_del) {
+    if (!h) return CFNEB_EINVAL;
+    if (n_ins) *n_ins = 0;
+    if (n_del) *n_del = 0;
+    std::vector<double> dl(h->d.S);
+    int rc = cfneb_get_segment_lengths(h, dl.data());
+    if (rc) return rc;
+    int pstar = -1;
+    CK(cudaMemcpyAsync(&pstar, &h->d.ctl->pstar, sizeof(int), cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    // (i) delete the interior, non-climbing image q minimising d_{q-1} + d_q if below d_delete and P > 3
+    if (h->P > 3) {
+        int best = -1;
+        double bs = 0.0;
+        for (int q = 1; q <= h->P - 2; ++q) {
+            if (q == pstar) continue;
+            const double s = dl[q - 1] + dl[q];
+            if (best < 0 || s < bs) { best = q; bs = s; }
+        }
+        if (best > 0 && bs < d_delete) {
+            rc = cfneb_delete_image(h, best);
+            if (rc) return rc;
+            if (n_del) *n_del = 1;
+            rc = cfneb_get_segment_lengths(h, dl.data());
+            if (rc) return rc;
+        }
+    }
+    // (ii) insert at the midpoint of the longest segment if above d_insert and P < max_images
+    int q = 0;
+    for (int k = 1; k <= h->P - 2; ++k)
+        if (dl[k] > dl[q]) q = k;
+    if (dl[q] > d_insert && h->P < h->d.S) {
+        rc = cfneb_insert_image(h, q);
+        if (rc) return rc;
+        if (n_ins) *n_ins = 1;
+    }
+    return sync_status(h);
+}
+
+int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, double *energies) {
+    if (!h) return CFNEB_EINVAL;
+    const Dev &d = h->d;
+    const size_t N3 = (size_t)d.N * 3, P = h->P;
+    double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3, *dE = dcell + P * 9;
+    launch_cell_prep(d, 0, MODE_GEOMETRY_ONLY, h->st);
+    launch_export_path(d, dpos, dcell, dE, h->st);
+    if (pos) CK(cudaMemcpyAsync(pos, dpos, P * N3 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (cells) CK(cudaMemcpyAsync(cells, dcell, P * 9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (energies) CK(cudaMemcpyAsync(energies, dE, P * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (n_images) *n_images = h->P;
+    return sync_status(h);
+}
+
+int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells) {
+    if (!h || !pos || !cells) return CFNEB_EINVAL;
+    const Dev &d = h->d;
+    const size_t N3 = (size_t)d.N * 3, P = h->P;
+    double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3;
+    CK(cudaMemcpyAsync(dpos, pos, P * N3 * sizeof(double), cudaMemcpyHostToDevice, h->st));
+    CK(cudaMemcpyAsync(dcell, cells, P * 9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
+    launch_input_map(d, dpos, dcell, 0, h->P, h->st);
+    launch_reset_fire(d, h->st);
+    int rc = force_rebuild_all(h);
+    if (rc) return rc;
+    enqueue_evaluate_all(h);
+    return sync_status(h);
+}
+
+int cfneb_get_state(cfneb_t *h, double *X, double *v) {
+    if (!h) return CFNEB_EINVAL;
+    const Dev &d = h->d;
+    const size_t n = (size_t)h->P * (d.N + 3) * 3;
+    double *dX = static_cast<double *>(d.scratch), *dv = dX + n;
+    launch_export_state(d, dX, dv, h->st);
+    if (X) CK(cudaMemcpyAsync(X, dX, n * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (v) CK(cudaMemcpyAsync(v, dv, n * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    return sync_status(h);
+}
+
+int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, double *energies) {
+    if (!h) return CFNEB_EINVAL;
+    const Dev &d = h->d;
+    const size_t N3 = (size_t)d.N * 3, P = h->P;
+    launch_cell_prep(d, 1, MODE_STEP, h->st);
+    launch_neighbor_build(d, 1, h->st);
+    launch_force(d, 1, h->st);
+    launch_reduce(d, h->st);
+    launch_finalize(d, 1, h->st);
+    launch_scalar(d, 1, h->st);
+    launch_materialize_fneb(d, h->st);
+    double *dF = static_cast<double *>(d.scratch), *dV = dF + P * N3, *dE = dV + P * 9;
+    launch_export_forces(d, dF, dV, dE, h->st);
+    if (F) CK(cudaMemcpyAsync(F, dF, P * N3 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (virial) CK(cudaMemcpyAsync(virial, dV, P * 9 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (energies) CK(cudaMemcpyAsync(energies, dE, P * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (f_neb)
+        CK(cudaMemcpyAsync(f_neb, d.fneb, P * (size_t)(d.N + 3) * 3 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    return sync_status(h);
+}
+
+int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int32_t *list, int32_t *shift) {
+    if (!h) return CFNEB_EINVAL;
+    if (image < 0 || image >= h->P) return CFNEB_ERANGE;
+    const Dev &d = h->d;
+    const int slot = h->order[image];
+    const int one = 1;
+    CK(cudaMemcpyAsync(&d.geom[slot].force_rebuild, &one, sizeof(int), cudaMemcpyHostToDevice, h->st));
+    launch_cell_prep(d, 0, MODE_STEP, h->st);
+    launch_neighbor_build(d, 0, h->st);
+    const size_t n = (size_t)d.N * d.cap;
+    int *dcount = static_cast<int *>(d.scratch), *dlist = dcount + ((d.N + 63) / 64) * 64, *dshift = dlist + n;
+    launch_unpack_neighbors(d, slot, dcount, dlist, dshift, h->st);
+    if (count) CK(cudaMemcpyAsync(count, dcount, sizeof(int) * d.N, cudaMemcpyDeviceToHost, h->st));
+    if (list) CK(cudaMemcpyAsync(list, dlist, sizeof(int) * n, cudaMemcpyDeviceToHost, h->st));
+    if (shift) CK(cudaMemcpyAsync(shift, dshift, sizeof(int) * 3 * n, cudaMemcpyDeviceToHost, h->st));
+    return sync_status(h);
+}
+
+int cfneb_get_status(cfneb_t *h, cfneb_status *out) {
+    if (!h || !out) return CFNEB_EINVAL;
+    Ctl c;
+    CK(cudaMemcpyAsync(&c, h->d.ctl, sizeof c, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    memset(out, 0, sizeof *out);
+    out->steps = (int64_t)c.steps;
+    out->rebuilds = (int64_t)c.rebuilds;
+    out->n_images = c.P;
+    out->climb_index = c.pstar;
+    out->error = c.error;
+    out->n_pos = c.n_pos;
+    out->max_neighbors_seen = c.max_nbr_seen;
+    unsigned long long b = c.fmax_bits;
+    double f2;
+    memcpy(&f2, &b, sizeof f2);
+    out->fmax = sqrt(f2);
+    out->barrier = c.barrier;
+    out->dt = c.dt;
+    out->alpha = c.alpha;
+    out->cell_factor = h->d.lam;
+    out->path_length = c.path_length;
+    CK(cudaGetLastError());
+    return CFNEB_OK;
+}
+
+void cfneb_destroy(cfneb_t *h) {
+    if (!h) return;
+    if (h->st) cudaStreamSynchronize(h->st);
+    if (h->exec) cudaGraphExecDestroy(h->exec);
+    if (h->graph) cudaGraphDestroy(h->graph);
+    if (h->have_events)
+        for (int k = 0; k <= CFNEB_NKERNELS; ++k) cudaEventDestroy(h->ev[k]);
+    if (h->own_stream && h->st) cudaStreamDestroy(h->st);
+    delete h;
+}
+
+const char *cfneb_strerror(int code) {
+    switch (code) {
+        case CFNEB_OK: return "ok";
+        case CFNEB_EINVAL: return "invalid argument (or zero tangent)";
+        case CFNEB_ENOMEM: return "workspace too small";
+        case CFNEB_ECUDA: return "CUDA runtime error";
+        case CFNEB_ENEIGH_OVERFLOW: return "neighbour list overflow (raise max_neighbors)";
+        case CFNEB_ECELL: return "cell not positive definite / singular / periodic shift out of range";
+        case CFNEB_ENAN: return "NaN or Inf in energies or reductions";
+        case CFNEB_ERANGE: return "image index out of range / endpoint or climbing image / band full";
+        default: return "unknown error";
+    }
+}
+
+const char *cfneb_last_cuda_error(void) { return g_cuda_err; }
+
+int cfneb_util_fp64_peak(void *cuda_stream, double *tflops) {
+    if (!tflops) return CFNEB_EINVAL;
+    const double t = run_fp64_peak(static_cast<cudaStream_t>(cuda_stream));
+    if (!(t > 0.0)) {
+        snprintf(g_cuda_err, sizeof g_cuda_err, "fp64 peak kernel failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return CFNEB_ECUDA;
+    }
+    *tflops = t;
+    return CFNEB_OK;
+}
+
+}  // extern "C"

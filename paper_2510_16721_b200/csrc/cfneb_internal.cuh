@@ -1,0 +1,190 @@
+// cfneb_internal.cuh -- device-side layout and launch wrappers shared by the CUDA translation units.
+// (Product code: shares nothing with oracle/.)
+//
+// HBM layout (fp64 SoA, one "slot" per image; path position p -> slot through the order table, so
+// insertion / deletion never moves atom data):
+//   X    [2][S][3][Npad]   R~ of Eq. 10, double-buffered (K6 reads X_{p-1}, X_p, X_{p+1} of buffer src,
+//                          writes buffer dst); rows padded with zeros to Npad (multiple of 32)
+//   v, F [S][3][Npad]      FIRE velocity, Cartesian force (Eq. 5)
+//   Rc   [S][Npad] double4 Cartesian position R = R~ D packed as one 32-byte sector per atom;
+//                          .w carries F'(rho_i) between the two Finnis-Sinclair passes
+//   Xc   [2][S][9], vc [S][9]   cell block lam*B (Eq. 17) and its velocity
+//   nbr_list [S][cap][Npad] uint32: j | shift code << 23, k-major so that a warp reads 128 contiguous bytes
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/cfneb.h"
+
+namespace cfn {
+
+constexpr int kThreadsAtom = 128;      // force / neighbour / position kernels: 1 atom per thread
+constexpr int kThreadsStream = 256;    // K4 / K6: 2 atoms per thread (double2)
+constexpr int kAtomsPerStreamBlock = kThreadsStream * 2;
+constexpr int kNDots = 10;             // pp, mm, pm, Gp, Gm, GG, Gv, pv, mv, vv
+constexpr int kNForcePart = 8;         // E, Vxx, Vyy, Vzz, Vxy, Vxz, Vyz, (embedding energy)
+constexpr uint32_t kIdxMask = 0x7FFFFFu;
+constexpr int kShiftBits = 23;
+constexpr uint32_t kCodeCenter = 4u | (4u << 3) | (4u << 6);
+constexpr int kMaxAtoms = 1 << 23;
+
+enum { DOT_PP = 0, DOT_MM, DOT_PM, DOT_GP, DOT_GM, DOT_GG, DOT_GV, DOT_PV, DOT_MV, DOT_VV };
+
+// Device-resident control block: everything the graph needs to run step after step with no host round trip.
+struct Ctl {
+    int P;            // current number of images
+    int cur;          // X buffer holding the latest coordinates
+    int src, dst;     // set by K5 for K6 of the same step
+    int error;        // sticky CFNEB_E* code
+    int first;        // FIRE: skip the power test on the first step after a (re)start (A2)
+    int n_pos;
+    int pstar;        // climbing image (path position) of the last step
+    int max_nbr_seen;
+    int pad0;
+    unsigned long long steps;
+    unsigned long long rebuilds;
+    double dt, alpha;
+    double cv, cf, sdt;   // K6: v_new = cv v + cf f ; X_new = X + sdt v_new
+    unsigned long long fmax_bits;  // max row norm^2 of f as ordered bits (atomicMax target)
+    double barrier, path_length;
+};
+
+// Per-slot geometry written by K0.
+struct Geom {
+    double D[9], Dinv[9], h[9], Dlast[9];
+    double vol;
+    double acc;        // accumulated bound on pair-distance change since the last list build
+    int nb[3];         // bins per axis (>= 3: adjacent-bin stencil; 1: explicit periodic shifts)
+    int reach[3];      // stencil half-width per axis
+    int rebuild;       // this step rebuilds the list of this slot
+    int force_rebuild; // set by host paths (create / insert / set_path)
+    int since;         // steps since last build
+    int pad;
+};
+
+struct Dev {
+    int N, Npad, S, cap;
+    int potential, cell_mode, climb, fire_nmin, rebuild_every;
+    int nblk_atom, nblk_stream, nbins_max;
+    int nb_cap[3];
+    double pot[12];
+    double k_spring, lam;
+    double dt0, dtmax, maxstep, finc, fdec, astart, fa;
+    double skin, r_cut, r_list;
+    double h0[9], h0inv[9];
+    Ctl *ctl;
+    int *order;               // [S] path position -> slot
+    Geom *geom;               // [S]
+    double *X, *v, *F;        // see header comment
+    double *fneb;             // parity-hook scratch [S][(N+3)*3], external row-major layout
+    double4 *Rc;
+    double4 *Sw;              // [S][Npad] wrapped fractional coordinates + packed floors, for the list build
+    double4 *binned;          // [S][Npad] Sw in bin order, .w = packed (atom index, floors)
+    double *Xc, *vc;
+    double *E, *V, *Gc;       // [S], [S][9], [S][9]
+    double *dots, *coef;      // [S][10], [S][4]
+    double *part_force;       // [S][nblk_atom][8]
+    double *part_dots;        // [S][nblk_stream][10]
+    unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
+    int *nbr_count;           // [S][Npad]
+    uint32_t *nbr_list;       // [S][cap][Npad]
+    int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
+    int *bin_cursor;          // [S][nbins_max]
+    int *bin_members;         // [S][Npad]
+    int *atom_bin;            // [S][Npad]
+    void *scratch;            // staging for host transfers / hooks
+    size_t scratch_bytes;
+};
+
+// ---- small 3x3 helpers, row-major ----
+__host__ __device__ inline double det3(const double *m) {
+    return m[0] * (m[4] * m[8] - m[5] * m[7]) - m[1] * (m[3] * m[8] - m[5] * m[6]) + m[2] * (m[3] * m[7] - m[4] * m[6]);
+}
+__host__ __device__ inline void inv3(const double *m, double *o) {
+    double id = 1.0 / det3(m);
+    o[0] = (m[4] * m[8] - m[5] * m[7]) * id; o[1] = (m[2] * m[7] - m[1] * m[8]) * id; o[2] = (m[1] * m[5] - m[2] * m[4]) * id;
+    o[3] = (m[5] * m[6] - m[3] * m[8]) * id; o[4] = (m[0] * m[8] - m[2] * m[6]) * id; o[5] = (m[2] * m[3] - m[0] * m[5]) * id;
+    o[6] = (m[3] * m[7] - m[4] * m[6]) * id; o[7] = (m[1] * m[6] - m[0] * m[7]) * id; o[8] = (m[0] * m[4] - m[1] * m[3]) * id;
+}
+__host__ __device__ inline void mul3(const double *a, const double *b, double *c) {  // c = a b
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) c[3 * i + j] = a[3 * i] * b[j] + a[3 * i + 1] * b[3 + j] + a[3 * i + 2] * b[6 + j];
+}
+__host__ __device__ inline void mul3_abt(const double *a, const double *b, double *c) {  // c = a b^T
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) c[3 * i + j] = a[3 * i] * b[3 * j] + a[3 * i + 1] * b[3 * j + 1] + a[3 * i + 2] * b[3 * j + 2];
+}
+__host__ __device__ inline void mul3_atb(const double *a, const double *b, double *c) {  // c = a^T b
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) c[3 * i + j] = a[i] * b[j] + a[3 + i] * b[3 + j] + a[6 + i] * b[6 + j];
+}
+
+// launch modes
+enum { MODE_STEP = 0, MODE_GEOMETRY_ONLY = 1 };
+
+// ---- launch wrappers (each enqueues on `st`; p_lo = 1: movable images, 0: all images) ----
+void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_dev, int p_first, int count, cudaStream_t st);
+void launch_interpolate(const Dev &d, int P, cudaStream_t st);
+void launch_cell_prep(const Dev &d, int p_lo, int mode, cudaStream_t st);                 // K0 + positions
+void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st);                      // K1
+void launch_force(const Dev &d, int p_lo, cudaStream_t st);                               // K2
+void launch_reduce(const Dev &d, cudaStream_t st);                                        // K4 (atom rows)
+void launch_finalize(const Dev &d, int p_lo, cudaStream_t st);                            // K4 second stage
+void launch_scalar(const Dev &d, int dry, cudaStream_t st);                               // K5
+void launch_update(const Dev &d, cudaStream_t st);                                        // K6
+void launch_materialize_fneb(const Dev &d, cudaStream_t st);                              // parity hook
+void launch_midpoint(const Dev &d, int slot_a, int slot_b, int slot_new, cudaStream_t st);  // K7
+void launch_reset_fire(const Dev &d, cudaStream_t st);
+void launch_segment_lengths(const Dev &d, double *out_dev, cudaStream_t st);
+void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_out, int *shift_out, cudaStream_t st);
+void launch_export_path(const Dev &d, double *pos_out, double *cells_out, double *E_out, cudaStream_t st);
+void launch_export_state(const Dev &d, double *X_out, double *v_out, cudaStream_t st);
+void launch_export_forces(const Dev &d, double *F_out, double *V_out, double *E_out, cudaStream_t st);
+double run_fp64_peak(cudaStream_t st);
+
+// ordered-bits helpers for atomicMax on non-negative doubles
+__device__ inline unsigned long long nonneg_bits(double x) { return (unsigned long long)__double_as_longlong(x); }
+__device__ inline double bits_nonneg(unsigned long long b) { return __longlong_as_double((long long)b); }
+
+__device__ inline void set_error(Ctl *ctl, int code) { atomicCAS(&ctl->error, 0, code); }
+
+// block-wide sum of NV values per thread; result valid in thread 0. blockDim.x a multiple of 32, <= 1024.
+// Fixed tree: the result depends only on the inputs, never on scheduling (bitwise repeatable).
+template <int NV>
+__device__ inline void block_sum(double (&val)[NV], double *smem /* [32*NV] */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int q = 0; q < NV; ++q) {
+        double x = val[q];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+        if (lane == 0) smem[warp * NV + q] = x;
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            double x = (lane < nwarp) ? smem[lane * NV + q] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
+            val[q] = x;
+        }
+    }
+    __syncthreads();
+}
+
+__device__ inline double block_max(double x, double *smem /* [32] */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_down_sync(0xffffffffu, x, o));
+    if (lane == 0) smem[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+        x = (lane < nwarp) ? smem[lane] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x = fmax(x, __shfl_down_sync(0xffffffffu, x, o));
+    }
+    __syncthreads();
+    return x;  // valid in thread 0
+}
+
+}  // namespace cfn

@@ -1,0 +1,274 @@
+// kernels_neb.cu -- the band-level half of the iteration: K4 segmented reductions, K5 scalar kernel
+// (improved tangent, climbing image, FIRE scalars), K6 fused NEB force + cell filter + FIRE update.
+//
+// Per movable image p with tau+ = X_{p+1} - X_p, tau- = X_p - X_{p-1} (generalized coordinates
+// X = [R~ ; lam B], Eq. 17) and generalized force G = [F D^T ; D^-T V D^-1 / lam] (Eq. 12, 17):
+//   tangent (ref [13])  tau = a tau+ + b tau-  with (a, b) chosen from E_{p-1}, E_p, E_{p+1}
+//   Eq. 1           f = G - (G.t)t + k(|tau+| - |tau-|) t ,  t = tau/|tau|
+//   climbing image (ref [12]) f = G - 2 (G.t) t
+// Both have the form f = G + c1 tau+ + c2 tau- with per-image scalars c1, c2, so every band-level scalar
+// FIRE needs (f.v, |f|, |v|, |v_new|) follows from ten dot products per image taken in ONE pass over
+// X, F, v (K4); K6 then streams the same arrays once more and writes X_new, v_new.
+#include "cfneb_internal.cuh"
+
+namespace cfn {
+
+__device__ inline double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
+__device__ inline void st2(double *p, double2 v) { *reinterpret_cast<double2 *>(p) = v; }
+
+// ------------------------------------------------------------------------------------------------
+// K4: ten dot products over the atom rows of each movable image; per-block partials.
+// grid (nblk_stream, S-2), 256 threads, two atoms per thread (128-bit loads on SoA rows).
+__global__ void __launch_bounds__(kThreadsStream) reduce_kernel(Dev d) {
+    const int p = blockIdx.y + 1;
+    if (p > d.ctl->P - 2) return;
+    const int sm = d.order[p - 1], s0 = d.order[p], sp = d.order[p + 1];
+    __shared__ double sD[9];
+    __shared__ double red[32 * kNDots];
+    if (threadIdx.x < 9) sD[threadIdx.x] = d.geom[s0].D[threadIdx.x];
+    __syncthreads();
+    const size_t img = (size_t)3 * d.Npad;
+    const double *Xb = d.X + (size_t)d.ctl->cur * d.S * img;
+    const double *Xm = Xb + sm * img, *X0 = Xb + s0 * img, *Xp = Xb + sp * img;
+    const double *F = d.F + s0 * img, *V = d.v + s0 * img;
+    const int i = 2 * (blockIdx.x * kThreadsStream + threadIdx.x);
+    double acc[kNDots];
+#pragma unroll
+    for (int q = 0; q < kNDots; ++q) acc[q] = 0.0;
+    if (i < d.Npad) {
+        double2 f[3], xm[3], x0[3], xp[3], vv[3];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            const size_t o = (size_t)c * d.Npad + i;
+            f[c] = ld2(F + o);
+            xm[c] = ld2(Xm + o);
+            x0[c] = ld2(X0 + o);
+            xp[c] = ld2(Xp + o);
+            vv[c] = ld2(V + o);
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            // G = F D^T (Eq. 12): G_c = sum_m F_m D[c][m]
+            const double gx = f[0].x * sD[3 * c] + f[1].x * sD[3 * c + 1] + f[2].x * sD[3 * c + 2];
+            const double gy = f[0].y * sD[3 * c] + f[1].y * sD[3 * c + 1] + f[2].y * sD[3 * c + 2];
+            const double tpx = xp[c].x - x0[c].x, tpy = xp[c].y - x0[c].y;
+            const double tmx = x0[c].x - xm[c].x, tmy = x0[c].y - xm[c].y;
+            acc[DOT_PP] += tpx * tpx + tpy * tpy;
+            acc[DOT_MM] += tmx * tmx + tmy * tmy;
+            acc[DOT_PM] += tpx * tmx + tpy * tmy;
+            acc[DOT_GP] += gx * tpx + gy * tpy;
+            acc[DOT_GM] += gx * tmx + gy * tmy;
+            acc[DOT_GG] += gx * gx + gy * gy;
+            acc[DOT_GV] += gx * vv[c].x + gy * vv[c].y;
+            acc[DOT_PV] += tpx * vv[c].x + tpy * vv[c].y;
+            acc[DOT_MV] += tmx * vv[c].x + tmy * vv[c].y;
+            acc[DOT_VV] += vv[c].x * vv[c].x + vv[c].y * vv[c].y;
+        }
+    }
+    block_sum<kNDots>(acc, red);
+    if (threadIdx.x == 0) {
+        double *out = d.part_dots + ((size_t)s0 * d.nblk_stream + blockIdx.x) * kNDots;
+#pragma unroll
+        for (int q = 0; q < kNDots; ++q) out[q] = acc[q];
+    }
+}
+
+// K4 second stage, one block per image: E, V from the force partials; G_cell (Eq. 17 / Eq. 14); the ten
+// dots completed with the three cell rows.  Fixed summation order (bitwise repeatable).
+__global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
+    const int p = blockIdx.x + p_lo;
+    const int P = d.ctl->P;
+    if (p > P - 1 - p_lo) return;
+    const int slot = d.order[p];
+    __shared__ double red[32 * kNDots];
+    __shared__ double sGc[9];
+    double a8[kNForcePart];
+#pragma unroll
+    for (int q = 0; q < kNForcePart; ++q) a8[q] = 0.0;
+    const double *pf = d.part_force + (size_t)slot * d.nblk_atom * kNForcePart;
+    for (int b = threadIdx.x; b < d.nblk_atom; b += blockDim.x)
+#pragma unroll
+        for (int q = 0; q < kNForcePart; ++q) a8[q] += pf[(size_t)b * kNForcePart + q];
+    block_sum<kNForcePart>(a8, red);
+    if (threadIdx.x == 0) {
+        const double E = a8[0] + a8[7];
+        const double V[9] = {a8[1], a8[4], a8[5], a8[4], a8[2], a8[6], a8[5], a8[6], a8[3]};
+        d.E[slot] = E;
+        double Gc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+        const Geom *g = d.geom + slot;
+        if (d.cell_mode != CFNEB_CELL_FIXED) {
+            double T[9];
+            mul3_atb(g->Dinv, V, T);  // D^-T V   (Eq. 13-14)
+            if (d.cell_mode == CFNEB_CELL_B) mul3(T, g->Dinv, Gc);  // D^-T V D^-1 (Eq. 16-17, as printed)
+            else for (int k = 0; k < 9; ++k) Gc[k] = T[k];
+            for (int k = 0; k < 9; ++k) Gc[k] /= d.lam;
+        }
+        for (int k = 0; k < 9; ++k) {
+            d.V[slot * 9 + k] = V[k];
+            d.Gc[slot * 9 + k] = Gc[k];
+            sGc[k] = Gc[k];
+        }
+        if (!isfinite(E)) set_error(d.ctl, CFNEB_ENAN);
+    }
+    if (p < 1 || p > P - 2) return;  // endpoints: energy only (block-uniform)
+    __syncthreads();
+    double a10[kNDots];
+#pragma unroll
+    for (int q = 0; q < kNDots; ++q) a10[q] = 0.0;
+    const double *pd = d.part_dots + (size_t)slot * d.nblk_stream * kNDots;
+    for (int b = threadIdx.x; b < d.nblk_stream; b += blockDim.x)
+#pragma unroll
+        for (int q = 0; q < kNDots; ++q) a10[q] += pd[(size_t)b * kNDots + q];
+    block_sum<kNDots>(a10, red);
+    if (threadIdx.x == 0) {
+        const int sm = d.order[p - 1], sp = d.order[p + 1];
+        const double *Xc = d.Xc + (size_t)d.ctl->cur * d.S * 9;
+        for (int k = 0; k < 9; ++k) {
+            const double tp = Xc[sp * 9 + k] - Xc[slot * 9 + k], tm = Xc[slot * 9 + k] - Xc[sm * 9 + k];
+            const double g = sGc[k], v = d.vc[slot * 9 + k];
+            a10[DOT_PP] += tp * tp; a10[DOT_MM] += tm * tm; a10[DOT_PM] += tp * tm;
+            a10[DOT_GP] += g * tp;  a10[DOT_GM] += g * tm;  a10[DOT_GG] += g * g;
+            a10[DOT_GV] += g * v;   a10[DOT_PV] += tp * v;  a10[DOT_MV] += tm * v;  a10[DOT_VV] += v * v;
+        }
+        for (int q = 0; q < kNDots; ++q) d.dots[slot * kNDots + q] = a10[q];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// K5: one block.  Tangent weights and c1, c2 per image in parallel; band totals and the FIRE state
+// machine (O7: one state for the whole band, readings A1-A4) by thread 0 in path order.
+__global__ void __launch_bounds__(128) scalar_kernel(Dev d, int dry) {
+    Ctl *ctl = d.ctl;
+    const int P = ctl->P;
+    __shared__ int s_pstar;
+    if (threadIdx.x == 0) {
+        int ps = -1;
+        if (d.climb) {  // climbing image: argmax of interior energies, lowest index on an exact tie
+            double best = 0.0;
+            for (int p = 1; p <= P - 2; ++p) {
+                const double e = d.E[d.order[p]];
+                if (ps < 0 || e > best) { best = e; ps = p; }
+            }
+        }
+        s_pstar = ps;
+    }
+    __syncthreads();
+    const int pstar = s_pstar;
+    for (int p = 1 + threadIdx.x; p <= P - 2; p += blockDim.x) {
+        const int slot = d.order[p];
+        const double Em = d.E[d.order[p - 1]], E0 = d.E[slot], Ep = d.E[d.order[p + 1]];
+        const double *dt = d.dots + slot * kNDots;
+        double a, b;  // tau = a tau+ + b tau-   (improved tangent, ref [13])
+        if (Ep > E0 && E0 > Em) { a = 1.0; b = 0.0; }
+        else if (Ep < E0 && E0 < Em) { a = 0.0; b = 1.0; }
+        else {
+            const double dp = fabs(Ep - E0), dm = fabs(Em - E0);
+            const double dmax = fmax(dp, dm), dmin = fmin(dp, dm);
+            if (Ep > Em) { a = dmax; b = dmin; } else { a = dmin; b = dmax; }
+        }
+        const double t2 = a * a * dt[DOT_PP] + 2.0 * a * b * dt[DOT_PM] + b * b * dt[DOT_MM];
+        double c1 = 0.0, c2 = 0.0;
+        if (!(t2 > 0.0)) set_error(ctl, isfinite(t2) ? CFNEB_EINVAL : CFNEB_ENAN);
+        else {
+            const double nt = sqrt(t2);
+            const double Gt = (a * dt[DOT_GP] + b * dt[DOT_GM]) / nt;  // G . t^
+            double coef;
+            if (p == pstar) coef = -2.0 * Gt;
+            else coef = -Gt + d.k_spring * (sqrt(dt[DOT_PP]) - sqrt(dt[DOT_MM]));
+            c1 = coef * a / nt;
+            c2 = coef * b / nt;
+        }
+        double *co = d.coef + slot * 4;
+        co[0] = c1;
+        co[1] = c2;
+        co[2] = dt[DOT_GV] + c1 * dt[DOT_PV] + c2 * dt[DOT_MV];  // f . v
+        co[3] = dt[DOT_GG] + c1 * c1 * dt[DOT_PP] + c2 * c2 * dt[DOT_MM] +
+                2.0 * (c1 * dt[DOT_GP] + c2 * dt[DOT_GM] + c1 * c2 * dt[DOT_PM]);  // f . f
+    }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    double fv = 0.0, ff = 0.0, vv = 0.0, len = 0.0;
+    for (int p = 1; p <= P - 2; ++p) {
+        const int slot = d.order[p];
+        fv += d.coef[slot * 4 + 2];
+        ff += d.coef[slot * 4 + 3];
+        vv += d.dots[slot * kNDots + DOT_VV];
+        len += sqrt(d.dots[slot * kNDots + DOT_PP]);
+        if (p == 1) len += sqrt(d.dots[slot * kNDots + DOT_MM]);
+    }
+    if (ff < 0.0) ff = 0.0;  // round-off of the one-pass algebra near convergence
+    if (!isfinite(fv) || !isfinite(ff) || !isfinite(vv)) set_error(ctl, CFNEB_ENAN);
+    ctl->pstar = pstar;
+    ctl->path_length = len;
+    {
+        int pb = pstar;
+        if (pb < 0) {
+            double best = 0.0;
+            for (int p = 1; p <= P - 2; ++p) {
+                const double e = d.E[d.order[p]];
+                if (pb < 0 || e > best) { best = e; pb = p; }
+            }
+        }
+        ctl->barrier = (pb > 0) ? d.E[d.order[pb]] - d.E[d.order[0]] : 0.0;
+    }
+    if (dry) return;
+    ctl->fmax_bits = 0ull;  // K6 of this step takes the max row norm of f (O8)
+    // ---- FIRE (O7) ----
+    double dt = ctl->dt, alpha = ctl->alpha, cv, cf;
+    int n_pos = ctl->n_pos;
+    if (ctl->first) {  // A2: no power test on the first step after a (re)start; v = 0
+        ctl->first = 0;
+        cv = 0.0;
+        cf = dt;
+        vv = 0.0;
+        fv = 0.0;
+    } else if (fv > 0.0) {
+        const double mix = (ff > 0.0) ? alpha * sqrt(vv / ff) : 0.0;  // alpha |v| / |f|
+        cv = 1.0 - alpha;
+        if (n_pos > d.fire_nmin) {
+            dt = fmin(dt * d.finc, d.dtmax);
+            alpha *= d.fa;
+        }
+        n_pos += 1;
+        cf = mix + dt;
+    } else {
+        cv = 0.0;
+        alpha = d.astart;
+        dt *= d.fdec;
+        n_pos = 0;
+        cf = dt;
+    }
+    // |v_new|^2 with v_new = cv v + cf f;  Delta = dt v_new, limited to maxstep sqrt(movable rows) (A4)
+    double vn2 = cv * cv * vv + 2.0 * cv * cf * fv + cf * cf * ff;
+    if (vn2 < 0.0) vn2 = 0.0;
+    const double nd = dt * sqrt(vn2);
+    const double limit = d.maxstep * sqrt((double)(P - 2) * (double)(d.N + 3));
+    double s = 1.0;
+    if (nd > limit) s = limit / nd;
+    ctl->dt = dt;
+    ctl->alpha = alpha;
+    ctl->n_pos = n_pos;
+    ctl->cv = cv;
+    ctl->cf = cf;
+    ctl->sdt = s * dt;
+    ctl->src = ctl->cur;
+    ctl->dst = 1 - ctl->cur;
+    ctl->cur = 1 - ctl->cur;
+    ctl->steps += 1ull;
+}
+
+void launch_reduce(const Dev &d, cudaStream_t st) {
+    if (d.S < 3) return;
+    dim3 grid(d.nblk_stream, d.S - 2);
+    reduce_kernel<<<grid, kThreadsStream, 0, st>>>(d);
+}
+
+void launch_finalize(const Dev &d, int p_lo, cudaStream_t st) {
+    const int nimg = d.S - 2 * p_lo;
+    if (nimg <= 0) return;
+    finalize_kernel<<<nimg, 256, 0, st>>>(d, p_lo);
+}
+
+void launch_scalar(const Dev &d, int dry, cudaStream_t st) { scalar_kernel<<<1, 128, 0, st>>>(d, dry); }
+
+}  // namespace cfn

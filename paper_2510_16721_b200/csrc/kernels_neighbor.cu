@@ -1,0 +1,215 @@
+// kernels_neighbor.cu -- K1: per-image cell-list neighbour build under PBC ("neighbors in i's local
+// environment under PBC"; O2).  Entry (i; j, n) iff |(s_j - s_i + n) h| < r_list strictly and
+// (j, n) != (i, 0), with s = R~ h0^-1 the unwrapped fractional coordinates (Eq. 10), so that the periodic
+// shift n is defined relative to the stored coordinates and r^ij = R_j - R_i + n h.
+//
+// Bins live in wrapped fractional space: axis a has nb_a = floor(w_a / r_list) bins (w_a = perpendicular
+// width) and a +-1 stencil when nb_a >= 3, otherwise one bin and explicit shifts m_a in [-reach, reach]
+// (boxes smaller than 2 r_list: an atom then sees several periodic images of the same neighbour, itself
+// included).  Every kernel exits at once for images whose list is still valid (Geom::rebuild == 0).
+//
+// Determinism: bins are filled with atomics, then each bin is sorted by atom index, so list order (and with
+// it the summation order of the force kernel) is a function of the coordinates only.
+#include "cfneb_internal.cuh"
+
+namespace cfn {
+
+__device__ inline bool image_active(const Dev &d, int p_lo, int y, int &slot) {
+    const int p = y + p_lo;
+    if (p > d.ctl->P - 1 - p_lo) return false;
+    slot = d.order[p];
+    return d.geom[slot].rebuild != 0;
+}
+
+// Exclusive scan of the bin populations of one image (one block per image); also primes the fill cursors.
+__global__ void __launch_bounds__(1024) bin_scan_kernel(Dev d, int p_lo) {
+    int slot;
+    if (!image_active(d, p_lo, blockIdx.x, slot)) return;
+    const Geom *g = d.geom + slot;
+    const int nbins = g->nb[0] * g->nb[1] * g->nb[2];
+    int *bc = d.bin_count + (size_t)slot * (d.nbins_max + 1);
+    int *cur = d.bin_cursor + (size_t)slot * d.nbins_max;
+    const int T = blockDim.x, tid = threadIdx.x;
+    const int per = (nbins + T) / T;  // covers nbins + 1 entries
+    const int lo = min(tid * per, nbins + 1), hi = min(lo + per, nbins + 1);
+    int sum = 0;
+    for (int b = lo; b < hi; ++b) sum += bc[b];
+    __shared__ int s[1024];
+    s[tid] = sum;
+    __syncthreads();
+    for (int off = 1; off < T; off <<= 1) {
+        int t = (tid >= off) ? s[tid - off] : 0;
+        __syncthreads();
+        s[tid] += t;
+        __syncthreads();
+    }
+    int base = s[tid] - sum;
+    for (int b = lo; b < hi; ++b) {
+        int c = bc[b];
+        bc[b] = base;
+        if (b < nbins) cur[b] = base;
+        base += c;
+    }
+}
+
+__global__ void __launch_bounds__(kThreadsAtom) bin_fill_kernel(Dev d, int p_lo) {
+    int slot;
+    if (!image_active(d, p_lo, blockIdx.y, slot)) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.N) return;
+    const int bin = d.atom_bin[(size_t)slot * d.Npad + i];
+    const int pos = atomicAdd(d.bin_cursor + (size_t)slot * d.nbins_max + bin, 1);
+    d.bin_members[(size_t)slot * d.Npad + pos] = i;
+}
+
+// One thread per bin: sort the members by atom index, then write the bin-ordered coordinate array.
+__global__ void __launch_bounds__(128) bin_sort_kernel(Dev d, int p_lo) {
+    int slot;
+    if (!image_active(d, p_lo, blockIdx.y, slot)) return;
+    const Geom *g = d.geom + slot;
+    const int nbins = g->nb[0] * g->nb[1] * g->nb[2];
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= nbins) return;
+    const int *bc = d.bin_count + (size_t)slot * (d.nbins_max + 1);
+    int *mem = d.bin_members + (size_t)slot * d.Npad;
+    const int lo = bc[b], hi = bc[b + 1];
+    for (int q = lo + 1; q < hi; ++q) {  // insertion sort (bins hold a few tens of atoms)
+        int x = mem[q], r = q - 1;
+        while (r >= lo && mem[r] > x) { mem[r + 1] = mem[r]; --r; }
+        mem[r + 1] = x;
+    }
+    const double4 *Sw = d.Sw + (size_t)slot * d.Npad;
+    double4 *out = d.binned + (size_t)slot * d.Npad;
+    for (int q = lo; q < hi; ++q) {
+        const int i = mem[q];
+        double4 w = Sw[i];
+        unsigned long long fl = (unsigned long long)__double_as_longlong(w.w);
+        w.w = __longlong_as_double((long long)((unsigned long long)i | (fl << kShiftBits)));
+        out[q] = w;
+    }
+}
+
+__device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
+    if (nb >= 3) {
+        int t = bi + dlt;
+        m = (t < 0) ? -1 : (t >= nb ? 1 : 0);
+        bj = t - m * nb;
+    } else {
+        bj = 0;
+        m = dlt;
+    }
+}
+
+// One thread per atom: scan the stencil bins, test |ds h|^2 < r_list^2, append (j | code << 23) k-major.
+__global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, int p_lo) {
+    int slot;
+    if (!image_active(d, p_lo, blockIdx.y, slot)) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = i < d.N;
+    int cnt = 0;
+    bool bad_shift = false;
+    if (valid) {
+    const Geom *g = d.geom + slot;
+    const int nb0 = g->nb[0], nb1 = g->nb[1], nb2 = g->nb[2];
+    const int re0 = g->reach[0], re1 = g->reach[1], re2 = g->reach[2];
+    double h[9];
+#pragma unroll
+    for (int k = 0; k < 9; ++k) h[k] = g->h[k];
+    const double4 si = d.Sw[(size_t)slot * d.Npad + i];
+    const unsigned long long fli = (unsigned long long)__double_as_longlong(si.w);
+    const int fi0 = (int)(fli & 1023u), fi1 = (int)((fli >> 10) & 1023u), fi2 = (int)((fli >> 20) & 1023u);
+    const int bin = d.atom_bin[(size_t)slot * d.Npad + i];
+    const int bi0 = bin / (nb1 * nb2), bi1 = (bin / nb2) % nb1, bi2 = bin % nb2;
+    const int *bc = d.bin_count + (size_t)slot * (d.nbins_max + 1);
+    const double4 *binned = d.binned + (size_t)slot * d.Npad;
+    uint32_t *list = d.nbr_list + (size_t)slot * d.cap * d.Npad + i;
+    const double rl2 = d.r_list * d.r_list;
+    for (int d0 = -re0; d0 <= re0; ++d0) {
+        int bj0, m0;
+        stencil_axis(nb0, bi0, d0, bj0, m0);
+        for (int d1 = -re1; d1 <= re1; ++d1) {
+            int bj1, m1;
+            stencil_axis(nb1, bi1, d1, bj1, m1);
+            for (int d2 = -re2; d2 <= re2; ++d2) {
+                int bj2, m2;
+                stencil_axis(nb2, bi2, d2, bj2, m2);
+                const int b = (bj0 * nb1 + bj1) * nb2 + bj2;
+                const int lo = bc[b], hi = bc[b + 1];
+                for (int q = lo; q < hi; ++q) {
+                    const double4 c = binned[q];
+                    const double s0 = c.x - si.x + (double)m0, s1 = c.y - si.y + (double)m1, s2 = c.z - si.z + (double)m2;
+                    const double rx = s0 * h[0] + s1 * h[3] + s2 * h[6];
+                    const double ry = s0 * h[1] + s1 * h[4] + s2 * h[7];
+                    const double rz = s0 * h[2] + s1 * h[5] + s2 * h[8];
+                    const double r2 = rx * rx + ry * ry + rz * rz;
+                    if (r2 < rl2) {
+                        const unsigned long long pk = (unsigned long long)__double_as_longlong(c.w);
+                        const int j = (int)(pk & kIdxMask);
+                        const int n0 = m0 - (int)((pk >> kShiftBits) & 1023u) + fi0;
+                        const int n1 = m1 - (int)((pk >> (kShiftBits + 10)) & 1023u) + fi1;
+                        const int n2 = m2 - (int)((pk >> (kShiftBits + 20)) & 1023u) + fi2;
+                        if (j == i && n0 == 0 && n1 == 0 && n2 == 0) continue;
+                        if (cnt < d.cap) {
+                            if (n0 < -4 || n0 > 3 || n1 < -4 || n1 > 3 || n2 < -4 || n2 > 3) bad_shift = true;
+                            const uint32_t code = (uint32_t)((n0 + 4) & 7) | ((uint32_t)((n1 + 4) & 7) << 3) |
+                                                  ((uint32_t)((n2 + 4) & 7) << 6);
+                            list[(size_t)cnt * d.Npad] = (uint32_t)j | (code << kShiftBits);
+                        }
+                        ++cnt;
+                    }
+                }
+            }
+        }
+    }
+    d.nbr_count[(size_t)slot * d.Npad + i] = min(cnt, d.cap);
+    }  // valid
+    if (cnt > d.cap) set_error(d.ctl, CFNEB_ENEIGH_OVERFLOW);
+    if (bad_shift) set_error(d.ctl, CFNEB_ECELL);
+    // block-level max, then one atomic per block
+    __shared__ int s_max;
+    if (threadIdx.x == 0) s_max = 0;
+    __syncthreads();
+    atomicMax(&s_max, cnt);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_max > d.ctl->max_nbr_seen) atomicMax(&d.ctl->max_nbr_seen, s_max);
+}
+
+// Parity hook: list of one slot in the external layout count[N], list[N][cap] (-1 padded), shift[N][cap][3].
+__global__ void unpack_neighbors_kernel(Dev d, int slot, int *count_out, int *list_out, int *shift_out) {
+    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (e >= (size_t)d.N * d.cap) return;
+    const int i = (int)(e / d.cap), k = (int)(e % d.cap);
+    const int c = d.nbr_count[(size_t)slot * d.Npad + i];
+    if (k == 0) count_out[i] = c;
+    int j = -1, n0 = 0, n1 = 0, n2 = 0;
+    if (k < c) {
+        const uint32_t w = d.nbr_list[((size_t)slot * d.cap + k) * d.Npad + i];
+        j = (int)(w & kIdxMask);
+        const uint32_t code = w >> kShiftBits;
+        n0 = (int)(code & 7u) - 4;
+        n1 = (int)((code >> 3) & 7u) - 4;
+        n2 = (int)((code >> 6) & 7u) - 4;
+    }
+    list_out[e] = j;
+    shift_out[3 * e] = n0;
+    shift_out[3 * e + 1] = n1;
+    shift_out[3 * e + 2] = n2;
+}
+
+void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st) {
+    const int nimg = d.S - 2 * p_lo;
+    if (nimg <= 0) return;
+    bin_scan_kernel<<<nimg, 1024, 0, st>>>(d, p_lo);
+    dim3 ga(d.nblk_atom, nimg);
+    bin_fill_kernel<<<ga, kThreadsAtom, 0, st>>>(d, p_lo);
+    dim3 gb((d.nbins_max + 127) / 128, nimg);
+    bin_sort_kernel<<<gb, 128, 0, st>>>(d, p_lo);
+    neighbor_search_kernel<<<ga, kThreadsAtom, 0, st>>>(d, p_lo);
+}
+
+void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_out, int *shift_out, cudaStream_t st) {
+    const size_t n = (size_t)d.N * d.cap;
+    unpack_neighbors_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d, slot, count_out, list_out, shift_out);
+}
+
+}  // namespace cfn

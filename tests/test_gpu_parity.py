@@ -1,0 +1,373 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle on the same
+seeded inputs.  Tolerances are BASELINE.json north_star's: neighbour lists bit-exact after sorting; per-atom
+forces, energies and virials to relative 1e-10; one full NEB step to relative 1e-9; converged barrier to 1e-4.
+
+"relative" for an array means max|a - b| <= tol * max|b| (the array's own scale): forces and virials of a
+near-equilibrium crystal are sums of cancelling pair terms, so an element-wise relative error is undefined at
+the zeros; DESIGN.md "Tolerances" derives this form.
+"""
+import numpy as np
+import pytest
+
+from cfneb_workloads import CONFIGS, build_workload
+
+pytestmark = pytest.mark.gpu
+
+TOL_FORCE = 1e-10
+TOL_STEP = 1e-9
+
+
+def rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    s = np.max(np.abs(b))
+    return float(np.max(np.abs(a - b)) / (s if s > 0 else 1.0))
+
+
+def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_images=None, **over):
+    """(oracle band, GPU band) on configs[k] inputs."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(k, n_images)
+    climb = spec.climb if climb is None else climb
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=climb,
+                   cell_mode=cell_mode, cell_factor=cell_factor, fire=spec.fire, skin=spec.skin,
+                   max_neighbors=spec.max_neighbors)
+    prm = cf.params_for(spec, cell_factor=cell_factor, cell_mode=cell_mode, climb=int(climb), max_images=max_images, **over)
+    gpu = cf.CFNEB(pos, cells, prm)
+    return spec, orc, gpu
+
+
+def sorted_triples(count, lst, shift):
+    out = []
+    for i in range(len(count)):
+        c = int(count[i])
+        t = np.concatenate([np.full((c, 1), i), lst[i, :c, None], shift[i, :c]], axis=1)
+        out.append(t)
+    t = np.concatenate(out, axis=0)
+    return t[np.lexsort(t.T[::-1])]
+
+
+# ---------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("k", [0, 1, 2])
+def test_neighbor_lists_bit_exact_after_sorting(k):
+    from oracle import forcefield as ff
+    spec, orc, gpu = make_pair(k)
+    ev = orc.evaluator
+    r_list = spec.r_cut + spec.skin
+    for image in sorted({0, 1, orc.P // 2, orc.P - 1}):
+        Rt, D = ev.deformation(orc.band.X[image])
+        h = orc.h0 @ D
+        cnt, lst, sh = ff.neighbors(Rt, orc.h0, h, r_list, spec.max_neighbors, brute=(k == 0))
+        # guard: no pair within 1e-9 of the list radius (membership would be rounding-dependent, A20/A24)
+        gc, gl, gs = gpu.get_neighbors(image)
+        assert np.array_equal(np.sort(gc), np.sort(cnt)) and np.array_equal(gc, cnt)
+        a, b = sorted_triples(gc, gl, gs), sorted_triples(cnt, lst, sh)
+        assert a.shape == b.shape and np.array_equal(a, b)
+        # symmetry (i; j, n) <=> (j; i, -n)
+        fl = a.copy()
+        fl[:, [0, 1]] = fl[:, [1, 0]]
+        fl[:, 2:] *= -1
+        assert np.array_equal(fl[np.lexsort(fl.T[::-1])], a)
+    gpu.close()
+
+
+@pytest.mark.parametrize("k,lam", [(0, 1.0), (0, 0.0), (1, 1.0), (2, 1.0), (2, 0.0)])
+def test_forces_energies_virials_and_neb_force(k, lam):
+    spec, orc, gpu = make_pair(k, cell_factor=lam)
+    f_or = orc.band.forces()
+    last = orc.evaluator.last
+    F, V, fneb, E = gpu.get_forces()
+    P = orc.P
+    assert rel(E, orc.band.E) < TOL_FORCE
+    assert rel(E[1:-1] - E[0], orc.band.E[1:-1] - orc.band.E[0]) < 1e-8  # energy differences along the band
+    assert rel(F[1:-1], last["F"]) < TOL_FORCE
+    assert rel(V[1:-1], last["V"]) < TOL_FORCE
+    for p in range(1, P - 1):
+        assert rel(F[p], last["F"][p - 1]) < TOL_FORCE
+        assert rel(fneb[p], f_or[p]) < TOL_STEP
+    assert np.all(fneb[0] == 0) and np.all(fneb[-1] == 0)
+    st = gpu.get_status()
+    assert st.climb_index == orc.band.pstar
+    assert abs(st.barrier - orc.band.barrier) < 1e-9 * max(1.0, abs(orc.band.E[0]))
+    if lam == 0.0:
+        from oracle.cfneb import auto_cell_factor
+        assert abs(st.cell_factor - auto_cell_factor(orc.h0, orc.N)) < 1e-12 * st.cell_factor
+    gpu.close()
+
+
+@pytest.mark.parametrize("k,lam,nsteps", [(0, 1.0, 30), (0, 0.0, 30), (1, 0.0, 20), (2, 0.0, 12), (2, 1.0, 6)])
+def test_neb_steps_match_oracle(k, lam, nsteps):
+    """X and v after 1, 2, ... n full iterations (K0-K6) against the oracle's step()."""
+    spec, orc, gpu = make_pair(k, cell_factor=lam)
+    X0, _ = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg, X0) < 1e-14 and np.all(vg == 0)
+    checks = sorted({1, 2, 3, nsteps // 2, nsteps})
+    done = 0
+    for n in checks:
+        orc.step(n - done)
+        gpu.step(n - done)
+        done = n
+        Xo, vo = orc.get_state()
+        Xg, vg = gpu.get_state()
+        dX = rel(Xg - X0, Xo - X0)  # the displacement, not the (much larger) coordinate, carries the step
+        dv = rel(vg, vo)
+        growth = 4.0 ** (n - 1) if n < 6 else 1e3  # round-off is amplified by later steps, not by the first
+        assert dX < TOL_STEP * min(growth, 1e3), (n, dX)
+        assert dv < TOL_STEP * min(growth, 1e3), (n, dv)
+        st = gpu.get_status()
+        assert st.steps == n and st.error == 0
+        assert abs(st.fmax - orc.band.fmax) <= 1e-8 * orc.band.fmax
+        assert abs(st.dt - orc.band.fire.dt) < 1e-15 and abs(st.alpha - orc.band.fire.alpha) < 1e-15
+        assert st.n_pos == orc.band.fire.n_pos
+    gpu.close()
+
+
+def test_first_step_is_exact_to_1e9():
+    """The north-star number: ONE full NEB step to 1e-9 relative, every config the oracle finishes in seconds."""
+    for k in (0, 1, 2):
+        spec, orc, gpu = make_pair(k, cell_factor=0.0)
+        X0, _ = orc.get_state()
+        orc.step(1)
+        gpu.step(1)
+        Xo, vo = orc.get_state()
+        Xg, vg = gpu.get_state()
+        assert rel(Xg - X0, Xo - X0) < TOL_STEP and rel(vg, vo) < TOL_STEP
+        assert rel(Xg, Xo) < 1e-13
+        gpu.close()
+
+
+def test_c0_converged_barrier_matches_oracle():
+    spec, orc, gpu = make_pair(0, cell_factor=0.0)
+    orc.run(1e-4, 3000)
+    for _ in range(60):
+        gpu.step(50)
+        if gpu.get_status().fmax < 1e-4:
+            break
+    st = gpu.get_status()
+    assert st.fmax < 1e-4 and st.error == 0
+    assert st.climb_index == orc.band.pstar == 3
+    assert abs(st.barrier - orc.band.barrier) < 1e-4
+    assert 4.9 < st.barrier < 5.1
+    pos, cells, E = gpu.get_path()
+    assert abs(E[0] - E[-1]) < 1e-9  # symmetric hop
+    gpu.close()
+
+
+def test_c1_barrier_after_fixed_budget():
+    spec, orc, gpu = make_pair(1, cell_factor=0.0)
+    orc.run(1e-3, 1500)
+    n = orc.band.nsteps
+    gpu.step(n)
+    st = gpu.get_status()
+    assert st.steps == n
+    assert abs(st.barrier - orc.band.barrier) < 1e-4
+    assert st.fmax < 2e-3
+    gpu.close()
+
+
+@pytest.mark.parametrize("mode", [0, 2])
+def test_cell_modes_fixed_and_D(mode):
+    """CELL_FIXED (no cell force) and the Eq. 14 D-variant follow the oracle too."""
+    spec, orc, gpu = make_pair(0, cell_factor=1.0, cell_mode=mode)
+    X0, _ = orc.get_state()
+    orc.step(5)
+    gpu.step(5)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
+    if mode == 0:
+        assert np.array_equal(Xg[:, -3:], X0[:, -3:])
+    gpu.close()
+
+
+def test_no_climbing_image():
+    spec, orc, gpu = make_pair(1, cell_factor=0.0, climb=False)
+    X0, _ = orc.get_state()
+    orc.step(3)
+    gpu.step(3)
+    Xo, _ = orc.get_state()
+    Xg, _ = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < 1e-8
+    assert gpu.get_status().climb_index == -1
+    gpu.close()
+
+
+def test_insert_delete_and_adapt_follow_oracle():
+    spec, orc, gpu = make_pair(1, cell_factor=0.0, max_images=14)
+    orc.max_images = 14
+    orc.step(4)
+    gpu.step(4)
+    orc.insert_image(2)
+    gpu.insert_image(2)
+    assert gpu.P == orc.P == 10
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg, Xo) < 1e-12 and np.all(vg == 0)
+    assert np.array_equal(Xg[3], 0.5 * (Xg[2] + Xg[4]))  # midpoint exact
+    orc.step(3)
+    gpu.step(3)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg, Xo) < 1e-11 and rel(vg, vo) < 1e-7
+    assert np.isfinite(gpu.get_path(positions=False)[2]).all()
+    q = 7 if gpu.get_status().climb_index != 7 else 6
+    orc.delete_image(q)
+    gpu.delete_image(q)
+    assert gpu.P == orc.P == 9
+    orc.step(2)
+    gpu.step(2)
+    assert rel(gpu.get_state()[0], orc.get_state()[0]) < 1e-11
+    d = gpu.get_segment_lengths()
+    assert rel(d, orc.band.segment_lengths()) < 1e-10
+    # adaptive control: thresholds that force one insertion, then one deletion
+    di, dd = 0.9 * d.max(), 0.0
+    assert gpu.adapt(di, dd) == orc.adapt(di, dd) == (1, 0)
+    assert gpu.P == orc.P == 10
+    d = gpu.get_segment_lengths()
+    di, dd = 10 * d.max(), 1.01 * np.min(d[:-1] + d[1:]) + 1.0
+    ro, rg = orc.adapt(di, dd), gpu.adapt(di, dd)
+    assert ro == rg and rg[1] == 1
+    assert rel(gpu.get_state()[0], orc.get_state()[0]) < 1e-11
+    orc.step(2)
+    gpu.step(2)
+    assert rel(gpu.get_state()[0], orc.get_state()[0]) < 1e-10
+    gpu.close()
+
+
+def test_image_control_errors():
+    import paper_2510_16721_b200 as cf
+    spec, orc, gpu = make_pair(0)
+    for bad in (-1, 6, 99):
+        with pytest.raises(cf.CfnebError) as e:
+            gpu.insert_image(bad)
+        assert e.value.code == cf.binding.ERANGE
+    with pytest.raises(cf.CfnebError):  # band full (max_images = 7)
+        gpu.insert_image(1)
+    for bad in (0, 6, 7):
+        with pytest.raises(cf.CfnebError):
+            gpu.delete_image(bad)
+    gpu.step(1)
+    with pytest.raises(cf.CfnebError):  # the climbing image may not be deleted
+        gpu.delete_image(gpu.get_status().climb_index)
+    gpu.close()
+
+
+def test_create_errors_and_sticky_device_errors():
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(0)
+    with pytest.raises(cf.CfnebError) as e:  # neighbour capacity too small: sticky device error surfaces in create
+        cf.CFNEB(pos, cells, cf.params_for(spec, max_neighbors=16))
+    assert e.value.code == cf.binding.ENEIGH_OVERFLOW
+    with pytest.raises(cf.CfnebError) as e:
+        cf.CFNEB(pos[:2], cells[:2], cf.params_for(spec), n_images=2)
+    assert e.value.code == cf.binding.EINVAL
+    bad = cells.copy()
+    bad[3] = 0.0
+    with pytest.raises(cf.CfnebError) as e:
+        cf.CFNEB(pos, bad, cf.params_for(spec))
+    assert e.value.code == cf.binding.ECELL
+    with pytest.raises(cf.CfnebError) as e:  # more images than capacity
+        cf.CFNEB(pos, cells, cf.params_for(spec, max_images=5))
+    assert e.value.code == cf.binding.ERANGE
+    with pytest.raises(cf.CfnebError):  # identical interior images: zero tangent
+        p2 = pos.copy()
+        p2[:] = pos[0]
+        c2 = cells.copy()
+        c2[:] = cells[0]
+        g = cf.CFNEB(p2, c2, cf.params_for(spec))
+        g.step(1)
+        g.get_state()
+
+
+def test_endpoints_only_constructor_and_get_path_roundtrip():
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(1)
+    gpu = cf.CFNEB(pos[[0, -1]], cells[[0, -1]], cf.params_for(spec), n_images=9)
+    p, c, E = gpu.get_path()
+    assert p.shape == pos.shape and rel(p[0], pos[0]) < 1e-15 and rel(p[-1], pos[-1]) < 1e-14
+    assert rel(c[0], cells[0]) < 1e-15 and rel(c[-1], cells[-1]) < 1e-14
+    X, _ = gpu.get_state()
+    for q in range(9):  # linear in the generalized coordinates
+        assert rel(X[q], X[0] + q / 8.0 * (X[-1] - X[0])) < 1e-14
+    # explicit-path constructor: get_path returns what went in (cells rotation-free: inputs here are symmetric D)
+    g2 = cf.CFNEB(pos, cells, cf.params_for(spec))
+    p2, c2, E2 = g2.get_path()
+    assert rel(p2, pos) < 1e-14 and rel(c2, cells) < 1e-14
+    # set_path round trip restarts from the same state
+    X_before, _ = g2.get_state()
+    E_before = g2.get_path(positions=False)[2]
+    g2.step(3)
+    assert not np.array_equal(g2.get_state()[0], X_before)
+    g2.set_path(pos, cells)
+    assert np.array_equal(g2.get_state()[0], X_before) and np.all(g2.get_state()[1] == 0)
+    assert np.array_equal(g2.get_path(positions=False)[2], E_before)
+    st = g2.get_status()
+    assert st.dt == spec.fire["dt0"] and st.n_pos == 0
+    gpu.close()
+    g2.close()
+
+
+def test_rotated_final_endpoint_gives_the_same_band():
+    """P:110 / P:124: B = D D^T removes rigid rotations -- a final endpoint supplied rotated by Q changes nothing."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(0)
+    th = 0.3
+    Q = np.array([[np.cos(th), -np.sin(th), 0], [np.sin(th), np.cos(th), 0], [0, 0, 1.0]])
+    pos_r, cells_r = pos.copy(), cells.copy()
+    pos_r[-1] = pos[-1] @ Q
+    cells_r[-1] = cells[-1] @ Q
+    a = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    b = cf.CFNEB(pos_r, cells_r, cf.params_for(spec, cell_factor=0.0))
+    a.step(25)
+    b.step(25)
+    Xa, _ = a.get_state()
+    Xb, _ = b.get_state()
+    assert rel(Xb, Xa) < 1e-10
+    assert abs(a.get_status().barrier - b.get_status().barrier) < 1e-9
+    pa, ca, _ = a.get_path()
+    pb, cb, _ = b.get_path()
+    assert rel(cb, ca) < 1e-10  # returned un-rotated (documented in include/cfneb.h)
+    a.close()
+    b.close()
+
+
+def test_bitwise_repeatable():
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(2)
+    out = []
+    for _ in range(2):
+        g = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+        g.step(8)
+        out.append(g.get_state())
+        g.close()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
+
+
+def test_neighbor_list_reuse_equals_fresh_lists():
+    """Verlet-list reuse (skin) must not change the result: rebuild_every = 1 forces fresh lists each step."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(2)
+    a = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    b = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, rebuild_every=1))
+    a.step(40)
+    b.step(40)
+    sa, sb = a.get_status(), b.get_status()
+    assert sb.rebuilds > sa.rebuilds
+    # list order differs between the two (summation order), so equality is to round-off, not bitwise
+    assert rel(a.get_state()[0], b.get_state()[0]) < 1e-11
+    a.close()
+    b.close()
+
+
+def test_step_timed_matches_graph_step():
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(1)
+    a = cf.CFNEB(pos, cells, cf.params_for(spec))
+    b = cf.CFNEB(pos, cells, cf.params_for(spec))
+    a.step(5)
+    ms = b.step_timed(5)
+    assert ms.shape == (6,) and np.all(ms >= 0) and ms[2] > 0
+    assert np.array_equal(a.get_state()[0], b.get_state()[0])
+    a.close()
+    b.close()
