@@ -1,0 +1,380 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CFNEB hot path (BASELINE.json `metric`) on B200, one JSON line on stdout.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (K0-K6 of DESIGN.md: cell map, neighbour-list upkeep, batched
+force / energy / virial, one-pass reductions, tangent + climbing image + FIRE scalars, fused update) over all
+images of the band.  metric = atom x image x NEB-steps per second, counted over the MOVABLE images
+(N (P-2) per step, reading A23); the N P figure is printed alongside in `config`.
+
+  value      K graph-launched steps (cfneb_step), state resident in HBM, CUDA events on the library's stream,
+             barrier + synchronize on both sides, max over ranks.
+  roofline   the projection + FIRE kernels (K4 reduce + K6 update) the metric names: algorithmic bytes
+             (192 B per atom-image-step) / their CUDA-event time per step, measured live by
+             cfneb_step_timed over K further steps of the same band; against MEASURED_PEAKS.json hbm_gbs.
+             `kernels` carries every class's time share and the force kernel's fp64 "alu" fraction.
+  e2e        the same metric through the C ABI with HOST (pinned) buffers: every step uploads the whole path
+             (cfneb_set_path), runs one iteration (cfneb_step) and reads the path back (cfneb_get_path).
+  cpu_baseline  the oracle as it stands, on this box's host cores, on a bounded sample of the same workload.
+
+N > 1: the path does not shard (BASELINE.json: one GPU, no collectives) -- "replicas only": every rank runs the
+same band on its own GPU; value = all ranks' units / max-over-ranks time.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "atom_image_neb_steps_per_s"
+UNIT = "atom*image*steps/s"
+ALGO_BYTES_PER_UNIT = 192.0  # K4 reads X, F, v (72 B); K6 reads X, F, v (72 B), writes X_new, v (48 B)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", type=int, default=4, help="index into BASELINE.json configs (default 4: 101306 x 100)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=5)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+# ------------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index = index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        self.thread = threading.Thread(target=self._read, daemon=True)
+        self.thread.start()
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.2] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                smax.append(float(f[1]))
+                power.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def measured_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def ncu_traffic(workload, kernel):
+    """dram bytes per launch of `kernel` from the committed ncu --set full capture, if one exists."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    if not os.path.exists(path):
+        return None
+    with open(path) as fh:
+        d = json.load(fh)
+    return d.get(workload, {}).get(kernel)
+
+
+# ------------------------------------------------------------------------------------------------------------
+def host_cores():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+ORACLE_RATE = 1.5e4  # atom-images per second per thread, order of magnitude only (sizes the bounded sample)
+
+
+def oracle_sample_plan(k, total_steps, budget_s):
+    """Choose a bounded sample of configs[k] for the oracle: (n_images, dims or None, threads, description)."""
+    from cfneb_workloads import CONFIGS
+    spec = CONFIGS[k]
+    cores = host_cores()
+    movable = spec.n_images - 2
+    threads = max(1, min(cores, movable, 16))
+    if spec.lattice != "bcc_bain":
+        return spec.n_images, None, threads, "full config (%d atoms x %d images)" % (spec.n_atoms, spec.n_images)
+    m = threads  # one image per thread: the only parallelism the oracle has is over images
+    per_step = budget_s / max(total_steps + 2.0, 1.0)  # + 2: the two endpoint evaluations at construction
+    atoms = int(min(spec.n_atoms, max(432, per_step * ORACLE_RATE)))
+    if atoms >= 0.5 * spec.n_atoms:
+        return m + 2, None, threads, "%d consecutive movable images (mid-path) of the %d, all %d atoms" % (m, movable, spec.n_atoms)
+    n = max(6, int(round((atoms / 2.0) ** (1.0 / 3.0))))
+    return (m + 2, (n, n, n), threads,
+            "%d movable images of a %dx%dx%d bcc cell (%d atoms) built by the same recipe as the %d-atom config"
+            % (m, n, n, n, 2 * n ** 3, spec.n_atoms))
+
+
+def run_oracle(k, steps, warmup, budget_s):
+    """Time `steps` oracle iterations (after `warmup`) on a bounded sample.  Returns a dict."""
+    from cfneb_workloads import build_workload
+    from oracle import cfneb as oc
+    n_images, dims, threads, what = oracle_sample_plan(k, steps + warmup, budget_s)
+    spec, pos, cells = build_workload(k, dims=dims)
+    P = pos.shape[0]
+    if n_images < P:  # consecutive images around the middle of the path, between the two true endpoints
+        lo = max(1, (P - (n_images - 2)) // 2)
+        idx = [0] + list(range(lo, lo + n_images - 2)) + [P - 1]
+        pos, cells = pos[idx], cells[idx]
+    band = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb,
+                    cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors, threads=threads)
+    for _ in range(warmup):
+        band.step(1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        band.step(1)
+    dt = time.perf_counter() - t0
+    units = pos.shape[1] * (pos.shape[0] - 2) * steps
+    return {"value": units / dt, "unit": UNIT, "cores": threads, "kind": "oracle", "host_cores": host_cores(),
+            "sample": "%s; %d timed step(s) after %d warm-up" % (what, steps, warmup), "seconds": dt,
+            "ms_per_step": 1e3 * dt / max(steps, 1), "n_atoms": int(pos.shape[1]), "n_images": int(pos.shape[0])}
+
+
+def build_cfg(k):
+    from cfneb_workloads import CONFIGS
+    return CONFIGS[k]
+
+
+def workload_name(k):
+    spec = build_cfg(k)
+    return "configs[%d] %s: %d atoms x %d images, fp64" % (k, spec.name, spec.n_atoms, spec.n_images)
+
+
+def main_reference(args):
+    """--impl reference: the oracle as it stands on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    r = run_oracle(args.config, args.steps, args.warmup, budget_s=150.0)
+    spec = build_cfg(args.config)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(args.config), "potential": "finnis_sinclair_morse" if spec.potential else "lj_shifted_force",
+                   "sample": r["sample"], "runs_on": "host CPU (oracle/, plain fp64 C + numpy)"},
+        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------------
+def main_ours(args):
+    import torch
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import build_workload
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the CFNEB path has no CPU fallback")
+    cf.lib()  # fail loudly if libcfneb.so is missing
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    k = args.config
+    spec, pos, cells = build_workload(k)
+    P, N = pos.shape[0], pos.shape[1]
+    prm = cf.params_for(spec, cell_factor=0.0)
+    band = cf.CFNEB(pos, cells, prm, device="cuda:%d" % local)
+    stream = band.stream
+    units_per_step = N * (P - 2)
+
+    # ---- device-resident throughput: W warm-up + K timed graph-launched steps ----
+    band.step(args.warmup)
+    band.synchronize()
+    st0 = band.get_status()
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    t_wall0 = time.time()
+    e0.record(stream)
+    band.step(args.steps)
+    e1.record(stream)
+    stream.synchronize()
+    barrier()
+    t_wall1 = time.time()
+    ms_total = max_over_ranks(e0.elapsed_time(e1))
+    st1 = band.get_status()
+    if st1.error != 0:
+        raise RuntimeError("device error %d during the timed region" % st1.error)
+    ms_per_step = ms_total / args.steps
+    value = world * units_per_step * args.steps / (ms_total * 1e-3)
+
+    # ---- per-kernel-class CUDA-event times over K further steps of the same band (roofline) ----
+    kms = band.step_timed(args.steps) / args.steps  # ms per step per class
+    clocks = sampler.stop(t_wall0, time.time())
+    peak, peak_src = measured_peaks()
+    t_proj = (kms[cf.binding.K_REDUCE] + kms[cf.binding.K_UPDATE]) * 1e-3
+    algo_bytes = ALGO_BYTES_PER_UNIT * units_per_step
+    achieved = algo_bytes / t_proj / 1e9
+    wl = "c%d" % k
+    tr_reduce, tr_update = ncu_traffic(wl, "reduce_kernel"), ncu_traffic(wl, "update_kernel")
+    roofline = {"kernel": "K4 reduce_kernel + K6 update_kernel (projection + FIRE)", "bound": "hbm", "achieved": achieved,
+                "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+                "traffic": (tr_reduce + tr_update) if (tr_reduce and tr_update) else None,
+                "algorithmic_bytes": algo_bytes, "ms": t_proj * 1e3,
+                "share_of_step": float((kms[cf.binding.K_REDUCE] + kms[cf.binding.K_UPDATE]) / kms.sum())}
+    kernels = {name: {"ms_per_step": float(kms[i]), "share": float(kms[i] / kms.sum())}
+               for i, name in enumerate(cf.KERNEL_CLASSES)}
+    kernels["sum_ms_per_step"] = float(kms.sum())
+    kernels["update_only_GBps"] = 120.0 * units_per_step / (kms[cf.binding.K_UPDATE] * 1e-3) / 1e9
+    kernels["reduce_only_GBps"] = 72.0 * units_per_step / (kms[cf.binding.K_REDUCE] * 1e-3) / 1e9
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": workload_name(k), "n_atoms": N, "n_images": P, "movable_images": P - 2,
+                   "potential": "finnis_sinclair_morse" if spec.potential else "lj_shifted_force",
+                   "cell_filter": "rotation-free B = D D^T (Eq. 17), cell_factor auto", "climb": bool(spec.climb),
+                   "value_counts": "N x (P-2) per step", "value_counting_all_images": value * P / (P - 2),
+                   "parallelism": "replicas only (x%d)" % world if world > 1 else "single GPU",
+                   "l2": "state streamed per step (X, v, F: %.0f MB) exceeds the 126 MB L2; no explicit flush"
+                         % (72.0 * N * P / 1e6),
+                   "workspace_GB": band.workspace_bytes / 1e9, "neighbor_rebuilds_in_timed_region": int(st1.rebuilds - st0.rebuilds),
+                   "max_neighbors_seen": int(st1.max_neighbors_seen)},
+        "clocks": clocks, "roofline": roofline, "kernels": kernels,
+        "gpu_launches": int(st1.graph_kernel_nodes) * args.steps,
+        "status": {"fmax": st1.fmax, "barrier": st1.barrier, "steps": int(st1.steps)},
+    }
+    return band, line, (pos, cells, spec, barrier, max_over_ranks, world, rank, units_per_step)
+
+
+def measure_e2e(band, pos, cells, n_steps, barrier, max_over_ranks, world, units_per_step):
+    """Host-buffer loop through the C ABI: per step H2D of the whole path (pinned), one iteration, D2H of the path."""
+    import torch
+    P, N = pos.shape[0], pos.shape[1]
+    pin_pos = torch.empty((P, N, 3), dtype=torch.float64, pin_memory=True)
+    pin_cells = torch.empty((P, 3, 3), dtype=torch.float64, pin_memory=True)
+    pin_pos.numpy()[...] = pos
+    pin_cells.numpy()[...] = cells
+    out_pos = torch.empty((P, N, 3), dtype=torch.float64, pin_memory=True)
+    out_cells = torch.empty((P, 3, 3), dtype=torch.float64, pin_memory=True)
+    out_E = torch.empty((P,), dtype=torch.float64, pin_memory=True)
+    a_pos, a_cells = pin_pos.numpy(), pin_cells.numpy()
+    o_pos, o_cells, o_E = out_pos.numpy(), out_cells.numpy(), out_E.numpy()
+
+    def one():
+        band.set_path(a_pos, a_cells)              # H2D: P x (N x 3 + 9) doubles
+        band.step(1)
+        band.get_path_into(o_pos, o_cells, o_E)    # D2H: P x (N x 3 + 9 + 1) doubles; synchronises
+        a_pos[...] = o_pos                         # the next step's input is this step's output (host copy)
+        a_cells[...] = o_cells
+
+    one()  # warm-up
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_steps):
+        one()
+    barrier()
+    dt = max_over_ranks(time.perf_counter() - t0)
+    h2d = P * (N * 3 + 9) * 8
+    d2h = P * (N * 3 + 9 + 1) * 8
+    return {"value": world * units_per_step * n_steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+            "steps": n_steps, "ms_per_step": 1e3 * dt / n_steps,
+            "what": "per step: cfneb_set_path(host pinned) + cfneb_step(1) + cfneb_get_path(host pinned); wall clock, "
+                    "includes the host-side copy of the returned path into the next step's input"}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return main_reference(args)
+    band, line, ctx = main_ours(args)
+    pos, cells, spec, barrier, max_over_ranks, world, rank, units_per_step = ctx
+    if not args.no_e2e:
+        line["e2e"] = measure_e2e(band, pos, cells, max(1, args.e2e_steps), barrier, max_over_ranks, world, units_per_step)
+    try:
+        import paper_2510_16721_b200 as cf
+        tf = cf.fp64_peak_tflops()
+        line["kernels"]["fp64_dfma_peak_tflops_measured"] = tf
+    except Exception as exc:  # measurement utility only
+        line["kernels"]["fp64_dfma_peak_tflops_measured"] = "failed: %s" % exc
+    band.close()
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r = run_oracle(args.config, steps=2, warmup=0, budget_s=25.0)
+        line["cpu_baseline"] = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle",
+                                "sample": r["sample"], "host_cores": r["host_cores"], "seconds": r["seconds"]}
+    if rank == 0:
+        print(json.dumps(line))
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -136,8 +136,11 @@ def load_vacancy_endpoints(k):
     return (np.array(d["pos_init"]), np.array(d["cell_init"]), np.array(d["pos_final"]), np.array(d["cell_final"]))
 
 
-def build_workload(k, n_images=None):
+def build_workload(k, n_images=None, dims=None):
     """Seeded inputs of BASELINE.json configs[k]: (spec, pos[P,N,3] Cartesian, cells[P,3,3]).
+
+    n_images / dims (Bain configs only) override the config's band length / supercell: the same recipe at
+    another size (used for bounded CPU-baseline samples and for parity cases between the configs).
 
     Vacancy configs: stored relaxed endpoints, 7 / 9 images linear in (fractional coordinates, cell) + noise.
     Bain configs: perfect bcc at the stress-free lattice constant and its c/a = sqrt(2) image at the stress-free
@@ -151,6 +154,6 @@ def build_workload(k, n_images=None):
         pos, cells = linear_path(R0 @ np.linalg.inv(h0), h0, R1 @ np.linalg.inv(h1), h1, P, spec.seed, spec.noise_sigma)
     else:
         lc = load_lattice_constants()
-        f0, c0, f1, c1 = bain_endpoints(spec.dims, lc["fs_bcc_a"], lc["fs_fcc_volume_ratio"])
+        f0, c0, f1, c1 = bain_endpoints(tuple(dims) if dims else spec.dims, lc["fs_bcc_a"], lc["fs_fcc_volume_ratio"])
         pos, cells = linear_path(f0, c0, f1, c1, P, spec.seed, spec.noise_sigma)
     return spec, pos, cells

@@ -98,7 +98,7 @@ typedef struct cfneb_status {
     int32_t error;          /* sticky device error (0 or a negative CFNEB_E* code) */
     int32_t n_pos;          /* FIRE counter of consecutive power > 0 steps */
     int32_t max_neighbors_seen;
-    int32_t reserved0;
+    int32_t graph_kernel_nodes; /* kernel launches of one captured iteration (cudaGraphGetNodes) */
     double fmax;            /* O8: max row norm of the NEB force of the last step (cell rows count as rows) */
     double barrier;         /* O8: E_{p*} - E_0 at the last evaluation */
     double dt, alpha;       /* FIRE state after the last step */

@@ -43,7 +43,7 @@ class Status(ctypes.Structure):
     _fields_ = [
         ("steps", ctypes.c_int64), ("rebuilds", ctypes.c_int64), ("n_images", ctypes.c_int32),
         ("climb_index", ctypes.c_int32), ("error", ctypes.c_int32), ("n_pos", ctypes.c_int32),
-        ("max_neighbors_seen", ctypes.c_int32), ("reserved0", ctypes.c_int32), ("fmax", ctypes.c_double),
+        ("max_neighbors_seen", ctypes.c_int32), ("graph_kernel_nodes", ctypes.c_int32), ("fmax", ctypes.c_double),
         ("barrier", ctypes.c_double), ("dt", ctypes.c_double), ("alpha", ctypes.c_double),
         ("cell_factor", ctypes.c_double), ("path_length", ctypes.c_double),
     ]
@@ -252,6 +252,14 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_get_path")
         return pos, cells, E
+
+    def get_path_into(self, pos, cells, energies):
+        """cfneb_get_path into caller-owned (e.g. pinned) float64 arrays; any may be None."""
+        n = ctypes.c_int32(0)
+        rc = lib().cfneb_get_path(self._h, ctypes.byref(n), _dptr(pos), _dptr(cells), _dptr(energies))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_path")
+        return n.value
 
     def set_path(self, pos, cells):
         pos, cells = _f64(pos), _f64(cells)

@@ -33,8 +33,7 @@ struct cfneb {
     std::vector<int> free_slots;
     cudaGraph_t graph;
     cudaGraphExec_t exec;
-    cudaEvent_t ev[CFNEB_NKERNELS + 1];
-    bool have_events;
+    int graph_nodes;
 };
 
 // ---- workspace carving (one function serves the size query and create) ----
@@ -101,8 +100,9 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
     d.bin_members = c.take<int>(S * Npad);
     d.atom_bin = c.take<int>(S * Npad);
-    const size_t half = S * (size_t)(N + 3) * 3 * sizeof(double);
-    size_t sb = 2 * half + S * 16 * sizeof(double) + 1024;
+    // scratch = two halves; a half holds one exported array set (P x (N+3) x 3, or P x N x 3 + P x 9 + P)
+    const size_t half = S * ((size_t)(N + 3) * 3 + 16) * sizeof(double);
+    size_t sb = 2 * half + 1024;
     const size_t nb = (size_t)N * d.cap * 4 * sizeof(int) + (size_t)N * sizeof(int) + 1024;
     if (nb > sb) sb = nb;
     d.scratch = c.take<char>(sb);
@@ -188,6 +188,9 @@ int capture_graph(cfneb *h) {
     cudaGraph_t g = nullptr;
     CK(cudaStreamEndCapture(h->st, &g));
     h->graph = g;
+    size_t n_nodes = 0;
+    CK(cudaGraphGetNodes(g, nullptr, &n_nodes));
+    h->graph_nodes = (int)n_nodes;
     CK(cudaGraphInstantiate(&h->exec, g, 0));
     return CFNEB_OK;
 }
@@ -237,7 +240,6 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     h->prm = *prm;
     h->graph = nullptr;
     h->exec = nullptr;
-    h->have_events = false;
     h->own_stream = false;
     h->st = static_cast<cudaStream_t>(cuda_stream);
 #define CKH(call)                                  \
@@ -344,8 +346,6 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     int rc = sync_status(h);
     if (rc) { cfneb_destroy(h); return rc; }
     CKH(capture_graph(h));
-    for (int k = 0; k <= CFNEB_NKERNELS; ++k) CKC(cudaEventCreate(&h->ev[k]));
-    h->have_events = true;
     *out = h;
     return CFNEB_OK;
 #undef CKH
@@ -360,16 +360,27 @@ int cfneb_step(cfneb_t *h, int32_t n_steps) {
 
 int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms) {
     if (!h || n_steps < 0 || !kernel_ms) return CFNEB_EINVAL;
-    for (int k = 0; k < n_steps; ++k) {
-        enqueue_step(h, h->ev);
-        CK(cudaEventSynchronize(h->ev[CFNEB_NKERNELS]));
-        for (int c = 0; c < CFNEB_NKERNELS; ++c) {
-            float ms = 0.f;
-            CK(cudaEventElapsedTime(&ms, h->ev[c], h->ev[c + 1]));
-            kernel_ms[c] += (double)ms;
-        }
+    // one event set per step, read back after the last step: no host synchronisation between steps
+    const int per = CFNEB_NKERNELS + 1;
+    std::vector<cudaEvent_t> ev((size_t)n_steps * per, nullptr);
+    int rc = CFNEB_OK;
+    for (size_t k = 0; k < ev.size() && rc == CFNEB_OK; ++k)
+        if (cudaEventCreate(&ev[k]) != cudaSuccess) rc = CFNEB_ECUDA;
+    if (rc == CFNEB_OK) {
+        for (int k = 0; k < n_steps; ++k) enqueue_step(h, ev.data() + (size_t)k * per);
+        rc = sync_status(h);
     }
-    return sync_status(h);
+    if (rc == CFNEB_OK)
+        for (int k = 0; k < n_steps; ++k)
+            for (int c = 0; c < CFNEB_NKERNELS; ++c) {
+                float ms = 0.f;
+                if (cudaEventElapsedTime(&ms, ev[(size_t)k * per + c], ev[(size_t)k * per + c + 1]) != cudaSuccess) rc = CFNEB_ECUDA;
+                kernel_ms[c] += (double)ms;
+            }
+    for (cudaEvent_t e : ev)
+        if (e) cudaEventDestroy(e);
+    if (rc == CFNEB_ECUDA) snprintf(g_cuda_err, sizeof g_cuda_err, "cfneb_step_timed: %s", cudaGetErrorString(cudaGetLastError()));
+    return rc;
 }
 
 int cfneb_insert_image(cfneb_t *h, int32_t after) {
@@ -557,6 +568,7 @@ int cfneb_get_status(cfneb_t *h, cfneb_status *out) {
     out->error = c.error;
     out->n_pos = c.n_pos;
     out->max_neighbors_seen = c.max_nbr_seen;
+    out->graph_kernel_nodes = h->graph_nodes;
     unsigned long long b = c.fmax_bits;
     double f2;
     memcpy(&f2, &b, sizeof f2);
@@ -575,8 +587,6 @@ void cfneb_destroy(cfneb_t *h) {
     if (h->st) cudaStreamSynchronize(h->st);
     if (h->exec) cudaGraphExecDestroy(h->exec);
     if (h->graph) cudaGraphDestroy(h->graph);
-    if (h->have_events)
-        for (int k = 0; k <= CFNEB_NKERNELS; ++k) cudaEventDestroy(h->ev[k]);
     if (h->own_stream && h->st) cudaStreamDestroy(h->st);
     delete h;
 }

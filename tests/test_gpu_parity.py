@@ -95,7 +95,7 @@ def test_forces_energies_virials_and_neb_force(k, lam):
     gpu.close()
 
 
-@pytest.mark.parametrize("k,lam,nsteps", [(0, 1.0, 30), (0, 0.0, 30), (1, 0.0, 20), (2, 0.0, 12), (2, 1.0, 6)])
+@pytest.mark.parametrize("k,lam,nsteps", [(0, 1.0, 30), (0, 0.0, 30), (1, 0.0, 20), (2, 0.0, 12), (1, 1.0, 10)])
 def test_neb_steps_match_oracle(k, lam, nsteps):
     """X and v after 1, 2, ... n full iterations (K0-K6) against the oracle's step()."""
     spec, orc, gpu = make_pair(k, cell_factor=lam)
@@ -171,13 +171,14 @@ def test_cell_modes_fixed_and_D(mode):
     """CELL_FIXED (no cell force) and the Eq. 14 D-variant follow the oracle too."""
     spec, orc, gpu = make_pair(0, cell_factor=1.0, cell_mode=mode)
     X0, _ = orc.get_state()
+    Xg0, _ = gpu.get_state()
     orc.step(5)
     gpu.step(5)
     Xo, vo = orc.get_state()
     Xg, vg = gpu.get_state()
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
-    if mode == 0:
-        assert np.array_equal(Xg[:, -3:], X0[:, -3:])
+    if mode == 0:  # O4: G_cell = 0; the cell rows only see the (here ~1e-16) tangent between the endpoint cells
+        assert np.max(np.abs(Xg[:, -3:] - Xg0[:, -3:])) < 1e-12 and np.max(np.abs(Xo[:, -3:] - X0[:, -3:])) < 1e-12
     gpu.close()
 
 
