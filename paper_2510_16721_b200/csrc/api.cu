@@ -1,6 +1,7 @@
 // api.cu -- the C ABI of include/cfneb.h: handle, workspace carving, CUDA-graph capture of one CFNEB
 // iteration (K0-K6), host-side image control (O9) and the parity / checkpoint hooks.
 // All arithmetic of the method runs in the kernels; this file only marshals, launches and copies.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -77,6 +78,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     Carver c{static_cast<char *>(base), 0};
     d.ctl = c.take<Ctl>(1);
     d.order = c.take<int>(S);
+    d.perm = c.take<int>(Npad);
     d.geom = c.take<Geom>(S);
     d.X = c.take<double>(2 * S * img);
     d.v = c.take<double>(S * img);
@@ -96,6 +98,8 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.dispmax = c.take<unsigned long long>(S);
     d.nbr_count = c.take<int>(S * Npad);
     d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad);
+    d.nbr_in = c.take<uint32_t>(S * (size_t)d.cap * Npad);
+    d.nbr_in_count = c.take<int>(S * Npad);
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
     d.bin_members = c.take<int>(S * Npad);
@@ -119,6 +123,35 @@ void perp_widths(const double *h, double *w) {
         const double cx = b[1] * c[2] - b[2] * c[1], cy = b[2] * c[0] - b[0] * c[2], cz = b[0] * c[1] - b[1] * c[0];
         w[a] = vol / sqrt(cx * cx + cy * cy + cz * cz);
     }
+}
+
+// Spatial storage order: Morton order of a grid of edge ~ r_list / 2 over the initial endpoint (ties by the
+// caller's index).  perm[internal] = caller's index.  Any order is correct; this one keeps the neighbours of
+// consecutive atoms close in memory.
+void spatial_order(int N, const double *pos, const double *cell, double r_list, std::vector<int> &perm) {
+    double inv[9], w[3];
+    inv3(cell, inv);
+    perp_widths(cell, w);
+    int n[3];
+    for (int a = 0; a < 3; ++a) n[a] = std::max(1, std::min(1023, (int)floor(w[a] / (0.5 * r_list))));
+    std::vector<unsigned long long> key(N);
+    for (int i = 0; i < N; ++i) {
+        const double *r = pos + 3 * (size_t)i;
+        unsigned c[3];
+        for (int a = 0; a < 3; ++a) {
+            double s = r[0] * inv[a] + r[1] * inv[3 + a] + r[2] * inv[6 + a];
+            s -= floor(s);
+            int b = (int)(s * n[a]);
+            c[a] = (unsigned)std::max(0, std::min(n[a] - 1, std::isfinite(s) ? b : 0));
+        }
+        unsigned long long m = 0;
+        for (int bit = 0; bit < 10; ++bit)
+            for (int a = 0; a < 3; ++a) m |= (unsigned long long)((c[a] >> bit) & 1u) << (3 * bit + a);
+        key[i] = m;
+    }
+    perm.resize(N);
+    for (int i = 0; i < N; ++i) perm[i] = i;
+    std::stable_sort(perm.begin(), perm.end(), [&](int a, int b) { return key[a] < key[b]; });
 }
 
 int device_error(cfneb *h, int *code) {
@@ -312,6 +345,13 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     c0.alpha = d.astart;
     CKC(cudaMemcpyAsync(d.ctl, &c0, sizeof c0, cudaMemcpyHostToDevice, h->st));
     CKH(upload_order(h));
+    {
+        std::vector<int> perm;
+        spatial_order(n_atoms, pos_init, cell_init, d.r_list, perm);
+        perm.resize(d.Npad, 0);
+        CKC(cudaMemcpyAsync(d.perm, perm.data(), sizeof(int) * d.Npad, cudaMemcpyHostToDevice, h->st));
+        CKC(cudaStreamSynchronize(h->st));  // `perm` is a temporary
+    }
 
     // stage the host inputs: pos [n][N][3] then cells [n][9]
     const size_t N3 = (size_t)n_atoms * 3;

@@ -2,7 +2,9 @@
 // (Product code: shares nothing with oracle/.)
 //
 // HBM layout (fp64 SoA, one "slot" per image; path position p -> slot through the order table, so
-// insertion / deletion never moves atom data):
+// insertion / deletion never moves atom data).  Atoms are stored in a spatial (Morton) order fixed at create
+// -- consecutive threads own neighbouring atoms, so the position gathers of a block stay inside L1 -- and
+// `perm` maps back to the caller's order at the boundary (input map, exports, parity hooks):
 //   X    [2][S][3][Npad]   R~ of Eq. 10, double-buffered (K6 reads X_{p-1}, X_p, X_{p+1} of buffer src,
 //                          writes buffer dst); rows padded with zeros to Npad (multiple of 32)
 //   v, F [S][3][Npad]      FIRE velocity, Cartesian force (Eq. 5)
@@ -73,6 +75,7 @@ struct Dev {
     double h0[9], h0inv[9];
     Ctl *ctl;
     int *order;               // [S] path position -> slot
+    int *perm;                // [Npad] internal atom index -> caller's atom index (spatial order, see api.cu)
     Geom *geom;               // [S]
     double *X, *v, *F;        // see header comment
     double *fneb;             // parity-hook scratch [S][(N+3)*3], external row-major layout
@@ -86,7 +89,10 @@ struct Dev {
     double *part_dots;        // [S][nblk_stream][10]
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
     int *nbr_count;           // [S][Npad]
-    uint32_t *nbr_list;       // [S][cap][Npad]
+    uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), rebuilt when stale
+    uint32_t *nbr_in;         // [S][cap][Npad]  in-range list of the current step: plain entries from k = 0 up,
+                              //                 taper-zone entries from k = cap-1 down (written by K2a every step)
+    int *nbr_in_count;        // [S][Npad]       n_plain | n_taper << 16
     int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
     int *bin_cursor;          // [S][nbins_max]
     int *bin_members;         // [S][Npad]

@@ -74,7 +74,7 @@ __global__ void input_map_kernel(Dev d, const double *__restrict__ pos, const do
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const size_t img = (size_t)3 * d.Npad, buf = (size_t)d.S * img;
     if (i < d.N) {
-        const double *r = pos + ((size_t)p * d.N + i) * 3;
+        const double *r = pos + ((size_t)p * d.N + d.perm[i]) * 3;  // caller's order -> spatial storage order
         for (int c = 0; c < 3; ++c) {
             double x = r[0] * Dinv[c] + r[1] * Dinv[3 + c] + r[2] * Dinv[6 + c];  // R~ = R D^-1 (Eq. 10)
             d.X[slot * img + (size_t)c * d.Npad + i] = x;

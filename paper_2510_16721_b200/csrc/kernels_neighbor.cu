@@ -176,15 +176,16 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
 
 // Parity hook: list of one slot in the external layout count[N], list[N][cap] (-1 padded), shift[N][cap][3].
 __global__ void unpack_neighbors_kernel(Dev d, int slot, int *count_out, int *list_out, int *shift_out) {
-    const size_t e = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (e >= (size_t)d.N * d.cap) return;
-    const int i = (int)(e / d.cap), k = (int)(e % d.cap);
+    const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= (size_t)d.N * d.cap) return;
+    const int i = (int)(t / d.cap), k = (int)(t % d.cap);  // internal (storage-order) atom index
+    const size_t e = (size_t)d.perm[i] * d.cap + k;         // row of the caller's atom
     const int c = d.nbr_count[(size_t)slot * d.Npad + i];
-    if (k == 0) count_out[i] = c;
+    if (k == 0) count_out[d.perm[i]] = c;
     int j = -1, n0 = 0, n1 = 0, n2 = 0;
     if (k < c) {
         const uint32_t w = d.nbr_list[((size_t)slot * d.cap + k) * d.Npad + i];
-        j = (int)(w & kIdxMask);
+        j = d.perm[w & kIdxMask];
         const uint32_t code = w >> kShiftBits;
         n0 = (int)(code & 7u) - 4;
         n1 = (int)((code >> 3) & 7u) - 4;

@@ -108,7 +108,7 @@ __global__ void materialize_fneb_kernel(Dev d) {
     const int rows = d.N + 3;
     const int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= rows) return;
-    double *out = d.fneb + ((size_t)p * rows + a) * 3;
+    double *out = d.fneb + ((size_t)p * rows + (a < d.N ? d.perm[a] : a)) * 3;
     if (p == 0 || p == P - 1) {
         out[0] = out[1] = out[2] = 0.0;
         return;
@@ -212,7 +212,7 @@ __global__ void export_path_kernel(Dev d, double *pos, double *cells, double *E)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < d.N && pos) {
         const double4 r = d.Rc[(size_t)slot * d.Npad + i];
-        double *o = pos + ((size_t)p * d.N + i) * 3;
+        double *o = pos + ((size_t)p * d.N + d.perm[i]) * 3;
         o[0] = r.x; o[1] = r.y; o[2] = r.z;
     }
     if (blockIdx.x == 0 && threadIdx.x < 9 && cells) cells[p * 9 + threadIdx.x] = d.geom[slot].h[threadIdx.x];
@@ -231,6 +231,7 @@ __global__ void export_state_kernel(Dev d, double *Xo, double *vo) {
     const double *Xb = d.X + ((size_t)d.ctl->cur * d.S + slot) * img;
     const double *Xc = d.Xc + ((size_t)d.ctl->cur * d.S + slot) * 9;
     const bool movable = p > 0 && p < P - 1;
+    const int ao = a < d.N ? d.perm[a] : a;  // row of the caller's layout
     for (int c = 0; c < 3; ++c) {
         double x, v;
         if (a < d.N) {
@@ -240,8 +241,8 @@ __global__ void export_state_kernel(Dev d, double *Xo, double *vo) {
             x = Xc[3 * (a - d.N) + c];
             v = d.vc[slot * 9 + 3 * (a - d.N) + c];
         }
-        if (Xo) Xo[((size_t)p * rows + a) * 3 + c] = x;
-        if (vo) vo[((size_t)p * rows + a) * 3 + c] = movable ? v : 0.0;
+        if (Xo) Xo[((size_t)p * rows + ao) * 3 + c] = x;
+        if (vo) vo[((size_t)p * rows + ao) * 3 + c] = movable ? v : 0.0;
     }
 }
 
@@ -252,7 +253,7 @@ __global__ void export_forces_kernel(Dev d, double *Fo, double *Vo, double *Eo) 
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < d.N && Fo) {
         const double *F = d.F + (size_t)slot * 3 * d.Npad;
-        double *o = Fo + ((size_t)p * d.N + i) * 3;
+        double *o = Fo + ((size_t)p * d.N + d.perm[i]) * 3;
         o[0] = F[i]; o[1] = F[d.Npad + i]; o[2] = F[2 * (size_t)d.Npad + i];
     }
     if (blockIdx.x == 0 && threadIdx.x < 9 && Vo) Vo[p * 9 + threadIdx.x] = d.V[slot * 9 + threadIdx.x];
