@@ -1,0 +1,124 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (configs[3], configs[4]).
+
+configs[4] (101 306 atoms x 100 images): the oracle is run on ALL images with every host core (one evaluation of
+the band at construction + one full step: about a minute on 16 cores), and every output is compared element by
+element: energies, per-atom forces, virials, f^NEB, then X and v after one full iteration (K0-K6), then the
+neighbour list of one mid-path image, bit-exact after sorting.
+
+configs[3] (9 826 atoms, 12 -> up to 32 images, adaptive): the GPU band and the oracle band run the same schedule
+(10 steps, adapt, ...) with the DESIGN.md thresholds; the image count, the inserted / deleted positions and the
+coordinates must agree after every control step.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from cfneb_workloads import build_workload
+
+pytestmark = pytest.mark.gpu
+
+TOL_FORCE = 1e-10
+TOL_STEP = 1e-9
+
+
+def rel(a, b):
+    a, b = np.asarray(a), np.asarray(b)
+    s = np.max(np.abs(b))
+    return float(np.max(np.abs(a - b)) / (s if s > 0 else 1.0))
+
+
+def host_threads():
+    try:
+        return len(os.sched_getaffinity(0))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+def test_c4_full_size_forces_and_one_step():
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    from oracle import forcefield as ff
+    spec, pos, cells = build_workload(4)
+    P, N = pos.shape[0], pos.shape[1]
+    assert (N, P) == (101306, 100)
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb,
+                   cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors,
+                   threads=host_threads())
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))  # the band bench.py builds
+    f_or = orc.band.forces()
+    last = orc.evaluator.last
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE
+    assert rel(V[1:-1], last["V"]) < TOL_FORCE
+    worst_f = max(rel(F[p], last["F"][p - 1]) for p in range(1, P - 1))
+    assert worst_f < TOL_FORCE, worst_f
+    worst_n = max(rel(fneb[p], f_or[p]) for p in range(1, P - 1))
+    assert worst_n < TOL_STEP, worst_n
+    st = gpu.get_status()
+    assert st.climb_index == orc.band.pstar
+    # the energies that decide tangent branches and the climbing image are not within round-off of a tie (A24)
+    dE = np.abs(np.diff(orc.band.E))
+    assert dE.min() > 1e-8 * np.abs(orc.band.E).max()
+    del F, V, fneb, f_or
+
+    # neighbour list of one mid-path image, bit-exact after sorting (counts and (j, shift) sets per atom)
+    image = P // 2
+    Rt, D = orc.evaluator.deformation(orc.band.X[image])
+    cnt, lst, sh = ff.neighbors(Rt, orc.h0, orc.h0 @ D, spec.r_cut + spec.skin, spec.max_neighbors)
+    gc, gl, gs = gpu.get_neighbors(image)
+    assert np.array_equal(gc, cnt)
+    key_o = np.where(lst >= 0, lst.astype(np.int64) * 512 + (sh[..., 0] + 4) * 64 + (sh[..., 1] + 4) * 8 + (sh[..., 2] + 4), -1)
+    key_g = np.where(gl >= 0, gl.astype(np.int64) * 512 + (gs[..., 0] + 4) * 64 + (gs[..., 1] + 4) * 8 + (gs[..., 2] + 4), -1)
+    assert np.array_equal(np.sort(key_g, axis=1), np.sort(key_o, axis=1))
+    del key_o, key_g, lst, sh, gl, gs
+
+    # one full iteration
+    X0, _ = orc.get_state()
+    orc.step(1)
+    gpu.step(1)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < TOL_STEP
+    assert rel(vg, vo) < TOL_STEP
+    st = gpu.get_status()
+    assert st.error == 0 and st.steps == 1
+    assert abs(st.fmax - orc.band.fmax) <= 1e-8 * orc.band.fmax
+    gpu.close()
+
+
+def test_c3_adaptive_band_follows_oracle():
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(3)
+    P0, N = pos.shape[0], pos.shape[1]
+    assert (N, P0) == (9826, 12)
+    max_images = 32
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb,
+                   cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors,
+                   threads=host_threads())
+    orc.max_images = max_images
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, max_images=max_images))
+    L0 = float(np.sum(orc.band.segment_lengths()))
+    assert abs(float(np.sum(gpu.get_segment_lengths())) - L0) < 1e-10 * L0
+    d_insert, d_delete = L0 / 28.0, L0 / 120.0  # DESIGN.md section 7 (reading A16)
+    grew = 0
+    for cycle in range(4):
+        orc.step(3)
+        gpu.step(3)
+        assert rel(gpu.get_segment_lengths(), orc.band.segment_lengths()) < 1e-9
+        ro, rg = orc.adapt(d_insert, d_delete), gpu.adapt(d_insert, d_delete)
+        assert ro == rg, (cycle, ro, rg)
+        grew += rg[0] - rg[1]
+        assert gpu.P == orc.P == P0 + grew
+        Xo, vo = orc.get_state()
+        Xg, vg = gpu.get_state()
+        assert rel(Xg, Xo) < 1e-11
+        if rg != (0, 0):
+            assert np.all(vg == 0)
+    assert grew > 0  # the initial spacing L0/11 exceeds d_insert = L0/28: the band must grow
+    orc.step(2)
+    gpu.step(2)
+    assert rel(gpu.get_state()[0], orc.get_state()[0]) < 1e-10
+    assert gpu.get_status().error == 0
+    gpu.close()
