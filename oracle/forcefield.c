@@ -297,8 +297,12 @@ int oracle_energy_force_virial(int N, const double *Rt, const double *h0, const 
     double rc2 = rcut * rcut;
     double *dF = NULL;
     double *rho = NULL;
-    double Etot = 0.0;
-    for (int k = 0; k < 9; ++k) V[k] = 0.0;
+    /* E (Eq. 4) and V (Eq. 8) are sums of N and ~100 N terms and the paper fixes no summation order.  Totals are
+     * accumulated in long double: a plain sequential double sum of 10^5 near-identical U_i (a perfect-lattice
+     * endpoint) carries a systematic error of ~1e-6 eV at |E| ~ 9e5 eV, which is visible in the barrier and in
+     * the energy-weighted tangent at extrema (O5). */
+    long double Etot = 0.0L, Vacc[9];
+    for (int k = 0; k < 9; ++k) Vacc[k] = 0.0L;
     for (int i = 0; i < 3 * N; ++i) F[i] = 0.0;
 
     if (kind == 1) { /* pass 1: densities rho_i = sum_j psi(r_ij), then F'(rho_i) */
@@ -348,7 +352,7 @@ int oracle_energy_force_virial(int N, const double *Rt, const double *h0, const 
             double f[3] = {fmag * r[0] / rr, fmag * r[1] / rr, fmag * r[2] / rr};
             for (int m = 0; m < 3; ++m) {
                 F[3 * i + m] += f[m];
-                for (int n = 0; n < 3; ++n) V[3 * m + n] += -0.5 * r[m] * f[n];
+                for (int n = 0; n < 3; ++n) Vacc[3 * m + n] += (long double)(-0.5 * r[m] * f[n]);
             }
         }
         if (kind == 1) {
@@ -359,7 +363,8 @@ int oracle_energy_force_virial(int N, const double *Rt, const double *h0, const 
         if (Ui) Ui[i] = ui;
         Etot += ui;
     }
-    *E = Etot;
+    *E = (double)Etot;
+    for (int k = 0; k < 9; ++k) V[k] = (double)Vacc[k];
     if (rho_out && rho) memcpy(rho_out, rho, sizeof(double) * (size_t)N);
     free(s); free(rho); free(dF);
     return ORACLE_OK;

@@ -296,6 +296,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     }
     Dev &d = h->d;
     carve(n_atoms, prm, dev_workspace, &d);
+    plan_stream_grids(d);
     d.potential = prm->potential;
     d.cell_mode = prm->cell_mode;
     d.climb = prm->climb ? 1 : 0;

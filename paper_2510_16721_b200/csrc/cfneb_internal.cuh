@@ -67,6 +67,8 @@ struct Dev {
     int N, Npad, S, cap;
     int potential, cell_mode, climb, fire_nmin, rebuild_every;
     int nblk_atom, nblk_stream, nbins_max;
+    int k4_variant, k6_variant;
+    int nblk_red, nblk_upd;   // K4 / K6: blocks per image, each striding over the image's nblk_stream tiles
     int nb_cap[3];
     double pot[12];
     double k_spring, lam;
@@ -86,7 +88,7 @@ struct Dev {
     double *E, *V, *Gc;       // [S], [S][9], [S][9]
     double *dots, *coef;      // [S][10], [S][4]
     double *part_force;       // [S][nblk_atom][8]
-    double *part_dots;        // [S][nblk_stream][10]
+    double *part_dots;        // [S][nblk_stream][10]  (the first nblk_red rows of an image are used)
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), rebuilt when stale
@@ -134,6 +136,7 @@ void launch_cell_prep(const Dev &d, int p_lo, int mode, cudaStream_t st);       
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st);                      // K1
 void launch_force(const Dev &d, int p_lo, cudaStream_t st);                               // K2
 void launch_reduce(const Dev &d, cudaStream_t st);                                        // K4 (atom rows)
+void plan_stream_grids(Dev &d);  // nblk_red / nblk_upd from the SM count and the kernels' occupancy
 void launch_finalize(const Dev &d, int p_lo, cudaStream_t st);                            // K4 second stage
 void launch_scalar(const Dev &d, int dry, cudaStream_t st);                               // K5
 void launch_update(const Dev &d, cudaStream_t st);                                        // K6

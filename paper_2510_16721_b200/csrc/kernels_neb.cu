@@ -10,6 +10,7 @@
 // FIRE needs (f.v, |f|, |v|, |v_new|) follows from ten dot products per image taken in ONE pass over
 // X, F, v (K4); K6 then streams the same arrays once more and writes X_new, v_new.
 #include "cfneb_internal.cuh"
+#include <stdlib.h>
 
 namespace cfn {
 
@@ -18,8 +19,14 @@ __device__ inline void st2(double *p, double2 v) { *reinterpret_cast<double2 *>(
 
 // ------------------------------------------------------------------------------------------------
 // K4: ten dot products over the atom rows of each movable image; per-block partials.
-// grid (nblk_stream, S-2), 256 threads, two atoms per thread (128-bit loads on SoA rows).
-__global__ void __launch_bounds__(kThreadsStream) reduce_kernel(Dev d) {
+// grid (nblk_red, S-2), 256 threads.  An image is cut into nblk_stream tiles of 512 atoms (two atoms per thread,
+// 128-bit loads on SoA rows); block b of an image takes tiles b, b + nblk_red, ... and keeps its ten sums in
+// registers across tiles, so the shuffle / shared-memory reduction runs once per block instead of once per
+// tile and loads of one block overlap the arithmetic of the others resident on the SM.  nblk_red is chosen so
+// that the grid fills an integer number of waves (plan_stream_grids).  Blocks of neighbouring images work on
+// the same tile index at about the same time, so X_{p-1} and X_{p+1} are L2 hits: DRAM sees X, F, v once (72 B).
+template <int MINB, int UNROLL>
+__global__ void __launch_bounds__(kThreadsStream, MINB) reduce_kernel(Dev d) {
     const int p = blockIdx.y + 1;
     if (p > d.ctl->P - 2) return;
     const int sm = d.order[p - 1], s0 = d.order[p], sp = d.order[p + 1];
@@ -31,38 +38,47 @@ __global__ void __launch_bounds__(kThreadsStream) reduce_kernel(Dev d) {
     const double *Xb = d.X + (size_t)d.ctl->cur * d.S * img;
     const double *Xm = Xb + sm * img, *X0 = Xb + s0 * img, *Xp = Xb + sp * img;
     const double *F = d.F + s0 * img, *V = d.v + s0 * img;
-    const int i = 2 * (blockIdx.x * kThreadsStream + threadIdx.x);
     double acc[kNDots];
 #pragma unroll
     for (int q = 0; q < kNDots; ++q) acc[q] = 0.0;
-    if (i < d.Npad) {
-        double2 f[3], xm[3], x0[3], xp[3], vv[3];
+    for (int tile = blockIdx.x; tile < d.nblk_stream; tile += UNROLL * gridDim.x) {
+        double2 f[UNROLL][3], xm[UNROLL][3], x0[UNROLL][3], xp[UNROLL][3], vv[UNROLL][3];
+        bool on[UNROLL];
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            const size_t o = (size_t)c * d.Npad + i;
-            f[c] = ld2(F + o);
-            xm[c] = ld2(Xm + o);
-            x0[c] = ld2(X0 + o);
-            xp[c] = ld2(Xp + o);
-            vv[c] = ld2(V + o);
+        for (int u = 0; u < UNROLL; ++u) {
+            const int t = tile + u * gridDim.x;
+            const int i = 2 * (t * kThreadsStream + threadIdx.x);
+            on[u] = t < d.nblk_stream && i < d.Npad;
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                const size_t o = (size_t)c * d.Npad + (on[u] ? i : 0);
+                f[u][c] = on[u] ? ld2(F + o) : make_double2(0.0, 0.0);
+                xm[u][c] = on[u] ? ld2(Xm + o) : make_double2(0.0, 0.0);
+                x0[u][c] = on[u] ? ld2(X0 + o) : make_double2(0.0, 0.0);
+                xp[u][c] = on[u] ? ld2(Xp + o) : make_double2(0.0, 0.0);
+                vv[u][c] = on[u] ? ld2(V + o) : make_double2(0.0, 0.0);
+            }
         }
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            // G = F D^T (Eq. 12): G_c = sum_m F_m D[c][m]
-            const double gx = f[0].x * sD[3 * c] + f[1].x * sD[3 * c + 1] + f[2].x * sD[3 * c + 2];
-            const double gy = f[0].y * sD[3 * c] + f[1].y * sD[3 * c + 1] + f[2].y * sD[3 * c + 2];
-            const double tpx = xp[c].x - x0[c].x, tpy = xp[c].y - x0[c].y;
-            const double tmx = x0[c].x - xm[c].x, tmy = x0[c].y - xm[c].y;
-            acc[DOT_PP] += tpx * tpx + tpy * tpy;
-            acc[DOT_MM] += tmx * tmx + tmy * tmy;
-            acc[DOT_PM] += tpx * tmx + tpy * tmy;
-            acc[DOT_GP] += gx * tpx + gy * tpy;
-            acc[DOT_GM] += gx * tmx + gy * tmy;
-            acc[DOT_GG] += gx * gx + gy * gy;
-            acc[DOT_GV] += gx * vv[c].x + gy * vv[c].y;
-            acc[DOT_PV] += tpx * vv[c].x + tpy * vv[c].y;
-            acc[DOT_MV] += tmx * vv[c].x + tmy * vv[c].y;
-            acc[DOT_VV] += vv[c].x * vv[c].x + vv[c].y * vv[c].y;
+        for (int u = 0; u < UNROLL; ++u) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                // G = F D^T (Eq. 12): G_c = sum_m F_m D[c][m]
+                const double gx = f[u][0].x * sD[3 * c] + f[u][1].x * sD[3 * c + 1] + f[u][2].x * sD[3 * c + 2];
+                const double gy = f[u][0].y * sD[3 * c] + f[u][1].y * sD[3 * c + 1] + f[u][2].y * sD[3 * c + 2];
+                const double tpx = xp[u][c].x - x0[u][c].x, tpy = xp[u][c].y - x0[u][c].y;
+                const double tmx = x0[u][c].x - xm[u][c].x, tmy = x0[u][c].y - xm[u][c].y;
+                acc[DOT_PP] += tpx * tpx + tpy * tpy;
+                acc[DOT_MM] += tmx * tmx + tmy * tmy;
+                acc[DOT_PM] += tpx * tmx + tpy * tmy;
+                acc[DOT_GP] += gx * tpx + gy * tpy;
+                acc[DOT_GM] += gx * tmx + gy * tmy;
+                acc[DOT_GG] += gx * gx + gy * gy;
+                acc[DOT_GV] += gx * vv[u][c].x + gy * vv[u][c].y;
+                acc[DOT_PV] += tpx * vv[u][c].x + tpy * vv[u][c].y;
+                acc[DOT_MV] += tmx * vv[u][c].x + tmy * vv[u][c].y;
+                acc[DOT_VV] += vv[u][c].x * vv[u][c].x + vv[u][c].y * vv[u][c].y;
+            }
         }
     }
     block_sum<kNDots>(acc, red);
@@ -116,7 +132,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
 #pragma unroll
     for (int q = 0; q < kNDots; ++q) a10[q] = 0.0;
     const double *pd = d.part_dots + (size_t)slot * d.nblk_stream * kNDots;
-    for (int b = threadIdx.x; b < d.nblk_stream; b += blockDim.x)
+    for (int b = threadIdx.x; b < d.nblk_red; b += blockDim.x)
 #pragma unroll
         for (int q = 0; q < kNDots; ++q) a10[q] += pd[(size_t)b * kNDots + q];
     block_sum<kNDots>(a10, red);
@@ -259,8 +275,46 @@ __global__ void __launch_bounds__(128) scalar_kernel(Dev d, int dry) {
 
 void launch_reduce(const Dev &d, cudaStream_t st) {
     if (d.S < 3) return;
-    dim3 grid(d.nblk_stream, d.S - 2);
-    reduce_kernel<<<grid, kThreadsStream, 0, st>>>(d);
+    dim3 grid(d.nblk_red, d.S - 2);
+    switch (d.k4_variant) {
+        case 1: reduce_kernel<2, 1><<<grid, kThreadsStream, 0, st>>>(d); break;
+        case 2: reduce_kernel<2, 2><<<grid, kThreadsStream, 0, st>>>(d); break;
+        default: reduce_kernel<3, 1><<<grid, kThreadsStream, 0, st>>>(d); break;
+    }
+}
+
+// Blocks per image for a streaming kernel that keeps `occ` blocks resident per SM: the smallest whole number
+// of waves w for which floor(w * slots / M) blocks per image fill >= 95 % of the w * slots block slots
+// (M = S - 2 images), never more than one block per tile.
+static int blocks_per_image(int tiles, int images, int slots) {
+    if (images < 1) return 1;
+    int best = 1;
+    double best_fill = 0.0;
+    for (int w = 1; w <= 8; ++w) {
+        int b = (w * slots) / images;
+        if (b < 1) continue;
+        if (b >= tiles) return tiles;
+        const double fill = (double)b * images / ((double)w * slots);
+        if (fill > best_fill + 1e-9) { best_fill = fill; best = b; }
+        if (fill >= 0.95) break;
+    }
+    return best < tiles ? best : tiles;
+}
+
+int update_blocks_per_sm(int variant);  // kernels_update.cu
+
+void plan_stream_grids(Dev &d) {
+    int dev = 0, sms = 148, occ_r = 3, occ_u = 2;
+    if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    const char *e4 = getenv("CFNEB_K4_VARIANT"), *e6 = getenv("CFNEB_K6_VARIANT");
+    d.k4_variant = e4 ? atoi(e4) : 1;  // measured on B200 at c4: <2,1> 5.50 TB/s, <3,1> 4.94 (spills), <2,2> 4.83
+    d.k6_variant = e6 ? atoi(e6) : 0;
+    occ_r = d.k4_variant == 0 ? 3 : 2;
+    occ_u = update_blocks_per_sm(d.k6_variant);
+    if (getenv("CFNEB_K4_OCC")) occ_r = atoi(getenv("CFNEB_K4_OCC"));
+    if (getenv("CFNEB_K6_OCC")) occ_u = atoi(getenv("CFNEB_K6_OCC"));
+    d.nblk_red = blocks_per_image(d.nblk_stream, d.S - 2, sms * occ_r);
+    d.nblk_upd = blocks_per_image(d.nblk_stream, d.S - 2, sms * occ_u);
 }
 
 void launch_finalize(const Dev &d, int p_lo, cudaStream_t st) {

@@ -8,11 +8,13 @@ namespace cfn {
 __device__ inline double2 ld2(const double *p) { return *reinterpret_cast<const double2 *>(p); }
 __device__ inline void st2(double *p, double2 v) { *reinterpret_cast<double2 *>(p) = v; }
 
-// grid (nblk_stream, S-2), 256 threads, two atoms per thread.
+// grid (nblk_upd, S-2), 256 threads, two atoms per thread and tile; block b of an image takes the 512-atom tiles
+// b, b + nblk_upd, ... (same tiling as K4, see reduce_kernel).
 //   f = F D^T + c1 tau+ + c2 tau-          (c1, c2 from K5: perpendicular projection + spring / climbing)
 //   v_new = cv v + cf f ;  X_new = X + sdt v_new     (cv, cf, sdt from K5: FIRE mixing, dt, step clip)
 // Also: max row norm of f (fmax, O8) and max |dR~_i|^2 of this image (neighbour-list skin test of K0).
-__global__ void __launch_bounds__(kThreadsStream) update_kernel(Dev d) {
+template <int MINB>
+__global__ void __launch_bounds__(kThreadsStream, MINB) update_kernel(Dev d) {
     const int p = blockIdx.y + 1;
     const Ctl *ctl = d.ctl;
     if (p > ctl->P - 2) return;
@@ -29,9 +31,10 @@ __global__ void __launch_bounds__(kThreadsStream) update_kernel(Dev d) {
     const double *Xm = Xs + sm * img, *X0 = Xs + s0 * img, *Xp = Xs + sp * img;
     const double *F = d.F + s0 * img;
     double *V = d.v + s0 * img;
-    const int i = 2 * (blockIdx.x * kThreadsStream + threadIdx.x);
-    double f2max = 0.0, d2max = 0.0;
-    if (i < d.Npad) {
+    double f2max = 0.0, v2max = 0.0;
+    for (int tile = blockIdx.x; tile < d.nblk_stream; tile += gridDim.x) {
+        const int i = 2 * (tile * kThreadsStream + threadIdx.x);
+        if (i >= d.Npad) continue;
         double2 f[3], xm[3], x0[3], xp[3], vv[3];
 #pragma unroll
         for (int c = 0; c < 3; ++c) {
@@ -60,9 +63,10 @@ __global__ void __launch_bounds__(kThreadsStream) update_kernel(Dev d) {
             f2x += fx * fx; f2y += fy * fy;
             v2x += vn.x * vn.x; v2y += vn.y * vn.y;
         }
-        f2max = fmax(f2x, f2y);
-        d2max = sdt * sdt * fmax(v2x, v2y);
+        f2max = fmax(f2max, fmax(f2x, f2y));
+        v2max = fmax(v2max, fmax(v2x, v2y));
     }
+    const double d2max = sdt * sdt * v2max;
     // cell block (three rows of the generalized vector): block 0, thread 0 of every image
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         const double *Xcs = d.Xc + (size_t)ctl->src * d.S * 9;
@@ -262,9 +266,12 @@ __global__ void export_forces_kernel(Dev d, double *Fo, double *Vo, double *Eo) 
 
 void launch_update(const Dev &d, cudaStream_t st) {
     if (d.S < 3) return;
-    dim3 grid(d.nblk_stream, d.S - 2);
-    update_kernel<<<grid, kThreadsStream, 0, st>>>(d);
+    dim3 grid(d.nblk_upd, d.S - 2);
+    if (d.k6_variant == 1) update_kernel<2><<<grid, kThreadsStream, 0, st>>>(d);
+    else update_kernel<3><<<grid, kThreadsStream, 0, st>>>(d);
 }
+
+int update_blocks_per_sm(int variant) { return variant == 1 ? 2 : 3; }
 
 void launch_materialize_fneb(const Dev &d, cudaStream_t st) {
     dim3 grid((d.N + 3 + 127) / 128, d.S);
