@@ -86,6 +86,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.Rc = c.take<double4>(S * Npad);
     d.Sw = c.take<double4>(S * Npad);
     d.binned = c.take<double4>(S * Npad);
+    d.binned_c = c.take<float4>(S * Npad);
     d.Xc = c.take<double>(2 * S * 9);
     d.vc = c.take<double>(S * 9);
     d.E = c.take<double>(S);
@@ -97,9 +98,9 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.part_dots = c.take<double>(S * d.nblk_stream * kNDots);
     d.dispmax = c.take<unsigned long long>(S);
     d.nbr_count = c.take<int>(S * Npad);
-    d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad);
-    d.nbr_in = c.take<uint32_t>(S * (size_t)d.cap * Npad);
-    d.nbr_in_count = c.take<int>(S * Npad);
+    d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 8 * Npad);  // 8 rows of slack for the force kernels' look-ahead
+    d.nbr_tmp = c.take<uint32_t>(S * (size_t)d.cap * Npad);
+    d.nbr_bkt = c.take<unsigned char>(S * (size_t)d.cap * Npad);
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
     d.bin_members = c.take<int>(S * Npad);

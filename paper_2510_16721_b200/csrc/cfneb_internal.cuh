@@ -84,6 +84,7 @@ struct Dev {
     double4 *Rc;
     double4 *Sw;              // [S][Npad] wrapped fractional coordinates + packed floors, for the list build
     double4 *binned;          // [S][Npad] Sw in bin order, .w = packed (atom index, floors)
+    float4 *binned_c;         // [S][Npad] fp32 Cartesian wrapped positions in bin order (prefilter of the search)
     double *Xc, *vc;
     double *E, *V, *Gc;       // [S], [S][9], [S][9]
     double *dots, *coef;      // [S][10], [S][4]
@@ -91,10 +92,9 @@ struct Dev {
     double *part_dots;        // [S][nblk_stream][10]  (the first nblk_red rows of an image are used)
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
     int *nbr_count;           // [S][Npad]
-    uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), rebuilt when stale
-    uint32_t *nbr_in;         // [S][cap][Npad]  in-range list of the current step: plain entries from k = 0 up,
-                              //                 taper-zone entries from k = cap-1 down (written by K2a every step)
-    int *nbr_in_count;        // [S][Npad]       n_plain | n_taper << 16
+    uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
+    uint32_t *nbr_tmp;        // [S][cap][Npad]  unsorted list of a rebuild (scratch of K1)
+    unsigned char *nbr_bkt;   // [S][cap][Npad]  r^2 bucket of each unsorted entry (scratch of K1)
     int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
     int *bin_cursor;          // [S][nbins_max]
     int *bin_members;         // [S][Npad]

@@ -13,24 +13,25 @@
 //                     (two passes: densities, then forces; F'(rho_i) rides in Rc[i].w so that the second
 //                     pass gathers position and F'(rho_j) from the same 32-byte sector).
 //
-// One thread per atom, full neighbour lists, no fp64 atomics.  The first form of this kernel walked the Verlet
-// list (r < r_cut + skin) entry by entry with `if (r < r_cut)` and `if (r > r_on)` inside the loop; ncu
-// (profiles/r1a) showed 61 % lane utilisation and the fp64 pipe 35 % busy: in a warp of 32 different atoms some
-// lane is always in the taper zone and some lane always out of range, so every lane paid for every path, and
-// the gather latency sat on the critical path of a long dependent fp64 chain.  Now each thread runs two
-// phases over a private shared-memory queue (64 entries, [k][thread] so bank = lane):
-//   phase A  stream the list 4 entries at a time (coalesced k-major list read, one 256-bit gather of the
-//            neighbour's position sector each, r^2 only) and push the entries inside r_cut onto the queue --
-//            plain ones (r <= r_on) from the front, taper-zone ones from the back;
-//   phase B  when a queue in the warp is about to fill (or the list ends) evaluate the queue: the plain loop
-//            carries no taper arithmetic, the taper loop no branch, two pairs per thread are in flight, and
-//            the math (rsqrt, exp) is branch-free with constant-bank coefficients.
+// One thread per atom, full neighbour lists, no fp64 atomics.  History (ncu evidence under profiles/):
+//   r1a  entry-by-entry walk of the Verlet list with `if (r < r_cut)`, `if (r > r_on)` per lane: 61 % lane
+//        utilisation, fp64 pipe 35 % busy (every lane paid for every path).
+//   r1b  a per-step compaction pass (K2a) wrote an in-range list split plain / taper, K2b walked it: force pass
+//        fp64 pipe 61 %, but the compaction pass cost more than the force pass (10.4 ms vs 8.1 ms at c4: 80
+//        non-fp64 instructions per list entry, 9 GB of list traffic, gathers stalled on a 37 % L1 hit rate).
+//   r1c  (this file) the Verlet list is sorted by distance when it is built (kernels_neighbor.cu), so in a solid
+//        the k-th entry of all 32 atoms of a warp lies in the same neighbour shell and the per-entry decisions are
+//        warp-uniform nearly always.  Both passes are now one plain loop, two entries per iteration, with three
+//        warp-level cases: nobody in range -> skip; nobody in the taper zone -> plain formula; otherwise the
+//        general formula (taper with t = 1 selected for r <= r_on).  Lanes that disagree are masked, never
+//        branched.  List entries are fetched two iterations ahead and the neighbour sectors one iteration ahead,
+//        so gather latency is off the dependent fp64 chain; the math (rsqrt, exp) is branch-free with
+//        constant-bank coefficients.
 // Per-thread sums run in list order and block partials through a fixed tree: bitwise repeatable.
 #include "cfneb_internal.cuh"
 
 namespace cfn {
 
-constexpr int kQ = 32;  // queued r^2 values per thread (32 KB of shared memory per 128-thread block)
 constexpr unsigned kFull = 0xffffffffu;
 
 __device__ __forceinline__ double4 ld256(const double4 *p) {  // one LDG.E.256 instead of two LDG.E.128
@@ -67,6 +68,8 @@ __device__ __forceinline__ double rsqrt_nr(double x) {
 
 // exp(x) for |x| < 700 (pair arguments are O(1)): x = k ln2 + r, degree-13 Taylor polynomial on |r| <= ln2/2
 // (remainder 4e-18), 2^k by exponent arithmetic.  No under/overflow branches; coefficients from the constant bank.
+// (Horner on purpose: an Estrin form with dependent depth 6 instead of 13 measured 3 % slower at c4 -- the kernel
+// is bound by issue slots, every fp64 instruction holding its scheduler for two cycles, not by chain latency.)
 __constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
                                  1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
 __device__ __forceinline__ double exp_nb(double x) {
@@ -93,7 +96,7 @@ __device__ __forceinline__ void add_pair(Acc &a, double s, double u, double dx, 
 }
 
 struct LJc { double eps4, sig2, rc, phi_c, dphi_c; };
-struct FSc { double Dm, a, r0, beta, rr0, A, r_on, inv_w, pi_w; };
+struct FSc { double Dm, a, r0, beta, rr0, A, r_on, inv_w, pi_w, k3; };
 
 // LJ shifted-force pair: fmag / r and the half pair energy
 __device__ __forceinline__ void lj_pair(const LJc &c, double r2, double &s, double &u) {
@@ -104,18 +107,20 @@ __device__ __forceinline__ void lj_pair(const LJc &c, double r2, double &s, doub
 }
 
 // FS force pair (second pass).  TAPER = false: r <= r_on, t = 1, t' = 0.
-template <bool TAPER>
+// SHARE: beta == 2 alpha, so e^{-beta (r - rho_r0)} = e^{beta (rho_r0 - r0)} (e^{-alpha (r - r0)})^2 and the second
+// exponential is one multiplication (k3 is that constant factor, computed once per thread).
+template <bool TAPER, bool SHARE>
 __device__ __forceinline__ void fs_pair(const FSc &c, double r2, double dF_sum, double &s, double &u) {
     const double rinv = rsqrt_nr(r2), r = r2 * rinv;
     const double e1 = exp_nb(-c.a * (r - c.r0)), e2 = e1 * e1;
     const double m = c.Dm * (e2 - 2.0 * e1), dm = 2.0 * c.a * c.Dm * (e1 - e2);
-    const double e3 = exp_nb(-c.beta * (r - c.rr0));
+    const double e3 = SHARE ? c.k3 * e2 : exp_nb(-c.beta * (r - c.rr0));
     double fmag;
     if (TAPER) {
         double sn, cs;
         sincospi((r - c.r_on) * c.inv_w, &sn, &cs);
         double t = 0.5 * (1.0 + cs), dt = -0.5 * sn * c.pi_w;
-        if (r <= c.r_on) { t = 1.0; dt = 0.0; }  // the queues are split on r^2; keep the definition exact at the edge
+        if (r <= c.r_on) { t = 1.0; dt = 0.0; }  // lanes outside the taper zone on the general path
         u = 0.5 * (m * t);
         fmag = dm * t + m * dt + dF_sum * (e3 * (dt - c.beta * t));
     } else {
@@ -150,6 +155,7 @@ struct PotC {
         if (POT == CFNEB_POT_FS_MORSE) {
             fs.Dm = d.pot[0]; fs.a = d.pot[1]; fs.r0 = d.pot[2]; fs.beta = d.pot[3]; fs.rr0 = d.pot[4]; fs.A = d.pot[5];
             fs.r_on = d.pot[6]; fs.inv_w = 1.0 / (d.pot[7] - d.pot[6]); fs.pi_w = 3.14159265358979323846 * fs.inv_w;
+            fs.k3 = exp(fs.beta * (fs.rr0 - fs.r0));
             ron2 = fs.r_on * fs.r_on;
         } else {
             lj.eps4 = 4.0 * d.pot[0]; lj.sig2 = d.pot[1] * d.pot[1]; lj.rc = d.pot[2];
@@ -160,17 +166,45 @@ struct PotC {
     }
 };
 
-// K2a: classify the Verlet list of every atom into the in-range list of this step (plain entries from the
-// front, taper-zone entries from the back of the atom's column of nbr_in) and, for FS, accumulate the density
-// rho_i: plain r^2 values go through the shared-memory queue and are evaluated densely, the taper entries at the
-// end.  Writes F'(rho_i) into Rc[i].w and the per-block embedding energy.
-template <int POT>
-__global__ void __launch_bounds__(kThreadsAtom, 4) classify_kernel(Dev d, int p_lo) {
+// Walks the (distance-sorted) Verlet column of one atom two entries per iteration: body(k, code0, code1, rj0, rj1)
+// sees entries k, k + 1 (shift codes and the neighbours' 32-byte sectors).  Entries are fetched two iterations
+// and sectors one iteration ahead of use; the loop is unrolled over the two pipeline stages so that no register
+// is rotated.  Rows past an atom's count hold a stand-in entry that is out of range by construction
+// (kernels_neighbor.cu), and the list carries 8 rows of slack, so no load is predicated.
+template <class Body>
+__device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_t stride, const double4 *Rc, int cnt_w,
+                                          Body body) {
+    uint32_t a0 = lp[0], a1 = lp[stride], b0 = lp[2 * stride], b1 = lp[3 * stride];
+    double4 sa0 = ld256(Rc + (a0 & kIdxMask)), sa1 = ld256(Rc + (a1 & kIdxMask)), sb0, sb1;
+    lp += 4 * stride;
+    for (int k = 0; k < cnt_w; k += 4) {
+        sb0 = ld256(Rc + (b0 & kIdxMask));
+        sb1 = ld256(Rc + (b1 & kIdxMask));
+        {
+            const uint32_t c0 = a0 >> kShiftBits, c1 = a1 >> kShiftBits;
+            a0 = lp[0];
+            a1 = lp[stride];
+            body(k, c0, c1, sa0, sa1);
+        }
+        if (k + 2 >= cnt_w) break;
+        sa0 = ld256(Rc + (a0 & kIdxMask));
+        sa1 = ld256(Rc + (a1 & kIdxMask));
+        {
+            const uint32_t c0 = b0 >> kShiftBits, c1 = b1 >> kShiftBits;
+            b0 = lp[2 * stride];
+            b1 = lp[3 * stride];
+            body(k + 2, c0, c1, sb0, sb1);
+        }
+        lp += 4 * stride;
+    }
+}
+
+// K2a (FS only): densities rho_i = sum_j psi(r_ij) over the Verlet list; writes F'(rho_i) into Rc[i].w and the
+// per-block embedding energy.
+__global__ void __launch_bounds__(kThreadsAtom, 4) density_kernel(Dev d, int p_lo) {
     const int p = blockIdx.y + p_lo;
     if (p > d.ctl->P - 1 - p_lo) return;
     const int slot = d.order[p];
-    constexpr bool FS = POT == CFNEB_POT_FS_MORSE;
-    __shared__ double s_q[FS ? kQ * kThreadsAtom : 1];
     __shared__ double sh[9];
     __shared__ double red[32];
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
@@ -178,81 +212,38 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) classify_kernel(Dev d, int p_
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
     double4 *Rc = d.Rc + (size_t)slot * d.Npad;
-    const size_t col = (size_t)slot * d.cap * d.Npad + i;
-    const uint32_t *lp = d.nbr_list + col;
-    uint32_t *ip = d.nbr_in + col;
-    double *q = s_q + threadIdx.x;  // entry c of this thread at q[c * kThreadsAtom]
-    PotC<POT> pc;
+    PotC<CFNEB_POT_FS_MORSE> pc;
     pc.load(d);
 
-    double4 ri = make_double4(0.0, 0.0, 0.0, 0.0);
+    // idle lanes sit far away from everything (every r^2 ~ 1e60: out of range, finite) and walk the last column
+    double4 ri = make_double4(1e30, 1e30, 1e30, 0.0);
     int cnt = 0;
     if (valid) {
         ri = ld256(Rc + i);
         cnt = d.nbr_count[(size_t)slot * d.Npad + i];
     }
-    const uint32_t self = (uint32_t)(valid ? i : 0) | (kCodeCenter << kShiftBits);  // stand-in entry of idle lanes
-    const int cnt_w = __reduce_max_sync(kFull, cnt);
-    const int last = d.cap - 1;
+    const int cnt_w = min(__reduce_max_sync(kFull, cnt), d.cap);
+    const int cap = d.cap;
     double rho = 0.0;
-    int n_pl = 0, n_tp = 0, n_q = 0;
-
-    // The list entries of iteration k+1 are loaded before the gathers of iteration k are consumed, so the
-    // (DRAM-streamed) list read never sits on the critical path.
-    uint32_t en[4];
-#pragma unroll
-    for (int u = 0; u < 4; ++u) en[u] = (u < cnt) ? lp[(size_t)u * d.Npad] : self;
-    int k = 0;
-    while (k < cnt_w) {
-        do {  // phase A: four list entries in flight
-            uint32_t e[4];
-            double4 rj[4];
-#pragma unroll
-            for (int u = 0; u < 4; ++u) { e[u] = en[u]; rj[u] = ld256(Rc + (e[u] & kIdxMask)); }
-#pragma unroll
-            for (int u = 0; u < 4; ++u) en[u] = (k + 4 + u < cnt) ? lp[(size_t)(k + 4 + u) * d.Npad] : self;
-#pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                double dx, dy, dz, r2;
-                pair_vec(ri, rj[u], e[u] >> kShiftBits, sh, dx, dy, dz, r2);
-                const bool in = (k + u < cnt) && r2 < pc.rc2;
-                const bool tp = FS && in && r2 > pc.ron2;
-                if (in && !tp) {
-                    ip[(size_t)n_pl * d.Npad] = e[u];
-                    ++n_pl;
-                    if (FS) { q[n_q * kThreadsAtom] = r2; ++n_q; }
-                }
-                if (tp) { ip[(size_t)(last - n_tp) * d.Npad] = e[u]; ++n_tp; }
-            }
-            k += 4;
-        } while (k < cnt_w && !(FS && __any_sync(kFull, n_q > kQ - 4)));
-        if (FS) {  // phase B: dense evaluation of the queued r^2, two pairs in flight
-            const int nq_w = __reduce_max_sync(kFull, n_q);
-            for (int c = 0; c < nq_w; c += 2) {
-                const bool a0 = c < n_q, a1 = c + 1 < n_q;
-                const double r20 = a0 ? q[c * kThreadsAtom] : 1.0, r21 = a1 ? q[(c + 1) * kThreadsAtom] : 1.0;
-                const double p0 = fs_density<false>(pc.fs, r20), p1 = fs_density<false>(pc.fs, r21);
-                rho += a0 ? p0 : 0.0;
-                rho += a1 ? p1 : 0.0;
-            }
-            n_q = 0;
+    walk_list(d.nbr_list + (size_t)slot * d.cap * d.Npad + min(i, d.Npad - 1), d.Npad, Rc, cnt_w,
+              [&](int k, uint32_t c0, uint32_t c1, const double4 &rj0, const double4 &rj1) {
+        double dx, dy, dz, r20, r21;
+        pair_vec(ri, rj0, c0, sh, dx, dy, dz, r20);
+        pair_vec(ri, rj1, c1, sh, dx, dy, dz, r21);
+        const bool in0 = r20 < pc.rc2, in1 = r21 < pc.rc2 && k + 1 < cap;
+        if (!__any_sync(kFull, in0 || in1)) return;
+        const bool tp = (in0 && r20 > pc.ron2) || (in1 && r21 > pc.ron2);
+        double p0, p1;
+        if (!__any_sync(kFull, tp)) {
+            p0 = fs_density<false>(pc.fs, r20);
+            p1 = fs_density<false>(pc.fs, r21);
+        } else {
+            p0 = fs_density<true>(pc.fs, r20);
+            p1 = fs_density<true>(pc.fs, r21);
         }
-    }
-    if (valid) d.nbr_in_count[(size_t)slot * d.Npad + i] = n_pl | (n_tp << 16);
-    if (!FS) return;
-
-    const int ntp_w = __reduce_max_sync(kFull, n_tp);
-    uint32_t et = (0 < n_tp) ? ip[(size_t)last * d.Npad] : self;
-    for (int c = 0; c < ntp_w; ++c) {  // taper-zone entries, read back from this thread's own column
-        const bool a0 = c < n_tp;
-        const uint32_t e0 = et;
-        const double4 rj0 = ld256(Rc + (e0 & kIdxMask));
-        et = (c + 1 < n_tp) ? ip[(size_t)(last - c - 1) * d.Npad] : self;
-        double dx, dy, dz, r2;
-        pair_vec(ri, rj0, e0 >> kShiftBits, sh, dx, dy, dz, r2);
-        const double p0 = fs_density<true>(pc.fs, a0 ? r2 : 1.0);
-        rho += a0 ? p0 : 0.0;
-    }
+        if (in0) rho += p0;
+        if (in1) rho += p1;
+    });
     double emb[1] = {0.0};
     if (valid) {
         double dF = 0.0;
@@ -267,9 +258,8 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) classify_kernel(Dev d, int p_
     if (threadIdx.x == 0) d.part_force[((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart + 7] = emb[0];
 }
 
-// K2b: forces, energies and the virial over the in-range list of K2a.  No shared-memory queue, so the whole
-// L1 serves the position gathers; two pairs per thread in flight; the taper loop runs last.
-template <int POT>
+// K2b: forces, energies and the virial over the Verlet list.
+template <int POT, bool SHARE>
 __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo) {
     const int p = blockIdx.y + p_lo;
     if (p > d.ctl->P - 1 - p_lo) return;
@@ -282,59 +272,41 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo)
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
     const double4 *Rc = d.Rc + (size_t)slot * d.Npad;
-    const uint32_t *ip = d.nbr_in + (size_t)slot * d.cap * d.Npad + i;
     PotC<POT> pc;
     pc.load(d);
 
-    double4 ri = make_double4(0.0, 0.0, 0.0, 0.0);
-    int n_pl = 0, n_tp = 0;
+    double4 ri = make_double4(1e30, 1e30, 1e30, 0.0);  // idle lanes: see density_kernel
+    int cnt = 0;
     if (valid) {
         ri = ld256(Rc + i);
-        const int c = d.nbr_in_count[(size_t)slot * d.Npad + i];
-        n_pl = c & 0xffff;
-        n_tp = c >> 16;
+        cnt = d.nbr_count[(size_t)slot * d.Npad + i];
     }
-    const uint32_t self = (uint32_t)(valid ? i : 0) | (kCodeCenter << kShiftBits);
-    const int last = d.cap - 1;
+    const int cnt_w = min(__reduce_max_sync(kFull, cnt), d.cap);
+    const int cap = d.cap;
     Acc acc = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
-
-    const int npl_w = __reduce_max_sync(kFull, n_pl);
-    uint32_t en0 = (0 < n_pl) ? ip[0] : self, en1 = (1 < n_pl) ? ip[d.Npad] : self;  // entries one iteration ahead
-    for (int c = 0; c < npl_w; c += 2) {
-        const bool a0 = c < n_pl, a1 = c + 1 < n_pl;
-        const uint32_t e0 = en0, e1 = en1;
-        const double4 rj0 = ld256(Rc + (e0 & kIdxMask)), rj1 = ld256(Rc + (e1 & kIdxMask));
-        en0 = (c + 2 < n_pl) ? ip[(size_t)(c + 2) * d.Npad] : self;
-        en1 = (c + 3 < n_pl) ? ip[(size_t)(c + 3) * d.Npad] : self;
+    walk_list(d.nbr_list + (size_t)slot * d.cap * d.Npad + min(i, d.Npad - 1), d.Npad, Rc, cnt_w,
+              [&](int k, uint32_t c0, uint32_t c1, const double4 &rj0, const double4 &rj1) {
         double dx0, dy0, dz0, r20, dx1, dy1, dz1, r21, s0, u0, s1, u1;
-        pair_vec(ri, rj0, e0 >> kShiftBits, sh, dx0, dy0, dz0, r20);
-        pair_vec(ri, rj1, e1 >> kShiftBits, sh, dx1, dy1, dz1, r21);
-        r20 = a0 ? r20 : 1.0;
-        r21 = a1 ? r21 : 1.0;
+        pair_vec(ri, rj0, c0, sh, dx0, dy0, dz0, r20);
+        pair_vec(ri, rj1, c1, sh, dx1, dy1, dz1, r21);
+        const bool in0 = r20 < pc.rc2, in1 = r21 < pc.rc2 && k + 1 < cap;
+        if (!__any_sync(kFull, in0 || in1)) return;
+        const bool tp = FS && ((in0 && r20 > pc.ron2) || (in1 && r21 > pc.ron2));
         if (FS) {
-            fs_pair<false>(pc.fs, r20, ri.w + rj0.w, s0, u0);
-            fs_pair<false>(pc.fs, r21, ri.w + rj1.w, s1, u1);
+            if (!__any_sync(kFull, tp)) {
+                fs_pair<false, SHARE>(pc.fs, r20, ri.w + rj0.w, s0, u0);
+                fs_pair<false, SHARE>(pc.fs, r21, ri.w + rj1.w, s1, u1);
+            } else {
+                fs_pair<true, SHARE>(pc.fs, r20, ri.w + rj0.w, s0, u0);
+                fs_pair<true, SHARE>(pc.fs, r21, ri.w + rj1.w, s1, u1);
+            }
         } else {
             lj_pair(pc.lj, r20, s0, u0);
             lj_pair(pc.lj, r21, s1, u1);
         }
-        add_pair(acc, a0 ? s0 : 0.0, a0 ? u0 : 0.0, dx0, dy0, dz0);
-        add_pair(acc, a1 ? s1 : 0.0, a1 ? u1 : 0.0, dx1, dy1, dz1);
-    }
-    if (FS) {
-        const int ntp_w = __reduce_max_sync(kFull, n_tp);
-        uint32_t et = (0 < n_tp) ? ip[(size_t)last * d.Npad] : self;
-        for (int c = 0; c < ntp_w; ++c) {
-            const bool a0 = c < n_tp;
-            const uint32_t e0 = et;
-            const double4 rj0 = ld256(Rc + (e0 & kIdxMask));
-            et = (c + 1 < n_tp) ? ip[(size_t)(last - c - 1) * d.Npad] : self;
-            double dx0, dy0, dz0, r20, s0, u0;
-            pair_vec(ri, rj0, e0 >> kShiftBits, sh, dx0, dy0, dz0, r20);
-            fs_pair<true>(pc.fs, a0 ? r20 : 1.0, ri.w + rj0.w, s0, u0);
-            add_pair(acc, a0 ? s0 : 0.0, a0 ? u0 : 0.0, dx0, dy0, dz0);
-        }
-    }
+        if (in0) add_pair(acc, s0, u0, dx0, dy0, dz0);
+        if (in1) add_pair(acc, s1, u1, dx1, dy1, dz1);
+    });
     if (valid) {
         double *F = d.F + (size_t)slot * 3 * d.Npad;
         F[i] = acc.fx;
@@ -356,11 +328,11 @@ void launch_force(const Dev &d, int p_lo, cudaStream_t st) {
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
     if (d.potential == CFNEB_POT_LJ_SF) {
-        classify_kernel<CFNEB_POT_LJ_SF><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
-        force_kernel<CFNEB_POT_LJ_SF><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+        force_kernel<CFNEB_POT_LJ_SF, false><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
     } else {
-        classify_kernel<CFNEB_POT_FS_MORSE><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
-        force_kernel<CFNEB_POT_FS_MORSE><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+        density_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+        if (d.pot[3] == 2.0 * d.pot[1]) force_kernel<CFNEB_POT_FS_MORSE, true><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+        else force_kernel<CFNEB_POT_FS_MORSE, false><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
     }
 }
 

@@ -10,6 +10,11 @@
 //
 // Determinism: bins are filled with atomics, then each bin is sorted by atom index, so list order (and with
 // it the summation order of the force kernel) is a function of the coordinates only.
+//
+// Radial order: each atom's list is stored sorted by distance at build time (stable counting sort on 64 buckets
+// of r^2).  In a solid the k-th nearest neighbour of every atom of a warp then lies in the same shell, so the
+// force kernels' per-entry decisions (inside r_cut? inside the taper zone?) are nearly warp-uniform and are
+// taken as warp-level branches with no per-step compaction pass.
 #include "cfneb_internal.cuh"
 
 namespace cfn {
@@ -80,12 +85,17 @@ __global__ void __launch_bounds__(128) bin_sort_kernel(Dev d, int p_lo) {
     }
     const double4 *Sw = d.Sw + (size_t)slot * d.Npad;
     double4 *out = d.binned + (size_t)slot * d.Npad;
+    float4 *outc = d.binned_c + (size_t)slot * d.Npad;
     for (int q = lo; q < hi; ++q) {
         const int i = mem[q];
         double4 w = Sw[i];
         unsigned long long fl = (unsigned long long)__double_as_longlong(w.w);
         w.w = __longlong_as_double((long long)((unsigned long long)i | (fl << kShiftBits)));
         out[q] = w;
+        // fp32 Cartesian copy of the wrapped position for the search's prefilter
+        outc[q] = make_float4((float)(w.x * g->h[0] + w.y * g->h[3] + w.z * g->h[6]),
+                              (float)(w.x * g->h[1] + w.y * g->h[4] + w.z * g->h[7]),
+                              (float)(w.x * g->h[2] + w.y * g->h[5] + w.z * g->h[8]), 0.f);
     }
 }
 
@@ -100,14 +110,25 @@ __device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
     }
 }
 
-// One thread per atom: scan the stencil bins, test |ds h|^2 < r_list^2, append (j | code << 23) k-major.
+// One thread per atom: scan the stencil bins four candidates at a time (the four fp32 loads are independent, so
+// the scan is not a chain of dependent L2 latencies), prefilter on fp32 Cartesian coordinates, decide membership
+// by the exact fp64 test |ds h|^2 < r_list^2, append (j | code << 23) k-major to the atom's column of nbr_tmp
+// with its r^2 bucket, then counting-sort the column into nbr_list (histogram kept in shared memory during the
+// scan).  Rows cnt..cap-1 of the column are filled with a stand-in entry (the atom itself shifted by -4 cell
+// vectors along axis 0: farther than r_list whenever a list can be built at all), so the force kernels read
+// any row below cap without a bounds test and find it out of range.
+constexpr int kRadialBuckets = 64;
+constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, int p_lo) {
     int slot;
     if (!image_active(d, p_lo, blockIdx.y, slot)) return;
+    __shared__ unsigned short s_hist[kRadialBuckets * kThreadsAtom];
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
     int cnt = 0;
     bool bad_shift = false;
+    unsigned short *hist = s_hist + threadIdx.x;
+    for (int b = 0; b < kRadialBuckets; ++b) hist[b * kThreadsAtom] = 0;
     if (valid) {
     const Geom *g = d.geom + slot;
     const int nb0 = g->nb[0], nb1 = g->nb[1], nb2 = g->nb[2];
@@ -120,10 +141,23 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
     const int fi0 = (int)(fli & 1023u), fi1 = (int)((fli >> 10) & 1023u), fi2 = (int)((fli >> 20) & 1023u);
     const int bin = d.atom_bin[(size_t)slot * d.Npad + i];
     const int bi0 = bin / (nb1 * nb2), bi1 = (bin / nb2) % nb1, bi2 = bin % nb2;
-    const int *bc = d.bin_count + (size_t)slot * (d.nbins_max + 1);
-    const double4 *binned = d.binned + (size_t)slot * d.Npad;
-    uint32_t *list = d.nbr_list + (size_t)slot * d.cap * d.Npad + i;
-    const double rl2 = d.r_list * d.r_list;
+    const int *__restrict__ bc = d.bin_count + (size_t)slot * (d.nbins_max + 1);
+    const double4 *__restrict__ binned = d.binned + (size_t)slot * d.Npad;
+    const float4 *__restrict__ binned_c = d.binned_c + (size_t)slot * d.Npad;
+    // fp32 prefilter: candidates are first tested on fp32 Cartesian coordinates against r_list + margin, the margin
+    // covering the rounding of coordinates of magnitude <= L = the cell's largest extent including the shifts
+    // (fp32 eps 1.2e-7; 64 eps L is >10x the worst case of the 3 subtractions and 3 products).  Only those that
+    // pass (about one in six) take the exact fp64 test below, which alone decides membership.
+    const float cix = (float)(si.x * h[0] + si.y * h[3] + si.z * h[6]), ciy = (float)(si.x * h[1] + si.y * h[4] + si.z * h[7]),
+                ciz = (float)(si.x * h[2] + si.y * h[5] + si.z * h[8]);
+    double Lext = 0.0;
+    for (int k = 0; k < 9; ++k) Lext += fabs(h[k]);
+    const float rlf = (float)(d.r_list + 64.0 * 1.2e-7 * 2.0 * Lext * (1.0 + max(re0, max(re1, re2))));
+    const float rl2f = rlf * rlf;
+    uint32_t *__restrict__ list = d.nbr_list + (size_t)slot * d.cap * d.Npad + i;
+    uint32_t *__restrict__ tmp = d.nbr_tmp + (size_t)slot * d.cap * d.Npad + i;
+    unsigned char *__restrict__ bkt = d.nbr_bkt + (size_t)slot * d.cap * d.Npad + i;
+    const double rl2 = d.r_list * d.r_list, bscale = (double)kRadialBuckets / rl2;
     for (int d0 = -re0; d0 <= re0; ++d0) {
         int bj0, m0;
         stencil_axis(nb0, bi0, d0, bj0, m0);
@@ -135,34 +169,84 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
                 stencil_axis(nb2, bi2, d2, bj2, m2);
                 const int b = (bj0 * nb1 + bj1) * nb2 + bj2;
                 const int lo = bc[b], hi = bc[b + 1];
-                for (int q = lo; q < hi; ++q) {
-                    const double4 c = binned[q];
-                    const double s0 = c.x - si.x + (double)m0, s1 = c.y - si.y + (double)m1, s2 = c.z - si.z + (double)m2;
-                    const double rx = s0 * h[0] + s1 * h[3] + s2 * h[6];
-                    const double ry = s0 * h[1] + s1 * h[4] + s2 * h[7];
-                    const double rz = s0 * h[2] + s1 * h[5] + s2 * h[8];
-                    const double r2 = rx * rx + ry * ry + rz * rz;
-                    if (r2 < rl2) {
-                        const unsigned long long pk = (unsigned long long)__double_as_longlong(c.w);
-                        const int j = (int)(pk & kIdxMask);
-                        const int n0 = m0 - (int)((pk >> kShiftBits) & 1023u) + fi0;
-                        const int n1 = m1 - (int)((pk >> (kShiftBits + 10)) & 1023u) + fi1;
-                        const int n2 = m2 - (int)((pk >> (kShiftBits + 20)) & 1023u) + fi2;
-                        if (j == i && n0 == 0 && n1 == 0 && n2 == 0) continue;
-                        if (cnt < d.cap) {
-                            if (n0 < -4 || n0 > 3 || n1 < -4 || n1 > 3 || n2 < -4 || n2 > 3) bad_shift = true;
-                            const uint32_t code = (uint32_t)((n0 + 4) & 7) | ((uint32_t)((n1 + 4) & 7) << 3) |
-                                                  ((uint32_t)((n2 + 4) & 7) << 6);
-                            list[(size_t)cnt * d.Npad] = (uint32_t)j | (code << kShiftBits);
+                // own position minus the periodic shift of this stencil bin, fp32
+                const float ox = cix - (float)(m0 * h[0] + m1 * h[3] + m2 * h[6]), oy = ciy - (float)(m0 * h[1] + m1 * h[4] + m2 * h[7]),
+                            oz = ciz - (float)(m0 * h[2] + m1 * h[5] + m2 * h[8]);
+                for (int q0 = lo; q0 < hi; q0 += 4) {
+                    float4 cf[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) cf[u] = binned_c[min(q0 + u, hi - 1)];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) {
+                        const int q = q0 + u;
+                        const float fx = cf[u].x - ox, fy = cf[u].y - oy, fz = cf[u].z - oz;
+                        if (q >= hi || !(fx * fx + fy * fy + fz * fz < rl2f)) continue;
+                        const double4 c = binned[q];
+                        const double s0 = c.x - si.x + (double)m0, s1 = c.y - si.y + (double)m1, s2 = c.z - si.z + (double)m2;
+                        const double rx = s0 * h[0] + s1 * h[3] + s2 * h[6];
+                        const double ry = s0 * h[1] + s1 * h[4] + s2 * h[7];
+                        const double rz = s0 * h[2] + s1 * h[5] + s2 * h[8];
+                        const double r2 = rx * rx + ry * ry + rz * rz;
+                        if (r2 < rl2) {
+                            const unsigned long long pk = (unsigned long long)__double_as_longlong(c.w);
+                            const int j = (int)(pk & kIdxMask);
+                            const int n0 = m0 - (int)((pk >> kShiftBits) & 1023u) + fi0;
+                            const int n1 = m1 - (int)((pk >> (kShiftBits + 10)) & 1023u) + fi1;
+                            const int n2 = m2 - (int)((pk >> (kShiftBits + 20)) & 1023u) + fi2;
+                            if (j == i && n0 == 0 && n1 == 0 && n2 == 0) continue;
+                            if (cnt < d.cap) {
+                                if (n0 < -4 || n0 > 3 || n1 < -4 || n1 > 3 || n2 < -4 || n2 > 3) bad_shift = true;
+                                if (n0 == -4 && n1 == 0 && n2 == 0) bad_shift = true;  // reserved for the stand-in entry
+                                const uint32_t code = (uint32_t)((n0 + 4) & 7) | ((uint32_t)((n1 + 4) & 7) << 3) |
+                                                      ((uint32_t)((n2 + 4) & 7) << 6);
+                                const int bk = min((int)(r2 * bscale), kRadialBuckets - 1);
+                                tmp[(size_t)cnt * d.Npad] = (uint32_t)j | (code << kShiftBits);
+                                bkt[(size_t)cnt * d.Npad] = (unsigned char)bk;
+                                hist[bk * kThreadsAtom] += 1;
+                            }
+                            ++cnt;
                         }
-                        ++cnt;
                     }
                 }
             }
         }
     }
-    d.nbr_count[(size_t)slot * d.Npad + i] = min(cnt, d.cap);
+    const int n = min(cnt, d.cap);
+    d.nbr_count[(size_t)slot * d.Npad + i] = n;
+    // stable counting sort by r^2 bucket: exclusive starts, then placement (scan order kept inside a bucket),
+    // four entries per round so that the global loads of a round are independent
+    int start = 0;
+    for (int b = 0; b < kRadialBuckets; ++b) {
+        const int c = hist[b * kThreadsAtom];
+        hist[b * kThreadsAtom] = (unsigned short)start;
+        start += c;
+    }
+    for (int k0 = 0; k0 < n; k0 += 4) {
+        uint32_t t[4];
+        int bk[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const size_t o = (size_t)min(k0 + u, n - 1) * d.Npad;
+            t[u] = tmp[o];
+            bk[u] = bkt[o];
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            if (k0 + u >= n) break;
+            unsigned short &cur = hist[bk[u] * kThreadsAtom];
+            list[(size_t)cur * d.Npad] = t[u];
+            cur += 1;
+        }
+    }
     }  // valid
+    {   // stand-in rows cnt..cap-1 (idle lanes of the last block included: their columns exist up to Npad)
+        const int i_pad = blockIdx.x * blockDim.x + threadIdx.x;
+        if (i_pad < d.Npad) {
+            uint32_t *col = d.nbr_list + (size_t)slot * d.cap * d.Npad + i_pad;
+            const uint32_t far = (uint32_t)(valid ? i : 0) | (kCodeFar << kShiftBits);
+            for (int k = valid ? min(cnt, d.cap) : 0; k < d.cap; ++k) col[(size_t)k * d.Npad] = far;
+        }
+    }
     if (cnt > d.cap) set_error(d.ctl, CFNEB_ENEIGH_OVERFLOW);
     if (bad_shift) set_error(d.ctl, CFNEB_ECELL);
     // block-level max, then one atomic per block
