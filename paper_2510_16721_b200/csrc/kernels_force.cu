@@ -66,21 +66,61 @@ __device__ __forceinline__ double rsqrt_nr(double x) {
     return fma(y * e, fma(0.375, e, 0.5), y);
 }
 
-// exp(x) for |x| < 700 (pair arguments are O(1)): x = k ln2 + r, degree-13 Taylor polynomial on |r| <= ln2/2
-// (remainder 4e-18), 2^k by exponent arithmetic.  No under/overflow branches; coefficients from the constant bank.
-// (Horner on purpose: an Estrin form with dependent depth 6 instead of 13 measured 3 % slower at c4 -- the kernel
-// is bound by issue slots, every fp64 instruction holding its scheduler for two cycles, not by chain latency.)
-__constant__ double kExpC[14] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
-                                 1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0};
-__device__ __forceinline__ double exp_nb(double x) {
-    const double t = fma(x, 1.4426950408889634074, 6755399441055744.0);
+// exp(x) for |x| < 700 (pair arguments are O(1)):  x = (32 k + j) ln2/32 + r,  exp(x) = 2^k T[j] e^r with
+// T[j] = 2^(j/32) from a 32-entry table in shared memory and e^r - 1 = r + r^2 (1/2 + r/6 + ... + r^4/720) on
+// |r| <= ln2/64 (remainder 3.5e-18); 2^k by exponent arithmetic.  11 fp64 instructions instead of the 17 of a
+// degree-13 polynomial on |r| <= ln2/2: the kernels are bound by issue slots, and every fp64 instruction holds
+// its scheduler for two.  Max relative error 1.9e-16 against long double over [-8, 3].  No under/overflow
+// branches (out-of-range lanes may produce garbage; they are masked, never trapped).
+__constant__ double kExp2Table[32] = {
+    1.0, 1.0218971486541166, 1.0442737824274138, 1.0671404006768237, 1.0905077326652577, 1.1143867425958924,
+    1.1387886347566916, 1.1637248587775775, 1.189207115002721, 1.215247359980469, 1.241857812073484,
+    1.2690509571917332, 1.2968395546510096, 1.3252366431597413, 1.3542555469368927, 1.383909881963832,
+    1.4142135623730951, 1.4451808069770467, 1.4768261459394993, 1.5091644275934228, 1.5422108254079407,
+    1.5759808451078865, 1.6104903319492543, 1.645755478153965, 1.681792830507429, 1.718619298122478,
+    1.7562521603732995, 1.7947090750031072, 1.8340080864093424, 1.8741676341103, 1.9152065613971474,
+    1.9571441241754002};
+__device__ __forceinline__ double exp_nb(double x, const double *T /* shared */) {
+    const double t = fma(x, 46.166241308446828384, 6755399441055744.0);  // 32/ln2; integer part lands in the low word
     const double kf = t - 6755399441055744.0;
-    double r = fma(kf, -6.93147180369123816490e-01, x);
-    r = fma(kf, -1.90821492927058770002e-10, r);
-    double p = kExpC[13];
+    double r = fma(kf, -2.16608493865351192653e-02, x);  // ln2/32 in two pieces
+    r = fma(kf, -5.96317165397058656257e-12, r);
+    const int n = __double2loint(t);
+    const double Tj = T[n & 31];
+    const double r2 = r * r;
+    const double in = fma(fma(fma(fma(1.0 / 720, r, 1.0 / 120), r, 1.0 / 24), r, 1.0 / 6), r, 0.5);
+    const double q = fma(r2, in, r);
+    const double p = fma(Tj, q, Tj);
+    return __hiloint2double(__double2hiint(p) + ((n >> 5) << 20), __double2loint(p));
+}
+
+// cos(pi x) and sin(pi x) for x in [0, 1] (the taper variable): with y = x - 1/2, cos(pi x) = -sin(pi y) and
+// sin(pi x) = cos(pi y); Taylor polynomials in y^2 to y^21 / y^22 (|pi y| <= pi/2), max abs error 3e-16 against
+// long double.  About half the instructions of sincospi (no range reduction, no quadrant logic).
+__constant__ double kSinPi[11] = {3.1415926535897931, -5.1677127800499703, 2.5501640398773455, -0.59926452932079211,
+                                  0.082145886611128233, -0.0073704309457143504, 0.00046630280576761255,
+                                  -2.1915353447830217e-05, 7.9520540014755126e-07, -2.2948428997269873e-08,
+                                  5.392664662608129e-10};
+__constant__ double kCosPi[12] = {1.0, -4.934802200544679, 4.0587121264167685, -1.3352627688545895,
+                                  0.23533063035889321, -0.025806891390014061, 0.0019295743094039231,
+                                  -0.0001046381049248457, 4.3030695870329473e-06, -1.3878952462213771e-07,
+                                  3.6047307974625011e-09, -7.7007071306013539e-11};
+__device__ __forceinline__ double cospi01(double x) {
+    const double y = x - 0.5, z = y * y;
+    double s = kSinPi[10];
 #pragma unroll
-    for (int n = 12; n >= 0; --n) p = fma(p, r, kExpC[n]);
-    return __hiloint2double(__double2hiint(p) + (__double2loint(t) << 20), __double2loint(p));
+    for (int k = 9; k >= 0; --k) s = fma(s, z, kSinPi[k]);
+    return -(s * y);
+}
+__device__ __forceinline__ void sincospi01(double x, double &sn, double &cs) {
+    const double y = x - 0.5, z = y * y;
+    double s = kSinPi[10], c = kCosPi[11];
+#pragma unroll
+    for (int k = 9; k >= 0; --k) s = fma(s, z, kSinPi[k]);
+#pragma unroll
+    for (int k = 10; k >= 0; --k) c = fma(c, z, kCosPi[k]);
+    cs = -(s * y);
+    sn = c;
 }
 
 struct Acc {  // per-thread sums of one atom
@@ -110,15 +150,15 @@ __device__ __forceinline__ void lj_pair(const LJc &c, double r2, double &s, doub
 // SHARE: beta == 2 alpha, so e^{-beta (r - rho_r0)} = e^{beta (rho_r0 - r0)} (e^{-alpha (r - r0)})^2 and the second
 // exponential is one multiplication (k3 is that constant factor, computed once per thread).
 template <bool TAPER, bool SHARE>
-__device__ __forceinline__ void fs_pair(const FSc &c, double r2, double dF_sum, double &s, double &u) {
+__device__ __forceinline__ void fs_pair(const FSc &c, const double *T, double r2, double dF_sum, double &s, double &u) {
     const double rinv = rsqrt_nr(r2), r = r2 * rinv;
-    const double e1 = exp_nb(-c.a * (r - c.r0)), e2 = e1 * e1;
+    const double e1 = exp_nb(-c.a * (r - c.r0), T), e2 = e1 * e1;
     const double m = c.Dm * (e2 - 2.0 * e1), dm = 2.0 * c.a * c.Dm * (e1 - e2);
-    const double e3 = SHARE ? c.k3 * e2 : exp_nb(-c.beta * (r - c.rr0));
+    const double e3 = SHARE ? c.k3 * e2 : exp_nb(-c.beta * (r - c.rr0), T);
     double fmag;
     if (TAPER) {
         double sn, cs;
-        sincospi((r - c.r_on) * c.inv_w, &sn, &cs);
+        sincospi01((r - c.r_on) * c.inv_w, sn, cs);
         double t = 0.5 * (1.0 + cs), dt = -0.5 * sn * c.pi_w;
         if (r <= c.r_on) { t = 1.0; dt = 0.0; }  // lanes outside the taper zone on the general path
         u = 0.5 * (m * t);
@@ -132,11 +172,11 @@ __device__ __forceinline__ void fs_pair(const FSc &c, double r2, double dF_sum, 
 
 // FS density pair (first pass)
 template <bool TAPER>
-__device__ __forceinline__ double fs_density(const FSc &c, double r2) {
+__device__ __forceinline__ double fs_density(const FSc &c, const double *T, double r2) {
     const double r = r2 * rsqrt_nr(r2);
-    double psi = exp_nb(-c.beta * (r - c.rr0));
+    double psi = exp_nb(-c.beta * (r - c.rr0), T);
     if (TAPER) {
-        double t = 0.5 * (1.0 + cospi((r - c.r_on) * c.inv_w));
+        double t = 0.5 * (1.0 + cospi01((r - c.r_on) * c.inv_w));
         if (r <= c.r_on) t = 1.0;
         psi *= t;
     }
@@ -207,7 +247,9 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) density_kernel(Dev d, int p_l
     const int slot = d.order[p];
     __shared__ double sh[9];
     __shared__ double red[32];
+    __shared__ double sT[32];
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
+    if (threadIdx.x < 32) sT[threadIdx.x] = kExp2Table[threadIdx.x];
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
@@ -235,11 +277,11 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) density_kernel(Dev d, int p_l
         const bool tp = (in0 && r20 > pc.ron2) || (in1 && r21 > pc.ron2);
         double p0, p1;
         if (!__any_sync(kFull, tp)) {
-            p0 = fs_density<false>(pc.fs, r20);
-            p1 = fs_density<false>(pc.fs, r21);
+            p0 = fs_density<false>(pc.fs, sT, r20);
+            p1 = fs_density<false>(pc.fs, sT, r21);
         } else {
-            p0 = fs_density<true>(pc.fs, r20);
-            p1 = fs_density<true>(pc.fs, r21);
+            p0 = fs_density<true>(pc.fs, sT, r20);
+            p1 = fs_density<true>(pc.fs, sT, r21);
         }
         if (in0) rho += p0;
         if (in1) rho += p1;
@@ -267,7 +309,9 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo)
     constexpr bool FS = POT == CFNEB_POT_FS_MORSE;
     __shared__ double sh[9];
     __shared__ double red[32 * 7];
+    __shared__ double sT[32];
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
+    if (threadIdx.x < 32) sT[threadIdx.x] = kExp2Table[threadIdx.x];
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
@@ -294,11 +338,11 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo)
         const bool tp = FS && ((in0 && r20 > pc.ron2) || (in1 && r21 > pc.ron2));
         if (FS) {
             if (!__any_sync(kFull, tp)) {
-                fs_pair<false, SHARE>(pc.fs, r20, ri.w + rj0.w, s0, u0);
-                fs_pair<false, SHARE>(pc.fs, r21, ri.w + rj1.w, s1, u1);
+                fs_pair<false, SHARE>(pc.fs, sT, r20, ri.w + rj0.w, s0, u0);
+                fs_pair<false, SHARE>(pc.fs, sT, r21, ri.w + rj1.w, s1, u1);
             } else {
-                fs_pair<true, SHARE>(pc.fs, r20, ri.w + rj0.w, s0, u0);
-                fs_pair<true, SHARE>(pc.fs, r21, ri.w + rj1.w, s1, u1);
+                fs_pair<true, SHARE>(pc.fs, sT, r20, ri.w + rj0.w, s0, u0);
+                fs_pair<true, SHARE>(pc.fs, sT, r21, ri.w + rj1.w, s1, u1);
             }
         } else {
             lj_pair(pc.lj, r20, s0, u0);
