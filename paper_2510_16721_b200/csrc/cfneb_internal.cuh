@@ -28,6 +28,8 @@ constexpr uint32_t kIdxMask = 0x7FFFFFu;
 constexpr int kShiftBits = 23;
 constexpr uint32_t kCodeCenter = 4u | (4u << 3) | (4u << 6);
 constexpr int kMaxAtoms = 1 << 23;
+constexpr int kInnerBuckets = 56;      // radial buckets of the list sort: uniform in r^2 on [0, r_cut^2)
+constexpr int kTailBuckets = 8;        // ... and on [r_cut^2, r_list^2)
 
 enum { DOT_PP = 0, DOT_MM, DOT_PM, DOT_GP, DOT_GM, DOT_GG, DOT_GV, DOT_PV, DOT_MV, DOT_VV };
 
@@ -93,6 +95,7 @@ struct Dev {
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
+    unsigned short *nbr_tail; // [S][kTailBuckets][Npad] number of entries below tail bucket t (list sorted by bucket)
     uint32_t *nbr_tmp;        // [S][cap][Npad]  unsorted list of a rebuild (scratch of K1)
     unsigned char *nbr_bkt;   // [S][cap][Npad]  r^2 bucket of each unsorted entry (scratch of K1)
     int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
@@ -153,6 +156,17 @@ double run_fp64_peak(cudaStream_t st);
 // ordered-bits helpers for atomicMax on non-negative doubles
 __device__ inline unsigned long long nonneg_bits(double x) { return (unsigned long long)__double_as_longlong(x); }
 __device__ inline double bits_nonneg(unsigned long long b) { return __longlong_as_double((long long)b); }
+
+// Index t of the first tail bucket whose entries cannot be inside r_cut now: they were built at
+// r >= sqrt(r_cut^2 + t (r_list^2 - r_cut^2) / kTailBuckets) and no pair distance has changed by more than acc
+// since (Geom::acc, the bound the rebuild decision uses).  kTailBuckets = walk the whole list.
+__device__ inline int first_dead_tail_bucket(double r_cut, double r_list, double acc) {
+    const double rc2 = r_cut * r_cut, step = (r_list * r_list - rc2) / kTailBuckets;
+    const double need = r_cut + acc + 1e-9 * r_cut;
+    for (int t = 0; t < kTailBuckets; ++t)
+        if (sqrt(rc2 + t * step) >= need) return t;
+    return kTailBuckets;
+}
 
 __device__ inline void set_error(Ctl *ctl, int code) { atomicCAS(&ctl->error, 0, code); }
 

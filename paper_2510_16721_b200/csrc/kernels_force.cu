@@ -260,9 +260,11 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) density_kernel(Dev d, int p_l
     // idle lanes sit far away from everything (every r^2 ~ 1e60: out of range, finite) and walk the last column
     double4 ri = make_double4(1e30, 1e30, 1e30, 0.0);
     int cnt = 0;
+    const int t_dead = first_dead_tail_bucket(d.r_cut, d.r_list, d.geom[slot].acc);  // block-uniform
     if (valid) {
         ri = ld256(Rc + i);
-        cnt = d.nbr_count[(size_t)slot * d.Npad + i];
+        cnt = t_dead < kTailBuckets ? (int)d.nbr_tail[((size_t)slot * kTailBuckets + t_dead) * d.Npad + i]
+                                    : d.nbr_count[(size_t)slot * d.Npad + i];
     }
     const int cnt_w = min(__reduce_max_sync(kFull, cnt), d.cap);
     const int cap = d.cap;
@@ -321,9 +323,11 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo)
 
     double4 ri = make_double4(1e30, 1e30, 1e30, 0.0);  // idle lanes: see density_kernel
     int cnt = 0;
+    const int t_dead = first_dead_tail_bucket(d.r_cut, d.r_list, d.geom[slot].acc);  // block-uniform
     if (valid) {
         ri = ld256(Rc + i);
-        cnt = d.nbr_count[(size_t)slot * d.Npad + i];
+        cnt = t_dead < kTailBuckets ? (int)d.nbr_tail[((size_t)slot * kTailBuckets + t_dead) * d.Npad + i]
+                                    : d.nbr_count[(size_t)slot * d.Npad + i];
     }
     const int cnt_w = min(__reduce_max_sync(kFull, cnt), d.cap);
     const int cap = d.cap;

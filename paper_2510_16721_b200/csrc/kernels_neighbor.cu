@@ -14,7 +14,10 @@
 // Radial order: each atom's list is stored sorted by distance at build time (stable counting sort on 64 buckets
 // of r^2).  In a solid the k-th nearest neighbour of every atom of a warp then lies in the same shell, so the
 // force kernels' per-entry decisions (inside r_cut? inside the taper zone?) are nearly warp-uniform and are
-// taken as warp-level branches with no per-step compaction pass.
+// taken as warp-level branches with no per-step compaction pass.  The last kTailBuckets buckets divide
+// [r_cut^2, r_list^2): the build also stores, per atom, how many entries lie below each of them, and a force
+// kernel stops its walk at the first tail bucket that cannot have come inside r_cut yet, given the image's
+// accumulated displacement bound Geom::acc (tail_rows()).
 #include "cfneb_internal.cuh"
 
 namespace cfn {
@@ -122,7 +125,7 @@ __device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
 // nbr_list (histogram kept in shared memory during the flushes).  Rows cnt..cap-1 are filled with a stand-in
 // entry (the atom itself shifted by -4 cell vectors along axis 0: farther than r_list whenever a list can be
 // built at all), so the force kernels read any row below cap without a bounds test and find it out of range.
-constexpr int kRadialBuckets = 64;
+constexpr int kRadialBuckets = kInnerBuckets + kTailBuckets;
 constexpr int kQueue = 32;
 constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, int p_lo) {
@@ -167,7 +170,9 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
     uint32_t *__restrict__ list = d.nbr_list + (size_t)slot * d.cap * d.Npad + ic;
     uint32_t *__restrict__ tmp = d.nbr_tmp + (size_t)slot * d.cap * d.Npad + ic;
     unsigned char *__restrict__ bkt = d.nbr_bkt + (size_t)slot * d.cap * d.Npad + ic;
-    const double rl2 = d.r_list * d.r_list, bscale = (double)kRadialBuckets / rl2;
+    // radial buckets: kInnerBuckets uniform in r^2 below r_cut^2, kTailBuckets uniform between r_cut^2 and r_list^2
+    const double rl2 = d.r_list * d.r_list, rc2 = d.r_cut * d.r_cut;
+    const double bscale_in = (double)kInnerBuckets / rc2, bscale_tail = rl2 > rc2 ? (double)kTailBuckets / (rl2 - rc2) : 0.0;
     int nq = 0;
 
     auto flush = [&]() {
@@ -196,7 +201,8 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
                 if (n0 == -4 && n1 == 0 && n2 == 0) bad_shift = true;  // reserved for the stand-in entry
                 const uint32_t code = (uint32_t)((n0 + 4) & 7) | ((uint32_t)((n1 + 4) & 7) << 3) |
                                       ((uint32_t)((n2 + 4) & 7) << 6);
-                const int bk = min((int)(r2 * bscale), kRadialBuckets - 1);
+                const int bk = r2 < rc2 ? min((int)(r2 * bscale_in), kInnerBuckets - 1)
+                                        : kInnerBuckets + min((int)((r2 - rc2) * bscale_tail), kTailBuckets - 1);
                 tmp[(size_t)cnt * d.Npad] = (uint32_t)j | (code << kShiftBits);
                 bkt[(size_t)cnt * d.Npad] = (unsigned char)bk;
                 hist[bk * kThreadsAtom] += 1;
@@ -247,9 +253,11 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
     // stable counting sort by r^2 bucket: exclusive starts, then placement (scan order kept inside a bucket),
     // four entries per round so that the global loads of a round are independent
     int start = 0;
+    unsigned short *tail = d.nbr_tail + (size_t)slot * kTailBuckets * d.Npad + i;
     for (int b = 0; b < kRadialBuckets; ++b) {
         const int c = hist[b * kThreadsAtom];
         hist[b * kThreadsAtom] = (unsigned short)start;
+        if (b >= kInnerBuckets) tail[(size_t)(b - kInnerBuckets) * d.Npad] = (unsigned short)start;  // entries below tail bucket b - 56
         start += c;
     }
     for (int k0 = 0; k0 < n; k0 += 4) {
