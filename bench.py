@@ -116,13 +116,37 @@ def measured_peaks():
 
 
 def ncu_traffic(workload, kernel):
-    """dram bytes per launch of `kernel` from the committed ncu --set full capture, if one exists."""
-    path = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu --set full
+    capture (profiles/dram_traffic.csv: workload,kernel,read_bytes,write_bytes,source), or None."""
+    path = os.path.join(ROOT, "profiles", "dram_traffic.csv")
     if not os.path.exists(path):
         return None
     with open(path) as fh:
-        d = json.load(fh)
-    return d.get(workload, {}).get(kernel)
+        for line in fh:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 4 and f[0] == workload and f[1] == kernel:
+                return float(f[2]) + float(f[3])
+    return None
+
+
+# fp64 operations per in-range pair as the formulas of kernels_force.cu are written (FMA = 2, everything else = 1;
+# DESIGN.md section 5): density pass plain / taper, force pass plain / taper (beta = 2 alpha: one exponential).
+FLOPS_DENSITY = (40.0, 70.0)
+FLOPS_FORCE = (71.0, 131.0)
+
+
+def bain_pair_counts(cells, dims, r_on, r_cut):
+    """In-range pairs per atom (plain, taper-zone) of every image of a perfect bcc supercell (dims conventional
+    cells per axis) under the image's cell: lattice vectors v = (n + basis) a with |v| <= r_on, r_on < |v| < r_cut."""
+    rng = np.arange(-5, 6)
+    g = np.stack(np.meshgrid(rng, rng, rng, indexing="ij"), -1).reshape(-1, 3).astype(np.float64)
+    frac = np.concatenate([g, g + 0.5])
+    frac = frac[np.any(frac != 0.0, axis=1)]
+    out = []
+    for h in cells:
+        r = np.linalg.norm(frac @ (np.asarray(h) / np.asarray(dims, dtype=np.float64)[:, None]), axis=1)
+        out.append((int(np.sum(r <= r_on)), int(np.sum((r > r_on) & (r < r_cut)))))
+    return out
 
 
 # ------------------------------------------------------------------------------------------------------------
@@ -291,6 +315,19 @@ def main_ours(args):
     kernels["sum_ms_per_step"] = float(kms.sum())
     kernels["update_only_GBps"] = 120.0 * units_per_step / (kms[cf.binding.K_UPDATE] * 1e-3) / 1e9
     kernels["reduce_only_GBps"] = 72.0 * units_per_step / (kms[cf.binding.K_REDUCE] * 1e-3) / 1e9
+    # the dominant kernel class (K2 density + force) against the fp64 ALU: algorithmic fp64 operations of the
+    # in-range pairs of this band (counted on the perfect lattice of every movable image) / its live time
+    roofline_force = None
+    if spec.lattice == "bcc_bain":
+        pc = bain_pair_counts(cells[1:P - 1], spec.dims, spec.pot[6], spec.pot[7])
+        flop = N * sum(npl * (FLOPS_DENSITY[0] + FLOPS_FORCE[0]) + ntp * (FLOPS_DENSITY[1] + FLOPS_FORCE[1]) for npl, ntp in pc)
+        t_force = kms[cf.binding.K_FORCE] * 1e-3
+        roofline_force = {"kernel": "K2 density_kernel + force_kernel", "bound": "alu", "achieved": flop / t_force / 1e12,
+                          "peak": None, "unit": "TFLOP/s", "frac": None, "algorithmic_flop": flop, "ms": t_force * 1e3,
+                          "in_range_pairs_per_atom_mean": float(np.mean([a + b for a, b in pc])),
+                          "taper_zone_pairs_per_atom_mean": float(np.mean([b for _, b in pc])),
+                          "peak_source": "measured DFMA chain, cfneb_util_fp64_peak (no fp64 figure in MEASURED_PEAKS.json)",
+                          "share_of_step": float(kms[cf.binding.K_FORCE] / kms.sum())}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -305,7 +342,7 @@ def main_ours(args):
                          % (72.0 * N * P / 1e6),
                    "workspace_GB": band.workspace_bytes / 1e9, "neighbor_rebuilds_in_timed_region": int(st1.rebuilds - st0.rebuilds),
                    "max_neighbors_seen": int(st1.max_neighbors_seen)},
-        "clocks": clocks, "roofline": roofline, "kernels": kernels,
+        "clocks": clocks, "roofline": roofline, "roofline_force": roofline_force, "kernels": kernels,
         "gpu_launches": int(st1.graph_kernel_nodes) * args.steps,
         "status": {"fmax": st1.fmax, "barrier": st1.barrier, "steps": int(st1.steps)},
     }
@@ -326,26 +363,29 @@ def measure_e2e(band, pos, cells, n_steps, barrier, max_over_ranks, world, units
     a_pos, a_cells = pin_pos.numpy(), pin_cells.numpy()
     o_pos, o_cells, o_E = out_pos.numpy(), out_cells.numpy(), out_E.numpy()
 
-    def one():
-        band.set_path(a_pos, a_cells)              # H2D: P x (N x 3 + 9) doubles
-        band.step(1)
-        band.get_path_into(o_pos, o_cells, o_E)    # D2H: P x (N x 3 + 9 + 1) doubles; synchronises
-        a_pos[...] = o_pos                         # the next step's input is this step's output (host copy)
-        a_cells[...] = o_cells
+    bufs = [(a_pos, a_cells), (o_pos, o_cells)]
 
-    one()  # warm-up
+    def one(i):
+        (ip, ic), (op, oc) = bufs[i & 1], bufs[1 - (i & 1)]
+        band.set_path(ip, ic)                      # H2D: P x (N x 3 + 9) doubles
+        band.step(1)
+        band.get_path_into(op, oc, o_E)            # D2H: P x (N x 3 + 9 + 1) doubles; synchronises
+        # the next step's input is this step's output: the two pinned buffer pairs swap roles
+
+    one(0)  # warm-up
     barrier()
     t0 = time.perf_counter()
-    for _ in range(n_steps):
-        one()
+    for i in range(1, n_steps + 1):
+        one(i)
     barrier()
     dt = max_over_ranks(time.perf_counter() - t0)
     h2d = P * (N * 3 + 9) * 8
     d2h = P * (N * 3 + 9 + 1) * 8
     return {"value": world * units_per_step * n_steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "steps": n_steps, "ms_per_step": 1e3 * dt / n_steps,
-            "what": "per step: cfneb_set_path(host pinned) + cfneb_step(1) + cfneb_get_path(host pinned); wall clock, "
-                    "includes the host-side copy of the returned path into the next step's input"}
+            "what": "per step: cfneb_set_path(host pinned) + cfneb_step(1) + cfneb_get_path(host pinned); wall clock; "
+                    "set_path replaces the whole path, so every step also rebuilds all neighbour lists and "
+                    "re-evaluates the endpoints"}
 
 
 def main():
@@ -360,6 +400,9 @@ def main():
         import paper_2510_16721_b200 as cf
         tf = cf.fp64_peak_tflops()
         line["kernels"]["fp64_dfma_peak_tflops_measured"] = tf
+        if line.get("roofline_force"):
+            line["roofline_force"]["peak"] = tf
+            line["roofline_force"]["frac"] = line["roofline_force"]["achieved"] / tf
     except Exception as exc:  # measurement utility only
         line["kernels"]["fp64_dfma_peak_tflops_measured"] = "failed: %s" % exc
     band.close()

@@ -98,7 +98,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.part_dots = c.take<double>(S * d.nblk_stream * kNDots);
     d.dispmax = c.take<unsigned long long>(S);
     d.nbr_count = c.take<int>(S * Npad);
-    d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 8 * Npad);  // 8 rows of slack for the force kernels' look-ahead
+    d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 16 * Npad);  // 16 rows of slack for the force kernels' look-ahead
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
     d.nbr_tmp = c.take<uint32_t>(S * (size_t)d.cap * Npad);
     d.nbr_bkt = c.take<unsigned char>(S * (size_t)d.cap * Npad);

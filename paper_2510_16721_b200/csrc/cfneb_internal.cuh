@@ -69,7 +69,6 @@ struct Dev {
     int N, Npad, S, cap;
     int potential, cell_mode, climb, fire_nmin, rebuild_every;
     int nblk_atom, nblk_stream, nbins_max;
-    int k4_variant, k6_variant;
     int nblk_red, nblk_upd;   // K4 / K6: blocks per image, each striding over the image's nblk_stream tiles
     int nb_cap[3];
     double pot[12];

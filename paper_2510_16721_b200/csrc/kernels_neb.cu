@@ -10,7 +10,6 @@
 // FIRE needs (f.v, |f|, |v|, |v_new|) follows from ten dot products per image taken in ONE pass over
 // X, F, v (K4); K6 then streams the same arrays once more and writes X_new, v_new.
 #include "cfneb_internal.cuh"
-#include <stdlib.h>
 
 namespace cfn {
 
@@ -276,11 +275,7 @@ __global__ void __launch_bounds__(128) scalar_kernel(Dev d, int dry) {
 void launch_reduce(const Dev &d, cudaStream_t st) {
     if (d.S < 3) return;
     dim3 grid(d.nblk_red, d.S - 2);
-    switch (d.k4_variant) {
-        case 1: reduce_kernel<2, 1><<<grid, kThreadsStream, 0, st>>>(d); break;
-        case 2: reduce_kernel<2, 2><<<grid, kThreadsStream, 0, st>>>(d); break;
-        default: reduce_kernel<3, 1><<<grid, kThreadsStream, 0, st>>>(d); break;
-    }
+    reduce_kernel<2, 1><<<grid, kThreadsStream, 0, st>>>(d);
 }
 
 // Blocks per image for a streaming kernel that keeps `occ` blocks resident per SM: the smallest whole number
@@ -301,18 +296,15 @@ static int blocks_per_image(int tiles, int images, int slots) {
     return best < tiles ? best : tiles;
 }
 
-int update_blocks_per_sm(int variant);  // kernels_update.cu
+int update_blocks_per_sm();  // kernels_update.cu
 
 void plan_stream_grids(Dev &d) {
     int dev = 0, sms = 148, occ_r = 3, occ_u = 2;
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    const char *e4 = getenv("CFNEB_K4_VARIANT"), *e6 = getenv("CFNEB_K6_VARIANT");
-    d.k4_variant = e4 ? atoi(e4) : 1;  // measured on B200 at c4: <2,1> 5.50 TB/s, <3,1> 4.94 (spills), <2,2> 4.83
-    d.k6_variant = e6 ? atoi(e6) : 0;
-    occ_r = d.k4_variant == 0 ? 3 : 2;
-    occ_u = update_blocks_per_sm(d.k6_variant);
-    if (getenv("CFNEB_K4_OCC")) occ_r = atoi(getenv("CFNEB_K4_OCC"));
-    if (getenv("CFNEB_K6_OCC")) occ_u = atoi(getenv("CFNEB_K6_OCC"));
+    // measured on B200 at c4 (profiles/): reduce <2 blocks/SM, 1 tile in flight> 5.5 TB/s (114 registers, no spill;
+    // <3, 1> spills and reaches 4.9, <2, 2> 4.8); update <3 blocks/SM> 6.2 TB/s (76 registers; <2> 5.9)
+    occ_r = 2;
+    occ_u = update_blocks_per_sm();
     d.nblk_red = blocks_per_image(d.nblk_stream, d.S - 2, sms * occ_r);
     d.nblk_upd = blocks_per_image(d.nblk_stream, d.S - 2, sms * occ_u);
 }

@@ -267,11 +267,10 @@ __global__ void export_forces_kernel(Dev d, double *Fo, double *Vo, double *Eo) 
 void launch_update(const Dev &d, cudaStream_t st) {
     if (d.S < 3) return;
     dim3 grid(d.nblk_upd, d.S - 2);
-    if (d.k6_variant == 1) update_kernel<2><<<grid, kThreadsStream, 0, st>>>(d);
-    else update_kernel<3><<<grid, kThreadsStream, 0, st>>>(d);
+    update_kernel<3><<<grid, kThreadsStream, 0, st>>>(d);
 }
 
-int update_blocks_per_sm(int variant) { return variant == 1 ? 2 : 3; }
+int update_blocks_per_sm() { return 3; }
 
 void launch_materialize_fneb(const Dev &d, cudaStream_t st) {
     dim3 grid((d.N + 3 + 127) / 128, d.S);
