@@ -241,29 +241,20 @@ def main_ours(args):
     import paper_2510_16721_b200 as cf
     from cfneb_workloads import build_workload
 
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    from paper_2510_16721_b200.replicas import Ranks
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the CFNEB path has no CPU fallback")
     cf.lib()  # fail loudly if libcfneb.so is missing
     torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    ranks = Ranks("nccl", torch.device("cuda", local))
+    rank, world = ranks.rank, ranks.world
 
     def barrier():
-        if dist is not None:
-            dist.barrier()
+        ranks.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
+    max_over_ranks = ranks.max_over_ranks
 
     k = args.config
     spec, pos, cells = build_workload(k)
@@ -346,7 +337,7 @@ def main_ours(args):
         "gpu_launches": int(st1.graph_kernel_nodes) * args.steps,
         "status": {"fmax": st1.fmax, "barrier": st1.barrier, "steps": int(st1.steps)},
     }
-    return band, line, (pos, cells, spec, barrier, max_over_ranks, world, rank, units_per_step)
+    return band, line, (pos, cells, spec, barrier, max_over_ranks, world, rank, units_per_step, ranks)
 
 
 def measure_e2e(band, pos, cells, n_steps, barrier, max_over_ranks, world, units_per_step):
@@ -393,7 +384,7 @@ def main():
     if args.impl == "reference":
         return main_reference(args)
     band, line, ctx = main_ours(args)
-    pos, cells, spec, barrier, max_over_ranks, world, rank, units_per_step = ctx
+    pos, cells, spec, barrier, max_over_ranks, world, rank, units_per_step, ranks = ctx
     if not args.no_e2e:
         line["e2e"] = measure_e2e(band, pos, cells, max(1, args.e2e_steps), barrier, max_over_ranks, world, units_per_step)
     try:
@@ -412,10 +403,7 @@ def main():
                                 "sample": r["sample"], "host_cores": r["host_cores"], "seconds": r["seconds"]}
     if rank == 0:
         print(json.dumps(line))
-    if world > 1:
-        import torch.distributed as dist
-        dist.barrier()
-        dist.destroy_process_group()
+    ranks.close()
     return 0
 
 
