@@ -11,6 +11,11 @@ image distribution, `adapt()`).  Composition of O0-O9:
   O4 generalized force      cellfilter.generalized_force    Eq. 17
   O5-O8                     neb.py                          Eq. 1, refs [12], [13]
   O9 adaptive control       adapt() below                   P:128 (reading A16 -- parity unpinned)
+
+External pressure (reading A25; the paper's graphite band is "under 40GPa", Fig. 3 caption, without
+equations): a hydrostatic pressure p replaces U by the enthalpy H = U + p Omega, Omega = |det h|.  With the
+right-multiplication strain of Eq. 2, Omega(eps) = Omega det(I + eps), so by Eq. 3 the virial of H is
+V - p Omega I; H is the energy the tangent (O5), the climbing image (O6) and the barrier (O8) see.
 """
 import numpy as np
 
@@ -28,7 +33,7 @@ class CrystalEvaluator:
     """Callback for neb.Band: X = [R~ ; lam*B] -> (E, G) through O1-O4."""
 
     def __init__(self, h0, potential, pot, r_list, max_neighbors, lam=1.0, cell_mode=cf.CELL_B, brute=False,
-                 threads=None):
+                 threads=None, pressure=0.0):
         self.h0 = np.array(h0, dtype=np.float64)
         self.potential = int(potential)
         self.pot = np.array(pot, dtype=np.float64)
@@ -38,6 +43,7 @@ class CrystalEvaluator:
         self.cell_mode = cell_mode
         self.brute = brute
         self.threads = threads
+        self.pressure = float(pressure)
         self.last = None  # (F, V, D, h) of the last evaluation, for parity hooks
 
     def deformation(self, X):
@@ -54,6 +60,13 @@ class CrystalEvaluator:
             hs.append(self.h0 @ D)  # h = h0 D
         E, F, V = ff.eval_images(np.stack(Rts), self.h0, np.stack(hs), self.potential, self.pot, self.r_list,
                                  self.cap, brute=self.brute, threads=self.threads)
+        if self.pressure != 0.0:  # A25: H = U + p Omega;  V_H = V - p Omega I  (Eq. 2-3)
+            E = np.array(E, dtype=np.float64)
+            V = np.array(V, dtype=np.float64)
+            for q in range(len(X_list)):
+                omega = abs(np.linalg.det(hs[q]))
+                E[q] += self.pressure * omega
+                V[q] -= self.pressure * omega * np.eye(3)
         G = [cf.generalized_force(F[q], V[q], Ds[q], self.lam, self.cell_mode) for q in range(len(X_list))]
         self.last = dict(F=F, V=V, D=np.stack(Ds), h=np.stack(hs))
         return list(E), G
@@ -63,7 +76,7 @@ class CFNEB:
     """Cell-filter NEB band.  pos[P,N,3] Cartesian, cells[P,3,3] (rows = lattice vectors)."""
 
     def __init__(self, pos, cells, potential, pot, r_cut, k_spring=1.0, climb=True, cell_mode=cf.CELL_B,
-                 cell_factor=1.0, fire=None, skin=0.3, max_neighbors=128, brute=False, threads=None):
+                 cell_factor=1.0, fire=None, skin=0.3, max_neighbors=128, brute=False, threads=None, pressure=0.0):
         pos = np.asarray(pos, dtype=np.float64)
         cells = np.asarray(cells, dtype=np.float64)
         self.N = pos.shape[1]
@@ -76,7 +89,7 @@ class CFNEB:
             Rt, B, D = cf.input_mapping(pos[p], cells[p], self.h0)
             X.append(cf.pack(Rt, D if cell_mode == cf.CELL_D else B, self.lam))
         self.evaluator = CrystalEvaluator(self.h0, potential, pot, r_cut + skin, max_neighbors, self.lam, cell_mode,
-                                          brute, threads)
+                                          brute, threads, pressure)
         self.band = Band(X, self.evaluator, k_spring=k_spring, climb=climb, fire=self.fire_params,
                          post_update=self._post_update)
 
@@ -177,7 +190,7 @@ class CFNEB:
 
 
 def relax_endpoint(R, h, potential, pot, r_cut, fmax_tol=1e-4, max_steps=20000, cell_factor=0.0, fire=None,
-                   skin=0.3, max_neighbors=128, cell_mode=cf.CELL_B):
+                   skin=0.3, max_neighbors=128, cell_mode=cf.CELL_B, pressure=0.0):
     """Cell-filter FIRE relaxation of one structure (BASELINE.json configs: "both endpoints cell-relaxed").
 
     Same generalized coordinates and forces as the band (O0-O4, O7) with f = G (no NEB projection).
@@ -187,7 +200,7 @@ def relax_endpoint(R, h, potential, pot, r_cut, fmax_tol=1e-4, max_steps=20000, 
     h0 = np.asarray(h, dtype=np.float64)
     N = R.shape[0]
     lam = auto_cell_factor(h0, N) if cell_factor == 0 else float(cell_factor)
-    ev = CrystalEvaluator(h0, potential, pot, r_cut + skin, max_neighbors, lam, cell_mode)
+    ev = CrystalEvaluator(h0, potential, pot, r_cut + skin, max_neighbors, lam, cell_mode, pressure=pressure)
     Rt, B, D = cf.input_mapping(R, h0, h0)
     X = cf.pack(Rt, B, lam)
     fire = Fire((1,) + X.shape, **(fire or {}))
