@@ -72,6 +72,10 @@ enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default)
  *   skin: neighbour-list skin; lists hold pairs with r < r_cut + skin and are rebuilt on the device
  *         when the accumulated displacement bound exceeds skin, or every rebuild_every steps (0 = never
  *         by count).  max_neighbors: list capacity per atom.  max_images: capacity of the band.
+ *   pressure: external hydrostatic pressure p in energy / length^3 (reading A25; the paper's graphite band is
+ *         "under 40GPa").  The band then relaxes the enthalpy H = U + p Omega: every energy the library
+ *         reports or uses (tangent, climbing image, barrier, cfneb_get_path / cfneb_get_forces) is H, and the
+ *         virial is V - p Omega I (Eq. 2-3).  0 = none.
  */
 typedef struct cfneb_params {
     int32_t potential;
@@ -87,6 +91,7 @@ typedef struct cfneb_params {
     double cell_factor;
     double fire_dt0, fire_dtmax, fire_maxstep, fire_finc, fire_fdec, fire_astart, fire_fa;
     double skin;
+    double pressure;
 } cfneb_params;
 
 /* Snapshot written by cfneb_get_status (synchronises the stream). */

@@ -34,7 +34,7 @@ class Params(ctypes.Structure):
         ("pot", ctypes.c_double * 12), ("k_spring", ctypes.c_double), ("cell_factor", ctypes.c_double),
         ("fire_dt0", ctypes.c_double), ("fire_dtmax", ctypes.c_double), ("fire_maxstep", ctypes.c_double),
         ("fire_finc", ctypes.c_double), ("fire_fdec", ctypes.c_double), ("fire_astart", ctypes.c_double),
-        ("fire_fa", ctypes.c_double), ("skin", ctypes.c_double),
+        ("fire_fa", ctypes.c_double), ("skin", ctypes.c_double), ("pressure", ctypes.c_double),
     ]
 
 

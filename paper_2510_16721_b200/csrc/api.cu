@@ -56,7 +56,7 @@ bool valid_params(int32_t n_atoms, const cfneb_params *prm) {
     if (prm->potential != CFNEB_POT_LJ_SF && prm->potential != CFNEB_POT_FS_MORSE) return false;
     if (prm->cell_mode < CFNEB_CELL_FIXED || prm->cell_mode > CFNEB_CELL_D) return false;
     if (prm->max_images < 3 || prm->max_neighbors < 1 || prm->max_neighbors > 4096) return false;
-    if (!(prm->skin >= 0.0) || !(prm->cell_factor >= 0.0)) return false;
+    if (!(prm->skin >= 0.0) || !(prm->cell_factor >= 0.0) || !isfinite(prm->pressure)) return false;
     const double rc = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
     if (!(rc > 0.0)) return false;
     if (prm->potential == CFNEB_POT_FS_MORSE && !(prm->pot[7] > prm->pot[6])) return false;
@@ -249,6 +249,7 @@ void cfneb_default_params(cfneb_params *prm) {
     prm->fire_dt0 = 0.1; prm->fire_dtmax = 1.0; prm->fire_maxstep = 0.2;
     prm->fire_finc = 1.1; prm->fire_fdec = 0.5; prm->fire_astart = 0.1; prm->fire_fa = 0.99;
     prm->skin = 0.3;
+    prm->pressure = 0.0;
 }
 
 size_t cfneb_workspace_bytes(int32_t n_atoms, const cfneb_params *prm) {
@@ -309,6 +310,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     d.dt0 = prm->fire_dt0; d.dtmax = prm->fire_dtmax; d.maxstep = prm->fire_maxstep;
     d.finc = prm->fire_finc; d.fdec = prm->fire_fdec; d.astart = prm->fire_astart; d.fa = prm->fire_fa;
     d.skin = prm->skin;
+    d.pressure = prm->pressure;
     d.r_cut = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
     d.r_list = d.r_cut + d.skin;
     memcpy(d.h0, cell_init, sizeof d.h0);  // A7: reference cell = cell of the initial endpoint

@@ -73,6 +73,7 @@ struct Dev {
     int nb_cap[3];
     double pot[12];
     double k_spring, lam;
+    double pressure;          // external hydrostatic pressure (A25): E <- U + p Omega, V <- V - p Omega I in finalize_kernel
     double dt0, dtmax, maxstep, finc, fdec, astart, fa;
     double skin, r_cut, r_list;
     double h0[9], h0inv[9];

@@ -106,11 +106,13 @@ __global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
         for (int q = 0; q < kNForcePart; ++q) a8[q] += pf[(size_t)b * kNForcePart + q];
     block_sum<kNForcePart>(a8, red);
     if (threadIdx.x == 0) {
-        const double E = a8[0] + a8[7];
-        const double V[9] = {a8[1], a8[4], a8[5], a8[4], a8[2], a8[6], a8[5], a8[6], a8[3]};
+        const Geom *g = d.geom + slot;
+        // external pressure (A25): enthalpy H = U + p Omega and its virial V - p Omega I (Eq. 2-3)
+        const double pv = d.pressure * fabs(g->vol);
+        const double E = a8[0] + a8[7] + pv;
+        const double V[9] = {a8[1] - pv, a8[4], a8[5], a8[4], a8[2] - pv, a8[6], a8[5], a8[6], a8[3] - pv};
         d.E[slot] = E;
         double Gc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-        const Geom *g = d.geom + slot;
         if (d.cell_mode != CFNEB_CELL_FIXED) {
             double T[9];
             mul3_atb(g->Dinv, V, T);  // D^-T V   (Eq. 13-14)

@@ -23,7 +23,7 @@ def rel(a, b):
     return float(np.max(np.abs(a - b)) / (s if s > 0 else 1.0))
 
 
-def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_images=None, **over):
+def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_images=None, pressure=0.0, **over):
     """(oracle band, GPU band) on configs[k] inputs."""
     import paper_2510_16721_b200 as cf
     from oracle import cfneb as oc
@@ -31,8 +31,9 @@ def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_im
     climb = spec.climb if climb is None else climb
     orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=climb,
                    cell_mode=cell_mode, cell_factor=cell_factor, fire=spec.fire, skin=spec.skin,
-                   max_neighbors=spec.max_neighbors)
-    prm = cf.params_for(spec, cell_factor=cell_factor, cell_mode=cell_mode, climb=int(climb), max_images=max_images, **over)
+                   max_neighbors=spec.max_neighbors, pressure=pressure)
+    prm = cf.params_for(spec, cell_factor=cell_factor, cell_mode=cell_mode, climb=int(climb), max_images=max_images,
+                        pressure=float(pressure), **over)
     gpu = cf.CFNEB(pos, cells, prm)
     return spec, orc, gpu
 
@@ -179,6 +180,30 @@ def test_cell_modes_fixed_and_D(mode):
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
     if mode == 0:  # O4: G_cell = 0; the cell rows only see the (here ~1e-16) tangent between the endpoint cells
         assert np.max(np.abs(Xg[:, -3:] - Xg0[:, -3:])) < 1e-12 and np.max(np.abs(Xo[:, -3:] - X0[:, -3:])) < 1e-12
+    gpu.close()
+
+
+@pytest.mark.parametrize("k,mode,p_ext", [(0, 1, 0.7), (0, 2, 0.7), (2, 1, 0.25)])
+def test_external_pressure_enthalpy_band(k, mode, p_ext):
+    """Reading A25 ("under 40GPa"): H = U + p Omega and V - p Omega I, in both cell coordinates (Eq. 14, Eq. 17).
+    0.25 eV/A^3 = 40 GPa for the Finnis-Sinclair band."""
+    spec, orc, gpu = make_pair(k, cell_factor=0.0, cell_mode=mode, pressure=p_ext, n_images=5 if k == 2 else None)
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE
+    assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
+    assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    # the pressure term is a large part of what is being compared
+    _, cells, _ = orc.get_path()
+    assert p_ext * abs(np.linalg.det(cells[1])) > 0.05 * abs(orc.band.E[1] - p_ext * abs(np.linalg.det(cells[1])))
+    X0, _ = orc.get_state()
+    orc.step(4)
+    gpu.step(4)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
+    st = gpu.get_status()
+    assert st.error == 0 and abs(st.barrier - orc.band.barrier) < 1e-9 * max(1.0, abs(orc.band.barrier))
     gpu.close()
 
 
