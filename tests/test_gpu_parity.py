@@ -397,3 +397,55 @@ def test_step_timed_matches_graph_step():
     assert np.array_equal(a.get_state()[0], b.get_state()[0])
     a.close()
     b.close()
+
+
+def _triclinic_band(dims, shear, sigma, n_images, seed):
+    """A sheared (triclinic) Bain-like band with strongly displaced atoms, some of them outside the cell (unwrapped
+    coordinates, A17): bins, periodic shifts and the general formula (taper) paths all see irregular input."""
+    from cfneb_workloads import bain_endpoints, linear_path, load_lattice_constants, splitmix64_normals
+    lc = load_lattice_constants()
+    f0, c0, f1, c1 = bain_endpoints(dims, lc["fs_bcc_a"], lc["fs_fcc_volume_ratio"])
+    S = np.eye(3) + np.array(shear, dtype=np.float64)
+    c0, c1 = c0 @ S, c1 @ S
+    pos, cells = linear_path(f0, c0, f1, c1, n_images, seed, 1e-3)
+    kick = splitmix64_normals(seed + 100, pos[0].size).reshape(pos[0].shape) * sigma
+    pos = pos + kick[None]                      # the same disorder in every image, endpoints included
+    pos[:, ::7] += cells[:, 0:1, :]             # every 7th atom moved out by one lattice vector
+    pos[:, 3::11] -= cells[:, 2:3, :] + cells[:, 1:2, :]
+    return pos, cells
+
+
+@pytest.mark.parametrize("dims,n_images", [((3, 3, 4), 5), ((7, 5, 9), 4)])
+def test_triclinic_disordered_band_with_unwrapped_atoms(dims, n_images):
+    """Edge cases in one band: triclinic cell, N not a multiple of 32 or 128 (72 / 630 atoms), a box narrower than
+    2 r_list (explicit periodic shifts, atoms seeing several images of one neighbour) or with >= 3 bins per axis,
+    atoms stored outside the cell, disorder of 0.15 A (no two atoms share a shell)."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    from oracle import forcefield as ff
+    spec = CONFIGS[2]
+    pos, cells = _triclinic_band(dims, [[0, 0.08, -0.05], [0.03, 0, 0.11], [-0.07, 0.02, 0]], 0.15, n_images, 11)
+    N = pos.shape[1]
+    assert N % 32 != 0
+    cap = 256
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=True, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=cap)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, max_neighbors=cap, max_images=n_images))
+    # neighbour list of an interior image, bit-exact after sorting
+    Rt, D = orc.evaluator.deformation(orc.band.X[1])
+    cnt, lst, sh = ff.neighbors(Rt, orc.h0, orc.h0 @ D, spec.r_cut + spec.skin, cap)
+    gc, gl, gs = gpu.get_neighbors(1)
+    assert np.array_equal(gc, cnt)
+    assert np.array_equal(sorted_triples(gc, gl, gs), sorted_triples(cnt, lst, sh))
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE
+    assert rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
+    assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    X0, _ = orc.get_state()
+    orc.step(3)
+    gpu.step(3)
+    assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
+    assert gpu.get_status().error == 0
+    gpu.close()
