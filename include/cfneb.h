@@ -171,6 +171,23 @@ CFNEB_API int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t 
 /* Segment lengths d_p = |X_{p+1} - X_p|, p = 0..P-2, at the current X (HOST, P-1 doubles). Synchronises. */
 CFNEB_API int cfneb_get_segment_lengths(cfneb_t *h, double *d);
 
+/*
+ * Cell-filter FIRE relaxation of the two endpoints on the device (the step before the band in every
+ * BASELINE.json config: "both endpoints cell-relaxed"; the paper's workflow starts from relaxed end states).
+ * Each endpoint is relaxed as an independent structure in the band's generalized coordinates X = [R~ ; lam B] with
+ * f = G (Eq. 12, 17; no tangent, no springs) and its own FIRE state (O7, step limit maxstep sqrt(N + 3)); an
+ * endpoint stops when the max row norm of its G is below fmax_tol (tested before every update) and the call returns
+ * when both have stopped or after max_steps updates.  The interior images are not touched while this runs.
+ *   rebuild_band != 0: afterwards the band is rebuilt from the relaxed endpoints exactly as cfneb_create without an
+ *       explicit path would: h0 := relaxed cell of image 0 (A7), lam (A13) recomputed, interior images linear in X,
+ *       FIRE restarted, neighbour lists rebuilt, the iteration graph re-captured.
+ *   rebuild_band == 0: only the endpoints change; FIRE of the band is restarted.
+ * Outputs (each may be NULL): steps_done[2] updates taken per endpoint, fmax_out[2] and energy_out[2] at the final
+ * states.  Synchronises.
+ */
+CFNEB_API int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_t rebuild_band,
+                                    int32_t *steps_done, double *fmax_out, double *energy_out);
+
 /* Current path: *n_images = P; pos P*N*3 Cartesian (R = R~ D), cells P*9 (h = h0 D, D = sqrt(B):
  * rotation-free), energies P (of the last evaluation; NaN for an image inserted since).
  * Any of pos/cells/energies may be NULL.  Synchronises. */

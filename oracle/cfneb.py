@@ -190,18 +190,21 @@ class CFNEB:
 
 
 def relax_endpoint(R, h, potential, pot, r_cut, fmax_tol=1e-4, max_steps=20000, cell_factor=0.0, fire=None,
-                   skin=0.3, max_neighbors=128, cell_mode=cf.CELL_B, pressure=0.0):
+                   skin=0.3, max_neighbors=128, cell_mode=cf.CELL_B, pressure=0.0, h_ref=None):
     """Cell-filter FIRE relaxation of one structure (BASELINE.json configs: "both endpoints cell-relaxed").
 
     Same generalized coordinates and forces as the band (O0-O4, O7) with f = G (no NEB projection).
+    h_ref: reference cell h0 of the generalized coordinates ("a reference cell", A7); default the structure's
+    own cell.  A band relaxes its final endpoint in the frame of its initial endpoint's cell.
     Returns (R, h, E, fmax, n_steps).
     """
     R = np.asarray(R, dtype=np.float64)
-    h0 = np.asarray(h, dtype=np.float64)
+    h = np.asarray(h, dtype=np.float64)
+    h0 = h if h_ref is None else np.asarray(h_ref, dtype=np.float64)
     N = R.shape[0]
     lam = auto_cell_factor(h0, N) if cell_factor == 0 else float(cell_factor)
     ev = CrystalEvaluator(h0, potential, pot, r_cut + skin, max_neighbors, lam, cell_mode, pressure=pressure)
-    Rt, B, D = cf.input_mapping(R, h0, h0)
+    Rt, B, D = cf.input_mapping(R, h, h0)
     X = cf.pack(Rt, B, lam)
     fire = Fire((1,) + X.shape, **(fire or {}))
     E, fmax, it = np.nan, np.inf, 0

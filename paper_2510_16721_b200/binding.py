@@ -19,7 +19,8 @@ KERNEL_CLASSES = ("cell_prep", "neighbor", "force", "reduce", "scalar", "update"
 
 EXPORTS = (
     "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_timed",
-    "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_get_segment_lengths", "cfneb_get_path",
+    "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
+    "cfneb_get_path",
     "cfneb_set_path", "cfneb_get_state", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
     "cfneb_destroy", "cfneb_strerror", "cfneb_last_cuda_error", "cfneb_util_fp64_peak",
 )
@@ -84,7 +85,7 @@ def lib():
     for name, args in (
         ("cfneb_step", [vp, i32]), ("cfneb_step_timed", [vp, i32, dp]), ("cfneb_insert_image", [vp, i32]),
         ("cfneb_delete_image", [vp, i32]), ("cfneb_adapt", [vp, f64, f64, ip, ip]),
-        ("cfneb_get_segment_lengths", [vp, dp]), ("cfneb_get_path", [vp, ip, dp, dp, dp]),
+        ("cfneb_relax_endpoints", [vp, f64, i32, i32, ip, dp, dp]), ("cfneb_get_segment_lengths", [vp, dp]), ("cfneb_get_path", [vp, ip, dp, dp, dp]),
         ("cfneb_set_path", [vp, dp, dp]), ("cfneb_get_state", [vp, dp, dp]),
         ("cfneb_get_forces", [vp, dp, dp, dp, dp]), ("cfneb_get_neighbors", [vp, i32, ip, ip, ip]),
         ("cfneb_get_status", [vp, ctypes.POINTER(Status)]), ("cfneb_util_fp64_peak", [vp, dp]),
@@ -221,6 +222,16 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_adapt")
         return ni.value, nd.value
+
+    def relax_endpoints(self, fmax_tol, max_steps, rebuild_band=True):
+        """cfneb_relax_endpoints: returns (steps[2], fmax[2], energy[2])."""
+        steps = (ctypes.c_int32 * 2)()
+        fmax = (ctypes.c_double * 2)()
+        en = (ctypes.c_double * 2)()
+        rc = lib().cfneb_relax_endpoints(self._h, float(fmax_tol), int(max_steps), int(bool(rebuild_band)), steps, fmax, en)
+        if rc:
+            raise CfnebError(rc, "cfneb_relax_endpoints")
+        return [steps[0], steps[1]], [fmax[0], fmax[1]], [en[0], en[1]]
 
     # -- views -----------------------------------------------------------------------------------------
     def get_status(self):

@@ -96,6 +96,8 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.coef = c.take<double>(S * 4);
     d.part_force = c.take<double>(S * d.nblk_atom * kNForcePart);
     d.part_dots = c.take<double>(S * d.nblk_stream * kNDots);
+    d.relax = c.take<RelaxState>(2);
+    d.part_relax = c.take<double>((size_t)2 * d.nblk_stream * 4);
     d.dispmax = c.take<unsigned long long>(S);
     d.nbr_count = c.take<int>(S * Npad);
     d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 16 * Npad);  // 16 rows of slack for the force kernels' look-ahead
@@ -217,6 +219,33 @@ int upload_order(cfneb *h) {
     return CFNEB_OK;
 }
 
+// Reference cell h0 (A7), lam (A13) and the per-axis bin caps, from the two endpoint cells.
+int set_reference_frame(cfneb *h, const double *cell_init, const double *cell_final) {
+    Dev &d = h->d;
+    memcpy(d.h0, cell_init, sizeof d.h0);  // A7: reference cell = cell of the initial endpoint
+    inv3(d.h0, d.h0inv);
+    // A13: lam = 0 selects Omega0^(1/3) N^(1/6); lam = 1 is the paper's equations literally
+    d.lam = h->prm.cell_factor > 0.0 ? h->prm.cell_factor : cbrt(fabs(det3(cell_init))) * pow((double)d.N, 1.0 / 6.0);
+    // per-axis bin caps from the larger endpoint cell, with headroom; product <= nbins_max
+    double w0[3], w1[3];
+    perp_widths(cell_init, w0);
+    perp_widths(cell_final, w1);
+    for (int a = 0; a < 3; ++a) {
+        const double w = fmax(w0[a], w1[a]) * 1.5;
+        d.nb_cap[a] = (int)floor(w / d.r_list);
+        if (d.nb_cap[a] < 3) d.nb_cap[a] = 3;
+    }
+    while ((long long)d.nb_cap[0] * d.nb_cap[1] * d.nb_cap[2] > d.nbins_max) {
+        int a = 0;
+        if (d.nb_cap[1] > d.nb_cap[a]) a = 1;
+        if (d.nb_cap[2] > d.nb_cap[a]) a = 2;
+        if (d.nb_cap[a] <= 3) break;
+        d.nb_cap[a] -= 1;
+    }
+    if ((long long)d.nb_cap[0] * d.nb_cap[1] * d.nb_cap[2] > d.nbins_max) return CFNEB_EINVAL;
+    return CFNEB_OK;
+}
+
 int capture_graph(cfneb *h) {
     CK(cudaStreamBeginCapture(h->st, cudaStreamCaptureModeRelaxed));
     enqueue_step(h, nullptr);
@@ -313,28 +342,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     d.pressure = prm->pressure;
     d.r_cut = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
     d.r_list = d.r_cut + d.skin;
-    memcpy(d.h0, cell_init, sizeof d.h0);  // A7: reference cell = cell of the initial endpoint
-    inv3(d.h0, d.h0inv);
-    // A13: lam = 0 selects Omega0^(1/3) N^(1/6); lam = 1 is the paper's equations literally
-    d.lam = prm->cell_factor > 0.0 ? prm->cell_factor : cbrt(fabs(vol0)) * pow((double)n_atoms, 1.0 / 6.0);
-    {  // per-axis bin caps from the larger endpoint cell, with headroom; product <= nbins_max
-        double w0[3], w1[3];
-        perp_widths(cell_init, w0);
-        perp_widths(cell_final, w1);
-        for (int a = 0; a < 3; ++a) {
-            const double w = fmax(w0[a], w1[a]) * 1.5;
-            d.nb_cap[a] = (int)floor(w / d.r_list);
-            if (d.nb_cap[a] < 3) d.nb_cap[a] = 3;
-        }
-        while ((long long)d.nb_cap[0] * d.nb_cap[1] * d.nb_cap[2] > d.nbins_max) {
-            int a = 0;
-            if (d.nb_cap[1] > d.nb_cap[a]) a = 1;
-            if (d.nb_cap[2] > d.nb_cap[a]) a = 2;
-            if (d.nb_cap[a] <= 3) break;
-            d.nb_cap[a] -= 1;
-        }
-        if ((long long)d.nb_cap[0] * d.nb_cap[1] * d.nb_cap[2] > d.nbins_max) { cfneb_destroy(h); return CFNEB_EINVAL; }
-    }
+    if (set_reference_frame(h, cell_init, cell_final) != CFNEB_OK) { cfneb_destroy(h); return CFNEB_EINVAL; }
     h->P = n_images;
     h->order.resize(n_images);
     for (int p = 0; p < n_images; ++p) h->order[p] = p;
@@ -519,6 +527,77 @@ int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, in
         if (n_ins) *n_ins = 1;
     }
     return sync_status(h);
+}
+
+int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_t rebuild_band, int32_t *steps_done,
+                          double *fmax_out, double *energy_out) {
+    if (!h || !(fmax_tol >= 0.0) || max_steps < 0) return CFNEB_EINVAL;
+    const Dev &d = h->d;
+    cudaStream_t st = h->st;
+    launch_relax_init(d, st);
+    RelaxState rs[2];
+    memset(rs, 0, sizeof rs);
+    int done = 0;
+    const int chunk = 20;
+    while (done < max_steps) {
+        const int n = std::min(chunk, max_steps - done);
+        for (int k = 0; k < n; ++k) {
+            launch_cell_prep(d, kEndpointsOnly, MODE_STEP, st);
+            launch_neighbor_build(d, kEndpointsOnly, st);
+            launch_force(d, kEndpointsOnly, st);
+            launch_finalize(d, kEndpointsOnly, st);
+            launch_relax_step(d, fmax_tol, st);
+        }
+        done += n;
+        CK(cudaMemcpyAsync(rs, d.relax, sizeof rs, cudaMemcpyDeviceToHost, st));
+        int rc = sync_status(h);
+        if (rc) return rc;
+        if (rs[0].frozen && rs[1].frozen) break;
+    }
+    // energies / forces of the final endpoint states (the last update may have moved them)
+    launch_cell_prep(d, kEndpointsOnly, MODE_STEP, st);
+    launch_neighbor_build(d, kEndpointsOnly, st);
+    launch_force(d, kEndpointsOnly, st);
+    launch_finalize(d, kEndpointsOnly, st);
+    launch_relax_step(d, 1e300, st);  // tol = inf: measures fmax and E, freezes, moves nothing
+    CK(cudaMemcpyAsync(rs, d.relax, sizeof rs, cudaMemcpyDeviceToHost, st));
+    int rc = sync_status(h);
+    if (rc) return rc;
+    for (int e = 0; e < 2; ++e) {
+        if (steps_done) steps_done[e] = rs[e].steps;
+        if (fmax_out) fmax_out[e] = rs[e].fmax;
+        if (energy_out) energy_out[e] = rs[e].E;
+    }
+    launch_relax_init(d, st);  // endpoint velocities back to zero
+    if (!rebuild_band) {
+        launch_reset_fire(d, st);
+        return sync_status(h);
+    }
+    // rebuild the band from the relaxed endpoints exactly as cfneb_create(endpoints only) would:
+    // h0 := relaxed cell of image 0 (A7), lam (A13), interior images linear in X, fresh lists, new graph
+    const size_t N3 = (size_t)d.N * 3, P = h->P;
+    double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3, *dE = dcell + P * 9;
+    launch_cell_prep(d, 0, MODE_GEOMETRY_ONLY, st);
+    launch_export_path(d, dpos, dcell, dE, st);
+    double cell0[9], cell1[9];
+    CK(cudaMemcpyAsync(cell0, dcell, sizeof cell0, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(cell1, dcell + (P - 1) * 9, sizeof cell1, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (h->exec) { cudaGraphExecDestroy(h->exec); h->exec = nullptr; }
+    if (h->graph) { cudaGraphDestroy(h->graph); h->graph = nullptr; }
+    rc = set_reference_frame(h, cell0, cell1);
+    if (rc) return rc;
+    // the exported Cartesian endpoints sit in the first half of the scratch area; input_map reads them there
+    launch_input_map(h->d, dpos, dcell, 0, 1, st);
+    launch_input_map(h->d, dpos + (P - 1) * N3, dcell + (P - 1) * 9, (int)P - 1, 1, st);
+    launch_interpolate(h->d, (int)P, st);
+    launch_reset_fire(h->d, st);
+    rc = force_rebuild_all(h);
+    if (rc) return rc;
+    enqueue_evaluate_all(h);
+    rc = sync_status(h);
+    if (rc) return rc;
+    return capture_graph(h);
 }
 
 int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, double *energies) {

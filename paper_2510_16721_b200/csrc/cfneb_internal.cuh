@@ -52,6 +52,14 @@ struct Ctl {
     double barrier, path_length;
 };
 
+// FIRE state of one endpoint during cfneb_relax_endpoints (kernels_relax.cu); device resident.
+struct RelaxState {
+    double dt, alpha;
+    double cv, cf, sdt;   // v_new = cv v + cf G ; X_new = X + sdt v_new
+    double fmax, E;       // max row norm of G and energy at the last evaluation
+    int n_pos, first, frozen, steps;
+};
+
 // Per-slot geometry written by K0.
 struct Geom {
     double D[9], Dinv[9], h[9], Dlast[9];
@@ -91,6 +99,8 @@ struct Dev {
     double *E, *V, *Gc;       // [S], [S][9], [S][9]
     double *dots, *coef;      // [S][10], [S][4]
     double *part_force;       // [S][nblk_atom][8]
+    RelaxState *relax;        // [2]
+    double *part_relax;       // [2][nblk_stream][4]
     double *part_dots;        // [S][nblk_stream][10]  (the first nblk_red rows of an image are used)
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
     int *nbr_count;           // [S][Npad]
@@ -132,6 +142,16 @@ __host__ __device__ inline void mul3_atb(const double *a, const double *b, doubl
 // launch modes
 enum { MODE_STEP = 0, MODE_GEOMETRY_ONLY = 1 };
 
+// Image selection of the per-image kernels: p_lo = 1 the movable images 1..P-2, p_lo = 0 all images,
+// p_lo = kEndpointsOnly the two endpoints (endpoint relaxation).  y = the block's image coordinate.
+constexpr int kEndpointsOnly = -1;
+__device__ inline bool image_of(int y, int p_lo, int P, int &p) {
+    if (p_lo == kEndpointsOnly) { p = y ? P - 1 : 0; return y < 2; }
+    p = y + p_lo;
+    return p <= P - 1 - p_lo;
+}
+inline int images_in_grid(int S, int p_lo) { return p_lo == kEndpointsOnly ? 2 : S - 2 * p_lo; }
+
 // ---- launch wrappers (each enqueues on `st`; p_lo = 1: movable images, 0: all images) ----
 void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_dev, int p_first, int count, cudaStream_t st);
 void launch_interpolate(const Dev &d, int P, cudaStream_t st);
@@ -146,6 +166,8 @@ void launch_update(const Dev &d, cudaStream_t st);                              
 void launch_materialize_fneb(const Dev &d, cudaStream_t st);                              // parity hook
 void launch_midpoint(const Dev &d, int slot_a, int slot_b, int slot_new, cudaStream_t st);  // K7
 void launch_reset_fire(const Dev &d, cudaStream_t st);
+void launch_relax_init(const Dev &d, cudaStream_t st);                                    // endpoint relaxation
+void launch_relax_step(const Dev &d, double fmax_tol, cudaStream_t st);
 void launch_segment_lengths(const Dev &d, double *out_dev, cudaStream_t st);
 void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_out, int *shift_out, cudaStream_t st);
 void launch_export_path(const Dev &d, double *pos_out, double *cells_out, double *E_out, cudaStream_t st);

@@ -118,9 +118,9 @@ __global__ void interpolate_kernel(Dev d, int P) {
 // K0: per image, D = sqrt(B), D^-1, h = h0 D, Omega; staleness bound of the neighbour list and the
 // rebuild decision; zeroes the bin counters of images that rebuild.
 __global__ void cell_prep_kernel(Dev d, int p_lo, int mode) {
-    const int p = blockIdx.x + p_lo;
     const int P = d.ctl->P;
-    if (p > P - 1 - p_lo) return;
+    int p;
+    if (!image_of(blockIdx.x, p_lo, P, p)) return;
     const int slot = d.order[p];
     Geom *g = d.geom + slot;
     __shared__ int s_rebuild, s_nbins;
@@ -184,8 +184,8 @@ __global__ void cell_prep_kernel(Dev d, int p_lo, int mode) {
 // Cartesian positions Rc = R~ D (one 32-byte sector per atom); when the slot rebuilds its list also
 // wrapped fractional coordinates s = R~ h0^-1 (image independent, Eq. 10), bin index and bin population.
 __global__ void __launch_bounds__(kThreadsAtom) positions_kernel(Dev d, int p_lo, int mode) {
-    const int p = blockIdx.y + p_lo;
-    if (p > d.ctl->P - 1 - p_lo) return;
+    int p;
+    if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= d.N) return;
@@ -241,7 +241,7 @@ void launch_interpolate(const Dev &d, int P, cudaStream_t st) {
 }
 
 void launch_cell_prep(const Dev &d, int p_lo, int mode, cudaStream_t st) {
-    const int nimg = d.S - 2 * p_lo;
+    const int nimg = images_in_grid(d.S, p_lo);
     cell_prep_kernel<<<nimg, 128, 0, st>>>(d, p_lo, mode);
     dim3 grid(d.nblk_atom, nimg);
     positions_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo, mode);

@@ -277,8 +277,8 @@ __device__ __forceinline__ void walk_list4(const uint32_t *__restrict__ lp, size
 // K2a (FS only): densities rho_i = sum_j psi(r_ij) over the Verlet list; writes F'(rho_i) into Rc[i].w and the
 // per-block embedding energy.
 __global__ void __launch_bounds__(kThreadsAtom, 4) density_kernel(Dev d, int p_lo) {
-    const int p = blockIdx.y + p_lo;
-    if (p > d.ctl->P - 1 - p_lo) return;
+    int p;
+    if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     __shared__ double sh[9];
     __shared__ double red[32];
@@ -348,8 +348,8 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) density_kernel(Dev d, int p_l
 // K2b: forces, energies and the virial over the Verlet list.
 template <int POT, bool SHARE>
 __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo) {
-    const int p = blockIdx.y + p_lo;
-    if (p > d.ctl->P - 1 - p_lo) return;
+    int p;
+    if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     constexpr bool FS = POT == CFNEB_POT_FS_MORSE;
     __shared__ double sh[9];
@@ -415,7 +415,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo)
 }
 
 void launch_force(const Dev &d, int p_lo, cudaStream_t st) {
-    const int nimg = d.S - 2 * p_lo;
+    const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
     if (d.potential == CFNEB_POT_LJ_SF) {

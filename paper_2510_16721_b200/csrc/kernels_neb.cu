@@ -91,9 +91,9 @@ __global__ void __launch_bounds__(kThreadsStream, MINB) reduce_kernel(Dev d) {
 // K4 second stage, one block per image: E, V from the force partials; G_cell (Eq. 17 / Eq. 14); the ten
 // dots completed with the three cell rows.  Fixed summation order (bitwise repeatable).
 __global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
-    const int p = blockIdx.x + p_lo;
     const int P = d.ctl->P;
-    if (p > P - 1 - p_lo) return;
+    int p;
+    if (!image_of(blockIdx.x, p_lo, P, p)) return;
     const int slot = d.order[p];
     __shared__ double red[32 * kNDots];
     __shared__ double sGc[9];
@@ -312,7 +312,7 @@ void plan_stream_grids(Dev &d) {
 }
 
 void launch_finalize(const Dev &d, int p_lo, cudaStream_t st) {
-    const int nimg = d.S - 2 * p_lo;
+    const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     finalize_kernel<<<nimg, 256, 0, st>>>(d, p_lo);
 }

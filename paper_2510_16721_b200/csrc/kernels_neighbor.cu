@@ -23,8 +23,8 @@
 namespace cfn {
 
 __device__ inline bool image_active(const Dev &d, int p_lo, int y, int &slot) {
-    const int p = y + p_lo;
-    if (p > d.ctl->P - 1 - p_lo) return false;
+    int p;
+    if (!image_of(y, p_lo, d.ctl->P, p)) return false;
     slot = d.order[p];
     return d.geom[slot].rebuild != 0;
 }
@@ -321,7 +321,7 @@ __global__ void unpack_neighbors_kernel(Dev d, int slot, int *count_out, int *li
 }
 
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st) {
-    const int nimg = d.S - 2 * p_lo;
+    const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     bin_scan_kernel<<<nimg, 1024, 0, st>>>(d, p_lo);
     dim3 ga(d.nblk_atom, nimg);

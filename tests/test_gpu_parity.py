@@ -449,3 +449,79 @@ def test_triclinic_disordered_band_with_unwrapped_atoms(dims, n_images):
     assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
     assert gpu.get_status().error == 0
     gpu.close()
+
+
+def _unrelaxed_endpoints(kind):
+    """Two unrelaxed end states: LJ vacancy hop off the stress-free lattice constant, or a noisy FS Bain pair."""
+    from cfneb_workloads import bain_endpoints, splitmix64_normals, vacancy_endpoints_unrelaxed
+    if kind == "lj":
+        spec = CONFIGS[0]
+        f0, cell, f1, _ = vacancy_endpoints_unrelaxed(2, 1.60)
+        return spec, f0 @ cell, cell, f1 @ cell, cell.copy()
+    spec = CONFIGS[2]
+    f0, c0, f1, c1 = bain_endpoints((3, 3, 4), 2.15, 1.05)
+    kick = splitmix64_normals(21, f0.size).reshape(f0.shape) * 0.03
+    return spec, f0 @ c0 + kick, c0, f1 @ c1 + kick, c1
+
+
+@pytest.mark.parametrize("kind", ["lj", "fs"])
+def test_relax_endpoints_follows_oracle_trajectory(kind):
+    """cfneb_relax_endpoints, 25 updates with no convergence stop: both endpoints follow the oracle's single-structure
+    cell-filter FIRE (final endpoint in the frame of the initial cell) step for step."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    spec, R0, h0, R1, h1 = _unrelaxed_endpoints(kind)
+    n = 25
+    kw = dict(fmax_tol=0.0, max_steps=n, cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=256)
+    Ra, ha, _, _, ita = oc.relax_endpoint(R0, h0, spec.potential, spec.pot, spec.r_cut, **kw)
+    Rb, hb, _, _, itb = oc.relax_endpoint(R1, h1, spec.potential, spec.pot, spec.r_cut, h_ref=h0, **kw)
+    gpu = cf.CFNEB(np.stack([R0, R1]), np.stack([h0, h1]), cf.params_for(spec, cell_factor=0.0, max_neighbors=256, max_images=5),
+                   n_images=5)
+    steps, fmax, en = gpu.relax_endpoints(0.0, n, rebuild_band=False)
+    assert steps == [n, n]
+    pos, cells, E = gpu.get_path()
+    assert rel(pos[0] - R0, Ra - R0) < 1e-8 and rel(cells[0] - h0, ha - h0) < 1e-8
+    assert rel(pos[-1] - R1, Rb - R1) < 1e-8 and rel(cells[-1] - h1, hb - h1) < 1e-8
+    assert np.max(np.abs(Ra - R0)) > 1e-3  # something moved
+    assert gpu.get_status().error == 0
+    gpu.close()
+
+
+def test_relax_endpoints_converges_and_rebuilds_the_band():
+    """To convergence (fmax < 1e-7): energies and update counts of both endpoints equal the oracle's; with
+    rebuild_band the band is the one cfneb_create would build from the relaxed endpoints (h0 = relaxed cell of
+    image 0, interior linear in X) and then steps with the oracle band built from the exported path."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    spec, R0, h0, R1, h1 = _unrelaxed_endpoints("lj")
+    tol = 1e-7
+    kw = dict(fmax_tol=tol, max_steps=4000, cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=256)
+    Ra, ha, Ea, fa, ita = oc.relax_endpoint(R0, h0, spec.potential, spec.pot, spec.r_cut, **kw)
+    Rb, hb, Eb, fb, itb = oc.relax_endpoint(R1, h1, spec.potential, spec.pot, spec.r_cut, h_ref=h0, **kw)
+    assert fa < tol and fb < tol
+    P = 7
+    gpu = cf.CFNEB(np.stack([R0, R1]), np.stack([h0, h1]), cf.params_for(spec, cell_factor=0.0, max_neighbors=256, max_images=P),
+                   n_images=P)
+    steps, fmax, en = gpu.relax_endpoints(tol, 4000, rebuild_band=True)
+    assert max(fmax) < tol
+    assert abs(steps[0] - ita) <= 1 and abs(steps[1] - itb) <= 1
+    assert abs(en[0] - Ea) < 1e-9 * abs(Ea) and abs(en[1] - Eb) < 1e-9 * abs(Eb)
+    pos, cells, E = gpu.get_path()
+    assert rel(pos[0], Ra) < 1e-7 and rel(cells[0], ha) < 1e-7 and rel(pos[-1], Rb) < 1e-7 and rel(cells[-1], hb) < 1e-7
+    X, v = gpu.get_state()
+    lam = gpu.get_status().cell_factor
+    assert abs(lam - oc.auto_cell_factor(cells[0], R0.shape[0])) < 1e-12 * lam      # lam from the relaxed cell (A13)
+    assert np.max(np.abs(X[0][-3:] - lam * np.eye(3))) < 1e-12 * lam                # image 0 is the reference: B = I
+    for p in range(1, P - 1):
+        t = p / (P - 1)
+        assert np.max(np.abs(X[p] - (X[0] + t * (X[-1] - X[0])))) < 1e-12 * np.max(np.abs(X[0]))
+    assert np.all(v == 0)
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=True, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=256)
+    X0, _ = orc.get_state()
+    assert rel(X, X0) < 1e-12
+    orc.step(4)
+    gpu.step(4)
+    assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
+    assert gpu.get_status().error == 0
+    gpu.close()
