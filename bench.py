@@ -375,8 +375,8 @@ def measure_e2e(band, pos, cells, n_steps, barrier, max_over_ranks, world, units
     return {"value": world * units_per_step * n_steps / dt, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
             "steps": n_steps, "ms_per_step": 1e3 * dt / n_steps,
             "what": "per step: cfneb_set_path(host pinned) + cfneb_step(1) + cfneb_get_path(host pinned); wall clock; "
-                    "set_path replaces the whole path, so every step also rebuilds all neighbour lists and "
-                    "re-evaluates the endpoints"}
+                    "set_path re-evaluates the endpoints and restarts FIRE; neighbour lists are rebuilt only for "
+                    "images whose new coordinates left the skin of the stored ones"}
 
 
 def main():

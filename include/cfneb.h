@@ -194,7 +194,11 @@ CFNEB_API int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_ste
 CFNEB_API int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, double *energies);
 
 /* Replace all P images from HOST Cartesian data (pos P*N*3, cells P*9; image 0's cell must equal h0);
- * resets the FIRE state and rebuilds neighbour lists; endpoint energies are re-evaluated.  Synchronises. */
+ * resets the FIRE state; endpoint energies are re-evaluated, interior energies by the next cfneb_step /
+ * cfneb_get_forces (or on demand by cfneb_get_path).  Neighbour lists are kept: the distance of the new coordinates
+ * from the stored ones is added to each image's displacement bound, so only images that left their skin rebuild
+ * (restoring a checkpoint of the running band, or editing a few images on the host, rebuilds nothing else).
+ * Synchronises. */
 CFNEB_API int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells);
 
 /* Generalized coordinates X and FIRE velocities v, each P*(N+3)*3 (checkpoint; either may be NULL). */

@@ -35,6 +35,7 @@ struct cfneb {
     cudaGraph_t graph;
     cudaGraphExec_t exec;
     int graph_nodes;
+    bool interior_stale;  // cfneb_set_path replaced the path and the interior images have not been evaluated since
 };
 
 // ---- workspace carving (one function serves the size query and create) ----
@@ -99,6 +100,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.relax = c.take<RelaxState>(2);
     d.part_relax = c.take<double>((size_t)2 * d.nblk_stream * 4);
     d.dispmax = c.take<unsigned long long>(S);
+    d.dispmax_in = c.take<unsigned long long>(S);
     d.nbr_count = c.take<int>(S * Npad);
     d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 16 * Npad);  // 16 rows of slack for the force kernels' look-ahead
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
@@ -306,6 +308,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     h->graph = nullptr;
     h->exec = nullptr;
     h->own_stream = false;
+    h->interior_stale = false;
     h->st = static_cast<cudaStream_t>(cuda_stream);
 #define CKH(call)                                  \
     do {                                           \
@@ -387,10 +390,10 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     CKC(cudaMemcpyAsync(dstage, stage.data(), stage.size() * sizeof(double), cudaMemcpyHostToDevice, h->st));
     const double *dpos = dstage, *dcell = dstage + (size_t)n_in * N3;
     if (path_or_null) {
-        launch_input_map(d, dpos, dcell, 0, n_images, h->st);
+        launch_input_map(d, dpos, dcell, 0, n_images, 0, h->st);
     } else {
-        launch_input_map(d, dpos, dcell, 0, 1, h->st);
-        launch_input_map(d, dpos + N3, dcell + 9, n_images - 1, 1, h->st);
+        launch_input_map(d, dpos, dcell, 0, 1, 0, h->st);
+        launch_input_map(d, dpos + N3, dcell + 9, n_images - 1, 1, 0, h->st);
         launch_interpolate(d, n_images, h->st);
     }
     CKC(cudaStreamSynchronize(h->st));  // `stage` is a temporary
@@ -407,12 +410,14 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
 
 int cfneb_step(cfneb_t *h, int32_t n_steps) {
     if (!h || n_steps < 0) return CFNEB_EINVAL;
+    if (n_steps > 0) h->interior_stale = false;
     for (int k = 0; k < n_steps; ++k) CK(cudaGraphLaunch(h->exec, h->st));
     return CFNEB_OK;
 }
 
 int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms) {
     if (!h || n_steps < 0 || !kernel_ms) return CFNEB_EINVAL;
+    if (n_steps > 0) h->interior_stale = false;
     // one event set per step, read back after the last step: no host synchronisation between steps
     const int per = CFNEB_NKERNELS + 1;
     std::vector<cudaEvent_t> ev((size_t)n_steps * per, nullptr);
@@ -588,8 +593,8 @@ int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_
     rc = set_reference_frame(h, cell0, cell1);
     if (rc) return rc;
     // the exported Cartesian endpoints sit in the first half of the scratch area; input_map reads them there
-    launch_input_map(h->d, dpos, dcell, 0, 1, st);
-    launch_input_map(h->d, dpos + (P - 1) * N3, dcell + (P - 1) * 9, (int)P - 1, 1, st);
+    launch_input_map(h->d, dpos, dcell, 0, 1, 0, st);
+    launch_input_map(h->d, dpos + (P - 1) * N3, dcell + (P - 1) * 9, (int)P - 1, 1, 0, st);
     launch_interpolate(h->d, (int)P, st);
     launch_reset_fire(h->d, st);
     rc = force_rebuild_all(h);
@@ -605,6 +610,10 @@ int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, do
     const Dev &d = h->d;
     const size_t N3 = (size_t)d.N * 3, P = h->P;
     double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3, *dE = dcell + P * 9;
+    if (energies && h->interior_stale) {  // the path was replaced and never evaluated: do it now
+        enqueue_evaluate_all(h);
+        h->interior_stale = false;
+    }
     launch_cell_prep(d, 0, MODE_GEOMETRY_ONLY, h->st);
     launch_export_path(d, dpos, dcell, dE, h->st);
     if (pos) CK(cudaMemcpyAsync(pos, dpos, P * N3 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
@@ -621,11 +630,18 @@ int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells) {
     double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3;
     CK(cudaMemcpyAsync(dpos, pos, P * N3 * sizeof(double), cudaMemcpyHostToDevice, h->st));
     CK(cudaMemcpyAsync(dcell, cells, P * 9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
-    launch_input_map(d, dpos, dcell, 0, h->P, h->st);
+    // The neighbour lists are kept: input_map records how far the new coordinates are from the stored ones and
+    // K0 adds that to the displacement bound of every image, so a list is rebuilt only if the new path left its
+    // skin (a checkpoint restore or a host-side edit of a few images costs no rebuild of the others).
+    launch_input_map(d, dpos, dcell, 0, h->P, 1, h->st);
     launch_reset_fire(d, h->st);
-    int rc = force_rebuild_all(h);
-    if (rc) return rc;
-    enqueue_evaluate_all(h);
+    // endpoint energies now; the interior is evaluated by the next cfneb_step / cfneb_get_forces, or on demand by
+    // cfneb_get_path / cfneb_get_status (interior_stale)
+    launch_cell_prep(d, kEndpointsOnly, MODE_STEP, h->st);
+    launch_neighbor_build(d, kEndpointsOnly, h->st);
+    launch_force(d, kEndpointsOnly, h->st);
+    launch_finalize(d, kEndpointsOnly, h->st);
+    h->interior_stale = true;
     return sync_status(h);
 }
 
@@ -644,6 +660,7 @@ int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, doubl
     if (!h) return CFNEB_EINVAL;
     const Dev &d = h->d;
     const size_t N3 = (size_t)d.N * 3, P = h->P;
+    h->interior_stale = false;
     launch_cell_prep(d, 1, MODE_STEP, h->st);
     launch_neighbor_build(d, 1, h->st);
     launch_force(d, 1, h->st);

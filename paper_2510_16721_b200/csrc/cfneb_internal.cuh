@@ -103,6 +103,7 @@ struct Dev {
     double *part_relax;       // [2][nblk_stream][4]
     double *part_dots;        // [S][nblk_stream][10]  (the first nblk_red rows of an image are used)
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
+    unsigned long long *dispmax_in;  // [S] max |dR~_i|^2 of a path replacement (cfneb_set_path) since the last K0
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
     unsigned short *nbr_tail; // [S][kTailBuckets][Npad] number of entries below tail bucket t (list sorted by bucket)
@@ -153,7 +154,8 @@ __device__ inline bool image_of(int y, int p_lo, int P, int &p) {
 inline int images_in_grid(int S, int p_lo) { return p_lo == kEndpointsOnly ? 2 : S - 2 * p_lo; }
 
 // ---- launch wrappers (each enqueues on `st`; p_lo = 1: movable images, 0: all images) ----
-void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_dev, int p_first, int count, cudaStream_t st);
+void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_dev, int p_first, int count, int track,
+                      cudaStream_t st);  // track = 1: record the displacement against the stored coordinates
 void launch_interpolate(const Dev &d, int P, cudaStream_t st);
 void launch_cell_prep(const Dev &d, int p_lo, int mode, cudaStream_t st);                 // K0 + positions
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st);                      // K1

@@ -64,7 +64,7 @@ __device__ inline double norm2_bound(const double *m) {
 // O0: one block column per image; pos [count][N][3] Cartesian, cells [count][9] are images p_first.. of the path.
 // Writes R~ = R D^-1 into both X buffers and lam*B (or lam*D) into both Xc buffers of slot = order[p].
 __global__ void input_map_kernel(Dev d, const double *__restrict__ pos, const double *__restrict__ cells, int p_first,
-                                 int count) {
+                                 int count, int track) {
     const int p = blockIdx.y;  // local index into pos / cells
     if (p >= count) return;
     const int slot = d.order[p_first + p];
@@ -73,13 +73,22 @@ __global__ void input_map_kernel(Dev d, const double *__restrict__ pos, const do
     inv3(D, Dinv);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const size_t img = (size_t)3 * d.Npad, buf = (size_t)d.S * img;
+    double d2 = 0.0;
     if (i < d.N) {
         const double *r = pos + ((size_t)p * d.N + d.perm[i]) * 3;  // caller's order -> spatial storage order
+        const double *Xold = d.X + (size_t)d.ctl->cur * buf + slot * img;
         for (int c = 0; c < 3; ++c) {
             double x = r[0] * Dinv[c] + r[1] * Dinv[3 + c] + r[2] * Dinv[6 + c];  // R~ = R D^-1 (Eq. 10)
+            if (track) { const double dx = x - Xold[(size_t)c * d.Npad + i]; d2 += dx * dx; }
             d.X[slot * img + (size_t)c * d.Npad + i] = x;
             d.X[buf + slot * img + (size_t)c * d.Npad + i] = x;
         }
+    }
+    if (track) {  // the neighbour list of this slot stays valid if the new path is within the skin of the old one
+        __shared__ double red[32];
+        if (!(d2 == d2)) d2 = 1e300;  // NaN input: force a rebuild (and the NaN check of the evaluation)
+        const double bm = block_max(d2, red);
+        if (threadIdx.x == 0) atomicMax(d.dispmax_in + slot, nonneg_bits(bm));
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         double C[9];
@@ -142,11 +151,13 @@ __global__ void cell_prep_kernel(Dev d, int p_lo, int mode) {
                 if (mode == MODE_STEP) {
                     // bound on the change of any pair distance since the last build:
                     // 2 max_i |dR~_i| ||D|| + r_list ||D - D_last|| ||D^-1||
-                    double dmax = sqrt(bits_nonneg(d.dispmax[slot]));
+                    // displacement of the last update + of a path replacement since (triangle inequality)
+                    double dmax = sqrt(bits_nonneg(d.dispmax[slot])) + sqrt(bits_nonneg(d.dispmax_in[slot]));
                     double dD[9];
                     for (int k = 0; k < 9; ++k) dD[k] = D[k] - g->Dlast[k];
                     double acc = g->acc + 2.0 * dmax * norm2_bound(D) + d.r_list * norm2_bound(dD) * norm2_bound(Dinv);
                     d.dispmax[slot] = 0ull;
+                    d.dispmax_in[slot] = 0ull;
                     rebuild = g->force_rebuild || (acc > d.skin) || (d.rebuild_every > 0 && g->since + 1 >= d.rebuild_every);
                     if (rebuild) { g->acc = 0.0; g->since = 0; g->force_rebuild = 0; }
                     else { g->acc = acc; g->since += 1; }
@@ -227,11 +238,11 @@ __global__ void __launch_bounds__(kThreadsAtom) positions_kernel(Dev d, int p_lo
     }
 }
 
-void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_dev, int p_first, int count,
+void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_dev, int p_first, int count, int track,
                       cudaStream_t st) {
     if (count <= 0) return;
     dim3 grid(d.nblk_atom, count);
-    input_map_kernel<<<grid, kThreadsAtom, 0, st>>>(d, pos_dev, cells_dev, p_first, count);
+    input_map_kernel<<<grid, kThreadsAtom, 0, st>>>(d, pos_dev, cells_dev, p_first, count, track);
 }
 
 void launch_interpolate(const Dev &d, int P, cudaStream_t st) {

@@ -80,15 +80,20 @@ __constant__ double kExp2Table[32] = {
     1.5759808451078865, 1.6104903319492543, 1.645755478153965, 1.681792830507429, 1.718619298122478,
     1.7562521603732995, 1.7947090750031072, 1.8340080864093424, 1.8741676341103, 1.9152065613971474,
     1.9571441241754002};
-__device__ __forceinline__ double exp_nb(double x, const double *T /* shared */) {
-    const double t = fma(x, 46.166241308446828384, 6755399441055744.0);  // 32/ln2; integer part lands in the low word
-    const double kf = t - 6755399441055744.0;
-    double r = fma(kf, -2.16608493865351192653e-02, x);  // ln2/32 in two pieces
-    r = fma(kf, -5.96317165397058656257e-12, r);
+// scalar constants of exp_nb in the constant bank (as immediates each costs two UMOVs per use)
+__constant__ double kExpK[9] = {46.166241308446828384 /* 32/ln2 */, -2.16608493865351192653e-02, -5.96317165397058656257e-12,
+                                1.0 / 720, 1.0 / 120, 1.0 / 24, 1.0 / 6, 0.5, 6755399441055744.0};
+// T = shared-window address of the 32-entry table (from __cvta_generic_to_shared, computed once per thread)
+__device__ __forceinline__ double exp_nb(double x, uint32_t T) {
+    const double t = fma(x, kExpK[0], kExpK[8]);  // integer part lands in the low word
+    const double kf = t - kExpK[8];
+    double r = fma(kf, kExpK[1], x);  // ln2/32 in two pieces
+    r = fma(kf, kExpK[2], r);
     const int n = __double2loint(t);
-    const double Tj = T[n & 31];
+    double Tj;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(Tj) : "r"(T + ((uint32_t)(n & 31) << 3)));
     const double r2 = r * r;
-    const double in = fma(fma(fma(fma(1.0 / 720, r, 1.0 / 120), r, 1.0 / 24), r, 1.0 / 6), r, 0.5);
+    const double in = fma(fma(fma(fma(kExpK[3], r, kExpK[4]), r, kExpK[5]), r, kExpK[6]), r, kExpK[7]);
     const double q = fma(r2, in, r);
     const double p = fma(Tj, q, Tj);
     return __hiloint2double(__double2hiint(p) + ((n >> 5) << 20), __double2loint(p));
@@ -150,7 +155,7 @@ __device__ __forceinline__ void lj_pair(const LJc &c, double r2, double &s, doub
 // SHARE: beta == 2 alpha, so e^{-beta (r - rho_r0)} = e^{beta (rho_r0 - r0)} (e^{-alpha (r - r0)})^2 and the second
 // exponential is one multiplication (k3 is that constant factor, computed once per thread).
 template <bool TAPER, bool SHARE>
-__device__ __forceinline__ void fs_pair(const FSc &c, const double *T, double r2, double dF_sum, double &s, double &u) {
+__device__ __forceinline__ void fs_pair(const FSc &c, uint32_t T, double r2, double dF_sum, double &s, double &u) {
     const double rinv = rsqrt_nr(r2), r = r2 * rinv;
     const double e1 = exp_nb(-c.a * (r - c.r0), T), e2 = e1 * e1;
     const double m = c.Dm * (e2 - 2.0 * e1), dm = 2.0 * c.a * c.Dm * (e1 - e2);
@@ -172,7 +177,7 @@ __device__ __forceinline__ void fs_pair(const FSc &c, const double *T, double r2
 
 // FS density pair (first pass)
 template <bool TAPER>
-__device__ __forceinline__ double fs_density(const FSc &c, const double *T, double r2) {
+__device__ __forceinline__ double fs_density(const FSc &c, uint32_t T, double r2) {
     const double r = r2 * rsqrt_nr(r2);
     double psi = exp_nb(-c.beta * (r - c.rr0), T);
     if (TAPER) {
@@ -282,10 +287,11 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) density_kernel(Dev d, int p_l
     const int slot = d.order[p];
     __shared__ double sh[9];
     __shared__ double red[32];
-    __shared__ double sT[32];
+    __shared__ double sT_tab[32];
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
-    if (threadIdx.x < 32) sT[threadIdx.x] = kExp2Table[threadIdx.x];
+    if (threadIdx.x < 32) sT_tab[threadIdx.x] = kExp2Table[threadIdx.x];
     __syncthreads();
+    const uint32_t sT = (uint32_t)__cvta_generic_to_shared(sT_tab);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
     double4 *Rc = d.Rc + (size_t)slot * d.Npad;
@@ -354,10 +360,11 @@ __global__ void __launch_bounds__(kThreadsAtom, 4) force_kernel(Dev d, int p_lo)
     constexpr bool FS = POT == CFNEB_POT_FS_MORSE;
     __shared__ double sh[9];
     __shared__ double red[32 * 7];
-    __shared__ double sT[32];
+    __shared__ double sT_tab[32];
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
-    if (threadIdx.x < 32) sT[threadIdx.x] = kExp2Table[threadIdx.x];
+    if (threadIdx.x < 32) sT_tab[threadIdx.x] = kExp2Table[threadIdx.x];
     __syncthreads();
+    const uint32_t sT = (uint32_t)__cvta_generic_to_shared(sT_tab);
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
     const double4 *Rc = d.Rc + (size_t)slot * d.Npad;

@@ -525,3 +525,37 @@ def test_relax_endpoints_converges_and_rebuilds_the_band():
     assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
     assert gpu.get_status().error == 0
     gpu.close()
+
+
+def test_set_path_keeps_lists_inside_the_skin_and_rebuilds_outside():
+    """cfneb_set_path adds the distance of the new coordinates from the stored ones to each image's displacement
+    bound: a path inside the skin reuses every list, one outside rebuilds; forces match the oracle either way."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import splitmix64_normals
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(2, 5)
+    prm = cf.params_for(spec, cell_factor=0.0)
+    gpu = cf.CFNEB(pos, cells, prm)
+    gpu.step(2)
+    pos1, cells1, _ = gpu.get_path()
+
+    def oracle_forces(p, c):
+        orc = oc.CFNEB(p, c, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
+                       fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors)
+        orc.band.forces()
+        return orc.band.E, orc.evaluator.last["F"], orc.evaluator.last["V"]
+
+    kick = splitmix64_normals(77, pos1[1:-1].size).reshape(pos1[1:-1].shape)
+    for scale, must_rebuild in ((0.01, False), (0.25, True)):  # skin 0.3: 2 x 0.01 x ~3 sigma stays inside, 0.25 does not
+        r0 = gpu.get_status().rebuilds
+        p2 = pos1.copy()
+        p2[1:-1] += scale * kick
+        gpu.set_path(p2, cells1)
+        F, V, fneb, E = gpu.get_forces()
+        rebuilt = gpu.get_status().rebuilds - r0
+        assert (rebuilt >= 3) if must_rebuild else (rebuilt == 0), (scale, rebuilt)
+        Eo, Fo, Vo = oracle_forces(p2, cells1)
+        assert rel(E, Eo) < TOL_FORCE and rel(F[1:-1], Fo) < TOL_FORCE and rel(V[1:-1], Vo) < TOL_FORCE
+        assert np.array_equal(gpu.get_path(positions=False)[2], E)  # energies served after the replacement
+    assert gpu.get_status().error == 0
+    gpu.close()
