@@ -183,9 +183,9 @@ void enqueue_step(cfneb *h, cudaEvent_t *ev) {
     launch_neighbor_build(d, 1, st);
     if (ev) cudaEventRecord(ev[2], st);
     launch_force(d, 1, st);
+    launch_finalize(d, 1, st);  // E, V, G_cell from the force partials: part of the force evaluation
     if (ev) cudaEventRecord(ev[3], st);
     launch_reduce(d, st);
-    launch_finalize(d, 1, st);
     if (ev) cudaEventRecord(ev[4], st);
     launch_scalar(d, 0, st);
     if (ev) cudaEventRecord(ev[5], st);
@@ -664,8 +664,8 @@ int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, doubl
     launch_cell_prep(d, 1, MODE_STEP, h->st);
     launch_neighbor_build(d, 1, h->st);
     launch_force(d, 1, h->st);
-    launch_reduce(d, h->st);
     launch_finalize(d, 1, h->st);
+    launch_reduce(d, h->st);
     launch_scalar(d, 1, h->st);
     launch_materialize_fneb(d, h->st);
     double *dF = static_cast<double *>(d.scratch), *dV = dF + P * N3, *dE = dV + P * 9;

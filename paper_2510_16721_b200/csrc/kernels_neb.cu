@@ -88,15 +88,14 @@ __global__ void __launch_bounds__(kThreadsStream, MINB) reduce_kernel(Dev d) {
     }
 }
 
-// K4 second stage, one block per image: E, V from the force partials; G_cell (Eq. 17 / Eq. 14); the ten
-// dots completed with the three cell rows.  Fixed summation order (bitwise repeatable).
+// Second stage of K2 / K3, one block per image: E, V from the force partials (+ the pressure terms);
+// G_cell (Eq. 17 / Eq. 14).  Fixed summation order (bitwise repeatable).  Does not depend on K4.
 __global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
     const int P = d.ctl->P;
     int p;
     if (!image_of(blockIdx.x, p_lo, P, p)) return;
     const int slot = d.order[p];
-    __shared__ double red[32 * kNDots];
-    __shared__ double sGc[9];
+    __shared__ double red[32 * kNForcePart];
     double a8[kNForcePart];
 #pragma unroll
     for (int q = 0; q < kNForcePart; ++q) a8[q] = 0.0;
@@ -123,51 +122,67 @@ __global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
         for (int k = 0; k < 9; ++k) {
             d.V[slot * 9 + k] = V[k];
             d.Gc[slot * 9 + k] = Gc[k];
-            sGc[k] = Gc[k];
         }
         if (!isfinite(E)) set_error(d.ctl, CFNEB_ENAN);
-    }
-    if (p < 1 || p > P - 2) return;  // endpoints: energy only (block-uniform)
-    __syncthreads();
-    double a10[kNDots];
-#pragma unroll
-    for (int q = 0; q < kNDots; ++q) a10[q] = 0.0;
-    const double *pd = d.part_dots + (size_t)slot * d.nblk_stream * kNDots;
-    for (int b = threadIdx.x; b < d.nblk_red; b += blockDim.x)
-#pragma unroll
-        for (int q = 0; q < kNDots; ++q) a10[q] += pd[(size_t)b * kNDots + q];
-    block_sum<kNDots>(a10, red);
-    if (threadIdx.x == 0) {
-        const int sm = d.order[p - 1], sp = d.order[p + 1];
-        const double *Xc = d.Xc + (size_t)d.ctl->cur * d.S * 9;
-        for (int k = 0; k < 9; ++k) {
-            const double tp = Xc[sp * 9 + k] - Xc[slot * 9 + k], tm = Xc[slot * 9 + k] - Xc[sm * 9 + k];
-            const double g = sGc[k], v = d.vc[slot * 9 + k];
-            a10[DOT_PP] += tp * tp; a10[DOT_MM] += tm * tm; a10[DOT_PM] += tp * tm;
-            a10[DOT_GP] += g * tp;  a10[DOT_GM] += g * tm;  a10[DOT_GG] += g * g;
-            a10[DOT_GV] += g * v;   a10[DOT_PV] += tp * v;  a10[DOT_MV] += tm * v;  a10[DOT_VV] += v * v;
-        }
-        for (int q = 0; q < kNDots; ++q) d.dots[slot * kNDots + q] = a10[q];
     }
 }
 
 // ------------------------------------------------------------------------------------------------
 // K5: one block.  Tangent weights and c1, c2 per image in parallel; band totals and the FIRE state
 // machine (O7: one state for the whole band, readings A1-A4) by thread 0 in path order.
-__global__ void __launch_bounds__(128) scalar_kernel(Dev d, int dry) {
+__global__ void __launch_bounds__(1024) scalar_kernel(Dev d, int dry) {
     Ctl *ctl = d.ctl;
     const int P = ctl->P;
     __shared__ int s_pstar;
-    if (threadIdx.x == 0) {
-        int ps = -1;
-        if (d.climb) {  // climbing image: argmax of interior energies, lowest index on an exact tie
-            double best = 0.0;
-            for (int p = 1; p <= P - 2; ++p) {
-                const double e = d.E[d.order[p]];
-                if (ps < 0 || e > best) { best = e; ps = p; }
+    {   // second stage of K4, one warp per image: the block partials of reduce_kernel summed in a fixed order
+        // (lane-strided, then a shuffle tree), completed with the three cell rows of the generalized vectors
+        const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+        const double *Xc = d.Xc + (size_t)ctl->cur * d.S * 9;
+        for (int p = 1 + warp; p <= P - 2; p += nwarp) {
+            const int slot = d.order[p];
+            double a10[kNDots];
+#pragma unroll
+            for (int q = 0; q < kNDots; ++q) a10[q] = 0.0;
+            const double *pd = d.part_dots + (size_t)slot * d.nblk_stream * kNDots;
+            for (int b = lane; b < d.nblk_red; b += 32)
+#pragma unroll
+                for (int q = 0; q < kNDots; ++q) a10[q] += pd[(size_t)b * kNDots + q];
+            if (lane < 9) {  // the nine cell components, one per lane
+                const int sm = d.order[p - 1], sp = d.order[p + 1], k = lane;
+                const double tp = Xc[sp * 9 + k] - Xc[slot * 9 + k], tm = Xc[slot * 9 + k] - Xc[sm * 9 + k];
+                const double g = d.Gc[slot * 9 + k], v = d.vc[slot * 9 + k];
+                a10[DOT_PP] += tp * tp; a10[DOT_MM] += tm * tm; a10[DOT_PM] += tp * tm;
+                a10[DOT_GP] += g * tp;  a10[DOT_GM] += g * tm;  a10[DOT_GG] += g * g;
+                a10[DOT_GV] += g * v;   a10[DOT_PV] += tp * v;  a10[DOT_MV] += tm * v;  a10[DOT_VV] += v * v;
             }
+#pragma unroll
+            for (int q = 0; q < kNDots; ++q)
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) a10[q] += __shfl_down_sync(0xffffffffu, a10[q], o);
+            if (lane == 0)
+                for (int q = 0; q < kNDots; ++q) d.dots[slot * kNDots + q] = a10[q];
         }
-        s_pstar = ps;
+        __syncthreads();
+    }
+    __shared__ int s_pmax;
+    if (threadIdx.x < 32) {  // argmax of the interior energies, lowest index on an exact tie: warp 0, lane-strided
+        const int lane = threadIdx.x;
+        int pb = -1;
+        double best = 0.0;
+        for (int p = 1 + lane; p <= P - 2; p += 32) {
+            const double e = d.E[d.order[p]];
+            if (pb < 0 || e > best) { best = e; pb = p; }
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double e2 = __shfl_down_sync(0xffffffffu, best, o);
+            const int p2 = __shfl_down_sync(0xffffffffu, pb, o);
+            if (p2 >= 0 && (pb < 0 || e2 > best || (e2 == best && p2 < pb))) { best = e2; pb = p2; }
+        }
+        if (lane == 0) {
+            s_pmax = pb;
+            s_pstar = d.climb ? pb : -1;  // climbing image (ref [12])
+        }
     }
     __syncthreads();
     const int pstar = s_pstar;
@@ -203,29 +218,34 @@ __global__ void __launch_bounds__(128) scalar_kernel(Dev d, int dry) {
                 2.0 * (c1 * dt[DOT_GP] + c2 * dt[DOT_GM] + c1 * c2 * dt[DOT_PM]);  // f . f
     }
     __syncthreads();
-    if (threadIdx.x != 0) return;
+    if (threadIdx.x >= 32) return;
+    // band totals: warp 0, lane-strided partial sums in path order, then a fixed shuffle tree
     double fv = 0.0, ff = 0.0, vv = 0.0, len = 0.0;
-    for (int p = 1; p <= P - 2; ++p) {
-        const int slot = d.order[p];
-        fv += d.coef[slot * 4 + 2];
-        ff += d.coef[slot * 4 + 3];
-        vv += d.dots[slot * kNDots + DOT_VV];
-        len += sqrt(d.dots[slot * kNDots + DOT_PP]);
-        if (p == 1) len += sqrt(d.dots[slot * kNDots + DOT_MM]);
+    {
+        const int lane = threadIdx.x;
+        for (int p = 1 + lane; p <= P - 2; p += 32) {
+            const int slot = d.order[p];
+            fv += d.coef[slot * 4 + 2];
+            ff += d.coef[slot * 4 + 3];
+            vv += d.dots[slot * kNDots + DOT_VV];
+            len += sqrt(d.dots[slot * kNDots + DOT_PP]);
+            if (p == 1) len += sqrt(d.dots[slot * kNDots + DOT_MM]);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            fv += __shfl_down_sync(0xffffffffu, fv, o);
+            ff += __shfl_down_sync(0xffffffffu, ff, o);
+            vv += __shfl_down_sync(0xffffffffu, vv, o);
+            len += __shfl_down_sync(0xffffffffu, len, o);
+        }
+        if (lane != 0) return;
     }
     if (ff < 0.0) ff = 0.0;  // round-off of the one-pass algebra near convergence
     if (!isfinite(fv) || !isfinite(ff) || !isfinite(vv)) set_error(ctl, CFNEB_ENAN);
     ctl->pstar = pstar;
     ctl->path_length = len;
     {
-        int pb = pstar;
-        if (pb < 0) {
-            double best = 0.0;
-            for (int p = 1; p <= P - 2; ++p) {
-                const double e = d.E[d.order[p]];
-                if (pb < 0 || e > best) { best = e; pb = p; }
-            }
-        }
+        const int pb = s_pmax;
         ctl->barrier = (pb > 0) ? d.E[d.order[pb]] - d.E[d.order[0]] : 0.0;
     }
     if (dry) return;
@@ -317,6 +337,6 @@ void launch_finalize(const Dev &d, int p_lo, cudaStream_t st) {
     finalize_kernel<<<nimg, 256, 0, st>>>(d, p_lo);
 }
 
-void launch_scalar(const Dev &d, int dry, cudaStream_t st) { scalar_kernel<<<1, 128, 0, st>>>(d, dry); }
+void launch_scalar(const Dev &d, int dry, cudaStream_t st) { scalar_kernel<<<1, 1024, 0, st>>>(d, dry); }
 
 }  // namespace cfn
