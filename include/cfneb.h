@@ -151,6 +151,15 @@ CFNEB_API int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_ini
  * synchronisation, no host<->device traffic. */
 CFNEB_API int cfneb_step(cfneb_t *h, int32_t n_steps);
 
+/*
+ * n_steps iterations with the adaptive control step O9 (the rule of cfneb_adapt, reading A16) decided and
+ * applied ON THE DEVICE after every adapt_every-th of them: segment lengths, at most one deletion and one midpoint
+ * insertion, order-table edit and FIRE restart are kernels on the handle's stream, so a run with adaptive images
+ * needs no host round trip either.  Asynchronous like cfneb_step; the host's view of P and of the order table is
+ * refreshed by the next call that needs it (cfneb_get_status reports the device's P).  adapt_every >= 1.
+ */
+CFNEB_API int cfneb_step_adaptive(cfneb_t *h, int32_t n_steps, int32_t adapt_every, double d_insert, double d_delete);
+
 /* Same iterations launched kernel by kernel with CUDA events between kernel classes; adds the
  * elapsed milliseconds per class, summed over the n_steps, to kernel_ms[CFNEB_NKERNELS] (HOST).
  * Synchronises.  For measurement only (bench.py roofline). */

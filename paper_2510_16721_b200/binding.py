@@ -18,7 +18,7 @@ K_CELLPREP, K_NEIGHBOR, K_FORCE, K_REDUCE, K_SCALAR, K_UPDATE, NKERNELS = 0, 1, 
 KERNEL_CLASSES = ("cell_prep", "neighbor", "force", "reduce", "scalar", "update")
 
 EXPORTS = (
-    "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_timed",
+    "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_adaptive", "cfneb_step_timed",
     "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
     "cfneb_get_path",
     "cfneb_set_path", "cfneb_get_state", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
@@ -83,7 +83,7 @@ def lib():
     L.cfneb_create.restype = ctypes.c_int
     L.cfneb_create.argtypes = [ctypes.POINTER(vp), i32, dp, dp, dp, dp, i32, dp, pp, vp, ctypes.c_size_t, vp]
     for name, args in (
-        ("cfneb_step", [vp, i32]), ("cfneb_step_timed", [vp, i32, dp]), ("cfneb_insert_image", [vp, i32]),
+        ("cfneb_step", [vp, i32]), ("cfneb_step_adaptive", [vp, i32, i32, f64, f64]), ("cfneb_step_timed", [vp, i32, dp]), ("cfneb_insert_image", [vp, i32]),
         ("cfneb_delete_image", [vp, i32]), ("cfneb_adapt", [vp, f64, f64, ip, ip]),
         ("cfneb_relax_endpoints", [vp, f64, i32, i32, ip, dp, dp]), ("cfneb_get_segment_lengths", [vp, dp]), ("cfneb_get_path", [vp, ip, dp, dp, dp]),
         ("cfneb_set_path", [vp, dp, dp]), ("cfneb_get_state", [vp, dp, dp]),
@@ -197,6 +197,13 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_step_timed")
         return ms
+
+    def step_adaptive(self, n, adapt_every, d_insert, d_delete):
+        """n iterations with the O9 control step taken on the device after every `adapt_every` of them; no
+        host synchronisation (cfneb_step_adaptive)."""
+        rc = lib().cfneb_step_adaptive(self._h, int(n), int(adapt_every), float(d_insert), float(d_delete))
+        if rc:
+            raise CfnebError(rc, "cfneb_step_adaptive")
 
     def synchronize(self):
         self._stream.synchronize()

@@ -35,6 +35,7 @@ struct cfneb {
     cudaGraph_t graph;
     cudaGraphExec_t exec;
     int graph_nodes;
+    bool mirror_dirty;    // the device edited P / order / free slots (cfneb_step_adaptive); host mirrors are stale
     bool interior_stale;  // cfneb_set_path replaced the path and the interior images have not been evaluated since
 };
 
@@ -79,6 +80,8 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     Carver c{static_cast<char *>(base), 0};
     d.ctl = c.take<Ctl>(1);
     d.order = c.take<int>(S);
+    d.free_stack = c.take<int>(S);
+    d.seglen = c.take<double>(S);
     d.perm = c.take<int>(Npad);
     d.geom = c.take<Geom>(S);
     d.X = c.take<double>(2 * S * img);
@@ -213,11 +216,32 @@ int force_rebuild_all(cfneb *h) {
 }
 
 int upload_order(cfneb *h) {
-    std::vector<int> full(h->d.S, 0);
+    std::vector<int> full(h->d.S, 0), fs(h->d.S, 0);
     for (int p = 0; p < h->P; ++p) full[p] = h->order[p];
+    const int n_free = (int)h->free_slots.size();
+    for (int k = 0; k < n_free; ++k) fs[k] = h->free_slots[k];
     CK(cudaMemcpyAsync(h->d.order, full.data(), sizeof(int) * h->d.S, cudaMemcpyHostToDevice, h->st));
+    CK(cudaMemcpyAsync(h->d.free_stack, fs.data(), sizeof(int) * h->d.S, cudaMemcpyHostToDevice, h->st));
     CK(cudaMemcpyAsync(&h->d.ctl->P, &h->P, sizeof(int), cudaMemcpyHostToDevice, h->st));
+    CK(cudaMemcpyAsync(&h->d.ctl->n_free, &n_free, sizeof(int), cudaMemcpyHostToDevice, h->st));
     CK(cudaStreamSynchronize(h->st));  // the host vectors above are temporaries
+    return CFNEB_OK;
+}
+
+// Host mirrors of P / order / free slots after the device edited them (cfneb_step_adaptive).  Synchronises.
+int sync_mirror(cfneb *h) {
+    if (!h->mirror_dirty) return CFNEB_OK;
+    Ctl c;
+    std::vector<int> ord(h->d.S), fs(h->d.S);
+    CK(cudaMemcpyAsync(&c, h->d.ctl, sizeof c, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaMemcpyAsync(ord.data(), h->d.order, sizeof(int) * h->d.S, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaMemcpyAsync(fs.data(), h->d.free_stack, sizeof(int) * h->d.S, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    if (c.P < 3 || c.P > h->d.S || c.n_free < 0 || c.n_free > h->d.S) return CFNEB_ERANGE;
+    h->P = c.P;
+    h->order.assign(ord.begin(), ord.begin() + c.P);
+    h->free_slots.assign(fs.begin(), fs.begin() + c.n_free);
+    h->mirror_dirty = false;
     return CFNEB_OK;
 }
 
@@ -309,6 +333,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     h->exec = nullptr;
     h->own_stream = false;
     h->interior_stale = false;
+    h->mirror_dirty = false;
     h->st = static_cast<cudaStream_t>(cuda_stream);
 #define CKH(call)                                  \
     do {                                           \
@@ -415,6 +440,20 @@ int cfneb_step(cfneb_t *h, int32_t n_steps) {
     return CFNEB_OK;
 }
 
+int cfneb_step_adaptive(cfneb_t *h, int32_t n_steps, int32_t adapt_every, double d_insert, double d_delete) {
+    if (!h || n_steps < 0 || adapt_every < 1) return CFNEB_EINVAL;
+    if (n_steps > 0) h->interior_stale = false;
+    for (int k = 1; k <= n_steps; ++k) {
+        CK(cudaGraphLaunch(h->exec, h->st));
+        if (k % adapt_every == 0) {
+            launch_adapt_device(h->d, d_insert, d_delete, h->st);
+            h->mirror_dirty = true;
+        }
+    }
+    CK(cudaGetLastError());
+    return CFNEB_OK;
+}
+
 int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms) {
     if (!h || n_steps < 0 || !kernel_ms) return CFNEB_EINVAL;
     if (n_steps > 0) h->interior_stale = false;
@@ -443,6 +482,7 @@ int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms) {
 
 int cfneb_insert_image(cfneb_t *h, int32_t after) {
     if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (after < 0 || after > h->P - 2) return CFNEB_ERANGE;
     if (h->P >= h->d.S || h->free_slots.empty()) return CFNEB_ERANGE;
     int pstar = -1;
@@ -467,6 +507,7 @@ int cfneb_insert_image(cfneb_t *h, int32_t after) {
 
 int cfneb_delete_image(cfneb_t *h, int32_t index) {
     if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (index < 1 || index > h->P - 2 || h->P <= 3) return CFNEB_ERANGE;
     int pstar = -1;
     CK(cudaMemcpyAsync(&pstar, &h->d.ctl->pstar, sizeof(int), cudaMemcpyDeviceToHost, h->st));
@@ -489,6 +530,7 @@ int cfneb_delete_image(cfneb_t *h, int32_t index) {
 
 int cfneb_get_segment_lengths(cfneb_t *h, double *dl) {
     if (!h || !dl) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     double *dev = static_cast<double *>(h->d.scratch);
     launch_segment_lengths(h->d, dev, h->st);
     CK(cudaMemcpyAsync(dl, dev, sizeof(double) * (h->P - 1), cudaMemcpyDeviceToHost, h->st));
@@ -497,6 +539,7 @@ int cfneb_get_segment_lengths(cfneb_t *h, double *dl) {
 
 int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, int32_t *n_del) {
     if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (n_ins) *n_ins = 0;
     if (n_del) *n_del = 0;
     std::vector<double> dl(h->d.S);
@@ -537,6 +580,7 @@ int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, in
 int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_t rebuild_band, int32_t *steps_done,
                           double *fmax_out, double *energy_out) {
     if (!h || !(fmax_tol >= 0.0) || max_steps < 0) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
     cudaStream_t st = h->st;
     launch_relax_init(d, st);
@@ -607,6 +651,7 @@ int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_
 
 int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, double *energies) {
     if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
     const size_t N3 = (size_t)d.N * 3, P = h->P;
     double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3, *dE = dcell + P * 9;
@@ -625,6 +670,7 @@ int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, do
 
 int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells) {
     if (!h || !pos || !cells) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
     const size_t N3 = (size_t)d.N * 3, P = h->P;
     double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3;
@@ -647,6 +693,7 @@ int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells) {
 
 int cfneb_get_state(cfneb_t *h, double *X, double *v) {
     if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
     const size_t n = (size_t)h->P * (d.N + 3) * 3;
     double *dX = static_cast<double *>(d.scratch), *dv = dX + n;
@@ -658,6 +705,7 @@ int cfneb_get_state(cfneb_t *h, double *X, double *v) {
 
 int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, double *energies) {
     if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
     const size_t N3 = (size_t)d.N * 3, P = h->P;
     h->interior_stale = false;
@@ -680,6 +728,7 @@ int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, doubl
 
 int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int32_t *list, int32_t *shift) {
     if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (image < 0 || image >= h->P) return CFNEB_ERANGE;
     const Dev &d = h->d;
     const int slot = h->order[image];

@@ -50,6 +50,11 @@ struct Ctl {
     double cv, cf, sdt;   // K6: v_new = cv v + cf f ; X_new = X + sdt v_new
     unsigned long long fmax_bits;  // max row norm^2 of f as ordered bits (atomicMax target)
     double barrier, path_length;
+    // device-side adaptive control (kernels_adapt.cu)
+    int n_free;                   // free-slot stack height (free_stack[0 .. n_free-1], top last)
+    int ins_a, ins_b, ins_new;    // slots of a pending midpoint insertion, ins_new < 0: none
+    int changed;                  // the last control step changed the band (FIRE restart pending)
+    int n_inserted, n_deleted;    // totals since create
 };
 
 // FIRE state of one endpoint during cfneb_relax_endpoints (kernels_relax.cu); device resident.
@@ -87,6 +92,8 @@ struct Dev {
     double h0[9], h0inv[9];
     Ctl *ctl;
     int *order;               // [S] path position -> slot
+    int *free_stack;          // [S] unused slots (device-side adaptive control)
+    double *seglen;           // [S] segment lengths of the last control step
     int *perm;                // [Npad] internal atom index -> caller's atom index (spatial order, see api.cu)
     Geom *geom;               // [S]
     double *X, *v, *F;        // see header comment
@@ -168,6 +175,7 @@ void launch_update(const Dev &d, cudaStream_t st);                              
 void launch_materialize_fneb(const Dev &d, cudaStream_t st);                              // parity hook
 void launch_midpoint(const Dev &d, int slot_a, int slot_b, int slot_new, cudaStream_t st);  // K7
 void launch_reset_fire(const Dev &d, cudaStream_t st);
+void launch_adapt_device(const Dev &d, double d_insert, double d_delete, cudaStream_t st);  // O9 on the device
 void launch_relax_init(const Dev &d, cudaStream_t st);                                    // endpoint relaxation
 void launch_relax_step(const Dev &d, double fmax_tol, cudaStream_t st);
 void launch_segment_lengths(const Dev &d, double *out_dev, cudaStream_t st);

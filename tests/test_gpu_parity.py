@@ -559,3 +559,45 @@ def test_set_path_keeps_lists_inside_the_skin_and_rebuilds_outside():
         assert np.array_equal(gpu.get_path(positions=False)[2], E)  # energies served after the replacement
     assert gpu.get_status().error == 0
     gpu.close()
+
+
+def test_device_side_adaptive_control_equals_host_side_and_oracle():
+    """cfneb_step_adaptive (O9 decided and applied by kernels, no host round trip) against the oracle's
+    `step(3); adapt()` loop and against the host-side cfneb_adapt on a second handle: same image counts, same
+    coordinates; afterwards host-side insert / delete still work on the refreshed mirrors."""
+    import paper_2510_16721_b200 as cf
+    spec, orc, gpu = make_pair(1, cell_factor=0.0, max_images=14)
+    _, _, host = make_pair(1, cell_factor=0.0, max_images=14)
+    orc.max_images = 14
+    L0 = float(np.sum(orc.band.segment_lengths()))
+    d_insert, d_delete = L0 / 10.0, L0 / 40.0   # the initial spacing L0/8 exceeds d_insert: the band grows
+    counts = []
+    for cycle in range(4):
+        orc.step(3)
+        counts.append(orc.adapt(d_insert, d_delete))
+        host.step(3)
+        assert host.adapt(d_insert, d_delete) == counts[-1]
+    gpu.step_adaptive(12, 3, d_insert, d_delete)     # one call, nothing read back in between
+    assert sum(c[0] for c in counts) > 0
+    assert gpu.P == orc.P == host.P
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    Xh, vh = host.get_state()
+    assert np.array_equal(Xg, Xh) and np.array_equal(vg, vh)       # device-side == host-side, bit for bit
+    assert rel(Xg, Xo) < 1e-11
+    # a deletion schedule too: thresholds that prune
+    d_insert2, d_delete2 = 10.0 * L0, 2.5 * L0 / (orc.P - 1)
+    orc.step(2)
+    co = orc.adapt(d_insert2, d_delete2)
+    gpu.step_adaptive(2, 2, d_insert2, d_delete2)
+    assert co == (0, 1) and gpu.P == orc.P
+    assert rel(gpu.get_state()[0], orc.get_state()[0]) < 1e-10
+    # host-side control on the refreshed mirrors
+    gpu.insert_image(0)
+    orc.insert_image(0)
+    gpu.step(2)
+    orc.step(2)
+    assert gpu.P == orc.P and rel(gpu.get_state()[0], orc.get_state()[0]) < 1e-9
+    assert gpu.get_status().error == 0
+    gpu.close()
+    host.close()
