@@ -370,6 +370,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     d.pressure = prm->pressure;
     d.r_cut = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
     d.r_list = d.r_cut + d.skin;
+    prepare_potential(d);
     if (set_reference_frame(h, cell_init, cell_final) != CFNEB_OK) { cfneb_destroy(h); return CFNEB_EINVAL; }
     h->P = n_images;
     h->order.resize(n_images);

@@ -85,6 +85,7 @@ struct Dev {
     int nblk_red, nblk_upd;   // K4 / K6: blocks per image, each striding over the image's nblk_stream tiles
     int nb_cap[3];
     double pot[12];
+    double potc[24];          // derived potential constants (kernels_force.cu: prepare_potential)
     double k_spring, lam;
     double pressure;          // external hydrostatic pressure (A25): E <- U + p Omega, V <- V - p Omega I in finalize_kernel
     double dt0, dtmax, maxstep, finc, fdec, astart, fa;
@@ -166,6 +167,7 @@ void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_d
 void launch_interpolate(const Dev &d, int P, cudaStream_t st);
 void launch_cell_prep(const Dev &d, int p_lo, int mode, cudaStream_t st);                 // K0 + positions
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st);                      // K1
+void prepare_potential(Dev &d);  // fills Dev::potc from pot / r_cut (host)
 void launch_force(const Dev &d, int p_lo, cudaStream_t st);                               // K2
 void launch_reduce(const Dev &d, cudaStream_t st);                                        // K4 (atom rows)
 void plan_stream_grids(Dev &d);  // nblk_red / nblk_upd from the SM count and the kernels' occupancy
