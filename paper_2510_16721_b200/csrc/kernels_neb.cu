@@ -24,8 +24,9 @@ __device__ inline void st2(double *p, double2 v) { *reinterpret_cast<double2 *>(
 // tile and loads of one block overlap the arithmetic of the others resident on the SM.  nblk_red is chosen so
 // that the grid fills an integer number of waves (plan_stream_grids).  Blocks of neighbouring images work on
 // the same tile index at about the same time, so X_{p-1} and X_{p+1} are L2 hits: DRAM sees X, F, v once (72 B).
-template <int MINB, int UNROLL>
-__global__ void __launch_bounds__(kThreadsStream, MINB) reduce_kernel(Dev d) {
+constexpr int kThreadsReduce = 256, kBlocksReduce = 2;  // measured at c4: 6.07 TB/s; <256,3> spills (4.9), <128,5> spills (5.0)
+template <int TR, int MINB, int UNROLL>
+__global__ void __launch_bounds__(TR, MINB) reduce_kernel(Dev d) {
     const int p = blockIdx.y + 1;
     if (p > d.ctl->P - 2) return;
     const int sm = d.order[p - 1], s0 = d.order[p], sp = d.order[p + 1];
@@ -40,14 +41,15 @@ __global__ void __launch_bounds__(kThreadsStream, MINB) reduce_kernel(Dev d) {
     double acc[kNDots];
 #pragma unroll
     for (int q = 0; q < kNDots; ++q) acc[q] = 0.0;
-    for (int tile = blockIdx.x; tile < d.nblk_stream; tile += UNROLL * gridDim.x) {
+    const int ntile = (d.Npad + 2 * TR - 1) / (2 * TR);
+    for (int tile = blockIdx.x; tile < ntile; tile += UNROLL * gridDim.x) {
         double2 f[UNROLL][3], xm[UNROLL][3], x0[UNROLL][3], xp[UNROLL][3], vv[UNROLL][3];
         bool on[UNROLL];
 #pragma unroll
         for (int u = 0; u < UNROLL; ++u) {
             const int t = tile + u * gridDim.x;
-            const int i = 2 * (t * kThreadsStream + threadIdx.x);
-            on[u] = t < d.nblk_stream && i < d.Npad;
+            const int i = 2 * (t * TR + threadIdx.x);
+            on[u] = t < ntile && i < d.Npad;
 #pragma unroll
             for (int c = 0; c < 3; ++c) {
                 const size_t o = (size_t)c * d.Npad + (on[u] ? i : 0);
@@ -297,7 +299,7 @@ __global__ void __launch_bounds__(1024) scalar_kernel(Dev d, int dry) {
 void launch_reduce(const Dev &d, cudaStream_t st) {
     if (d.S < 3) return;
     dim3 grid(d.nblk_red, d.S - 2);
-    reduce_kernel<2, 1><<<grid, kThreadsStream, 0, st>>>(d);
+    reduce_kernel<kThreadsReduce, kBlocksReduce, 1><<<grid, kThreadsReduce, 0, st>>>(d);
 }
 
 // Blocks per image for a streaming kernel that keeps `occ` blocks resident per SM: the smallest whole number
@@ -325,9 +327,10 @@ void plan_stream_grids(Dev &d) {
     if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     // measured on B200 at c4 (profiles/): reduce <2 blocks/SM, 1 tile in flight> 5.5 TB/s (114 registers, no spill;
     // <3, 1> spills and reaches 4.9, <2, 2> 4.8); update <3 blocks/SM> 6.2 TB/s (76 registers; <2> 5.9)
-    occ_r = 2;
+    occ_r = kBlocksReduce;
     occ_u = update_blocks_per_sm();
-    d.nblk_red = blocks_per_image(d.nblk_stream, d.S - 2, sms * occ_r);
+    d.nblk_red = blocks_per_image((d.Npad + 2 * kThreadsReduce - 1) / (2 * kThreadsReduce), d.S - 2, sms * occ_r);
+    if (d.nblk_red > d.nblk_stream) d.nblk_red = d.nblk_stream;  // part_dots holds nblk_stream rows per image
     d.nblk_upd = blocks_per_image(d.nblk_stream, d.S - 2, sms * occ_u);
 }
 
