@@ -12,7 +12,7 @@ images of the band.  metric = atom x image x NEB-steps per second, counted over 
              barrier + synchronize on both sides, max over ranks.
   roofline   the projection + FIRE kernels (K4 reduce + K6 update) the metric names: algorithmic bytes
              (192 B per atom-image-step) / their CUDA-event time per step, measured live by
-             cfneb_step_timed over K further steps of the same band; against MEASURED_PEAKS.json hbm_gbs.
+             cfneb_step_timed over min(K, 200) further steps of the same band; against MEASURED_PEAKS.json hbm_gbs.
              `kernels` carries every class's time share and the force kernel's fp64 "alu" fraction.
   e2e        the same metric through the C ABI with HOST (pinned) buffers: every step uploads the whole path
              (cfneb_set_path), runs one iteration (cfneb_step) and reads the path back (cfneb_get_path).
@@ -288,7 +288,8 @@ def main_ours(args):
     value = world * units_per_step * args.steps / (ms_total * 1e-3)
 
     # ---- per-kernel-class CUDA-event times over K further steps of the same band (roofline) ----
-    kms = band.step_timed(args.steps) / args.steps  # ms per step per class
+    n_bd = min(args.steps, 200)  # breakdown window: bounded, so that a long --steps run does not double its time
+    kms = band.step_timed(n_bd) / n_bd  # ms per step per class
     clocks = sampler.stop(t_wall0, time.time())
     peak, peak_src = measured_peaks()
     t_proj = (kms[cf.binding.K_REDUCE] + kms[cf.binding.K_UPDATE]) * 1e-3

@@ -22,7 +22,11 @@ def improved_tangent(X_prev, X, X_next, E_prev, E, E_next):
     else:
         dmax = max(abs(E_next - E), abs(E_prev - E))
         dmin = min(abs(E_next - E), abs(E_prev - E))
-        if E_next > E_prev:
+        if dmax == 0.0:
+            # A26: E_prev == E == E_next exactly (three images at the bottom of one basin, which a long band of a
+            # perfect crystal produces): both weights vanish and ref [13] defines no tangent; take the bisector.
+            tau = tp + tm
+        elif E_next > E_prev:
             tau = tp * dmax + tm * dmin
         else:  # includes the tie E_next == E_prev
             tau = tp * dmin + tm * dmax

@@ -198,7 +198,8 @@ __global__ void __launch_bounds__(1024) scalar_kernel(Dev d, int dry) {
         else {
             const double dp = fabs(Ep - E0), dm = fabs(Em - E0);
             const double dmax = fmax(dp, dm), dmin = fmin(dp, dm);
-            if (Ep > Em) { a = dmax; b = dmin; } else { a = dmin; b = dmax; }
+            if (dmax == 0.0) { a = 1.0; b = 1.0; }  // A26: three equal energies, the weights vanish: bisector
+            else if (Ep > Em) { a = dmax; b = dmin; } else { a = dmin; b = dmax; }
         }
         const double t2 = a * a * dt[DOT_PP] + 2.0 * a * b * dt[DOT_PM] + b * b * dt[DOT_MM];
         double c1 = 0.0, c2 = 0.0;

@@ -142,3 +142,22 @@ def test_c3_adaptive_band_follows_oracle():
     assert rel(gpu.get_state()[0], orc.get_state()[0]) < 1e-10
     assert gpu.get_status().error == 0
     gpu.close()
+
+
+def test_c4_long_run_survives_equal_energy_images():
+    """A 100-image band of a perfect crystal parks several images at the bottom of the end basins; after ~960
+    iterations three consecutive energies agree to the last bit and the weights of the improved tangent vanish
+    (reading A26: bisector).  The run must go on: 1100 iterations, no device error, finite state, BJ.configs[4]'s
+    500-step throughput run well inside."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(4)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    gpu.step(1100)
+    st = gpu.get_status()
+    assert st.error == 0 and st.steps == 1100
+    assert np.isfinite(st.fmax) and np.isfinite(st.barrier)
+    E = gpu.get_path(positions=False)[2]
+    assert np.all(np.isfinite(E))
+    seg = gpu.get_segment_lengths()
+    assert seg.min() > 0.0
+    gpu.close()

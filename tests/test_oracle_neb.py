@@ -108,6 +108,13 @@ def test_improved_tangent_branches_and_continuity():
     t1 = improved_tangent(Xm, X, Xp, 0.0, 1.0 - e, 1.0)[0]  # monotone: tau+
     t2 = improved_tangent(Xm, X, Xp, 0.0, 1.0 + e, 1.0)[0]  # maximum with dEmin -> 0
     assert np.abs(t1 / np.linalg.norm(t1) - t2 / np.linalg.norm(t2)).max() < 1e-10
+    # A26: three exactly equal energies (the weights of ref [13] both vanish): the bisector, never a zero tangent;
+    # one equal neighbour is still the ordinary extremum branch with dEmin = 0
+    assert np.array_equal(improved_tangent(Xm, X, Xp, 1.0, 1.0, 1.0)[0], tp + tm)
+    assert np.allclose(improved_tangent(Xm, X, Xp, 1.0, 1.0, 0.5)[0], tm * 0.5)
+    assert np.allclose(improved_tangent(Xm, X, Xp, 0.5, 1.0, 1.0)[0], tp * 0.5)
+    f = neb_force(rng.standard_normal((4, 3)), *improved_tangent(Xm, X, Xp, 1.0, 1.0, 1.0), 1.0, climbing=False)
+    assert np.all(np.isfinite(f))
 
 
 # ---------- Eq. 1 ----------
