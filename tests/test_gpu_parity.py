@@ -601,3 +601,31 @@ def test_device_side_adaptive_control_equals_host_side_and_oracle():
     assert gpu.get_status().error == 0
     gpu.close()
     host.close()
+
+
+def test_c2_converged_bain_barrier_equals_closed_form_saddle():
+    """configs[2] (2048 atoms x 16 images) run to fmax < 1e-6 on the device: the barrier is N times the saddle height of
+    the closed-form surface E(a, c) (tests/bain_surface.py) -- 252.6056 eV -- to BASELINE.json's 1e-4 eV."""
+    import paper_2510_16721_b200 as cf
+    from bain_surface import energy_per_atom, saddle
+    from cfneb_workloads import load_lattice_constants
+    spec, pos, cells = build_workload(2)
+    N = pos.shape[1]
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    for _ in range(40):
+        gpu.step(100)
+        if gpu.get_status().fmax < 1e-6:
+            break
+    st = gpu.get_status()
+    assert st.error == 0 and st.fmax < 1e-6
+    P_, C_, E_ = gpu.get_path()
+    a_bcc = load_lattice_constants()["fs_bcc_a"]
+    e_bcc = energy_per_atom(a_bcc, a_bcc, spec.pot)
+    assert abs(E_[0] / N - e_bcc) < 1e-11
+    h = C_[st.climb_index] / np.array(spec.dims, dtype=np.float64)[:, None]
+    assert np.abs(h - np.diag(np.diag(h))).max() < 1e-8
+    a_s, c_s, e_s, eig = saddle(h[0, 0], h[2, 2], spec.pot)
+    assert eig[0] < 0.0 < eig[1]
+    assert abs(st.barrier - N * (e_s - e_bcc)) < 1e-4
+    assert abs(st.barrier - 252.6056) < 1e-3
+    gpu.close()

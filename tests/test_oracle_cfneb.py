@@ -167,3 +167,29 @@ def test_adaptive_control_structural_invariants(c0):
     assert neb.adapt(d_insert=1e9, d_delete=0.0) == (0, 0)
     neb.max_images = 7
     assert neb.adapt(d_insert=0.0, d_delete=0.0) == (0, 0)
+
+
+def test_bain_band_barrier_equals_the_saddle_of_the_closed_form_surface():
+    """Pin of the Bain bands (BASELINE.json configs[2-4]) and of the whole crystal machinery on the FS potential with
+    cell degrees of freedom: CI-NEB in the cell-filter coordinates, run to fmax < 1e-6 on a 54-atom cell, must stop
+    at the saddle of the two-variable lattice-sum surface E(a, c) (tests/bain_surface.py: no tangent, no projection,
+    no cell filter, no optimizer in it).  Barrier per atom to 1e-9; the same number holds for any supercell."""
+    from bain_surface import energy_per_atom, saddle
+    from cfneb_workloads import build_workload
+    spec, pos, cells = build_workload(2, 9, dims=(3, 3, 3))
+    N = pos.shape[1]
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=True, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=256)
+    fmax = orc.run(1e-6, 8000)
+    assert fmax < 1e-6
+    P_, C_, E_ = orc.get_path()
+    a_bcc = load_lattice_constants()["fs_bcc_a"]
+    e_bcc = energy_per_atom(a_bcc, a_bcc, spec.pot)
+    assert abs(E_[0] / N - e_bcc) < 1e-12                           # endpoint energy = the lattice sum
+    h = C_[orc.band.pstar] / 3.0                                    # climbing image, per conventional cell
+    assert np.abs(h - np.diag(np.diag(h))).max() < 1e-9 and abs(h[0, 0] - h[1, 1]) < 1e-9   # it stayed tetragonal
+    a_s, c_s, e_s, eig = saddle(h[0, 0], h[2, 2], spec.pot)
+    assert eig[0] < 0.0 < eig[1]                                     # first-order saddle of the surface
+    assert 1.0 < c_s / a_s < np.sqrt(2.0)
+    assert abs(orc.band.barrier / N - (e_s - e_bcc)) < 1e-9
+    assert 0.12 < e_s - e_bcc < 0.13
