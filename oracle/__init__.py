@@ -18,8 +18,7 @@ Modules
   cfneb.py                       the crystal band: O0-O9 put together, one `step()` = one CFNEB iteration
   mullerbrown.py                 analytic 2-D Mueller-Brown surface (pin for neb.py)
 
-Parity pins: see DESIGN.md §"Oracle pins".  Unpinned (stated here as required): the Bain-path
-configs (c2-c4) have no external barrier value -- "parity unpinned" beyond oracle-vs-GPU and the
-invariants; the adaptive insertion/deletion rule (O9) is a reading of P:128 with structural
-invariants only -- "parity unpinned".
+Parity pins: see DESIGN.md section 4.  The Bain-path bands (c2-c4) are pinned by the saddle of the closed-form
+lattice-sum surface E(a, c) (tests/bain_surface.py).  Unpinned (stated here as required): the adaptive
+insertion/deletion rule (O9) is a reading of P:128 with structural invariants only -- "parity unpinned".
 """
