@@ -629,3 +629,35 @@ def test_c2_converged_bain_barrier_equals_closed_form_saddle():
     assert abs(st.barrier - N * (e_s - e_bcc)) < 1e-4
     assert abs(st.barrier - 252.6056) < 1e-3
     gpu.close()
+
+
+@pytest.mark.parametrize("k,over", [(0, dict(skin=0.0)), (2, dict(skin=0.0)), (2, dict(rebuild_every=1)),
+                                    (2, dict(max_neighbors=144)), (2, dict(max_neighbors=145)),
+                                    (0, dict(max_neighbors=97, skin=0.05))])
+def test_list_parameters_at_their_edges(k, over):
+    """skin = 0 (r_list = r_cut: no tail buckets, a rebuild whenever anything moves), rebuild_every = 1, and a list
+    capacity that is odd or (for the FS band) exactly the largest neighbour count: same forces and steps as the oracle,
+    whose own lists use the same skin."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(k, 5 if k == 2 else None)
+    skin = over.get("skin", spec.skin)
+    cap_o = 256
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
+                   fire=spec.fire, skin=skin, max_neighbors=cap_o)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, **over))
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE and rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE and rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    X0, _ = orc.get_state()
+    orc.step(4)
+    gpu.step(4)
+    assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
+    st = gpu.get_status()
+    assert st.error == 0
+    if "max_neighbors" in over and k == 2:
+        assert st.max_neighbors_seen == 144                         # capacity exactly reached (144) or odd, one above (145)
+    if over.get("rebuild_every") == 1 or skin == 0.0:
+        assert st.rebuilds >= 4 * (pos.shape[0] - 2)
+    gpu.close()
