@@ -104,6 +104,8 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.part_relax = c.take<double>((size_t)2 * d.nblk_stream * 4);
     d.dispmax = c.take<unsigned long long>(S);
     d.dispmax_in = c.take<unsigned long long>(S);
+    d.disptot = c.take<unsigned long long>(S);
+    d.Xb = c.take<double>(S * img);
     d.nbr_count = c.take<int>(S * Npad);
     d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 16 * Npad);  // 16 rows of slack for the force kernels' look-ahead
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);

@@ -67,9 +67,11 @@ struct RelaxState {
 
 // Per-slot geometry written by K0.
 struct Geom {
-    double D[9], Dinv[9], h[9], Dlast[9];
+    double D[9], Dinv[9], h[9];
+    double Dbuild[9];  // D when the neighbour list of this slot was built
+    double nDb, nDbinv; // spectral-norm bounds of Dbuild and of its inverse
     double vol;
-    double acc;        // accumulated bound on pair-distance change since the last list build
+    double acc;        // bound on the change of any pair distance since the last list build (K0, every step)
     int nb[3];         // bins per axis (>= 3: adjacent-bin stencil; 1: explicit periodic shifts)
     int reach[3];      // stencil half-width per axis
     int rebuild;       // this step rebuilds the list of this slot
@@ -111,6 +113,8 @@ struct Dev {
     double *part_relax;       // [2][nblk_stream][4]
     double *part_dots;        // [S][nblk_stream][10]  (the first nblk_red rows of an image are used)
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
+    unsigned long long *disptot;  // [S] max |R~_i - R~_i(build)|^2 at the last K0, as ordered bits
+    double *Xb;                   // [S][3][Npad] R~ at the last list build of each slot
     unsigned long long *dispmax_in;  // [S] max |dR~_i|^2 of a path replacement (cfneb_set_path) since the last K0
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale

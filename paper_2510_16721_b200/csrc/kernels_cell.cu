@@ -149,19 +149,34 @@ __global__ void cell_prep_kernel(Dev d, int p_lo, int mode) {
             if (ok) {
                 inv3(D, Dinv);
                 if (mode == MODE_STEP) {
-                    // bound on the change of any pair distance since the last build:
-                    // 2 max_i |dR~_i| ||D|| + r_list ||D - D_last|| ||D^-1||
-                    // displacement of the last update + of a path replacement since (triangle inequality)
-                    double dmax = sqrt(bits_nonneg(d.dispmax[slot])) + sqrt(bits_nonneg(d.dispmax_in[slot]));
+                    // Bound on the change of any pair distance since the list of this slot was built, for every pair
+                    // that was or is inside r_list (r = (dR~ + n h0) D):
+                    //   2 max_i |R~_i - R~_i(build)| max(||D||, ||Db||) + r_list ||D - Db|| max(||D^-1||, ||Db^-1||).
+                    // max_i |R~_i - R~_i(build)| was measured exactly by positions_kernel at the last K0 (disptot);
+                    // what moved since -- the last update (dispmax), a path replacement (dispmax_in) -- is added
+                    // by the triangle inequality.  Not cumulative: FIRE makes atoms oscillate, and the sum of per-step
+                    // maxima that this replaced was 6-16 times the true displacement at c4.
+                    const double dmax = sqrt(bits_nonneg(d.disptot[slot])) + sqrt(bits_nonneg(d.dispmax[slot])) +
+                                        sqrt(bits_nonneg(d.dispmax_in[slot]));
                     double dD[9];
-                    for (int k = 0; k < 9; ++k) dD[k] = D[k] - g->Dlast[k];
-                    double acc = g->acc + 2.0 * dmax * norm2_bound(D) + d.r_list * norm2_bound(dD) * norm2_bound(Dinv);
+                    for (int k = 0; k < 9; ++k) dD[k] = D[k] - g->Dbuild[k];
+                    const double nD = norm2_bound(D), nDinv = norm2_bound(Dinv);
+                    double acc = 2.0 * dmax * fmax(nD, g->nDb) + d.r_list * norm2_bound(dD) * fmax(nDinv, g->nDbinv);
                     d.dispmax[slot] = 0ull;
                     d.dispmax_in[slot] = 0ull;
-                    rebuild = g->force_rebuild || (acc > d.skin) || (d.rebuild_every > 0 && g->since + 1 >= d.rebuild_every);
-                    if (rebuild) { g->acc = 0.0; g->since = 0; g->force_rebuild = 0; }
-                    else { g->acc = acc; g->since += 1; }
-                    for (int k = 0; k < 9; ++k) g->Dlast[k] = D[k];
+                    d.disptot[slot] = 0ull;  // positions_kernel of this step measures it again
+                    rebuild = g->force_rebuild || !(acc <= d.skin) || (d.rebuild_every > 0 && g->since + 1 >= d.rebuild_every);
+                    if (rebuild) {
+                        acc = 0.0;
+                        g->since = 0;
+                        g->force_rebuild = 0;
+                        for (int k = 0; k < 9; ++k) g->Dbuild[k] = D[k];
+                        g->nDb = nD;
+                        g->nDbinv = nDinv;
+                    } else {
+                        g->since += 1;
+                    }
+                    g->acc = acc;
                 }
                 for (int k = 0; k < 9; ++k) { g->D[k] = D[k]; g->Dinv[k] = Dinv[k]; g->h[k] = h[k]; }
                 g->vol = vol;
@@ -199,8 +214,24 @@ __global__ void __launch_bounds__(kThreadsAtom) positions_kernel(Dev d, int p_lo
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= d.N) return;
     const Geom *g = d.geom + slot;
+    if (mode == MODE_STEP && !g->rebuild) {
+        // exact displacement of every atom from the coordinates its list was built at (K0 of the next step adds
+        // what the update in between moves); all threads of the block take part in the reduction
+        __shared__ double red[32];
+        double d2 = 0.0;
+        if (i < d.N) {
+            const double *Xc = d.X + ((size_t)d.ctl->cur * d.S + slot) * 3 * d.Npad;
+            const double *Xb = d.Xb + (size_t)slot * 3 * d.Npad;
+            const double ax = Xc[i] - Xb[i], ay = Xc[d.Npad + i] - Xb[d.Npad + i],
+                         az = Xc[2 * (size_t)d.Npad + i] - Xb[2 * (size_t)d.Npad + i];
+            d2 = ax * ax + ay * ay + az * az;
+            if (!(d2 == d2)) d2 = 1e300;
+        }
+        const double bm = block_max(d2, red);
+        if (threadIdx.x == 0) atomicMax(d.disptot + slot, nonneg_bits(bm));
+    }
+    if (i >= d.N) return;
     const double *X = d.X + ((size_t)d.ctl->cur * d.S + slot) * 3 * d.Npad;
     const double x = X[i], y = X[d.Npad + i], z = X[2 * (size_t)d.Npad + i];
     double4 r;
@@ -209,6 +240,10 @@ __global__ void __launch_bounds__(kThreadsAtom) positions_kernel(Dev d, int p_lo
     r.z = x * g->D[2] + y * g->D[5] + z * g->D[8];
     r.w = 0.0;
     d.Rc[(size_t)slot * d.Npad + i] = r;
+    if (mode == MODE_STEP && g->rebuild) {  // the list is built from these coordinates
+        double *Xb = d.Xb + (size_t)slot * 3 * d.Npad;
+        Xb[i] = x; Xb[d.Npad + i] = y; Xb[2 * (size_t)d.Npad + i] = z;
+    }
     if (mode == MODE_STEP && g->rebuild) {
         double s[3], sw[3];
         int fl[3], b[3];
