@@ -68,8 +68,7 @@ struct RelaxState {
 // Per-slot geometry written by K0.
 struct Geom {
     double D[9], Dinv[9], h[9];
-    double Dbuild[9];  // D when the neighbour list of this slot was built
-    double nDb, nDbinv; // spectral-norm bounds of Dbuild and of its inverse
+    double Dbinv[9];   // inverse of D at the time the neighbour list of this slot was built
     double vol;
     double acc;        // bound on the change of any pair distance since the last list build (K0, every step)
     int nb[3];         // bins per axis (>= 3: adjacent-bin stencil; 1: explicit periodic shifts)

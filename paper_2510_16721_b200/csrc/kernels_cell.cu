@@ -50,6 +50,37 @@ __device__ bool sqrt_spd3(const double *Bin, double *S) {
     return true;
 }
 
+// Smallest eigenvalue of a symmetric 3x3 matrix (cyclic Jacobi to convergence).
+__device__ double min_eig_sym3(const double *Cin) {
+    double A[9];
+    for (int i = 0; i < 3; ++i)
+        for (int j = 0; j < 3; ++j) A[3 * i + j] = 0.5 * (Cin[3 * i + j] + Cin[3 * j + i]);
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        const double off = A[1] * A[1] + A[2] * A[2] + A[5] * A[5];
+        const double dia = A[0] * A[0] + A[4] * A[4] + A[8] * A[8];
+        if (off <= 1e-33 * (dia + 2.0 * off) || off == 0.0) break;
+        for (int pq = 0; pq < 3; ++pq) {
+            const int p = (pq == 2) ? 1 : 0, q = (pq == 0) ? 1 : 2;
+            const double apq = A[3 * p + q];
+            if (apq == 0.0) continue;
+            const double theta = (A[3 * q + q] - A[3 * p + p]) / (2.0 * apq);
+            const double t = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
+            const double c = 1.0 / sqrt(t * t + 1.0), s = t * c;
+            for (int k = 0; k < 3; ++k) {
+                const double akp = A[3 * k + p], akq = A[3 * k + q];
+                A[3 * k + p] = c * akp - s * akq;
+                A[3 * k + q] = s * akp + c * akq;
+            }
+            for (int k = 0; k < 3; ++k) {
+                const double apk = A[3 * p + k], aqk = A[3 * q + k];
+                A[3 * p + k] = c * apk - s * aqk;
+                A[3 * q + k] = s * apk + c * aqk;
+            }
+        }
+    }
+    return fmin(A[0], fmin(A[4], A[8]));
+}
+
 // Upper bound of the spectral norm: ||m||_2 <= sqrt(||m||_1 ||m||_inf) (tight for the near-identity,
 // symmetric D of CELL_B, unlike the Frobenius norm).
 __device__ inline double norm2_bound(const double *m) {
@@ -149,19 +180,26 @@ __global__ void cell_prep_kernel(Dev d, int p_lo, int mode) {
             if (ok) {
                 inv3(D, Dinv);
                 if (mode == MODE_STEP) {
-                    // Bound on the change of any pair distance since the list of this slot was built, for every pair
-                    // that was or is inside r_list (r = (dR~ + n h0) D):
-                    //   2 max_i |R~_i - R~_i(build)| max(||D||, ||Db||) + r_list ||D - Db|| max(||D^-1||, ||Db^-1||).
-                    // max_i |R~_i - R~_i(build)| was measured exactly by positions_kernel at the last K0 (disptot);
-                    // what moved since -- the last update (dispmax), a path replacement (dispmax_in) -- is added
-                    // by the triangle inequality.  Not cumulative: FIRE makes atoms oscillate, and the sum of per-step
-                    // maxima that this replaced was 6-16 times the true displacement at c4.
+                    // How much closer than at the build any pair can be now.  With r = (dR~ + n h0) D, M = Db^-1 D and
+                    // d_i = R~_i - R~_i(build):   |r| >= sigma_min(M) |r_build| - 2 max_i |d_i| ||D||,   so a pair that
+                    // was outside r_list cannot be inside r_cut while
+                    //   acc = 2 max_i |d_i| ||D|| + r_list (1 - sigma_min(M))_+  <=  skin,
+                    // and a list entry built at r_build >= r_cut + acc is still outside r_cut (tail buckets of K2).
+                    // Only compression brings pairs in: an expanding or shearing cell costs nothing beyond
+                    // 1 - sigma_min (the norm ||D - Db|| used before was 2-3 x larger on the Bain band).
+                    // max_i |d_i| was measured exactly by positions_kernel at the last K0 (disptot); what moved since --
+                    // the last update (dispmax), a path replacement (dispmax_in) -- is added by the triangle inequality.
+                    // Not cumulative: FIRE makes atoms oscillate, and the sum of per-step maxima that this replaced was
+                    // 6-16 times the true displacement at c4.
                     const double dmax = sqrt(bits_nonneg(d.disptot[slot])) + sqrt(bits_nonneg(d.dispmax[slot])) +
                                         sqrt(bits_nonneg(d.dispmax_in[slot]));
-                    double dD[9];
-                    for (int k = 0; k < 9; ++k) dD[k] = D[k] - g->Dbuild[k];
-                    const double nD = norm2_bound(D), nDinv = norm2_bound(Dinv);
-                    double acc = 2.0 * dmax * fmax(nD, g->nDb) + d.r_list * norm2_bound(dD) * fmax(nDinv, g->nDbinv);
+                    double M[9], C[9];
+                    mul3(g->Dbinv, D, M);
+                    mul3_atb(M, M, C);  // M^T M
+                    const double lmin = min_eig_sym3(C);
+                    const double smin = lmin > 0.0 ? sqrt(lmin) : 0.0;
+                    const double shrink = 1.0 - smin;  // + a rounding allowance of the 3x3 arithmetic when it counts
+                    double acc = 2.0 * dmax * norm2_bound(D) + d.r_list * (shrink > 0.0 ? shrink * (1.0 + 1e-12) + 1e-14 : 0.0);
                     d.dispmax[slot] = 0ull;
                     d.dispmax_in[slot] = 0ull;
                     d.disptot[slot] = 0ull;  // positions_kernel of this step measures it again
@@ -170,9 +208,7 @@ __global__ void cell_prep_kernel(Dev d, int p_lo, int mode) {
                         acc = 0.0;
                         g->since = 0;
                         g->force_rebuild = 0;
-                        for (int k = 0; k < 9; ++k) g->Dbuild[k] = D[k];
-                        g->nDb = nD;
-                        g->nDbinv = nDinv;
+                        for (int k = 0; k < 9; ++k) g->Dbinv[k] = Dinv[k];
                     } else {
                         g->since += 1;
                     }
