@@ -661,3 +661,33 @@ def test_list_parameters_at_their_edges(k, over):
     if over.get("rebuild_every") == 1 or skin == 0.0:
         assert st.rebuilds >= 4 * (pos.shape[0] - 2)
     gpu.close()
+
+
+def test_list_reuse_under_compression_and_disorder_equals_fresh_lists():
+    """The staleness bound at work where it matters: a strongly disordered triclinic band under 80 GPa, whose cells
+    shrink by several per cent (pairs come inside r_cut that were outside r_list at the build) while atoms move by
+    more than the skin.  Reused lists must give the state that fresh lists (rebuild_every = 1) give, and the reuse
+    run must have rebuilt some lists on its own and skipped most."""
+    import paper_2510_16721_b200 as cf
+    spec = CONFIGS[2]
+    pos, cells = _triclinic_band((4, 4, 5), [[0, 0.05, -0.03], [0.02, 0, 0.06], [-0.04, 0.01, 0]], 0.12, 6, 5)
+    kw = dict(cell_factor=0.0, max_neighbors=256, max_images=6, pressure=0.5)
+    a = cf.CFNEB(pos, cells, cf.params_for(spec, **kw))
+    b = cf.CFNEB(pos, cells, cf.params_for(spec, rebuild_every=1, **kw))
+    vol0 = abs(np.linalg.det(a.get_path(positions=False)[1][2]))
+    n = 120
+    a.step(n)
+    b.step(n)
+    sa, sb = a.get_status(), b.get_status()
+    assert sa.error == 0 and sb.error == 0
+    movable = pos.shape[0] - 2
+    assert sb.rebuilds >= n * movable
+    assert 2 * movable < sa.rebuilds < sb.rebuilds // 3          # stale lists were detected, most steps reused theirs
+    Xa, Xb = a.get_state()[0], b.get_state()[0]
+    X0 = cf.CFNEB(pos, cells, cf.params_for(spec, **kw)).get_state()[0]
+    assert np.max(np.abs(Xa[:, :-3] - X0[:, :-3])) > spec.skin    # atoms moved by more than the skin
+    vol1 = abs(np.linalg.det(a.get_path(positions=False)[1][2]))
+    assert vol1 < 0.97 * vol0                                    # and the cell was compressed
+    assert rel(Xa - X0, Xb - X0) < 1e-9
+    a.close()
+    b.close()
