@@ -74,7 +74,7 @@ CONFIGS = [
     WorkloadSpec("c3_fs_bain_9826_adaptive", POT_FS_MORSE, fs_params(), "bcc_bain", (17, 17, 17), 9826, 12, 3,
                  fire=_FIRE_EV, n_steps=200, max_images=32, skin=0.3, max_neighbors=192),
     WorkloadSpec("c4_fs_bain_101306", POT_FS_MORSE, fs_params(), "bcc_bain", (37, 37, 37), 101306, 100, 4,
-                 fire=_FIRE_EV, n_steps=500, max_images=100, skin=0.3, max_neighbors=192),
+                 fire=_FIRE_EV, n_steps=500, max_images=100, skin=0.5, max_neighbors=224),
 ]
 
 
