@@ -29,6 +29,9 @@
 //        constant-bank coefficients.  The potential's constants and their products are precomputed on the
 //        host and read as constant-bank operands of the kernel parameter, which frees enough registers for
 //        five blocks (20 warps) per SM: 11.28 -> 10.93 ms at c4 (six blocks spill: 13.4 ms).
+//   Tried and dropped: the virial as sum_i R_i (x) F_i - 1/2 sum (n h) (x) f^ij (exact since f^ij = -f^ji bitwise;
+//   six FMAs and twelve registers per pair less).  Parity held, but one lane in ~14 has a shifted entry per
+//   iteration, so nearly every warp iteration took the shift branch: K2 3 % slower at c4.
 // Per-thread sums run in list order and block partials through a fixed tree: bitwise repeatable.
 #include "cfneb_internal.cuh"
 #include <math.h>
