@@ -32,6 +32,10 @@
 //   Tried and dropped: the virial as sum_i R_i (x) F_i - 1/2 sum (n h) (x) f^ij (exact since f^ij = -f^ji bitwise;
 //   six FMAs and twelve registers per pair less).  Parity held, but one lane in ~14 has a shifted entry per
 //   iteration, so nearly every warp iteration took the shift branch: K2 3 % slower at c4.
+//   Also tried and dropped: each list as an unshifted group (walked with no shift logic) followed by the entries
+//   with a periodic shift.  Parity held, K2 27 % slower: an atom near a cell face loses part of every shell to
+//   the second group, its k-th entry no longer lies in the shell of its warp neighbours, and the warp-level
+//   plain / taper dispatch degrades for the third of all atoms that sit within r_list of a face.
 // Per-thread sums run in list order and block partials through a fixed tree: bitwise repeatable.
 #include "cfneb_internal.cuh"
 #include <math.h>
