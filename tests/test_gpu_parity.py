@@ -691,3 +691,29 @@ def test_list_reuse_under_compression_and_disorder_equals_fresh_lists():
     assert rel(Xa - X0, Xb - X0) < 1e-9
     a.close()
     b.close()
+
+
+@pytest.mark.parametrize("beta,rho_r0", [(2.7, 2.3), (3.0, 2.1)])
+def test_fs_potential_with_general_density_exponent(beta, rho_r0):
+    """BASELINE.json's potential has beta = 2 alpha, for which the force kernel shares one exponential between the
+    pair and the density term; beta != 2 alpha takes the other template instance (two exponentials), and
+    beta = 2 alpha with rho_r0 != r0 exercises the constant factor of the shared form."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import fs_params
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(2, 5, dims=(4, 4, 4))
+    pot = fs_params(beta=beta, rho_r0=rho_r0)
+    orc = oc.CFNEB(pos, cells, spec.potential, pot, spec.r_cut, k_spring=spec.k_spring, climb=True, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, pot=list(pot)))
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE and rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE and rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    assert np.max(np.abs(orc.evaluator.last["F"])) > 1e-3     # off the stored lattice constant: real forces
+    X0, _ = orc.get_state()
+    orc.step(4)
+    gpu.step(4)
+    assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
+    assert gpu.get_status().error == 0
+    gpu.close()
