@@ -679,15 +679,17 @@ int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells) {
     double *dpos = static_cast<double *>(d.scratch), *dcell = dpos + P * N3;
     CK(cudaMemcpyAsync(dpos, pos, P * N3 * sizeof(double), cudaMemcpyHostToDevice, h->st));
     CK(cudaMemcpyAsync(dcell, cells, P * 9 * sizeof(double), cudaMemcpyHostToDevice, h->st));
-    // The neighbour lists are kept: input_map records how far the new coordinates are from the stored ones and
-    // K0 adds that to the displacement bound of every image, so a list is rebuilt only if the new path left its
-    // skin (a checkpoint restore or a host-side edit of a few images costs no rebuild of the others).
+    // The neighbour lists are kept: input_map records how far the new coordinates are from the stored ones, and the
+    // K0 pass over ALL images that follows adds that to every image's displacement bound, rebuilds the lists that
+    // left their skin and measures the exact displacement of the new path from the build-time coordinates -- so the
+    // bound never has to cover more than one replacement (a checkpoint restore or a host-side edit of a few images
+    // costs no rebuild of the others).
     launch_input_map(d, dpos, dcell, 0, h->P, 1, h->st);
     launch_reset_fire(d, h->st);
+    launch_cell_prep(d, 0, MODE_STEP, h->st);
+    launch_neighbor_build(d, 0, h->st);
     // endpoint energies now; the interior is evaluated by the next cfneb_step / cfneb_get_forces, or on demand by
-    // cfneb_get_path / cfneb_get_status (interior_stale)
-    launch_cell_prep(d, kEndpointsOnly, MODE_STEP, h->st);
-    launch_neighbor_build(d, kEndpointsOnly, h->st);
+    // cfneb_get_path (interior_stale)
     launch_force(d, kEndpointsOnly, h->st);
     launch_finalize(d, kEndpointsOnly, h->st);
     h->interior_stale = true;

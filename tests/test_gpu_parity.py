@@ -717,3 +717,30 @@ def test_fs_potential_with_general_density_exponent(beta, rho_r0):
     assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
     assert gpu.get_status().error == 0
     gpu.close()
+
+
+def test_two_path_replacements_in_a_row_keep_the_lists_valid():
+    """Two cfneb_set_path calls with no iteration between them, each inside the skin of the previous path but together
+    outside the skin of the coordinates the lists were built at: the staleness bound must see the sum."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import splitmix64_normals
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(2, 5)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    kick = splitmix64_normals(91, pos[1:-1].size).reshape(pos[1:-1].shape)
+    kick /= np.max(np.linalg.norm(kick, axis=2))             # largest atomic displacement = 1
+    r0 = gpu.get_status().rebuilds
+    p1 = pos.copy()
+    p1[1:-1] += 0.10 * kick                                  # 2 x 0.10 < skin 0.3: no rebuild
+    gpu.set_path(p1, cells)
+    assert gpu.get_status().rebuilds == r0
+    p2 = p1.copy()
+    p2[1:-1] += 0.10 * kick                                  # again inside the skin of p1, but 2 x 0.20 > 0.3 from the build
+    gpu.set_path(p2, cells)
+    F, V, fneb, E = gpu.get_forces()
+    assert gpu.get_status().rebuilds >= r0 + 3
+    orc = oc.CFNEB(p2, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors)
+    orc.band.forces()
+    assert rel(E, orc.band.E) < TOL_FORCE and rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    gpu.close()
