@@ -11,13 +11,15 @@ paper's Ti3O5 / graphite NEP workloads (up to 1e5
 atoms x 100 images, periodic solids, variable cell), which need trained weights
 and structures that are not available.
 """
-from .lattices import fcc_supercell, bcc_supercell, bain_final_cell
+from .lattices import fcc_supercell, bcc_supercell, bain_final_cell, diamond_supercell
 from .noise import splitmix64_normals
 from .configs import (
     CONFIGS,
     WorkloadSpec,
     lj_params,
     fs_params,
+    sw_params,
+    diamond_strain_band,
     vacancy_endpoints_unrelaxed,
     bain_endpoints,
     linear_path,
@@ -30,6 +32,9 @@ __all__ = [
     "fcc_supercell",
     "bcc_supercell",
     "bain_final_cell",
+    "diamond_supercell",
+    "sw_params",
+    "diamond_strain_band",
     "splitmix64_normals",
     "CONFIGS",
     "WorkloadSpec",

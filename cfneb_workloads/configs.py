@@ -11,11 +11,12 @@ from dataclasses import dataclass, field
 
 import numpy as np
 
-from .lattices import fcc_supercell, bcc_supercell, bain_final_cell
+from .lattices import fcc_supercell, bcc_supercell, bain_final_cell, diamond_supercell
 from .noise import splitmix64_normals
 
 POT_LJ_SF = 0
 POT_FS_MORSE = 1
+POT_SW = 2
 
 
 def lj_params(eps=1.0, sigma=1.0, rc=2.5):
@@ -23,6 +24,34 @@ def lj_params(eps=1.0, sigma=1.0, rc=2.5):
     p = np.zeros(12)
     p[0], p[1], p[2] = eps, sigma, rc
     return p
+
+
+def sw_params(eps=2.1683, sigma=2.0951, a=1.80, lam=21.0, gamma=1.20, A=7.049556277, B=0.6022245584, p=4.0, q=0.0):
+    """Stillinger-Weber parameters (the published silicon set: eV, Angstrom), padded to 12 doubles.
+
+    Layout: eps, sigma, a (cut-off r_c = a sigma), lambda, gamma, A, B, p, q.  The functional form lives in the
+    oracle and in the CUDA path separately; this is data only.
+    """
+    out = np.zeros(12)
+    out[:9] = [eps, sigma, a, lam, gamma, A, B, p, q]
+    return out
+
+
+def diamond_strain_band(dims, a, n_images, seed, sigma_noise, strain):
+    """A band of a diamond-cubic supercell between the cubic cell and the cell deformed by (I + strain), linear in the
+    cell, fractional coordinates fixed, Gaussian noise on every image (endpoints included) so that no atom sits on a
+    symmetric site.  Returns pos[P,N,3], cells[P,3,3]."""
+    frac, cell0 = diamond_supercell(dims[0], dims[1], dims[2], a)
+    cell1 = cell0 @ (np.eye(3) + np.asarray(strain, dtype=np.float64))
+    P, N = int(n_images), frac.shape[0]
+    noise = splitmix64_normals(seed, P * N * 3).reshape(P, N, 3) * sigma_noise
+    pos = np.empty((P, N, 3))
+    cells = np.empty((P, 3, 3))
+    for p in range(P):
+        t = p / (P - 1)
+        cells[p] = cell0 + t * (cell1 - cell0)
+        pos[p] = frac @ cells[p] + noise[p]
+    return pos, cells
 
 
 def fs_params(D=0.3, alpha=1.5, r0=2.5, beta=3.0, rho_r0=2.5, A=0.8, r_on=4.5, r_cut=5.0):

@@ -7,6 +7,7 @@ import numpy as np
 
 FCC_BASIS = np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.0], [0.5, 0.0, 0.5], [0.0, 0.5, 0.5]])
 BCC_BASIS = np.array([[0.0, 0.0, 0.0], [0.5, 0.5, 0.5]])
+DIAMOND_BASIS = np.concatenate([FCC_BASIS, FCC_BASIS + 0.25])
 
 
 def _supercell(basis, nx, ny, nz, a):
@@ -26,6 +27,11 @@ def fcc_supercell(nx, ny, nz, a):
 def bcc_supercell(nx, ny, nz, a):
     """Fractional coordinates (n,3) and cell (3,3) of an nx x ny x nz conventional bcc supercell."""
     return _supercell(BCC_BASIS, nx, ny, nz, a)
+
+
+def diamond_supercell(nx, ny, nz, a):
+    """Fractional coordinates (n,3) and cell (3,3) of an nx x ny x nz conventional diamond-cubic supercell (8 atoms each)."""
+    return _supercell(DIAMOND_BASIS, nx, ny, nz, a)
 
 
 def bain_final_cell(cell_bcc, volume_ratio=1.0):

@@ -282,6 +282,110 @@ static double pair_vector(const double *s, const double *h, int i, int j, const 
 }
 
 /*
+ * Stillinger-Weber potential (kind 2), a three-body potential: the paper's force formalism (Eq. 4-8)
+ * is written for exactly this class, U_i a function of ALL vectors r^ij of atom i's environment (the paper's own
+ * potential, NEP, is of this kind; its trained weights are not available).
+ *   pot = {eps, sigma, a, lambda, gamma, A, B, p, q};  r_c = a sigma
+ *   U_i = 1/2 sum_j phi2(r_ij) + sum_{j<k} h(r_ij, r_ik, cos theta_jik)
+ *   phi2(r) = A eps [B (sigma/r)^p - (sigma/r)^q] exp(sigma / (r - r_c))                       (r < r_c, else 0)
+ *   h = lambda eps (cos theta + 1/3)^2 exp(gamma sigma/(r_ij - r_c)) exp(gamma sigma/(r_ik - r_c))
+ * Partial forces p^ij = dU_i/dr^ij (a vector per list entry), then Eq. 5:  f^ij = p^ij - p^ji (force on i due
+ * to j), F_i = sum_j f^ij, and Eq. 8:  V = -1/2 sum_i sum_j r^ij (x) f^ij.
+ */
+static double sw_phi2(const double *p, double r, double *dphi) {
+    double eps = p[0], sig = p[1], rc = p[2] * p[1], A = p[5], B = p[6], pp = p[7], qq = p[8];
+    double sr = sig / r, e = exp(sig / (r - rc));
+    double tp = B * pow(sr, pp), tq = pow(sr, qq);
+    double br = tp - tq;
+    double dbr = (-pp * tp + qq * tq) / r;
+    *dphi = A * eps * (dbr * e + br * e * (-sig / ((r - rc) * (r - rc))));
+    return A * eps * br * e;
+}
+
+static int sw_partial_forces(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
+                             const int *list, const int *shift, double *Ui, double *part /* [N*cap*3] */) {
+    double eps = pot[0], sig = pot[1], rc = pot[2] * pot[1], lam = pot[3], gam = pot[4];
+    double rc2 = rc * rc;
+    for (int i = 0; i < N; ++i) {
+        int c = count[i] < cap ? count[i] : cap;
+        double ui = 0.0;
+        for (int k = 0; k < c; ++k) part[((size_t)i * cap + k) * 3] = part[((size_t)i * cap + k) * 3 + 1] = part[((size_t)i * cap + k) * 3 + 2] = 0.0;
+        for (int k = 0; k < c; ++k) {
+            double rj[3];
+            size_t ej = (size_t)i * cap + k;
+            double r2j = pair_vector(s, h, i, list[ej], shift + 3 * ej, rj);
+            if (!(r2j < rc2)) continue;
+            double dj = sqrt(r2j), dphi;
+            ui += 0.5 * sw_phi2(pot, dj, &dphi);
+            for (int m = 0; m < 3; ++m) part[ej * 3 + m] += 0.5 * dphi * rj[m] / dj;
+            double gj = exp(gam * sig / (dj - rc)), dgj = gj * (-gam * sig / ((dj - rc) * (dj - rc)));
+            for (int l = k + 1; l < c; ++l) { /* triplets (j, k') centred on i, each once */
+                double rk[3];
+                size_t ek = (size_t)i * cap + l;
+                double r2k = pair_vector(s, h, i, list[ek], shift + 3 * ek, rk);
+                if (!(r2k < rc2)) continue;
+                double dk = sqrt(r2k);
+                double gk = exp(gam * sig / (dk - rc)), dgk = gk * (-gam * sig / ((dk - rc) * (dk - rc)));
+                double cs = (rj[0] * rk[0] + rj[1] * rk[1] + rj[2] * rk[2]) / (dj * dk);
+                double w = cs + 1.0 / 3.0;
+                ui += lam * eps * w * w * gj * gk;
+                for (int m = 0; m < 3; ++m) {
+                    double dcos_j = (rk[m] / dk - cs * rj[m] / dj) / dj; /* d cos / d r^ij */
+                    double dcos_k = (rj[m] / dj - cs * rk[m] / dk) / dk; /* d cos / d r^ik */
+                    part[ej * 3 + m] += lam * eps * (2.0 * w * gj * gk * dcos_j + w * w * dgj * gk * rj[m] / dj);
+                    part[ek * 3 + m] += lam * eps * (2.0 * w * gj * gk * dcos_k + w * w * gj * dgk * rk[m] / dk);
+                }
+            }
+        }
+        Ui[i] = ui;
+    }
+    return ORACLE_OK;
+}
+
+static int sw_energy_force_virial(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
+                                  const int *list, const int *shift, double *E, double *F, double *V, double *Ui_out) {
+    double rc = pot[2] * pot[1], rc2 = rc * rc;
+    double *part = (double *)malloc(sizeof(double) * (size_t)N * cap * 3);
+    double *Ui = (double *)malloc(sizeof(double) * (size_t)N);
+    sw_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
+    long double Etot = 0.0L, Vacc[9];
+    for (int k = 0; k < 9; ++k) Vacc[k] = 0.0L;
+    for (int i = 0; i < 3 * N; ++i) F[i] = 0.0;
+    int status = ORACLE_OK;
+    for (int i = 0; i < N; ++i) {
+        int c = count[i] < cap ? count[i] : cap;
+        for (int k = 0; k < c; ++k) {
+            double r[3];
+            size_t e = (size_t)i * cap + k;
+            int j = list[e];
+            double r2 = pair_vector(s, h, i, j, shift + 3 * e, r);
+            if (!(r2 < rc2)) continue;
+            /* the mirror entry (j; i, -n) holds p^ji */
+            int cj = count[j] < cap ? count[j] : cap, found = -1;
+            for (int l = 0; l < cj; ++l) {
+                size_t e2 = (size_t)j * cap + l;
+                if (list[e2] == i && shift[3 * e2] == -shift[3 * e] && shift[3 * e2 + 1] == -shift[3 * e + 1] &&
+                    shift[3 * e2 + 2] == -shift[3 * e + 2]) { found = l; break; }
+            }
+            if (found < 0) { status = ORACLE_EINVAL; continue; }
+            size_t e2 = (size_t)j * cap + found;
+            double f[3];
+            for (int m = 0; m < 3; ++m) f[m] = part[e * 3 + m] - part[e2 * 3 + m]; /* Eq. 5 */
+            for (int m = 0; m < 3; ++m) {
+                F[3 * i + m] += f[m];
+                for (int n = 0; n < 3; ++n) Vacc[3 * m + n] += (long double)(-0.5 * r[m] * f[n]); /* Eq. 8 */
+            }
+        }
+        if (Ui_out) Ui_out[i] = Ui[i];
+        Etot += Ui[i];
+    }
+    *E = (double)Etot;
+    for (int k = 0; k < 9; ++k) V[k] = (double)Vacc[k];
+    free(part); free(Ui);
+    return status;
+}
+
+/*
  * Energy, forces, virial of one image from its neighbour list (Eq. 4, 5, 8).
  * Outputs: *E total energy; F[N*3] Cartesian forces; V[9] virial, V_mn = -1/2 sum r_m f_n;
  * Ui[N] per-atom energies (may be NULL); rho_out[N] FS densities (may be NULL).
@@ -289,10 +393,15 @@ static double pair_vector(const double *s, const double *h, int i, int j, const 
 int oracle_energy_force_virial(int N, const double *Rt, const double *h0, const double *h, int kind,
                                const double *pot, int cap, const int *count, const int *list, const int *shift,
                                double *E, double *F, double *V, double *Ui, double *rho_out) {
-    if (kind != 0 && kind != 1) return ORACLE_EINVAL;
+    if (kind != 0 && kind != 1 && kind != 2) return ORACLE_EINVAL;
     double *s = (double *)malloc(sizeof(double) * 3 * (size_t)N);
     int rc = fractional(N, Rt, h0, s);
     if (rc) { free(s); return rc; }
+    if (kind == 2) {
+        rc = sw_energy_force_virial(N, s, h, pot, cap, count, list, shift, E, F, V, Ui);
+        free(s);
+        return rc;
+    }
     double rcut = (kind == 0) ? pot[2] : pot[7];
     double rc2 = rcut * rcut;
     double *dF = NULL;

@@ -9,10 +9,10 @@ import itertools
 import numpy as np
 import pytest
 
-from cfneb_workloads import bcc_supercell, fcc_supercell, fs_params, lj_params
+from cfneb_workloads import bcc_supercell, diamond_supercell, fcc_supercell, fs_params, lj_params, sw_params
 from oracle import forcefield as ff
 
-LJ, FS = 0, 1
+LJ, FS, SW = 0, 1, 2
 
 
 def energy(R, h, kind, pot, rc, cap=400, brute=True):
@@ -113,6 +113,39 @@ def test_fs_bcc_shell_sum():
         assert np.allclose(V, V[0, 0] * np.eye(3), atol=1e-9)  # cubic symmetry: isotropic virial
 
 
+def test_stillinger_weber_textbook_points():
+    """The published silicon parametrisation has its two defining properties built in: the perfect diamond crystal at
+    a = 5.431 A has cohesive energy -2 eps = -4.3366 eV per atom (four bonds per atom at the pair minimum of depth
+    eps, every bond angle tetrahedral: cos theta = -1/3, so the three-body term vanishes), and that lattice is
+    stress free.  A trimer with a non-tetrahedral angle isolates the three-body term."""
+    pot = sw_params()
+    eps, sig, rc = pot[0], pot[1], pot[2] * pot[1]
+    frac, cell = diamond_supercell(2, 2, 2, 5.431)
+    nb = ff.neighbors(frac @ cell, cell, cell, rc + 0.3, 64)
+    E, F, V, Ui, _ = ff.energy_force_virial(frac @ cell, cell, cell, SW, pot, nb, per_atom=True)
+    assert np.all(nb[0] == 16)                                   # 4 first + 12 second neighbours inside r_c + 0.3
+    assert abs(E / len(frac) + 2.0 * eps) < 2e-4 * eps           # -2 eps to the precision of the published constants
+    assert np.allclose(Ui, Ui[0], atol=1e-12) and np.abs(F).max() < 1e-11
+    assert np.abs(V).max() < 2e-3 * len(frac) * eps              # stress free at the published lattice constant
+    # pair term alone: dimer at the bond length d = a sqrt(3)/4 has energy -eps (value and minimum)
+    d = 5.431 * np.sqrt(3.0) / 4.0
+    e = lambda r: dimer(r, SW, pot, rc)[0]
+    assert abs(e(d) + eps) < 1e-4 * eps
+    assert e(d - 0.01) > e(d) < e(d + 0.01)
+    assert e(rc - 1e-9) == pytest.approx(0.0, abs=1e-12) and e(rc + 0.1) == 0.0
+    # trimer: centre at the origin, two neighbours at distance d under angle theta: E = 2 phi2(d) + lam eps (cos + 1/3)^2 g(d)^2
+    for theta in (np.pi / 2, 2.0, np.arccos(-1.0 / 3.0)):
+        h = np.eye(3) * 40.0
+        R = np.array([[20.0, 20.0, 20.0], [20.0 + d, 20.0, 20.0], [20.0 + d * np.cos(theta), 20.0 + d * np.sin(theta), 20.0]])
+        E3 = energy(R, h, SW, pot, rc)[0]
+        d12 = np.linalg.norm(R[1] - R[2])
+        pair = 2.0 * e(d) + (e(d12) if d12 < rc else 0.0)
+        g = np.exp(pot[4] * sig / (d - rc))
+        # the end atoms see only one neighbour inside r_c unless d12 < r_c (then their own triplets count as well)
+        if d12 >= rc:
+            assert abs(E3 - pair - pot[3] * eps * (np.cos(theta) + 1.0 / 3.0) ** 2 * g * g) < 1e-12
+
+
 # ---------- finite differences: Eq. 5 (forces) and Eq. 3 (virial = -dU/d eps under h' = h(I+eps)) ----------
 
 def perturbed(kind, rng):
@@ -122,15 +155,22 @@ def perturbed(kind, rng):
         pot, rc = lj_params(), 2.5
         cell = cell @ (np.eye(3) + 0.03 * rng.standard_normal((3, 3)))
         R = frac @ cell + 0.05 * rng.standard_normal(frac.shape)
-    else:
+    elif kind == FS:
         frac, cell = bcc_supercell(2, 2, 3, 2.6)
         pot, rc = fs_params(), 5.0
         cell = cell @ (np.eye(3) + 0.03 * rng.standard_normal((3, 3)))
         R = frac @ cell + 0.08 * rng.standard_normal(frac.shape)
+    else:  # Stillinger-Weber, compressed diamond so that some second neighbours are inside the cut-off too
+        frac, cell = diamond_supercell(2, 2, 2, 5.2)
+        frac = frac[1:]  # vacancy
+        pot = sw_params()
+        rc = pot[2] * pot[1]
+        cell = cell @ (np.eye(3) + 0.03 * rng.standard_normal((3, 3)))
+        R = frac @ cell + 0.15 * rng.standard_normal(frac.shape)
     return R, cell, pot, rc
 
 
-@pytest.mark.parametrize("kind", [LJ, FS])
+@pytest.mark.parametrize("kind", [LJ, FS, SW])
 def test_forces_match_finite_differences(kind):
     rng = np.random.default_rng(11 + kind)
     R, h, pot, rc = perturbed(kind, rng)
@@ -145,7 +185,7 @@ def test_forces_match_finite_differences(kind):
     assert np.abs(F.sum(axis=0)).max() < 1e-11 * len(R)  # sum F = 0 (f^ij = -f^ji)
 
 
-@pytest.mark.parametrize("kind", [LJ, FS])
+@pytest.mark.parametrize("kind", [LJ, FS, SW])
 def test_virial_matches_strain_derivative(kind):
     rng = np.random.default_rng(5 + kind)
     R, h, pot, rc = perturbed(kind, rng)
@@ -185,7 +225,7 @@ def test_virial_sign_and_trace_zero_at_energy_minimum():
 
 # ---------- invariances ----------
 
-@pytest.mark.parametrize("kind", [LJ, FS])
+@pytest.mark.parametrize("kind", [LJ, FS, SW])
 def test_rigid_rotation_and_translation_invariance(kind):
     rng = np.random.default_rng(3 + kind)
     R, h, pot, rc = perturbed(kind, rng)
