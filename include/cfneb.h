@@ -57,7 +57,7 @@ enum {
     CFNEB_ERANGE = -7           /* bad image index, endpoint / climbing-image delete, more than max_images */
 };
 
-enum { CFNEB_POT_LJ_SF = 0, CFNEB_POT_FS_MORSE = 1 };
+enum { CFNEB_POT_LJ_SF = 0, CFNEB_POT_FS_MORSE = 1, CFNEB_POT_SW = 2 };
 enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default) */, CFNEB_CELL_D = 2 /* Eq. 14 */ };
 
 /*
@@ -66,6 +66,11 @@ enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default)
  *   potential = CFNEB_POT_FS_MORSE: pot = {D, alpha, r0, beta, rho_r0, A, r_on, r_cut}:
  *       v(r) = D[e^{-2 alpha (r-r0)} - 2 e^{-alpha (r-r0)}] t(r), rho_i = sum_j e^{-beta (r - rho_r0)} t(r),
  *       U_i = 1/2 sum_j v + F(rho_i), F = -A sqrt(rho), t = cosine taper from r_on to r_cut (O3, A21).
+ *   potential = CFNEB_POT_SW (Stillinger-Weber, three-body): pot = {eps, sigma, a, lambda, gamma, A, B, p, q}, r_c = a sigma:
+ *       U_i = 1/2 sum_j A eps [B (sigma/r)^p - (sigma/r)^q] e^{sigma/(r - r_c)}
+ *             + sum_{j<k} lambda eps (cos theta_jik + 1/3)^2 e^{gamma sigma/(r_ij - r_c)} e^{gamma sigma/(r_ik - r_c)},
+ *       evaluated through the partial forces p^ij = dU_i/dr^ij of Eq. 5 (f^ij = p^ij - p^ji) and Eq. 8; at most 32
+ *       neighbours inside r_c per atom (CFNEB_ENEIGH_OVERFLOW otherwise).
  *   k_spring: uniform spring constant of Eq. 1 (A14).  climb: 1 = climbing image (ref [12]).
  *   cell_factor: lam of A13; 0 = auto (Omega0^(1/3) N^(1/6)); 1 = the paper's equations literally.
  *   fire_*: FIRE constants of O7 (one state for the whole band).

@@ -55,11 +55,11 @@ struct Carver {
 
 bool valid_params(int32_t n_atoms, const cfneb_params *prm) {
     if (!prm || n_atoms < 1 || n_atoms >= kMaxAtoms) return false;
-    if (prm->potential != CFNEB_POT_LJ_SF && prm->potential != CFNEB_POT_FS_MORSE) return false;
+    if (prm->potential != CFNEB_POT_LJ_SF && prm->potential != CFNEB_POT_FS_MORSE && prm->potential != CFNEB_POT_SW) return false;
     if (prm->cell_mode < CFNEB_CELL_FIXED || prm->cell_mode > CFNEB_CELL_D) return false;
     if (prm->max_images < 3 || prm->max_neighbors < 1 || prm->max_neighbors > 4096) return false;
     if (!(prm->skin >= 0.0) || !(prm->cell_factor >= 0.0) || !isfinite(prm->pressure)) return false;
-    const double rc = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
+    const double rc = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->potential == CFNEB_POT_SW ? prm->pot[2] * prm->pot[1] : prm->pot[7];
     if (!(rc > 0.0)) return false;
     if (prm->potential == CFNEB_POT_FS_MORSE && !(prm->pot[7] > prm->pot[6])) return false;
     if (!(prm->fire_dt0 > 0.0) || !(prm->fire_dtmax > 0.0) || !(prm->fire_maxstep > 0.0)) return false;
@@ -111,6 +111,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
     d.nbr_tmp = c.take<uint32_t>(S * (size_t)d.cap * Npad);
     d.nbr_bkt = c.take<unsigned char>(S * (size_t)d.cap * Npad);
+    d.part = prm->potential == CFNEB_POT_SW ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
     d.bin_members = c.take<int>(S * Npad);
@@ -370,7 +371,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     d.finc = prm->fire_finc; d.fdec = prm->fire_fdec; d.astart = prm->fire_astart; d.fa = prm->fire_fa;
     d.skin = prm->skin;
     d.pressure = prm->pressure;
-    d.r_cut = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->pot[7];
+    d.r_cut = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->potential == CFNEB_POT_SW ? prm->pot[2] * prm->pot[1] : prm->pot[7];
     d.r_list = d.r_cut + d.skin;
     prepare_potential(d);
     if (set_reference_frame(h, cell_init, cell_final) != CFNEB_OK) { cfneb_destroy(h); return CFNEB_EINVAL; }

@@ -377,7 +377,9 @@ __global__ void __launch_bounds__(kThreadsAtom, 5) force_kernel(Dev d, int p_lo)
 void prepare_potential(Dev &d) {
     for (double &x : d.potc) x = 0.0;
     d.potc[kPotcRc2] = d.r_cut * d.r_cut;
-    if (d.potential == CFNEB_POT_FS_MORSE) {
+    if (d.potential == CFNEB_POT_SW) {
+        for (int k = 0; k < 9; ++k) d.potc[k] = d.pot[k];  // eps, sigma, a, lambda, gamma, A, B, p, q
+    } else if (d.potential == CFNEB_POT_FS_MORSE) {
         FSc c;
         c.Dm = d.pot[0]; c.a = d.pot[1]; c.r0 = d.pot[2]; c.beta = d.pot[3]; c.rr0 = d.pot[4]; c.A = d.pot[5];
         c.r_on = d.pot[6]; c.inv_w = 1.0 / (d.pot[7] - d.pot[6]); c.pi_w = 3.14159265358979323846 * c.inv_w;
@@ -399,7 +401,9 @@ void launch_force(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
-    if (d.potential == CFNEB_POT_LJ_SF) {
+    if (d.potential == CFNEB_POT_SW) {
+        launch_force_sw(d, p_lo, st);
+    } else if (d.potential == CFNEB_POT_LJ_SF) {
         force_kernel<CFNEB_POT_LJ_SF, false><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
     } else {
         density_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);

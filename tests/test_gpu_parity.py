@@ -744,3 +744,42 @@ def test_two_path_replacements_in_a_row_keep_the_lists_valid():
     orc.band.forces()
     assert rel(E, orc.band.E) < TOL_FORCE and rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
     gpu.close()
+
+
+def _sw_band(dims, n_images, a=5.35, strain=((0.0, 0.03, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.04))):
+    from cfneb_workloads import diamond_strain_band, sw_params
+    pot = sw_params()
+    pos, cells = diamond_strain_band(dims, a, n_images, 17, 0.08, strain)
+    return pot, pos, cells
+
+
+@pytest.mark.parametrize("dims,n_images", [((2, 2, 2), 5), ((3, 3, 4), 4)])
+def test_stillinger_weber_many_body_forces_and_steps(dims, n_images):
+    """The three-body potential through the paper's partial-force formalism (Eq. 5, 8) on the device against the
+    oracle: a disordered diamond band under strain; the 64-atom cell is narrower than 3 r_list (explicit periodic
+    shifts, mirror entries across the boundary), the 288-atom one uses the binned search."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    pot, pos, cells = _sw_band(dims, n_images)
+    rc = pot[2] * pot[1]
+    fire = dict(dt0=0.05, dtmax=0.5, maxstep=0.1, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+    orc = oc.CFNEB(pos, cells, 2, pot, rc, k_spring=1.0, climb=True, cell_factor=0.0, fire=fire, skin=0.3, max_neighbors=64)
+    prm = cf.default_params(potential=cf.POT_SW, pot=list(pot), k_spring=1.0, climb=1, cell_factor=0.0, skin=0.3,
+                            max_neighbors=64, max_images=n_images, fire=fire)
+    gpu = cf.CFNEB(pos, cells, prm)
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert np.max(np.abs(orc.evaluator.last["F"])) > 0.5          # real forces, three-body terms far from zero
+    assert rel(E, orc.band.E) < TOL_FORCE
+    assert rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
+    assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    X0, _ = orc.get_state()
+    orc.step(6)
+    gpu.step(6)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
+    st = gpu.get_status()
+    assert st.error == 0 and abs(st.barrier - orc.band.barrier) < 1e-9 * max(1.0, abs(orc.band.E[0]))
+    gpu.close()
