@@ -167,17 +167,18 @@ def oracle_sample_plan(k, total_steps, budget_s):
     cores = host_cores()
     movable = spec.n_images - 2
     threads = max(1, min(cores, movable, 16))
-    if spec.lattice != "bcc_bain":
+    if spec.lattice == "fcc_vacancy":
         return spec.n_images, None, threads, "full config (%d atoms x %d images)" % (spec.n_atoms, spec.n_images)
     m = threads  # one image per thread: the only parallelism the oracle has is over images
     per_step = budget_s / max(total_steps + 2.0, 1.0)  # + 2: the two endpoint evaluations at construction
     atoms = int(min(spec.n_atoms, max(432, per_step * ORACLE_RATE)))
     if atoms >= 0.5 * spec.n_atoms:
         return m + 2, None, threads, "%d consecutive movable images (mid-path) of the %d, all %d atoms" % (m, movable, spec.n_atoms)
-    n = max(6, int(round((atoms / 2.0) ** (1.0 / 3.0))))
+    per_cell = spec.n_atoms / float(np.prod(spec.dims))  # atoms per conventional cell (2 bcc, 8 diamond)
+    n = max(4, int(round((atoms / per_cell) ** (1.0 / 3.0))))
     return (m + 2, (n, n, n), threads,
-            "%d movable images of a %dx%dx%d bcc cell (%d atoms) built by the same recipe as the %d-atom config"
-            % (m, n, n, n, 2 * n ** 3, spec.n_atoms))
+            "%d movable images of a %dx%dx%d conventional-cell supercell (%d atoms) built by the same recipe as the %d-atom config"
+            % (m, n, n, n, int(round(per_cell * n ** 3)), spec.n_atoms))
 
 
 def run_oracle(k, steps, warmup, budget_s):
@@ -225,7 +226,7 @@ def main_reference(args):
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(args.config), "potential": "finnis_sinclair_morse" if spec.potential else "lj_shifted_force",
+        "config": {"workload": workload_name(args.config), "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber")[int(spec.potential)],
                    "sample": r["sample"], "runs_on": "host CPU (oracle/, plain fp64 C + numpy)"},
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
         "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -326,7 +327,7 @@ def main_ours(args):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": workload_name(k), "n_atoms": N, "n_images": P, "movable_images": P - 2,
-                   "potential": "finnis_sinclair_morse" if spec.potential else "lj_shifted_force",
+                   "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber")[int(spec.potential)],
                    "cell_filter": "rotation-free B = D D^T (Eq. 17), cell_factor auto", "climb": bool(spec.climb),
                    "value_counts": "N x (P-2) per step", "value_counting_all_images": value * P / (P - 2),
                    "parallelism": "replicas only (x%d)" % world if world > 1 else "single GPU",

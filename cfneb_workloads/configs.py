@@ -37,10 +37,10 @@ def sw_params(eps=2.1683, sigma=2.0951, a=1.80, lam=21.0, gamma=1.20, A=7.049556
     return out
 
 
-def diamond_strain_band(dims, a, n_images, seed, sigma_noise, strain):
+def diamond_strain_band(dims, a, n_images, seed, sigma_noise, strain, noise_endpoints=True):
     """A band of a diamond-cubic supercell between the cubic cell and the cell deformed by (I + strain), linear in the
-    cell, fractional coordinates fixed, Gaussian noise on every image (endpoints included) so that no atom sits on a
-    symmetric site.  Returns pos[P,N,3], cells[P,3,3]."""
+    cell, fractional coordinates fixed, Gaussian noise on every image (on the endpoints too unless noise_endpoints is
+    false) so that no atom sits on a symmetric site.  Returns pos[P,N,3], cells[P,3,3]."""
     frac, cell0 = diamond_supercell(dims[0], dims[1], dims[2], a)
     cell1 = cell0 @ (np.eye(3) + np.asarray(strain, dtype=np.float64))
     P, N = int(n_images), frac.shape[0]
@@ -50,7 +50,7 @@ def diamond_strain_band(dims, a, n_images, seed, sigma_noise, strain):
     for p in range(P):
         t = p / (P - 1)
         cells[p] = cell0 + t * (cell1 - cell0)
-        pos[p] = frac @ cells[p] + noise[p]
+        pos[p] = frac @ cells[p] + (noise[p] if (noise_endpoints or 0 < p < P - 1) else 0.0)
     return pos, cells
 
 
@@ -70,7 +70,7 @@ class WorkloadSpec:
     name: str
     potential: int
     pot: np.ndarray
-    lattice: str  # "fcc_vacancy" | "bcc_bain"
+    lattice: str  # "fcc_vacancy" | "bcc_bain" | "diamond_strain"
     dims: tuple
     n_atoms: int
     n_images: int
@@ -87,11 +87,15 @@ class WorkloadSpec:
 
     @property
     def r_cut(self):
+        if self.potential == POT_SW:
+            return float(self.pot[2] * self.pot[1])
         return float(self.pot[2] if self.potential == POT_LJ_SF else self.pot[7])
 
 
 _FIRE_LJ = dict(dt0=0.01, dtmax=0.05, maxstep=0.1, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
 _FIRE_EV = dict(dt0=0.1, dtmax=1.0, maxstep=0.2, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+_FIRE_SW = dict(dt0=0.02, dtmax=0.15, maxstep=0.05, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+_SW_STRAIN = ((0.0, 0.03, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.04))
 
 CONFIGS = [
     WorkloadSpec("c0_lj_vacancy_2x2x2", POT_LJ_SF, lj_params(), "fcc_vacancy", (2, 2, 2), 31, 7, 0,
@@ -104,6 +108,10 @@ CONFIGS = [
                  fire=_FIRE_EV, n_steps=200, max_images=32, skin=0.3, max_neighbors=192),
     WorkloadSpec("c4_fs_bain_101306", POT_FS_MORSE, fs_params(), "bcc_bain", (37, 37, 37), 101306, 100, 4,
                  fire=_FIRE_EV, n_steps=500, max_images=100, skin=0.5, max_neighbors=224),
+    # not a BASELINE.json config: the many-body (three-body) workload of SURVEY.md section 8(f) item 4, standing in for
+    # the paper's NEP potential -- Stillinger-Weber diamond, 16^3 conventional cells x 32 images under a general strain
+    WorkloadSpec("c5_sw_diamond_32768", POT_SW, sw_params(), "diamond_strain", (16, 16, 16), 32768, 32, 5,
+                 noise_sigma=0.02, climb=False, fire=_FIRE_SW, n_steps=200, max_images=32, skin=0.3, max_neighbors=64),
 ]
 
 
@@ -181,6 +189,9 @@ def build_workload(k, n_images=None, dims=None):
     if spec.lattice == "fcc_vacancy":
         R0, h0, R1, h1 = load_vacancy_endpoints(k)
         pos, cells = linear_path(R0 @ np.linalg.inv(h0), h0, R1 @ np.linalg.inv(h1), h1, P, spec.seed, spec.noise_sigma)
+    elif spec.lattice == "diamond_strain":
+        pos, cells = diamond_strain_band(tuple(dims) if dims else spec.dims, 5.431, P, spec.seed, spec.noise_sigma, _SW_STRAIN,
+                                         noise_endpoints=False)
     else:
         lc = load_lattice_constants()
         f0, c0, f1, c1 = bain_endpoints(tuple(dims) if dims else spec.dims, lc["fs_bcc_a"], lc["fs_fcc_volume_ratio"])

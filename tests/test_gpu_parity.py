@@ -783,3 +783,26 @@ def test_stillinger_weber_many_body_forces_and_steps(dims, n_images):
     st = gpu.get_status()
     assert st.error == 0 and abs(st.barrier - orc.band.barrier) < 1e-9 * max(1.0, abs(orc.band.E[0]))
     gpu.close()
+
+
+def test_stillinger_weber_band_converges_with_the_oracle():
+    """The many-body workload (cfneb_workloads config 5 at 216 atoms x 6 images: relaxed diamond to a generally strained
+    cell, no climbing image) run to convergence on the device and by the oracle: same energies along the band,
+    equally spaced images, endpoint at the -2 eps per atom of the published parametrisation."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(5, 6, dims=(3, 3, 3))
+    N = pos.shape[1]
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, max_images=6))
+    orc.step(260)
+    gpu.step(260)
+    st = gpu.get_status()
+    assert st.error == 0 and st.fmax < 1e-6 and orc.band.fmax < 1e-6 and st.climb_index == -1
+    Eg = gpu.get_path(positions=False)[2]
+    assert np.max(np.abs(Eg - orc.band.E)) < 1e-8
+    assert abs(Eg[0] / N + 2.0 * spec.pot[0]) < 2e-4 * spec.pot[0]
+    seg = gpu.get_segment_lengths()
+    assert np.max(seg) - np.min(seg) < 1e-4 * np.mean(seg)
+    gpu.close()
