@@ -806,3 +806,36 @@ def test_stillinger_weber_band_converges_with_the_oracle():
     seg = gpu.get_segment_lengths()
     assert np.max(seg) - np.min(seg) < 1e-4 * np.mean(seg)
     gpu.close()
+
+
+def test_relax_endpoints_stillinger_weber_finds_the_published_diamond():
+    """Endpoint relaxation on the device with the many-body potential: diamond compressed to a = 5.30 A (and a noisy,
+    stretched copy as the other endpoint) relaxes, cell and atoms together, to the crystal the published constants were
+    built for -- -2 eps per atom, a = 5.431 A -- and to the oracle's relaxed energy."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import diamond_supercell, splitmix64_normals, sw_params
+    from oracle import cfneb as oc
+    pot = sw_params()
+    rc = pot[2] * pot[1]
+    fire = dict(dt0=0.02, dtmax=0.15, maxstep=0.05, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+    frac, c0 = diamond_supercell(2, 2, 2, 5.30)
+    _, c1 = diamond_supercell(2, 2, 2, 5.52)
+    N = len(frac)
+    R0 = frac @ c0
+    R1 = frac @ c1 + 0.03 * splitmix64_normals(3, frac.size).reshape(frac.shape)
+    prm = cf.default_params(potential=cf.POT_SW, pot=list(pot), k_spring=1.0, climb=0, cell_factor=0.0, skin=0.3,
+                            max_neighbors=64, max_images=4, fire=fire)
+    gpu = cf.CFNEB(np.stack([R0, R1]), np.stack([c0, c1]), prm, n_images=4)
+    steps, fmax, en = gpu.relax_endpoints(1e-7, 6000, rebuild_band=True)
+    assert max(fmax) < 1e-7
+    Ra, ha, Ea, fa, ita = oc.relax_endpoint(R0, c0, 2, pot, rc, fmax_tol=1e-7, max_steps=6000, cell_factor=0.0, fire=fire,
+                                            skin=0.3, max_neighbors=64)
+    assert abs(en[0] - Ea) < 1e-9 * abs(Ea) and abs(steps[0] - ita) <= 1
+    pos, cells, E = gpu.get_path()
+    for e, h in ((en[0], cells[0]), (en[1], cells[-1])):
+        assert abs(e / N + 2.0 * pot[0]) < 2e-4 * pot[0]
+        a_eff = abs(np.linalg.det(h)) ** (1.0 / 3.0) / 2.0
+        assert abs(a_eff - 5.431) < 2e-3
+    assert abs(E[0] - E[-1]) < 1e-6                      # both endpoints are the same crystal: a flat band
+    assert gpu.get_status().error == 0
+    gpu.close()
