@@ -112,6 +112,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.nbr_tmp = c.take<uint32_t>(S * (size_t)d.cap * Npad);
     d.nbr_bkt = c.take<unsigned char>(S * (size_t)d.cap * Npad);
     d.part = prm->potential == CFNEB_POT_SW ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
+    d.nbr_mirror = prm->potential == CFNEB_POT_SW ? c.take<unsigned short>(S * (size_t)d.cap * Npad) : nullptr;
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
     d.bin_members = c.take<int>(S * Npad);

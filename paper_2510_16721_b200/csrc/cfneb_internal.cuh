@@ -119,6 +119,7 @@ struct Dev {
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
     unsigned short *nbr_tail; // [S][kTailBuckets][Npad] number of entries below tail bucket t (list sorted by bucket)
     uint32_t *nbr_tmp;        // [S][cap][Npad]  unsorted list of a rebuild (scratch of K1)
+    unsigned short *nbr_mirror; // [S][cap][Npad] row of the mirror entry (j; i, -n) of each entry (many-body potentials only)
     double *part;             // [S][cap][3][Npad] partial forces p^ij = dU_i/dr^ij per list entry (many-body potentials only)
     unsigned char *nbr_bkt;   // [S][cap][Npad]  r^2 bucket of each unsorted entry (scratch of K1)
     int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
@@ -173,6 +174,7 @@ void launch_cell_prep(const Dev &d, int p_lo, int mode, cudaStream_t st);       
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st);                      // K1
 void prepare_potential(Dev &d);  // fills Dev::potc from pot / r_cut (host)
 void launch_force(const Dev &d, int p_lo, cudaStream_t st);
+void launch_mirror_sw(const Dev &d, int p_lo, cudaStream_t st);                          // mirror rows after a list build
 void launch_force_sw(const Dev &d, int p_lo, cudaStream_t st);                            // K2, Stillinger-Weber (kernels_sw.cu)                               // K2
 void launch_reduce(const Dev &d, cudaStream_t st);                                        // K4 (atom rows)
 void plan_stream_grids(Dev &d);  // nblk_red / nblk_upd from the SM count and the kernels' occupancy

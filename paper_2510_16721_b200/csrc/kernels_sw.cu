@@ -3,7 +3,8 @@
 // (Eq. 4-8; the paper's own potential, NEP, is of this class -- its trained weights are not available,
 // SURVEY.md section 8(f) item 4):
 //   pass 1 (sw_partial_kernel)  U_i and the partial forces p^ij = dU_i/dr^ij, one vector per list entry, stored
-//   pass 2 (sw_force_kernel)    f^ij = p^ij - p^ji (Eq. 5; p^ji sits at the mirror entry (j; i, -n) of j's list),
+//   pass 2 (sw_force_kernel)    f^ij = p^ij - p^ji (Eq. 5; p^ji sits at the mirror entry (j; i, -n) of j's list,
+//                               whose row is tabulated once per list build by sw_mirror_kernel),
 //                               F_i = sum_j f^ij,  V = -1/2 sum_i sum_j r^ij (x) f^ij  (Eq. 8)
 //   U_i = 1/2 sum_j phi2(r_ij) + sum_{j<k} h(r_ij, r_ik, cos theta_jik),  r_c = a sigma,
 //   phi2(r) = A eps [B (sigma/r)^p - (sigma/r)^q] exp(sigma/(r - r_c)),
@@ -59,9 +60,6 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_partial_kernel(Dev d, int p_l
             double dx, dy, dz;
             shifted_vec(ri, Rc[e & kIdxMask], e >> kShiftBits, sh, dx, dy, dz);
             const double r2 = dx * dx + dy * dy + dz * dz;
-            part[(size_t)(k * 3 + 0) * d.Npad] = 0.0;
-            part[(size_t)(k * 3 + 1) * d.Npad] = 0.0;
-            part[(size_t)(k * 3 + 2) * d.Npad] = 0.0;
             if (r2 < rc2) {
                 if (n < kMaxEnv) {
                     ex[n] = dx; ey[n] = dy; ez[n] = dz; er[n] = sqrt(r2); ek[n] = k;
@@ -97,10 +95,13 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_partial_kernel(Dev d, int p_l
                 pz[b] += le * (c2 * (ez[a] * inv - cs * ez[b] * invk) * invk + rb * ez[b] * invk);
             }
         }
-        for (int a = 0; a < n; ++a) {
-            part[(size_t)(ek[a] * 3 + 0) * d.Npad] = px[a];
-            part[(size_t)(ek[a] * 3 + 1) * d.Npad] = py[a];
-            part[(size_t)(ek[a] * 3 + 2) * d.Npad] = pz[a];
+        // one write per list entry: the partial force of the in-range ones (ek ascending), zero for the others
+        for (int k = 0, a = 0; k < cnt; ++k) {
+            const bool hit = a < n && ek[a] == k;
+            part[(size_t)(k * 3 + 0) * d.Npad] = hit ? px[a] : 0.0;
+            part[(size_t)(k * 3 + 1) * d.Npad] = hit ? py[a] : 0.0;
+            part[(size_t)(k * 3 + 2) * d.Npad] = hit ? pz[a] : 0.0;
+            if (hit) ++a;
         }
     }
     block_sum<1>(ui, red);
@@ -124,9 +125,8 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
         const double4 *Rc = d.Rc + (size_t)slot * d.Npad;
         const uint32_t *lists = d.nbr_list + (size_t)slot * d.cap * d.Npad;
         const double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad;
-        const int *counts = d.nbr_count + (size_t)slot * d.Npad;
         const double4 ri = Rc[i];
-        const int cnt = counts[i];
+        const int cnt = d.nbr_count[(size_t)slot * d.Npad + i];
         for (int k = 0; k < cnt; ++k) {
             const uint32_t e = lists[(size_t)k * d.Npad + i];
             const uint32_t j = e & kIdxMask, code = e >> kShiftBits;
@@ -136,10 +136,8 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
             // mirror entry (j; i, -n): each 3-bit field n + 4 becomes 8 - (n + 4)
             const uint32_t rev = (uint32_t)i | ((((8u - (code & 7u)) & 7u) | (((8u - ((code >> 3) & 7u)) & 7u) << 3) |
                                                 (((8u - ((code >> 6) & 7u)) & 7u) << 6)) << kShiftBits);
-            const int cj = counts[j];
-            int l = 0;
-            while (l < cj && lists[(size_t)l * d.Npad + j] != rev) ++l;
-            if (l == cj) { set_error(d.ctl, CFNEB_EINVAL); continue; }
+            const int l = d.nbr_mirror[((size_t)slot * d.cap + k) * d.Npad + i];  // row of (j; i, -n), found at the list build
+            if (l >= d.cap || lists[(size_t)l * d.Npad + j] != rev) { set_error(d.ctl, CFNEB_EINVAL); continue; }
             const double gx = part[(size_t)(k * 3 + 0) * d.Npad + i] - part[(size_t)(l * 3 + 0) * d.Npad + j];  // Eq. 5
             const double gy = part[(size_t)(k * 3 + 1) * d.Npad + i] - part[(size_t)(l * 3 + 1) * d.Npad + j];
             const double gz = part[(size_t)(k * 3 + 2) * d.Npad + i] - part[(size_t)(l * 3 + 2) * d.Npad + j];
@@ -157,6 +155,36 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
 #pragma unroll
         for (int n = 0; n < 7; ++n) out[n] = out7[n];
     }
+}
+
+// After a list build: for every entry (i; j, n) the row of its mirror (j; i, -n) in j's list (cap if absent).
+__global__ void __launch_bounds__(kThreadsAtom) sw_mirror_kernel(Dev d, int p_lo) {
+    int p;
+    if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
+    const int slot = d.order[p];
+    if (!d.geom[slot].rebuild) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.N) return;
+    const uint32_t *lists = d.nbr_list + (size_t)slot * d.cap * d.Npad;
+    const int *counts = d.nbr_count + (size_t)slot * d.Npad;
+    const int cnt = counts[i];
+    for (int k = 0; k < cnt; ++k) {
+        const uint32_t e = lists[(size_t)k * d.Npad + i];
+        const uint32_t j = e & kIdxMask, code = e >> kShiftBits;
+        const uint32_t rev = (uint32_t)i | ((((8u - (code & 7u)) & 7u) | (((8u - ((code >> 3) & 7u)) & 7u) << 3) |
+                                            (((8u - ((code >> 6) & 7u)) & 7u) << 6)) << kShiftBits);
+        const int cj = counts[j];
+        int l = 0;
+        while (l < cj && lists[(size_t)l * d.Npad + j] != rev) ++l;
+        d.nbr_mirror[((size_t)slot * d.cap + k) * d.Npad + i] = (unsigned short)(l < cj ? l : d.cap);
+    }
+}
+
+void launch_mirror_sw(const Dev &d, int p_lo, cudaStream_t st) {
+    const int nimg = images_in_grid(d.S, p_lo);
+    if (nimg <= 0) return;
+    dim3 grid(d.nblk_atom, nimg);
+    sw_mirror_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
 }
 
 void launch_force_sw(const Dev &d, int p_lo, cudaStream_t st) {
