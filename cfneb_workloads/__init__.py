@@ -19,6 +19,7 @@ from .configs import (
     lj_params,
     fs_params,
     sw_params,
+    dn_params,
     diamond_strain_band,
     vacancy_endpoints_unrelaxed,
     bain_endpoints,
@@ -34,6 +35,7 @@ __all__ = [
     "bain_final_cell",
     "diamond_supercell",
     "sw_params",
+    "dn_params",
     "diamond_strain_band",
     "splitmix64_normals",
     "CONFIGS",

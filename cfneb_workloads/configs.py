@@ -17,6 +17,7 @@ from .noise import splitmix64_normals
 POT_LJ_SF = 0
 POT_FS_MORSE = 1
 POT_SW = 2
+POT_DNN = 3
 
 
 def lj_params(eps=1.0, sigma=1.0, rc=2.5):
@@ -34,6 +35,14 @@ def sw_params(eps=2.1683, sigma=2.0951, a=1.80, lam=21.0, gamma=1.20, A=7.049556
     """
     out = np.zeros(12)
     out[:9] = [eps, sigma, a, lam, gamma, A, B, p, q]
+    return out
+
+
+def dn_params(rc=4.2, K=4, M=3, L=3, H=8, seed=20251016):
+    """Descriptor-network stand-in for the paper's NEP potential: cut-off, number of radial descriptors, angular
+    radial functions, angular orders, hidden neurons, weight seed (layout of include/cfneb.h).  Data only."""
+    out = np.zeros(12)
+    out[:6] = [rc, K, M, L, H, seed]
     return out
 
 
@@ -89,12 +98,15 @@ class WorkloadSpec:
     def r_cut(self):
         if self.potential == POT_SW:
             return float(self.pot[2] * self.pot[1])
+        if self.potential == POT_DNN:
+            return float(self.pot[0])
         return float(self.pot[2] if self.potential == POT_LJ_SF else self.pot[7])
 
 
 _FIRE_LJ = dict(dt0=0.01, dtmax=0.05, maxstep=0.1, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
 _FIRE_EV = dict(dt0=0.1, dtmax=1.0, maxstep=0.2, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
 _FIRE_SW = dict(dt0=0.02, dtmax=0.15, maxstep=0.05, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+_FIRE_DNN = dict(dt0=0.005, dtmax=0.02, maxstep=0.002, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
 _SW_STRAIN = ((0.0, 0.03, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.04))
 
 CONFIGS = [
@@ -112,6 +124,10 @@ CONFIGS = [
     # the paper's NEP potential -- Stillinger-Weber diamond, 16^3 conventional cells x 32 images under a general strain
     WorkloadSpec("c5_sw_diamond_32768", POT_SW, sw_params(), "diamond_strain", (16, 16, 16), 32768, 32, 5,
                  noise_sigma=0.02, climb=False, fire=_FIRE_SW, n_steps=200, max_images=32, skin=0.3, max_neighbors=64),
+    # the same band with the descriptor-network potential (the shape of NEP, seeded weights): 16 neighbours inside the
+    # cut-off, 13 descriptors, 8 neurons.  The energy surface is arbitrary, so FIRE takes tiny steps: a cost workload
+    WorkloadSpec("c6_dnn_diamond_32768", POT_DNN, dn_params(), "diamond_strain", (16, 16, 16), 32768, 32, 6,
+                 noise_sigma=0.02, climb=False, fire=_FIRE_DNN, n_steps=100, max_images=32, skin=0.3, max_neighbors=64),
 ]
 
 

@@ -342,12 +342,19 @@ static int sw_partial_forces(int N, const double *s, const double *h, const doub
     return ORACLE_OK;
 }
 
-static int sw_energy_force_virial(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
+static int dn_partial_forces(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
+                             const int *list, const int *shift, double *Ui, double *part);
+
+/* Eq. 5 and Eq. 8 from stored partial forces; kind 2 = Stillinger-Weber, kind 3 = descriptor network */
+static int manybody_energy_force_virial(int kind, int N, const double *s, const double *h, const double *pot, int cap, const int *count,
                                   const int *list, const int *shift, double *E, double *F, double *V, double *Ui_out) {
-    double rc = pot[2] * pot[1], rc2 = rc * rc;
+    double rc = kind == 2 ? pot[2] * pot[1] : pot[0], rc2 = rc * rc;
     double *part = (double *)malloc(sizeof(double) * (size_t)N * cap * 3);
     double *Ui = (double *)malloc(sizeof(double) * (size_t)N);
-    sw_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
+    int prc = ORACLE_OK;
+    if (kind == 2) sw_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
+    else prc = dn_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
+    if (prc != ORACLE_OK) { free(part); free(Ui); return prc; }
     long double Etot = 0.0L, Vacc[9];
     for (int k = 0; k < 9; ++k) Vacc[k] = 0.0L;
     for (int i = 0; i < 3 * N; ++i) F[i] = 0.0;
@@ -386,6 +393,119 @@ static int sw_energy_force_virial(int N, const double *s, const double *h, const
 }
 
 /*
+ * Descriptor-network potential (kind 3): the SHAPE of the paper's NEP potential (radial and angular
+ * descriptors of the environment fed to a small neural network) with seeded weights -- the trained weights are not
+ * available, so this is a cost and data-flow stand-in, not a physical model.
+ *   pot = {r_c, K, M, L, H, seed}:  K radial, M x L angular descriptors (D = K + M L <= 16), H <= 8 hidden neurons
+ *   f_k(r) = 1/2 [T_k(x) + 1] fc(r),  x = 2 (r/r_c - 1)^2 - 1,  fc = 1/2 [1 + cos(pi r / r_c)]   (Chebyshev T_k)
+ *   q_k = sum_j f_k(r_ij)                                           k < K
+ *   q_{K + n L + l - 1} = sum_j sum_k f_n(r_ij) f_n(r_ik) P_l(cos theta_jik)     n < M, l = 1..L (all ordered pairs)
+ *   U_i = sum_mu W1_mu tanh(sum_d W0_{mu d} q_d - b0_mu)
+ * Weights: SplitMix64(seed) -> u in [0,1) -> w = 2u - 1, drawn in the order W0[mu][d] (times 0.3/8 for radial, 0.3/40
+ * for angular d), b0[mu] (times 0.5), W1[mu].  Partial forces p^ij = sum_d dU_i/dq_d dq_d/dr^ij; Eq. 5 and 8 as for SW.
+ */
+#define DN_MAXD 16
+#define DN_MAXH 8
+#define DN_MAXENV 64
+static void dn_weights(const double *pot, double *W0, double *b0, double *W1) {
+    int K = (int)pot[1], D = K + (int)pot[2] * (int)pot[3], H = (int)pot[4];
+    unsigned long long st = (unsigned long long)pot[5];
+    int total = H * D + 2 * H;
+    for (int t = 0; t < total; ++t) {
+        st += 0x9E3779B97F4A7C15ULL;
+        unsigned long long z = st;
+        z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+        z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+        z ^= z >> 31;
+        double w = 2.0 * ((double)(z >> 11) * (1.0 / 9007199254740992.0)) - 1.0;
+        if (t < H * D) W0[t] = w * ((t % D) < K ? 0.3 / 8.0 : 0.3 / 40.0);
+        else if (t < H * D + H) b0[t - H * D] = 0.5 * w;
+        else W1[t - H * D - H] = w;
+    }
+}
+
+static void dn_basis(double r, double rc, int nk, double *f, double *df) {
+    double fc = 0.5 * (1.0 + cos(PI * r / rc)), dfc = -0.5 * sin(PI * r / rc) * PI / rc;
+    double x = 2.0 * (r / rc - 1.0) * (r / rc - 1.0) - 1.0, dx = 4.0 * (r / rc - 1.0) / rc;
+    double Tm = 1.0, T = x, dTm = 0.0, dT = 1.0;
+    for (int k = 0; k < nk; ++k) {
+        double Tk = k == 0 ? 1.0 : T, dTk = k == 0 ? 0.0 : dT;
+        f[k] = 0.5 * (Tk + 1.0) * fc;
+        df[k] = 0.5 * dTk * dx * fc + 0.5 * (Tk + 1.0) * dfc;
+        if (k >= 1) {
+            double Tn = 2.0 * x * T - Tm, dTn = 2.0 * T + 2.0 * x * dT - dTm;
+            Tm = T; T = Tn; dTm = dT; dT = dTn;
+        }
+    }
+}
+
+static int dn_partial_forces(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
+                             const int *list, const int *shift, double *Ui, double *part) {
+    double rc = pot[0], rc2 = rc * rc;
+    int K = (int)pot[1], M = (int)pot[2], L = (int)pot[3], H = (int)pot[4], D = K + M * L;
+    int nk = K > M ? K : M;
+    if (D > DN_MAXD || H > DN_MAXH || L > 3 || nk > 8) return ORACLE_EINVAL;
+    double W0[DN_MAXH * DN_MAXD], b0[DN_MAXH], W1[DN_MAXH];
+    dn_weights(pot, W0, b0, W1);
+    for (int i = 0; i < N; ++i) {
+        int c = count[i] < cap ? count[i] : cap, n = 0;
+        double ex[DN_MAXENV][3], er[DN_MAXENV], f[DN_MAXENV][8], df[DN_MAXENV][8];
+        int ek[DN_MAXENV];
+        for (int k = 0; k < c; ++k) {
+            size_t e = (size_t)i * cap + k;
+            for (int m = 0; m < 3; ++m) part[e * 3 + m] = 0.0;
+            double r[3], r2 = pair_vector(s, h, i, list[e], shift + 3 * e, r);
+            if (!(r2 < rc2)) continue;
+            if (n >= DN_MAXENV) return ORACLE_ENEIGH_OVERFLOW;
+            ex[n][0] = r[0]; ex[n][1] = r[1]; ex[n][2] = r[2]; er[n] = sqrt(r2); ek[n] = k;
+            dn_basis(er[n], rc, nk, f[n], df[n]);
+            ++n;
+        }
+        double q[DN_MAXD];
+        for (int d = 0; d < D; ++d) q[d] = 0.0;
+        for (int a = 0; a < n; ++a)
+            for (int k = 0; k < K; ++k) q[k] += f[a][k];
+        for (int a = 0; a < n; ++a)
+            for (int b = 0; b < n; ++b) {
+                double cs = (ex[a][0] * ex[b][0] + ex[a][1] * ex[b][1] + ex[a][2] * ex[b][2]) / (er[a] * er[b]);
+                double P[3] = {cs, 0.5 * (3.0 * cs * cs - 1.0), 0.5 * (5.0 * cs * cs * cs - 3.0 * cs)};
+                for (int m = 0; m < M; ++m)
+                    for (int l = 0; l < L; ++l) q[K + m * L + l] += f[a][m] * f[b][m] * P[l];
+            }
+        double Fd[DN_MAXD], ui = 0.0;
+        for (int d = 0; d < D; ++d) Fd[d] = 0.0;
+        for (int mu = 0; mu < H; ++mu) {
+            double z = -b0[mu];
+            for (int d = 0; d < D; ++d) z += W0[mu * D + d] * q[d];
+            double t = tanh(z);
+            ui += W1[mu] * t;
+            for (int d = 0; d < D; ++d) Fd[d] += W1[mu] * (1.0 - t * t) * W0[mu * D + d];
+        }
+        Ui[i] = ui;
+        for (int a = 0; a < n; ++a) {
+            double p[3] = {0.0, 0.0, 0.0};
+            for (int k = 0; k < K; ++k)
+                for (int m = 0; m < 3; ++m) p[m] += Fd[k] * df[a][k] * ex[a][m] / er[a];
+            for (int b = 0; b < n; ++b) {
+                double cs = (ex[a][0] * ex[b][0] + ex[a][1] * ex[b][1] + ex[a][2] * ex[b][2]) / (er[a] * er[b]);
+                double P[3] = {cs, 0.5 * (3.0 * cs * cs - 1.0), 0.5 * (5.0 * cs * cs * cs - 3.0 * cs)};
+                double dP[3] = {1.0, 3.0 * cs, 0.5 * (15.0 * cs * cs - 3.0)};
+                for (int mm = 0; mm < M; ++mm)
+                    for (int l = 0; l < L; ++l) {
+                        double g = 2.0 * Fd[K + mm * L + l];
+                        for (int m = 0; m < 3; ++m) {
+                            double dcos = (ex[b][m] / er[b] - cs * ex[a][m] / er[a]) / er[a];
+                            p[m] += g * (df[a][mm] * f[b][mm] * P[l] * ex[a][m] / er[a] + f[a][mm] * f[b][mm] * dP[l] * dcos);
+                        }
+                    }
+            }
+            for (int m = 0; m < 3; ++m) part[((size_t)i * cap + ek[a]) * 3 + m] = p[m];
+        }
+    }
+    return ORACLE_OK;
+}
+
+/*
  * Energy, forces, virial of one image from its neighbour list (Eq. 4, 5, 8).
  * Outputs: *E total energy; F[N*3] Cartesian forces; V[9] virial, V_mn = -1/2 sum r_m f_n;
  * Ui[N] per-atom energies (may be NULL); rho_out[N] FS densities (may be NULL).
@@ -393,12 +513,12 @@ static int sw_energy_force_virial(int N, const double *s, const double *h, const
 int oracle_energy_force_virial(int N, const double *Rt, const double *h0, const double *h, int kind,
                                const double *pot, int cap, const int *count, const int *list, const int *shift,
                                double *E, double *F, double *V, double *Ui, double *rho_out) {
-    if (kind != 0 && kind != 1 && kind != 2) return ORACLE_EINVAL;
+    if (kind < 0 || kind > 3) return ORACLE_EINVAL;
     double *s = (double *)malloc(sizeof(double) * 3 * (size_t)N);
     int rc = fractional(N, Rt, h0, s);
     if (rc) { free(s); return rc; }
-    if (kind == 2) {
-        rc = sw_energy_force_virial(N, s, h, pot, cap, count, list, shift, E, F, V, Ui);
+    if (kind >= 2) {
+        rc = manybody_energy_force_virial(kind, N, s, h, pot, cap, count, list, shift, E, F, V, Ui);
         free(s);
         return rc;
     }

@@ -9,10 +9,10 @@ import itertools
 import numpy as np
 import pytest
 
-from cfneb_workloads import bcc_supercell, diamond_supercell, fcc_supercell, fs_params, lj_params, sw_params
+from cfneb_workloads import bcc_supercell, diamond_supercell, dn_params, fcc_supercell, fs_params, lj_params, sw_params
 from oracle import forcefield as ff
 
-LJ, FS, SW = 0, 1, 2
+LJ, FS, SW, DNN = 0, 1, 2, 3
 
 
 def energy(R, h, kind, pot, rc, cap=400, brute=True):
@@ -146,6 +146,58 @@ def test_stillinger_weber_textbook_points():
             assert abs(E3 - pair - pot[3] * eps * (np.cos(theta) + 1.0 / 3.0) ** 2 * g * g) < 1e-12
 
 
+def splitmix64(seed, n):
+    out, state, mask = [], seed, (1 << 64) - 1
+    for _ in range(n):
+        state = (state + 0x9E3779B97F4A7C15) & mask
+        z = state
+        z = ((z ^ (z >> 30)) * 0xBF58476D1CE4E5B9) & mask
+        z = ((z ^ (z >> 27)) * 0x94D049BB133111EB) & mask
+        out.append(z ^ (z >> 31))
+    return out
+
+
+def test_descriptor_network_energy_against_library_polynomials():
+    """CFNEB_POT_DNN (include/cfneb.h; the shape of the paper's NEP).  The generator is pinned on the published
+    SplitMix64 test vector (seed 1234567); the site energies of a small irregular cluster are then rebuilt from
+    numpy's Chebyshev and Legendre routines, a dense matrix product and tanh -- none of the oracle's loops."""
+    assert splitmix64(1234567, 3) == [6457827717110365317, 3203168211198807973, 9817491932198370423]
+    from numpy.polynomial import chebyshev, legendre
+    pot = dn_params(rc=3.0, K=4, M=3, L=3, H=8, seed=99)
+    rc, K, M, L, H = pot[0], 4, 3, 3, 8
+    D = K + M * L
+    u = 2.0 * (np.array([z >> 11 for z in splitmix64(99, H * D + 2 * H)], dtype=np.float64) / 2.0 ** 53) - 1.0
+    W0 = u[:H * D].reshape(H, D) * np.where(np.arange(D) < K, 0.3 / 8.0, 0.3 / 40.0)
+    b0, W1 = 0.5 * u[H * D:H * D + H], u[H * D + H:]
+    rng = np.random.default_rng(4)
+    R = 20.0 + 1.6 * rng.standard_normal((7, 3))
+    h = np.eye(3) * 40.0
+    E, F, V, Ui, _ = ff.energy_force_virial(R, h, h, DNN, pot, ff.neighbors(R, h, h, rc, 16, brute=True), per_atom=True)
+    expect = np.zeros(len(R))
+    n_in = 0
+    for i in range(len(R)):
+        rv = np.array([R[j] - R[i] for j in range(len(R)) if j != i and np.linalg.norm(R[j] - R[i]) < rc])
+        q = np.zeros(D)
+        if len(rv):
+            r = np.linalg.norm(rv, axis=1)
+            n_in += len(r)
+            fc = 0.5 * (1.0 + np.cos(np.pi * r / rc))
+            x = 2.0 * (r / rc - 1.0) ** 2 - 1.0
+            fk = np.array([0.5 * (chebyshev.chebval(x, np.eye(4)[k]) + 1.0) * fc for k in range(4)])  # [k, j]
+            q[:K] = fk[:K].sum(axis=1)
+            cosm = (rv @ rv.T) / np.outer(r, r)
+            for n in range(M):
+                for l in range(1, L + 1):
+                    q[K + n * L + l - 1] = np.sum(np.outer(fk[n], fk[n]) * legendre.legval(cosm, np.eye(4)[l]))
+        expect[i] = W1 @ np.tanh(W0 @ q - b0)
+    assert n_in >= 10                                  # the cluster is not a set of isolated atoms
+    assert np.allclose(Ui, expect, rtol=0, atol=1e-13)
+    assert abs(E - expect.sum()) < 1e-12
+    # an isolated atom has q = 0: U = -sum W1 tanh(b0)
+    R1 = np.array([[5.0, 5.0, 5.0], [25.0, 25.0, 25.0]])
+    assert abs(energy(R1, h, DNN, pot, rc)[0] - 2.0 * (W1 @ np.tanh(-b0))) < 1e-14
+
+
 # ---------- finite differences: Eq. 5 (forces) and Eq. 3 (virial = -dU/d eps under h' = h(I+eps)) ----------
 
 def perturbed(kind, rng):
@@ -160,6 +212,13 @@ def perturbed(kind, rng):
         pot, rc = fs_params(), 5.0
         cell = cell @ (np.eye(3) + 0.03 * rng.standard_normal((3, 3)))
         R = frac @ cell + 0.08 * rng.standard_normal(frac.shape)
+    elif kind == DNN:  # descriptor network on a compressed diamond lattice: about 16-28 neighbours inside the cut-off
+        frac, cell = diamond_supercell(2, 2, 2, 5.2)
+        frac = frac[1:]
+        pot = dn_params()
+        rc = pot[0]
+        cell = cell @ (np.eye(3) + 0.03 * rng.standard_normal((3, 3)))
+        R = frac @ cell + 0.15 * rng.standard_normal(frac.shape)
     else:  # Stillinger-Weber, compressed diamond so that some second neighbours are inside the cut-off too
         frac, cell = diamond_supercell(2, 2, 2, 5.2)
         frac = frac[1:]  # vacancy
@@ -170,7 +229,7 @@ def perturbed(kind, rng):
     return R, cell, pot, rc
 
 
-@pytest.mark.parametrize("kind", [LJ, FS, SW])
+@pytest.mark.parametrize("kind", [LJ, FS, SW, DNN])
 def test_forces_match_finite_differences(kind):
     rng = np.random.default_rng(11 + kind)
     R, h, pot, rc = perturbed(kind, rng)
@@ -185,7 +244,7 @@ def test_forces_match_finite_differences(kind):
     assert np.abs(F.sum(axis=0)).max() < 1e-11 * len(R)  # sum F = 0 (f^ij = -f^ji)
 
 
-@pytest.mark.parametrize("kind", [LJ, FS, SW])
+@pytest.mark.parametrize("kind", [LJ, FS, SW, DNN])
 def test_virial_matches_strain_derivative(kind):
     rng = np.random.default_rng(5 + kind)
     R, h, pot, rc = perturbed(kind, rng)
@@ -225,7 +284,7 @@ def test_virial_sign_and_trace_zero_at_energy_minimum():
 
 # ---------- invariances ----------
 
-@pytest.mark.parametrize("kind", [LJ, FS, SW])
+@pytest.mark.parametrize("kind", [LJ, FS, SW, DNN])
 def test_rigid_rotation_and_translation_invariance(kind):
     rng = np.random.default_rng(3 + kind)
     R, h, pot, rc = perturbed(kind, rng)
