@@ -226,7 +226,7 @@ def main_reference(args):
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(args.config), "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber")[int(spec.potential)],
+        "config": {"workload": workload_name(args.config), "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber", "descriptor_network")[int(spec.potential)],
                    "sample": r["sample"], "runs_on": "host CPU (oracle/, plain fp64 C + numpy)"},
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
         "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -327,7 +327,7 @@ def main_ours(args):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": workload_name(k), "n_atoms": N, "n_images": P, "movable_images": P - 2,
-                   "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber")[int(spec.potential)],
+                   "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber", "descriptor_network")[int(spec.potential)],
                    "cell_filter": "rotation-free B = D D^T (Eq. 17), cell_factor auto", "climb": bool(spec.climb),
                    "value_counts": "N x (P-2) per step", "value_counting_all_images": value * P / (P - 2),
                    "parallelism": "replicas only (x%d)" % world if world > 1 else "single GPU",

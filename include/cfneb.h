@@ -57,7 +57,7 @@ enum {
     CFNEB_ERANGE = -7           /* bad image index, endpoint / climbing-image delete, more than max_images */
 };
 
-enum { CFNEB_POT_LJ_SF = 0, CFNEB_POT_FS_MORSE = 1, CFNEB_POT_SW = 2 };
+enum { CFNEB_POT_LJ_SF = 0, CFNEB_POT_FS_MORSE = 1, CFNEB_POT_SW = 2, CFNEB_POT_DNN = 3 };
 enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default) */, CFNEB_CELL_D = 2 /* Eq. 14 */ };
 
 /*
@@ -71,6 +71,15 @@ enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default)
  *             + sum_{j<k} lambda eps (cos theta_jik + 1/3)^2 e^{gamma sigma/(r_ij - r_c)} e^{gamma sigma/(r_ik - r_c)},
  *       evaluated through the partial forces p^ij = dU_i/dr^ij of Eq. 5 (f^ij = p^ij - p^ji) and Eq. 8; at most 32
  *       neighbours inside r_c per atom (CFNEB_ENEIGH_OVERFLOW otherwise).
+ *   potential = CFNEB_POT_DNN (descriptor network: the SHAPE of the paper's NEP potential, P:138 -- radial and
+ *       angular descriptors of the environment into a one-hidden-layer network -- with seeded weights, because the
+ *       trained ones are not available: a cost and data-flow stand-in, not a physical model):
+ *       pot = {r_c, K, M, L, H, seed}, K, M <= 4 radial functions, L <= 3, H <= 8 neurons, D = K + M L <= 16:
+ *       f_k(r) = 1/2 [T_k(x) + 1] fc(r), x = 2 (r/r_c - 1)^2 - 1, fc = 1/2 [1 + cos(pi r / r_c)] (T_k Chebyshev),
+ *       q_k = sum_j f_k(r_ij) (k < K),  q_{K + n L + l - 1} = sum_j sum_k f_n(r_ij) f_n(r_ik) P_l(cos theta_jik)
+ *       (n < M, l = 1..L, all ordered pairs j, k including j = k),  U_i = sum_mu W1_mu tanh(sum_d W0_{mu d} q_d - b0_mu).
+ *       Weights: SplitMix64 stream from `seed`, u = (z >> 11) 2^-53, w = 2u - 1, in the order W0[mu][d] (scaled by
+ *       0.3/8 for d < K, 0.3/40 otherwise), b0[mu] (scaled by 0.5), W1[mu].  Same two passes as CFNEB_POT_SW.
  *   k_spring: uniform spring constant of Eq. 1 (A14).  climb: 1 = climbing image (ref [12]).
  *   cell_factor: lam of A13; 0 = auto (Omega0^(1/3) N^(1/6)); 1 = the paper's equations literally.
  *   fire_*: FIRE constants of O7 (one state for the whole band).

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcfneb.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ENEIGH_OVERFLOW, ECELL, ENAN, ERANGE = 0, -1, -2, -3, -4, -5, -6, -7
-POT_LJ_SF, POT_FS_MORSE, POT_SW = 0, 1, 2
+POT_LJ_SF, POT_FS_MORSE, POT_SW, POT_DNN = 0, 1, 2, 3
 CELL_FIXED, CELL_B, CELL_D = 0, 1, 2
 K_CELLPREP, K_NEIGHBOR, K_FORCE, K_REDUCE, K_SCALAR, K_UPDATE, NKERNELS = 0, 1, 2, 3, 4, 5, 6
 KERNEL_CLASSES = ("cell_prep", "neighbor", "force", "reduce", "scalar", "update")

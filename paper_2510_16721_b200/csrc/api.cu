@@ -53,14 +53,31 @@ struct Carver {
     }
 };
 
+double cutoff_of(const cfneb_params *prm) {
+    switch (prm->potential) {
+        case CFNEB_POT_LJ_SF: return prm->pot[2];
+        case CFNEB_POT_SW: return prm->pot[2] * prm->pot[1];
+        case CFNEB_POT_DNN: return prm->pot[0];
+        default: return prm->pot[7];
+    }
+}
+
+bool many_body(const cfneb_params *prm) { return prm->potential == CFNEB_POT_SW || prm->potential == CFNEB_POT_DNN; }
+
 bool valid_params(int32_t n_atoms, const cfneb_params *prm) {
     if (!prm || n_atoms < 1 || n_atoms >= kMaxAtoms) return false;
-    if (prm->potential != CFNEB_POT_LJ_SF && prm->potential != CFNEB_POT_FS_MORSE && prm->potential != CFNEB_POT_SW) return false;
+    if (prm->potential < CFNEB_POT_LJ_SF || prm->potential > CFNEB_POT_DNN) return false;
     if (prm->cell_mode < CFNEB_CELL_FIXED || prm->cell_mode > CFNEB_CELL_D) return false;
     if (prm->max_images < 3 || prm->max_neighbors < 1 || prm->max_neighbors > 4096) return false;
     if (!(prm->skin >= 0.0) || !(prm->cell_factor >= 0.0) || !isfinite(prm->pressure)) return false;
-    const double rc = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->potential == CFNEB_POT_SW ? prm->pot[2] * prm->pot[1] : prm->pot[7];
+    const double rc = cutoff_of(prm);
     if (!(rc > 0.0)) return false;
+    if (prm->potential == CFNEB_POT_DNN) {
+        const double *q = prm->pot;
+        for (int k = 1; k <= 5; ++k)
+            if (!(q[k] >= 0.0) || q[k] != floor(q[k]) || q[k] > 9.0e15) return false;
+        if (q[1] < 1 || q[1] > 4 || q[2] < 1 || q[2] > 4 || q[3] < 1 || q[3] > 3 || q[4] < 1 || q[4] > 8) return false;
+    }
     if (prm->potential == CFNEB_POT_FS_MORSE && !(prm->pot[7] > prm->pot[6])) return false;
     if (!(prm->fire_dt0 > 0.0) || !(prm->fire_dtmax > 0.0) || !(prm->fire_maxstep > 0.0)) return false;
     return true;
@@ -111,8 +128,9 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
     d.nbr_tmp = c.take<uint32_t>(S * (size_t)d.cap * Npad);
     d.nbr_bkt = c.take<unsigned char>(S * (size_t)d.cap * Npad);
-    d.part = prm->potential == CFNEB_POT_SW ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
-    d.nbr_mirror = prm->potential == CFNEB_POT_SW ? c.take<unsigned short>(S * (size_t)d.cap * Npad) : nullptr;
+    d.part = many_body(prm) ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
+    d.nbr_mirror = many_body(prm) ? c.take<unsigned short>(S * (size_t)d.cap * Npad) : nullptr;
+    d.dn_w = prm->potential == CFNEB_POT_DNN ? c.take<double>(kDnWeights) : nullptr;
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
     d.bin_members = c.take<int>(S * Npad);
@@ -372,7 +390,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     d.finc = prm->fire_finc; d.fdec = prm->fire_fdec; d.astart = prm->fire_astart; d.fa = prm->fire_fa;
     d.skin = prm->skin;
     d.pressure = prm->pressure;
-    d.r_cut = prm->potential == CFNEB_POT_LJ_SF ? prm->pot[2] : prm->potential == CFNEB_POT_SW ? prm->pot[2] * prm->pot[1] : prm->pot[7];
+    d.r_cut = cutoff_of(prm);
     d.r_list = d.r_cut + d.skin;
     prepare_potential(d);
     if (set_reference_frame(h, cell_init, cell_final) != CFNEB_OK) { cfneb_destroy(h); return CFNEB_EINVAL; }
@@ -390,6 +408,21 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     c0.dt = d.dt0;
     c0.alpha = d.astart;
     CKC(cudaMemcpyAsync(d.ctl, &c0, sizeof c0, cudaMemcpyHostToDevice, h->st));
+    if (d.potential == CFNEB_POT_DNN) {  // network weights: the SplitMix64 stream of include/cfneb.h
+        const int K = (int)d.pot[1], D = K + (int)d.pot[2] * (int)d.pot[3], H = (int)d.pot[4];
+        double w[kDnWeights] = {0.0};
+        uint64_t state = (uint64_t)d.pot[5];
+        for (int t = 0; t < H * D + 2 * H; ++t) {
+            uint64_t z = (state += 0x9E3779B97F4A7C15ull);
+            z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+            z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+            z ^= z >> 31;
+            const double u = 2.0 * ldexp((double)(z >> 11), -53) - 1.0;
+            w[t] = t < H * D ? u * (t % D < K ? 0.3 / 8.0 : 0.3 / 40.0) : t < H * D + H ? 0.5 * u : u;
+        }
+        CKC(cudaMemcpyAsync(d.dn_w, w, sizeof w, cudaMemcpyHostToDevice, h->st));
+        CKC(cudaStreamSynchronize(h->st));  // `w` is a temporary
+    }
     CKH(upload_order(h));
     {
         std::vector<int> perm;

@@ -28,6 +28,7 @@ constexpr uint32_t kIdxMask = 0x7FFFFFu;
 constexpr int kShiftBits = 23;
 constexpr uint32_t kCodeCenter = 4u | (4u << 3) | (4u << 6);
 constexpr int kMaxAtoms = 1 << 23;
+constexpr int kDnWeights = 8 * 16 + 2 * 8;  // CFNEB_POT_DNN: H <= 8, D <= 16
 constexpr int kInnerBuckets = 56;      // radial buckets of the list sort: uniform in r^2 on [0, r_cut^2)
 constexpr int kTailBuckets = 8;        // ... and on [r_cut^2, r_list^2)
 
@@ -119,6 +120,7 @@ struct Dev {
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
     unsigned short *nbr_tail; // [S][kTailBuckets][Npad] number of entries below tail bucket t (list sorted by bucket)
     uint32_t *nbr_tmp;        // [S][cap][Npad]  unsorted list of a rebuild (scratch of K1)
+    double *dn_w;               // [kDnWeights] W0[H][D], b0[H], W1[H] of CFNEB_POT_DNN
     unsigned short *nbr_mirror; // [S][cap][Npad] row of the mirror entry (j; i, -n) of each entry (many-body potentials only)
     double *part;             // [S][cap][3][Npad] partial forces p^ij = dU_i/dr^ij per list entry (many-body potentials only)
     unsigned char *nbr_bkt;   // [S][cap][Npad]  r^2 bucket of each unsorted entry (scratch of K1)
@@ -175,6 +177,8 @@ void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st);            
 void prepare_potential(Dev &d);  // fills Dev::potc from pot / r_cut (host)
 void launch_force(const Dev &d, int p_lo, cudaStream_t st);
 void launch_mirror_sw(const Dev &d, int p_lo, cudaStream_t st);                          // mirror rows after a list build
+void launch_force_dn(const Dev &d, int p_lo, cudaStream_t st);                            // K2, descriptor network (kernels_dn.cu)
+void launch_pair_forces_manybody(const Dev &d, int p_lo, cudaStream_t st);                // pass 2 of both (kernels_sw.cu)
 void launch_force_sw(const Dev &d, int p_lo, cudaStream_t st);                            // K2, Stillinger-Weber (kernels_sw.cu)                               // K2
 void launch_reduce(const Dev &d, cudaStream_t st);                                        // K4 (atom rows)
 void plan_stream_grids(Dev &d);  // nblk_red / nblk_upd from the SM count and the kernels' occupancy

@@ -377,7 +377,9 @@ __global__ void __launch_bounds__(kThreadsAtom, 5) force_kernel(Dev d, int p_lo)
 void prepare_potential(Dev &d) {
     for (double &x : d.potc) x = 0.0;
     d.potc[kPotcRc2] = d.r_cut * d.r_cut;
-    if (d.potential == CFNEB_POT_SW) {
+    if (d.potential == CFNEB_POT_DNN) {
+        // constants are read from Dev::pot, weights from Dev::dn_w
+    } else if (d.potential == CFNEB_POT_SW) {
         for (int k = 0; k < 9; ++k) d.potc[k] = d.pot[k];  // eps, sigma, a, lambda, gamma, A, B, p, q
     } else if (d.potential == CFNEB_POT_FS_MORSE) {
         FSc c;
@@ -403,6 +405,8 @@ void launch_force(const Dev &d, int p_lo, cudaStream_t st) {
     dim3 grid(d.nblk_atom, nimg);
     if (d.potential == CFNEB_POT_SW) {
         launch_force_sw(d, p_lo, st);
+    } else if (d.potential == CFNEB_POT_DNN) {
+        launch_force_dn(d, p_lo, st);
     } else if (d.potential == CFNEB_POT_LJ_SF) {
         force_kernel<CFNEB_POT_LJ_SF, false><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
     } else {

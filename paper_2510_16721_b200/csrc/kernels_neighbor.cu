@@ -329,7 +329,7 @@ void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st) {
     dim3 gb((d.nbins_max + 127) / 128, nimg);
     bin_sort_kernel<<<gb, 128, 0, st>>>(d, p_lo);
     neighbor_search_kernel<<<ga, kThreadsAtom, 0, st>>>(d, p_lo);
-    if (d.potential == CFNEB_POT_SW) launch_mirror_sw(d, p_lo, st);
+    if (d.potential == CFNEB_POT_SW || d.potential == CFNEB_POT_DNN) launch_mirror_sw(d, p_lo, st);
 }
 
 void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_out, int *shift_out, cudaStream_t st) {

@@ -118,8 +118,7 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
-    const SWc &c = *reinterpret_cast<const SWc *>(d.potc);
-    const double rc = c.a * c.sig, rc2 = rc * rc;
+    const double rc2 = d.r_cut * d.r_cut;
     double fx = 0.0, fy = 0.0, fz = 0.0, vxx = 0.0, vyy = 0.0, vzz = 0.0, vxy = 0.0, vxz = 0.0, vyz = 0.0;
     if (valid) {
         const double4 *Rc = d.Rc + (size_t)slot * d.Npad;
@@ -187,12 +186,19 @@ void launch_mirror_sw(const Dev &d, int p_lo, cudaStream_t st) {
     sw_mirror_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
 }
 
+void launch_pair_forces_manybody(const Dev &d, int p_lo, cudaStream_t st) {
+    const int nimg = images_in_grid(d.S, p_lo);
+    if (nimg <= 0) return;
+    dim3 grid(d.nblk_atom, nimg);
+    sw_force_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+}
+
 void launch_force_sw(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
     sw_partial_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
-    sw_force_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+    launch_pair_forces_manybody(d, p_lo, st);
 }
 
 }  // namespace cfn
