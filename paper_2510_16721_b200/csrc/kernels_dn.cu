@@ -8,17 +8,47 @@
 //   q_{nl}  = sum_j sum_k f_n(r_ij) f_n(r_ik) P_l(cos theta_jik)                 n < M, l = 1..L
 //   U_i     = sum_mu W1_mu tanh(sum_d W0_{mu d} q_d - b0_mu)
 //   p^ij    = sum_d (dU_i/dq_d) dq_d/dr^ij
-// One thread per atom: gather the in-range environment (<= 32 neighbours), descriptors, network forward and its
-// gradient with respect to the descriptors, then one sweep over the pairs of the environment for the partial forces.
-// The pair sums run over j < k and are doubled (the summand is symmetric); the j = k terms (cos = 1, P_l = 1) are
-// added separately.  Weights sit in shared memory, the per-thread environment in local memory.
+// The double sum over the environment is never formed.  With u = r/|r| and the moments of the environment
+//   S^(l)_n = sum_j f_n(r_ij) u_ij^(x)l      (l = 0..3: 1 + 3 + 6 + 10 = 20 independent components per n)
+// the powers of cos theta_jik = u_ij . u_ik factorise, sum_jk f f cos^l = |S^(l)|^2 (Frobenius norm), so
+//   q_{n1} = |S1|^2,  q_{n2} = 3/2 |S2|^2 - 1/2 S0^2,  q_{n3} = 5/2 |S3|^2 - 3/2 |S1|^2,  q_k = S0_k
+// and both the descriptors and the partial forces are linear-time in the number of neighbours.  One thread per atom
+// walks its list twice: first the 80 moments (registers), then -- after the network and dU/dS^(l)_n, which overwrite
+// the moments in place -- one partial force per list entry from the polynomial phi_n(u) = sum_c (dU/dS_nc) u^c:
+//   p^ij = sum_n [ f_n'(r) phi_n(u) u + f_n(r)/r (I - u u^T) grad_u phi_n(u) ].
+// No per-thread environment array, hence no limit on the atoms inside the cut-off other than the list capacity.
 #include "cfneb_internal.cuh"
 
 namespace cfn {
 
-constexpr int kDnEnv = 32, kDnK = 4, kDnD = 16, kDnH = 8;
+constexpr int kDnK = 4, kDnL = 3, kDnC = 20;  // radial functions, angular orders, moment components per function
 
-__global__ void __launch_bounds__(kThreadsAtom) dn_partial_kernel(Dev d, int p_lo) {
+// multiplicity of each independent component in the Frobenius norm of the symmetric tensors
+// order: 1 | x y z | xx yy zz xy xz yz | xxx yyy zzz xxy xxz yyx yyz zzx zzy xyz
+__device__ __forceinline__ void dn_monomials(double x, double y, double z, double (&m)[kDnC]) {
+    m[0] = 1.0; m[1] = x; m[2] = y; m[3] = z;
+    m[4] = x * x; m[5] = y * y; m[6] = z * z; m[7] = x * y; m[8] = x * z; m[9] = y * z;
+    m[10] = m[4] * x; m[11] = m[5] * y; m[12] = m[6] * z; m[13] = m[4] * y; m[14] = m[4] * z;
+    m[15] = m[5] * x; m[16] = m[5] * z; m[17] = m[6] * x; m[18] = m[6] * y; m[19] = m[7] * z;
+}
+
+// radial basis and its derivative with respect to r; t = r / r_c
+__device__ __forceinline__ void dn_basis(double t, double irc, double (&f)[kDnK], double (&df)[kDnK]) {
+    double sn, cs;
+    sincospi(t, &sn, &cs);
+    const double fc = 0.5 + 0.5 * cs, dfc = -0.5 * sn * (3.14159265358979323846 * irc);
+    const double x = 2.0 * (t - 1.0) * (t - 1.0) - 1.0, dx_dr = 4.0 * (t - 1.0) * irc;
+    const double T[kDnK] = {1.0, x, 2.0 * x * x - 1.0, (4.0 * x * x - 3.0) * x};  // Chebyshev, closed forms
+    const double dT[kDnK] = {0.0, 1.0, 4.0 * x, 12.0 * x * x - 3.0};
+#pragma unroll
+    for (int k = 0; k < kDnK; ++k) {
+        const double g = 0.5 * (T[k] + 1.0);
+        f[k] = g * fc;
+        df[k] = 0.5 * dT[k] * dx_dr * fc + g * dfc;
+    }
+}
+
+__global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
@@ -26,7 +56,6 @@ __global__ void __launch_bounds__(kThreadsAtom) dn_partial_kernel(Dev d, int p_l
     __shared__ double red[32];
     __shared__ double sW[kDnWeights];
     const int K = (int)d.pot[1], M = (int)d.pot[2], L = (int)d.pot[3], H = (int)d.pot[4], D = K + M * L;
-    const int nk = K > M ? K : M;
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
     for (int t = threadIdx.x; t < H * D + 2 * H; t += blockDim.x) sW[t] = d.dn_w[t];
     __syncthreads();
@@ -41,17 +70,11 @@ __global__ void __launch_bounds__(kThreadsAtom) dn_partial_kernel(Dev d, int p_l
         double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + i;  // part[(k * 3 + m) * Npad]
         const double4 ri = Rc[i];
         const int cnt = d.nbr_count[(size_t)slot * d.Npad + i];
-        double ux[kDnEnv], uy[kDnEnv], uz[kDnEnv], ir[kDnEnv];          // unit vectors and 1/r
-        double f[kDnK][kDnEnv], df[kDnK][kDnEnv];
-        double px[kDnEnv], py[kDnEnv], pz[kDnEnv];
-        int ek[kDnEnv];
-        int n = 0;
-        bool overflow = false;
-        for (int k = 0; k < cnt; ++k) {
+        auto pair_vec = [&](int k, double &dx, double &dy, double &dz) {
             const uint32_t e = lp[(size_t)k * d.Npad];
             const uint32_t code = e >> kShiftBits;
             const double4 rj = Rc[e & kIdxMask];
-            double dx = rj.x - ri.x, dy = rj.y - ri.y, dz = rj.z - ri.z;
+            dx = rj.x - ri.x; dy = rj.y - ri.y; dz = rj.z - ri.z;
             if (code != kCodeCenter) {
                 const double n0 = (double)((int)(code & 7u) - 4), n1 = (double)((int)((code >> 3) & 7u) - 4),
                              n2 = (double)((int)((code >> 6) & 7u) - 4);
@@ -59,101 +82,118 @@ __global__ void __launch_bounds__(kThreadsAtom) dn_partial_kernel(Dev d, int p_l
                 dy += n0 * sh[1] + n1 * sh[4] + n2 * sh[7];
                 dz += n0 * sh[2] + n1 * sh[5] + n2 * sh[8];
             }
-            const double r2 = dx * dx + dy * dy + dz * dz;
+            return dx * dx + dy * dy + dz * dz;
+        };
+        // walk 1: moments S[n][c] = sum_j f_n(r_ij) u_ij^c
+        double S[kDnK][kDnC];
+#pragma unroll
+        for (int n = 0; n < kDnK; ++n)
+#pragma unroll
+            for (int c = 0; c < kDnC; ++c) S[n][c] = 0.0;
+        for (int k = 0; k < cnt; ++k) {
+            double dx, dy, dz;
+            const double r2 = pair_vec(k, dx, dy, dz);
             if (!(r2 < rc2)) continue;
-            if (n >= kDnEnv) { overflow = true; continue; }
-            const double r = sqrt(r2), inv = 1.0 / r, t = r * irc;
-            ux[n] = dx * inv; uy[n] = dy * inv; uz[n] = dz * inv; ir[n] = inv; ek[n] = k;
-            double sn, cs;
-            sincospi(t, &sn, &cs);
-            const double fc = 0.5 + 0.5 * cs, dfc = -0.5 * sn * (3.14159265358979323846 * irc);
-            const double x = 2.0 * (t - 1.0) * (t - 1.0) - 1.0, dx_dr = 4.0 * (t - 1.0) * irc;
-            // Chebyshev polynomials T_0..T_3 and their derivatives, closed forms
-            const double T[kDnK] = {1.0, x, 2.0 * x * x - 1.0, (4.0 * x * x - 3.0) * x};
-            const double dT[kDnK] = {0.0, 1.0, 4.0 * x, 12.0 * x * x - 3.0};
+            const double inv = rsqrt(r2), r = r2 * inv;
+            double f[kDnK], df[kDnK], m[kDnC];
+            dn_basis(r * irc, irc, f, df);
+            dn_monomials(dx * inv, dy * inv, dz * inv, m);
 #pragma unroll
-            for (int k2 = 0; k2 < kDnK; ++k2) {
-                const double g = 0.5 * (T[k2] + 1.0);
-                f[k2][n] = k2 < nk ? g * fc : 0.0;
-                df[k2][n] = k2 < nk ? 0.5 * dT[k2] * dx_dr * fc + g * dfc : 0.0;
-            }
-            ++n;
+            for (int n = 0; n < kDnK; ++n)
+#pragma unroll
+                for (int c = 0; c < kDnC; ++c) S[n][c] += f[n] * m[c];
         }
-        if (overflow) set_error(d.ctl, CFNEB_ENEIGH_OVERFLOW);
-
-        // descriptors
-        double q[kDnD];
+        // descriptors of the angular channels (dense [n][l]; the radial ones are S[k][0])
+        double qa[kDnK][kDnL];
 #pragma unroll
-        for (int t = 0; t < kDnD; ++t) q[t] = 0.0;
-        for (int a = 0; a < n; ++a) {
-            for (int k = 0; k < K; ++k) q[k] += f[k][a];
-            for (int m = 0; m < M; ++m) {
-                const double w = f[m][a] * f[m][a];
-                for (int l = 0; l < L; ++l) q[K + m * L + l] += w;  // j = k: P_l(1) = 1
-            }
-            for (int b = a + 1; b < n; ++b) {
-                const double c = ux[a] * ux[b] + uy[a] * uy[b] + uz[a] * uz[b];
-                const double P[3] = {c, 1.5 * c * c - 0.5, (2.5 * c * c - 1.5) * c};
-                for (int m = 0; m < M; ++m) {
-                    const double w = 2.0 * f[m][a] * f[m][b];
-                    for (int l = 0; l < L; ++l) q[K + m * L + l] += w * P[l];
-                }
-            }
+        for (int n = 0; n < kDnK; ++n) {
+            const double s1 = S[n][1] * S[n][1] + S[n][2] * S[n][2] + S[n][3] * S[n][3];
+            const double s2 = S[n][4] * S[n][4] + S[n][5] * S[n][5] + S[n][6] * S[n][6] +
+                              2.0 * (S[n][7] * S[n][7] + S[n][8] * S[n][8] + S[n][9] * S[n][9]);
+            const double s3 = S[n][10] * S[n][10] + S[n][11] * S[n][11] + S[n][12] * S[n][12] +
+                              3.0 * (S[n][13] * S[n][13] + S[n][14] * S[n][14] + S[n][15] * S[n][15] + S[n][16] * S[n][16] +
+                                     S[n][17] * S[n][17] + S[n][18] * S[n][18]) +
+                              6.0 * S[n][19] * S[n][19];
+            qa[n][0] = s1;
+            qa[n][1] = 1.5 * s2 - 0.5 * S[n][0] * S[n][0];
+            qa[n][2] = 2.5 * s3 - 1.5 * s1;
         }
-        // network forward and dU/dq
-        double Fd[kDnD];
+        // network forward, and its gradient with respect to the descriptors (Fr radial, Fa angular)
+        double Fr[kDnK] = {0.0, 0.0, 0.0, 0.0}, Fa[kDnK][kDnL];
 #pragma unroll
-        for (int t = 0; t < kDnD; ++t) Fd[t] = 0.0;
+        for (int n = 0; n < kDnK; ++n)
+#pragma unroll
+            for (int l = 0; l < kDnL; ++l) Fa[n][l] = 0.0;
         for (int mu = 0; mu < H; ++mu) {
+            const double *w = W0 + mu * D;
             double z = -b0[mu];
-            for (int t = 0; t < D; ++t) z += W0[mu * D + t] * q[t];
+#pragma unroll
+            for (int k = 0; k < kDnK; ++k)
+                if (k < K) z += w[k] * S[k][0];
+#pragma unroll
+            for (int n = 0; n < kDnK; ++n)
+#pragma unroll
+                for (int l = 0; l < kDnL; ++l)
+                    if (n < M && l < L) z += w[K + n * L + l] * qa[n][l];
             const double th = tanh(z), g = W1[mu] * (1.0 - th * th);
             ui[0] += W1[mu] * th;
-            for (int t = 0; t < D; ++t) Fd[t] += g * W0[mu * D + t];
+#pragma unroll
+            for (int k = 0; k < kDnK; ++k)
+                if (k < K) Fr[k] += g * w[k];
+#pragma unroll
+            for (int n = 0; n < kDnK; ++n)
+#pragma unroll
+                for (int l = 0; l < kDnL; ++l)
+                    if (n < M && l < L) Fa[n][l] += g * w[K + n * L + l];
         }
-        // partial forces
-        for (int a = 0; a < n; ++a) {
-            double g = 0.0;
-            for (int k = 0; k < K; ++k) g += Fd[k] * df[k][a];
-            for (int m = 0; m < M; ++m) {
-                double s = 0.0;
-                for (int l = 0; l < L; ++l) s += Fd[K + m * L + l];
-                g += 2.0 * df[m][a] * f[m][a] * s;
-            }
-            px[a] = g * ux[a]; py[a] = g * uy[a]; pz[a] = g * uz[a];
+        // dU/dS, in place: S[n][c] := G[n][c]
+#pragma unroll
+        for (int n = 0; n < kDnK; ++n) {
+            S[n][0] = Fr[n] - Fa[n][1] * S[n][0];
+            const double g1 = 2.0 * Fa[n][0] - 3.0 * Fa[n][2], g2 = 3.0 * Fa[n][1], g3 = 5.0 * Fa[n][2];
+#pragma unroll
+            for (int c = 1; c < 4; ++c) S[n][c] *= g1;
+#pragma unroll
+            for (int c = 4; c < 7; ++c) S[n][c] *= g2;
+#pragma unroll
+            for (int c = 7; c < 10; ++c) S[n][c] *= 2.0 * g2;
+#pragma unroll
+            for (int c = 10; c < 13; ++c) S[n][c] *= g3;
+#pragma unroll
+            for (int c = 13; c < 19; ++c) S[n][c] *= 3.0 * g3;
+            S[n][19] *= 6.0 * g3;
         }
-        for (int a = 0; a < n; ++a)
-            for (int b = a + 1; b < n; ++b) {
-                const double c = ux[a] * ux[b] + uy[a] * uy[b] + uz[a] * uz[b];
-                const double P[3] = {c, 1.5 * c * c - 0.5, (2.5 * c * c - 1.5) * c};
-                const double dP[3] = {1.0, 3.0 * c, 7.5 * c * c - 1.5};
-                double ra = 0.0, rb = 0.0, cc = 0.0;
-                for (int m = 0; m < M; ++m) {
-                    double A = 0.0, B = 0.0;
-                    for (int l = 0; l < L; ++l) {
-                        A += Fd[K + m * L + l] * P[l];
-                        B += Fd[K + m * L + l] * dP[l];
-                    }
-                    ra += df[m][a] * f[m][b] * A;
-                    rb += f[m][a] * df[m][b] * A;
-                    cc += f[m][a] * f[m][b] * B;
+        // walk 2: one partial force per list entry (zero outside the cut-off)
+        for (int k = 0; k < cnt; ++k) {
+            double dx, dy, dz;
+            const double r2 = pair_vec(k, dx, dy, dz);
+            double px = 0.0, py = 0.0, pz = 0.0;
+            if (r2 < rc2) {
+                const double inv = rsqrt(r2), r = r2 * inv;
+                const double x = dx * inv, y = dy * inv, z = dz * inv;
+                double f[kDnK], df[kDnK], m[kDnC];
+                dn_basis(r * irc, irc, f, df);
+                dn_monomials(x, y, z, m);
+                double C[kDnC], dphi = 0.0;  // C = sum_n f_n G_n (coefficients of phi), dphi = sum_n f_n' phi_n(u)
+#pragma unroll
+                for (int c = 0; c < kDnC; ++c) {
+                    C[c] = f[0] * S[0][c] + f[1] * S[1][c] + f[2] * S[2][c] + f[3] * S[3][c];
+                    dphi += (df[0] * S[0][c] + df[1] * S[1][c] + df[2] * S[2][c] + df[3] * S[3][c]) * m[c];
                 }
-                ra *= 2.0; rb *= 2.0; cc *= 2.0;
-                // d cos / d r^ij = (u^ik - cos u^ij) / r_ij
-                const double ca = cc * ir[a], cb = cc * ir[b];
-                px[a] += ra * ux[a] + ca * (ux[b] - c * ux[a]);
-                py[a] += ra * uy[a] + ca * (uy[b] - c * uy[a]);
-                pz[a] += ra * uz[a] + ca * (uz[b] - c * uz[a]);
-                px[b] += rb * ux[b] + cb * (ux[a] - c * ux[b]);
-                py[b] += rb * uy[b] + cb * (uy[a] - c * uy[b]);
-                pz[b] += rb * uz[b] + cb * (uz[a] - c * uz[b]);
+                const double gx = C[1] + 2.0 * C[4] * x + C[7] * y + C[8] * z + 3.0 * C[10] * m[4] + 2.0 * C[13] * m[7] +
+                                  2.0 * C[14] * m[8] + C[15] * m[5] + C[17] * m[6] + C[19] * m[9];
+                const double gy = C[2] + 2.0 * C[5] * y + C[7] * x + C[9] * z + 3.0 * C[11] * m[5] + C[13] * m[4] +
+                                  2.0 * C[15] * m[7] + 2.0 * C[16] * m[9] + C[18] * m[6] + C[19] * m[8];
+                const double gz = C[3] + 2.0 * C[6] * z + C[8] * x + C[9] * y + 3.0 * C[12] * m[6] + C[14] * m[4] +
+                                  C[16] * m[5] + 2.0 * C[17] * m[8] + 2.0 * C[18] * m[9] + C[19] * m[7];
+                const double ug = x * gx + y * gy + z * gz;
+                px = dphi * x + inv * (gx - ug * x);
+                py = dphi * y + inv * (gy - ug * y);
+                pz = dphi * z + inv * (gz - ug * z);
             }
-        for (int k = 0, a = 0; k < cnt; ++k) {
-            const bool hit = a < n && ek[a] == k;
-            part[(size_t)(k * 3 + 0) * d.Npad] = hit ? px[a] : 0.0;
-            part[(size_t)(k * 3 + 1) * d.Npad] = hit ? py[a] : 0.0;
-            part[(size_t)(k * 3 + 2) * d.Npad] = hit ? pz[a] : 0.0;
-            if (hit) ++a;
+            part[(size_t)(k * 3 + 0) * d.Npad] = px;
+            part[(size_t)(k * 3 + 1) * d.Npad] = py;
+            part[(size_t)(k * 3 + 2) * d.Npad] = pz;
         }
     }
     block_sum<1>(ui, red);
