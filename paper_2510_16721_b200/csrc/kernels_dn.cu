@@ -48,7 +48,10 @@ __device__ __forceinline__ void dn_basis(double t, double irc, double (&f)[kDnK]
     }
 }
 
-__global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int p_lo) {
+#ifndef DN_MINB
+#define DN_MINB 2
+#endif
+__global__ void __launch_bounds__(kThreadsAtom, DN_MINB) dn_partial_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
@@ -70,10 +73,22 @@ __global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int 
         double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + i;  // part[(k * 3 + m) * Npad]
         const double4 ri = Rc[i];
         const int cnt = d.nbr_count[(size_t)slot * d.Npad + i];
+        // the list walk is software-pipelined: entry k + 2 and the coordinates of entry k + 1 are in flight while
+        // entry k is evaluated (the list has 16 rows of slack behind the last one; index 0 is a valid atom)
+        uint32_t e_nn;
+        double4 rj_n;
+        uint32_t e_n;
+        auto walk_begin = [&]() {
+            e_n = lp[0];
+            e_nn = lp[(size_t)d.Npad];
+            rj_n = Rc[e_n & kIdxMask];
+        };
         auto pair_vec = [&](int k, double &dx, double &dy, double &dz) {
-            const uint32_t e = lp[(size_t)k * d.Npad];
-            const uint32_t code = e >> kShiftBits;
-            const double4 rj = Rc[e & kIdxMask];
+            const uint32_t code = e_n >> kShiftBits;
+            const double4 rj = rj_n;
+            e_n = e_nn;
+            e_nn = lp[(size_t)(k + 2) * d.Npad];
+            rj_n = Rc[e_n & kIdxMask];
             dx = rj.x - ri.x; dy = rj.y - ri.y; dz = rj.z - ri.z;
             if (code != kCodeCenter) {
                 const double n0 = (double)((int)(code & 7u) - 4), n1 = (double)((int)((code >> 3) & 7u) - 4),
@@ -90,6 +105,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int 
         for (int n = 0; n < kDnK; ++n)
 #pragma unroll
             for (int c = 0; c < kDnC; ++c) S[n][c] = 0.0;
+        walk_begin();
         for (int k = 0; k < cnt; ++k) {
             double dx, dy, dz;
             const double r2 = pair_vec(k, dx, dy, dz);
@@ -164,6 +180,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int 
             S[n][19] *= 6.0 * g3;
         }
         // walk 2: one partial force per list entry (zero outside the cut-off)
+        walk_begin();
         for (int k = 0; k < cnt; ++k) {
             double dx, dy, dz;
             const double r2 = pair_vec(k, dx, dy, dz);
