@@ -18,6 +18,7 @@
 //   p^ij = sum_n [ f_n'(r) phi_n(u) u + f_n(r)/r (I - u u^T) grad_u phi_n(u) ].
 // No per-thread environment array, hence no limit on the atoms inside the cut-off other than the list capacity.
 #include "cfneb_internal.cuh"
+#include "trig01.cuh"
 
 namespace cfn {
 
@@ -35,7 +36,7 @@ __device__ __forceinline__ void dn_monomials(double x, double y, double z, doubl
 // radial basis and its derivative with respect to r; t = r / r_c
 __device__ __forceinline__ void dn_basis(double t, double irc, double (&f)[kDnK], double (&df)[kDnK]) {
     double sn, cs;
-    sincospi(t, &sn, &cs);
+    sincospi01(t, sn, cs);  // 0 < t < 1 inside the cut-off
     const double fc = 0.5 + 0.5 * cs, dfc = -0.5 * sn * (3.14159265358979323846 * irc);
     const double x = 2.0 * (t - 1.0) * (t - 1.0) - 1.0, dx_dr = 4.0 * (t - 1.0) * irc;
     const double T[kDnK] = {1.0, x, 2.0 * x * x - 1.0, (4.0 * x * x - 3.0) * x};  // Chebyshev, closed forms
@@ -48,17 +49,17 @@ __device__ __forceinline__ void dn_basis(double t, double irc, double (&f)[kDnK]
     }
 }
 
-#ifndef DN_MINB
-#define DN_MINB 2
-#endif
-__global__ void __launch_bounds__(kThreadsAtom, DN_MINB) dn_partial_kernel(Dev d, int p_lo) {
+// MT = number of radial functions with angular channels (pot[2]): the moments of order 1..3 of the others are never
+// formed, which frees their registers.
+template <int MT>
+__global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     __shared__ double sh[9];
     __shared__ double red[32];
     __shared__ double sW[kDnWeights];
-    const int K = (int)d.pot[1], M = (int)d.pot[2], L = (int)d.pot[3], H = (int)d.pot[4], D = K + M * L;
+    const int K = (int)d.pot[1], M = MT, L = (int)d.pot[3], H = (int)d.pot[4], D = K + M * L;
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
     for (int t = threadIdx.x; t < H * D + 2 * H; t += blockDim.x) sW[t] = d.dn_w[t];
     __syncthreads();
@@ -117,12 +118,13 @@ __global__ void __launch_bounds__(kThreadsAtom, DN_MINB) dn_partial_kernel(Dev d
 #pragma unroll
             for (int n = 0; n < kDnK; ++n)
 #pragma unroll
-                for (int c = 0; c < kDnC; ++c) S[n][c] += f[n] * m[c];
+                for (int c = 0; c < kDnC; ++c)
+                    if (c == 0 || n < MT) S[n][c] += f[n] * m[c];
         }
         // descriptors of the angular channels (dense [n][l]; the radial ones are S[k][0])
-        double qa[kDnK][kDnL];
+        double qa[kDnK][kDnL] = {};
 #pragma unroll
-        for (int n = 0; n < kDnK; ++n) {
+        for (int n = 0; n < MT; ++n) {
             const double s1 = S[n][1] * S[n][1] + S[n][2] * S[n][2] + S[n][3] * S[n][3];
             const double s2 = S[n][4] * S[n][4] + S[n][5] * S[n][5] + S[n][6] * S[n][6] +
                               2.0 * (S[n][7] * S[n][7] + S[n][8] * S[n][8] + S[n][9] * S[n][9]);
@@ -166,6 +168,7 @@ __global__ void __launch_bounds__(kThreadsAtom, DN_MINB) dn_partial_kernel(Dev d
 #pragma unroll
         for (int n = 0; n < kDnK; ++n) {
             S[n][0] = Fr[n] - Fa[n][1] * S[n][0];
+            if (n >= MT) continue;
             const double g1 = 2.0 * Fa[n][0] - 3.0 * Fa[n][2], g2 = 3.0 * Fa[n][1], g3 = 5.0 * Fa[n][2];
 #pragma unroll
             for (int c = 1; c < 4; ++c) S[n][c] *= g1;
@@ -194,8 +197,12 @@ __global__ void __launch_bounds__(kThreadsAtom, DN_MINB) dn_partial_kernel(Dev d
                 double C[kDnC], dphi = 0.0;  // C = sum_n f_n G_n (coefficients of phi), dphi = sum_n f_n' phi_n(u)
 #pragma unroll
                 for (int c = 0; c < kDnC; ++c) {
-                    C[c] = f[0] * S[0][c] + f[1] * S[1][c] + f[2] * S[2][c] + f[3] * S[3][c];
-                    dphi += (df[0] * S[0][c] + df[1] * S[1][c] + df[2] * S[2][c] + df[3] * S[3][c]) * m[c];
+                    double cc = 0.0, dc = 0.0;
+#pragma unroll
+                    for (int n = 0; n < kDnK; ++n)
+                        if (c == 0 || n < MT) { cc += f[n] * S[n][c]; dc += df[n] * S[n][c]; }
+                    C[c] = cc;
+                    dphi += dc * m[c];
                 }
                 const double gx = C[1] + 2.0 * C[4] * x + C[7] * y + C[8] * z + 3.0 * C[10] * m[4] + 2.0 * C[13] * m[7] +
                                   2.0 * C[14] * m[8] + C[15] * m[5] + C[17] * m[6] + C[19] * m[9];
@@ -221,7 +228,12 @@ void launch_force_dn(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
-    dn_partial_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+    switch ((int)d.pot[2]) {
+        case 1: dn_partial_kernel<1><<<grid, kThreadsAtom, 0, st>>>(d, p_lo); break;
+        case 2: dn_partial_kernel<2><<<grid, kThreadsAtom, 0, st>>>(d, p_lo); break;
+        case 3: dn_partial_kernel<3><<<grid, kThreadsAtom, 0, st>>>(d, p_lo); break;
+        default: dn_partial_kernel<4><<<grid, kThreadsAtom, 0, st>>>(d, p_lo); break;
+    }
     launch_pair_forces_manybody(d, p_lo, st);
 }
 
