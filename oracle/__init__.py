@@ -10,8 +10,9 @@ Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` / `--im
 legs may import, call, link or execute anything under `oracle/`.
 
 Modules
-  forcefield.c / forcefield.py   O2 neighbours (brute force = definition; cell list), O3 potentials,
-                                 forces, virial (Eq. 4-9)
+  forcefield.c / forcefield.py   O2 neighbours (brute force = definition; cell list), O3 potentials (LJ shifted
+                                 force, Finnis-Sinclair type, Stillinger-Weber, descriptor network of NEP's
+                                 shape with seeded weights), forces, virial (Eq. 4-9)
   cellfilter.py                  O0 input mapping, O1 cell map D = sqrt(B), O4 generalized force (Eq. 10-17)
   neb.py                         O5 improved tangent, O6 NEB / climbing-image force (Eq. 1), O7 FIRE,
                                  O8 measures; generic over a band of n-dof points with a callback

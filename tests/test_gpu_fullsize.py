@@ -1,4 +1,5 @@
-"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (configs[3], configs[4]).
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (configs[3], configs[4]; the
+many-body workloads 5 and 6 at their full atom count).
 
 configs[4] (101 306 atoms x 100 images): the oracle is run on ALL images with every host core (one evaluation of
 the band at construction + one full step: about a minute on 16 cores), and every output is compared element by
@@ -160,4 +161,33 @@ def test_c4_long_run_survives_equal_energy_images():
     assert np.all(np.isfinite(E))
     seg = gpu.get_segment_lengths()
     assert seg.min() > 0.0
+    gpu.close()
+
+
+@pytest.mark.parametrize("k", [5, 6])
+def test_many_body_workloads_at_full_atom_count(k):
+    """The many-body workloads bench.py --config 5 / 6 times (32 768 atoms; Stillinger-Weber and the descriptor
+    network of NEP's shape) at their full atom count in the same launch configuration, on the first, two mid-path and
+    the last image of the 32: energies, per-atom forces, virials and f^NEB element by element, then two full steps."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(k)
+    idx = [0, 15, 16, spec.n_images - 1]
+    pos, cells = pos[idx], cells[idx]
+    orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors, threads=min(4, host_threads()))
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, max_images=4))
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE
+    assert rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
+    assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    X0, _ = orc.get_state()
+    orc.step(2)
+    gpu.step(2)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < 1e-8 and rel(vg, vo) < 1e-8
+    assert gpu.get_status().error == 0
     gpu.close()
