@@ -886,3 +886,53 @@ def test_descriptor_network_parameter_errors():
         pot = dn_params(**bad)
         prm = cf.default_params(potential=cf.POT_DNN, pot=list(pot), max_images=3)
         assert cf.binding.workspace_bytes(64, prm) == 0
+
+
+def test_descriptor_network_with_the_rest_of_the_path():
+    """The descriptor-network potential through the parts of the path that do not know the potential: external
+    pressure with the Eq. 14 cell force (CELL_D), device-side adaptive control, and the endpoint relaxation -- each
+    against the oracle on a disordered strained diamond band."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import diamond_strain_band, dn_params
+    from oracle import cfneb as oc
+    from oracle import cellfilter as ocf
+    pot = dn_params(rc=3.9, K=3, M=2, L=3, H=6, seed=5)
+    pos, cells = diamond_strain_band((2, 2, 3), 5.35, 5, 31, 0.06, ((0.0, 0.04, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.05)))
+    fire = dict(dt0=0.02, dtmax=0.1, maxstep=0.02, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+    # pressure + CELL_D
+    orc = oc.CFNEB(pos, cells, 3, pot, pot[0], k_spring=1.0, climb=True, cell_factor=0.0, fire=fire, skin=0.3, max_neighbors=96,
+                   cell_mode=ocf.CELL_D, pressure=0.05)
+    prm = cf.default_params(potential=cf.POT_DNN, pot=list(pot), k_spring=1.0, climb=1, cell_factor=0.0, skin=0.3,
+                            max_neighbors=96, max_images=8, fire=fire, cell_mode=cf.CELL_D, pressure=0.05)
+    gpu = cf.CFNEB(pos, cells, prm)
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE and rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
+    assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    X0, _ = orc.get_state()
+    orc.step(5)
+    gpu.step(5)
+    assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
+    # an inserted image is evaluated with the same kernels
+    seg = gpu.get_segment_lengths()
+    p = int(np.argmax(seg))
+    gpu.insert_image(p)
+    orc.insert_image(p)
+    orc.step(3)
+    gpu.step(3)
+    Xo, Xg = orc.get_state()[0], gpu.get_state()[0]
+    assert Xg.shape == Xo.shape and rel(Xg, Xo) < 1e-9
+    assert gpu.get_status().error == 0
+    gpu.close()
+    # endpoint relaxation, 15 updates
+    kw = dict(fmax_tol=0.0, max_steps=15, cell_factor=0.0, fire=fire, skin=0.3, max_neighbors=96)
+    Ra, ha, _, _, _ = oc.relax_endpoint(pos[0], cells[0], 3, pot, pot[0], **kw)
+    prm2 = cf.default_params(potential=cf.POT_DNN, pot=list(pot), k_spring=1.0, climb=0, cell_factor=0.0, skin=0.3,
+                             max_neighbors=96, max_images=4, fire=fire)
+    gpu = cf.CFNEB(np.stack([pos[0], pos[-1]]), np.stack([cells[0], cells[-1]]), prm2, n_images=4)
+    steps, fmax, en = gpu.relax_endpoints(0.0, 15, rebuild_band=False)
+    p2, c2, _ = gpu.get_path()
+    assert steps == [15, 15]
+    assert rel(p2[0] - pos[0], Ra - pos[0]) < 1e-8 and rel(c2[0] - cells[0], ha - cells[0]) < 1e-8
+    assert gpu.get_status().error == 0
+    gpu.close()
