@@ -213,6 +213,15 @@ __device__ inline int first_dead_tail_bucket(double r_cut, double r_list, double
     return kTailBuckets;
 }
 
+// Rows of atom i's (distance-sorted) list that can hold a pair inside r_cut now: everything before the first dead
+// tail bucket.  The mirror entry (j; i, -n) of a row below this bound lies below j's bound (same distance, same
+// bucket; a pair whose two entries straddle a bucket edge by rounding is out of range by the margin of `need`).
+__device__ inline int live_rows(const Dev &d, int slot, int i) {
+    const int t_dead = first_dead_tail_bucket(d.r_cut, d.r_list, d.geom[slot].acc);
+    return t_dead < kTailBuckets ? (int)d.nbr_tail[((size_t)slot * kTailBuckets + t_dead) * d.Npad + i]
+                                 : d.nbr_count[(size_t)slot * d.Npad + i];
+}
+
 __device__ inline void set_error(Ctl *ctl, int code) { atomicCAS(&ctl->error, 0, code); }
 
 // block-wide sum of NV values per thread; result valid in thread 0. blockDim.x a multiple of 32, <= 1024.

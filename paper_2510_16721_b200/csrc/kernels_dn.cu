@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int 
         const uint32_t *lp = d.nbr_list + (size_t)slot * d.cap * d.Npad + i;
         double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + i;  // part[(k * 3 + m) * Npad]
         const double4 ri = Rc[i];
-        const int cnt = d.nbr_count[(size_t)slot * d.Npad + i];
+        const int cnt = live_rows(d, slot, i);  // rows past it cannot be in range and are neither written nor read
         // the list walk is software-pipelined: entry k + 2 and the coordinates of entry k + 1 are in flight while
         // entry k is evaluated (the list has 16 rows of slack behind the last one; index 0 is a valid atom)
         uint32_t e_nn;

@@ -50,7 +50,7 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_partial_kernel(Dev d, int p_l
         const uint32_t *lp = d.nbr_list + (size_t)slot * d.cap * d.Npad + i;
         double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + i;  // part[(k * 3 + m) * Npad]
         const double4 ri = Rc[i];
-        const int cnt = d.nbr_count[(size_t)slot * d.Npad + i];
+        const int cnt = live_rows(d, slot, i);  // rows past it cannot be in range and are neither written nor read
         double ex[kMaxEnv], ey[kMaxEnv], ez[kMaxEnv], er[kMaxEnv], px[kMaxEnv], py[kMaxEnv], pz[kMaxEnv];
         int ek[kMaxEnv];
         int n = 0;
@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
         const uint32_t *lists = d.nbr_list + (size_t)slot * d.cap * d.Npad;
         const double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad;
         const double4 ri = Rc[i];
-        const int cnt = d.nbr_count[(size_t)slot * d.Npad + i];
+        const int cnt = live_rows(d, slot, i);  // rows past it cannot be in range and are neither written nor read
         for (int k = 0; k < cnt; ++k) {
             const uint32_t e = lists[(size_t)k * d.Npad + i];
             const uint32_t j = e & kIdxMask, code = e >> kShiftBits;
