@@ -156,6 +156,81 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
     }
 }
 
+// Pass 2 for environments with many atoms inside the cut-off (descriptor network: 16 and more): U list rows per
+// iteration, their loads issued together in two rounds (entries and mirror rows; then coordinates of j and both
+// partial forces).  The walk is bound by the latency of these dependent gathers, not by bandwidth; a row past the
+// count is replaced by row 0 and masked.  Measured at c6: 1.10 -> 1.00 ms per K2.  Where most live rows are outside
+// the cut-off (Stillinger-Weber diamond: 4 of 5-16) the unconditional loads cost more than they hide (c5 0.50 ->
+// 0.54 ms), and loading the partial forces in a third round after the range test loses the gain (c6 1.10, c5 0.52):
+// that case keeps sw_force_kernel.
+template <int U>
+__global__ void __launch_bounds__(kThreadsAtom) pair_force_batched_kernel(Dev d, int p_lo) {
+    int p;
+    if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
+    const int slot = d.order[p];
+    __shared__ double sh[9];
+    __shared__ double red[32 * 7];
+    if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool valid = i < d.N;
+    const double rc2 = d.r_cut * d.r_cut;
+    double fx = 0.0, fy = 0.0, fz = 0.0, vxx = 0.0, vyy = 0.0, vzz = 0.0, vxy = 0.0, vxz = 0.0, vyz = 0.0;
+    if (valid) {
+        const double4 *Rc = d.Rc + (size_t)slot * d.Npad;
+        const uint32_t *lists = d.nbr_list + (size_t)slot * d.cap * d.Npad;
+        const double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad;
+        const double4 ri = Rc[i];
+        const int cnt = live_rows(d, slot, i);  // rows past it cannot be in range and are neither written nor read
+        const unsigned short *mir = d.nbr_mirror + (size_t)slot * d.cap * d.Npad + i;
+        for (int k0 = 0; k0 < cnt; k0 += U) {
+            uint32_t e[U];
+            int l[U];
+            bool live[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                live[u] = k0 + u < cnt;
+                const int k = live[u] ? k0 + u : 0;
+                e[u] = lists[(size_t)k * d.Npad + i];
+                l[u] = mir[(size_t)k * d.Npad];
+            }
+            double4 rj[U];
+            double q[U][3], pp[U][3];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const uint32_t j = e[u] & kIdxMask;
+                const int k = live[u] ? k0 + u : 0, lc = l[u] < d.cap ? l[u] : 0;
+                rj[u] = Rc[j];
+#pragma unroll
+                for (int m = 0; m < 3; ++m) {
+                    q[u][m] = part[(size_t)(lc * 3 + m) * d.Npad + j];
+                    pp[u][m] = part[(size_t)(k * 3 + m) * d.Npad + i];
+                }
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                double dx, dy, dz;
+                shifted_vec(ri, rj[u], e[u] >> kShiftBits, sh, dx, dy, dz);
+                if (!live[u] || !(dx * dx + dy * dy + dz * dz < rc2)) continue;
+                if (l[u] >= d.cap) { set_error(d.ctl, CFNEB_EINVAL); continue; }  // no mirror entry (j; i, -n)
+                const double gx = pp[u][0] - q[u][0], gy = pp[u][1] - q[u][1], gz = pp[u][2] - q[u][2];  // Eq. 5
+                fx += gx; fy += gy; fz += gz;
+                vxx += dx * gx; vyy += dy * gy; vzz += dz * gz;  // Eq. 8; the total is symmetric, the halves are summed
+                vxy += 0.5 * (dx * gy + dy * gx); vxz += 0.5 * (dx * gz + dz * gx); vyz += 0.5 * (dy * gz + dz * gy);
+            }
+        }
+        double *F = d.F + (size_t)slot * 3 * d.Npad;
+        F[i] = fx; F[d.Npad + i] = fy; F[2 * (size_t)d.Npad + i] = fz;
+    }
+    double out7[7] = {0.0, -0.5 * vxx, -0.5 * vyy, -0.5 * vzz, -0.5 * vxy, -0.5 * vxz, -0.5 * vyz};
+    block_sum<7>(out7, red);
+    if (threadIdx.x == 0) {
+        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+#pragma unroll
+        for (int n = 0; n < 7; ++n) out[n] = out7[n];
+    }
+}
+
 // After a list build: for every entry (i; j, n) the row of its mirror (j; i, -n) in j's list (cap if absent).
 __global__ void __launch_bounds__(kThreadsAtom) sw_mirror_kernel(Dev d, int p_lo) {
     int p;
@@ -190,7 +265,8 @@ void launch_pair_forces_manybody(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
-    sw_force_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+    if (d.potential == CFNEB_POT_DNN) pair_force_batched_kernel<4><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+    else sw_force_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
 }
 
 void launch_force_sw(const Dev &d, int p_lo, cudaStream_t st) {
