@@ -3,7 +3,8 @@
 // (Eq. 4-8; the paper's own potential, NEP, is of this class -- its trained weights are not available,
 // SURVEY.md section 8(f) item 4):
 //   pass 1 (sw_partial_kernel)  U_i and the partial forces p^ij = dU_i/dr^ij, one vector per list entry, stored
-//   pass 2 (sw_force_kernel)    f^ij = p^ij - p^ji (Eq. 5; p^ji sits at the mirror entry (j; i, -n) of j's list,
+//   pass 2 (sw_force_kernel; pair_force_batched_kernel for the descriptor network of kernels_dn.cu)
+//                               f^ij = p^ij - p^ji (Eq. 5; p^ji sits at the mirror entry (j; i, -n) of j's list,
 //                               whose row is tabulated once per list build by sw_mirror_kernel),
 //                               F_i = sum_j f^ij,  V = -1/2 sum_i sum_j r^ij (x) f^ij  (Eq. 8)
 //   U_i = 1/2 sum_j phi2(r_ij) + sum_{j<k} h(r_ij, r_ik, cos theta_jik),  r_c = a sigma,
