@@ -56,10 +56,18 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_partial_kernel(Dev d, int p_l
         int ek[kMaxEnv];
         int n = 0;
         bool overflow = false;
+        // entry k + 2 and the coordinates of entry k + 1 are in flight while entry k is tested (rows past the
+        // count are readable: stale or zero entries, 16 rows of slack)
+        uint32_t e_n = lp[0], e_nn = lp[(size_t)d.Npad];
+        double4 rj_n = Rc[e_n & kIdxMask];
         for (int k = 0; k < cnt; ++k) {
-            const uint32_t e = lp[(size_t)k * d.Npad];
+            const uint32_t e = e_n;
+            const double4 rj = rj_n;
+            e_n = e_nn;
+            e_nn = lp[(size_t)(k + 2) * d.Npad];
+            rj_n = Rc[e_n & kIdxMask];
             double dx, dy, dz;
-            shifted_vec(ri, Rc[e & kIdxMask], e >> kShiftBits, sh, dx, dy, dz);
+            shifted_vec(ri, rj, e >> kShiftBits, sh, dx, dy, dz);
             const double r2 = dx * dx + dy * dy + dz * dz;
             if (r2 < rc2) {
                 if (n < kMaxEnv) {
