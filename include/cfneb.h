@@ -125,6 +125,14 @@ typedef struct cfneb_status {
     double path_length;     /* sum_p |X_{p+1} - X_p| at the last evaluation */
 } cfneb_status;
 
+/* The scalar part of a checkpoint: the FIRE state of the band (O7; one state for the whole band, A3) and the
+ * iteration counter.  first = 1: the next step skips the power test (A2). */
+typedef struct cfneb_fire_state {
+    double dt, alpha;
+    int64_t steps;
+    int32_t n_pos, first;
+} cfneb_fire_state;
+
 /* Kernel classes timed by cfneb_step_timed. */
 enum {
     CFNEB_K_CELLPREP = 0,  /* K0  cell map D = sqrt(B), Cartesian positions */
@@ -142,7 +150,8 @@ enum {
 CFNEB_API void cfneb_default_params(cfneb_params *prm);
 
 /* Bytes of device workspace cfneb_create needs for n_atoms atoms and prm->max_images images
- * (0 on invalid arguments).  c4 (101306 atoms x 100 images, 160 neighbours): about 9 GB. */
+ * (0 on invalid arguments).  c4 (101306 atoms x 100 images, list capacity 224): 23.6 GB, of which 9.1 GB are the
+ * neighbour lists and 11.4 GB the scratch of a rebuild of all images at once. */
 CFNEB_API size_t cfneb_workspace_bytes(int32_t n_atoms, const cfneb_params *prm);
 
 /*
@@ -216,16 +225,45 @@ CFNEB_API int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_ste
  * Any of pos/cells/energies may be NULL.  Synchronises. */
 CFNEB_API int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, double *energies);
 
-/* Replace all P images from HOST Cartesian data (pos P*N*3, cells P*9; image 0's cell must equal h0);
- * resets the FIRE state; endpoint energies are re-evaluated, interior energies by the next cfneb_step /
- * cfneb_get_forces (or on demand by cfneb_get_path).  Neighbour lists are kept: the distance of the new coordinates
- * from the stored ones is added to each image's displacement bound, so only images that left their skin rebuild
- * (restoring a checkpoint of the running band, or editing a few images on the host, rebuilds nothing else).
- * Synchronises. */
+/* Replace all P images from HOST Cartesian data (pos P*N*3, cells P*9; image 0's cell must equal h0).
+ * This is a NEW PATH, not a resume: the FIRE state is reset (v = 0, dt = dt0, first step), and X is re-derived from
+ * the Cartesian data (R~ = R D^-1, B = D D^T), so it need not equal bit for bit the X it was exported from -- to
+ * continue a stopped band use cfneb_get_checkpoint / cfneb_set_state.  Endpoint energies are re-evaluated, interior
+ * energies by the next cfneb_step / cfneb_get_forces (or on demand by cfneb_get_path).  Neighbour lists are kept: the
+ * distance of the new coordinates from the stored ones is added to each image's displacement bound, so only images
+ * that left their skin rebuild (editing a few images on the host rebuilds nothing else).  Synchronises. */
 CFNEB_API int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells);
 
-/* Generalized coordinates X and FIRE velocities v, each P*(N+3)*3 (checkpoint; either may be NULL). */
+/* Generalized coordinates X and FIRE velocities v, each P*(N+3)*3 (either may be NULL).  Read only. */
 CFNEB_API int cfneb_get_state(cfneb_t *h, double *X, double *v);
+
+/*
+ * Checkpoint of the running band ("structural information is always kept and updated on GPU": this is the
+ * way out and back in).  Everything the next iteration depends on, so that
+ *     cfneb_get_checkpoint -> cfneb_destroy -> cfneb_create(same endpoints, same params, P images) -> cfneb_set_state
+ * continues BIT FOR BIT as the uninterrupted band would have:
+ *   X, v      P*(N+3)*3 each, as cfneb_get_state;
+ *   X_list    P*(N+3)*3: the generalized coordinates at which each image's neighbour list was last built (the
+ *             order of a list's entries fixes the summation order of the forces, so a resume replays the builds);
+ *   list_aux  P*4: per image {max_i |R~_i - R~_i(build)|^2 at the last cell map, max_i |dR~_i|^2 of the last update,
+ *             iterations since the build, 0} -- the staleness accounting that decides the next rebuild;
+ *   fire      the FIRE scalars and the iteration counter.
+ * All HOST, any may be NULL.  Read only; synchronises.
+ */
+CFNEB_API int cfneb_get_checkpoint(cfneb_t *h, double *X, double *v, double *X_list, double *list_aux,
+                                   cfneb_fire_state *fire);
+
+/*
+ * Restore a checkpoint into a band of the same P, N and parameters.  X is copied as given (no round trip through
+ * Cartesian coordinates), v as given (endpoint rows are ignored: zero); fire == NULL restarts FIRE (v is then zeroed).
+ * With X_list and list_aux the neighbour lists are rebuilt at X_list and the accounting restored, which makes the
+ * continuation bit-identical (given the atom order of the handle: the same pos_init at cfneb_create); with
+ * X_list == NULL the lists are built fresh at X and the continuation agrees to round-off only (summation order).
+ * Endpoint energies are re-evaluated, interior energies by the next step (as cfneb_set_path).  Synchronises.
+ * Errors: CFNEB_EINVAL (null X, X_list without list_aux, fire scalars out of range).
+ */
+CFNEB_API int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *X_list,
+                              const double *list_aux, const cfneb_fire_state *fire);
 
 /* Parity hook: evaluate forces at the CURRENT X without updating anything.  F: P*N*3 Cartesian forces
  * (Eq. 5), virial: P*9 (Eq. 8), f_neb: P*(N+3)*3 NEB force of Eq. 1 in generalized coordinates (zero rows

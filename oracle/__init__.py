@@ -20,6 +20,7 @@ Modules
   mullerbrown.py                 analytic 2-D Mueller-Brown surface (pin for neb.py)
 
 Parity pins: see DESIGN.md section 4.  The Bain-path bands (c2-c4) are pinned by the saddle of the closed-form
-lattice-sum surface E(a, c) (tests/bain_surface.py).  Unpinned (stated here as required): the adaptive
-insertion/deletion rule (O9) is a reading of P:128 with structural invariants only -- "parity unpinned".
+lattice-sum surface E(a, c) (tests/bain_surface.py).  The adaptive insertion/deletion rule (O9) is a reading of
+P:128 (the paper states the principle only); it is pinned by a hand-worked band whose expected deletion, insertion
+and order are written out from the rule's text (tests/test_oracle_cfneb.py).  No function here is unpinned.
 """

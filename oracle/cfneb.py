@@ -10,7 +10,7 @@ image distribution, `adapt()`).  Composition of O0-O9:
   O3 U, F, V                forcefield.c                    Eq. 4, 5, 8
   O4 generalized force      cellfilter.generalized_force    Eq. 17
   O5-O8                     neb.py                          Eq. 1, refs [12], [13]
-  O9 adaptive control       adapt() below                   P:128 (reading A16 -- parity unpinned)
+  O9 adaptive control       adapt() below                   P:128 (reading A16; hand-worked pin)
 
 External pressure (reading A25; the paper's graphite band is "under 40GPa", Fig. 3 caption, without
 equations): a hydrostatic pressure p replaces U by the enthalpy H = U + p Omega, Omega = |det h|.  With the
@@ -205,7 +205,7 @@ def relax_endpoint(R, h, potential, pot, r_cut, fmax_tol=1e-4, max_steps=20000, 
     lam = auto_cell_factor(h0, N) if cell_factor == 0 else float(cell_factor)
     ev = CrystalEvaluator(h0, potential, pot, r_cut + skin, max_neighbors, lam, cell_mode, pressure=pressure)
     Rt, B, D = cf.input_mapping(R, h, h0)
-    X = cf.pack(Rt, B, lam)
+    X = cf.pack(Rt, D if cell_mode == cf.CELL_D else B, lam)  # Eq. 14 coordinates (R~, D) / Eq. 17 (R~, B)
     fire = Fire((1,) + X.shape, **(fire or {}))
     E, fmax, it = np.nan, np.inf, 0
     for it in range(max_steps):
@@ -215,6 +215,7 @@ def relax_endpoint(R, h, potential, pot, r_cut, fmax_tol=1e-4, max_steps=20000, 
         if fmax < fmax_tol:
             break
         X = X + fire.step(G[None], X.shape[0])[0]
-        X[-3:] = 0.5 * (X[-3:] + X[-3:].T)
+        if cell_mode == cf.CELL_B:  # O7 step 4: B <- 1/2 (B + B^T); D of Eq. 14 is not symmetric in general
+            X[-3:] = 0.5 * (X[-3:] + X[-3:].T)
     Rt, D = ev.deformation(X)
     return Rt @ D, h0 @ D, E, fmax, it

@@ -21,7 +21,7 @@ EXPORTS = (
     "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_adaptive", "cfneb_step_timed",
     "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
     "cfneb_get_path",
-    "cfneb_set_path", "cfneb_get_state", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
+    "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
     "cfneb_destroy", "cfneb_strerror", "cfneb_last_cuda_error", "cfneb_util_fp64_peak",
 )
 
@@ -51,6 +51,12 @@ class Status(ctypes.Structure):
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_ if not k.startswith("reserved")}
+
+
+class FireState(ctypes.Structure):
+    """cfneb_fire_state (include/cfneb.h)."""
+    _fields_ = [("dt", ctypes.c_double), ("alpha", ctypes.c_double), ("steps", ctypes.c_int64),
+                ("n_pos", ctypes.c_int32), ("first", ctypes.c_int32)]
 
 
 class CfnebError(RuntimeError):
@@ -87,6 +93,8 @@ def lib():
         ("cfneb_delete_image", [vp, i32]), ("cfneb_adapt", [vp, f64, f64, ip, ip]),
         ("cfneb_relax_endpoints", [vp, f64, i32, i32, ip, dp, dp]), ("cfneb_get_segment_lengths", [vp, dp]), ("cfneb_get_path", [vp, ip, dp, dp, dp]),
         ("cfneb_set_path", [vp, dp, dp]), ("cfneb_get_state", [vp, dp, dp]),
+        ("cfneb_get_checkpoint", [vp, dp, dp, dp, dp, ctypes.POINTER(FireState)]),
+        ("cfneb_set_state", [vp, dp, dp, dp, dp, ctypes.POINTER(FireState)]),
         ("cfneb_get_forces", [vp, dp, dp, dp, dp]), ("cfneb_get_neighbors", [vp, i32, ip, ip, ip]),
         ("cfneb_get_status", [vp, ctypes.POINTER(Status)]), ("cfneb_util_fp64_peak", [vp, dp]),
     ):
@@ -293,6 +301,29 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_get_state")
         return X, v
+
+    def get_checkpoint(self):
+        """cfneb_get_checkpoint: dict(X, v, X_list, list_aux, fire) -- everything cfneb_set_state needs to continue
+        the band bit for bit in a new handle."""
+        P = self.P
+        X, v, Xl = (np.zeros((P, self.N + 3, 3)) for _ in range(3))
+        aux = np.zeros((P, 4))
+        fire = FireState()
+        rc = lib().cfneb_get_checkpoint(self._h, _dptr(X), _dptr(v), _dptr(Xl), _dptr(aux), ctypes.byref(fire))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_checkpoint")
+        return dict(X=X, v=v, X_list=Xl, list_aux=aux, fire=fire)
+
+    def set_state(self, X, v=None, X_list=None, list_aux=None, fire=None):
+        """cfneb_set_state; arrays may be caller-owned (e.g. pinned) float64 buffers."""
+        X = _f64(X)
+        v = _f64(v) if v is not None else None
+        X_list = _f64(X_list) if X_list is not None else None
+        list_aux = _f64(list_aux) if list_aux is not None else None
+        rc = lib().cfneb_set_state(self._h, _dptr(X), _dptr(v), _dptr(X_list), _dptr(list_aux),
+                                   ctypes.byref(fire) if fire is not None else None)
+        if rc:
+            raise CfnebError(rc, "cfneb_set_state")
 
     def get_forces(self, forces=True, f_neb=True):
         P = self.P

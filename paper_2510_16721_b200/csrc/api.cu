@@ -37,6 +37,20 @@ struct cfneb {
     int graph_nodes;
     bool mirror_dirty;    // the device edited P / order / free slots (cfneb_step_adaptive); host mirrors are stale
     bool interior_stale;  // cfneb_set_path replaced the path and the interior images have not been evaluated since
+    int device;           // CUDA device the workspace and the stream live on (current at cfneb_create)
+};
+
+// Every ABI entry runs with the handle's device current and puts the caller's back on return, so a handle on
+// cuda:1 works while cuda:0 is current.
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const cfneb *h) {
+        int cur = -1;
+        if (h && cudaGetDevice(&cur) == cudaSuccess && cur != h->device && cudaSetDevice(h->device) == cudaSuccess) prev = cur;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceGuard(const DeviceGuard &) = delete;
+    DeviceGuard &operator=(const DeviceGuard &) = delete;
 };
 
 // ---- workspace carving (one function serves the size query and create) ----
@@ -123,6 +137,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.dispmax_in = c.take<unsigned long long>(S);
     d.disptot = c.take<unsigned long long>(S);
     d.Xb = c.take<double>(S * img);
+    d.Xcb = c.take<double>(S * 9);
     d.nbr_count = c.take<int>(S * Npad);
     d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 16 * Npad);  // 16 rows of slack for the force kernels' look-ahead
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
@@ -294,6 +309,12 @@ int set_reference_frame(cfneb *h, const double *cell_init, const double *cell_fi
     return CFNEB_OK;
 }
 
+int no_graph() {  // a failed cfneb_relax_endpoints(rebuild_band) leaves the handle without its iteration graph
+    snprintf(g_cuda_err, sizeof g_cuda_err, "the handle has no iteration graph (an earlier cfneb_relax_endpoints failed while "
+             "rebuilding the band); destroy it and create a new one");
+    return CFNEB_ECUDA;
+}
+
 int capture_graph(cfneb *h) {
     CK(cudaStreamBeginCapture(h->st, cudaStreamCaptureModeRelaxed));
     enqueue_step(h, nullptr);
@@ -357,6 +378,8 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     h->interior_stale = false;
     h->mirror_dirty = false;
     h->st = static_cast<cudaStream_t>(cuda_stream);
+    h->device = 0;
+    cudaGetDevice(&h->device);
 #define CKH(call)                                  \
     do {                                           \
         int rc_ = (call);                          \
@@ -472,14 +495,18 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
 }
 
 int cfneb_step(cfneb_t *h, int32_t n_steps) {
+    DeviceGuard dev_guard(h);
     if (!h || n_steps < 0) return CFNEB_EINVAL;
+    if (!h->exec) return no_graph();
     if (n_steps > 0) h->interior_stale = false;
     for (int k = 0; k < n_steps; ++k) CK(cudaGraphLaunch(h->exec, h->st));
     return CFNEB_OK;
 }
 
 int cfneb_step_adaptive(cfneb_t *h, int32_t n_steps, int32_t adapt_every, double d_insert, double d_delete) {
+    DeviceGuard dev_guard(h);
     if (!h || n_steps < 0 || adapt_every < 1) return CFNEB_EINVAL;
+    if (!h->exec) return no_graph();
     if (n_steps > 0) h->interior_stale = false;
     for (int k = 1; k <= n_steps; ++k) {
         CK(cudaGraphLaunch(h->exec, h->st));
@@ -493,6 +520,7 @@ int cfneb_step_adaptive(cfneb_t *h, int32_t n_steps, int32_t adapt_every, double
 }
 
 int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms) {
+    DeviceGuard dev_guard(h);
     if (!h || n_steps < 0 || !kernel_ms) return CFNEB_EINVAL;
     if (n_steps > 0) h->interior_stale = false;
     // one event set per step, read back after the last step: no host synchronisation between steps
@@ -519,6 +547,7 @@ int cfneb_step_timed(cfneb_t *h, int32_t n_steps, double *kernel_ms) {
 }
 
 int cfneb_insert_image(cfneb_t *h, int32_t after) {
+    DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (after < 0 || after > h->P - 2) return CFNEB_ERANGE;
@@ -544,6 +573,7 @@ int cfneb_insert_image(cfneb_t *h, int32_t after) {
 }
 
 int cfneb_delete_image(cfneb_t *h, int32_t index) {
+    DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (index < 1 || index > h->P - 2 || h->P <= 3) return CFNEB_ERANGE;
@@ -567,6 +597,7 @@ int cfneb_delete_image(cfneb_t *h, int32_t index) {
 }
 
 int cfneb_get_segment_lengths(cfneb_t *h, double *dl) {
+    DeviceGuard dev_guard(h);
     if (!h || !dl) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     double *dev = static_cast<double *>(h->d.scratch);
@@ -576,6 +607,7 @@ int cfneb_get_segment_lengths(cfneb_t *h, double *dl) {
 }
 
 int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, int32_t *n_del) {
+    DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (n_ins) *n_ins = 0;
@@ -617,6 +649,7 @@ int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, in
 
 int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_t rebuild_band, int32_t *steps_done,
                           double *fmax_out, double *energy_out) {
+    DeviceGuard dev_guard(h);
     if (!h || !(fmax_tol >= 0.0) || max_steps < 0) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
@@ -688,6 +721,7 @@ int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_
 }
 
 int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, double *energies) {
+    DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
@@ -707,6 +741,7 @@ int cfneb_get_path(cfneb_t *h, int32_t *n_images, double *pos, double *cells, do
 }
 
 int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells) {
+    DeviceGuard dev_guard(h);
     if (!h || !pos || !cells) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
@@ -732,6 +767,7 @@ int cfneb_set_path(cfneb_t *h, const double *pos, const double *cells) {
 }
 
 int cfneb_get_state(cfneb_t *h, double *X, double *v) {
+    DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
@@ -743,7 +779,77 @@ int cfneb_get_state(cfneb_t *h, double *X, double *v) {
     return sync_status(h);
 }
 
+int cfneb_get_checkpoint(cfneb_t *h, double *X, double *v, double *X_list, double *list_aux, cfneb_fire_state *fire) {
+    DeviceGuard dev_guard(h);
+    if (!h) return CFNEB_EINVAL;
+    int rc = (X || v) ? cfneb_get_state(h, X, v) : sync_mirror(h);
+    if (rc) return rc;
+    const Dev &d = h->d;
+    const size_t n = (size_t)h->P * (d.N + 3) * 3;
+    if (X_list || list_aux) {
+        double *dX = static_cast<double *>(d.scratch), *daux = dX + n;
+        launch_export_list_state(d, dX, daux, h->st);
+        if (X_list) CK(cudaMemcpyAsync(X_list, dX, n * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+        if (list_aux) CK(cudaMemcpyAsync(list_aux, daux, (size_t)h->P * 4 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    }
+    if (fire) {
+        Ctl c;
+        CK(cudaMemcpyAsync(&c, d.ctl, sizeof c, cudaMemcpyDeviceToHost, h->st));
+        CK(cudaStreamSynchronize(h->st));
+        fire->dt = c.dt;
+        fire->alpha = c.alpha;
+        fire->steps = (int64_t)c.steps;
+        fire->n_pos = c.n_pos;
+        fire->first = c.first;
+    }
+    return sync_status(h);
+}
+
+int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *X_list, const double *list_aux,
+                    const cfneb_fire_state *fire) {
+    DeviceGuard dev_guard(h);
+    if (!h || !X || (X_list && !list_aux)) return CFNEB_EINVAL;
+    if (fire && (!(fire->dt > 0.0) || !(fire->alpha >= 0.0) || fire->n_pos < 0 || fire->steps < 0)) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
+    const Dev &d = h->d;
+    cudaStream_t st = h->st;
+    const size_t n = (size_t)h->P * (d.N + 3) * 3;
+    double *dX = static_cast<double *>(d.scratch), *dv = dX + n;
+    int rc;
+    if (X_list) {  // replay the list builds: lists at X_list, then the coordinates proper
+        CK(cudaMemcpyAsync(dX, X_list, n * sizeof(double), cudaMemcpyHostToDevice, st));
+        launch_import_state(d, dX, nullptr, st);
+        CK(cudaStreamSynchronize(st));
+        rc = force_rebuild_all(h);
+        if (rc) return rc;
+        launch_cell_prep(d, 0, MODE_STEP, st);
+        launch_neighbor_build(d, 0, st);
+    }
+    CK(cudaMemcpyAsync(dX, X, n * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (v && fire) CK(cudaMemcpyAsync(dv, v, n * sizeof(double), cudaMemcpyHostToDevice, st));
+    launch_import_state(d, dX, (v && fire) ? dv : nullptr, st);
+    if (!(v && fire)) launch_reset_fire(d, st);  // no velocities, or no FIRE state to go with them: a restart
+    CK(cudaStreamSynchronize(st));  // dX / dv are reused below
+    if (!X_list) {
+        rc = force_rebuild_all(h);
+        if (rc) return rc;
+    }
+    double *daux = dX;
+    if (X_list) CK(cudaMemcpyAsync(daux, list_aux, (size_t)h->P * 4 * sizeof(double), cudaMemcpyHostToDevice, st));
+    launch_import_aux(d, daux, X_list ? 1 : 0, fire ? 1 : 0, fire ? fire->dt : 0.0, fire ? fire->alpha : 0.0,
+                      fire ? fire->n_pos : 0, fire ? (fire->first ? 1 : 0) : 1,
+                      fire ? (unsigned long long)fire->steps : 0ull, st);
+    // endpoint energies at the restored coordinates (their lists: replayed above, or fresh)
+    launch_cell_prep(d, X_list ? kEndpointsOnly : 0, MODE_STEP, st);
+    launch_neighbor_build(d, X_list ? kEndpointsOnly : 0, st);
+    launch_force(d, kEndpointsOnly, st);
+    launch_finalize(d, kEndpointsOnly, st);
+    h->interior_stale = true;
+    return sync_status(h);
+}
+
 int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, double *energies) {
+    DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
@@ -767,6 +873,7 @@ int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, doubl
 }
 
 int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int32_t *list, int32_t *shift) {
+    DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     if (image < 0 || image >= h->P) return CFNEB_ERANGE;
@@ -786,6 +893,7 @@ int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int32_t *list
 }
 
 int cfneb_get_status(cfneb_t *h, cfneb_status *out) {
+    DeviceGuard dev_guard(h);
     if (!h || !out) return CFNEB_EINVAL;
     Ctl c;
     CK(cudaMemcpyAsync(&c, h->d.ctl, sizeof c, cudaMemcpyDeviceToHost, h->st));
@@ -814,6 +922,7 @@ int cfneb_get_status(cfneb_t *h, cfneb_status *out) {
 
 void cfneb_destroy(cfneb_t *h) {
     if (!h) return;
+    DeviceGuard dev_guard(h);
     if (h->st) cudaStreamSynchronize(h->st);
     if (h->exec) cudaGraphExecDestroy(h->exec);
     if (h->graph) cudaGraphDestroy(h->graph);

@@ -23,7 +23,7 @@ constexpr int kThreadsAtom = 128;      // force / neighbour / position kernels: 
 constexpr int kThreadsStream = 256;    // K4 / K6: 2 atoms per thread (double2)
 constexpr int kAtomsPerStreamBlock = kThreadsStream * 2;
 constexpr int kNDots = 10;             // pp, mm, pm, Gp, Gm, GG, Gv, pv, mv, vv
-constexpr int kNForcePart = 8;         // E, Vxx, Vyy, Vzz, Vxy, Vxz, Vyz, (embedding energy)
+constexpr int kNForcePart = 10;        // E pair, Vxx, Vyy, Vzz, Vxy, Vxz, Vyz, E site (embedding / many-body), low words of [0], [7]
 constexpr uint32_t kIdxMask = 0x7FFFFFu;
 constexpr int kShiftBits = 23;
 constexpr uint32_t kCodeCenter = 4u | (4u << 3) | (4u << 6);
@@ -108,13 +108,14 @@ struct Dev {
     double *Xc, *vc;
     double *E, *V, *Gc;       // [S], [S][9], [S][9]
     double *dots, *coef;      // [S][10], [S][4]
-    double *part_force;       // [S][nblk_atom][8]
+    double *part_force;       // [S][nblk_atom][kNForcePart]
     RelaxState *relax;        // [2]
     double *part_relax;       // [2][nblk_stream][4]
     double *part_dots;        // [S][nblk_stream][10]  (the first nblk_red rows of an image are used)
     unsigned long long *dispmax;  // [S] max |dR~_i|^2 of the last update, as ordered bits
     unsigned long long *disptot;  // [S] max |R~_i - R~_i(build)|^2 at the last K0, as ordered bits
     double *Xb;                   // [S][3][Npad] R~ at the last list build of each slot
+    double *Xcb;                  // [S][9] cell rows lam B (lam D) at the last list build (checkpoint: the build is replayed)
     unsigned long long *dispmax_in;  // [S] max |dR~_i|^2 of a path replacement (cfneb_set_path) since the last K0
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
@@ -195,6 +196,10 @@ void launch_segment_lengths(const Dev &d, double *out_dev, cudaStream_t st);
 void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_out, int *shift_out, cudaStream_t st);
 void launch_export_path(const Dev &d, double *pos_out, double *cells_out, double *E_out, cudaStream_t st);
 void launch_export_state(const Dev &d, double *X_out, double *v_out, cudaStream_t st);
+void launch_export_list_state(const Dev &d, double *Xl_out, double *aux_out, cudaStream_t st);  // checkpoint
+void launch_import_state(const Dev &d, const double *X_in, const double *v_in, cudaStream_t st);
+void launch_import_aux(const Dev &d, const double *aux_in, int have_aux, int have_fire, double dt, double alpha, int n_pos,
+                       int first, unsigned long long steps, cudaStream_t st);
 void launch_export_forces(const Dev &d, double *F_out, double *V_out, double *E_out, cudaStream_t st);
 double run_fp64_peak(cudaStream_t st);
 
@@ -245,6 +250,48 @@ __device__ inline void block_sum(double (&val)[NV], double *smem /* [32*NV] */) 
             for (int o = 16; o > 0; o >>= 1) x += __shfl_down_sync(0xffffffffu, x, o);
             val[q] = x;
         }
+    }
+    __syncthreads();
+}
+
+// Error-free addition (Knuth): s + e = a + b exactly.  Adds only: FMA contraction cannot touch it.
+__device__ inline void two_sum(double a, double b, double &s, double &e) {
+    s = a + b;
+    const double bb = s - a;
+    e = (a - (s - bb)) + (b - bb);
+}
+// (hi, lo) += (h2, l2) in two-double arithmetic (lo stays a small correction; not renormalised)
+__device__ inline void dd_add(double &hi, double &lo, double h2, double l2) {
+    double s, e;
+    two_sum(hi, h2, s, e);
+    hi = s;
+    lo += l2 + e;
+}
+// Block-wide sum of one two-double value per thread, same fixed tree as block_sum; result (normalised) in thread 0.
+// The image energy is a sum of ~1e5 site energies of the same sign (|E| ~ 9e5 eV at configs[4]) whose DIFFERENCES
+// between neighbouring images (~0.3 eV) weight the improved tangent at an extremum (O5): a plain tree loses a few
+// ulp(E) ~ 1e-10 in its last levels, which is 1e-9 of those weights.  Carried in two doubles the total is the
+// correctly rounded sum of the per-thread values.
+__device__ inline void block_sum_dd(double &hi, double &lo, double *smem /* [64] */) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+        dd_add(hi, lo, h2, l2);
+    }
+    if (lane == 0) { smem[2 * warp] = hi; smem[2 * warp + 1] = lo; }
+    __syncthreads();
+    if (warp == 0) {
+        hi = (lane < nwarp) ? smem[2 * lane] : 0.0;
+        lo = (lane < nwarp) ? smem[2 * lane + 1] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            const double h2 = __shfl_down_sync(0xffffffffu, hi, o), l2 = __shfl_down_sync(0xffffffffu, lo, o);
+            dd_add(hi, lo, h2, l2);
+        }
+        const double s = hi + lo;  // fast two-sum: |lo| << |hi|
+        lo -= s - hi;
+        hi = s;
     }
     __syncthreads();
 }

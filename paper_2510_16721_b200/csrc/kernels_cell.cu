@@ -208,7 +208,7 @@ __global__ void cell_prep_kernel(Dev d, int p_lo, int mode) {
                         acc = 0.0;
                         g->since = 0;
                         g->force_rebuild = 0;
-                        for (int k = 0; k < 9; ++k) g->Dbinv[k] = Dinv[k];
+                        for (int k = 0; k < 9; ++k) { g->Dbinv[k] = Dinv[k]; d.Xcb[slot * 9 + k] = xc[k]; }
                     } else {
                         g->since += 1;
                     }

@@ -57,7 +57,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int 
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     __shared__ double sh[9];
-    __shared__ double red[32];
+    __shared__ double red[64];
     __shared__ double sW[kDnWeights];
     const int K = (int)d.pot[1], M = MT, L = (int)d.pot[3], H = (int)d.pot[4], D = K + M * L;
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
@@ -220,8 +220,13 @@ __global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int 
             part[(size_t)(k * 3 + 2) * d.Npad] = pz;
         }
     }
-    block_sum<1>(ui, red);
-    if (threadIdx.x == 0) d.part_force[((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart + 7] = ui[0];
+    double ui_lo = 0.0;
+    block_sum_dd(ui[0], ui_lo, red);
+    if (threadIdx.x == 0) {
+        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        out[7] = ui[0];
+        out[9] = ui_lo;
+    }
 }
 
 void launch_force_dn(const Dev &d, int p_lo, cudaStream_t st) {

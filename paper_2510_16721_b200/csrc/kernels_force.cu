@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 7) density_kernel(Dev d, int p_l
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     __shared__ double sh[9];
-    __shared__ double red[32];
+    __shared__ double red2[64];
     __shared__ double sT_tab[32];
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
     if (threadIdx.x < 32) sT_tab[threadIdx.x] = kExp2Table[threadIdx.x];
@@ -271,8 +271,13 @@ __global__ void __launch_bounds__(kThreadsAtom, 7) density_kernel(Dev d, int p_l
         }
         Rc[i].w = dF;
     }
-    block_sum<1>(emb, red);
-    if (threadIdx.x == 0) d.part_force[((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart + 7] = emb[0];
+    double emb_lo = 0.0;
+    block_sum_dd(emb[0], emb_lo, red2);
+    if (threadIdx.x == 0) {
+        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        out[7] = emb[0];
+        out[9] = emb_lo;
+    }
 }
 
 // K2b: forces, energies and the virial over the Verlet list.
@@ -336,13 +341,17 @@ __global__ void __launch_bounds__(kThreadsAtom, 5) force_kernel(Dev d, int p_lo)
         F[d.Npad + i] = acc.fy;
         F[2 * (size_t)d.Npad + i] = acc.fz;
     }
-    double out7[7] = {acc.ui, -0.5 * acc.sxx, -0.5 * acc.syy, -0.5 * acc.szz, -0.5 * acc.sxy, -0.5 * acc.sxz, -0.5 * acc.syz};
-    block_sum<7>(out7, red);
+    double out6[6] = {-0.5 * acc.sxx, -0.5 * acc.syy, -0.5 * acc.szz, -0.5 * acc.sxy, -0.5 * acc.sxz, -0.5 * acc.syz};
+    block_sum<6>(out6, red);
+    double e_hi = acc.ui, e_lo = 0.0;  // the energy channel in two doubles (block_sum_dd)
+    block_sum_dd(e_hi, e_lo, red);
     if (threadIdx.x == 0) {
         double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        out[0] = e_hi;
+        out[8] = e_lo;
 #pragma unroll
-        for (int n = 0; n < 7; ++n) out[n] = out7[n];
-        if (POT == CFNEB_POT_LJ_SF) out[7] = 0.0;
+        for (int n = 0; n < 6; ++n) out[1 + n] = out6[n];
+        if (POT == CFNEB_POT_LJ_SF) { out[7] = 0.0; out[9] = 0.0; }
     }
 }
 

@@ -97,20 +97,27 @@ __global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.x, p_lo, P, p)) return;
     const int slot = d.order[p];
-    __shared__ double red[32 * kNForcePart];
-    double a8[kNForcePart];
+    __shared__ double red[32 * 8];
+    double a8[8];  // [1..6] the virial; [0], [7] unused here (the energy channels go through two doubles)
 #pragma unroll
-    for (int q = 0; q < kNForcePart; ++q) a8[q] = 0.0;
+    for (int q = 0; q < 8; ++q) a8[q] = 0.0;
+    double e_hi = 0.0, e_lo = 0.0;
     const double *pf = d.part_force + (size_t)slot * d.nblk_atom * kNForcePart;
-    for (int b = threadIdx.x; b < d.nblk_atom; b += blockDim.x)
+    for (int b = threadIdx.x; b < d.nblk_atom; b += blockDim.x) {
+        const double *q8 = pf + (size_t)b * kNForcePart;
 #pragma unroll
-        for (int q = 0; q < kNForcePart; ++q) a8[q] += pf[(size_t)b * kNForcePart + q];
-    block_sum<kNForcePart>(a8, red);
+        for (int q = 1; q < 7; ++q) a8[q] += q8[q];
+        dd_add(e_hi, e_lo, q8[0], q8[8]);  // pair energy, then site (embedding / many-body) energy of the block
+        dd_add(e_hi, e_lo, q8[7], q8[9]);
+    }
+    block_sum<8>(a8, red);
+    block_sum_dd(e_hi, e_lo, red);
     if (threadIdx.x == 0) {
         const Geom *g = d.geom + slot;
         // external pressure (A25): enthalpy H = U + p Omega and its virial V - p Omega I (Eq. 2-3)
         const double pv = d.pressure * fabs(g->vol);
-        const double E = a8[0] + a8[7] + pv;
+        dd_add(e_hi, e_lo, pv, 0.0);
+        const double E = e_hi + e_lo;
         const double V[9] = {a8[1] - pv, a8[4], a8[5], a8[4], a8[2] - pv, a8[6], a8[5], a8[6], a8[3] - pv};
         d.E[slot] = E;
         double Gc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};

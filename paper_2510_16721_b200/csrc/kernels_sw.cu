@@ -38,7 +38,7 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_partial_kernel(Dev d, int p_l
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     __shared__ double sh[9];
-    __shared__ double red[32];
+    __shared__ double red[64];
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -113,8 +113,13 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_partial_kernel(Dev d, int p_l
             if (hit) ++a;
         }
     }
-    block_sum<1>(ui, red);
-    if (threadIdx.x == 0) d.part_force[((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart + 7] = ui[0];
+    double ui_lo = 0.0;
+    block_sum_dd(ui[0], ui_lo, red);
+    if (threadIdx.x == 0) {
+        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        out[7] = ui[0];
+        out[9] = ui_lo;
+    }
 }
 
 __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo) {
@@ -162,6 +167,7 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
         double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
 #pragma unroll
         for (int n = 0; n < 7; ++n) out[n] = out7[n];
+        out[8] = 0.0;
     }
 }
 
@@ -237,6 +243,7 @@ __global__ void __launch_bounds__(kThreadsAtom) pair_force_batched_kernel(Dev d,
         double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
 #pragma unroll
         for (int n = 0; n < 7; ++n) out[n] = out7[n];
+        out[8] = 0.0;
     }
 }
 

@@ -250,6 +250,77 @@ __global__ void export_state_kernel(Dev d, double *Xo, double *vo) {
     }
 }
 
+// Checkpoint, second half: the generalized coordinates each image's neighbour list was built at (Xb, Xcb) and the
+// staleness accounting {max |R~_i - R~_i(build)|^2 at the last K0, max |dR~_i|^2 of the last update, steps since
+// the build, 0} -- what cfneb_set_state needs to replay the list builds and continue bit for bit.
+__global__ void export_list_state_kernel(Dev d, double *Xo, double *aux) {
+    const int p = blockIdx.y;
+    const int P = d.ctl->P;
+    if (p >= P) return;
+    const int slot = d.order[p];
+    const int rows = d.N + 3;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a == 0 && aux) {
+        aux[4 * p + 0] = bits_nonneg(d.disptot[slot]);
+        aux[4 * p + 1] = bits_nonneg(d.dispmax[slot]);
+        aux[4 * p + 2] = (double)d.geom[slot].since;
+        aux[4 * p + 3] = 0.0;
+    }
+    if (a >= rows || !Xo) return;
+    const double *Xb = d.Xb + (size_t)slot * 3 * d.Npad;
+    const int ao = a < d.N ? d.perm[a] : a;
+    for (int c = 0; c < 3; ++c)
+        Xo[((size_t)p * rows + ao) * 3 + c] = a < d.N ? Xb[(size_t)c * d.Npad + a] : d.Xcb[slot * 9 + 3 * (a - d.N) + c];
+}
+
+// Inverse of export_state_kernel: X (and v, if given) from the caller's layout into both coordinate buffers.
+__global__ void import_state_kernel(Dev d, const double *__restrict__ Xi, const double *__restrict__ vi) {
+    const int p = blockIdx.y;
+    const int P = d.ctl->P;
+    if (p >= P) return;
+    const int slot = d.order[p];
+    const int rows = d.N + 3;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= rows) return;
+    const size_t img = (size_t)3 * d.Npad, buf = (size_t)d.S * img;
+    const bool movable = p > 0 && p < P - 1;
+    const int ai = a < d.N ? d.perm[a] : a;
+    for (int c = 0; c < 3; ++c) {
+        const double x = Xi[((size_t)p * rows + ai) * 3 + c];
+        const double v = (vi && movable) ? vi[((size_t)p * rows + ai) * 3 + c] : 0.0;
+        if (a < d.N) {
+            d.X[slot * img + (size_t)c * d.Npad + a] = x;
+            d.X[buf + slot * img + (size_t)c * d.Npad + a] = x;
+            if (vi) d.v[slot * img + (size_t)c * d.Npad + a] = v;
+        } else {
+            const int k = 3 * (a - d.N) + c;
+            d.Xc[slot * 9 + k] = x;
+            d.Xc[(size_t)d.S * 9 + slot * 9 + k] = x;
+            if (vi) d.vc[slot * 9 + k] = v;
+        }
+    }
+}
+
+__global__ void import_aux_kernel(Dev d, const double *aux, int have_aux, int have_fire, double dt, double alpha, int n_pos,
+                                  int first, unsigned long long steps) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (have_aux && p < d.ctl->P) {
+        const int slot = d.order[p];
+        d.disptot[slot] = nonneg_bits(aux[4 * p + 0]);
+        d.dispmax[slot] = nonneg_bits(aux[4 * p + 1]);
+        d.dispmax_in[slot] = 0ull;
+        d.geom[slot].since = (int)aux[4 * p + 2];
+    }
+    if (p == 0 && have_fire) {
+        Ctl *c = d.ctl;
+        c->dt = dt;
+        c->alpha = alpha;
+        c->n_pos = n_pos;
+        c->first = first;
+        c->steps = steps;
+    }
+}
+
 __global__ void export_forces_kernel(Dev d, double *Fo, double *Vo, double *Eo) {
     const int p = blockIdx.y;
     if (p >= d.ctl->P) return;
@@ -296,6 +367,21 @@ void launch_export_path(const Dev &d, double *pos_out, double *cells_out, double
 void launch_export_state(const Dev &d, double *X_out, double *v_out, cudaStream_t st) {
     dim3 grid((d.N + 3 + 127) / 128, d.S);
     export_state_kernel<<<grid, 128, 0, st>>>(d, X_out, v_out);
+}
+
+void launch_export_list_state(const Dev &d, double *Xl_out, double *aux_out, cudaStream_t st) {
+    dim3 grid((d.N + 3 + 127) / 128, d.S);
+    export_list_state_kernel<<<grid, 128, 0, st>>>(d, Xl_out, aux_out);
+}
+
+void launch_import_state(const Dev &d, const double *X_in, const double *v_in, cudaStream_t st) {
+    dim3 grid((d.N + 3 + 127) / 128, d.S);
+    import_state_kernel<<<grid, 128, 0, st>>>(d, X_in, v_in);
+}
+
+void launch_import_aux(const Dev &d, const double *aux_in, int have_aux, int have_fire, double dt, double alpha, int n_pos,
+                       int first, unsigned long long steps, cudaStream_t st) {
+    import_aux_kernel<<<(d.S + 127) / 128, 128, 0, st>>>(d, aux_in, have_aux, have_fire, dt, alpha, n_pos, first, steps);
 }
 
 void launch_export_forces(const Dev &d, double *F_out, double *V_out, double *E_out, cudaStream_t st) {

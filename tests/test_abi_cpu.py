@@ -63,6 +63,9 @@ def test_workspace_bytes_and_argument_errors_need_no_device(cf):
     assert L.cfneb_step(None, 1) == -1 and L.cfneb_get_status(None, None) == -1
     assert L.cfneb_relax_endpoints(None, 1e-3, 10, 1, None, None, None) == -1
     assert L.cfneb_step_adaptive(None, 1, 1, 1.0, 0.1) == -1
+    assert L.cfneb_get_checkpoint(None, None, None, None, None, None) == -1
+    assert L.cfneb_set_state(None, None, None, None, None, None) == -1
+    assert ctypes.sizeof(cf.FireState) == 32
     for code in range(0, -8, -1):
         assert len(L.cfneb_strerror(code)) > 1
     L.cfneb_destroy(None)  # documented no-op

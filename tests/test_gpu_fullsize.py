@@ -54,28 +54,20 @@ def test_c4_full_size_forces_and_one_step():
     assert rel(V[1:-1], last["V"]) < TOL_FORCE
     worst_f = max(rel(F[p], last["F"][p - 1]) for p in range(1, P - 1))
     assert worst_f < TOL_FORCE, worst_f
-    # f^NEB.  At an energy extremum the improved tangent (O5) mixes tau+ and tau- with the weights
-    # |E_{p+-1} - E_p|: differences of ~0.3 eV between totals of ~9e5 eV, so the 1e-14 relative round-off of the
-    # energy sums (3e-8 eV) reaches the weights at 1e-7 and f^NEB of that image at ~1e-9.  For
-    # those images both sides therefore take the tangent decision from ONE set of energies (the GPU's, already
-    # checked against the oracle's above): the oracle's own O5 / O6 functions are evaluated at the oracle's X
-    # and G with those energies.  All other images (upwind branches: no energy enters the weights) and, loosely,
-    # the extremum images too are compared against the untouched oracle band.
-    from oracle import neb as on
+    # f^NEB of EVERY image against the untouched oracle band at 1e-9.  At an energy extremum the improved tangent (O5)
+    # mixes tau+ and tau- with the weights |E_{p+-1} - E_p|: differences of ~0.3 eV between totals of ~9e5 eV, so the
+    # energies must agree to about one ulp (1.2e-10 eV) for the weights to agree to 1e-9.  Both sides carry the
+    # total in extended precision (the oracle in long double, the kernels in two doubles: block_sum_dd), so each
+    # is the correctly rounded sum of its own site energies; measured: <= 1 ulp on the interior images, 3 ulp on the
+    # perfect-lattice endpoint (identical site energies, identical per-atom rounding), f^NEB 5e-11 at the extremum.
     Eo = orc.band.E
-    assert np.max(np.abs(E - Eo)) < 1e-12 * np.max(np.abs(Eo))
+    assert np.max(np.abs(E - Eo)) < 8 * np.spacing(np.max(np.abs(Eo)))
     n_mixed = 0
     for p in range(1, P - 1):
         upwind = (Eo[p + 1] > Eo[p] > Eo[p - 1]) or (Eo[p + 1] < Eo[p] < Eo[p - 1])
-        if upwind:
-            assert rel(fneb[p], f_or[p]) < TOL_STEP, p
-            continue
-        n_mixed += 1
-        assert rel(fneb[p], f_or[p]) < 1e-7, p
-        tau, tp, tm = on.improved_tangent(orc.band.X[p - 1], orc.band.X[p], orc.band.X[p + 1], E[p - 1], E[p], E[p + 1])
-        f_same_E = on.neb_force(orc.band.G[p], tau, tp, tm, spec.k_spring, climbing=(p == orc.band.pstar))
-        assert rel(fneb[p], f_same_E) < TOL_STEP, p
-    assert 1 <= n_mixed <= 3  # the Bain band has one maximum (the climbing image)
+        n_mixed += 0 if upwind else 1
+        assert rel(fneb[p], f_or[p]) < TOL_STEP, (p, upwind)
+    assert 1 <= n_mixed <= 3  # the Bain band has one maximum (the climbing image): the energy-weighted branch is exercised
     st = gpu.get_status()
     assert st.climb_index == orc.band.pstar
     # the energies that decide tangent branches and the climbing image are not within round-off of a tie (A24)

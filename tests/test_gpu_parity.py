@@ -38,6 +38,19 @@ def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_im
     return spec, orc, gpu
 
 
+def first_step_exact(orc, gpu):
+    """ONE full iteration on both sides from the current (identical) state: displacement and velocity to 1e-9
+    (BASELINE.json north_star), before round-off is amplified by the dynamics.  Returns X before the step."""
+    X0, _ = orc.get_state()
+    orc.step(1)
+    gpu.step(1)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < TOL_STEP, rel(Xg - X0, Xo - X0)
+    assert rel(vg, vo) < TOL_STEP, rel(vg, vo)
+    return X0
+
+
 def sorted_triples(count, lst, shift):
     out = []
     for i in range(len(count)):
@@ -59,7 +72,11 @@ def test_neighbor_lists_bit_exact_after_sorting(k):
         Rt, D = ev.deformation(orc.band.X[image])
         h = orc.h0 @ D
         cnt, lst, sh = ff.neighbors(Rt, orc.h0, h, r_list, spec.max_neighbors, brute=(k == 0))
-        # guard: no pair within 1e-9 of the list radius (membership would be rounding-dependent, A20/A24)
+        # guard: no pair within 1e-9 of the list radius (membership would be rounding-dependent, A20/A24):
+        # the oracle's own search at r_list (1 -+ 1e-9) finds the same neighbours
+        c_lo = ff.neighbors(Rt, orc.h0, h, r_list * (1.0 - 1e-9), spec.max_neighbors, brute=(k == 0))[0]
+        c_hi = ff.neighbors(Rt, orc.h0, h, r_list * (1.0 + 1e-9), spec.max_neighbors, brute=(k == 0))[0]
+        assert np.array_equal(c_lo, cnt) and np.array_equal(c_hi, cnt), "a pair sits within 1e-9 of the list radius"
         gc, gl, gs = gpu.get_neighbors(image)
         assert np.array_equal(np.sort(gc), np.sort(cnt)) and np.array_equal(gc, cnt)
         a, b = sorted_triples(gc, gl, gs), sorted_triples(cnt, lst, sh)
@@ -171,10 +188,10 @@ def test_c1_barrier_after_fixed_budget():
 def test_cell_modes_fixed_and_D(mode):
     """CELL_FIXED (no cell force) and the Eq. 14 D-variant follow the oracle too."""
     spec, orc, gpu = make_pair(0, cell_factor=1.0, cell_mode=mode)
-    X0, _ = orc.get_state()
     Xg0, _ = gpu.get_state()
-    orc.step(5)
-    gpu.step(5)
+    X0 = first_step_exact(orc, gpu)
+    orc.step(4)
+    gpu.step(4)
     Xo, vo = orc.get_state()
     Xg, vg = gpu.get_state()
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
@@ -196,9 +213,9 @@ def test_external_pressure_enthalpy_band(k, mode, p_ext):
     # the pressure term is a large part of what is being compared
     _, cells, _ = orc.get_path()
     assert p_ext * abs(np.linalg.det(cells[1])) > 0.05 * abs(orc.band.E[1] - p_ext * abs(np.linalg.det(cells[1])))
-    X0, _ = orc.get_state()
-    orc.step(4)
-    gpu.step(4)
+    X0 = first_step_exact(orc, gpu)
+    orc.step(3)
+    gpu.step(3)
     Xo, vo = orc.get_state()
     Xg, vg = gpu.get_state()
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
@@ -370,6 +387,55 @@ def test_bitwise_repeatable():
     assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1])
 
 
+@pytest.mark.parametrize("k,n_before,n_after,over", [(2, 25, 30, dict()), (1, 7, 12, dict(cell_mode=2)), (2, 13, 20, dict(rebuild_every=9))])
+def test_checkpoint_resume_is_bit_exact(k, n_before, n_after, over):
+    """cfneb_get_checkpoint -> cfneb_destroy -> cfneb_create -> cfneb_set_state continues the band bit for bit
+    (SURVEY.md section 5 checkpoint row; "structural information is always kept and updated on GPU"): X, v, the
+    FIRE scalars, and -- because the order of a list's entries fixes the summation order -- the coordinates each
+    neighbour list was built at with its staleness accounting.  The windows straddle list rebuilds on both sides."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(k)
+    prm = cf.params_for(spec, cell_factor=0.0, **over)
+    a = cf.CFNEB(pos, cells, prm)
+    a.step(n_before)
+    ck = a.get_checkpoint()
+    st_ck = a.get_status()
+    a.step(n_after)
+    Xa, va = a.get_state()
+    sa = a.get_status()
+    a.close()
+    assert ck["fire"].steps == n_before and ck["fire"].first == 0
+    assert np.any(ck["X_list"] != ck["X"])                    # some list is older than the checkpoint
+    b = cf.CFNEB(pos, cells, prm)                             # a new handle from the same inputs
+    b.step(3)                                                 # ... in some other state
+    b.set_state(ck["X"], ck["v"], ck["X_list"], ck["list_aux"], ck["fire"])
+    Xb0, vb0 = b.get_state()
+    assert np.array_equal(Xb0, ck["X"]) and np.array_equal(vb0, ck["v"])
+    sb0 = b.get_status()
+    assert (sb0.dt, sb0.alpha, sb0.n_pos, sb0.steps) == (st_ck.dt, st_ck.alpha, st_ck.n_pos, n_before)
+    r0 = sb0.rebuilds
+    b.step(n_after)
+    Xb, vb = b.get_state()
+    sb = b.get_status()
+    assert np.array_equal(Xb, Xa) and np.array_equal(vb, va)
+    assert (sb.dt, sb.alpha, sb.n_pos, sb.fmax, sb.barrier, sb.steps) == (sa.dt, sa.alpha, sa.n_pos, sa.fmax, sa.barrier, sa.steps)
+    if k == 2:
+        assert sb.rebuilds > r0                               # the resumed window rebuilt lists on its own as well
+    # without X_list the lists are fresh: same band to round-off, FIRE state still restored
+    c = cf.CFNEB(pos, cells, prm)
+    c.set_state(ck["X"], ck["v"], None, None, ck["fire"])
+    c.step(n_after)
+    Xc, vc = c.get_state()
+    assert rel(Xc - ck["X"], Xa - ck["X"]) < 1e-9 and c.get_status().n_pos == sa.n_pos
+    # no FIRE state: a restart from the stored coordinates (v = 0, dt = dt0, first step)
+    c.set_state(ck["X"])
+    assert np.all(c.get_state()[1] == 0) and c.get_status().dt == spec.fire["dt0"]
+    with pytest.raises(cf.CfnebError):
+        c.set_state(ck["X"], ck["v"], ck["X_list"], None, ck["fire"])   # X_list without its accounting
+    b.close()
+    c.close()
+
+
 def test_neighbor_list_reuse_equals_fresh_lists():
     """Verlet-list reuse (skin) must not change the result: rebuild_every = 1 forces fresh lists each step."""
     import paper_2510_16721_b200 as cf
@@ -464,24 +530,28 @@ def _unrelaxed_endpoints(kind):
     return spec, f0 @ c0 + kick, c0, f1 @ c1 + kick, c1
 
 
-@pytest.mark.parametrize("kind", ["lj", "fs"])
-def test_relax_endpoints_follows_oracle_trajectory(kind):
+@pytest.mark.parametrize("kind,mode", [("lj", 1), ("fs", 1), ("lj", 2), ("fs", 2), ("lj", 0)])
+def test_relax_endpoints_follows_oracle_trajectory(kind, mode):
     """cfneb_relax_endpoints, 25 updates with no convergence stop: both endpoints follow the oracle's single-structure
-    cell-filter FIRE (final endpoint in the frame of the initial cell) step for step."""
+    cell-filter FIRE (final endpoint in the frame of the initial cell) step for step, in the Eq. 17 coordinates
+    (CELL_B), the Eq. 14 coordinates (CELL_D) and with the cell fixed."""
     import paper_2510_16721_b200 as cf
     from oracle import cfneb as oc
     spec, R0, h0, R1, h1 = _unrelaxed_endpoints(kind)
     n = 25
-    kw = dict(fmax_tol=0.0, max_steps=n, cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=256)
+    kw = dict(fmax_tol=0.0, max_steps=n, cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=256, cell_mode=mode)
     Ra, ha, _, _, ita = oc.relax_endpoint(R0, h0, spec.potential, spec.pot, spec.r_cut, **kw)
     Rb, hb, _, _, itb = oc.relax_endpoint(R1, h1, spec.potential, spec.pot, spec.r_cut, h_ref=h0, **kw)
-    gpu = cf.CFNEB(np.stack([R0, R1]), np.stack([h0, h1]), cf.params_for(spec, cell_factor=0.0, max_neighbors=256, max_images=5),
-                   n_images=5)
+    gpu = cf.CFNEB(np.stack([R0, R1]), np.stack([h0, h1]),
+                   cf.params_for(spec, cell_factor=0.0, max_neighbors=256, max_images=5, cell_mode=mode), n_images=5)
     steps, fmax, en = gpu.relax_endpoints(0.0, n, rebuild_band=False)
     assert steps == [n, n]
     pos, cells, E = gpu.get_path()
-    assert rel(pos[0] - R0, Ra - R0) < 1e-8 and rel(cells[0] - h0, ha - h0) < 1e-8
-    assert rel(pos[-1] - R1, Rb - R1) < 1e-8 and rel(cells[-1] - h1, hb - h1) < 1e-8
+    assert rel(pos[0] - R0, Ra - R0) < 1e-8 and rel(pos[-1] - R1, Rb - R1) < 1e-8
+    if mode == 0:   # cell fixed: nothing but the atoms moves
+        assert np.array_equal(ha, h0) and rel(cells[0], h0) < 1e-15 and rel(cells[-1], hb) < 1e-14
+    else:
+        assert rel(cells[0] - h0, ha - h0) < 1e-8 and rel(cells[-1] - h1, hb - h1) < 1e-8
     assert np.max(np.abs(Ra - R0)) > 1e-3  # something moved
     assert gpu.get_status().error == 0
     gpu.close()
@@ -774,9 +844,9 @@ def test_stillinger_weber_many_body_forces_and_steps(dims, n_images):
     assert rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
     assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
     assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
-    X0, _ = orc.get_state()
-    orc.step(6)
-    gpu.step(6)
+    X0 = first_step_exact(orc, gpu)
+    orc.step(5)
+    gpu.step(5)
     Xo, vo = orc.get_state()
     Xg, vg = gpu.get_state()
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
@@ -868,9 +938,9 @@ def test_descriptor_network_many_body_forces_and_steps(dims, n_images, net):
     assert rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
     assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
     assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
-    X0, _ = orc.get_state()
-    orc.step(6)
-    gpu.step(6)
+    X0 = first_step_exact(orc, gpu)
+    orc.step(5)
+    gpu.step(5)
     Xo, vo = orc.get_state()
     Xg, vg = gpu.get_state()
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
@@ -909,9 +979,9 @@ def test_descriptor_network_with_the_rest_of_the_path():
     F, V, fneb, E = gpu.get_forces()
     assert rel(E, orc.band.E) < TOL_FORCE and rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
     assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
-    X0, _ = orc.get_state()
-    orc.step(5)
-    gpu.step(5)
+    X0 = first_step_exact(orc, gpu)
+    orc.step(4)
+    gpu.step(4)
     assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
     # an inserted image is evaluated with the same kernels
     seg = gpu.get_segment_lengths()

@@ -1,7 +1,8 @@
 """Pins for oracle/cfneb.py (the crystal band): the vacancy-hop barrier of BASELINE.json configs[0] against
 an independent constrained relaxation, rotation-freeness of the band, the stored lattice
-constants, structural invariants of the adaptive control (O9, "parity unpinned": the paper gives no rule),
-and the one-pass reduction algebra of SURVEY.md §8(d)."""
+constants, the adaptive control (O9: structural invariants, and a hand-worked band whose expected deletion,
+insertion and resulting order are written out from the rule of reading A16), and the one-pass reduction algebra
+of SURVEY.md §8(d)."""
 import numpy as np
 import pytest
 
@@ -167,6 +168,71 @@ def test_adaptive_control_structural_invariants(c0):
     assert neb.adapt(d_insert=1e9, d_delete=0.0) == (0, 0)
     neb.max_images = 7
     assert neb.adapt(d_insert=0.0, d_delete=0.0) == (0, 0)
+
+
+def _line_band(xs, pstar):
+    """A band of 1-row, 1-column images at the given abscissae (no crystal behind it): only what adapt() touches."""
+    from oracle.neb import Band
+    neb = object.__new__(oc.CFNEB)
+    neb.fire_params = {}
+    neb.band = Band([np.array([[x]]) for x in xs], lambda Xs: ([0.0] * len(Xs), [np.zeros((1, 1)) for _ in Xs]))
+    neb.band.pstar = pstar
+    return neb
+
+
+def _abscissae(neb):
+    return [float(x[0, 0]) for x in neb.band.X]
+
+
+def test_adaptive_control_hand_worked_band():
+    """Pin of O9 ("inserting or removing replicas based on local spacing in configuration space"; rule = reading
+    A16).  Every expected index and order below is worked out by hand from the rule's text,
+    not by oracle code.
+
+    Six images on a line at x = 0, 1, 1.2, 1.5, 3.5, 4.5: segment lengths d = 1, 0.2, 0.3, 2, 1.
+    Rule (i): delete the interior, non-climbing image q minimising d_{q-1} + d_q if that sum < d_delete:
+        q = 1: 1 + 0.2 = 1.2;  q = 2: 0.2 + 0.3 = 0.5;  q = 3: 0.3 + 2 = 2.3;  q = 4: 2 + 1 = 3.
+    Rule (ii), on the band after (i): insert the midpoint of the longest segment if it is longer than d_insert."""
+    xs = [0.0, 1.0, 1.2, 1.5, 3.5, 4.5]
+    # climbing image 4 (x = 3.5): the minimum 0.5 belongs to image 2 (x = 1.2) -> deleted.  Then d = 1, 0.5, 2, 1:
+    # segment 2 (1.5 -> 3.5) is the longest -> midpoint 2.5 inserted after image 2.  The climbing image keeps x = 3.5:
+    # index 4 -> 3 (deletion below it) -> 4 (insertion below it).
+    neb = _line_band(xs, pstar=4)
+    assert neb.adapt(d_insert=1.5, d_delete=0.6) == (1, 1)
+    assert _abscissae(neb) == [0.0, 1.0, 1.5, 2.5, 3.5, 4.5] and neb.band.pstar == 4 and neb.P == 6
+    assert neb.band.fire.first and np.all(neb.band.fire.v == 0) and neb.band.fire.v.shape[0] == 4  # FIRE restarted
+    # the sum must be BELOW d_delete (0.5 is not < 0.5), the segment ABOVE d_insert (2 is not > 2)
+    neb = _line_band(xs, pstar=4)
+    assert neb.adapt(d_insert=2.0, d_delete=0.5) == (0, 0) and _abscissae(neb) == xs
+    # deletion only: the insertion test sees the band after the deletion (longest segment still 2)
+    neb = _line_band(xs, pstar=4)
+    assert neb.adapt(d_insert=2.5, d_delete=0.6) == (0, 1) and _abscissae(neb) == [0.0, 1.0, 1.5, 3.5, 4.5]
+    assert neb.band.pstar == 3
+    # the min-sum image IS the climbing image (p* = 2): it is never a candidate.  The smallest sum among the others
+    # is q = 1 (1.2): not below d_delete = 1.0 -> nothing deleted although 0.5 < 1.0 ...
+    neb = _line_band(xs, pstar=2)
+    assert neb.adapt(d_insert=1e9, d_delete=1.0) == (0, 0) and _abscissae(neb) == xs and neb.band.pstar == 2
+    # ... and with d_delete = 1.3 image 1 (x = 1) goes, the climbing image moves from index 2 to 1, x = 1.2 kept
+    neb = _line_band(xs, pstar=2)
+    assert neb.adapt(d_insert=1e9, d_delete=1.3) == (0, 1) and _abscissae(neb) == [0.0, 1.2, 1.5, 3.5, 4.5]
+    assert neb.band.pstar == 1
+    # insertion below the climbing image shifts it up; insertion above does not.  d = 1, 0.2, 0.3, 2, 1 -> segment 3
+    neb = _line_band(xs, pstar=4)
+    assert neb.adapt(d_insert=1.9, d_delete=0.0) == (1, 0) and _abscissae(neb) == [0.0, 1.0, 1.2, 1.5, 2.5, 3.5, 4.5]
+    assert neb.band.pstar == 5
+    neb = _line_band(xs, pstar=1)
+    assert neb.adapt(d_insert=1.9, d_delete=0.0) == (1, 0) and neb.band.pstar == 1
+    # ties go to the lowest index (A16): equispaced band 0..4 with p* = 2 -> sums all 2 -> image 1 deleted; then
+    # d = 2, 1, 1 -> segment 0 inserted at x = 1 again.  max_images caps the insertion, P > 3 the deletion.
+    neb = _line_band([0.0, 1.0, 2.0, 3.0, 4.0], pstar=2)
+    assert neb.adapt(d_insert=1e9, d_delete=2.5) == (0, 1) and _abscissae(neb) == [0.0, 2.0, 3.0, 4.0]
+    neb = _line_band([0.0, 1.0, 2.0, 3.0, 4.0], pstar=3)
+    assert neb.adapt(d_insert=0.5, d_delete=0.0) == (1, 0) and _abscissae(neb) == [0.0, 0.5, 1.0, 2.0, 3.0, 4.0]
+    neb = _line_band([0.0, 1.0, 2.0, 3.0, 4.0], pstar=3)
+    neb.max_images = 5
+    assert neb.adapt(d_insert=0.5, d_delete=0.0) == (0, 0)
+    neb = _line_band([0.0, 1.0, 2.0], pstar=-1)
+    assert neb.adapt(d_insert=1e9, d_delete=1e9) == (0, 0)   # P = 3: the last interior image stays
 
 
 def test_bain_band_barrier_equals_the_saddle_of_the_closed_form_surface():
