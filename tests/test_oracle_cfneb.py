@@ -170,6 +170,24 @@ def test_adaptive_control_structural_invariants(c0):
     assert neb.adapt(d_insert=0.0, d_delete=0.0) == (0, 0)
 
 
+def test_relax_endpoint_in_every_cell_mode():
+    """relax_endpoint in the Eq. 14 coordinates (R~, D) must stop at the same crystal as in the Eq. 17 coordinates
+    (R~, B) -- the minimum does not depend on the coordinates it is searched in -- and with the cell fixed it must not
+    move the cell while still lowering the energy (the pin of the CELL_D / CELL_FIXED branches)."""
+    spec = CONFIGS[0]
+    f0, cell, _, _ = vacancy_endpoints_unrelaxed(2, 1.60)   # off the stress-free lattice constant
+    kw = dict(fmax_tol=1e-8, max_steps=6000, cell_factor=0.0, fire=spec.fire)
+    out = {m: oc.relax_endpoint(f0 @ cell, cell, 0, spec.pot, 2.5, cell_mode=m, **kw) for m in (cf.CELL_B, cf.CELL_D, cf.CELL_FIXED)}
+    (Rb, hb, Eb, fb, _), (Rd, hd, Ed, fd, _), (Rf, hf, Ef, ff_, _) = out[cf.CELL_B], out[cf.CELL_D], out[cf.CELL_FIXED]
+    assert fb < 1e-8 and fd < 1e-8 and ff_ < 1e-8
+    assert abs(Eb - Ed) < 1e-10 and abs(np.linalg.det(hb) - np.linalg.det(hd)) < 1e-6
+    assert np.abs(hd - hd.T).max() < 1e-7        # no torque on a cubic cell: D stays symmetric although Eq. 14 does not force it
+    assert np.array_equal(hf, cell) and Eb < Ef - 1.0
+    nb = ff.neighbors(f0 @ cell, cell, cell, 2.5, 128)
+    E_start = ff.energy_force_virial(f0 @ cell, cell, cell, 0, spec.pot, nb)[0]
+    assert Ef < E_start - 1e-3                   # the atoms around the vacancy relaxed
+
+
 def _line_band(xs, pstar):
     """A band of 1-row, 1-column images at the given abscissae (no crystal behind it): only what adapt() touches."""
     from oracle.neb import Band
