@@ -392,7 +392,7 @@ def test_checkpoint_resume_is_bit_exact(k, n_before, n_after, over):
     """cfneb_get_checkpoint -> cfneb_destroy -> cfneb_create -> cfneb_set_state continues the band bit for bit
     (SURVEY.md section 5 checkpoint row; "structural information is always kept and updated on GPU"): X, v, the
     FIRE scalars, and -- because the order of a list's entries fixes the summation order -- the coordinates each
-    neighbour list was built at with its staleness accounting.  The windows straddle list rebuilds on both sides."""
+    neighbour list was built at with its staleness accounting (incl. the count-down of rebuild_every)."""
     import paper_2510_16721_b200 as cf
     spec, pos, cells = build_workload(k)
     prm = cf.params_for(spec, cell_factor=0.0, **over)
@@ -419,8 +419,8 @@ def test_checkpoint_resume_is_bit_exact(k, n_before, n_after, over):
     sb = b.get_status()
     assert np.array_equal(Xb, Xa) and np.array_equal(vb, va)
     assert (sb.dt, sb.alpha, sb.n_pos, sb.fmax, sb.barrier, sb.steps) == (sa.dt, sa.alpha, sa.n_pos, sa.fmax, sa.barrier, sa.steps)
-    if k == 2:
-        assert sb.rebuilds > r0                               # the resumed window rebuilt lists on its own as well
+    if over.get("rebuild_every"):
+        assert sb.rebuilds > r0 and sa.rebuilds > st_ck.rebuilds   # both windows rebuilt lists, at the same iterations
     # without X_list the lists are fresh: same band to round-off, FIRE state still restored
     c = cf.CFNEB(pos, cells, prm)
     c.set_state(ck["X"], ck["v"], None, None, ck["fire"])
