@@ -93,6 +93,7 @@ class WorkloadSpec:
     fire: dict = field(default_factory=dict)
     skin: float = 0.3
     max_neighbors: int = 128
+    disorder_sigma: float = 0.0  # static Gaussian displacement of every atom, the same in all images (endpoints too)
 
     @property
     def r_cut(self):
@@ -128,6 +129,11 @@ CONFIGS = [
     # cut-off, 13 descriptors, 8 neurons.  The energy surface is arbitrary, so FIRE takes tiny steps: a cost workload
     WorkloadSpec("c6_dnn_diamond_32768", POT_DNN, dn_params(), "diamond_strain", (16, 16, 16), 32768, 32, 6,
                  noise_sigma=0.02, climb=False, fire=_FIRE_DNN, n_steps=100, max_images=32, skin=0.3, max_neighbors=64),
+    # not a BASELINE.json config: configs[4] with every atom displaced by a static Gaussian kick of 0.12 A (the same in
+    # all images, endpoints included) -- the paper's large bands are nucleated, locally disordered structures (P:18,
+    # P:22), where the k-th neighbours of a warp's atoms no longer share a shell.  Throughput only.
+    WorkloadSpec("c7_fs_bain_101306_disordered", POT_FS_MORSE, fs_params(), "bcc_bain", (37, 37, 37), 101306, 100, 4,
+                 fire=_FIRE_EV, n_steps=500, max_images=100, skin=0.5, max_neighbors=224, disorder_sigma=0.12),
 ]
 
 
@@ -212,4 +218,7 @@ def build_workload(k, n_images=None, dims=None):
         lc = load_lattice_constants()
         f0, c0, f1, c1 = bain_endpoints(tuple(dims) if dims else spec.dims, lc["fs_bcc_a"], lc["fs_fcc_volume_ratio"])
         pos, cells = linear_path(f0, c0, f1, c1, P, spec.seed, spec.noise_sigma)
+        if spec.disorder_sigma > 0.0:
+            kick = splitmix64_normals(spec.seed + 100, pos[0].size).reshape(pos[0].shape) * spec.disorder_sigma
+            pos = pos + kick[None]
     return spec, pos, cells

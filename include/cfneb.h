@@ -200,6 +200,18 @@ CFNEB_API int cfneb_delete_image(cfneb_t *h, int32_t index);
  * d_insert and P < max_images) with d_p = |X_{p+1} - X_p|.  Synchronises.  n_ins/n_del may be NULL. */
 CFNEB_API int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, int32_t *n_del);
 
+/*
+ * Arc-length re-parametrisation of the band (the image distribution is "automatically adjusted ... based on
+ * local spacing in configuration space"; reading A27): every interior image moves to arc length p L / (P - 1) along
+ * the band's own polyline in the generalized coordinates X, s_p = sum_{q<p} |X_{q+1} - X_q|, by linear interpolation
+ * on the segment that contains that point.  hold_climbing != 0: the climbing image of the last step stays where it is
+ * and the images on each side of it are redistributed between it and their endpoint.  Endpoints never move; P and the
+ * image order are unchanged; FIRE restarts (v = 0, dt = dt0) as after an insertion.  Runs as kernels on the handle's
+ * stream: asynchronous, no host round trip, so it can sit between cfneb_step calls of a running band.  The moved
+ * images' energies are NaN until the next step; their neighbour lists are kept while the move stays inside the skin.
+ */
+CFNEB_API int cfneb_reparametrize(cfneb_t *h, int32_t hold_climbing);
+
 /* Segment lengths d_p = |X_{p+1} - X_p|, p = 0..P-2, at the current X (HOST, P-1 doubles). Synchronises. */
 CFNEB_API int cfneb_get_segment_lengths(cfneb_t *h, double *d);
 

@@ -184,6 +184,34 @@ class CFNEB:
             b.pstar -= 1
         b.P -= 1
 
+    # -- O10: arc-length re-parametrisation ("the image distribution is automatically adjusted ... based on
+    #    local spacing in configuration space"; reading A27) -------------------------------
+    def reparametrize(self, hold_climbing=True):
+        """Redistribute the interior images at equal arc length along the band's own polyline in X.
+
+        With s_p = sum_{q<p} |X_{q+1} - X_q| and L = s_{P-1}, image p moves to the point of the polyline at arc length
+        p L / (P-1): X_q + t (X_{q+1} - X_q) on the segment q that contains it.  hold_climbing: the climbing image
+        stays where it is and each side of it is redistributed on its own with its own number of images (the
+        saddle estimate is not smeared).  Endpoints never move.  FIRE restarts as after any O9 change."""
+        b = self.band
+        old = [x.copy() for x in b.X]
+        d = b.segment_lengths()
+        s = np.concatenate([[0.0], np.cumsum(d)])
+        knots = [0, b.P - 1]
+        if hold_climbing and 0 < b.pstar < b.P - 1:
+            knots = [0, b.pstar, b.P - 1]
+        for lo, hi in zip(knots[:-1], knots[1:]):
+            for p in range(lo + 1, hi):
+                target = s[lo] + (s[hi] - s[lo]) * (p - lo) / (hi - lo)
+                q = lo
+                while q < hi - 1 and s[q + 1] <= target:   # segment q with s_q <= target < s_{q+1}
+                    q += 1
+                t = (target - s[q]) / (s[q + 1] - s[q]) if s[q + 1] > s[q] else 0.0
+                x = old[q] + t * (old[q + 1] - old[q])
+                b.X[p] = self._post_update(x) if hasattr(self, "cell_mode") else x
+                b.E[p] = np.nan  # evaluated on the next step
+        self._reset_fire()
+
     def _reset_fire(self):
         b = self.band
         b.fire = Fire((b.P - 2,) + b.X[0].shape, **self.fire_params)

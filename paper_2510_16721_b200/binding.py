@@ -19,7 +19,7 @@ KERNEL_CLASSES = ("cell_prep", "neighbor", "force", "reduce", "scalar", "update"
 
 EXPORTS = (
     "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_adaptive", "cfneb_step_timed",
-    "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
+    "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_reparametrize", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
     "cfneb_get_path",
     "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
     "cfneb_destroy", "cfneb_strerror", "cfneb_last_cuda_error", "cfneb_util_fp64_peak",
@@ -90,7 +90,7 @@ def lib():
     L.cfneb_create.argtypes = [ctypes.POINTER(vp), i32, dp, dp, dp, dp, i32, dp, pp, vp, ctypes.c_size_t, vp]
     for name, args in (
         ("cfneb_step", [vp, i32]), ("cfneb_step_adaptive", [vp, i32, i32, f64, f64]), ("cfneb_step_timed", [vp, i32, dp]), ("cfneb_insert_image", [vp, i32]),
-        ("cfneb_delete_image", [vp, i32]), ("cfneb_adapt", [vp, f64, f64, ip, ip]),
+        ("cfneb_delete_image", [vp, i32]), ("cfneb_adapt", [vp, f64, f64, ip, ip]), ("cfneb_reparametrize", [vp, i32]),
         ("cfneb_relax_endpoints", [vp, f64, i32, i32, ip, dp, dp]), ("cfneb_get_segment_lengths", [vp, dp]), ("cfneb_get_path", [vp, ip, dp, dp, dp]),
         ("cfneb_set_path", [vp, dp, dp]), ("cfneb_get_state", [vp, dp, dp]),
         ("cfneb_get_checkpoint", [vp, dp, dp, dp, dp, ctypes.POINTER(FireState)]),
@@ -237,6 +237,12 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_adapt")
         return ni.value, nd.value
+
+    def reparametrize(self, hold_climbing=True):
+        """cfneb_reparametrize: interior images to equal arc length along the band's polyline (asynchronous)."""
+        rc = lib().cfneb_reparametrize(self._h, int(bool(hold_climbing)))
+        if rc:
+            raise CfnebError(rc, "cfneb_reparametrize")
 
     def relax_endpoints(self, fmax_tol, max_steps, rebuild_band=True):
         """cfneb_relax_endpoints: returns (steps[2], fmax[2], energy[2])."""

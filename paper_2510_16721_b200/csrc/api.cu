@@ -103,7 +103,8 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.N = N;
     d.Npad = (N + 31) / 32 * 32;
     d.S = prm->max_images;
-    d.cap = prm->max_neighbors;
+    d.cap = (prm->max_neighbors + 1) & ~1;  // even: the pair kernels walk two rows per iteration without a bound check
+    d.cap_user = prm->max_neighbors;
     d.nblk_atom = (N + kThreadsAtom - 1) / kThreadsAtom;
     d.nblk_stream = (d.Npad + kAtomsPerStreamBlock - 1) / kAtomsPerStreamBlock;
     d.nbins_max = N > 64 ? N : 64;
@@ -112,7 +113,9 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.ctl = c.take<Ctl>(1);
     d.order = c.take<int>(S);
     d.free_stack = c.take<int>(S);
-    d.seglen = c.take<double>(S);
+    d.seglen = c.take<double>(2 * S);
+    d.plan_q = c.take<int>(S);
+    d.plan_t = c.take<double>(S);
     d.perm = c.take<int>(Npad);
     d.geom = c.take<Geom>(S);
     d.X = c.take<double>(2 * S * img);
@@ -153,7 +156,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     // scratch = two halves; a half holds one exported array set (P x (N+3) x 3, or P x N x 3 + P x 9 + P)
     const size_t half = S * ((size_t)(N + 3) * 3 + 16) * sizeof(double);
     size_t sb = 2 * half + 1024;
-    const size_t nb = (size_t)N * d.cap * 4 * sizeof(int) + (size_t)N * sizeof(int) + 1024;
+    const size_t nb = (size_t)N * d.cap_user * 4 * sizeof(int) + (size_t)N * sizeof(int) + 1024;
     if (nb > sb) sb = nb;
     d.scratch = c.take<char>(sb);
     d.scratch_bytes = sb;
@@ -647,6 +650,15 @@ int cfneb_adapt(cfneb_t *h, double d_insert, double d_delete, int32_t *n_ins, in
     return sync_status(h);
 }
 
+int cfneb_reparametrize(cfneb_t *h, int32_t hold_climbing) {
+    DeviceGuard dev_guard(h);
+    if (!h) return CFNEB_EINVAL;
+    launch_reparametrize(h->d, hold_climbing ? 1 : 0, h->st);
+    h->interior_stale = true;
+    CK(cudaGetLastError());
+    return CFNEB_OK;
+}
+
 int cfneb_relax_endpoints(cfneb_t *h, double fmax_tol, int32_t max_steps, int32_t rebuild_band, int32_t *steps_done,
                           double *fmax_out, double *energy_out) {
     DeviceGuard dev_guard(h);
@@ -883,7 +895,7 @@ int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int32_t *list
     CK(cudaMemcpyAsync(&d.geom[slot].force_rebuild, &one, sizeof(int), cudaMemcpyHostToDevice, h->st));
     launch_cell_prep(d, 0, MODE_STEP, h->st);
     launch_neighbor_build(d, 0, h->st);
-    const size_t n = (size_t)d.N * d.cap;
+    const size_t n = (size_t)d.N * d.cap_user;
     int *dcount = static_cast<int *>(d.scratch), *dlist = dcount + ((d.N + 63) / 64) * 64, *dshift = dlist + n;
     launch_unpack_neighbors(d, slot, dcount, dlist, dshift, h->st);
     if (count) CK(cudaMemcpyAsync(count, dcount, sizeof(int) * d.N, cudaMemcpyDeviceToHost, h->st));

@@ -81,7 +81,8 @@ struct Geom {
 };
 
 struct Dev {
-    int N, Npad, S, cap;
+    int N, Npad, S, cap;      // cap: list rows per atom = max_neighbors rounded up to even
+    int cap_user;             // max_neighbors as given: the overflow threshold and the row length of cfneb_get_neighbors
     int potential, cell_mode, climb, fire_nmin, rebuild_every;
     int nblk_atom, nblk_stream, nbins_max;
     int nblk_red, nblk_upd;   // K4 / K6: blocks per image, each striding over the image's nblk_stream tiles
@@ -96,7 +97,9 @@ struct Dev {
     Ctl *ctl;
     int *order;               // [S] path position -> slot
     int *free_stack;          // [S] unused slots (device-side adaptive control)
-    double *seglen;           // [S] segment lengths of the last control step
+    double *seglen;           // [2 S] segment lengths of the last control step; second half: running arc length
+    int *plan_q;              // [S] re-parametrisation: image p moves onto segment plan_q[p] ...
+    double *plan_t;           // [S] ... at the fraction plan_t[p] (kernels_adapt.cu)
     int *perm;                // [Npad] internal atom index -> caller's atom index (spatial order, see api.cu)
     Geom *geom;               // [S]
     double *X, *v, *F;        // see header comment
@@ -190,6 +193,7 @@ void launch_materialize_fneb(const Dev &d, cudaStream_t st);                    
 void launch_midpoint(const Dev &d, int slot_a, int slot_b, int slot_new, cudaStream_t st);  // K7
 void launch_reset_fire(const Dev &d, cudaStream_t st);
 void launch_adapt_device(const Dev &d, double d_insert, double d_delete, cudaStream_t st);  // O9 on the device
+void launch_reparametrize(const Dev &d, int hold_climbing, cudaStream_t st);                // equal arc length (A27)
 void launch_relax_init(const Dev &d, cudaStream_t st);                                    // endpoint relaxation
 void launch_relax_step(const Dev &d, double fmax_tol, cudaStream_t st);
 void launch_segment_lengths(const Dev &d, double *out_dev, cudaStream_t st);

@@ -286,7 +286,7 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
             for (int k = valid ? min(cnt, d.cap) : 0; k < d.cap; ++k) col[(size_t)k * d.Npad] = far;
         }
     }
-    if (cnt > d.cap) set_error(d.ctl, CFNEB_ENEIGH_OVERFLOW);
+    if (cnt > d.cap_user) set_error(d.ctl, CFNEB_ENEIGH_OVERFLOW);
     if (bad_shift) set_error(d.ctl, CFNEB_ECELL);
     // block-level max, then one atomic per block
     __shared__ int s_max;
@@ -300,9 +300,9 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
 // Parity hook: list of one slot in the external layout count[N], list[N][cap] (-1 padded), shift[N][cap][3].
 __global__ void unpack_neighbors_kernel(Dev d, int slot, int *count_out, int *list_out, int *shift_out) {
     const size_t t = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= (size_t)d.N * d.cap) return;
-    const int i = (int)(t / d.cap), k = (int)(t % d.cap);  // internal (storage-order) atom index
-    const size_t e = (size_t)d.perm[i] * d.cap + k;         // row of the caller's atom
+    if (t >= (size_t)d.N * d.cap_user) return;
+    const int i = (int)(t / d.cap_user), k = (int)(t % d.cap_user);  // internal (storage-order) atom index
+    const size_t e = (size_t)d.perm[i] * d.cap_user + k;             // row of the caller's atom
     const int c = d.nbr_count[(size_t)slot * d.Npad + i];
     if (k == 0) count_out[d.perm[i]] = c;
     int j = -1, n0 = 0, n1 = 0, n2 = 0;
@@ -333,7 +333,7 @@ void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st) {
 }
 
 void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_out, int *shift_out, cudaStream_t st) {
-    const size_t n = (size_t)d.N * d.cap;
+    const size_t n = (size_t)d.N * d.cap_user;
     unpack_neighbors_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(d, slot, count_out, list_out, shift_out);
 }
 

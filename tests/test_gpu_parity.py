@@ -278,6 +278,59 @@ def test_insert_delete_and_adapt_follow_oracle():
     gpu.close()
 
 
+@pytest.mark.parametrize("k,hold", [(1, True), (1, False), (2, True)])
+def test_reparametrize_follows_oracle(k, hold):
+    """cfneb_reparametrize (kernels on the stream, nothing read back) against oracle.reparametrize: a band whose images
+    were bunched by hand goes to equal arc length along its own polyline; endpoints and the held climbing image do not
+    move by a bit; the band then keeps stepping with the oracle (lists kept or rebuilt by the staleness bound)."""
+    spec, orc, gpu = make_pair(k, cell_factor=0.0, n_images=9 if k == 2 else None)
+    orc.step(4)
+    gpu.step(4)
+    # bunch the images: pull every interior image but the climbing one towards its lower neighbour
+    ps = orc.band.pstar
+    assert gpu.get_status().climb_index == ps
+    pos, cells, _ = orc.get_path()
+    for p in range(1, orc.P - 1):
+        if p != ps and p % 2 == 1:
+            pos[p] = 0.7 * pos[p] + 0.3 * pos[p - 1]
+            cells[p] = 0.7 * cells[p] + 0.3 * cells[p - 1]
+    from oracle import cfneb as oc
+    orc2 = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
+                    fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors)
+    gpu.set_path(pos, cells)
+    orc2.step(1)
+    gpu.step(1)
+    assert gpu.get_status().climb_index == orc2.band.pstar
+    Xb, _ = gpu.get_state()
+    d_before = gpu.get_segment_lengths()
+    assert d_before.max() > 1.3 * d_before.min()
+    orc2.reparametrize(hold_climbing=hold)
+    gpu.reparametrize(hold_climbing=hold)
+    Xo, vo = orc2.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - Xb, Xo - Xb) < 1e-10 and np.all(vg == 0)
+    assert np.array_equal(Xg[0], Xb[0]) and np.array_equal(Xg[-1], Xb[-1])
+    pstar = orc2.band.pstar
+    if hold:
+        assert np.array_equal(Xg[pstar], Xb[pstar])
+        for lo, hi in ((0, pstar), (pstar, orc2.P - 1)):   # equal arc length on each side, measured along the old polyline
+            seg = np.array([np.linalg.norm(Xb[q + 1] - Xb[q]) for q in range(lo, hi)])
+            assert abs(sum(np.linalg.norm(Xg[q + 1] - Xg[q]) for q in range(lo, hi)) - seg.sum()) < 1e-2 * seg.sum()
+    d_after = gpu.get_segment_lengths()
+    assert rel(d_after, orc2.band.segment_lengths()) < 1e-10
+    if not hold:
+        assert d_after.max() < 1.02 * d_after.min()          # the polyline is nearly straight: chords ~ arcs
+    st = gpu.get_status()
+    assert st.dt == spec.fire["dt0"] and st.n_pos == 0 and st.error == 0
+    orc2.step(3)
+    gpu.step(3)
+    Xo2, _ = orc2.get_state()
+    Xg2, _ = gpu.get_state()
+    assert rel(Xg2 - Xg, Xo2 - Xo) < 1e-7
+    assert np.all(np.isfinite(gpu.get_path(positions=False)[2])) and gpu.get_status().error == 0
+    gpu.close()
+
+
 def test_image_control_errors():
     import paper_2510_16721_b200 as cf
     spec, orc, gpu = make_pair(0)

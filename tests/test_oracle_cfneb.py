@@ -253,6 +253,66 @@ def test_adaptive_control_hand_worked_band():
     assert neb.adapt(d_insert=1e9, d_delete=1e9) == (0, 0)   # P = 3: the last interior image stays
 
 
+def _plane_band(pts, pstar):
+    from oracle.neb import Band
+    neb = object.__new__(oc.CFNEB)
+    neb.fire_params = {}
+    neb.band = Band([np.array([p], dtype=float) for p in pts], lambda Xs: ([0.0] * len(Xs), [np.zeros((1, 2)) for _ in Xs]))
+    neb.band.pstar = pstar
+    return neb
+
+
+def test_reparametrize_equal_arc_length():
+    """Pin of the arc-length re-parametrisation (reading A27 of P:128): hand-worked polylines, the straight-line case
+    (equal chords to 1e-12), identity on an equispaced band, every new image on the old polyline at arc length
+    p L / (P - 1), endpoints untouched, the climbing image held."""
+    pts = lambda neb: [tuple(float(c) for c in x[0]) for x in neb.band.X]
+    # L-shaped polyline (0,0) -> (1,0) -> (1,3), bunched images: length 4, five images -> arc lengths 1, 2, 3
+    neb = _plane_band([(0, 0), (0.25, 0), (0.5, 0), (1, 0), (1, 3)], pstar=-1)
+    neb.reparametrize(hold_climbing=True)
+    assert pts(neb) == [(0.0, 0.0), (1.0, 0.0), (1.0, 1.0), (1.0, 2.0), (1.0, 3.0)]
+    assert neb.band.fire.first and np.all(neb.band.fire.v == 0) and np.all(np.isnan(neb.band.E[1:-1]))
+    # the same band with the climbing image (index 3, the corner) held: two images share the first leg of length 1,
+    # none lies on the second
+    neb = _plane_band([(0, 0), (0.25, 0), (0.5, 0), (1, 0), (1, 3)], pstar=3)
+    neb.reparametrize(hold_climbing=True)
+    assert np.allclose(np.array(pts(neb)), [(0, 0), (1 / 3, 0), (2 / 3, 0), (1, 0), (1, 3)], atol=1e-15)
+    neb = _plane_band([(0, 0), (0.25, 0), (0.5, 0), (1, 0), (1, 3)], pstar=3)
+    neb.reparametrize(hold_climbing=False)
+    assert pts(neb) == [(0.0, 0.0), (1.0, 0.0), (1.0, 1.0), (1.0, 2.0), (1.0, 3.0)]
+    # straight line, unequal spacing -> equal chords
+    rng = np.random.default_rng(5)
+    u = rng.standard_normal(2)
+    ts = np.array([0.0, 0.03, 0.4, 0.45, 0.5, 0.97, 1.0])
+    neb = _plane_band([tuple(t * u) for t in ts], pstar=-1)
+    neb.reparametrize()
+    dl = neb.band.segment_lengths()
+    assert np.abs(dl - dl.mean()).max() < 1e-12 * dl.mean()
+    # equispaced band: identity to round-off
+    neb = _plane_band([tuple(t * u) for t in np.linspace(0, 1, 7)], pstar=-1)
+    before = np.stack(neb.band.X)
+    neb.reparametrize()
+    assert np.abs(np.stack(neb.band.X) - before).max() < 1e-15
+    # general polyline in the plane: every new image lies on the old polyline at arc length p L / (P - 1)
+    old = rng.standard_normal((9, 2)).cumsum(axis=0)
+    neb = _plane_band([tuple(p) for p in old], pstar=-1)
+    neb.reparametrize()
+    new = np.stack(neb.band.X)[:, 0]
+    seg = np.linalg.norm(np.diff(old, axis=0), axis=1)
+    s = np.concatenate([[0], np.cumsum(seg)])
+    assert np.array_equal(new[0], old[0]) and np.array_equal(new[-1], old[-1])
+    for p in range(1, 8):
+        best = None
+        for q in range(8):   # brute force: closest point of every old segment
+            a, b_ = old[q], old[q + 1]
+            t = np.clip(np.dot(new[p] - a, b_ - a) / np.dot(b_ - a, b_ - a), 0, 1)
+            dist = np.linalg.norm(new[p] - (a + t * (b_ - a)))
+            arc = s[q] + t * seg[q]
+            if abs(arc - p * s[-1] / 8) < 1e-9:
+                best = dist if best is None else min(best, dist)
+        assert best is not None and best < 1e-12
+
+
 def test_bain_band_barrier_equals_the_saddle_of_the_closed_form_surface():
     """Pin of the Bain bands (BASELINE.json configs[2-4]) and of the whole crystal machinery on the FS potential with
     cell degrees of freedom: CI-NEB in the cell-filter coordinates, run to fmax < 1e-6 on a 54-atom cell, must stop
