@@ -20,6 +20,8 @@ from .configs import (
     fs_params,
     sw_params,
     dn_params,
+    nep_params,
+    two_sublattice_types,
     diamond_strain_band,
     vacancy_endpoints_unrelaxed,
     bain_endpoints,
@@ -36,6 +38,8 @@ __all__ = [
     "diamond_supercell",
     "sw_params",
     "dn_params",
+    "nep_params",
+    "two_sublattice_types",
     "diamond_strain_band",
     "splitmix64_normals",
     "CONFIGS",

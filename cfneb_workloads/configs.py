@@ -18,6 +18,7 @@ POT_LJ_SF = 0
 POT_FS_MORSE = 1
 POT_SW = 2
 POT_DNN = 3
+POT_NEP = 4
 
 
 def lj_params(eps=1.0, sigma=1.0, rc=2.5):
@@ -44,6 +45,21 @@ def dn_params(rc=4.2, K=4, M=3, L=3, H=8, seed=20251016):
     out = np.zeros(12)
     out[:6] = [rc, K, M, L, H, seed]
     return out
+
+
+def nep_params(rc_r=7.0, rc_a=4.6, n_r=6, n_a=4, k_r=8, k_a=8, L=4, H=32, n_types=2, seed=20251016):
+    """NEP-shaped potential (the descriptor network widened to the shape of NEP proper): radial / angular cut-offs,
+    radial descriptors, angular radial functions, basis sizes, Legendre orders, hidden neurons, atom types, weight
+    seed (layout of include/cfneb.h).  Data only."""
+    out = np.zeros(12)
+    out[:10] = [rc_r, rc_a, n_r, n_a, k_r, k_a, L, H, n_types, seed]
+    return out
+
+
+def two_sublattice_types(n_atoms, n_types=2):
+    """Atom types of the synthetic two-species crystal: zincblende ordering of the diamond generators' atom order
+    (8 basis atoms per conventional cell, the first four on one fcc sublattice, the last four on the other)."""
+    return (((np.arange(n_atoms) % 8) // 4) % max(int(n_types), 1)).astype(np.int32)
 
 
 def diamond_strain_band(dims, a, n_images, seed, sigma_noise, strain, noise_endpoints=True):
@@ -96,7 +112,14 @@ class WorkloadSpec:
     disorder_sigma: float = 0.0  # static Gaussian displacement of every atom, the same in all images (endpoints too)
 
     @property
+    def types(self):
+        """Atom types (NEP-shaped potential only; None otherwise)."""
+        return two_sublattice_types(self.n_atoms, int(self.pot[8])) if self.potential == POT_NEP else None
+
+    @property
     def r_cut(self):
+        if self.potential == POT_NEP:
+            return float(self.pot[0])
         if self.potential == POT_SW:
             return float(self.pot[2] * self.pot[1])
         if self.potential == POT_DNN:
@@ -108,6 +131,7 @@ _FIRE_LJ = dict(dt0=0.01, dtmax=0.05, maxstep=0.1, nmin=5, finc=1.1, fdec=0.5, a
 _FIRE_EV = dict(dt0=0.1, dtmax=1.0, maxstep=0.2, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
 _FIRE_SW = dict(dt0=0.02, dtmax=0.15, maxstep=0.05, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
 _FIRE_DNN = dict(dt0=0.005, dtmax=0.02, maxstep=0.002, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+_FIRE_NEP = dict(dt0=0.005, dtmax=0.02, maxstep=0.002, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
 _SW_STRAIN = ((0.0, 0.03, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.04))
 
 CONFIGS = [
@@ -134,6 +158,12 @@ CONFIGS = [
     # P:22), where the k-th neighbours of a warp's atoms no longer share a shell.  Throughput only.
     WorkloadSpec("c7_fs_bain_101306_disordered", POT_FS_MORSE, fs_params(), "bcc_bain", (37, 37, 37), 101306, 100, 4,
                  fire=_FIRE_EV, n_steps=500, max_images=100, skin=0.5, max_neighbors=224, disorder_sigma=0.12),
+    # not a BASELINE.json config: the many-body workload at the shape and cost of NEP proper (SURVEY.md section 8(f)
+    # item 4) -- the c5 band as a two-species (zincblende-ordered) crystal, 70 atoms inside the radial
+    # cut-off of 7 A and 28 inside the angular one of 4.6 A, 6 + 4 x 4 = 22 descriptors, Legendre orders 1..4, 32 neurons
+    # per type, type-pair expansion coefficients.  Seeded weights: cost and data flow, no physics.
+    WorkloadSpec("c8_nep_diamond_32768", POT_NEP, nep_params(), "diamond_strain", (16, 16, 16), 32768, 32, 8,
+                 noise_sigma=0.02, climb=False, fire=_FIRE_NEP, n_steps=100, max_images=32, skin=0.3, max_neighbors=128),
 ]
 
 

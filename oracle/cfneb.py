@@ -33,7 +33,7 @@ class CrystalEvaluator:
     """Callback for neb.Band: X = [R~ ; lam*B] -> (E, G) through O1-O4."""
 
     def __init__(self, h0, potential, pot, r_list, max_neighbors, lam=1.0, cell_mode=cf.CELL_B, brute=False,
-                 threads=None, pressure=0.0):
+                 threads=None, pressure=0.0, types=None):
         self.h0 = np.array(h0, dtype=np.float64)
         self.potential = int(potential)
         self.pot = np.array(pot, dtype=np.float64)
@@ -44,6 +44,7 @@ class CrystalEvaluator:
         self.brute = brute
         self.threads = threads
         self.pressure = float(pressure)
+        self.types = None if types is None else np.ascontiguousarray(types, dtype=np.int32)  # NEP-shaped potential only
         self.last = None  # (F, V, D, h) of the last evaluation, for parity hooks
 
     def deformation(self, X):
@@ -58,6 +59,7 @@ class CrystalEvaluator:
             Rts.append(Rt)
             Ds.append(D)
             hs.append(self.h0 @ D)  # h = h0 D
+        ff.set_types(self.types)
         E, F, V = ff.eval_images(np.stack(Rts), self.h0, np.stack(hs), self.potential, self.pot, self.r_list,
                                  self.cap, brute=self.brute, threads=self.threads)
         if self.pressure != 0.0:  # A25: H = U + p Omega;  V_H = V - p Omega I  (Eq. 2-3)
@@ -76,7 +78,8 @@ class CFNEB:
     """Cell-filter NEB band.  pos[P,N,3] Cartesian, cells[P,3,3] (rows = lattice vectors)."""
 
     def __init__(self, pos, cells, potential, pot, r_cut, k_spring=1.0, climb=True, cell_mode=cf.CELL_B,
-                 cell_factor=1.0, fire=None, skin=0.3, max_neighbors=128, brute=False, threads=None, pressure=0.0):
+                 cell_factor=1.0, fire=None, skin=0.3, max_neighbors=128, brute=False, threads=None, pressure=0.0,
+                 types=None):
         pos = np.asarray(pos, dtype=np.float64)
         cells = np.asarray(cells, dtype=np.float64)
         self.N = pos.shape[1]
@@ -89,7 +92,7 @@ class CFNEB:
             Rt, B, D = cf.input_mapping(pos[p], cells[p], self.h0)
             X.append(cf.pack(Rt, D if cell_mode == cf.CELL_D else B, self.lam))
         self.evaluator = CrystalEvaluator(self.h0, potential, pot, r_cut + skin, max_neighbors, self.lam, cell_mode,
-                                          brute, threads, pressure)
+                                          brute, threads, pressure, types)
         self.band = Band(X, self.evaluator, k_spring=k_spring, climb=climb, fire=self.fire_params,
                          post_update=self._post_update)
 
@@ -218,7 +221,7 @@ class CFNEB:
 
 
 def relax_endpoint(R, h, potential, pot, r_cut, fmax_tol=1e-4, max_steps=20000, cell_factor=0.0, fire=None,
-                   skin=0.3, max_neighbors=128, cell_mode=cf.CELL_B, pressure=0.0, h_ref=None):
+                   skin=0.3, max_neighbors=128, cell_mode=cf.CELL_B, pressure=0.0, h_ref=None, types=None):
     """Cell-filter FIRE relaxation of one structure (BASELINE.json configs: "both endpoints cell-relaxed").
 
     Same generalized coordinates and forces as the band (O0-O4, O7) with f = G (no NEB projection).
@@ -231,7 +234,7 @@ def relax_endpoint(R, h, potential, pot, r_cut, fmax_tol=1e-4, max_steps=20000, 
     h0 = h if h_ref is None else np.asarray(h_ref, dtype=np.float64)
     N = R.shape[0]
     lam = auto_cell_factor(h0, N) if cell_factor == 0 else float(cell_factor)
-    ev = CrystalEvaluator(h0, potential, pot, r_cut + skin, max_neighbors, lam, cell_mode, pressure=pressure)
+    ev = CrystalEvaluator(h0, potential, pot, r_cut + skin, max_neighbors, lam, cell_mode, pressure=pressure, types=types)
     Rt, B, D = cf.input_mapping(R, h, h0)
     X = cf.pack(Rt, D if cell_mode == cf.CELL_D else B, lam)  # Eq. 14 coordinates (R~, D) / Eq. 17 (R~, B)
     fire = Fire((1,) + X.shape, **(fire or {}))

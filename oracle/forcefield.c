@@ -344,16 +344,19 @@ static int sw_partial_forces(int N, const double *s, const double *h, const doub
 
 static int dn_partial_forces(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
                              const int *list, const int *shift, double *Ui, double *part);
+static int nep_partial_forces(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
+                              const int *list, const int *shift, double *Ui, double *part);
 
-/* Eq. 5 and Eq. 8 from stored partial forces; kind 2 = Stillinger-Weber, kind 3 = descriptor network */
+/* Eq. 5 and Eq. 8 from stored partial forces; kind 2 = Stillinger-Weber, kind 3 = descriptor network, kind 4 = NEP shape */
 static int manybody_energy_force_virial(int kind, int N, const double *s, const double *h, const double *pot, int cap, const int *count,
                                   const int *list, const int *shift, double *E, double *F, double *V, double *Ui_out) {
-    double rc = kind == 2 ? pot[2] * pot[1] : pot[0], rc2 = rc * rc;
+    double rc = kind == 2 ? pot[2] * pot[1] : pot[0], rc2 = rc * rc; /* kind 4: pot[0] = the radial (larger) cut-off */
     double *part = (double *)malloc(sizeof(double) * (size_t)N * cap * 3);
     double *Ui = (double *)malloc(sizeof(double) * (size_t)N);
     int prc = ORACLE_OK;
     if (kind == 2) sw_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
-    else prc = dn_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
+    else if (kind == 3) prc = dn_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
+    else prc = nep_partial_forces(N, s, h, pot, cap, count, list, shift, Ui, part);
     if (prc != ORACLE_OK) { free(part); free(Ui); return prc; }
     long double Etot = 0.0L, Vacc[9];
     for (int k = 0; k < 9; ++k) Vacc[k] = 0.0L;
@@ -506,6 +509,177 @@ static int dn_partial_forces(int N, const double *s, const double *h, const doub
 }
 
 /*
+ * NEP-shaped potential (kind 4): the descriptor network above widened to the shape of the paper's force field proper
+ * ("NEP-trained force field"; P:132's throughput is dominated by it): separate radial and angular cut-offs,
+ * two atom types with type-pair expansion coefficients, basis sizes and descriptor counts as parameters, Legendre
+ * orders up to 4, one network per type with tens of neurons.  Seeded weights: a cost and data-flow stand-in.
+ *   pot = {rc_r, rc_a, n_r, n_a, k_r, k_a, L, H, n_types, seed}: n_r, n_a <= 8; k_r, k_a <= 12; L <= 4; H <= 64; types <= 2
+ *   f_k(r; rc) = 1/2 [T_k(x) + 1] fc(r; rc),  x = 2 (r/rc - 1)^2 - 1,  fc = 1/2 [1 + cos(pi r / rc)]  (r < rc, else 0)
+ *   g^R_n(r) = sum_{k<k_r} cR[I][J][n][k] f_k(r; rc_r),  g^A_n(r) = sum_{k<k_a} cA[I][J][n][k] f_k(r; rc_a)
+ *       (I = type of the centre atom i, J = type of the neighbour j)
+ *   q_n = sum_j g^R_n(r_ij)                                                                n < n_r
+ *   q_{n_r + n L + l - 1} = sum_j sum_k g^A_n(r_ij) g^A_n(r_ik) P_l(cos theta_jik)         n < n_a, l = 1..L
+ *       (all ordered pairs of neighbours inside rc_a, j = k included; P_l Legendre)
+ *   U_i = sum_mu W1[I][mu] tanh(sum_d W0[I][mu][d] q_d - b0[I][mu])                         D = n_r + n_a L
+ * Weights: one SplitMix64(seed) stream, u in [0,1) -> w = 2u - 1, drawn in the order
+ *   for I: W0[I][mu][d] (times 0.04 for d < n_r, 0.004 otherwise), b0[I][mu] (times 0.5), W1[I][mu];
+ *   then cR[I][J][n][k], then cA[I][J][n][k] (each w as drawn).
+ * Atom types: oracle_set_types() (test infrastructure state; default all 0).
+ * Partial forces p^ij = sum_d dU_i/dq_d dq_d/dr^ij; Eq. 5 and Eq. 8 as for the other many-body potentials.
+ */
+#define NEP_MAXN 8
+#define NEP_MAXK 12
+#define NEP_MAXH 64
+#define NEP_MAXD (NEP_MAXN + NEP_MAXN * 4)
+#define NEP_MAXENV 256
+static int *g_types = NULL;
+static int g_ntypes_len = 0;
+
+void oracle_set_types(const int *types, int n) {
+    free(g_types);
+    g_types = NULL;
+    g_ntypes_len = 0;
+    if (types && n > 0) {
+        g_types = (int *)malloc(sizeof(int) * (size_t)n);
+        memcpy(g_types, types, sizeof(int) * (size_t)n);
+        g_ntypes_len = n;
+    }
+}
+
+static int type_of(int i) { return (g_types && i < g_ntypes_len) ? g_types[i] : 0; }
+
+typedef struct {
+    double W0[2][NEP_MAXH * NEP_MAXD], b0[2][NEP_MAXH], W1[2][NEP_MAXH];
+    double cR[2][2][NEP_MAXN][NEP_MAXK], cA[2][2][NEP_MAXN][NEP_MAXK];
+} nep_weights_t;
+
+static double splitmix_next(unsigned long long *st) {
+    *st += 0x9E3779B97F4A7C15ULL;
+    unsigned long long z = *st;
+    z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ULL;
+    z = (z ^ (z >> 27)) * 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return 2.0 * ((double)(z >> 11) * (1.0 / 9007199254740992.0)) - 1.0;
+}
+
+static void nep_weights(const double *pot, nep_weights_t *w) {
+    int nr = (int)pot[2], na = (int)pot[3], kr = (int)pot[4], ka = (int)pot[5], L = (int)pot[6], H = (int)pot[7], T = (int)pot[8];
+    int D = nr + na * L;
+    unsigned long long st = (unsigned long long)pot[9];
+    memset(w, 0, sizeof *w);
+    for (int I = 0; I < T; ++I) {
+        for (int mu = 0; mu < H; ++mu)
+            for (int d = 0; d < D; ++d) w->W0[I][mu * D + d] = splitmix_next(&st) * (d < nr ? 0.04 : 0.004);
+        for (int mu = 0; mu < H; ++mu) w->b0[I][mu] = 0.5 * splitmix_next(&st);
+        for (int mu = 0; mu < H; ++mu) w->W1[I][mu] = splitmix_next(&st);
+    }
+    for (int I = 0; I < T; ++I)
+        for (int J = 0; J < T; ++J)
+            for (int n = 0; n < nr; ++n)
+                for (int k = 0; k < kr; ++k) w->cR[I][J][n][k] = splitmix_next(&st);
+    for (int I = 0; I < T; ++I)
+        for (int J = 0; J < T; ++J)
+            for (int n = 0; n < na; ++n)
+                for (int k = 0; k < ka; ++k) w->cA[I][J][n][k] = splitmix_next(&st);
+}
+
+static int nep_partial_forces(int N, const double *s, const double *h, const double *pot, int cap, const int *count,
+                              const int *list, const int *shift, double *Ui, double *part) {
+    double rcr = pot[0], rca = pot[1];
+    int nr = (int)pot[2], na = (int)pot[3], kr = (int)pot[4], ka = (int)pot[5], L = (int)pot[6], H = (int)pot[7], T = (int)pot[8];
+    int D = nr + na * L;
+    if (nr < 1 || nr > NEP_MAXN || na < 1 || na > NEP_MAXN || kr < 1 || kr > NEP_MAXK || ka < 1 || ka > NEP_MAXK || L < 1 ||
+        L > 4 || H < 1 || H > NEP_MAXH || T < 1 || T > 2 || !(rcr > 0.0) || !(rca > 0.0) || rca > rcr)
+        return ORACLE_EINVAL;
+    nep_weights_t *w = (nep_weights_t *)malloc(sizeof *w);
+    nep_weights(pot, w);
+    int status = ORACLE_OK;
+    for (int i = 0; i < N && status == ORACLE_OK; ++i) {
+        int I = type_of(i);
+        int c = count[i] < cap ? count[i] : cap, n = 0;
+        static __thread double ex[NEP_MAXENV][3], er[NEP_MAXENV], gR[NEP_MAXENV][NEP_MAXN], dgR[NEP_MAXENV][NEP_MAXN],
+            gA[NEP_MAXENV][NEP_MAXN], dgA[NEP_MAXENV][NEP_MAXN];
+        static __thread int ek[NEP_MAXENV], inA[NEP_MAXENV];
+        for (int k = 0; k < c; ++k) {
+            size_t e = (size_t)i * cap + k;
+            for (int m = 0; m < 3; ++m) part[e * 3 + m] = 0.0;
+            double r[3], r2 = pair_vector(s, h, i, list[e], shift + 3 * e, r);
+            if (!(r2 < rcr * rcr)) continue;
+            if (n >= NEP_MAXENV) { status = ORACLE_ENEIGH_OVERFLOW; break; }
+            int J = type_of(list[e]);
+            double f[NEP_MAXK], df[NEP_MAXK];
+            ex[n][0] = r[0]; ex[n][1] = r[1]; ex[n][2] = r[2]; er[n] = sqrt(r2); ek[n] = k;
+            dn_basis(er[n], rcr, kr, f, df);
+            for (int q = 0; q < nr; ++q) {
+                double g = 0.0, dg = 0.0;
+                for (int b = 0; b < kr; ++b) { g += w->cR[I][J][q][b] * f[b]; dg += w->cR[I][J][q][b] * df[b]; }
+                gR[n][q] = g; dgR[n][q] = dg;
+            }
+            inA[n] = er[n] < rca;
+            if (inA[n]) {
+                dn_basis(er[n], rca, ka, f, df);
+                for (int q = 0; q < na; ++q) {
+                    double g = 0.0, dg = 0.0;
+                    for (int b = 0; b < ka; ++b) { g += w->cA[I][J][q][b] * f[b]; dg += w->cA[I][J][q][b] * df[b]; }
+                    gA[n][q] = g; dgA[n][q] = dg;
+                }
+            }
+            ++n;
+        }
+        if (status != ORACLE_OK) break;
+        double q[NEP_MAXD];
+        for (int d = 0; d < D; ++d) q[d] = 0.0;
+        for (int a = 0; a < n; ++a)
+            for (int m = 0; m < nr; ++m) q[m] += gR[a][m];
+        for (int a = 0; a < n; ++a) {
+            if (!inA[a]) continue;
+            for (int b = 0; b < n; ++b) {
+                if (!inA[b]) continue;
+                double cs = (ex[a][0] * ex[b][0] + ex[a][1] * ex[b][1] + ex[a][2] * ex[b][2]) / (er[a] * er[b]);
+                double P[4] = {cs, 0.5 * (3.0 * cs * cs - 1.0), 0.5 * (5.0 * cs * cs * cs - 3.0 * cs),
+                               0.125 * (35.0 * cs * cs * cs * cs - 30.0 * cs * cs + 3.0)};
+                for (int m = 0; m < na; ++m)
+                    for (int l = 0; l < L; ++l) q[nr + m * L + l] += gA[a][m] * gA[b][m] * P[l];
+            }
+        }
+        double Fd[NEP_MAXD], ui = 0.0;
+        for (int d = 0; d < D; ++d) Fd[d] = 0.0;
+        for (int mu = 0; mu < H; ++mu) {
+            double z = -w->b0[I][mu];
+            for (int d = 0; d < D; ++d) z += w->W0[I][mu * D + d] * q[d];
+            double t = tanh(z);
+            ui += w->W1[I][mu] * t;
+            for (int d = 0; d < D; ++d) Fd[d] += w->W1[I][mu] * (1.0 - t * t) * w->W0[I][mu * D + d];
+        }
+        Ui[i] = ui;
+        for (int a = 0; a < n; ++a) {
+            double p[3] = {0.0, 0.0, 0.0};
+            for (int m2 = 0; m2 < nr; ++m2)
+                for (int m = 0; m < 3; ++m) p[m] += Fd[m2] * dgR[a][m2] * ex[a][m] / er[a];
+            if (inA[a])
+                for (int b = 0; b < n; ++b) {
+                    if (!inA[b]) continue;
+                    double cs = (ex[a][0] * ex[b][0] + ex[a][1] * ex[b][1] + ex[a][2] * ex[b][2]) / (er[a] * er[b]);
+                    double P[4] = {cs, 0.5 * (3.0 * cs * cs - 1.0), 0.5 * (5.0 * cs * cs * cs - 3.0 * cs),
+                                   0.125 * (35.0 * cs * cs * cs * cs - 30.0 * cs * cs + 3.0)};
+                    double dP[4] = {1.0, 3.0 * cs, 0.5 * (15.0 * cs * cs - 3.0), 0.125 * (140.0 * cs * cs * cs - 60.0 * cs)};
+                    for (int mm = 0; mm < na; ++mm)
+                        for (int l = 0; l < L; ++l) {
+                            double g = 2.0 * Fd[nr + mm * L + l];
+                            for (int m = 0; m < 3; ++m) {
+                                double dcos = (ex[b][m] / er[b] - cs * ex[a][m] / er[a]) / er[a];
+                                p[m] += g * (dgA[a][mm] * gA[b][mm] * P[l] * ex[a][m] / er[a] + gA[a][mm] * gA[b][mm] * dP[l] * dcos);
+                            }
+                        }
+                }
+            for (int m = 0; m < 3; ++m) part[((size_t)i * cap + ek[a]) * 3 + m] = p[m];
+        }
+    }
+    free(w);
+    return status;
+}
+
+/*
  * Energy, forces, virial of one image from its neighbour list (Eq. 4, 5, 8).
  * Outputs: *E total energy; F[N*3] Cartesian forces; V[9] virial, V_mn = -1/2 sum r_m f_n;
  * Ui[N] per-atom energies (may be NULL); rho_out[N] FS densities (may be NULL).
@@ -513,7 +687,7 @@ static int dn_partial_forces(int N, const double *s, const double *h, const doub
 int oracle_energy_force_virial(int N, const double *Rt, const double *h0, const double *h, int kind,
                                const double *pot, int cap, const int *count, const int *list, const int *shift,
                                double *E, double *F, double *V, double *Ui, double *rho_out) {
-    if (kind < 0 || kind > 3) return ORACLE_EINVAL;
+    if (kind < 0 || kind > 4) return ORACLE_EINVAL;
     double *s = (double *)malloc(sizeof(double) * 3 * (size_t)N);
     int rc = fractional(N, Rt, h0, s);
     if (rc) { free(s); return rc; }

@@ -27,6 +27,8 @@ def lib():
         _lib.oracle_energy_force_virial.argtypes = [c_int, dp, dp, dp, c_int, dp, c_int, ip, ip, ip, dp, dp, dp, dp, dp]
         _lib.oracle_eval_images.restype = c_int
         _lib.oracle_eval_images.argtypes = [c_int, c_int, dp, dp, dp, c_int, dp, c_dbl, c_int, c_int, dp, dp, dp]
+        _lib.oracle_set_types.restype = None
+        _lib.oracle_set_types.argtypes = [ip, c_int]
         _lib.oracle_max_threads.restype = c_int
         _lib.oracle_set_threads.restype = None
         _lib.oracle_set_threads.argtypes = [c_int]
@@ -46,6 +48,15 @@ class OracleError(RuntimeError):
     def __init__(self, code):
         super().__init__("oracle error %d" % code)
         self.code = code
+
+
+def set_types(types):
+    """Atom types (0 / 1) of the NEP-shaped potential (kind 4) for all later evaluations; None = all 0."""
+    if types is None:
+        lib().oracle_set_types(None, 0)
+        return
+    t = np.ascontiguousarray(types, dtype=np.int32)
+    lib().oracle_set_types(_i(t), int(t.size))
 
 
 def max_threads():
