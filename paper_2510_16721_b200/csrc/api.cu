@@ -106,6 +106,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.cap = (prm->max_neighbors + 1) & ~1;  // even: the pair kernels walk two rows per iteration without a bound check
     d.cap_user = prm->max_neighbors;
     d.nblk_atom = (N + kThreadsAtom - 1) / kThreadsAtom;
+    d.nblk_force = many_body(prm) ? d.nblk_atom : (N + kThreadsPair - 1) / kThreadsPair;
     d.nblk_stream = (d.Npad + kAtomsPerStreamBlock - 1) / kAtomsPerStreamBlock;
     d.nbins_max = N > 64 ? N : 64;
     const size_t S = d.S, Npad = d.Npad, img = 3 * Npad;
@@ -132,7 +133,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.Gc = c.take<double>(S * 9);
     d.dots = c.take<double>(S * kNDots);
     d.coef = c.take<double>(S * 4);
-    d.part_force = c.take<double>(S * d.nblk_atom * kNForcePart);
+    d.part_force = c.take<double>(S * d.nblk_force * kNForcePart);
     d.part_dots = c.take<double>(S * d.nblk_stream * kNDots);
     d.relax = c.take<RelaxState>(2);
     d.part_relax = c.take<double>((size_t)2 * d.nblk_stream * 4);
@@ -144,8 +145,15 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.nbr_count = c.take<int>(S * Npad);
     d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 16 * Npad);  // 16 rows of slack for the force kernels' look-ahead
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
-    d.nbr_tmp = c.take<uint32_t>(S * (size_t)d.cap * Npad);
-    d.nbr_bkt = c.take<unsigned char>(S * (size_t)d.cap * Npad);
+    d.rebuild_slots = c.take<int>(S);
+    {   // K1 scratch: one region per resident block of the search kernel (sized for the largest device we know)
+        int dev = 0, sms = 148;
+        if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        d.n_sm = sms;
+        d.n_search_blocks = sms * search_blocks_per_sm();
+        d.scr_tmp = c.take<uint32_t>((size_t)d.n_search_blocks * d.cap * kThreadsAtom);
+        d.scr_bkt = c.take<unsigned char>((size_t)d.n_search_blocks * d.cap * kThreadsAtom);
+    }
     d.part = many_body(prm) ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
     d.nbr_mirror = many_body(prm) ? c.take<unsigned short>(S * (size_t)d.cap * Npad) : nullptr;
     d.dn_w = prm->potential == CFNEB_POT_DNN ? c.take<double>(kDnWeights) : nullptr;

@@ -19,7 +19,11 @@
 
 namespace cfn {
 
-constexpr int kThreadsAtom = 128;      // force / neighbour / position kernels: 1 atom per thread
+constexpr int kThreadsAtom = 128;      // neighbour / position / many-body kernels: 1 atom per thread
+#ifndef CFNEB_PAIR_THREADS
+#define CFNEB_PAIR_THREADS 128
+#endif
+constexpr int kThreadsPair = CFNEB_PAIR_THREADS;  // pair-potential K2 kernels (density, force): 1 atom per thread
 constexpr int kThreadsStream = 256;    // K4 / K6: 2 atoms per thread (double2)
 constexpr int kAtomsPerStreamBlock = kThreadsStream * 2;
 constexpr int kNDots = 10;             // pp, mm, pm, Gp, Gm, GG, Gv, pv, mv, vv
@@ -56,6 +60,7 @@ struct Ctl {
     int ins_a, ins_b, ins_new;    // slots of a pending midpoint insertion, ins_new < 0: none
     int changed;                  // the last control step changed the band (FIRE restart pending)
     int n_inserted, n_deleted;    // totals since create
+    int n_rebuild;                // images whose neighbour list is rebuilt this step (rebuild_slots[0 .. n_rebuild-1])
 };
 
 // FIRE state of one endpoint during cfneb_relax_endpoints (kernels_relax.cu); device resident.
@@ -85,6 +90,9 @@ struct Dev {
     int cap_user;             // max_neighbors as given: the overflow threshold and the row length of cfneb_get_neighbors
     int potential, cell_mode, climb, fire_nmin, rebuild_every;
     int nblk_atom, nblk_stream, nbins_max;
+    int nblk_force;           // blocks per image of the K2 kernels that write part_force (pair kernels: kThreadsPair atoms each)
+    int n_sm;                 // multiprocessors of the device
+    int n_search_blocks;      // grid of neighbor_search_kernel (resident blocks: n_sm x blocks per SM)
     int nblk_red, nblk_upd;   // K4 / K6: blocks per image, each striding over the image's nblk_stream tiles
     int nb_cap[3];
     double pot[12];
@@ -111,7 +119,7 @@ struct Dev {
     double *Xc, *vc;
     double *E, *V, *Gc;       // [S], [S][9], [S][9]
     double *dots, *coef;      // [S][10], [S][4]
-    double *part_force;       // [S][nblk_atom][kNForcePart]
+    double *part_force;       // [S][nblk_force][kNForcePart]
     RelaxState *relax;        // [2]
     double *part_relax;       // [2][nblk_stream][4]
     double *part_dots;        // [S][nblk_stream][10]  (the first nblk_red rows of an image are used)
@@ -123,11 +131,12 @@ struct Dev {
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
     unsigned short *nbr_tail; // [S][kTailBuckets][Npad] number of entries below tail bucket t (list sorted by bucket)
-    uint32_t *nbr_tmp;        // [S][cap][Npad]  unsorted list of a rebuild (scratch of K1)
     double *dn_w;               // [kDnWeights] W0[H][D], b0[H], W1[H] of CFNEB_POT_DNN
     unsigned short *nbr_mirror; // [S][cap][Npad] row of the mirror entry (j; i, -n) of each entry (many-body potentials only)
     double *part;             // [S][cap][3][Npad] partial forces p^ij = dU_i/dr^ij per list entry (many-body potentials only)
-    unsigned char *nbr_bkt;   // [S][cap][Npad]  r^2 bucket of each unsorted entry (scratch of K1)
+    int *rebuild_slots;       // [S] compact list of the slots that rebuild this step (K1)
+    uint32_t *scr_tmp;        // [n_search_blocks][cap][128] unsorted column of the block's current work item (K1 scratch)
+    unsigned char *scr_bkt;   // [n_search_blocks][cap][128] r^2 bucket of each unsorted entry
     int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
     int *bin_cursor;          // [S][nbins_max]
     int *bin_members;         // [S][Npad]
@@ -178,6 +187,7 @@ void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_d
 void launch_interpolate(const Dev &d, int P, cudaStream_t st);
 void launch_cell_prep(const Dev &d, int p_lo, int mode, cudaStream_t st);                 // K0 + positions
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st);                      // K1
+int search_blocks_per_sm();
 void prepare_potential(Dev &d);  // fills Dev::potc from pot / r_cut (host)
 void launch_force(const Dev &d, int p_lo, cudaStream_t st);
 void launch_mirror_sw(const Dev &d, int p_lo, cudaStream_t st);                          // mirror rows after a list build

@@ -223,7 +223,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 2) dn_partial_kernel(Dev d, int 
     double ui_lo = 0.0;
     block_sum_dd(ui[0], ui_lo, red);
     if (threadIdx.x == 0) {
-        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
         out[7] = ui[0];
         out[9] = ui_lo;
     }

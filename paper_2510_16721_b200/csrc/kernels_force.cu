@@ -182,6 +182,8 @@ __device__ __forceinline__ double fs_density(const FSc &c, uint32_t T, double r2
 // and sectors one iteration ahead of use; the loop is unrolled over the two pipeline stages so that no register
 // is rotated.  Rows past an atom's count hold a stand-in entry that is out of range by construction
 // (kernels_neighbor.cu), and the list carries 8 rows of slack, so no load is predicated.
+__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 template <class Body>
 __device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_t stride, const double4 *Rc, int cnt_w,
                                           Body body) {
@@ -189,6 +191,12 @@ __device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_
     double4 sa0 = ld256(Rc + (a0 & kIdxMask)), sa1 = ld256(Rc + (a1 & kIdxMask)), sb0, sb1;
     lp += 4 * stride;
     for (int k = 0; k < cnt_w; k += 4) {
+#if CFNEB_PF_ROWS
+        // the list streams from HBM once per pass: pull the rows CFNEB_PF_ROWS ahead into L2 (a register-free look-ahead
+        // on top of the two-stage one; ncu: 22 % of the density kernel's samples waited on the first use of an entry)
+#pragma unroll
+        for (int u = 0; u < 4; ++u) prefetch_l2(lp + (size_t)(CFNEB_PF_ROWS - 4 + u) * stride);
+#endif
         sb0 = ld256(Rc + (b0 & kIdxMask));
         sb1 = ld256(Rc + (b1 & kIdxMask));
         {
@@ -213,7 +221,16 @@ __device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_
 // K2a (FS only): densities rho_i = sum_j psi(r_ij) over the Verlet list; writes F'(rho_i) into Rc[i].w and the
 // per-block embedding energy.  Two entries per iteration in 70 registers: seven blocks (28 warps) per SM measured
 // 10.66 ms for K2 at c4 against 10.94 with four entries per iteration at five blocks.
-__global__ void __launch_bounds__(kThreadsAtom, 7) density_kernel(Dev d, int p_lo) {
+#ifndef CFNEB_DENSITY_BLOCKS
+#define CFNEB_DENSITY_BLOCKS (7 * 128 / CFNEB_PAIR_THREADS)
+#endif
+#ifndef CFNEB_FORCE_BLOCKS
+#define CFNEB_FORCE_BLOCKS (5 * 128 / CFNEB_PAIR_THREADS)
+#endif
+#ifndef CFNEB_PF_ROWS
+#define CFNEB_PF_ROWS 0
+#endif
+__global__ void __launch_bounds__(kThreadsPair, CFNEB_DENSITY_BLOCKS) density_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
@@ -274,7 +291,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 7) density_kernel(Dev d, int p_l
     double emb_lo = 0.0;
     block_sum_dd(emb[0], emb_lo, red2);
     if (threadIdx.x == 0) {
-        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
         out[7] = emb[0];
         out[9] = emb_lo;
     }
@@ -282,7 +299,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 7) density_kernel(Dev d, int p_l
 
 // K2b: forces, energies and the virial over the Verlet list.
 template <int POT, bool SHARE>
-__global__ void __launch_bounds__(kThreadsAtom, 5) force_kernel(Dev d, int p_lo) {
+__global__ void __launch_bounds__(kThreadsPair, CFNEB_FORCE_BLOCKS) force_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
@@ -346,7 +363,7 @@ __global__ void __launch_bounds__(kThreadsAtom, 5) force_kernel(Dev d, int p_lo)
     double e_hi = acc.ui, e_lo = 0.0;  // the energy channel in two doubles (block_sum_dd)
     block_sum_dd(e_hi, e_lo, red);
     if (threadIdx.x == 0) {
-        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
         out[0] = e_hi;
         out[8] = e_lo;
 #pragma unroll
@@ -383,17 +400,17 @@ void prepare_potential(Dev &d) {
 void launch_force(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
-    dim3 grid(d.nblk_atom, nimg);
+    dim3 grid(d.nblk_force, nimg);
     if (d.potential == CFNEB_POT_SW) {
         launch_force_sw(d, p_lo, st);
     } else if (d.potential == CFNEB_POT_DNN) {
         launch_force_dn(d, p_lo, st);
     } else if (d.potential == CFNEB_POT_LJ_SF) {
-        force_kernel<CFNEB_POT_LJ_SF, false><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+        force_kernel<CFNEB_POT_LJ_SF, false><<<grid, kThreadsPair, 0, st>>>(d, p_lo);
     } else {
-        density_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
-        if (d.pot[3] == 2.0 * d.pot[1]) force_kernel<CFNEB_POT_FS_MORSE, true><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
-        else force_kernel<CFNEB_POT_FS_MORSE, false><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+        density_kernel<<<grid, kThreadsPair, 0, st>>>(d, p_lo);
+        if (d.pot[3] == 2.0 * d.pot[1]) force_kernel<CFNEB_POT_FS_MORSE, true><<<grid, kThreadsPair, 0, st>>>(d, p_lo);
+        else force_kernel<CFNEB_POT_FS_MORSE, false><<<grid, kThreadsPair, 0, st>>>(d, p_lo);
     }
 }
 

@@ -102,8 +102,8 @@ __global__ void __launch_bounds__(256) finalize_kernel(Dev d, int p_lo) {
 #pragma unroll
     for (int q = 0; q < 8; ++q) a8[q] = 0.0;
     double e_hi = 0.0, e_lo = 0.0;
-    const double *pf = d.part_force + (size_t)slot * d.nblk_atom * kNForcePart;
-    for (int b = threadIdx.x; b < d.nblk_atom; b += blockDim.x) {
+    const double *pf = d.part_force + (size_t)slot * d.nblk_force * kNForcePart;
+    for (int b = threadIdx.x; b < d.nblk_force; b += blockDim.x) {
         const double *q8 = pf + (size_t)b * kNForcePart;
 #pragma unroll
         for (int q = 1; q < 7; ++q) a8[q] += q8[q];

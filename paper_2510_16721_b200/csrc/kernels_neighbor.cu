@@ -125,15 +125,45 @@ __device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
 // nbr_list (histogram kept in shared memory during the flushes).  Rows cnt..cap-1 are filled with a stand-in
 // entry (the atom itself shifted by -4 cell vectors along axis 0: farther than r_list whenever a list can be
 // built at all), so the force kernels read any row below cap without a bounds test and find it out of range.
+// Compact list of the images (slots) of the selected set whose list is rebuilt this step, in path order.
+__global__ void rebuild_list_kernel(Dev d, int p_lo) {
+    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+    const int P = d.ctl->P;
+    const int ny = p_lo == kEndpointsOnly ? 2 : d.S - 2 * p_lo;
+    int n = 0;
+    for (int y = 0; y < ny; ++y) {
+        int p;
+        if (!image_of(y, p_lo, P, p)) continue;
+        const int slot = d.order[p];
+        if (d.geom[slot].rebuild) d.rebuild_slots[n++] = slot;
+    }
+    d.ctl->n_rebuild = n;
+}
+
 constexpr int kRadialBuckets = kInnerBuckets + kTailBuckets;
 constexpr int kQueue = 32;
 constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
-__global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, int p_lo) {
-    int slot;
-    if (!image_active(d, p_lo, blockIdx.y, slot)) return;
+#ifndef CFNEB_SEARCH_BLOCKS
+#define CFNEB_SEARCH_BLOCKS 5
+#endif
+#ifndef CFNEB_SEARCH_HSMEM
+#define CFNEB_SEARCH_HSMEM 0
+#endif
+// Round 2: the grid has a fixed size (CFNEB_SEARCH_BLOCKS blocks per multiprocessor) and takes its work items
+// (rebuilding image, block of 128 atoms) from the compact list of rebuild_list_kernel -- a step in which no list is
+// stale costs one exit per resident block instead of 77 616 -- and the unsorted column / bucket scratch of a block
+// is a region of its own, reused item after item (scr_tmp, scr_bkt: 143 KB per block, L2 resident), instead of two
+// arrays of the size of the list itself (round 1: 11.4 GB of workspace, 2.8 x the list in DRAM writes per rebuild).
+__global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_search_kernel(Dev d) {
     __shared__ unsigned short s_hist[kRadialBuckets * kThreadsAtom];
     __shared__ uint32_t s_queue[kQueue * kThreadsAtom];
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    __shared__ double s_h[9];
+    __shared__ int s_max;
+    if (threadIdx.x == 0) s_max = 0;
+    const int n_items = d.ctl->n_rebuild * d.nblk_atom;
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
+    const int slot = d.rebuild_slots[item / d.nblk_atom];
+    const int i = (item % d.nblk_atom) * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
     const int ic = valid ? i : 0;  // idle lanes shadow atom 0 with empty bin ranges
     int cnt = 0;
@@ -146,11 +176,18 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
     const int re0 = g->reach[0], re1 = g->reach[1], re2 = g->reach[2];
     if (re0 > 3 || re1 > 3 || re2 > 3) {  // periodic shifts are stored in 3 bits per axis
         if (threadIdx.x == 0) set_error(d.ctl, CFNEB_ECELL);
-        return;
+        continue;
     }
+#if CFNEB_SEARCH_HSMEM
+    __syncthreads();  // every thread is done with the previous item's cell matrix
+    if (threadIdx.x < 9) s_h[threadIdx.x] = g->h[threadIdx.x];
+    __syncthreads();
+    const double *h = s_h;  // in shared memory: eighteen registers fewer per thread
+#else
     double h[9];
 #pragma unroll
     for (int k = 0; k < 9; ++k) h[k] = g->h[k];
+#endif
     const double4 si = d.Sw[(size_t)slot * d.Npad + ic];
     const unsigned long long fli = (unsigned long long)__double_as_longlong(si.w);
     const int fi0 = (int)(fli & 1023u), fi1 = (int)((fli >> 10) & 1023u), fi2 = (int)((fli >> 20) & 1023u);
@@ -168,8 +205,8 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
     const float rlf = (float)(d.r_list + 64.0 * 1.2e-7 * 2.0 * Lext * (1.0 + max(re0, max(re1, re2))));
     const float rl2f = rlf * rlf;
     uint32_t *__restrict__ list = d.nbr_list + (size_t)slot * d.cap * d.Npad + ic;
-    uint32_t *__restrict__ tmp = d.nbr_tmp + (size_t)slot * d.cap * d.Npad + ic;
-    unsigned char *__restrict__ bkt = d.nbr_bkt + (size_t)slot * d.cap * d.Npad + ic;
+    uint32_t *__restrict__ tmp = d.scr_tmp + (size_t)blockIdx.x * d.cap * kThreadsAtom + threadIdx.x;
+    unsigned char *__restrict__ bkt = d.scr_bkt + (size_t)blockIdx.x * d.cap * kThreadsAtom + threadIdx.x;
     // radial buckets: kInnerBuckets uniform in r^2 below r_cut^2, kTailBuckets uniform between r_cut^2 and r_list^2
     const double rl2 = d.r_list * d.r_list, rc2 = d.r_cut * d.r_cut;
     const double bscale_in = (double)kInnerBuckets / rc2, bscale_tail = rl2 > rc2 ? (double)kTailBuckets / (rl2 - rc2) : 0.0;
@@ -203,8 +240,8 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
                                       ((uint32_t)((n2 + 4) & 7) << 6);
                 const int bk = r2 < rc2 ? min((int)(r2 * bscale_in), kInnerBuckets - 1)
                                         : kInnerBuckets + min((int)((r2 - rc2) * bscale_tail), kTailBuckets - 1);
-                tmp[(size_t)cnt * d.Npad] = (uint32_t)j | (code << kShiftBits);
-                bkt[(size_t)cnt * d.Npad] = (unsigned char)bk;
+                tmp[(size_t)cnt * kThreadsAtom] = (uint32_t)j | (code << kShiftBits);
+                bkt[(size_t)cnt * kThreadsAtom] = (unsigned char)bk;
                 hist[bk * kThreadsAtom] += 1;
             }
             ++cnt;
@@ -265,7 +302,7 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
         int bk[4];
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            const size_t o = (size_t)min(k0 + u, n - 1) * d.Npad;
+            const size_t o = (size_t)min(k0 + u, n - 1) * kThreadsAtom;
             t[u] = tmp[o];
             bk[u] = bkt[o];
         }
@@ -279,7 +316,7 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
     }
     }  // valid
     {   // stand-in rows cnt..cap-1 (idle lanes of the last block included: their columns exist up to Npad)
-        const int i_pad = blockIdx.x * blockDim.x + threadIdx.x;
+        const int i_pad = i;
         if (i_pad < d.Npad) {
             uint32_t *col = d.nbr_list + (size_t)slot * d.cap * d.Npad + i_pad;
             const uint32_t far = (uint32_t)(valid ? i : 0) | (kCodeFar << kShiftBits);
@@ -288,11 +325,9 @@ __global__ void __launch_bounds__(kThreadsAtom) neighbor_search_kernel(Dev d, in
     }
     if (cnt > d.cap_user) set_error(d.ctl, CFNEB_ENEIGH_OVERFLOW);
     if (bad_shift) set_error(d.ctl, CFNEB_ECELL);
-    // block-level max, then one atomic per block
-    __shared__ int s_max;
-    if (threadIdx.x == 0) s_max = 0;
-    __syncthreads();
     atomicMax(&s_max, cnt);
+    }  // work items
+    // block-level max, then one atomic per block
     __syncthreads();
     if (threadIdx.x == 0 && s_max > d.ctl->max_nbr_seen) atomicMax(&d.ctl->max_nbr_seen, s_max);
 }
@@ -323,14 +358,17 @@ __global__ void unpack_neighbors_kernel(Dev d, int slot, int *count_out, int *li
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
+    rebuild_list_kernel<<<1, 32, 0, st>>>(d, p_lo);
     bin_scan_kernel<<<nimg, 1024, 0, st>>>(d, p_lo);
     dim3 ga(d.nblk_atom, nimg);
     bin_fill_kernel<<<ga, kThreadsAtom, 0, st>>>(d, p_lo);
     dim3 gb((d.nbins_max + 127) / 128, nimg);
     bin_sort_kernel<<<gb, 128, 0, st>>>(d, p_lo);
-    neighbor_search_kernel<<<ga, kThreadsAtom, 0, st>>>(d, p_lo);
+    neighbor_search_kernel<<<d.n_search_blocks, kThreadsAtom, 0, st>>>(d);
     if (d.potential == CFNEB_POT_SW || d.potential == CFNEB_POT_DNN) launch_mirror_sw(d, p_lo, st);
 }
+
+int search_blocks_per_sm() { return CFNEB_SEARCH_BLOCKS; }
 
 void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_out, int *shift_out, cudaStream_t st) {
     const size_t n = (size_t)d.N * d.cap_user;

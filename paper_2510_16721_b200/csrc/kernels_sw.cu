@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_partial_kernel(Dev d, int p_l
     double ui_lo = 0.0;
     block_sum_dd(ui[0], ui_lo, red);
     if (threadIdx.x == 0) {
-        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
         out[7] = ui[0];
         out[9] = ui_lo;
     }
@@ -164,7 +164,7 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
     double out7[7] = {0.0, -0.5 * vxx, -0.5 * vyy, -0.5 * vzz, -0.5 * vxy, -0.5 * vxz, -0.5 * vyz};
     block_sum<7>(out7, red);
     if (threadIdx.x == 0) {
-        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
 #pragma unroll
         for (int n = 0; n < 7; ++n) out[n] = out7[n];
         out[8] = 0.0;
@@ -240,7 +240,7 @@ __global__ void __launch_bounds__(kThreadsAtom) pair_force_batched_kernel(Dev d,
     double out7[7] = {0.0, -0.5 * vxx, -0.5 * vyy, -0.5 * vzz, -0.5 * vxy, -0.5 * vxz, -0.5 * vyz};
     block_sum<7>(out7, red);
     if (threadIdx.x == 0) {
-        double *out = d.part_force + ((size_t)slot * d.nblk_atom + blockIdx.x) * kNForcePart;
+        double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
 #pragma unroll
         for (int n = 0; n < 7; ++n) out[n] = out7[n];
         out[8] = 0.0;
