@@ -41,6 +41,7 @@ if ROOT not in sys.path:
 
 METRIC = "atom_image_neb_steps_per_s"
 UNIT = "atom*image*steps/s"
+POTENTIAL_NAMES = ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber", "descriptor_network", "nep_shaped_network")
 ALGO_BYTES_PER_UNIT = 192.0  # K4 reads X, F, v (72 B); K6 reads X, F, v (72 B), writes X_new, v (48 B)
 
 
@@ -196,8 +197,13 @@ def run_oracle(k, steps, warmup, budget_s):
         lo = max(1, (P - (n_images - 2)) // 2)
         idx = [0] + list(range(lo, lo + n_images - 2)) + [P - 1]
         pos, cells = pos[idx], cells[idx]
+    types = None
+    if spec.types is not None:  # NEP-shaped potential: the generators' two-species ordering at the sample's atom count
+        from cfneb_workloads import two_sublattice_types
+        types = two_sublattice_types(pos.shape[1], int(spec.pot[8]))
     band = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb,
-                    cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors, threads=threads)
+                    cell_factor=0.0, fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors, threads=threads,
+                    types=types)
     for _ in range(warmup):
         band.step(1)
     t0 = time.perf_counter()
@@ -230,7 +236,7 @@ def main_reference(args):
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(args.config), "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber", "descriptor_network")[int(spec.potential)],
+        "config": {"workload": workload_name(args.config), "potential": POTENTIAL_NAMES[int(spec.potential)],
                    "sample": r["sample"], "runs_on": "host CPU (oracle/, plain fp64 C + numpy)"},
         "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "kind": "oracle", "sample": r["sample"]},
         "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -345,7 +351,7 @@ def main_ours(args):
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic",
         "config": {"workload": workload_name(k), "n_atoms": N, "n_images": P, "movable_images": P - 2,
-                   "potential": ("lj_shifted_force", "finnis_sinclair_morse", "stillinger_weber", "descriptor_network")[int(spec.potential)],
+                   "potential": POTENTIAL_NAMES[int(spec.potential)],
                    "cell_filter": "rotation-free B = D D^T (Eq. 17), cell_factor auto", "climb": bool(spec.climb),
                    "value_counts": "N x (P-2) per step", "value_counting_all_images": value * P / (P - 2),
                    "parallelism": "replicas only (x%d)" % world if world > 1 else "single GPU",

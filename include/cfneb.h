@@ -57,7 +57,7 @@ enum {
     CFNEB_ERANGE = -7           /* bad image index, endpoint / climbing-image delete, more than max_images */
 };
 
-enum { CFNEB_POT_LJ_SF = 0, CFNEB_POT_FS_MORSE = 1, CFNEB_POT_SW = 2, CFNEB_POT_DNN = 3 };
+enum { CFNEB_POT_LJ_SF = 0, CFNEB_POT_FS_MORSE = 1, CFNEB_POT_SW = 2, CFNEB_POT_DNN = 3, CFNEB_POT_NEP = 4 };
 enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default) */, CFNEB_CELL_D = 2 /* Eq. 14 */ };
 
 /*
@@ -80,6 +80,20 @@ enum { CFNEB_CELL_FIXED = 0, CFNEB_CELL_B = 1 /* Eq. 17, rotation-free (default)
  *       (n < M, l = 1..L, all ordered pairs j, k including j = k),  U_i = sum_mu W1_mu tanh(sum_d W0_{mu d} q_d - b0_mu).
  *       Weights: SplitMix64 stream from `seed`, u = (z >> 11) 2^-53, w = 2u - 1, in the order W0[mu][d] (scaled by
  *       0.3/8 for d < K, 0.3/40 otherwise), b0[mu] (scaled by 0.5), W1[mu].  Same two passes as CFNEB_POT_SW.
+ *   potential = CFNEB_POT_NEP (the descriptor network widened to the shape and cost of the paper's force field proper,
+ *       P:138 "NEP-trained force field"; seeded weights, a cost and data-flow stand-in):
+ *       pot = {rc_r, rc_a, n_r, n_a, k_r, k_a, L, H, n_types, seed}: rc_a <= rc_r; n_r, n_a <= 8 radial descriptors /
+ *       angular radial functions; k_r, k_a <= 12 basis functions; L <= 4; H <= 64 neurons; n_types <= 2 (`types`):
+ *       f_k(r; rc) as above with its own cut-off,  g^R_n(r) = sum_{k<k_r} cR[I][J][n][k] f_k(r; rc_r),
+ *       g^A_n(r) = sum_{k<k_a} cA[I][J][n][k] f_k(r; rc_a)   (I = type of atom i, J = type of the neighbour),
+ *       q_n = sum_j g^R_n(r_ij) (n < n_r),  q_{n_r + n L + l - 1} = sum_j sum_k g^A_n(r_ij) g^A_n(r_ik) P_l(cos theta_jik)
+ *       (n < n_a, l = 1..L, neighbours inside rc_a, all ordered pairs including j = k),
+ *       U_i = sum_mu W1[I][mu] tanh(sum_d W0[I][mu][d] q_d - b0[I][mu]).
+ *       Weights: one SplitMix64 stream from `seed`, w = 2u - 1, drawn in the order: for each type I: W0[I][mu][d]
+ *       (scaled by 0.04 for d < n_r, 0.004 otherwise), b0[I][mu] (scaled by 0.5), W1[I][mu]; then cR[I][J][n][k];
+ *       then cA[I][J][n][k].  The neighbour lists use rc_r.  Same two passes as CFNEB_POT_SW.
+ *   types: CFNEB_POT_NEP only: HOST pointer to n_atoms atom types in [0, n_types), read by cfneb_create and not
+ *       retained (NULL = all atoms of type 0).
  *   k_spring: uniform spring constant of Eq. 1 (A14).  climb: 1 = climbing image (ref [12]).
  *   cell_factor: lam of A13; 0 = auto (Omega0^(1/3) N^(1/6)); 1 = the paper's equations literally.
  *   fire_*: FIRE constants of O7 (one state for the whole band).
@@ -106,6 +120,7 @@ typedef struct cfneb_params {
     double fire_dt0, fire_dtmax, fire_maxstep, fire_finc, fire_fdec, fire_astart, fire_fa;
     double skin;
     double pressure;
+    const int32_t *types;
 } cfneb_params;
 
 /* Snapshot written by cfneb_get_status (synchronises the stream). */

@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libcfneb.so")
 
 OK, EINVAL, ENOMEM, ECUDA, ENEIGH_OVERFLOW, ECELL, ENAN, ERANGE = 0, -1, -2, -3, -4, -5, -6, -7
-POT_LJ_SF, POT_FS_MORSE, POT_SW, POT_DNN = 0, 1, 2, 3
+POT_LJ_SF, POT_FS_MORSE, POT_SW, POT_DNN, POT_NEP = 0, 1, 2, 3, 4
 CELL_FIXED, CELL_B, CELL_D = 0, 1, 2
 K_CELLPREP, K_NEIGHBOR, K_FORCE, K_REDUCE, K_SCALAR, K_UPDATE, NKERNELS = 0, 1, 2, 3, 4, 5, 6
 KERNEL_CLASSES = ("cell_prep", "neighbor", "force", "reduce", "scalar", "update")
@@ -36,6 +36,7 @@ class Params(ctypes.Structure):
         ("fire_dt0", ctypes.c_double), ("fire_dtmax", ctypes.c_double), ("fire_maxstep", ctypes.c_double),
         ("fire_finc", ctypes.c_double), ("fire_fdec", ctypes.c_double), ("fire_astart", ctypes.c_double),
         ("fire_fa", ctypes.c_double), ("skin", ctypes.c_double), ("pressure", ctypes.c_double),
+        ("types", ctypes.POINTER(ctypes.c_int32)),
     ]
 
 
@@ -131,6 +132,10 @@ def default_params(**kw):
     fire = kw.pop("fire", None) or {}
     for k, v in fire.items():
         setattr(p, "fire_" + k, v)
+    types = kw.pop("types", None)
+    if types is not None:  # kept alive by the Params object: cfneb_create reads it
+        p._types = np.ascontiguousarray(types, dtype=np.int32)
+        p.types = p._types.ctypes.data_as(ctypes.POINTER(ctypes.c_int32))
     pot = kw.pop("pot", None)
     if pot is not None:
         for k in range(12):

@@ -72,15 +72,18 @@ double cutoff_of(const cfneb_params *prm) {
         case CFNEB_POT_LJ_SF: return prm->pot[2];
         case CFNEB_POT_SW: return prm->pot[2] * prm->pot[1];
         case CFNEB_POT_DNN: return prm->pot[0];
+        case CFNEB_POT_NEP: return prm->pot[0];  // the radial (larger) cut-off
         default: return prm->pot[7];
     }
 }
 
-bool many_body(const cfneb_params *prm) { return prm->potential == CFNEB_POT_SW || prm->potential == CFNEB_POT_DNN; }
+bool many_body(const cfneb_params *prm) {
+    return prm->potential == CFNEB_POT_SW || prm->potential == CFNEB_POT_DNN || prm->potential == CFNEB_POT_NEP;
+}
 
 bool valid_params(int32_t n_atoms, const cfneb_params *prm) {
     if (!prm || n_atoms < 1 || n_atoms >= kMaxAtoms) return false;
-    if (prm->potential < CFNEB_POT_LJ_SF || prm->potential > CFNEB_POT_DNN) return false;
+    if (prm->potential < CFNEB_POT_LJ_SF || prm->potential > CFNEB_POT_NEP) return false;
     if (prm->cell_mode < CFNEB_CELL_FIXED || prm->cell_mode > CFNEB_CELL_D) return false;
     if (prm->max_images < 3 || prm->max_neighbors < 1 || prm->max_neighbors > 4096) return false;
     if (!(prm->skin >= 0.0) || !(prm->cell_factor >= 0.0) || !isfinite(prm->pressure)) return false;
@@ -91,6 +94,14 @@ bool valid_params(int32_t n_atoms, const cfneb_params *prm) {
         for (int k = 1; k <= 5; ++k)
             if (!(q[k] >= 0.0) || q[k] != floor(q[k]) || q[k] > 9.0e15) return false;
         if (q[1] < 1 || q[1] > 4 || q[2] < 1 || q[2] > 4 || q[3] < 1 || q[3] > 3 || q[4] < 1 || q[4] > 8) return false;
+    }
+    if (prm->potential == CFNEB_POT_NEP) {
+        const double *q = prm->pot;
+        for (int k = 2; k <= 9; ++k)
+            if (!(q[k] >= 0.0) || q[k] != floor(q[k]) || q[k] > 9.0e15) return false;
+        if (!(q[1] > 0.0) || q[1] > q[0]) return false;                                        // rc_a <= rc_r
+        if (q[2] < 1 || q[2] > 8 || q[3] < 1 || q[3] > 8 || q[4] < 1 || q[4] > 12 || q[5] < 1 || q[5] > 12) return false;
+        if (q[6] < 1 || q[6] > 4 || q[7] < 1 || q[7] > 64 || q[8] < 1 || q[8] > 2) return false;
     }
     if (prm->potential == CFNEB_POT_FS_MORSE && !(prm->pot[7] > prm->pot[6])) return false;
     if (!(prm->fire_dt0 > 0.0) || !(prm->fire_dtmax > 0.0) || !(prm->fire_maxstep > 0.0)) return false;
@@ -106,7 +117,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.cap = (prm->max_neighbors + 1) & ~1;  // even: the pair kernels walk two rows per iteration without a bound check
     d.cap_user = prm->max_neighbors;
     d.nblk_atom = (N + kThreadsAtom - 1) / kThreadsAtom;
-    d.nblk_force = many_body(prm) ? d.nblk_atom : (N + kThreadsPair - 1) / kThreadsPair;
+    d.nblk_force = prm->potential == CFNEB_POT_NEP ? (N + 31) / 32 : many_body(prm) ? d.nblk_atom : (N + kThreadsPair - 1) / kThreadsPair;
     d.nblk_stream = (d.Npad + kAtomsPerStreamBlock - 1) / kAtomsPerStreamBlock;
     d.nbins_max = N > 64 ? N : 64;
     const size_t S = d.S, Npad = d.Npad, img = 3 * Npad;
@@ -156,7 +167,10 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     }
     d.part = many_body(prm) ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
     d.nbr_mirror = many_body(prm) ? c.take<unsigned short>(S * (size_t)d.cap * Npad) : nullptr;
-    d.dn_w = prm->potential == CFNEB_POT_DNN ? c.take<double>(kDnWeights) : nullptr;
+    d.dn_w = prm->potential == CFNEB_POT_DNN ? c.take<double>(kDnWeights)
+             : prm->potential == CFNEB_POT_NEP ? c.take<double>(nep_weight_count(prm->pot)) : nullptr;
+    d.types = prm->potential == CFNEB_POT_NEP ? c.take<int>(Npad) : nullptr;
+    d.nep_S = prm->potential == CFNEB_POT_NEP ? c.take<double>(S * (size_t)prm->pot[3] * 35 * Npad) : nullptr;
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
     d.bin_members = c.take<int>(S * Npad);
@@ -464,6 +478,20 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
         perm.resize(d.Npad, 0);
         CKC(cudaMemcpyAsync(d.perm, perm.data(), sizeof(int) * d.Npad, cudaMemcpyHostToDevice, h->st));
         CKC(cudaStreamSynchronize(h->st));  // `perm` is a temporary
+        if (d.potential == CFNEB_POT_NEP) {  // atom types in storage order; the weight stream of include/cfneb.h
+            const int T = (int)d.pot[8];
+            std::vector<int> ty(d.Npad, 0);
+            for (int i = 0; i < n_atoms; ++i) {
+                const int t = prm->types ? prm->types[perm[i]] : 0;
+                if (t < 0 || t >= T) { cfneb_destroy(h); return CFNEB_EINVAL; }
+                ty[i] = t;
+            }
+            std::vector<double> w(nep_weight_count(d.pot));
+            nep_fill_weights(d.pot, w.data());
+            CKC(cudaMemcpyAsync(d.types, ty.data(), sizeof(int) * d.Npad, cudaMemcpyHostToDevice, h->st));
+            CKC(cudaMemcpyAsync(d.dn_w, w.data(), sizeof(double) * w.size(), cudaMemcpyHostToDevice, h->st));
+            CKC(cudaStreamSynchronize(h->st));  // temporaries
+        }
     }
 
     // stage the host inputs: pos [n][N][3] then cells [n][9]

@@ -131,7 +131,9 @@ struct Dev {
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
     unsigned short *nbr_tail; // [S][kTailBuckets][Npad] number of entries below tail bucket t (list sorted by bucket)
-    double *dn_w;               // [kDnWeights] W0[H][D], b0[H], W1[H] of CFNEB_POT_DNN
+    double *dn_w;               // [kDnWeights] W0[H][D], b0[H], W1[H] of CFNEB_POT_DNN; CFNEB_POT_NEP: see kernels_nep.cu
+    int *types;                 // [Npad] atom types in storage order (CFNEB_POT_NEP)
+    double *nep_S;              // [S][n_a][35][Npad] moments of the angular channels between the two walks (CFNEB_POT_NEP)
     unsigned short *nbr_mirror; // [S][cap][Npad] row of the mirror entry (j; i, -n) of each entry (many-body potentials only)
     double *part;             // [S][cap][3][Npad] partial forces p^ij = dU_i/dr^ij per list entry (many-body potentials only)
     int *rebuild_slots;       // [S] compact list of the slots that rebuild this step (K1)
@@ -192,6 +194,9 @@ void prepare_potential(Dev &d);  // fills Dev::potc from pot / r_cut (host)
 void launch_force(const Dev &d, int p_lo, cudaStream_t st);
 void launch_mirror_sw(const Dev &d, int p_lo, cudaStream_t st);                          // mirror rows after a list build
 void launch_force_dn(const Dev &d, int p_lo, cudaStream_t st);                            // K2, descriptor network (kernels_dn.cu)
+void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st);                           // K2, NEP-shaped potential (kernels_nep.cu)
+int nep_weight_count(const double *pot);
+void nep_fill_weights(const double *pot, double *w);  // host: the SplitMix64 weight stream of include/cfneb.h
 void launch_pair_forces_manybody(const Dev &d, int p_lo, cudaStream_t st);                // pass 2 of both (kernels_sw.cu)
 void launch_force_sw(const Dev &d, int p_lo, cudaStream_t st);                            // K2, Stillinger-Weber (kernels_sw.cu)                               // K2
 void launch_reduce(const Dev &d, cudaStream_t st);                                        // K4 (atom rows)

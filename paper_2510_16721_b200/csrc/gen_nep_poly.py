@@ -41,19 +41,20 @@ def main():
             p, v = (e[0], e[1], e[2] - 1), "z"
         out.append("    m[%d] = m[%d] * %s;" % (i, idx[p], v))
     out.append("}")
-    out.append("// value phi = sum_c C_c m_c and gradient (d phi / dx, dy, dz) from the monomials of degree <= 3")
-    out.append("__device__ __forceinline__ void nep_poly_grad(const double (&C)[kNepC], const double (&m)[kNepC], double &gx, double &gy,")
-    out.append("                                              double &gz) {")
-    for var, name in ((0, "gx"), (1, "gy"), (2, "gz")):
-        terms = []
-        for i, e in enumerate(EXPS):
-            if e[var] == 0:
-                continue
-            p = list(e)
-            p[var] -= 1
-            k = e[var]
-            terms.append("%sC[%d] * m[%d]" % ("" if k == 1 else "%d.0 * " % k, i, idx[tuple(p)]))
-        out.append("    %s = %s;" % (name, " + ".join(terms)))
+    out.append("// Gradient of phi(u) = sum_c C_c m_c(u), degree by degree: g[l-1] = grad of the degree-l part, l = 1..4, from")
+    out.append("// the monomials of degree <= 3.  (Euler: u . g[l-1] = l phi_l, so the value follows from the gradients.)")
+    out.append("__device__ __forceinline__ void nep_poly_grad(const double (&C)[kNepC], const double (&m)[kNepC], double (&g)[4][3]) {")
+    for deg in range(1, 5):
+        for var in range(3):
+            terms = []
+            for i, e in enumerate(EXPS):
+                if sum(e) != deg or e[var] == 0:
+                    continue
+                p = list(e)
+                p[var] -= 1
+                k = e[var]
+                terms.append("%sC[%d] * m[%d]" % ("" if k == 1 else "%d.0 * " % k, i, idx[tuple(p)]))
+            out.append("    g[%d][%d] = %s;" % (deg - 1, var, " + ".join(terms)))
     out.append("}")
     out.append("}  // namespace cfn")
     print("\n".join(out))

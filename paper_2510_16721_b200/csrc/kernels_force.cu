@@ -375,7 +375,7 @@ __global__ void __launch_bounds__(kThreadsPair, CFNEB_FORCE_BLOCKS) force_kernel
 void prepare_potential(Dev &d) {
     for (double &x : d.potc) x = 0.0;
     d.potc[kPotcRc2] = d.r_cut * d.r_cut;
-    if (d.potential == CFNEB_POT_DNN) {
+    if (d.potential == CFNEB_POT_DNN || d.potential == CFNEB_POT_NEP) {
         // constants are read from Dev::pot, weights from Dev::dn_w
     } else if (d.potential == CFNEB_POT_SW) {
         for (int k = 0; k < 9; ++k) d.potc[k] = d.pot[k];  // eps, sigma, a, lambda, gamma, A, B, p, q
@@ -405,6 +405,8 @@ void launch_force(const Dev &d, int p_lo, cudaStream_t st) {
         launch_force_sw(d, p_lo, st);
     } else if (d.potential == CFNEB_POT_DNN) {
         launch_force_dn(d, p_lo, st);
+    } else if (d.potential == CFNEB_POT_NEP) {
+        launch_force_nep(d, p_lo, st);
     } else if (d.potential == CFNEB_POT_LJ_SF) {
         force_kernel<CFNEB_POT_LJ_SF, false><<<grid, kThreadsPair, 0, st>>>(d, p_lo);
     } else {

@@ -365,7 +365,7 @@ void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st) {
     dim3 gb((d.nbins_max + 127) / 128, nimg);
     bin_sort_kernel<<<gb, 128, 0, st>>>(d, p_lo);
     neighbor_search_kernel<<<d.n_search_blocks, kThreadsAtom, 0, st>>>(d);
-    if (d.potential == CFNEB_POT_SW || d.potential == CFNEB_POT_DNN) launch_mirror_sw(d, p_lo, st);
+    if (d.potential == CFNEB_POT_SW || d.potential == CFNEB_POT_DNN || d.potential == CFNEB_POT_NEP) launch_mirror_sw(d, p_lo, st);
 }
 
 int search_blocks_per_sm() { return CFNEB_SEARCH_BLOCKS; }

@@ -281,7 +281,7 @@ void launch_pair_forces_manybody(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
-    if (d.potential == CFNEB_POT_DNN) pair_force_batched_kernel<4><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+    if (d.potential == CFNEB_POT_DNN || d.potential == CFNEB_POT_NEP) pair_force_batched_kernel<4><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
     else sw_force_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
 }
 

@@ -43,11 +43,20 @@ __device__ __forceinline__ void nep_monomials(double x, double y, double z, doub
     m[33] = m[19] * y;
     m[34] = m[19] * z;
 }
-// value phi = sum_c C_c m_c and gradient (d phi / dx, dy, dz) from the monomials of degree <= 3
-__device__ __forceinline__ void nep_poly_grad(const double (&C)[kNepC], const double (&m)[kNepC], double &gx, double &gy,
-                                              double &gz) {
-    gx = C[1] * m[0] + 2.0 * C[4] * m[1] + C[5] * m[2] + C[6] * m[3] + 3.0 * C[10] * m[4] + 2.0 * C[11] * m[5] + 2.0 * C[12] * m[6] + C[13] * m[7] + C[14] * m[8] + C[15] * m[9] + 4.0 * C[20] * m[10] + 3.0 * C[21] * m[11] + 3.0 * C[22] * m[12] + 2.0 * C[23] * m[13] + 2.0 * C[24] * m[14] + 2.0 * C[25] * m[15] + C[26] * m[16] + C[27] * m[17] + C[28] * m[18] + C[29] * m[19];
-    gy = C[2] * m[0] + C[5] * m[1] + 2.0 * C[7] * m[2] + C[8] * m[3] + C[11] * m[4] + 2.0 * C[13] * m[5] + C[14] * m[6] + 3.0 * C[16] * m[7] + 2.0 * C[17] * m[8] + C[18] * m[9] + C[21] * m[10] + 2.0 * C[23] * m[11] + C[24] * m[12] + 3.0 * C[26] * m[13] + 2.0 * C[27] * m[14] + C[28] * m[15] + 4.0 * C[30] * m[16] + 3.0 * C[31] * m[17] + 2.0 * C[32] * m[18] + C[33] * m[19];
-    gz = C[3] * m[0] + C[6] * m[1] + C[8] * m[2] + 2.0 * C[9] * m[3] + C[12] * m[4] + C[14] * m[5] + 2.0 * C[15] * m[6] + C[17] * m[7] + 2.0 * C[18] * m[8] + 3.0 * C[19] * m[9] + C[22] * m[10] + C[24] * m[11] + 2.0 * C[25] * m[12] + C[27] * m[13] + 2.0 * C[28] * m[14] + 3.0 * C[29] * m[15] + C[31] * m[16] + 2.0 * C[32] * m[17] + 3.0 * C[33] * m[18] + 4.0 * C[34] * m[19];
+// Gradient of phi(u) = sum_c C_c m_c(u), degree by degree: g[l-1] = grad of the degree-l part, l = 1..4, from
+// the monomials of degree <= 3.  (Euler: u . g[l-1] = l phi_l, so the value follows from the gradients.)
+__device__ __forceinline__ void nep_poly_grad(const double (&C)[kNepC], const double (&m)[kNepC], double (&g)[4][3]) {
+    g[0][0] = C[1] * m[0];
+    g[0][1] = C[2] * m[0];
+    g[0][2] = C[3] * m[0];
+    g[1][0] = 2.0 * C[4] * m[1] + C[5] * m[2] + C[6] * m[3];
+    g[1][1] = C[5] * m[1] + 2.0 * C[7] * m[2] + C[8] * m[3];
+    g[1][2] = C[6] * m[1] + C[8] * m[2] + 2.0 * C[9] * m[3];
+    g[2][0] = 3.0 * C[10] * m[4] + 2.0 * C[11] * m[5] + 2.0 * C[12] * m[6] + C[13] * m[7] + C[14] * m[8] + C[15] * m[9];
+    g[2][1] = C[11] * m[4] + 2.0 * C[13] * m[5] + C[14] * m[6] + 3.0 * C[16] * m[7] + 2.0 * C[17] * m[8] + C[18] * m[9];
+    g[2][2] = C[12] * m[4] + C[14] * m[5] + 2.0 * C[15] * m[6] + C[17] * m[7] + 2.0 * C[18] * m[8] + 3.0 * C[19] * m[9];
+    g[3][0] = 4.0 * C[20] * m[10] + 3.0 * C[21] * m[11] + 3.0 * C[22] * m[12] + 2.0 * C[23] * m[13] + 2.0 * C[24] * m[14] + 2.0 * C[25] * m[15] + C[26] * m[16] + C[27] * m[17] + C[28] * m[18] + C[29] * m[19];
+    g[3][1] = C[21] * m[10] + 2.0 * C[23] * m[11] + C[24] * m[12] + 3.0 * C[26] * m[13] + 2.0 * C[27] * m[14] + C[28] * m[15] + 4.0 * C[30] * m[16] + 3.0 * C[31] * m[17] + 2.0 * C[32] * m[18] + C[33] * m[19];
+    g[3][2] = C[22] * m[10] + C[24] * m[11] + 2.0 * C[25] * m[12] + C[27] * m[13] + 2.0 * C[28] * m[14] + 3.0 * C[29] * m[15] + C[31] * m[16] + 2.0 * C[32] * m[17] + 3.0 * C[33] * m[18] + 4.0 * C[34] * m[19];
 }
 }  // namespace cfn

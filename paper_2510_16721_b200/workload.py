@@ -8,5 +8,8 @@ def params_for(spec, cell_factor=1.0, cell_mode=CELL_B, max_images=None, max_nei
               climb=int(bool(spec.climb)), cell_mode=int(cell_mode), cell_factor=float(cell_factor),
               skin=float(spec.skin), max_neighbors=int(max_neighbors or spec.max_neighbors),
               max_images=int(max_images or max(spec.max_images, spec.n_images)), fire=dict(spec.fire))
+    types = getattr(spec, "types", None)
+    if types is not None:
+        kw["types"] = types
     kw.update(overrides)
     return default_params(**kw)

@@ -34,7 +34,7 @@ def test_library_exports_every_declared_symbol(cf):
 
 
 def test_params_struct_layout_and_defaults(cf):
-    assert ctypes.sizeof(cf.Params) == 8 * 4 + (12 + 2 + 7 + 1 + 1) * 8
+    assert ctypes.sizeof(cf.Params) == 8 * 4 + (12 + 2 + 7 + 1 + 1) * 8 + 8   # ... + the types pointer
     p = cf.default_params()
     assert (p.potential, p.cell_mode, p.climb, p.fire_nmin) == (cf.POT_LJ_SF, cf.CELL_B, 1, 5)
     assert (p.fire_dt0, p.fire_dtmax, p.fire_maxstep, p.fire_finc, p.fire_fdec, p.fire_astart, p.fire_fa) == (

@@ -156,10 +156,10 @@ def test_c4_long_run_survives_equal_energy_images():
     gpu.close()
 
 
-@pytest.mark.parametrize("k", [5, 6])
+@pytest.mark.parametrize("k", [5, 6, 8])
 def test_many_body_workloads_at_full_atom_count(k):
-    """The many-body workloads bench.py --config 5 / 6 times (32 768 atoms; Stillinger-Weber and the descriptor
-    network of NEP's shape) at their full atom count in the same launch configuration, on the first, two mid-path and
+    """The many-body workloads bench.py --config 5 / 6 / 8 times (32 768 atoms; Stillinger-Weber, the descriptor
+    network, and the NEP-shaped potential with two cut-offs and two atom types) at their full atom count in the same launch configuration, on the first, two mid-path and
     the last image of the 32: energies, per-atom forces, virials and f^NEB element by element, then two full steps."""
     import paper_2510_16721_b200 as cf
     from oracle import cfneb as oc
@@ -167,7 +167,8 @@ def test_many_body_workloads_at_full_atom_count(k):
     idx = [0, 15, 16, spec.n_images - 1]
     pos, cells = pos[idx], cells[idx]
     orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
-                   fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors, threads=min(4, host_threads()))
+                   fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors, threads=min(4, host_threads()),
+                   types=spec.types)
     gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0, max_images=4))
     f_or = orc.band.forces()
     F, V, fneb, E = gpu.get_forces()

@@ -1001,6 +1001,67 @@ def test_descriptor_network_many_body_forces_and_steps(dims, n_images, net):
     gpu.close()
 
 
+@pytest.mark.parametrize("dims,n_images,net", [
+    ((2, 2, 2), 4, dict()),
+    ((3, 3, 3), 3, dict()),
+    ((2, 2, 3), 3, dict(rc_r=5.2, rc_a=3.2, n_r=3, n_a=2, k_r=5, k_a=4, L=2, H=9, n_types=1, seed=7)),
+    ((2, 2, 2), 3, dict(rc_r=4.4, rc_a=4.4, n_r=8, n_a=8, k_r=12, k_a=12, L=4, H=64, n_types=2, seed=3)),
+    ((2, 2, 2), 4, dict(rc_r=6.1, rc_a=2.9, n_r=1, n_a=5, k_r=1, k_a=3, L=3, H=2, n_types=2, seed=12))])
+def test_nep_shaped_potential_forces_and_steps(dims, n_images, net):
+    """CFNEB_POT_NEP -- the shape of the paper's force field proper: two cut-offs, two atom types with type-pair
+    expansion coefficients, Legendre orders to 4, tens of neurons per type -- against the oracle: energies, forces,
+    virials, f^NEB, one exact step, then five more.  Disordered, strained two-species diamond bands; the default
+    shape has 70 atoms inside the radial and 28 inside the angular cut-off; the cells are narrower than 2 r_list
+    (atoms see several images of one neighbour).  The other shapes exercise the lane split: one and two passes over
+    the angular channels (n_a = 2, 5, 8), the largest network, a single neuron, a single type, rc_a = rc_r."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import diamond_strain_band, nep_params, two_sublattice_types
+    from oracle import cfneb as oc
+    pot = nep_params(**net)
+    pos, cells = diamond_strain_band(dims, 5.35, n_images, 29, 0.08, ((0.0, 0.03, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.04)))
+    N = pos.shape[1]
+    types = two_sublattice_types(N, int(pot[8]))
+    # steps large enough that the displacement (dt0^2 f ~ 1e-5) stands clear of the round-off of the coordinates (~1e-15)
+    fire = dict(dt0=0.05, dtmax=0.1, maxstep=0.01, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+    cap = 320
+    orc = oc.CFNEB(pos, cells, 4, pot, pot[0], k_spring=1.0, climb=True, cell_factor=0.0, fire=fire, skin=0.3, max_neighbors=cap,
+                   types=types)
+    prm = cf.default_params(potential=cf.POT_NEP, pot=list(pot), k_spring=1.0, climb=1, cell_factor=0.0, skin=0.3,
+                            max_neighbors=cap, max_images=n_images, fire=fire, types=types)
+    gpu = cf.CFNEB(pos, cells, prm)
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert np.max(np.abs(orc.evaluator.last["F"])) > 1e-3
+    assert rel(E, orc.band.E) < TOL_FORCE
+    assert rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    assert rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
+    assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    X0 = first_step_exact(orc, gpu)
+    orc.step(5)
+    gpu.step(5)
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
+    assert gpu.get_status().error == 0
+    gpu.close()
+
+
+def test_nep_shaped_potential_parameter_errors():
+    """Out-of-range shapes are refused (workspace size 0); a type outside [0, n_types) is refused by cfneb_create."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import diamond_strain_band, nep_params
+    for bad in (dict(L=5), dict(n_r=9), dict(n_a=0), dict(k_r=13), dict(H=65), dict(n_types=3), dict(rc_a=8.0), dict(rc_r=0.0)):
+        prm = cf.default_params(potential=cf.POT_NEP, pot=list(nep_params(**bad)), max_images=3)
+        assert cf.binding.workspace_bytes(64, prm) == 0
+    pos, cells = diamond_strain_band((2, 2, 2), 5.35, 3, 1, 0.05, ((0.0, 0.02, 0.0), (0.0, 0.0, 0.0), (0.0, 0.0, 0.02)))
+    types = np.zeros(pos.shape[1], dtype=np.int32)
+    types[5] = 2
+    prm = cf.default_params(potential=cf.POT_NEP, pot=list(nep_params()), max_images=3, max_neighbors=320, types=types)
+    with pytest.raises(cf.CfnebError) as e:
+        cf.CFNEB(pos, cells, prm)
+    assert e.value.code == cf.binding.EINVAL
+
+
 def test_descriptor_network_parameter_errors():
     """Out-of-range network shapes are refused (workspace size 0)."""
     import paper_2510_16721_b200 as cf
