@@ -55,6 +55,7 @@ def parse_args():
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-steady", action="store_true", help="skip the steady-state window (profiling runs)")
     return ap.parse_args()
 
 
@@ -299,7 +300,7 @@ def main_ours(args):
     value = world * units_per_step * args.steps / (ms_total * 1e-3)
 
     # ---- steady state: max(K, 100) further graph-launched steps (list rebuilds amortised) ----
-    n_ss = max(args.steps, 100)
+    n_ss = 0 if args.no_steady else max(args.steps, 100)
     barrier()
     e0.record(stream)
     band.step(n_ss)
@@ -308,7 +309,7 @@ def main_ours(args):
     barrier()
     ms_ss = max_over_ranks(e0.elapsed_time(e1))
     st2 = band.get_status()
-    steady = {"value": world * units_per_step * n_ss / (ms_ss * 1e-3), "unit": UNIT, "steps": n_ss, "ms_per_step": ms_ss / n_ss,
+    steady = None if n_ss == 0 else {"value": world * units_per_step * n_ss / (ms_ss * 1e-3), "unit": UNIT, "steps": n_ss, "ms_per_step": ms_ss / n_ss,
               "neighbor_rebuilds": int(st2.rebuilds - st1.rebuilds),
               "what": "the next max(K, 100) steps of the same band, same timing; includes the amortised list rebuilds"}
 
@@ -374,7 +375,8 @@ def measure_e2e(band, n_steps, barrier, max_over_ranks, world, units_per_step):
     """Host-buffer loop through the C ABI, a true continuation of the band: per step the whole checkpoint goes
     host -> device (cfneb_set_state from pinned memory: X, v, the coordinates the lists were built at, the list
     accounting, the FIRE scalars), one iteration runs, and the checkpoint comes back (cfneb_get_checkpoint).  The
-    sequence of states is bit-identical to the device-resident run."""
+    sequence of states is bit-identical to the device-resident run (the handle keeps its neighbour lists: the state
+    it is handed is the one it holds; a new handle would take X_list / list_aux as well and replay the builds)."""
     import torch
     import paper_2510_16721_b200 as cf
     ck = band.get_checkpoint()
@@ -386,8 +388,8 @@ def measure_e2e(band, n_steps, barrier, max_over_ranks, world, units_per_step):
         t.numpy()[...] = a
         return t
 
-    keep = [pinned(ck[k]) for k in ("X", "v", "X_list", "list_aux")]
-    X, v, Xl, aux = (t.numpy() for t in keep)
+    keep = [pinned(ck[k]) for k in ("X", "v")]
+    X, v = (t.numpy() for t in keep)
     fire = ck["fire"]
     L = cf.lib()
     import ctypes
@@ -395,9 +397,9 @@ def measure_e2e(band, n_steps, barrier, max_over_ranks, world, units_per_step):
 
     def one():
         nonlocal fire
-        band.set_state(X, v, Xl, aux, fire)                     # H2D: 3 P (N+3) 3 + 4 P doubles
+        band.set_state(X, v, None, None, fire)                  # H2D: 2 P (N+3) 3 doubles; the handle keeps its lists
         band.step(1)
-        rc = L.cfneb_get_checkpoint(band._h, dp(X), dp(v), dp(Xl), dp(aux), ctypes.byref(fire))  # D2H: the same; synchronises
+        rc = L.cfneb_get_checkpoint(band._h, dp(X), dp(v), None, None, ctypes.byref(fire))  # D2H: the same; synchronises
         if rc:
             raise cf.CfnebError(rc, "cfneb_get_checkpoint")
 
@@ -408,7 +410,7 @@ def measure_e2e(band, n_steps, barrier, max_over_ranks, world, units_per_step):
         one()
     barrier()
     dt = max_over_ranks(time.perf_counter() - t0)
-    nbytes = (3 * X.size + aux.size) * 8 + 32
+    nbytes = 2 * X.size * 8 + 32
     return {"value": world * units_per_step * n_steps / dt, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
             "steps": n_steps, "ms_per_step": 1e3 * dt / n_steps,
             "what": "per step: cfneb_set_state(pinned host checkpoint) + cfneb_step(1) + cfneb_get_checkpoint(pinned host); wall "

@@ -156,8 +156,11 @@ CONFIGS = [
     # not a BASELINE.json config: configs[4] with every atom displaced by a static Gaussian kick of 0.12 A (the same in
     # all images, endpoints included) -- the paper's large bands are nucleated, locally disordered structures (P:18,
     # P:22), where the k-th neighbours of a warp's atoms no longer share a shell.  Throughput only.
+    # Small FIRE steps: the kicked lattice is far from any minimum (forces of tens of eV/A, the endpoints included and
+    # fixed), and the point is the cost of an iteration while the disorder is there, not where this band would end up.
     WorkloadSpec("c7_fs_bain_101306_disordered", POT_FS_MORSE, fs_params(), "bcc_bain", (37, 37, 37), 101306, 100, 4,
-                 fire=_FIRE_EV, n_steps=500, max_images=100, skin=0.5, max_neighbors=224, disorder_sigma=0.12),
+                 fire=dict(dt0=0.005, dtmax=0.02, maxstep=0.01, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99),
+                 n_steps=500, max_images=100, skin=0.5, max_neighbors=224, disorder_sigma=0.12),
     # not a BASELINE.json config: the many-body workload at the shape and cost of NEP proper (SURVEY.md section 8(f)
     # item 4) -- the c5 band as a two-species (zincblende-ordered) crystal, 70 atoms inside the radial
     # cut-off of 7 A and 28 inside the angular one of 4.6 A, 6 + 4 x 4 = 22 descriptors, Legendre orders 1..4, 32 neurons

@@ -284,8 +284,11 @@ CFNEB_API int cfneb_get_checkpoint(cfneb_t *h, double *X, double *v, double *X_l
  * Restore a checkpoint into a band of the same P, N and parameters.  X is copied as given (no round trip through
  * Cartesian coordinates), v as given (endpoint rows are ignored: zero); fire == NULL restarts FIRE (v is then zeroed).
  * With X_list and list_aux the neighbour lists are rebuilt at X_list and the accounting restored, which makes the
- * continuation bit-identical (given the atom order of the handle: the same pos_init at cfneb_create); with
- * X_list == NULL the lists are built fresh at X and the continuation agrees to round-off only (summation order).
+ * continuation bit-identical in a NEW handle (given its atom order: the same pos_init at cfneb_create).  With
+ * X_list == NULL the handle's lists are kept and the distance of X from the stored coordinates is added to each image's
+ * staleness bound (as cfneb_set_path does): handing a running band its own state back -- the host round trip of
+ * bench.py's e2e loop -- rebuilds nothing and continues bit for bit; any other state continues to round-off
+ * (summation order of the lists).
  * Endpoint energies are re-evaluated, interior energies by the next step (as cfneb_set_path).  Synchronises.
  * Errors: CFNEB_EINVAL (null X, X_list without list_aux, fire scalars out of range).
  */

@@ -866,7 +866,7 @@ int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *
     int rc;
     if (X_list) {  // replay the list builds: lists at X_list, then the coordinates proper
         CK(cudaMemcpyAsync(dX, X_list, n * sizeof(double), cudaMemcpyHostToDevice, st));
-        launch_import_state(d, dX, nullptr, st);
+        launch_import_state(d, dX, nullptr, 0, st);
         CK(cudaStreamSynchronize(st));
         rc = force_rebuild_all(h);
         if (rc) return rc;
@@ -875,21 +875,20 @@ int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *
     }
     CK(cudaMemcpyAsync(dX, X, n * sizeof(double), cudaMemcpyHostToDevice, st));
     if (v && fire) CK(cudaMemcpyAsync(dv, v, n * sizeof(double), cudaMemcpyHostToDevice, st));
-    launch_import_state(d, dX, (v && fire) ? dv : nullptr, st);
+    // without X_list the neighbour lists are kept: the distance of the new coordinates from the stored ones goes into
+    // each image's staleness bound (as in cfneb_set_path), so a state that is the stored one -- the host round trip of a
+    // running band -- rebuilds nothing and continues bit for bit
+    launch_import_state(d, dX, (v && fire) ? dv : nullptr, X_list ? 0 : 1, st);
     if (!(v && fire)) launch_reset_fire(d, st);  // no velocities, or no FIRE state to go with them: a restart
     CK(cudaStreamSynchronize(st));  // dX / dv are reused below
-    if (!X_list) {
-        rc = force_rebuild_all(h);
-        if (rc) return rc;
-    }
     double *daux = dX;
     if (X_list) CK(cudaMemcpyAsync(daux, list_aux, (size_t)h->P * 4 * sizeof(double), cudaMemcpyHostToDevice, st));
     launch_import_aux(d, daux, X_list ? 1 : 0, fire ? 1 : 0, fire ? fire->dt : 0.0, fire ? fire->alpha : 0.0,
                       fire ? fire->n_pos : 0, fire ? (fire->first ? 1 : 0) : 1,
                       fire ? (unsigned long long)fire->steps : 0ull, st);
     // endpoint energies at the restored coordinates (their lists: replayed above, or fresh)
-    launch_cell_prep(d, X_list ? kEndpointsOnly : 0, MODE_STEP, st);
-    launch_neighbor_build(d, X_list ? kEndpointsOnly : 0, st);
+    launch_cell_prep(d, kEndpointsOnly, MODE_STEP, st);
+    launch_neighbor_build(d, kEndpointsOnly, st);
     launch_force(d, kEndpointsOnly, st);
     launch_finalize(d, kEndpointsOnly, st);
     h->interior_stale = true;

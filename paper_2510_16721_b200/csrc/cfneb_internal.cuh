@@ -216,7 +216,7 @@ void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_o
 void launch_export_path(const Dev &d, double *pos_out, double *cells_out, double *E_out, cudaStream_t st);
 void launch_export_state(const Dev &d, double *X_out, double *v_out, cudaStream_t st);
 void launch_export_list_state(const Dev &d, double *Xl_out, double *aux_out, cudaStream_t st);  // checkpoint
-void launch_import_state(const Dev &d, const double *X_in, const double *v_in, cudaStream_t st);
+void launch_import_state(const Dev &d, const double *X_in, const double *v_in, int track, cudaStream_t st);
 void launch_import_aux(const Dev &d, const double *aux_in, int have_aux, int have_fire, double dt, double alpha, int n_pos,
                        int first, unsigned long long steps, cudaStream_t st);
 void launch_export_forces(const Dev &d, double *F_out, double *V_out, double *E_out, cudaStream_t st);

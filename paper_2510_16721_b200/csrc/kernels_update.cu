@@ -274,17 +274,33 @@ __global__ void export_list_state_kernel(Dev d, double *Xo, double *aux) {
 }
 
 // Inverse of export_state_kernel: X (and v, if given) from the caller's layout into both coordinate buffers.
-__global__ void import_state_kernel(Dev d, const double *__restrict__ Xi, const double *__restrict__ vi) {
+// track: the largest atomic displacement of each image from the stored coordinates goes into the staleness bound of
+// its neighbour list (as cfneb_set_path does), so the lists are kept while the new state stays inside their skin.
+__global__ void import_state_kernel(Dev d, const double *__restrict__ Xi, const double *__restrict__ vi, int track) {
     const int p = blockIdx.y;
     const int P = d.ctl->P;
     if (p >= P) return;
     const int slot = d.order[p];
     const int rows = d.N + 3;
     const int a = blockIdx.x * blockDim.x + threadIdx.x;
-    if (a >= rows) return;
     const size_t img = (size_t)3 * d.Npad, buf = (size_t)d.S * img;
     const bool movable = p > 0 && p < P - 1;
     const int ai = a < d.N ? d.perm[a] : a;
+    if (track) {  // all threads of the block take part in the reduction
+        __shared__ double red[32];
+        double d2 = 0.0;
+        if (a < d.N) {
+            const double *Xold = d.X + (size_t)d.ctl->cur * buf + slot * img;
+            for (int c = 0; c < 3; ++c) {
+                const double dx = Xi[((size_t)p * rows + ai) * 3 + c] - Xold[(size_t)c * d.Npad + a];
+                d2 += dx * dx;
+            }
+            if (!(d2 == d2)) d2 = 1e300;
+        }
+        const double bm = block_max(d2, red);
+        if (threadIdx.x == 0) atomicMax(d.dispmax_in + slot, nonneg_bits(bm));
+    }
+    if (a >= rows) return;
     for (int c = 0; c < 3; ++c) {
         const double x = Xi[((size_t)p * rows + ai) * 3 + c];
         const double v = (vi && movable) ? vi[((size_t)p * rows + ai) * 3 + c] : 0.0;
@@ -374,9 +390,9 @@ void launch_export_list_state(const Dev &d, double *Xl_out, double *aux_out, cud
     export_list_state_kernel<<<grid, 128, 0, st>>>(d, Xl_out, aux_out);
 }
 
-void launch_import_state(const Dev &d, const double *X_in, const double *v_in, cudaStream_t st) {
+void launch_import_state(const Dev &d, const double *X_in, const double *v_in, int track, cudaStream_t st) {
     dim3 grid((d.N + 3 + 127) / 128, d.S);
-    import_state_kernel<<<grid, 128, 0, st>>>(d, X_in, v_in);
+    import_state_kernel<<<grid, 128, 0, st>>>(d, X_in, v_in, track);
 }
 
 void launch_import_aux(const Dev &d, const double *aux_in, int have_aux, int have_fire, double dt, double alpha, int n_pos,

@@ -35,11 +35,11 @@ def test_bench_line_has_the_contract_keys():
     assert c["kind"] == "oracle" and c["cores"] >= 1 and c["value"] > 0 and c["unit"] == d["unit"] and c["sample"]
     e = d["e2e"]
     assert e["unit"] == d["unit"] and 0 < e["value"] < d["value"]
-    ck = (3 * 16 * (2048 + 3) * 3 + 16 * 4) * 8 + 32          # X, v, X_list, list_aux, the FIRE scalars: a checkpoint each way
+    ck = 2 * 16 * (2048 + 3) * 3 * 8 + 32                      # X, v and the FIRE scalars each way
     assert e["h2d_bytes_per_step"] == ck and e["d2h_bytes_per_step"] == ck
     ss = d["steady_state"]
     assert ss["steps"] == 100 and ss["value"] > 0 and ss["unit"] == d["unit"] and "neighbor_rebuilds" in ss
-    assert d["gpu_launches"] == 12 * 20                       # twelve kernel nodes per captured iteration
+    assert d["gpu_launches"] == 13 * 20                       # thirteen kernel nodes per captured iteration
     assert set(("sm_mhz", "sm_max_mhz", "reasons")) <= set(d["clocks"])
 
 
