@@ -17,11 +17,12 @@
 //
 // Work split (round 1's descriptor kernel held all channels of an atom in one thread: 236 registers, 8 warps per
 // multiprocessor).  FOUR LANES PER ATOM: lane q of a quad owns the angular channels n = q, q + 4 and the radial
-// descriptors n = q, q + 4, and a quarter of the neurons.  All four walk the same list rows (their loads coalesce into
-// one request); each accumulates the 35 moments of ONE channel per walk in registers, parks them in a scratch array
-// (one 280-byte column per atom and channel), the quad exchanges descriptors and descriptor gradients by shuffles, and
-// a second walk per channel evaluates phi_n(u) = sum_c G_nc u^c and its gradient and sums the four lanes' partial
-// forces by two shuffle steps before one lane writes them.  Network weights and expansion coefficients sit in shared
+// a quarter of the neurons.  The list is walked four rows at a time, ONE ROW PER LANE: a lane forms the pair vector, the
+// two radial bases and the expansions g_n of its row once, then the rows go round the quad by shuffles and every lane
+// adds each row to the 35 moments of its own channel (registers); the moments are parked in a scratch array (one
+// 280-byte column per atom and channel), the quad exchanges descriptors and descriptor gradients by shuffles, and a
+// second walk of the same shape evaluates phi_n(u) = sum_c G_nc u^c and its gradient per channel and hands the three
+// components back to the row's lane, which writes them once.  Network weights and expansion coefficients sit in shared
 // memory.  No per-thread environment array, hence no limit on the atoms inside the cut-offs but the list capacity.
 #include "cfneb_internal.cuh"
 #include "nep_poly.cuh"
@@ -31,6 +32,9 @@ namespace cfn {
 
 constexpr int kNepMaxN = 8, kNepMaxK = 12, kNepMaxH = 64, kNepMaxL = 4;
 constexpr int kNepThreads = 128;  // 32 atoms x 4 lanes
+#ifndef CFNEB_NEP_BLOCKS
+#define CFNEB_NEP_BLOCKS 2
+#endif
 
 struct NepShape {
     int nr, na, kr, ka, L, H, T, D;
@@ -74,7 +78,10 @@ __device__ __forceinline__ void nep_basis(double t, double irc, int K, double (&
     }
 }
 
-__global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int p_lo) {
+// KMAX: basis functions held per row (the smallest of 4, 8, 12 that covers k_r and k_a): the loops over them are
+// unrolled so that the basis stays in registers.
+template <int KMAX>
+__global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
@@ -121,9 +128,21 @@ __global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int 
         return dx * dx + dy * dy + dz * dz;
     };
 
-    // ---- walk 1 (one per angular channel of this lane; the first also takes the radial descriptors) ----
-    double qR[2] = {0.0, 0.0};               // radial descriptors n = q, q + 4
-    double qA[2][kNepMaxL] = {};             // angular descriptors of the channels n = q, q + 4
+    const int base_lane = (threadIdx.x & 31) & ~3;
+    auto sel4 = [](const double (&a)[4], int c) { return c == 0 ? a[0] : c == 1 ? a[1] : c == 2 ? a[2] : a[3]; };
+    auto shf = [&](double v, int src) { return __shfl_sync(quad_mask, v, base_lane + src); };
+    auto quad_sum = [&](double v) {
+        v += __shfl_xor_sync(quad_mask, v, 1);
+        return v + __shfl_xor_sync(quad_mask, v, 2);
+    };
+
+    // ---- walk 1: the list is taken four rows at a time, ONE ROW PER LANE: the lane forms the pair vector, the radial
+    // basis and the expansions g_n of its row (nothing of that is done four times), then the rows go round the quad
+    // (step t: lane q takes the row of lane q + t) and each lane adds every row to the moments of its own channel ----
+    double qR[kNepMaxN];                      // radial descriptors: partial sums over this lane's rows, then all of them
+#pragma unroll
+    for (int n = 0; n < kNepMaxN; ++n) qR[n] = 0.0;
+    double qA[2][kNepMaxL] = {};              // angular descriptors of the channels n = q, q + 4
     const int npass = (sp.na + 3) / 4;
     for (int pass = 0; pass < npass; ++pass) {
         const int n = q + 4 * pass;
@@ -131,35 +150,61 @@ __global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int 
         double S[kNepC];
 #pragma unroll
         for (int c = 0; c < kNepC; ++c) S[c] = 0.0;
-        for (int k = 0; k < cnt; ++k) {
-            int J;
-            double dx, dy, dz;
-            const double r2 = pair_vec(k, J, dx, dy, dz);
-            if (!(r2 < rcr2)) continue;
-            const double inv = rsqrt(r2), r = r2 * inv;
-            if (pass == 0) {
-                double f[kNepMaxK], df[kNepMaxK];
-                nep_basis<kNepMaxK>(r * ircr, ircr, sp.kr, f, df);
+        for (int k0 = 0; k0 < cnt; k0 += 4) {
+            const int kk = k0 + q;
+            int J = 0;
+            double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1e300;
+            if (kk < cnt) r2 = pair_vec(kk, J, dx, dy, dz);
+            double x = 0.0, y = 0.0, z = 0.0, g4[4] = {0.0, 0.0, 0.0, 0.0};
+            if (r2 < rcr2) {
+                const double inv = rsqrt(r2), r = r2 * inv;
+                x = dx * inv; y = dy * inv; z = dz * inv;
+                if (pass == 0) {
+                    double f[KMAX], df[KMAX];
+                    nep_basis<KMAX>(r * ircr, ircr, sp.kr, f, df);
+                    const double *c = cRb + (size_t)J * sp.nr * sp.kr;
 #pragma unroll
-                for (int h2 = 0; h2 < 2; ++h2) {
-                    const int nn = q + 4 * h2;
-                    if (nn < sp.nr) {
-                        const double *c = cRb + ((size_t)J * sp.nr + nn) * sp.kr;
-                        double g = 0.0;
-                        for (int b = 0; b < sp.kr; ++b) g += c[b] * f[b];
-                        qR[h2] += g;
+                    for (int nn = 0; nn < kNepMaxN; ++nn)
+                        if (nn < sp.nr) {
+                            double g = 0.0;
+#pragma unroll
+                            for (int b = 0; b < KMAX; ++b)
+                                if (b < sp.kr) g += c[nn * sp.kr + b] * f[b];
+                            qR[nn] += g;
+                        }
+                }
+                if (r2 < rca2) {
+                    double f[KMAX], df[KMAX];
+                    nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
+#pragma unroll
+                    for (int c4 = 0; c4 < 4; ++c4) {
+                        const int nn = 4 * pass + c4;
+                        if (nn < sp.na) {
+                            const double *c = cAb + ((size_t)J * sp.na + nn) * sp.ka;
+                            double g = 0.0;
+#pragma unroll
+                            for (int b = 0; b < KMAX; ++b)
+                                if (b < sp.ka) g += c[b] * f[b];
+                            g4[c4] = g;
+                        }
                     }
                 }
             }
-            if (own && r2 < rca2) {
-                double f[kNepMaxK], df[kNepMaxK], m[kNepC];
-                nep_basis<kNepMaxK>(r * irca, irca, sp.ka, f, df);
-                const double *c = cAb + ((size_t)J * sp.na + n) * sp.ka;
-                double g = 0.0;
-                for (int b = 0; b < sp.ka; ++b) g += c[b] * f[b];
-                nep_monomials(dx * inv, dy * inv, dz * inv, m);
+            const double inA = r2 < rca2 ? 1.0 : 0.0;
 #pragma unroll
-                for (int cc = 0; cc < kNepC; ++cc) S[cc] += g * m[cc];
+            for (int t = 0; t < 4; ++t) {
+                const int src = (q + t) & 3;
+                // the value lane src wants from this lane in step t is the g of ITS channel: lane src = q + t reads q's
+                // register, so q presents g4[(q - t) & 3]... seen from the reader: it reads g4[own channel] of lane src
+                const double gs = t == 0 ? sel4(g4, q) : shf(sel4(g4, (q - t) & 3), src);
+                const double xs = t == 0 ? x : shf(x, src), ys = t == 0 ? y : shf(y, src), zs = t == 0 ? z : shf(z, src);
+                const double as = t == 0 ? inA : shf(inA, src);
+                if (own && as != 0.0) {
+                    double m[kNepC];
+                    nep_monomials(xs, ys, zs, m);
+#pragma unroll
+                    for (int cc = 0; cc < kNepC; ++cc) S[cc] += gs * m[cc];
+                }
             }
         }
         if (own && valid) {
@@ -176,36 +221,40 @@ __global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int 
             qA[pass][3] = 0.125 * (35.0 * A[4] - 30.0 * A[2] + 3.0 * A[0]);
         }
     }
+#pragma unroll
+    for (int n = 0; n < kNepMaxN; ++n) qR[n] = quad_sum(qR[n]);  // every lane now holds all radial descriptors
 
-    // ---- the network: every lane needs all descriptors; each takes the neurons mu = q, q + 4, ... ----
-    // descriptor d lives in lane (d mod 4 for radial n = d; angular channel n -> lane n mod 4): gather by quad shuffles
+    // ---- the network: each lane takes the neurons mu = q, q + 4, ...; the angular descriptors come from their owners ----
     double ui = 0.0;
-    double FdR[2] = {0.0, 0.0}, FdA[2][kNepMaxL] = {};
+    double FdR[kNepMaxN], FdA[2][kNepMaxL] = {};
+#pragma unroll
+    for (int n = 0; n < kNepMaxN; ++n) FdR[n] = 0.0;
     {
-        double z[kNepMaxH / 4];
+        double zt[kNepMaxH / 4];
 #pragma unroll
         for (int t = 0; t < kNepMaxH / 4; ++t) {
             const int mu = q + 4 * t;
-            z[t] = mu < sp.H ? -b0[mu] : 0.0;
+            zt[t] = mu < sp.H ? -b0[mu] : 0.0;
         }
-        const int base_lane = (threadIdx.x & 31) & ~3;
         for (int dsc = 0; dsc < sp.D; ++dsc) {
-            // owner lane and register of descriptor dsc
-            int ol, hh, ll = 0;
-            bool radial = dsc < sp.nr;
-            if (radial) { ol = dsc & 3; hh = dsc >> 2; }
-            else { const int n = (dsc - sp.nr) / sp.L; ll = (dsc - sp.nr) % sp.L; ol = n & 3; hh = n >> 2; }
-            double mine = radial ? (hh ? qR[1] : qR[0]) : (hh ? qA[1][0] : qA[0][0]);
-            if (!radial) {
+            double v;
+            if (dsc < sp.nr) {
+                v = 0.0;
+#pragma unroll
+                for (int n = 0; n < kNepMaxN; ++n)
+                    if (n == dsc) v = qR[n];
+            } else {
+                const int n = (dsc - sp.nr) / sp.L, ll = (dsc - sp.nr) % sp.L, hh = n >> 2;
+                double mine = hh ? qA[1][0] : qA[0][0];
                 if (ll == 1) mine = hh ? qA[1][1] : qA[0][1];
                 if (ll == 2) mine = hh ? qA[1][2] : qA[0][2];
                 if (ll == 3) mine = hh ? qA[1][3] : qA[0][3];
+                v = shf(mine, n & 3);
             }
-            const double v = __shfl_sync(quad_mask, mine, base_lane + ol);
 #pragma unroll
             for (int t = 0; t < kNepMaxH / 4; ++t) {
                 const int mu = q + 4 * t;
-                if (mu < sp.H) z[t] += W0[mu * sp.D + dsc] * v;
+                if (mu < sp.H) zt[t] += W0[mu * sp.D + dsc] * v;
             }
         }
         double gmu[kNepMaxH / 4];
@@ -214,12 +263,12 @@ __global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int 
             const int mu = q + 4 * t;
             gmu[t] = 0.0;
             if (mu < sp.H) {
-                const double th = tanh(z[t]);
+                const double th = tanh(zt[t]);
                 ui += W1[mu] * th;
                 gmu[t] = W1[mu] * (1.0 - th * th);
             }
         }
-        // dU/dq_d = sum_mu gmu W0[mu][d]: partial over this lane's neurons, summed over the quad, kept by the owner
+        // dU/dq_d = sum_mu gmu W0[mu][d]: partial over this lane's neurons, summed over the quad
         for (int dsc = 0; dsc < sp.D; ++dsc) {
             double v = 0.0;
 #pragma unroll
@@ -227,10 +276,11 @@ __global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int 
                 const int mu = q + 4 * t;
                 if (mu < sp.H) v += gmu[t] * W0[mu * sp.D + dsc];
             }
-            v += __shfl_xor_sync(quad_mask, v, 1);
-            v += __shfl_xor_sync(quad_mask, v, 2);
+            v = quad_sum(v);
             if (dsc < sp.nr) {
-                if ((dsc & 3) == q) { if (dsc >> 2) FdR[1] = v; else FdR[0] = v; }
+#pragma unroll
+                for (int n = 0; n < kNepMaxN; ++n)
+                    if (n == dsc) FdR[n] = v;  // all lanes keep the radial ones
             } else {
                 const int n = (dsc - sp.nr) / sp.L, ll = (dsc - sp.nr) % sp.L;
                 if ((n & 3) == q) {
@@ -240,12 +290,13 @@ __global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int 
                 }
             }
         }
-        ui += __shfl_xor_sync(quad_mask, ui, 1);
-        ui += __shfl_xor_sync(quad_mask, ui, 2);
+        ui = quad_sum(ui);
         if (q != 0 || !valid) ui = 0.0;  // one lane per atom carries the site energy
     }
 
-    // ---- walk 2 (one per pass): partial forces.  Lane sums of the quad are combined per list row ----
+    // ---- walk 2 (one per pass), again one row per lane: the lane prepares its row (pair vector, bases, g_n and g_n'
+    // of the pass's four channels, the radial part of the partial force), the rows go round the quad, every lane
+    // evaluates ITS channel's polynomial for each row and hands the three components back to the row's lane ----
     for (int pass = 0; pass < npass; ++pass) {
         const int n = q + 4 * pass;
         const bool own = n < sp.na;
@@ -260,61 +311,88 @@ __global__ void __launch_bounds__(kNepThreads, 3) nep_partial_kernel(Dev d, int 
                 G[cc] = (own && valid) ? 2.0 * cf[l] * kNepMult[cc] * scr[(size_t)(n * kNepC + cc) * d.Npad] : 0.0;
             }
         }
-        for (int k = 0; k < cnt; ++k) {
-            int J;
-            double dx, dy, dz;
-            const double r2 = pair_vec(k, J, dx, dy, dz);
+        for (int k0 = 0; k0 < cnt; k0 += 4) {
+            const int kk = k0 + q;
+            int J = 0;
+            double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1e300;
+            if (kk < cnt) r2 = pair_vec(kk, J, dx, dy, dz);
+            double x = 0.0, y = 0.0, z = 0.0, inv = 0.0, g4[4] = {0.0, 0.0, 0.0, 0.0}, dg4[4] = {0.0, 0.0, 0.0, 0.0};
             double px = 0.0, py = 0.0, pz = 0.0;
             if (r2 < rcr2) {
-                const double inv = rsqrt(r2), r = r2 * inv;
-                const double x = dx * inv, y = dy * inv, z = dz * inv;
+                inv = rsqrt(r2);
+                const double r = r2 * inv;
+                x = dx * inv; y = dy * inv; z = dz * inv;
                 if (pass == 0) {  // radial descriptors: sum_n Fd_n g'_n(r) u
-                    double f[kNepMaxK], df[kNepMaxK];
-                    nep_basis<kNepMaxK>(r * ircr, ircr, sp.kr, f, df);
-                    double s = 0.0;
+                    double f[KMAX], df[KMAX];
+                    nep_basis<KMAX>(r * ircr, ircr, sp.kr, f, df);
+                    const double *c = cRb + (size_t)J * sp.nr * sp.kr;
+                    double sr = 0.0;
 #pragma unroll
-                    for (int h2 = 0; h2 < 2; ++h2) {
-                        const int nn = q + 4 * h2;
+                    for (int nn = 0; nn < kNepMaxN; ++nn)
                         if (nn < sp.nr) {
-                            const double *c = cRb + ((size_t)J * sp.nr + nn) * sp.kr;
                             double dg = 0.0;
-                            for (int b = 0; b < sp.kr; ++b) dg += c[b] * df[b];
-                            s += (h2 ? FdR[1] : FdR[0]) * dg;
+#pragma unroll
+                            for (int b = 0; b < KMAX; ++b)
+                                if (b < sp.kr) dg += c[nn * sp.kr + b] * df[b];
+                            sr += FdR[nn] * dg;
+                        }
+                    px = sr * x; py = sr * y; pz = sr * z;
+                }
+                if (r2 < rca2) {
+                    double f[KMAX], df[KMAX];
+                    nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
+#pragma unroll
+                    for (int c4 = 0; c4 < 4; ++c4) {
+                        const int nn = 4 * pass + c4;
+                        if (nn < sp.na) {
+                            const double *c = cAb + ((size_t)J * sp.na + nn) * sp.ka;
+                            double g = 0.0, dg = 0.0;
+#pragma unroll
+                            for (int b = 0; b < KMAX; ++b)
+                                if (b < sp.ka) { g += c[b] * f[b]; dg += c[b] * df[b]; }
+                            g4[c4] = g;
+                            dg4[c4] = dg;
                         }
                     }
-                    px = s * x; py = s * y; pz = s * z;
                 }
-                if (own && r2 < rca2) {
-                    double f[kNepMaxK], df[kNepMaxK], m[kNepC];
-                    nep_basis<kNepMaxK>(r * irca, irca, sp.ka, f, df);
-                    const double *c = cAb + ((size_t)J * sp.na + n) * sp.ka;
-                    double g = 0.0, dg = 0.0;
-                    for (int b = 0; b < sp.ka; ++b) { g += c[b] * f[b]; dg += c[b] * df[b]; }
-                    nep_monomials(x, y, z, m);  // only the monomials of degree <= 3 are read below
+            }
+            const double inA = r2 < rca2 ? 1.0 : 0.0;
+#pragma unroll
+            for (int t = 0; t < 4; ++t) {
+                const int src = (q + t) & 3;
+                const double gs = t == 0 ? sel4(g4, q) : shf(sel4(g4, (q - t) & 3), src);
+                const double dgs = t == 0 ? sel4(dg4, q) : shf(sel4(dg4, (q - t) & 3), src);
+                const double xs = t == 0 ? x : shf(x, src), ys = t == 0 ? y : shf(y, src), zs = t == 0 ? z : shf(z, src);
+                const double is = t == 0 ? inv : shf(inv, src), as = t == 0 ? inA : shf(inA, src);
+                double cx = 0.0, cy = 0.0, cz = 0.0;
+                if (own && as != 0.0) {
+                    double m[kNepC];
+                    nep_monomials(xs, ys, zs, m);  // only the monomials of degree <= 3 are read below
                     double gl[4][3];
                     nep_poly_grad(G, m, gl);
                     double phi = G[0], ug = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
 #pragma unroll
                     for (int l = 0; l < 4; ++l) {  // u . grad phi_l = l phi_l (Euler)
-                        const double t = x * gl[l][0] + y * gl[l][1] + z * gl[l][2];
-                        ug += t;
-                        phi += t * (1.0 / (l + 1));
+                        const double tt = xs * gl[l][0] + ys * gl[l][1] + zs * gl[l][2];
+                        ug += tt;
+                        phi += tt * (1.0 / (l + 1));
                         gx += gl[l][0]; gy += gl[l][1]; gz += gl[l][2];
                     }
-                    const double gi = g * inv, dphi = dg * phi;
-                    px += dphi * x + gi * (gx - ug * x);
-                    py += dphi * y + gi * (gy - ug * y);
-                    pz += dphi * z + gi * (gz - ug * z);
+                    const double gi = gs * is, dphi = dgs * phi;
+                    cx = dphi * xs + gi * (gx - ug * xs);
+                    cy = dphi * ys + gi * (gy - ug * ys);
+                    cz = dphi * zs + gi * (gz - ug * zs);
                 }
+                // back to the row's lane: in step t this lane's row was evaluated by lane q - t
+                const int ev = (q - t) & 3;
+                px += t == 0 ? cx : shf(cx, ev);
+                py += t == 0 ? cy : shf(cy, ev);
+                pz += t == 0 ? cz : shf(cz, ev);
             }
-            // the quad's four contributions; lane m < 3 then owns component m
-            px += __shfl_xor_sync(quad_mask, px, 1); px += __shfl_xor_sync(quad_mask, px, 2);
-            py += __shfl_xor_sync(quad_mask, py, 1); py += __shfl_xor_sync(quad_mask, py, 2);
-            pz += __shfl_xor_sync(quad_mask, pz, 1); pz += __shfl_xor_sync(quad_mask, pz, 2);
-            if (q < 3) {
-                double *o = part + (size_t)(k * 3 + q) * d.Npad;
-                const double v = q == 0 ? px : q == 1 ? py : pz;
-                *o = pass ? *o + v : v;
+            if (kk < cnt) {
+                double *o = part + (size_t)(kk * 3) * d.Npad;
+                if (pass) { px += o[0]; py += o[d.Npad]; pz += o[2 * (size_t)d.Npad]; }
+                o[0] = px; o[d.Npad] = py; o[2 * (size_t)d.Npad] = pz;
             }
         }
     }
@@ -358,10 +436,15 @@ void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st) {
     const size_t smem = (size_t)nep_weight_count(d.pot) * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
-        cudaFuncSetAttribute(nep_partial_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        cudaFuncSetAttribute(nep_partial_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        cudaFuncSetAttribute(nep_partial_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+        cudaFuncSetAttribute(nep_partial_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
         attr_set = true;
     }
-    nep_partial_kernel<<<grid, kNepThreads, smem, st>>>(d, p_lo);
+    const int kmax = (int)(d.pot[4] > d.pot[5] ? d.pot[4] : d.pot[5]);
+    if (kmax <= 4) nep_partial_kernel<4><<<grid, kNepThreads, smem, st>>>(d, p_lo);
+    else if (kmax <= 8) nep_partial_kernel<8><<<grid, kNepThreads, smem, st>>>(d, p_lo);
+    else nep_partial_kernel<12><<<grid, kNepThreads, smem, st>>>(d, p_lo);
     launch_pair_forces_manybody(d, p_lo, st);
 }
 
