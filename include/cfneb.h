@@ -165,8 +165,8 @@ enum {
 CFNEB_API void cfneb_default_params(cfneb_params *prm);
 
 /* Bytes of device workspace cfneb_create needs for n_atoms atoms and prm->max_images images
- * (0 on invalid arguments).  c4 (101306 atoms x 100 images, list capacity 224): 23.6 GB, of which 9.1 GB are the
- * neighbour lists and 11.4 GB the scratch of a rebuild of all images at once. */
+ * (0 on invalid arguments).  c4 (101306 atoms x 100 images, list capacity 224): 12.4 GB, of which 9.1 GB are the
+ * neighbour lists. */
 CFNEB_API size_t cfneb_workspace_bytes(int32_t n_atoms, const cfneb_params *prm);
 
 /*

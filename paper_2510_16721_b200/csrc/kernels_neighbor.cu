@@ -60,24 +60,25 @@ __global__ void __launch_bounds__(1024) bin_scan_kernel(Dev d, int p_lo) {
     }
 }
 
-__global__ void __launch_bounds__(kThreadsAtom) bin_fill_kernel(Dev d, int p_lo) {
-    int slot;
-    if (!image_active(d, p_lo, blockIdx.y, slot)) return;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= d.N) return;
-    const int bin = d.atom_bin[(size_t)slot * d.Npad + i];
-    const int pos = atomicAdd(d.bin_cursor + (size_t)slot * d.nbins_max + bin, 1);
-    d.bin_members[(size_t)slot * d.Npad + pos] = i;
+// (bin_fill and bin_sort run on grids of fixed size over the compact list of rebuilding images, like the search.)
+__global__ void __launch_bounds__(kThreadsAtom) bin_fill_kernel(Dev d) {
+    const long long total = (long long)d.ctl->n_rebuild * d.N;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const int slot = d.rebuild_slots[t / d.N], i = (int)(t % d.N);
+        const int bin = d.atom_bin[(size_t)slot * d.Npad + i];
+        const int pos = atomicAdd(d.bin_cursor + (size_t)slot * d.nbins_max + bin, 1);
+        d.bin_members[(size_t)slot * d.Npad + pos] = i;
+    }
 }
 
 // One thread per bin: sort the members by atom index, then write the bin-ordered coordinate array.
-__global__ void __launch_bounds__(128) bin_sort_kernel(Dev d, int p_lo) {
-    int slot;
-    if (!image_active(d, p_lo, blockIdx.y, slot)) return;
+__global__ void __launch_bounds__(128) bin_sort_kernel(Dev d) {
+    const long long total = (long long)d.ctl->n_rebuild * d.nbins_max;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+    const int slot = d.rebuild_slots[t / d.nbins_max], b = (int)(t % d.nbins_max);
     const Geom *g = d.geom + slot;
     const int nbins = g->nb[0] * g->nb[1] * g->nb[2];
-    const int b = blockIdx.x * blockDim.x + threadIdx.x;
-    if (b >= nbins) return;
+    if (b >= nbins) continue;
     const int *bc = d.bin_count + (size_t)slot * (d.nbins_max + 1);
     int *mem = d.bin_members + (size_t)slot * d.Npad;
     const int lo = bc[b], hi = bc[b + 1];
@@ -100,6 +101,7 @@ __global__ void __launch_bounds__(128) bin_sort_kernel(Dev d, int p_lo) {
                               (float)(w.x * g->h[1] + w.y * g->h[4] + w.z * g->h[7]),
                               (float)(w.x * g->h[2] + w.y * g->h[5] + w.z * g->h[8]), 0.f);
     }
+    }  // work items
 }
 
 __device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
@@ -126,18 +128,36 @@ __device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
 // entry (the atom itself shifted by -4 cell vectors along axis 0: farther than r_list whenever a list can be
 // built at all), so the force kernels read any row below cap without a bounds test and find it out of range.
 // Compact list of the images (slots) of the selected set whose list is rebuilt this step, in path order.
-__global__ void rebuild_list_kernel(Dev d, int p_lo) {
-    if (threadIdx.x != 0 || blockIdx.x != 0) return;
+__global__ void __launch_bounds__(256) rebuild_list_kernel(Dev d, int p_lo) {
     const int P = d.ctl->P;
     const int ny = p_lo == kEndpointsOnly ? 2 : d.S - 2 * p_lo;
-    int n = 0;
-    for (int y = 0; y < ny; ++y) {
-        int p;
-        if (!image_of(y, p_lo, P, p)) continue;
-        const int slot = d.order[p];
-        if (d.geom[slot].rebuild) d.rebuild_slots[n++] = slot;
+    __shared__ int s_warp[8], s_base;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) s_base = 0;
+    __syncthreads();
+    for (int y0 = 0; y0 < ny; y0 += 256) {  // 256 images per round, compacted in path order
+        const int y = y0 + threadIdx.x;
+        int p, slot = -1;
+        bool on = false;
+        if (y < ny && image_of(y, p_lo, P, p)) {
+            slot = d.order[p];
+            on = d.geom[slot].rebuild != 0;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, on);
+        if (lane == 0) s_warp[warp] = __popc(m);
+        __syncthreads();
+        int off = s_base;
+        for (int w = 0; w < warp; ++w) off += s_warp[w];
+        if (on) d.rebuild_slots[off + __popc(m & ((1u << lane) - 1u))] = slot;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            int t = 0;
+            for (int w = 0; w < 8; ++w) t += s_warp[w];
+            s_base += t;
+        }
+        __syncthreads();
     }
-    d.ctl->n_rebuild = n;
+    if (threadIdx.x == 0) d.ctl->n_rebuild = s_base;
 }
 
 constexpr int kRadialBuckets = kInnerBuckets + kTailBuckets;
@@ -152,8 +172,9 @@ constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 // Round 2: the grid has a fixed size (CFNEB_SEARCH_BLOCKS blocks per multiprocessor) and takes its work items
 // (rebuilding image, block of 128 atoms) from the compact list of rebuild_list_kernel -- a step in which no list is
 // stale costs one exit per resident block instead of 77 616 -- and the unsorted column / bucket scratch of a block
-// is a region of its own, reused item after item (scr_tmp, scr_bkt: 143 KB per block, L2 resident), instead of two
-// arrays of the size of the list itself (round 1: 11.4 GB of workspace, 2.8 x the list in DRAM writes per rebuild).
+// is a region of its own, reused item after item (scr_tmp, scr_bkt: 143 KB per block), instead of two arrays of the
+// size of the list itself (round 1: 11.4 GB of workspace; DRAM writes per rebuild 2.8 -> 2.3 x the list: the 106 MB of
+// scratch of the resident blocks only partly stay in the L2).
 __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_search_kernel(Dev d) {
     __shared__ unsigned short s_hist[kRadialBuckets * kThreadsAtom];
     __shared__ uint32_t s_queue[kQueue * kThreadsAtom];
@@ -358,12 +379,10 @@ __global__ void unpack_neighbors_kernel(Dev d, int slot, int *count_out, int *li
 void launch_neighbor_build(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
-    rebuild_list_kernel<<<1, 32, 0, st>>>(d, p_lo);
+    rebuild_list_kernel<<<1, 256, 0, st>>>(d, p_lo);
     bin_scan_kernel<<<nimg, 1024, 0, st>>>(d, p_lo);
-    dim3 ga(d.nblk_atom, nimg);
-    bin_fill_kernel<<<ga, kThreadsAtom, 0, st>>>(d, p_lo);
-    dim3 gb((d.nbins_max + 127) / 128, nimg);
-    bin_sort_kernel<<<gb, 128, 0, st>>>(d, p_lo);
+    bin_fill_kernel<<<d.n_sm * 8, kThreadsAtom, 0, st>>>(d);
+    bin_sort_kernel<<<d.n_sm * 8, 128, 0, st>>>(d);
     neighbor_search_kernel<<<d.n_search_blocks, kThreadsAtom, 0, st>>>(d);
     if (d.potential == CFNEB_POT_SW || d.potential == CFNEB_POT_DNN || d.potential == CFNEB_POT_NEP) launch_mirror_sw(d, p_lo, st);
 }
