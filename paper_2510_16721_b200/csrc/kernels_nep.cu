@@ -89,34 +89,59 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     __shared__ double sh[9];
     __shared__ double red[64];
     const NepShape sp = nep_shape(d.pot);
-    const int nW = nep_weights_size(sp);
+    const int nNet = sp.T * nep_net_size(sp);
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
-    for (int t = threadIdx.x; t < nW; t += blockDim.x) sW[t] = d.dn_w[t];
+    for (int t = threadIdx.x; t < nNet; t += blockDim.x) sW[t] = d.dn_w[t];
+    // expansion coefficients zero-padded to [T][T][8][KMAX] (radial, then angular): the loops over channels and basis
+    // functions then run to their compile-time bounds with no guards, and a row of coefficients is KMAX aligned doubles
+    double *cRp = sW + ((nNet + 1) & ~1), *cAp = cRp + sp.T * sp.T * kNepMaxN * KMAX;
+    for (int t = threadIdx.x; t < sp.T * sp.T * kNepMaxN * KMAX; t += blockDim.x) {
+        const int b = t % KMAX, nn = (t / KMAX) % kNepMaxN, IJ = t / (KMAX * kNepMaxN);
+        cRp[t] = (nn < sp.nr && b < sp.kr) ? d.dn_w[nNet + (IJ * sp.nr + nn) * sp.kr + b] : 0.0;
+        cAp[t] = (nn < sp.na && b < sp.ka) ? d.dn_w[nNet + sp.T * sp.T * sp.nr * sp.kr + (IJ * sp.na + nn) * sp.ka + b] : 0.0;
+    }
     __syncthreads();
     const int q = threadIdx.x & 3;                                     // lane of the quad
     const int i = blockIdx.x * (kNepThreads / 4) + (threadIdx.x >> 2);  // atom of the quad
     const bool valid = i < d.N;
     const int ic = valid ? i : 0;
-    const unsigned quad_mask = 0xFu << ((threadIdx.x & 31) & ~3);  // the quad's lanes: its shuffles run inside loops whose
-                                                                   // trip count (the atom's list length) differs between quads
+    const unsigned quad_mask = 0xffffffffu;  // see cnt_w below
     const double rcr = d.pot[0], rca = d.pot[1], rcr2 = rcr * rcr, rca2 = rca * rca, ircr = 1.0 / rcr, irca = 1.0 / rca;
     const int I = d.types[ic];
     const double *net = sW + I * nep_net_size(sp);
     const double *W0 = net, *b0 = net + sp.H * sp.D, *W1 = b0 + sp.H;
-    const double *cRb = sW + sp.T * nep_net_size(sp) + (size_t)I * sp.T * sp.nr * sp.kr;   // [J][n][k]
-    const double *cAb = sW + sp.T * nep_net_size(sp) + sp.T * sp.T * sp.nr * sp.kr + (size_t)I * sp.T * sp.na * sp.ka;
+    const double *cRb = cRp + (size_t)I * sp.T * kNepMaxN * KMAX;   // [J][n][k], padded
+    const double *cAb = cAp + (size_t)I * sp.T * kNepMaxN * KMAX;
     const double4 *Rc = d.Rc + (size_t)slot * d.Npad;
     const uint32_t *lp = d.nbr_list + (size_t)slot * d.cap * d.Npad + ic;
     double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + ic;  // part[(k * 3 + m) * Npad]
     double *scr = d.nep_S + ((size_t)slot * sp.na * kNepC) * d.Npad + ic;  // scr[(n * kNepC + c) * Npad]
     const double4 ri = Rc[ic];
     const int cnt = valid ? live_rows(d, slot, ic) : 0;  // rows past it cannot be in range
+    // every loop over list rows runs to the longest list of the warp (rows past a quad's own count are skipped by
+    // `kk < cnt`): all 32 lanes reach every shuffle, so the shuffles take the full mask
+    const int cnt_w = __reduce_max_sync(0xffffffffu, cnt);
 
-    auto pair_vec = [&](int k, int &J, double &dx, double &dy, double &dz) {
-        const uint32_t e = lp[(size_t)k * d.Npad];
-        const uint32_t j = e & kIdxMask, code = e >> kShiftBits;
-        const double4 rj = Rc[j];
-        J = d.types[j];
+    // The rows of a lane (kk = q, q + 4, ...) are software-pipelined: the list entry two rows ahead and the neighbour's
+    // sector and type one row ahead are in flight while a row is evaluated (two resident warps per scheduler cannot
+    // hide the two dependent loads otherwise).  Rows past the end stand in with the atom itself and are never used.
+    uint32_t e_nn, e_n;
+    double4 rj_n;
+    int J_n;
+    auto walk_begin = [&]() {
+        e_n = q < cnt ? lp[(size_t)q * d.Npad] : (uint32_t)ic | (kCodeCenter << kShiftBits);
+        e_nn = q + 4 < cnt ? lp[(size_t)(q + 4) * d.Npad] : e_n;
+        rj_n = Rc[e_n & kIdxMask];
+        J_n = d.types[e_n & kIdxMask];
+    };
+    auto pair_vec = [&](int k, int &J, double &dx, double &dy, double &dz) {  // row k of this lane; advances the pipeline
+        const uint32_t code = e_n >> kShiftBits;
+        const double4 rj = rj_n;
+        J = J_n;
+        e_n = e_nn;
+        e_nn = k + 8 < cnt ? lp[(size_t)(k + 8) * d.Npad] : e_n;
+        rj_n = Rc[e_n & kIdxMask];
+        J_n = d.types[e_n & kIdxMask];
         dx = rj.x - ri.x; dy = rj.y - ri.y; dz = rj.z - ri.z;
         if (code != kCodeCenter) {
             const double n0 = (double)((int)(code & 7u) - 4), n1 = (double)((int)((code >> 3) & 7u) - 4),
@@ -150,7 +175,8 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
         double S[kNepC];
 #pragma unroll
         for (int c = 0; c < kNepC; ++c) S[c] = 0.0;
-        for (int k0 = 0; k0 < cnt; k0 += 4) {
+        walk_begin();
+        for (int k0 = 0; k0 < cnt_w; k0 += 4) {
             const int kk = k0 + q;
             int J = 0;
             double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1e300;
@@ -162,31 +188,25 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
                 if (pass == 0) {
                     double f[KMAX], df[KMAX];
                     nep_basis<KMAX>(r * ircr, ircr, sp.kr, f, df);
-                    const double *c = cRb + (size_t)J * sp.nr * sp.kr;
+                    const double *c = cRb + (size_t)J * kNepMaxN * KMAX;
 #pragma unroll
-                    for (int nn = 0; nn < kNepMaxN; ++nn)
-                        if (nn < sp.nr) {
-                            double g = 0.0;
+                    for (int nn = 0; nn < kNepMaxN; ++nn) {
+                        double g = 0.0;
 #pragma unroll
-                            for (int b = 0; b < KMAX; ++b)
-                                if (b < sp.kr) g += c[nn * sp.kr + b] * f[b];
-                            qR[nn] += g;
-                        }
+                        for (int b = 0; b < KMAX; ++b) g += c[nn * KMAX + b] * f[b];
+                        qR[nn] += g;
+                    }
                 }
                 if (r2 < rca2) {
                     double f[KMAX], df[KMAX];
                     nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
 #pragma unroll
                     for (int c4 = 0; c4 < 4; ++c4) {
-                        const int nn = 4 * pass + c4;
-                        if (nn < sp.na) {
-                            const double *c = cAb + ((size_t)J * sp.na + nn) * sp.ka;
-                            double g = 0.0;
+                        const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
+                        double g = 0.0;
 #pragma unroll
-                            for (int b = 0; b < KMAX; ++b)
-                                if (b < sp.ka) g += c[b] * f[b];
-                            g4[c4] = g;
-                        }
+                        for (int b = 0; b < KMAX; ++b) g += c[b] * f[b];
+                        g4[c4] = g;
                     }
                 }
             }
@@ -311,7 +331,8 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
                 G[cc] = (own && valid) ? 2.0 * cf[l] * kNepMult[cc] * scr[(size_t)(n * kNepC + cc) * d.Npad] : 0.0;
             }
         }
-        for (int k0 = 0; k0 < cnt; k0 += 4) {
+        walk_begin();
+        for (int k0 = 0; k0 < cnt_w; k0 += 4) {
             const int kk = k0 + q;
             int J = 0;
             double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1e300;
@@ -325,17 +346,15 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
                 if (pass == 0) {  // radial descriptors: sum_n Fd_n g'_n(r) u
                     double f[KMAX], df[KMAX];
                     nep_basis<KMAX>(r * ircr, ircr, sp.kr, f, df);
-                    const double *c = cRb + (size_t)J * sp.nr * sp.kr;
+                    const double *c = cRb + (size_t)J * kNepMaxN * KMAX;
                     double sr = 0.0;
 #pragma unroll
-                    for (int nn = 0; nn < kNepMaxN; ++nn)
-                        if (nn < sp.nr) {
-                            double dg = 0.0;
+                    for (int nn = 0; nn < kNepMaxN; ++nn) {
+                        double dg = 0.0;
 #pragma unroll
-                            for (int b = 0; b < KMAX; ++b)
-                                if (b < sp.kr) dg += c[nn * sp.kr + b] * df[b];
-                            sr += FdR[nn] * dg;
-                        }
+                        for (int b = 0; b < KMAX; ++b) dg += c[nn * KMAX + b] * df[b];
+                        sr += FdR[nn] * dg;
+                    }
                     px = sr * x; py = sr * y; pz = sr * z;
                 }
                 if (r2 < rca2) {
@@ -343,16 +362,12 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
                     nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
 #pragma unroll
                     for (int c4 = 0; c4 < 4; ++c4) {
-                        const int nn = 4 * pass + c4;
-                        if (nn < sp.na) {
-                            const double *c = cAb + ((size_t)J * sp.na + nn) * sp.ka;
-                            double g = 0.0, dg = 0.0;
+                        const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
+                        double g = 0.0, dg = 0.0;
 #pragma unroll
-                            for (int b = 0; b < KMAX; ++b)
-                                if (b < sp.ka) { g += c[b] * f[b]; dg += c[b] * df[b]; }
-                            g4[c4] = g;
-                            dg4[c4] = dg;
-                        }
+                        for (int b = 0; b < KMAX; ++b) { g += c[b] * f[b]; dg += c[b] * df[b]; }
+                        g4[c4] = g;
+                        dg4[c4] = dg;
                     }
                 }
             }
@@ -433,7 +448,9 @@ void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_force, nimg);
-    const size_t smem = (size_t)nep_weight_count(d.pot) * sizeof(double);
+    const NepShape sp = nep_shape(d.pot);
+    const int kmax = (int)(d.pot[4] > d.pot[5] ? d.pot[4] : d.pot[5]), KM = kmax <= 4 ? 4 : kmax <= 8 ? 8 : 12;
+    const size_t smem = ((size_t)((sp.T * nep_net_size(sp) + 1) & ~1) + 2 * (size_t)sp.T * sp.T * kNepMaxN * KM) * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(nep_partial_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
@@ -441,7 +458,6 @@ void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st) {
         cudaFuncSetAttribute(nep_partial_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
         attr_set = true;
     }
-    const int kmax = (int)(d.pot[4] > d.pot[5] ? d.pot[4] : d.pot[5]);
     if (kmax <= 4) nep_partial_kernel<4><<<grid, kNepThreads, smem, st>>>(d, p_lo);
     else if (kmax <= 8) nep_partial_kernel<8><<<grid, kNepThreads, smem, st>>>(d, p_lo);
     else nep_partial_kernel<12><<<grid, kNepThreads, smem, st>>>(d, p_lo);
