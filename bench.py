@@ -18,8 +18,8 @@ images of the band.  metric = atom x image x NEB-steps per second, counted over 
              between neighbour-list rebuilds (an image rebuilds its list only when it left its skin: ~0.8 image
              rebuilds per step at configs[4]); `value` stays the K-step figure the contract asks for.
   e2e        the same metric through the C ABI with HOST (pinned) buffers, as a true continuation of the band:
-             every step restores the checkpoint from host memory (cfneb_set_state: X, v, FIRE state, list state),
-             runs one iteration (cfneb_step) and writes the checkpoint back (cfneb_get_checkpoint).
+             every step is one cfneb_step_hosted call: X, v and the FIRE scalars host -> device (image blocks on a
+             second stream, evaluated while later blocks arrive), one iteration, X, v and the scalars back.
   cpu_baseline  the oracle as it stands, on this box's host cores, on a bounded sample of the same workload.
 
 N > 1: the path does not shard (BASELINE.json: one GPU, no collectives) -- "replicas only": every rank runs the
@@ -372,16 +372,12 @@ def main_ours(args):
 
 
 def measure_e2e(band, n_steps, barrier, max_over_ranks, world, units_per_step):
-    """Host-buffer loop through the C ABI, a true continuation of the band: per step the whole checkpoint goes
-    host -> device (cfneb_set_state from pinned memory: X, v, the coordinates the lists were built at, the list
-    accounting, the FIRE scalars), one iteration runs, and the checkpoint comes back (cfneb_get_checkpoint).  The
-    sequence of states is bit-identical to the device-resident run (the handle keeps its neighbour lists: the state
-    it is handed is the one it holds; a new handle would take X_list / list_aux as well and replay the builds)."""
+    """Host-buffer loop through the C ABI, a true continuation of the band whose state lives in pinned host memory:
+    every step is one cfneb_step_hosted call -- X, v and the FIRE scalars go host -> device (in image blocks on a
+    second stream, each block evaluated while the next ones are on their way), the iteration runs, and X, v and
+    the scalars come back.  The sequence of states is bit-identical to the device-resident run (GPU test)."""
     import torch
-    import paper_2510_16721_b200 as cf
     ck = band.get_checkpoint()
-    shape = ck["X"].shape
-    P = shape[0]
 
     def pinned(a):
         t = torch.empty(a.shape, dtype=torch.float64, pin_memory=True)
@@ -391,30 +387,19 @@ def measure_e2e(band, n_steps, barrier, max_over_ranks, world, units_per_step):
     keep = [pinned(ck[k]) for k in ("X", "v")]
     X, v = (t.numpy() for t in keep)
     fire = ck["fire"]
-    L = cf.lib()
-    import ctypes
-    dp = lambda a: a.ctypes.data_as(ctypes.POINTER(ctypes.c_double))
 
-    def one():
-        nonlocal fire
-        band.set_state(X, v, None, None, fire)                  # H2D: 2 P (N+3) 3 doubles; the handle keeps its lists
-        band.step(1)
-        rc = L.cfneb_get_checkpoint(band._h, dp(X), dp(v), None, None, ctypes.byref(fire))  # D2H: the same; synchronises
-        if rc:
-            raise cf.CfnebError(rc, "cfneb_get_checkpoint")
-
-    one()  # warm-up
+    band.step_hosted(X, v, fire)  # warm-up
     barrier()
     t0 = time.perf_counter()
     for _ in range(n_steps):
-        one()
+        band.step_hosted(X, v, fire)
     barrier()
     dt = max_over_ranks(time.perf_counter() - t0)
     nbytes = 2 * X.size * 8 + 32
     return {"value": world * units_per_step * n_steps / dt, "unit": UNIT, "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
             "steps": n_steps, "ms_per_step": 1e3 * dt / n_steps,
-            "what": "per step: cfneb_set_state(pinned host checkpoint) + cfneb_step(1) + cfneb_get_checkpoint(pinned host); wall "
-                    "clock; a continuation (velocities, FIRE state and list state restored), bit-identical to the resident run"}
+            "what": "per step: cfneb_step_hosted(pinned host X, v, FIRE scalars in; the same out); wall clock; a continuation, "
+                    "bit-identical to the resident run; uploads in 10 image blocks overlapped with the force evaluation"}
 
 
 def main():

@@ -295,6 +295,20 @@ CFNEB_API int cfneb_get_checkpoint(cfneb_t *h, double *X, double *v, double *X_l
 CFNEB_API int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *X_list,
                               const double *list_aux, const cfneb_fire_state *fire);
 
+/*
+ * One iteration of a band whose state is kept in HOST memory (pinned memory for full copy speed): X and v, each
+ * P*(N+3)*3 as in cfneb_get_state, and the FIRE scalars go in, the iteration runs, and the new X, v and scalars come
+ * back in the same buffers.  The same arithmetic, bit for bit, as
+ *     cfneb_set_state(h, X, v, NULL, NULL, fire); cfneb_step(h, 1); cfneb_get_checkpoint(h, X, v, NULL, NULL, fire);
+ * (the handle keeps its neighbour lists; see cfneb_set_state), but the upload is cut into n_blocks blocks of
+ * consecutive images (0 = 10) sent on a second stream, and each block is evaluated -- cell map, list upkeep, forces:
+ * an image needs only its own coordinates for that -- while the later blocks are still on their way; only the
+ * reductions, the FIRE scalars and the update wait for the last block ("structural information is always kept and
+ * updated on GPU", is the fast path; this is the way to step a band that does not live there).  Synchronises.
+ * Errors: CFNEB_EINVAL (null pointers, scalars out of range), CFNEB_ERANGE (4096 images or more).
+ */
+CFNEB_API int cfneb_step_hosted(cfneb_t *h, double *X, double *v, cfneb_fire_state *fire, int32_t n_blocks);
+
 /* Parity hook: evaluate forces at the CURRENT X without updating anything.  F: P*N*3 Cartesian forces
  * (Eq. 5), virial: P*9 (Eq. 8), f_neb: P*(N+3)*3 NEB force of Eq. 1 in generalized coordinates (zero rows
  * for endpoints), energies: P.  Any may be NULL.  Synchronises. */

@@ -21,7 +21,7 @@ EXPORTS = (
     "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_adaptive", "cfneb_step_timed",
     "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_reparametrize", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
     "cfneb_get_path",
-    "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
+    "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_step_hosted", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
     "cfneb_destroy", "cfneb_strerror", "cfneb_last_cuda_error", "cfneb_util_fp64_peak",
 )
 
@@ -96,6 +96,7 @@ def lib():
         ("cfneb_set_path", [vp, dp, dp]), ("cfneb_get_state", [vp, dp, dp]),
         ("cfneb_get_checkpoint", [vp, dp, dp, dp, dp, ctypes.POINTER(FireState)]),
         ("cfneb_set_state", [vp, dp, dp, dp, dp, ctypes.POINTER(FireState)]),
+        ("cfneb_step_hosted", [vp, dp, dp, ctypes.POINTER(FireState), i32]),
         ("cfneb_get_forces", [vp, dp, dp, dp, dp]), ("cfneb_get_neighbors", [vp, i32, ip, ip, ip]),
         ("cfneb_get_status", [vp, ctypes.POINTER(Status)]), ("cfneb_util_fp64_peak", [vp, dp]),
     ):
@@ -335,6 +336,15 @@ class CFNEB:
                                    ctypes.byref(fire) if fire is not None else None)
         if rc:
             raise CfnebError(rc, "cfneb_set_state")
+
+    def step_hosted(self, X, v, fire, n_blocks=0):
+        """cfneb_step_hosted: one iteration of a band whose state (X, v: C-contiguous float64 arrays, updated in place;
+        fire: FireState, updated in place) lives in host memory."""
+        if not (X.flags.c_contiguous and v.flags.c_contiguous and X.dtype == np.float64 and v.dtype == np.float64):
+            raise ValueError("X and v must be C-contiguous float64 arrays (they are updated in place)")
+        rc = lib().cfneb_step_hosted(self._h, _dptr(X), _dptr(v), ctypes.byref(fire), int(n_blocks))
+        if rc:
+            raise CfnebError(rc, "cfneb_step_hosted")
 
     def get_forces(self, forces=True, f_neb=True):
         P = self.P

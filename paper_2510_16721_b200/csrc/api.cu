@@ -38,6 +38,8 @@ struct cfneb {
     bool mirror_dirty;    // the device edited P / order / free slots (cfneb_step_adaptive); host mirrors are stale
     bool interior_stale;  // cfneb_set_path replaced the path and the interior images have not been evaluated since
     int device;           // CUDA device the workspace and the stream live on (current at cfneb_create)
+    cudaStream_t st2;     // copy stream of cfneb_step_hosted (created on first use)
+    std::vector<cudaEvent_t> ev_blocks;  // one event per image block of cfneb_step_hosted
 };
 
 // Every ABI entry runs with the handle's device current and puts the caller's back on return, so a handle on
@@ -404,6 +406,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     h->mirror_dirty = false;
     h->st = static_cast<cudaStream_t>(cuda_stream);
     h->device = 0;
+    h->st2 = nullptr;
     cudaGetDevice(&h->device);
 #define CKH(call)                                  \
     do {                                           \
@@ -866,7 +869,7 @@ int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *
     int rc;
     if (X_list) {  // replay the list builds: lists at X_list, then the coordinates proper
         CK(cudaMemcpyAsync(dX, X_list, n * sizeof(double), cudaMemcpyHostToDevice, st));
-        launch_import_state(d, dX, nullptr, 0, st);
+        launch_import_state(d, dX, nullptr, 0, 0, h->P, st);
         CK(cudaStreamSynchronize(st));
         rc = force_rebuild_all(h);
         if (rc) return rc;
@@ -878,7 +881,7 @@ int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *
     // without X_list the neighbour lists are kept: the distance of the new coordinates from the stored ones goes into
     // each image's staleness bound (as in cfneb_set_path), so a state that is the stored one -- the host round trip of a
     // running band -- rebuilds nothing and continues bit for bit
-    launch_import_state(d, dX, (v && fire) ? dv : nullptr, X_list ? 0 : 1, st);
+    launch_import_state(d, dX, (v && fire) ? dv : nullptr, X_list ? 0 : 1, 0, h->P, st);
     if (!(v && fire)) launch_reset_fire(d, st);  // no velocities, or no FIRE state to go with them: a restart
     CK(cudaStreamSynchronize(st));  // dX / dv are reused below
     double *daux = dX;
@@ -893,6 +896,68 @@ int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *
     launch_finalize(d, kEndpointsOnly, st);
     h->interior_stale = true;
     return sync_status(h);
+}
+
+int cfneb_step_hosted(cfneb_t *h, double *X, double *v, cfneb_fire_state *fire, int32_t n_blocks) {
+    DeviceGuard dev_guard(h);
+    if (!h || !X || !v || !fire || n_blocks < 0) return CFNEB_EINVAL;
+    if (!(fire->dt > 0.0) || !(fire->alpha >= 0.0) || fire->n_pos < 0 || fire->steps < 0) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
+    const Dev &d = h->d;
+    cudaStream_t st = h->st;
+    const int P = h->P;
+    if (P >= 4096) return CFNEB_ERANGE;  // image_block() packs first and count into 12 bits each
+    if (n_blocks == 0) n_blocks = 10;
+    if (n_blocks > P) n_blocks = P;
+    if (!h->st2) CK(cudaStreamCreateWithFlags(&h->st2, cudaStreamNonBlocking));
+    while ((int)h->ev_blocks.size() < n_blocks + 1) {
+        cudaEvent_t e;
+        CK(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+        h->ev_blocks.push_back(e);
+    }
+    const size_t row = (size_t)(d.N + 3) * 3, n = (size_t)P * row;
+    double *dX = static_cast<double *>(d.scratch), *dv = dX + n;
+    // the copy stream starts after everything enqueued on the handle's stream so far (the staging area may be in use)
+    CK(cudaEventRecord(h->ev_blocks[n_blocks], st));
+    CK(cudaStreamWaitEvent(h->st2, h->ev_blocks[n_blocks], 0));
+    launch_import_aux(d, nullptr, 0, 1, fire->dt, fire->alpha, fire->n_pos, fire->first ? 1 : 0, (unsigned long long)fire->steps, st);
+    h->interior_stale = false;
+    for (int b = 0; b < n_blocks; ++b) {
+        const int a = (int)((long long)P * b / n_blocks), e = (int)((long long)P * (b + 1) / n_blocks), cnt = e - a;
+        if (cnt <= 0) continue;
+        CK(cudaMemcpyAsync(dX + a * row, X + a * row, cnt * row * sizeof(double), cudaMemcpyHostToDevice, h->st2));
+        CK(cudaMemcpyAsync(dv + a * row, v + a * row, cnt * row * sizeof(double), cudaMemcpyHostToDevice, h->st2));
+        CK(cudaEventRecord(h->ev_blocks[b], h->st2));
+        CK(cudaStreamWaitEvent(st, h->ev_blocks[b], 0));
+        // K0-K2 of an image need only that image's coordinates: the block is evaluated while the next ones arrive
+        launch_import_state(d, dX, dv, 1, a, cnt, st);
+        const int sel = image_block(a, cnt);
+        launch_cell_prep(d, sel, MODE_STEP, st);
+        launch_neighbor_build(d, sel, st);
+        launch_force(d, sel, st);
+        launch_finalize(d, sel, st);
+    }
+    // the endpoints as cfneb_set_state evaluates them (their energies enter the tangents of images 1 and P - 2)
+    launch_cell_prep(d, kEndpointsOnly, MODE_STEP, st);
+    launch_neighbor_build(d, kEndpointsOnly, st);
+    launch_force(d, kEndpointsOnly, st);
+    launch_finalize(d, kEndpointsOnly, st);
+    launch_reduce(d, st);
+    launch_scalar(d, 0, st);
+    launch_update(d, st);
+    launch_export_state(d, dX, dv, st);
+    CK(cudaMemcpyAsync(X, dX, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(v, dv, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    Ctl c;
+    CK(cudaMemcpyAsync(&c, d.ctl, sizeof c, cudaMemcpyDeviceToHost, st));
+    int rc = sync_status(h);
+    if (rc) return rc;
+    fire->dt = c.dt;
+    fire->alpha = c.alpha;
+    fire->steps = (int64_t)c.steps;
+    fire->n_pos = c.n_pos;
+    fire->first = c.first;
+    return CFNEB_OK;
 }
 
 int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, double *energies) {
@@ -973,6 +1038,8 @@ void cfneb_destroy(cfneb_t *h) {
     if (h->st) cudaStreamSynchronize(h->st);
     if (h->exec) cudaGraphExecDestroy(h->exec);
     if (h->graph) cudaGraphDestroy(h->graph);
+    for (cudaEvent_t e : h->ev_blocks) cudaEventDestroy(e);
+    if (h->st2) cudaStreamDestroy(h->st2);
     if (h->own_stream && h->st) cudaStreamDestroy(h->st);
     delete h;
 }

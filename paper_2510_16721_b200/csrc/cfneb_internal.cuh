@@ -174,14 +174,24 @@ __host__ __device__ inline void mul3_atb(const double *a, const double *b, doubl
 enum { MODE_STEP = 0, MODE_GEOMETRY_ONLY = 1 };
 
 // Image selection of the per-image kernels: p_lo = 1 the movable images 1..P-2, p_lo = 0 all images,
-// p_lo = kEndpointsOnly the two endpoints (endpoint relaxation).  y = the block's image coordinate.
+// p_lo = kEndpointsOnly the two endpoints (endpoint relaxation), p_lo = image_block(first, count) the movable images
+// among `count` consecutive path positions from `first` (cfneb_step_hosted: image blocks are evaluated while later
+// blocks are still on their way from the host).  y = the block's image coordinate.
 constexpr int kEndpointsOnly = -1;
-__device__ inline bool image_of(int y, int p_lo, int P, int &p) {
+__host__ __device__ inline int image_block(int first, int count) { return -2 - (first | (count << 12)); }  // first, count < 4096
+__host__ __device__ inline bool image_of(int y, int p_lo, int P, int &p) {
     if (p_lo == kEndpointsOnly) { p = y ? P - 1 : 0; return y < 2; }
+    if (p_lo < kEndpointsOnly) {
+        const int code = -2 - p_lo;
+        p = (code & 4095) + y;
+        return y < (code >> 12) && p >= 1 && p <= P - 2;
+    }
     p = y + p_lo;
     return p <= P - 1 - p_lo;
 }
-inline int images_in_grid(int S, int p_lo) { return p_lo == kEndpointsOnly ? 2 : S - 2 * p_lo; }
+__host__ __device__ inline int images_in_grid(int S, int p_lo) {
+    return p_lo == kEndpointsOnly ? 2 : p_lo < kEndpointsOnly ? ((-2 - p_lo) >> 12) : S - 2 * p_lo;
+}
 
 // ---- launch wrappers (each enqueues on `st`; p_lo = 1: movable images, 0: all images) ----
 void launch_input_map(const Dev &d, const double *pos_dev, const double *cells_dev, int p_first, int count, int track,
@@ -216,7 +226,8 @@ void launch_unpack_neighbors(const Dev &d, int slot, int *count_out, int *list_o
 void launch_export_path(const Dev &d, double *pos_out, double *cells_out, double *E_out, cudaStream_t st);
 void launch_export_state(const Dev &d, double *X_out, double *v_out, cudaStream_t st);
 void launch_export_list_state(const Dev &d, double *Xl_out, double *aux_out, cudaStream_t st);  // checkpoint
-void launch_import_state(const Dev &d, const double *X_in, const double *v_in, int track, cudaStream_t st);
+void launch_import_state(const Dev &d, const double *X_in, const double *v_in, int track, int p_first, int count,
+                         cudaStream_t st);  // images p_first .. p_first + count - 1 of the path
 void launch_import_aux(const Dev &d, const double *aux_in, int have_aux, int have_fire, double dt, double alpha, int n_pos,
                        int first, unsigned long long steps, cudaStream_t st);
 void launch_export_forces(const Dev &d, double *F_out, double *V_out, double *E_out, cudaStream_t st);

@@ -130,7 +130,7 @@ __device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
 // Compact list of the images (slots) of the selected set whose list is rebuilt this step, in path order.
 __global__ void __launch_bounds__(256) rebuild_list_kernel(Dev d, int p_lo) {
     const int P = d.ctl->P;
-    const int ny = p_lo == kEndpointsOnly ? 2 : d.S - 2 * p_lo;
+    const int ny = images_in_grid(d.S, p_lo);
     __shared__ int s_warp[8], s_base;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x == 0) s_base = 0;

@@ -276,10 +276,11 @@ __global__ void export_list_state_kernel(Dev d, double *Xo, double *aux) {
 // Inverse of export_state_kernel: X (and v, if given) from the caller's layout into both coordinate buffers.
 // track: the largest atomic displacement of each image from the stored coordinates goes into the staleness bound of
 // its neighbour list (as cfneb_set_path does), so the lists are kept while the new state stays inside their skin.
-__global__ void import_state_kernel(Dev d, const double *__restrict__ Xi, const double *__restrict__ vi, int track) {
-    const int p = blockIdx.y;
+__global__ void import_state_kernel(Dev d, const double *__restrict__ Xi, const double *__restrict__ vi, int track, int p_first,
+                                    int count) {
+    const int p = p_first + blockIdx.y;
     const int P = d.ctl->P;
-    if (p >= P) return;
+    if ((int)blockIdx.y >= count || p >= P) return;
     const int slot = d.order[p];
     const int rows = d.N + 3;
     const int a = blockIdx.x * blockDim.x + threadIdx.x;
@@ -390,9 +391,11 @@ void launch_export_list_state(const Dev &d, double *Xl_out, double *aux_out, cud
     export_list_state_kernel<<<grid, 128, 0, st>>>(d, Xl_out, aux_out);
 }
 
-void launch_import_state(const Dev &d, const double *X_in, const double *v_in, int track, cudaStream_t st) {
-    dim3 grid((d.N + 3 + 127) / 128, d.S);
-    import_state_kernel<<<grid, 128, 0, st>>>(d, X_in, v_in, track);
+void launch_import_state(const Dev &d, const double *X_in, const double *v_in, int track, int p_first, int count,
+                         cudaStream_t st) {
+    if (count <= 0) return;
+    dim3 grid((d.N + 3 + 127) / 128, count);
+    import_state_kernel<<<grid, 128, 0, st>>>(d, X_in, v_in, track, p_first, count);
 }
 
 void launch_import_aux(const Dev &d, const double *aux_in, int have_aux, int have_fire, double dt, double alpha, int n_pos,

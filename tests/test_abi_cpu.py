@@ -65,6 +65,7 @@ def test_workspace_bytes_and_argument_errors_need_no_device(cf):
     assert L.cfneb_step_adaptive(None, 1, 1, 1.0, 0.1) == -1
     assert L.cfneb_get_checkpoint(None, None, None, None, None, None) == -1
     assert L.cfneb_set_state(None, None, None, None, None, None) == -1
+    assert L.cfneb_step_hosted(None, None, None, None, 0) == -1 and L.cfneb_reparametrize(None, 1) == -1
     assert ctypes.sizeof(cf.FireState) == 32
     for code in range(0, -8, -1):
         assert len(L.cfneb_strerror(code)) > 1

@@ -489,6 +489,37 @@ def test_checkpoint_resume_is_bit_exact(k, n_before, n_after, over):
     c.close()
 
 
+@pytest.mark.parametrize("k,n_blocks,over", [(2, 0, dict()), (2, 3, dict(rebuild_every=4)), (1, 1, dict(cell_mode=2)), (0, 7, dict())])
+def test_step_hosted_is_bit_identical_to_the_resident_band(k, n_blocks, over):
+    """cfneb_step_hosted -- the state lives in host memory, image blocks are evaluated while later blocks are still
+    being uploaded -- gives, bit for bit, the states of the device-resident band (graph-launched cfneb_step), list
+    rebuilds included, for any number of blocks."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(k)
+    prm = cf.params_for(spec, cell_factor=0.0, **over)
+    a = cf.CFNEB(pos, cells, prm)
+    b = cf.CFNEB(pos, cells, prm)
+    a.step(3)
+    b.step(3)
+    ck = b.get_checkpoint()
+    X, v, fire = np.ascontiguousarray(ck["X"]), np.ascontiguousarray(ck["v"]), ck["fire"]
+    for it in range(9):
+        a.step(1)
+        b.step_hosted(X, v, fire, n_blocks)
+        Xa, va = a.get_state()
+        assert np.array_equal(X, Xa) and np.array_equal(v, va), it
+        sa = a.get_status()
+        assert (fire.dt, fire.alpha, fire.n_pos, fire.steps, fire.first) == (sa.dt, sa.alpha, sa.n_pos, sa.steps, 0)
+    sb = b.get_status()
+    assert sb.error == 0 and sb.fmax == sa.fmax and sb.barrier == sa.barrier
+    assert sb.rebuilds >= sa.rebuilds   # (the hosted step keeps the two endpoint lists up as well: rebuild_every counts for them too)
+    with pytest.raises(cf.CfnebError):
+        bad = cf.FireState(dt=-1.0, alpha=0.1, steps=0, n_pos=0, first=1)
+        b.step_hosted(X, v, bad)
+    a.close()
+    b.close()
+
+
 def test_neighbor_list_reuse_equals_fresh_lists():
     """Verlet-list reuse (skin) must not change the result: rebuild_every = 1 forces fresh lists each step."""
     import paper_2510_16721_b200 as cf
