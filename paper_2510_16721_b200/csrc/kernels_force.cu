@@ -182,8 +182,6 @@ __device__ __forceinline__ double fs_density(const FSc &c, uint32_t T, double r2
 // and sectors one iteration ahead of use; the loop is unrolled over the two pipeline stages so that no register
 // is rotated.  Rows past an atom's count hold a stand-in entry that is out of range by construction
 // (kernels_neighbor.cu), and the list carries 8 rows of slack, so no load is predicated.
-__device__ __forceinline__ void prefetch_l2(const void *p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-
 template <class Body>
 __device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_t stride, const double4 *Rc, int cnt_w,
                                           Body body) {
@@ -191,12 +189,6 @@ __device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_
     double4 sa0 = ld256(Rc + (a0 & kIdxMask)), sa1 = ld256(Rc + (a1 & kIdxMask)), sb0, sb1;
     lp += 4 * stride;
     for (int k = 0; k < cnt_w; k += 4) {
-#if CFNEB_PF_ROWS
-        // the list streams from HBM once per pass: pull the rows CFNEB_PF_ROWS ahead into L2 (a register-free look-ahead
-        // on top of the two-stage one; ncu: 22 % of the density kernel's samples waited on the first use of an entry)
-#pragma unroll
-        for (int u = 0; u < 4; ++u) prefetch_l2(lp + (size_t)(CFNEB_PF_ROWS - 4 + u) * stride);
-#endif
         sb0 = ld256(Rc + (b0 & kIdxMask));
         sb1 = ld256(Rc + (b1 & kIdxMask));
         {
@@ -221,14 +213,12 @@ __device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_
 // K2a (FS only): densities rho_i = sum_j psi(r_ij) over the Verlet list; writes F'(rho_i) into Rc[i].w and the
 // per-block embedding energy.  Two entries per iteration in 70 registers: seven blocks (28 warps) per SM measured
 // 10.66 ms for K2 at c4 against 10.94 with four entries per iteration at five blocks.
+// Resident blocks per multiprocessor (tuning knobs; the measured alternatives are in profiles/r2_k2_experiments.md)
 #ifndef CFNEB_DENSITY_BLOCKS
 #define CFNEB_DENSITY_BLOCKS (7 * 128 / CFNEB_PAIR_THREADS)
 #endif
 #ifndef CFNEB_FORCE_BLOCKS
 #define CFNEB_FORCE_BLOCKS (5 * 128 / CFNEB_PAIR_THREADS)
-#endif
-#ifndef CFNEB_PF_ROWS
-#define CFNEB_PF_ROWS 0
 #endif
 __global__ void __launch_bounds__(kThreadsPair, CFNEB_DENSITY_BLOCKS) density_kernel(Dev d, int p_lo) {
     int p;

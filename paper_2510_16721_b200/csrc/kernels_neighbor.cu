@@ -166,9 +166,6 @@ constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 #ifndef CFNEB_SEARCH_BLOCKS
 #define CFNEB_SEARCH_BLOCKS 5
 #endif
-#ifndef CFNEB_SEARCH_HSMEM
-#define CFNEB_SEARCH_HSMEM 0
-#endif
 // Round 2: the grid has a fixed size (CFNEB_SEARCH_BLOCKS blocks per multiprocessor) and takes its work items
 // (rebuilding image, block of 128 atoms) from the compact list of rebuild_list_kernel -- a step in which no list is
 // stale costs one exit per resident block instead of 77 616 -- and the unsorted column / bucket scratch of a block
@@ -178,7 +175,6 @@ constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_search_kernel(Dev d) {
     __shared__ unsigned short s_hist[kRadialBuckets * kThreadsAtom];
     __shared__ uint32_t s_queue[kQueue * kThreadsAtom];
-    __shared__ double s_h[9];
     __shared__ int s_max;
     if (threadIdx.x == 0) s_max = 0;
     const int n_items = d.ctl->n_rebuild * d.nblk_atom;
@@ -199,16 +195,9 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
         if (threadIdx.x == 0) set_error(d.ctl, CFNEB_ECELL);
         continue;
     }
-#if CFNEB_SEARCH_HSMEM
-    __syncthreads();  // every thread is done with the previous item's cell matrix
-    if (threadIdx.x < 9) s_h[threadIdx.x] = g->h[threadIdx.x];
-    __syncthreads();
-    const double *h = s_h;  // in shared memory: eighteen registers fewer per thread
-#else
     double h[9];
 #pragma unroll
     for (int k = 0; k < 9; ++k) h[k] = g->h[k];
-#endif
     const double4 si = d.Sw[(size_t)slot * d.Npad + ic];
     const unsigned long long fli = (unsigned long long)__double_as_longlong(si.w);
     const int fi0 = (int)(fli & 1023u), fi1 = (int)((fli >> 10) & 1023u), fi2 = (int)((fli >> 20) & 1023u);
