@@ -520,6 +520,79 @@ def test_step_hosted_is_bit_identical_to_the_resident_band(k, n_blocks, over):
     b.close()
 
 
+def test_hosted_step_and_checkpoint_after_image_control():
+    """The state calls on a band whose image count and slot order were changed on the device (cfneb_step_adaptive) and on
+    the host (insert / delete): cfneb_step_hosted and a checkpoint resume in a second handle, brought to the same image
+    count by the same control calls, stay bit-identical to the resident band."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(1)
+    prm = cf.params_for(spec, cell_factor=0.0, max_images=14)
+    a = cf.CFNEB(pos, cells, prm)
+    b = cf.CFNEB(pos, cells, prm)
+    L0 = float(np.sum(a.get_segment_lengths()))
+    for g in (a, b):
+        g.step_adaptive(6, 3, L0 / 10.0, L0 / 40.0)     # grows the band on the device
+        g.insert_image(1)
+        g.delete_image(4 if g.get_status().climb_index != 4 else 5)
+        g.step(2)
+    P = a.P
+    assert P == b.P and P > 9
+    ck = b.get_checkpoint()
+    assert ck["X"].shape[0] == P
+    X, v, fire = np.ascontiguousarray(ck["X"]), np.ascontiguousarray(ck["v"]), ck["fire"]
+    for it in range(4):
+        a.step(1)
+        b.step_hosted(X, v, fire, 4)
+        Xa, va = a.get_state()
+        assert np.array_equal(X, Xa) and np.array_equal(v, va), it
+    # resume in a third handle that reached the same P by another route: same endpoints, images inserted anywhere
+    c = cf.CFNEB(pos, cells, prm)
+    while c.P < P:
+        c.insert_image(0)
+    ck = a.get_checkpoint()
+    c.set_state(ck["X"], ck["v"], ck["X_list"], ck["list_aux"], ck["fire"])
+    a.step(5)
+    c.step(5)
+    assert np.array_equal(a.get_state()[0], c.get_state()[0]) and np.array_equal(a.get_state()[1], c.get_state()[1])
+    for g in (a, b, c):
+        assert g.get_status().error == 0
+        g.close()
+
+
+def test_reparametrize_edge_cases():
+    """P = 3 with the single interior image held (nothing moves), P = 3 not held (the image goes to mid arc length),
+    the small c0 box with periodic self-images, and two calls in a row (the second is the identity to round-off)."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(0)
+    g = cf.CFNEB(pos[[0, 2, 6]], cells[[0, 2, 6]], cf.params_for(spec, cell_factor=0.0, max_images=3))
+    g.step(2)
+    X0, _ = g.get_state()
+    assert g.get_status().climb_index == 1
+    g.reparametrize(hold_climbing=True)
+    assert np.array_equal(g.get_state()[0], X0)
+    g.reparametrize(hold_climbing=False)
+    X1, v1 = g.get_state()
+    d = g.get_segment_lengths()
+    assert abs(d[0] - d[1]) < 0.35 * d.mean() and np.all(v1 == 0)    # on the old polyline at half its arc length
+    tot0 = np.linalg.norm(X0[1] - X0[0]) + np.linalg.norm(X0[2] - X0[1])
+    assert abs(np.linalg.norm(X1[1] - X0[0]) - 0.5 * tot0) < 1e-9 * tot0 or abs(np.linalg.norm(X1[1] - X0[2]) - 0.5 * tot0) < 1e-9 * tot0
+    g.step(2)
+    assert g.get_status().error == 0 and np.all(np.isfinite(g.get_path(positions=False)[2]))
+    g.close()
+    g = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    g.step(3)
+    g.reparametrize(hold_climbing=False)
+    Xa, _ = g.get_state()
+    g.reparametrize(hold_climbing=False)
+    Xb, _ = g.get_state()
+    assert np.max(np.abs(Xb - Xa)) < 1e-3 * np.max(np.abs(Xa)) and np.array_equal(Xb[0], Xa[0]) and np.array_equal(Xb[-1], Xa[-1])
+    da = g.get_segment_lengths()
+    assert da.max() < 1.05 * da.min()
+    g.step(3)
+    assert g.get_status().error == 0
+    g.close()
+
+
 def test_neighbor_list_reuse_equals_fresh_lists():
     """Verlet-list reuse (skin) must not change the result: rebuild_every = 1 forces fresh lists each step."""
     import paper_2510_16721_b200 as cf
@@ -1073,6 +1146,56 @@ def test_nep_shaped_potential_forces_and_steps(dims, n_images, net):
     Xo, vo = orc.get_state()
     Xg, vg = gpu.get_state()
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
+    assert gpu.get_status().error == 0
+    gpu.close()
+
+
+def test_nep_shaped_potential_with_the_rest_of_the_path():
+    """The NEP-shaped potential through the parts of the path that do not know the potential: external pressure with the
+    Eq. 14 cell force, an inserted image, re-parametrisation, endpoint relaxation -- against the oracle."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import diamond_strain_band, nep_params, two_sublattice_types
+    from oracle import cfneb as oc
+    from oracle import cellfilter as ocf
+    pot = nep_params(rc_r=5.6, rc_a=3.9, n_r=4, n_a=3, k_r=6, k_a=5, L=4, H=12, n_types=2, seed=5)
+    pos, cells = diamond_strain_band((2, 2, 3), 5.35, 5, 31, 0.06, ((0.0, 0.04, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.05)))
+    types = two_sublattice_types(pos.shape[1], 2)
+    fire = dict(dt0=0.05, dtmax=0.1, maxstep=0.01, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+    orc = oc.CFNEB(pos, cells, 4, pot, pot[0], k_spring=1.0, climb=True, cell_factor=0.0, fire=fire, skin=0.3, max_neighbors=256,
+                   cell_mode=ocf.CELL_D, pressure=0.05, types=types)
+    prm = cf.default_params(potential=cf.POT_NEP, pot=list(pot), k_spring=1.0, climb=1, cell_factor=0.0, skin=0.3,
+                            max_neighbors=256, max_images=8, fire=fire, cell_mode=cf.CELL_D, pressure=0.05, types=types)
+    gpu = cf.CFNEB(pos, cells, prm)
+    f_or = orc.band.forces()
+    F, V, fneb, E = gpu.get_forces()
+    assert rel(E, orc.band.E) < TOL_FORCE and rel(V[1:-1], orc.evaluator.last["V"]) < TOL_FORCE
+    assert rel(fneb[1:-1], np.stack(f_or[1:-1])) < TOL_STEP
+    X0 = first_step_exact(orc, gpu)
+    orc.step(3)
+    gpu.step(3)
+    assert rel(gpu.get_state()[0] - X0, orc.get_state()[0] - X0) < 1e-7
+    p = int(np.argmax(gpu.get_segment_lengths()))
+    gpu.insert_image(p)
+    orc.insert_image(p)
+    orc.step(2)
+    gpu.step(2)
+    orc.reparametrize(hold_climbing=True)
+    gpu.reparametrize(hold_climbing=True)
+    orc.step(2)
+    gpu.step(2)
+    Xo, Xg = orc.get_state()[0], gpu.get_state()[0]
+    assert Xg.shape == Xo.shape and rel(Xg, Xo) < 1e-9
+    assert gpu.get_status().error == 0
+    gpu.close()
+    kw = dict(fmax_tol=0.0, max_steps=10, cell_factor=0.0, fire=fire, skin=0.3, max_neighbors=256, types=types)
+    Ra, ha, _, _, _ = oc.relax_endpoint(pos[0], cells[0], 4, pot, pot[0], **kw)
+    prm2 = cf.default_params(potential=cf.POT_NEP, pot=list(pot), k_spring=1.0, climb=0, cell_factor=0.0, skin=0.3,
+                             max_neighbors=256, max_images=4, fire=fire, types=types)
+    gpu = cf.CFNEB(np.stack([pos[0], pos[-1]]), np.stack([cells[0], cells[-1]]), prm2, n_images=4)
+    steps, fmax, en = gpu.relax_endpoints(0.0, 10, rebuild_band=False)
+    p2, c2, _ = gpu.get_path()
+    assert steps == [10, 10]
+    assert rel(p2[0] - pos[0], Ra - pos[0]) < 1e-8 and rel(c2[0] - cells[0], ha - cells[0]) < 1e-8
     assert gpu.get_status().error == 0
     gpu.close()
 
