@@ -135,6 +135,21 @@ def ncu_traffic(workload, kernel):
     return None
 
 
+def ncu_pipe(workload, kernel):
+    """fp64-pipe and issue-slot utilisation of `kernel` from the committed ncu capture (profiles/pipe_utilisation.csv:
+    workload,kernel,fp64 pipe %,issue active %,source), or None.  Context for the ALU roofline: the pair kernels are
+    bound by instruction issue (an fp64 instruction holds its scheduler for two cycles), not by the flop count."""
+    path = os.path.join(ROOT, "profiles", "pipe_utilisation.csv")
+    if not os.path.exists(path):
+        return None
+    with open(path) as fh:
+        for line in fh:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) >= 4 and f[0] == workload and f[1] == kernel:
+                return {"fp64_pipe_frac": float(f[2]) / 100.0, "issue_active_frac": float(f[3]) / 100.0}
+    return None
+
+
 # fp64 operations per in-range pair as the formulas of kernels_force.cu are written (FMA = 2, everything else = 1;
 # DESIGN.md section 5): density pass plain / taper, force pass plain / taper (beta = 2 alpha: one exponential).
 FLOPS_DENSITY = (40.0, 70.0)
@@ -345,7 +360,10 @@ def main_ours(args):
                           "in_range_pairs_per_atom_mean": float(np.mean([a + b for a, b in pc])),
                           "taper_zone_pairs_per_atom_mean": float(np.mean([b for _, b in pc])),
                           "peak_source": "measured DFMA chain, cfneb_util_fp64_peak (no fp64 figure in MEASURED_PEAKS.json)",
-                          "share_of_step": float(kms[cf.binding.K_FORCE] / kms.sum())}
+                          "share_of_step": float(kms[cf.binding.K_FORCE] / kms.sum()),
+                          "ncu": {"force_kernel": ncu_pipe("c4", "force_kernel"), "density_kernel": ncu_pipe("c4", "density_kernel"),
+                                  "note": "committed ncu capture of configs[4] (profiles/r2_ncu_full_c4.txt): share of the fp64 pipe's and "
+                                          "of the issue slots' peak; 2 x fp64 + other instructions = 91 % of the scheduler cycles"}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
