@@ -158,6 +158,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.nbr_count = c.take<int>(S * Npad);
     d.nbr_list = c.take<uint32_t>(S * (size_t)d.cap * Npad + 16 * Npad);  // 16 rows of slack for the force kernels' look-ahead
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
+    d.nbr_edge = prm->potential == CFNEB_POT_NEP ? c.take<unsigned short>(S * (size_t)kEdgeRows * Npad) : nullptr;
     d.rebuild_slots = c.take<int>(S);
     {   // K1 scratch: one region per resident block of the search kernel (sized for the largest device we know)
         int dev = 0, sms = 148;
@@ -172,6 +173,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.dn_w = prm->potential == CFNEB_POT_DNN ? c.take<double>(kDnWeights)
              : prm->potential == CFNEB_POT_NEP ? c.take<double>(nep_weight_count(prm->pot)) : nullptr;
     d.types = prm->potential == CFNEB_POT_NEP ? c.take<int>(Npad) : nullptr;
+    d.nep_q = prm->potential == CFNEB_POT_NEP ? c.take<double>(S * (size_t)8 * Npad) : nullptr;
     d.nep_S = prm->potential == CFNEB_POT_NEP ? c.take<double>(S * (size_t)prm->pot[3] * 35 * Npad) : nullptr;
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);
@@ -443,6 +445,8 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     d.pressure = prm->pressure;
     d.r_cut = cutoff_of(prm);
     d.r_list = d.r_cut + d.skin;
+    d.edge_b0 = prm->potential == CFNEB_POT_NEP
+                    ? (int)floor(prm->pot[1] * prm->pot[1] / (d.r_cut * d.r_cut) * kInnerBuckets) : 0;
     prepare_potential(d);
     if (set_reference_frame(h, cell_init, cell_final) != CFNEB_OK) { cfneb_destroy(h); return CFNEB_EINVAL; }
     h->P = n_images;

@@ -35,6 +35,7 @@ constexpr int kMaxAtoms = 1 << 23;
 constexpr int kDnWeights = 8 * 16 + 2 * 8;  // CFNEB_POT_DNN: H <= 8, D <= 16
 constexpr int kInnerBuckets = 56;      // radial buckets of the list sort: uniform in r^2 on [0, r_cut^2)
 constexpr int kTailBuckets = 8;        // ... and on [r_cut^2, r_list^2)
+constexpr int kEdgeRows = 12;          // inner bucket edges from Dev::edge_b0 on whose list offsets are kept (Dev::nbr_edge)
 
 enum { DOT_PP = 0, DOT_MM, DOT_PM, DOT_GP, DOT_GM, DOT_GG, DOT_GV, DOT_PV, DOT_MV, DOT_VV };
 
@@ -131,8 +132,12 @@ struct Dev {
     int *nbr_count;           // [S][Npad]
     uint32_t *nbr_list;       // [S][cap][Npad]  Verlet list (r < r_cut + skin), sorted by distance at build, rebuilt when stale
     unsigned short *nbr_tail; // [S][kTailBuckets][Npad] number of entries below tail bucket t (list sorted by bucket)
+    unsigned short *nbr_edge; // [S][kEdgeRows][Npad] number of entries below inner bucket edge_b0 + q (NEP: the rows
+                              // that can lie inside the angular cut-off; nullptr for the other potentials)
+    int edge_b0;              // first inner bucket edge kept: the last one at or below the inner radius (NEP: rc_a)
     double *dn_w;               // [kDnWeights] W0[H][D], b0[H], W1[H] of CFNEB_POT_DNN; CFNEB_POT_NEP: see kernels_nep.cu
     int *types;                 // [Npad] atom types in storage order (CFNEB_POT_NEP)
+    double *nep_q;              // [S][8][Npad] radial descriptors q_n (radial kernel 1 -> quad kernel), then dU/dq_n (-> radial kernel 2)
     double *nep_S;              // [S][n_a][35][Npad] moments of the angular channels between the two walks (CFNEB_POT_NEP)
     unsigned short *nbr_mirror; // [S][cap][Npad] row of the mirror entry (j; i, -n) of each entry (many-body potentials only)
     double *part;             // [S][cap][3][Npad] partial forces p^ij = dU_i/dr^ij per list entry (many-body potentials only)

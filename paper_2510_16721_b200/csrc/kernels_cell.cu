@@ -274,7 +274,7 @@ __global__ void __launch_bounds__(kThreadsAtom) positions_kernel(Dev d, int p_lo
     r.x = x * g->D[0] + y * g->D[3] + z * g->D[6];
     r.y = x * g->D[1] + y * g->D[4] + z * g->D[7];
     r.z = x * g->D[2] + y * g->D[5] + z * g->D[8];
-    r.w = 0.0;
+    r.w = d.types ? (double)d.types[i] : 0.0;  // NEP: the atom type rides in the sector (FS: F'(rho), K2a)
     d.Rc[(size_t)slot * d.Npad + i] = r;
     if (mode == MODE_STEP && g->rebuild) {  // the list is built from these coordinates
         double *Xb = d.Xb + (size_t)slot * 3 * d.Npad;

@@ -301,9 +301,11 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
     // four entries per round so that the global loads of a round are independent
     int start = 0;
     unsigned short *tail = d.nbr_tail + (size_t)slot * kTailBuckets * d.Npad + i;
+    unsigned short *edge = d.nbr_edge ? d.nbr_edge + (size_t)slot * kEdgeRows * d.Npad + i : nullptr;
     for (int b = 0; b < kRadialBuckets; ++b) {
         const int c = hist[b * kThreadsAtom];
         hist[b * kThreadsAtom] = (unsigned short)start;
+        if (edge && (unsigned)(b - d.edge_b0) < (unsigned)kEdgeRows) edge[(size_t)(b - d.edge_b0) * d.Npad] = (unsigned short)start;
         if (b >= kInnerBuckets) tail[(size_t)(b - kInnerBuckets) * d.Npad] = (unsigned short)start;  // entries below tail bucket b - 56
         start += c;
     }

@@ -30,10 +30,10 @@
 
 namespace cfn {
 
-constexpr int kNepMaxN = 8, kNepMaxK = 12, kNepMaxH = 64, kNepMaxL = 4;
+constexpr int kNepMaxN = 8, kNepMaxH = 64, kNepMaxL = 4, kNepMaxD = kNepMaxN + kNepMaxN * kNepMaxL;
 constexpr int kNepThreads = 128;  // 32 atoms x 4 lanes
 #ifndef CFNEB_NEP_BLOCKS
-#define CFNEB_NEP_BLOCKS 2
+#define CFNEB_NEP_BLOCKS 3
 #endif
 
 struct NepShape {
@@ -46,8 +46,11 @@ __host__ __device__ inline NepShape nep_shape(const double *pot) {
     s.D = s.nr + s.na * s.L;
     return s;
 }
-// layout of Dev::dn_w for this potential: per type [W0 H*D | b0 H | W1 H], then cR [T][T][nr][kr], then cA [T][T][na][ka]
-__host__ __device__ inline int nep_net_size(const NepShape &s) { return s.H * s.D + 2 * s.H; }
+// layout of Dev::dn_w for this potential: per type [W0t D*Hp | b0 Hp | W1 Hp] (first layer transposed to [d][mu], the
+// neurons zero-padded to Hp, a multiple of four: the quad kernel copies it to shared memory as it is), then
+// cR [T][T][nr][kr], then cA [T][T][na][ka]
+__host__ __device__ inline int nep_hp(const NepShape &s) { return (s.H + 3) & ~3; }
+__host__ __device__ inline int nep_net_size(const NepShape &s) { return s.D * nep_hp(s) + 2 * nep_hp(s); }
 __host__ __device__ inline int nep_weights_size(const NepShape &s) {
     return s.T * nep_net_size(s) + s.T * s.T * (s.nr * s.kr + s.na * s.ka);
 }
@@ -78,6 +81,163 @@ __device__ __forceinline__ void nep_basis(double t, double irc, int K, double (&
     }
 }
 
+__device__ __forceinline__ const double4 *Rc_of(const Dev &d, int slot) { return d.Rc + (size_t)slot * d.Npad; }
+
+// Rows of atom i's (distance-sorted) list that can hold a pair inside the angular cut-off now: everything before the
+// first kept inner bucket edge that is at least rc_a + acc (built at or beyond that edge, moved by at most acc since:
+// the reasoning of live_rows).  All live rows when no kept edge is far enough.
+__device__ inline int nep_angular_rows(const Dev &d, int slot, int i) {
+    const double rc2 = d.r_cut * d.r_cut, need = d.pot[1] + d.geom[slot].acc + 1e-9 * d.r_cut;
+    for (int e = 0; e < kEdgeRows; ++e) {
+        const int b = d.edge_b0 + e;
+        if (b <= kInnerBuckets && sqrt(rc2 * b / kInnerBuckets) >= need)
+            return min((int)d.nbr_edge[((size_t)slot * kEdgeRows + e) * d.Npad + i], d.cap);
+    }
+    return live_rows(d, slot, i);
+}
+
+// One atom per thread over all live rows of its list, entry two rows and sector one row ahead of use:
+// body(k, rj, dx, dy, dz, r2) for the rows k < cnt of this thread (rj.w = type of the neighbour).
+template <class Body>
+__device__ __forceinline__ void nep_walk_rows(const Dev &d, const uint32_t *lp, const double4 *Rc, const double4 &ri,
+                                              const double *sh, int cnt, Body body) {
+    if (cnt <= 0) return;
+    uint32_t e0 = lp[0], e1 = lp[(size_t)min(1, cnt - 1) * d.Npad];
+    double4 rj = Rc[e0 & kIdxMask];
+    for (int k = 0; k < cnt; ++k) {
+        const uint32_t code = e0 >> kShiftBits;
+        const double4 rc = rj;
+        e0 = e1;
+        e1 = lp[(size_t)min(k + 2, cnt - 1) * d.Npad];
+        rj = Rc[e0 & kIdxMask];
+        double dx = rc.x - ri.x, dy = rc.y - ri.y, dz = rc.z - ri.z;
+        if (code != kCodeCenter) {
+            const double n0 = (double)((int)(code & 7u) - 4), n1 = (double)((int)((code >> 3) & 7u) - 4),
+                         n2 = (double)((int)((code >> 6) & 7u) - 4);
+            dx += n0 * sh[0] + n1 * sh[3] + n2 * sh[6];
+            dy += n0 * sh[1] + n1 * sh[4] + n2 * sh[7];
+            dz += n0 * sh[2] + n1 * sh[5] + n2 * sh[8];
+        }
+        body(k, rc, dx, dy, dz, dx * dx + dy * dy + dz * dz);
+    }
+}
+
+constexpr int kNepRadialThreads = 128;
+#ifndef CFNEB_NEP_RADIAL_BLOCKS
+#define CFNEB_NEP_RADIAL_BLOCKS 4
+#endif
+
+// Radial descriptors q_n = sum_j sum_k cR[I][J][n][k] f_k(r_ij; rc_r) -> Dev::nep_q.  One atom per thread; the sum
+// over the environment is taken per neighbour type on the basis functions, B[J][k] = sum_{j of type J} f_k(r_ij),
+// and the coefficients are applied once per atom (k_r adds per row instead of n_r k_r multiply-adds).
+template <int KMAX, int NT>
+__global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) nep_radial_desc_kernel(Dev d, int p_lo) {
+    int p;
+    if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
+    const int slot = d.order[p];
+    __shared__ double sh[9];
+    if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.N) return;
+    const NepShape sp = nep_shape(d.pot);
+    const double rcr = d.pot[0], rcr2 = rcr * rcr, ircr = 1.0 / rcr;
+    const double4 *Rc = Rc_of(d, slot);
+    const double4 ri = Rc[i];
+    double B[NT][KMAX];
+#pragma unroll
+    for (int J = 0; J < NT; ++J)
+#pragma unroll
+        for (int k = 0; k < KMAX; ++k) B[J][k] = 0.0;
+    nep_walk_rows(d, d.nbr_list + (size_t)slot * d.cap * d.Npad + i, Rc, ri, sh, live_rows(d, slot, i),
+                  [&](int, const double4 &rj, double, double, double, double r2) {
+        if (r2 < rcr2) {
+            double f[KMAX], df[KMAX];
+            nep_basis<KMAX>(r2 * rsqrt(r2) * ircr, ircr, sp.kr, f, df);
+            if (NT == 1) {
+#pragma unroll
+                for (int k = 0; k < KMAX; ++k) B[0][k] += f[k];
+            } else {
+                const double m1 = rj.w, m0 = 1.0 - m1;  // type of the neighbour as a weight
+#pragma unroll
+                for (int k = 0; k < KMAX; ++k) {
+                    B[0][k] = fma(m0, f[k], B[0][k]);
+                    B[NT - 1][k] = fma(m1, f[k], B[NT - 1][k]);
+                }
+            }
+        }
+    });
+    const int I = (int)ri.w;
+    const double *cR = d.dn_w + sp.T * nep_net_size(sp) + (size_t)I * sp.T * sp.nr * sp.kr;  // [J][n][k]
+    double *qscr = d.nep_q + (size_t)slot * kNepMaxN * d.Npad + i;
+    for (int n = 0; n < sp.nr; ++n) {
+        double qn = 0.0;
+#pragma unroll
+        for (int J = 0; J < NT; ++J)
+#pragma unroll
+            for (int k = 0; k < KMAX; ++k)
+                if (k < sp.kr) qn = fma(cR[(J * sp.nr + n) * sp.kr + k], B[J][k], qn);
+        qscr[(size_t)n * d.Npad] = qn;
+    }
+}
+
+// Radial part of the partial forces, p^ij += sum_n dU/dq_n g_n'(r_ij) u_ij = [sum_k w[J][k] f_k'(r_ij)] u_ij with
+// w[J][k] = sum_n dU/dq_n cR[I][J][n][k] formed once per atom (dU/dq_n from the quad kernel in Dev::nep_q).  One atom
+// per thread over all live rows; the rows below the angular count already hold the angular part (quad kernel).
+template <int KMAX, int NT>
+__global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) nep_radial_force_kernel(Dev d, int p_lo) {
+    int p;
+    if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
+    const int slot = d.order[p];
+    __shared__ double sh[9];
+    if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= d.N) return;
+    const NepShape sp = nep_shape(d.pot);
+    const double rcr = d.pot[0], rcr2 = rcr * rcr, ircr = 1.0 / rcr;
+    const double4 *Rc = Rc_of(d, slot);
+    const double4 ri = Rc[i];
+    const int I = (int)ri.w;
+    const double *cR = d.dn_w + sp.T * nep_net_size(sp) + (size_t)I * sp.T * sp.nr * sp.kr;  // [J][n][k]
+    const double *qscr = d.nep_q + (size_t)slot * kNepMaxN * d.Npad + i;
+    double w[NT][KMAX];
+#pragma unroll
+    for (int J = 0; J < NT; ++J)
+#pragma unroll
+        for (int k = 0; k < KMAX; ++k) w[J][k] = 0.0;
+    for (int n = 0; n < sp.nr; ++n) {
+        const double Fd = qscr[(size_t)n * d.Npad];
+#pragma unroll
+        for (int J = 0; J < NT; ++J)
+#pragma unroll
+            for (int k = 0; k < KMAX; ++k)
+                if (k < sp.kr) w[J][k] = fma(Fd, cR[(J * sp.nr + n) * sp.kr + k], w[J][k]);
+    }
+    const int cntA = nep_angular_rows(d, slot, i);
+    double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + i;  // part[(k * 3 + m) * Npad]
+    nep_walk_rows(d, d.nbr_list + (size_t)slot * d.cap * d.Npad + i, Rc, ri, sh, live_rows(d, slot, i),
+                  [&](int k, const double4 &rj, double dx, double dy, double dz, double r2) {
+        double *o = part + (size_t)(k * 3) * d.Npad;
+        double px = 0.0, py = 0.0, pz = 0.0;
+        if (k < cntA) { px = o[0]; py = o[d.Npad]; pz = o[2 * (size_t)d.Npad]; }
+        if (r2 < rcr2) {
+            const double inv = rsqrt(r2);
+            double f[KMAX], df[KMAX];
+            nep_basis<KMAX>(r2 * inv * ircr, ircr, sp.kr, f, df);
+            double s0 = 0.0, s1 = 0.0;
+#pragma unroll
+            for (int k2 = 0; k2 < KMAX; ++k2) {
+                s0 = fma(w[0][k2], df[k2], s0);
+                if (NT > 1) s1 = fma(w[NT - 1][k2], df[k2], s1);
+            }
+            const double sr = (NT > 1 ? fma(rj.w, s1 - s0, s0) : s0) * inv;
+            px = fma(sr, dx, px); py = fma(sr, dy, py); pz = fma(sr, dz, pz);
+        }
+        o[0] = px; o[d.Npad] = py; o[2 * (size_t)d.Npad] = pz;
+    });
+}
+
 // KMAX: basis functions held per row (the smallest of 4, 8, 12 that covers k_r and k_a): the loops over them are
 // unrolled so that the basis stays in registers.
 template <int KMAX>
@@ -88,16 +248,17 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     extern __shared__ double sW[];  // all weights of the potential
     __shared__ double sh[9];
     __shared__ double red[64];
+    __shared__ double sQ[(kNepThreads / 4) * (kNepMaxD + 1)];  // descriptors, then their gradients, one row per quad
     const NepShape sp = nep_shape(d.pot);
-    const int nNet = sp.T * nep_net_size(sp);
+    const int nNet = sp.T * nep_net_size(sp);  // offset of the expansion coefficients in Dev::dn_w
+    const int Hp = nep_hp(sp), netp = nep_net_size(sp);
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
     for (int t = threadIdx.x; t < nNet; t += blockDim.x) sW[t] = d.dn_w[t];
-    // expansion coefficients zero-padded to [T][T][8][KMAX] (radial, then angular): the loops over channels and basis
-    // functions then run to their compile-time bounds with no guards, and a row of coefficients is KMAX aligned doubles
-    double *cRp = sW + ((nNet + 1) & ~1), *cAp = cRp + sp.T * sp.T * kNepMaxN * KMAX;
+    // angular expansion coefficients zero-padded to [T][T][8][KMAX]: the loops over channels and basis functions then
+    // run to their compile-time bounds with no guards, and a row of coefficients is KMAX aligned doubles
+    double *cAp = sW + ((nNet + 1) & ~1);
     for (int t = threadIdx.x; t < sp.T * sp.T * kNepMaxN * KMAX; t += blockDim.x) {
         const int b = t % KMAX, nn = (t / KMAX) % kNepMaxN, IJ = t / (KMAX * kNepMaxN);
-        cRp[t] = (nn < sp.nr && b < sp.kr) ? d.dn_w[nNet + (IJ * sp.nr + nn) * sp.kr + b] : 0.0;
         cAp[t] = (nn < sp.na && b < sp.ka) ? d.dn_w[nNet + sp.T * sp.T * sp.nr * sp.kr + (IJ * sp.na + nn) * sp.ka + b] : 0.0;
     }
     __syncthreads();
@@ -106,18 +267,17 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     const bool valid = i < d.N;
     const int ic = valid ? i : 0;
     const unsigned quad_mask = 0xffffffffu;  // see cnt_w below
-    const double rcr = d.pot[0], rca = d.pot[1], rcr2 = rcr * rcr, rca2 = rca * rca, ircr = 1.0 / rcr, irca = 1.0 / rca;
-    const int I = d.types[ic];
-    const double *net = sW + I * nep_net_size(sp);
-    const double *W0 = net, *b0 = net + sp.H * sp.D, *W1 = b0 + sp.H;
-    const double *cRb = cRp + (size_t)I * sp.T * kNepMaxN * KMAX;   // [J][n][k], padded
+    const double rca = d.pot[1], rca2 = rca * rca, irca = 1.0 / rca;
+    const double4 ri = Rc_of(d, slot)[ic];
+    const int I = (int)ri.w;
+    const double *W0t = sW + I * netp, *b0 = W0t + sp.D * Hp, *W1 = b0 + Hp;
     const double *cAb = cAp + (size_t)I * sp.T * kNepMaxN * KMAX;
-    const double4 *Rc = d.Rc + (size_t)slot * d.Npad;
+    const double4 *Rc = Rc_of(d, slot);
     const uint32_t *lp = d.nbr_list + (size_t)slot * d.cap * d.Npad + ic;
     double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + ic;  // part[(k * 3 + m) * Npad]
     double *scr = d.nep_S + ((size_t)slot * sp.na * kNepC) * d.Npad + ic;  // scr[(n * kNepC + c) * Npad]
-    const double4 ri = Rc[ic];
-    const int cnt = valid ? live_rows(d, slot, ic) : 0;  // rows past it cannot be in range
+    double *qscr = d.nep_q + (size_t)slot * kNepMaxN * d.Npad + ic;       // qscr[n * Npad]
+    const int cnt = valid ? nep_angular_rows(d, slot, ic) : 0;  // rows past it cannot be inside rc_a
     // every loop over list rows runs to the longest list of the warp (rows past a quad's own count are skipped by
     // `kk < cnt`): all 32 lanes reach every shuffle, so the shuffles take the full mask
     const int cnt_w = __reduce_max_sync(0xffffffffu, cnt);
@@ -127,21 +287,18 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     // hide the two dependent loads otherwise).  Rows past the end stand in with the atom itself and are never used.
     uint32_t e_nn, e_n;
     double4 rj_n;
-    int J_n;
     auto walk_begin = [&]() {
         e_n = q < cnt ? lp[(size_t)q * d.Npad] : (uint32_t)ic | (kCodeCenter << kShiftBits);
         e_nn = q + 4 < cnt ? lp[(size_t)(q + 4) * d.Npad] : e_n;
         rj_n = Rc[e_n & kIdxMask];
-        J_n = d.types[e_n & kIdxMask];
     };
     auto pair_vec = [&](int k, int &J, double &dx, double &dy, double &dz) {  // row k of this lane; advances the pipeline
         const uint32_t code = e_n >> kShiftBits;
         const double4 rj = rj_n;
-        J = J_n;
+        J = (int)rj.w;  // positions_kernel puts the type there
         e_n = e_nn;
         e_nn = k + 8 < cnt ? lp[(size_t)(k + 8) * d.Npad] : e_n;
         rj_n = Rc[e_n & kIdxMask];
-        J_n = d.types[e_n & kIdxMask];
         dx = rj.x - ri.x; dy = rj.y - ri.y; dz = rj.z - ri.z;
         if (code != kCodeCenter) {
             const double n0 = (double)((int)(code & 7u) - 4), n1 = (double)((int)((code >> 3) & 7u) - 4),
@@ -164,9 +321,6 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     // ---- walk 1: the list is taken four rows at a time, ONE ROW PER LANE: the lane forms the pair vector, the radial
     // basis and the expansions g_n of its row (nothing of that is done four times), then the rows go round the quad
     // (step t: lane q takes the row of lane q + t) and each lane adds every row to the moments of its own channel ----
-    double qR[kNepMaxN];                      // radial descriptors: partial sums over this lane's rows, then all of them
-#pragma unroll
-    for (int n = 0; n < kNepMaxN; ++n) qR[n] = 0.0;
     double qA[2][kNepMaxL] = {};              // angular descriptors of the channels n = q, q + 4
     const int npass = (sp.na + 3) / 4;
     for (int pass = 0; pass < npass; ++pass) {
@@ -182,32 +336,18 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
             double dx = 0.0, dy = 0.0, dz = 0.0, r2 = 1e300;
             if (kk < cnt) r2 = pair_vec(kk, J, dx, dy, dz);
             double x = 0.0, y = 0.0, z = 0.0, g4[4] = {0.0, 0.0, 0.0, 0.0};
-            if (r2 < rcr2) {
+            if (r2 < rca2) {
                 const double inv = rsqrt(r2), r = r2 * inv;
                 x = dx * inv; y = dy * inv; z = dz * inv;
-                if (pass == 0) {
-                    double f[KMAX], df[KMAX];
-                    nep_basis<KMAX>(r * ircr, ircr, sp.kr, f, df);
-                    const double *c = cRb + (size_t)J * kNepMaxN * KMAX;
+                double f[KMAX], df[KMAX];
+                nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
 #pragma unroll
-                    for (int nn = 0; nn < kNepMaxN; ++nn) {
-                        double g = 0.0;
+                for (int c4 = 0; c4 < 4; ++c4) {
+                    const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
+                    double g = 0.0;
 #pragma unroll
-                        for (int b = 0; b < KMAX; ++b) g += c[nn * KMAX + b] * f[b];
-                        qR[nn] += g;
-                    }
-                }
-                if (r2 < rca2) {
-                    double f[KMAX], df[KMAX];
-                    nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
-#pragma unroll
-                    for (int c4 = 0; c4 < 4; ++c4) {
-                        const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
-                        double g = 0.0;
-#pragma unroll
-                        for (int b = 0; b < KMAX; ++b) g += c[b] * f[b];
-                        g4[c4] = g;
-                    }
+                    for (int b = 0; b < KMAX; ++b) g += c[b] * f[b];
+                    g4[c4] = g;
                 }
             }
             const double inA = r2 < rca2 ? 1.0 : 0.0;
@@ -241,75 +381,67 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
             qA[pass][3] = 0.125 * (35.0 * A[4] - 30.0 * A[2] + 3.0 * A[0]);
         }
     }
-#pragma unroll
-    for (int n = 0; n < kNepMaxN; ++n) qR[n] = quad_sum(qR[n]);  // every lane now holds all radial descriptors
-
-    // ---- the network: each lane takes the neurons mu = q, q + 4, ...; the angular descriptors come from their owners ----
+    // ---- the network: each lane takes the neurons mu = q, q + 4, ...; the radial descriptors come from
+    // nep_radial_desc_kernel (Dev::nep_q), the angular ones from their owners in the quad.  Weights in shared memory
+    // as W0t[d][mu] with the neurons zero-padded to a multiple of four: a padded neuron has tanh(0) = 0 and W1 = 0 ----
     double ui = 0.0;
-    double FdR[kNepMaxN], FdA[2][kNepMaxL] = {};
-#pragma unroll
-    for (int n = 0; n < kNepMaxN; ++n) FdR[n] = 0.0;
+    double FdA[2][kNepMaxL] = {};
     {
+        const int nt = Hp >> 2;  // neurons per lane
         double zt[kNepMaxH / 4];
 #pragma unroll
-        for (int t = 0; t < kNepMaxH / 4; ++t) {
-            const int mu = q + 4 * t;
-            zt[t] = mu < sp.H ? -b0[mu] : 0.0;
-        }
-        for (int dsc = 0; dsc < sp.D; ++dsc) {
-            double v;
-            if (dsc < sp.nr) {
-                v = 0.0;
+        for (int t = 0; t < kNepMaxH / 4; ++t) zt[t] = t < nt ? -b0[q + 4 * t] : 0.0;
+        // the descriptors of the quad's atom, side by side in shared memory (one short loop instead of an unrolled
+        // ladder of shuffles)
+        double *sq = sQ + (threadIdx.x >> 2) * (kNepMaxD + 1);  // odd stride: the quads of a warp on distinct banks
+        for (int n = q; n < sp.nr; n += 4) sq[n] = valid ? qscr[(size_t)n * d.Npad] : 0.0;
 #pragma unroll
-                for (int n = 0; n < kNepMaxN; ++n)
-                    if (n == dsc) v = qR[n];
-            } else {
-                const int n = (dsc - sp.nr) / sp.L, ll = (dsc - sp.nr) % sp.L, hh = n >> 2;
-                double mine = hh ? qA[1][0] : qA[0][0];
-                if (ll == 1) mine = hh ? qA[1][1] : qA[0][1];
-                if (ll == 2) mine = hh ? qA[1][2] : qA[0][2];
-                if (ll == 3) mine = hh ? qA[1][3] : qA[0][3];
-                v = shf(mine, n & 3);
-            }
+        for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+            for (int ll = 0; ll < kNepMaxL; ++ll)
+                if (q + 4 * hh < sp.na && ll < sp.L) sq[sp.nr + (q + 4 * hh) * sp.L + ll] = qA[hh][ll];
+        __syncwarp();
+        for (int dsc = 0; dsc < sp.D; ++dsc) {
+            const double v = sq[dsc];
+            const double *w = W0t + dsc * Hp + q;
 #pragma unroll
             for (int t = 0; t < kNepMaxH / 4; ++t) {
-                const int mu = q + 4 * t;
-                if (mu < sp.H) zt[t] += W0[mu * sp.D + dsc] * v;
+                if (t >= nt) break;
+                zt[t] = fma(w[4 * t], v, zt[t]);
             }
         }
+        __syncwarp();
         double gmu[kNepMaxH / 4];
 #pragma unroll
         for (int t = 0; t < kNepMaxH / 4; ++t) {
-            const int mu = q + 4 * t;
             gmu[t] = 0.0;
-            if (mu < sp.H) {
-                const double th = tanh(zt[t]);
-                ui += W1[mu] * th;
-                gmu[t] = W1[mu] * (1.0 - th * th);
+            if (t < nt) {
+                const double th = tanh(zt[t]), w1 = W1[q + 4 * t];
+                ui = fma(w1, th, ui);
+                gmu[t] = w1 * (1.0 - th * th);
             }
         }
         // dU/dq_d = sum_mu gmu W0[mu][d]: partial over this lane's neurons, summed over the quad
+        // (the radial ones go to nep_radial_force_kernel through Dev::nep_q, the angular ones back to their owners)
         for (int dsc = 0; dsc < sp.D; ++dsc) {
+            const double *w = W0t + dsc * Hp + q;
             double v = 0.0;
 #pragma unroll
             for (int t = 0; t < kNepMaxH / 4; ++t) {
-                const int mu = q + 4 * t;
-                if (mu < sp.H) v += gmu[t] * W0[mu * sp.D + dsc];
+                if (t >= nt) break;
+                v = fma(gmu[t], w[4 * t], v);
             }
             v = quad_sum(v);
-            if (dsc < sp.nr) {
-#pragma unroll
-                for (int n = 0; n < kNepMaxN; ++n)
-                    if (n == dsc) FdR[n] = v;  // all lanes keep the radial ones
-            } else {
-                const int n = (dsc - sp.nr) / sp.L, ll = (dsc - sp.nr) % sp.L;
-                if ((n & 3) == q) {
-#pragma unroll
-                    for (int l2 = 0; l2 < kNepMaxL; ++l2)
-                        if (l2 == ll) { if (n >> 2) FdA[1][l2] = v; else FdA[0][l2] = v; }
-                }
-            }
+            if (q == (dsc & 3)) sq[dsc] = v;
         }
+        __syncwarp();
+        for (int n = q; n < sp.nr; n += 4)
+            if (valid) qscr[(size_t)n * d.Npad] = sq[n];
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh)
+#pragma unroll
+            for (int ll = 0; ll < kNepMaxL; ++ll)
+                if (q + 4 * hh < sp.na && ll < sp.L) FdA[hh][ll] = sq[sp.nr + (q + 4 * hh) * sp.L + ll];
         ui = quad_sum(ui);
         if (q != 0 || !valid) ui = 0.0;  // one lane per atom carries the site energy
     }
@@ -339,36 +471,20 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
             if (kk < cnt) r2 = pair_vec(kk, J, dx, dy, dz);
             double x = 0.0, y = 0.0, z = 0.0, inv = 0.0, g4[4] = {0.0, 0.0, 0.0, 0.0}, dg4[4] = {0.0, 0.0, 0.0, 0.0};
             double px = 0.0, py = 0.0, pz = 0.0;
-            if (r2 < rcr2) {
+            if (r2 < rca2) {
                 inv = rsqrt(r2);
                 const double r = r2 * inv;
                 x = dx * inv; y = dy * inv; z = dz * inv;
-                if (pass == 0) {  // radial descriptors: sum_n Fd_n g'_n(r) u
-                    double f[KMAX], df[KMAX];
-                    nep_basis<KMAX>(r * ircr, ircr, sp.kr, f, df);
-                    const double *c = cRb + (size_t)J * kNepMaxN * KMAX;
-                    double sr = 0.0;
+                double f[KMAX], df[KMAX];
+                nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
 #pragma unroll
-                    for (int nn = 0; nn < kNepMaxN; ++nn) {
-                        double dg = 0.0;
+                for (int c4 = 0; c4 < 4; ++c4) {
+                    const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
+                    double g = 0.0, dg = 0.0;
 #pragma unroll
-                        for (int b = 0; b < KMAX; ++b) dg += c[nn * KMAX + b] * df[b];
-                        sr += FdR[nn] * dg;
-                    }
-                    px = sr * x; py = sr * y; pz = sr * z;
-                }
-                if (r2 < rca2) {
-                    double f[KMAX], df[KMAX];
-                    nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
-#pragma unroll
-                    for (int c4 = 0; c4 < 4; ++c4) {
-                        const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
-                        double g = 0.0, dg = 0.0;
-#pragma unroll
-                        for (int b = 0; b < KMAX; ++b) { g += c[b] * f[b]; dg += c[b] * df[b]; }
-                        g4[c4] = g;
-                        dg4[c4] = dg;
-                    }
+                    for (int b = 0; b < KMAX; ++b) { g += c[b] * f[b]; dg += c[b] * df[b]; }
+                    g4[c4] = g;
+                    dg4[c4] = dg;
                 }
             }
             const double inA = r2 < rca2 ? 1.0 : 0.0;
@@ -433,24 +549,40 @@ void nep_fill_weights(const double *pot, double *w) {
         z ^= z >> 31;
         return 2.0 * ((double)(z >> 11) * (1.0 / 9007199254740992.0)) - 1.0;
     };
-    for (int I = 0; I < s.T; ++I) {
+    const int Hp = nep_hp(s);
+    for (int I = 0; I < s.T; ++I) {  // stream order: W0[mu][d], b0[mu], W1[mu]
         double *net = w + (size_t)I * nep_net_size(s);
-        for (int t = 0; t < s.H * s.D; ++t) net[t] = next() * ((t % s.D) < s.nr ? 0.04 : 0.004);
-        for (int t = 0; t < s.H; ++t) net[s.H * s.D + t] = 0.5 * next();
-        for (int t = 0; t < s.H; ++t) net[s.H * s.D + s.H + t] = next();
+        for (int t = 0; t < nep_net_size(s); ++t) net[t] = 0.0;
+        for (int t = 0; t < s.H * s.D; ++t) net[(t % s.D) * Hp + t / s.D] = next() * ((t % s.D) < s.nr ? 0.04 : 0.004);
+        for (int t = 0; t < s.H; ++t) net[s.D * Hp + t] = 0.5 * next();
+        for (int t = 0; t < s.H; ++t) net[s.D * Hp + Hp + t] = next();
     }
     double *c = w + (size_t)s.T * nep_net_size(s);
     const int nc = s.T * s.T * (s.nr * s.kr + s.na * s.ka);
     for (int t = 0; t < nc; ++t) c[t] = next();
 }
 
+template <int KMAX>
+static void launch_nep_radial(const Dev &d, int p_lo, dim3 grid, bool force, cudaStream_t st) {
+    const int nt = (int)d.pot[8];
+    if (force) {
+        if (nt <= 1) nep_radial_force_kernel<KMAX, 1><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
+        else nep_radial_force_kernel<KMAX, 2><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
+    } else {
+        if (nt <= 1) nep_radial_desc_kernel<KMAX, 1><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
+        else nep_radial_desc_kernel<KMAX, 2><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
+    }
+}
+
+// Pass 1 in three launches: radial descriptors (one atom per thread, all live rows), the quad kernel (angular rows,
+// network, angular partial forces), the radial partial forces (one atom per thread); then pass 2 (kernels_sw.cu).
 void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
-    dim3 grid(d.nblk_force, nimg);
     const NepShape sp = nep_shape(d.pot);
-    const int kmax = (int)(d.pot[4] > d.pot[5] ? d.pot[4] : d.pot[5]), KM = kmax <= 4 ? 4 : kmax <= 8 ? 8 : 12;
-    const size_t smem = ((size_t)((sp.T * nep_net_size(sp) + 1) & ~1) + 2 * (size_t)sp.T * sp.T * kNepMaxN * KM) * sizeof(double);
+    const dim3 grid(d.nblk_force, nimg), grid_r((d.N + kNepRadialThreads - 1) / kNepRadialThreads, nimg);
+    const int KR = sp.kr <= 4 ? 4 : sp.kr <= 8 ? 8 : 12, KA = sp.ka <= 4 ? 4 : sp.ka <= 8 ? 8 : 12;
+    const size_t smem = ((size_t)((sp.T * nep_net_size(sp) + 1) & ~1) + (size_t)sp.T * sp.T * kNepMaxN * KA) * sizeof(double);
     static bool attr_set = false;
     if (!attr_set) {
         cudaFuncSetAttribute(nep_partial_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
@@ -458,9 +590,15 @@ void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st) {
         cudaFuncSetAttribute(nep_partial_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
         attr_set = true;
     }
-    if (kmax <= 4) nep_partial_kernel<4><<<grid, kNepThreads, smem, st>>>(d, p_lo);
-    else if (kmax <= 8) nep_partial_kernel<8><<<grid, kNepThreads, smem, st>>>(d, p_lo);
-    else nep_partial_kernel<12><<<grid, kNepThreads, smem, st>>>(d, p_lo);
+    for (int force = 0; force < 2; ++force) {
+        if (KR == 4) launch_nep_radial<4>(d, p_lo, grid_r, force, st);
+        else if (KR == 8) launch_nep_radial<8>(d, p_lo, grid_r, force, st);
+        else launch_nep_radial<12>(d, p_lo, grid_r, force, st);
+        if (force) break;
+        if (KA == 4) nep_partial_kernel<4><<<grid, kNepThreads, smem, st>>>(d, p_lo);
+        else if (KA == 8) nep_partial_kernel<8><<<grid, kNepThreads, smem, st>>>(d, p_lo);
+        else nep_partial_kernel<12><<<grid, kNepThreads, smem, st>>>(d, p_lo);
+    }
     launch_pair_forces_manybody(d, p_lo, st);
 }
 
