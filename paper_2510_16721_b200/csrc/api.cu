@@ -174,6 +174,8 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
              : prm->potential == CFNEB_POT_NEP ? c.take<double>(nep_weight_count(prm->pot)) : nullptr;
     d.types = prm->potential == CFNEB_POT_NEP ? c.take<int>(Npad) : nullptr;
     d.nep_q = prm->potential == CFNEB_POT_NEP ? c.take<double>(S * (size_t)8 * Npad) : nullptr;
+    d.nep_kr_pad = prm->potential == CFNEB_POT_NEP ? nep_kr_padded(prm->pot) : 0;
+    d.nep_w = prm->potential == CFNEB_POT_NEP ? c.take<double>(S * (size_t)Npad * (size_t)prm->pot[8] * d.nep_kr_pad) : nullptr;
     d.nep_S = prm->potential == CFNEB_POT_NEP ? c.take<double>(S * (size_t)prm->pot[3] * 35 * Npad) : nullptr;
     d.bin_count = c.take<int>(S * ((size_t)d.nbins_max + 1));
     d.bin_cursor = c.take<int>(S * (size_t)d.nbins_max);

@@ -137,7 +137,9 @@ struct Dev {
     int edge_b0;              // first inner bucket edge kept: the last one at or below the inner radius (NEP: rc_a)
     double *dn_w;               // [kDnWeights] W0[H][D], b0[H], W1[H] of CFNEB_POT_DNN; CFNEB_POT_NEP: see kernels_nep.cu
     int *types;                 // [Npad] atom types in storage order (CFNEB_POT_NEP)
-    double *nep_q;              // [S][8][Npad] radial descriptors q_n (radial kernel 1 -> quad kernel), then dU/dq_n (-> radial kernel 2)
+    double *nep_q;              // [S][8][Npad] radial descriptors q_n (nep_radial_desc_kernel -> quad kernel)
+    double *nep_w;              // [S][Npad][n_types][nep_kr_pad] w_i[J][k] = sum_n dU_i/dq_n cR[I][J][n][k] (quad kernel -> nep_radial_pair_kernel)
+    int nep_kr_pad;             // k_r rounded up to 4, 8 or 12
     double *nep_S;              // [S][n_a][35][Npad] moments of the angular channels between the two walks (CFNEB_POT_NEP)
     unsigned short *nbr_mirror; // [S][cap][Npad] row of the mirror entry (j; i, -n) of each entry (many-body potentials only)
     double *part;             // [S][cap][3][Npad] partial forces p^ij = dU_i/dr^ij per list entry (many-body potentials only)
@@ -211,6 +213,7 @@ void launch_mirror_sw(const Dev &d, int p_lo, cudaStream_t st);                 
 void launch_force_dn(const Dev &d, int p_lo, cudaStream_t st);                            // K2, descriptor network (kernels_dn.cu)
 void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st);                           // K2, NEP-shaped potential (kernels_nep.cu)
 int nep_weight_count(const double *pot);
+int nep_kr_padded(const double *pot);
 void nep_fill_weights(const double *pot, double *w);  // host: the SplitMix64 weight stream of include/cfneb.h
 void launch_pair_forces_manybody(const Dev &d, int p_lo, cudaStream_t st);                // pass 2 of both (kernels_sw.cu)
 void launch_force_sw(const Dev &d, int p_lo, cudaStream_t st);                            // K2, Stillinger-Weber (kernels_sw.cu)                               // K2
@@ -260,6 +263,27 @@ __device__ inline int live_rows(const Dev &d, int slot, int i) {
     const int t_dead = first_dead_tail_bucket(d.r_cut, d.r_list, d.geom[slot].acc);
     return t_dead < kTailBuckets ? (int)d.nbr_tail[((size_t)slot * kTailBuckets + t_dead) * d.Npad + i]
                                  : d.nbr_count[(size_t)slot * d.Npad + i];
+}
+
+// Rows of atom i's (distance-sorted) list that can hold a pair inside the angular cut-off now: everything before the
+// first kept inner bucket edge that is at least rc_a + acc (built at or beyond that edge, moved by at most acc since:
+// the reasoning of live_rows).  All live rows when no kept edge is far enough.
+__device__ inline int nep_angular_rows(const Dev &d, int slot, int i) {
+    const double rc2 = d.r_cut * d.r_cut, need = d.pot[1] + d.geom[slot].acc + 1e-9 * d.r_cut;
+    for (int e = 0; e < kEdgeRows; ++e) {
+        const int b = d.edge_b0 + e;
+        if (b <= kInnerBuckets && sqrt(rc2 * b / kInnerBuckets) >= need)
+            return min((int)d.nbr_edge[((size_t)slot * kEdgeRows + e) * d.Npad + i], d.cap);
+    }
+    return live_rows(d, slot, i);
+}
+
+// 1/sqrt(x) for normal x > 0: hardware seed (2^-22) + one cubically convergent step; no special cases.
+__device__ __forceinline__ double rsqrt_nr(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-(x * y), y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
 }
 
 __device__ inline void set_error(Ctl *ctl, int code) { atomicCAS(&ctl->error, 0, code); }

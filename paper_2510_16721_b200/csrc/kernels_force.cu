@@ -70,14 +70,6 @@ __device__ __forceinline__ void pair_vec(const double4 &ri, const double4 &rj, u
     r2 = fma(dz, dz, fma(dy, dy, dx * dx));
 }
 
-// 1/sqrt(x) for normal x > 0: hardware seed (2^-22) + one cubically convergent step; no special cases.
-__device__ __forceinline__ double rsqrt_nr(double x) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double e = fma(-(x * y), y, 1.0);
-    return fma(y * e, fma(0.375, e, 0.5), y);
-}
-
 // exp(x) for |x| < 700 (pair arguments are O(1)):  x = (32 k + j) ln2/32 + r,  exp(x) = 2^k T[j] e^r with
 // T[j] = 2^(j/32) from a 32-entry table in shared memory and e^r - 1 = r + r^2 (1/2 + r/6 + ... + r^4/720) on
 // |r| <= ln2/64 (remainder 3.5e-18); 2^k by exponent arithmetic.  11 fp64 instructions instead of the 17 of a

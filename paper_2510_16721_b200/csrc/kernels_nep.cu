@@ -47,9 +47,9 @@ __host__ __device__ inline NepShape nep_shape(const double *pot) {
     return s;
 }
 // layout of Dev::dn_w for this potential: per type [W0t D*Hp | b0 Hp | W1 Hp] (first layer transposed to [d][mu], the
-// neurons zero-padded to Hp, a multiple of four: the quad kernel copies it to shared memory as it is), then
+// neurons zero-padded to Hp, a multiple of eight: the quad kernel copies it to shared memory as it is), then
 // cR [T][T][nr][kr], then cA [T][T][na][ka]
-__host__ __device__ inline int nep_hp(const NepShape &s) { return (s.H + 3) & ~3; }
+__host__ __device__ inline int nep_hp(const NepShape &s) { return (s.H + 7) & ~7; }
 __host__ __device__ inline int nep_net_size(const NepShape &s) { return s.D * nep_hp(s) + 2 * nep_hp(s); }
 __host__ __device__ inline int nep_weights_size(const NepShape &s) {
     return s.T * nep_net_size(s) + s.T * s.T * (s.nr * s.kr + s.na * s.ka);
@@ -83,33 +83,23 @@ __device__ __forceinline__ void nep_basis(double t, double irc, int K, double (&
 
 __device__ __forceinline__ const double4 *Rc_of(const Dev &d, int slot) { return d.Rc + (size_t)slot * d.Npad; }
 
-// Rows of atom i's (distance-sorted) list that can hold a pair inside the angular cut-off now: everything before the
-// first kept inner bucket edge that is at least rc_a + acc (built at or beyond that edge, moved by at most acc since:
-// the reasoning of live_rows).  All live rows when no kept edge is far enough.
-__device__ inline int nep_angular_rows(const Dev &d, int slot, int i) {
-    const double rc2 = d.r_cut * d.r_cut, need = d.pot[1] + d.geom[slot].acc + 1e-9 * d.r_cut;
-    for (int e = 0; e < kEdgeRows; ++e) {
-        const int b = d.edge_b0 + e;
-        if (b <= kInnerBuckets && sqrt(rc2 * b / kInnerBuckets) >= need)
-            return min((int)d.nbr_edge[((size_t)slot * kEdgeRows + e) * d.Npad + i], d.cap);
-    }
-    return live_rows(d, slot, i);
-}
-
-// One atom per thread over all live rows of its list, entry two rows and sector one row ahead of use:
-// body(k, rj, dx, dy, dz, r2) for the rows k < cnt of this thread (rj.w = type of the neighbour).
+// One atom per thread over all live rows of its list, the loads software-pipelined:
+// body(k, j, rj, dx, dy, dz, r2) for the rows k < cnt of this thread (rj.w = type of the neighbour j).
 template <class Body>
 __device__ __forceinline__ void nep_walk_rows(const Dev &d, const uint32_t *lp, const double4 *Rc, const double4 &ri,
                                               const double *sh, int cnt, Body body) {
     if (cnt <= 0) return;
-    uint32_t e0 = lp[0], e1 = lp[(size_t)min(1, cnt - 1) * d.Npad];
-    double4 rj = Rc[e0 & kIdxMask];
+    const int last = cnt - 1;
+    // entries three rows and sectors two rows ahead of use (row indices clamped to the last row)
+    uint32_t e0 = lp[0], e1 = lp[(size_t)min(1, last) * d.Npad], e2 = lp[(size_t)min(2, last) * d.Npad];
+    double4 r0 = Rc[e0 & kIdxMask], r1 = Rc[e1 & kIdxMask];
     for (int k = 0; k < cnt; ++k) {
-        const uint32_t code = e0 >> kShiftBits;
-        const double4 rc = rj;
-        e0 = e1;
-        e1 = lp[(size_t)min(k + 2, cnt - 1) * d.Npad];
-        rj = Rc[e0 & kIdxMask];
+        const uint32_t code = e0 >> kShiftBits, j = e0 & kIdxMask;
+        const double4 rc = r0;
+        e0 = e1; e1 = e2;
+        e2 = lp[(size_t)min(k + 3, last) * d.Npad];
+        r0 = r1;
+        r1 = Rc[e1 & kIdxMask];
         double dx = rc.x - ri.x, dy = rc.y - ri.y, dz = rc.z - ri.z;
         if (code != kCodeCenter) {
             const double n0 = (double)((int)(code & 7u) - 4), n1 = (double)((int)((code >> 3) & 7u) - 4),
@@ -118,7 +108,7 @@ __device__ __forceinline__ void nep_walk_rows(const Dev &d, const uint32_t *lp, 
             dy += n0 * sh[1] + n1 * sh[4] + n2 * sh[7];
             dz += n0 * sh[2] + n1 * sh[5] + n2 * sh[8];
         }
-        body(k, rc, dx, dy, dz, dx * dx + dy * dy + dz * dz);
+        body(k, j, rc, dx, dy, dz, dx * dx + dy * dy + dz * dz);
     }
 }
 
@@ -150,10 +140,10 @@ __global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) ne
 #pragma unroll
         for (int k = 0; k < KMAX; ++k) B[J][k] = 0.0;
     nep_walk_rows(d, d.nbr_list + (size_t)slot * d.cap * d.Npad + i, Rc, ri, sh, live_rows(d, slot, i),
-                  [&](int, const double4 &rj, double, double, double, double r2) {
+                  [&](int, uint32_t, const double4 &rj, double, double, double, double r2) {
         if (r2 < rcr2) {
             double f[KMAX], df[KMAX];
-            nep_basis<KMAX>(r2 * rsqrt(r2) * ircr, ircr, sp.kr, f, df);
+            nep_basis<KMAX>(r2 * rsqrt_nr(r2) * ircr, ircr, sp.kr, f, df);
             if (NT == 1) {
 #pragma unroll
                 for (int k = 0; k < KMAX; ++k) B[0][k] += f[k];
@@ -181,61 +171,72 @@ __global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) ne
     }
 }
 
-// Radial part of the partial forces, p^ij += sum_n dU/dq_n g_n'(r_ij) u_ij = [sum_k w[J][k] f_k'(r_ij)] u_ij with
-// w[J][k] = sum_n dU/dq_n cR[I][J][n][k] formed once per atom (dU/dq_n from the quad kernel in Dev::nep_q).  One atom
-// per thread over all live rows; the rows below the angular count already hold the angular part (quad kernel).
+// Radial part of the forces, pair by pair (no partial forces stored): p^ij = [sum_k w_i[J][k] f_k'(r_ij)] u_ij with
+// w_i[J][k] = sum_n dU_i/dq_n cR[I][J][n][k] (formed once per atom by the quad kernel, Dev::nep_w), and the mirror term
+// of Eq. 5 is the same expression with j's coefficients for i's type, so
+//   f^ij = p^ij - p^ji = [sum_k (w_i[J][k] + w_j[I][k]) f_k'(r_ij)] u_ij
+// needs one 8 k_r-byte gather per row instead of a stored partial force and its mirror.  One atom per thread over all
+// live rows; writes F_i and the virial partials of this part, the angular part is added by pass 2 (kernels_sw.cu).
 template <int KMAX, int NT>
-__global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) nep_radial_force_kernel(Dev d, int p_lo) {
+__global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) nep_radial_pair_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
     __shared__ double sh[9];
+    __shared__ double red[32 * 6];
+    __shared__ double2 sWi[NT * (KMAX / 2) * kNepRadialThreads];  // this thread's w_i[J][k], two k per entry, thread-minor
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= d.N) return;
+    const bool valid = i < d.N;
     const NepShape sp = nep_shape(d.pot);
     const double rcr = d.pot[0], rcr2 = rcr * rcr, ircr = 1.0 / rcr;
     const double4 *Rc = Rc_of(d, slot);
-    const double4 ri = Rc[i];
-    const int I = (int)ri.w;
-    const double *cR = d.dn_w + sp.T * nep_net_size(sp) + (size_t)I * sp.T * sp.nr * sp.kr;  // [J][n][k]
-    const double *qscr = d.nep_q + (size_t)slot * kNepMaxN * d.Npad + i;
-    double w[NT][KMAX];
+    const double *wv = d.nep_w + (size_t)slot * d.Npad * (NT * KMAX);  // wv[(j * NT + J) * KMAX + k]
+    double fx = 0.0, fy = 0.0, fz = 0.0, vxx = 0.0, vyy = 0.0, vzz = 0.0, vxy = 0.0, vxz = 0.0, vyz = 0.0;
+    if (valid) {
+        const double4 ri = Rc[i];
+        const int I = (int)ri.w;
 #pragma unroll
-    for (int J = 0; J < NT; ++J)
+        for (int t = 0; t < NT * (KMAX / 2); ++t)
+            sWi[t * kNepRadialThreads + threadIdx.x] = reinterpret_cast<const double2 *>(wv + (size_t)i * NT * KMAX)[t];
+        nep_walk_rows(d, d.nbr_list + (size_t)slot * d.cap * d.Npad + i, Rc, ri, sh, live_rows(d, slot, i),
+                      [&](int, uint32_t j, const double4 &rj, double dx, double dy, double dz, double r2) {
+            if (r2 < rcr2) {
+                const double2 *wj = reinterpret_cast<const double2 *>(wv + ((size_t)j * NT + I) * KMAX);
+                double2 wjk[KMAX / 2];
 #pragma unroll
-        for (int k = 0; k < KMAX; ++k) w[J][k] = 0.0;
-    for (int n = 0; n < sp.nr; ++n) {
-        const double Fd = qscr[(size_t)n * d.Npad];
+                for (int k = 0; k < KMAX / 2; ++k) wjk[k] = wj[k];
+                const double inv = rsqrt_nr(r2);
+                double f[KMAX], df[KMAX];
+                nep_basis<KMAX>(r2 * inv * ircr, ircr, sp.kr, f, df);
+                const double2 *wi = sWi + (NT > 1 ? (int)rj.w : 0) * (KMAX / 2) * kNepRadialThreads + threadIdx.x;
+                double sa = 0.0, sb = 0.0;
 #pragma unroll
-        for (int J = 0; J < NT; ++J)
-#pragma unroll
-            for (int k = 0; k < KMAX; ++k)
-                if (k < sp.kr) w[J][k] = fma(Fd, cR[(J * sp.nr + n) * sp.kr + k], w[J][k]);
-    }
-    const int cntA = nep_angular_rows(d, slot, i);
-    double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad + i;  // part[(k * 3 + m) * Npad]
-    nep_walk_rows(d, d.nbr_list + (size_t)slot * d.cap * d.Npad + i, Rc, ri, sh, live_rows(d, slot, i),
-                  [&](int k, const double4 &rj, double dx, double dy, double dz, double r2) {
-        double *o = part + (size_t)(k * 3) * d.Npad;
-        double px = 0.0, py = 0.0, pz = 0.0;
-        if (k < cntA) { px = o[0]; py = o[d.Npad]; pz = o[2 * (size_t)d.Npad]; }
-        if (r2 < rcr2) {
-            const double inv = rsqrt(r2);
-            double f[KMAX], df[KMAX];
-            nep_basis<KMAX>(r2 * inv * ircr, ircr, sp.kr, f, df);
-            double s0 = 0.0, s1 = 0.0;
-#pragma unroll
-            for (int k2 = 0; k2 < KMAX; ++k2) {
-                s0 = fma(w[0][k2], df[k2], s0);
-                if (NT > 1) s1 = fma(w[NT - 1][k2], df[k2], s1);
+                for (int k = 0; k < KMAX / 2; ++k) {
+                    const double2 a = wi[k * kNepRadialThreads];
+                    sa = fma(a.x + wjk[k].x, df[2 * k], sa);
+                    sb = fma(a.y + wjk[k].y, df[2 * k + 1], sb);
+                }
+                const double sr = (sa + sb) * inv;
+                const double gx = sr * dx, gy = sr * dy, gz = sr * dz;  // f^ij of Eq. 5, radial part
+                fx += gx; fy += gy; fz += gz;
+                vxx = fma(dx, gx, vxx); vyy = fma(dy, gy, vyy); vzz = fma(dz, gz, vzz);  // Eq. 8 (central: symmetric)
+                vxy = fma(dx, gy, vxy); vxz = fma(dx, gz, vxz); vyz = fma(dy, gz, vyz);
             }
-            const double sr = (NT > 1 ? fma(rj.w, s1 - s0, s0) : s0) * inv;
-            px = fma(sr, dx, px); py = fma(sr, dy, py); pz = fma(sr, dz, pz);
-        }
-        o[0] = px; o[d.Npad] = py; o[2 * (size_t)d.Npad] = pz;
-    });
+        });
+        double *F = d.F + (size_t)slot * 3 * d.Npad;
+        F[i] = fx; F[d.Npad + i] = fy; F[2 * (size_t)d.Npad + i] = fz;
+    }
+    double out6[6] = {-0.5 * vxx, -0.5 * vyy, -0.5 * vzz, -0.5 * vxy, -0.5 * vxz, -0.5 * vyz};
+    block_sum<6>(out6, red);
+    if (threadIdx.x == 0) {
+        double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
+        out[0] = 0.0;
+#pragma unroll
+        for (int n = 0; n < 6; ++n) out[1 + n] = out6[n];
+        out[8] = 0.0;
+    }
 }
 
 // KMAX: basis functions held per row (the smallest of 4, 8, 12 that covers k_r and k_a): the loops over them are
@@ -245,7 +246,7 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
     const int slot = d.order[p];
-    extern __shared__ double sW[];  // all weights of the potential
+    extern __shared__ __align__(16) double sW[];  // all weights of the potential
     __shared__ double sh[9];
     __shared__ double red[64];
     __shared__ double sQ[(kNepThreads / 4) * (kNepMaxD + 1)];  // descriptors, then their gradients, one row per quad
@@ -311,7 +312,6 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     };
 
     const int base_lane = (threadIdx.x & 31) & ~3;
-    auto sel4 = [](const double (&a)[4], int c) { return c == 0 ? a[0] : c == 1 ? a[1] : c == 2 ? a[2] : a[3]; };
     auto shf = [&](double v, int src) { return __shfl_sync(quad_mask, v, base_lane + src); };
     auto quad_sum = [&](double v) {
         v += __shfl_xor_sync(quad_mask, v, 1);
@@ -337,13 +337,13 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
             if (kk < cnt) r2 = pair_vec(kk, J, dx, dy, dz);
             double x = 0.0, y = 0.0, z = 0.0, g4[4] = {0.0, 0.0, 0.0, 0.0};
             if (r2 < rca2) {
-                const double inv = rsqrt(r2), r = r2 * inv;
+                const double inv = rsqrt_nr(r2), r = r2 * inv;
                 x = dx * inv; y = dy * inv; z = dz * inv;
                 double f[KMAX], df[KMAX];
                 nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
 #pragma unroll
-                for (int c4 = 0; c4 < 4; ++c4) {
-                    const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
+                for (int c4 = 0; c4 < 4; ++c4) {  // g4[t]: the channel that lane q - t owns, read by it in step t
+                    const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + ((q - c4) & 3)) * KMAX;
                     double g = 0.0;
 #pragma unroll
                     for (int b = 0; b < KMAX; ++b) g += c[b] * f[b];
@@ -354,9 +354,9 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
                 const int src = (q + t) & 3;
-                // the value lane src wants from this lane in step t is the g of ITS channel: lane src = q + t reads q's
-                // register, so q presents g4[(q - t) & 3]... seen from the reader: it reads g4[own channel] of lane src
-                const double gs = t == 0 ? sel4(g4, q) : shf(sel4(g4, (q - t) & 3), src);
+                // step t: this lane reads from lane src = q + t the g of its own channel, which that lane holds as
+                // its g4[t] (channel (src - t) & 3 = q)
+                const double gs = t == 0 ? g4[0] : shf(g4[t], src);
                 const double xs = t == 0 ? x : shf(x, src), ys = t == 0 ? y : shf(y, src), zs = t == 0 ? z : shf(z, src);
                 const double as = t == 0 ? inA : shf(inA, src);
                 if (own && as != 0.0) {
@@ -381,16 +381,16 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
             qA[pass][3] = 0.125 * (35.0 * A[4] - 30.0 * A[2] + 3.0 * A[0]);
         }
     }
-    // ---- the network: each lane takes the neurons mu = q, q + 4, ...; the radial descriptors come from
+    // ---- the network: each lane takes a quarter of the neurons; the radial descriptors come from
     // nep_radial_desc_kernel (Dev::nep_q), the angular ones from their owners in the quad.  Weights in shared memory
-    // as W0t[d][mu] with the neurons zero-padded to a multiple of four: a padded neuron has tanh(0) = 0 and W1 = 0 ----
+    // as W0t[d][mu] with the neurons zero-padded to a multiple of eight: a padded neuron has tanh(0) = 0 and W1 = 0 ----
     double ui = 0.0;
     double FdA[2][kNepMaxL] = {};
     {
-        const int nt = Hp >> 2;  // neurons per lane
+        const int nt = Hp >> 2;  // neurons per lane (even): lane q takes mu = q nt .. q nt + nt - 1, read two at a time
         double zt[kNepMaxH / 4];
 #pragma unroll
-        for (int t = 0; t < kNepMaxH / 4; ++t) zt[t] = t < nt ? -b0[q + 4 * t] : 0.0;
+        for (int t = 0; t < kNepMaxH / 4; ++t) zt[t] = t < nt ? -b0[q * nt + t] : 0.0;
         // the descriptors of the quad's atom, side by side in shared memory (one short loop instead of an unrolled
         // ladder of shuffles)
         double *sq = sQ + (threadIdx.x >> 2) * (kNepMaxD + 1);  // odd stride: the quads of a warp on distinct banks
@@ -403,11 +403,13 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
         __syncwarp();
         for (int dsc = 0; dsc < sp.D; ++dsc) {
             const double v = sq[dsc];
-            const double *w = W0t + dsc * Hp + q;
+            const double2 *w = reinterpret_cast<const double2 *>(W0t + dsc * Hp + q * nt);
 #pragma unroll
-            for (int t = 0; t < kNepMaxH / 4; ++t) {
+            for (int t = 0; t < kNepMaxH / 4; t += 2) {
                 if (t >= nt) break;
-                zt[t] = fma(w[4 * t], v, zt[t]);
+                const double2 ww = w[t >> 1];
+                zt[t] = fma(ww.x, v, zt[t]);
+                zt[t + 1] = fma(ww.y, v, zt[t + 1]);
             }
         }
         __syncwarp();
@@ -416,27 +418,41 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
         for (int t = 0; t < kNepMaxH / 4; ++t) {
             gmu[t] = 0.0;
             if (t < nt) {
-                const double th = tanh(zt[t]), w1 = W1[q + 4 * t];
+                const double th = tanh(zt[t]), w1 = W1[q * nt + t];
                 ui = fma(w1, th, ui);
                 gmu[t] = w1 * (1.0 - th * th);
             }
         }
         // dU/dq_d = sum_mu gmu W0[mu][d]: partial over this lane's neurons, summed over the quad
-        // (the radial ones go to nep_radial_force_kernel through Dev::nep_q, the angular ones back to their owners)
+        // (the radial ones go on to nep_radial_pair_kernel as w_i, the angular ones back to their owners)
         for (int dsc = 0; dsc < sp.D; ++dsc) {
-            const double *w = W0t + dsc * Hp + q;
-            double v = 0.0;
+            const double2 *w = reinterpret_cast<const double2 *>(W0t + dsc * Hp + q * nt);
+            double v = 0.0, v2 = 0.0;
 #pragma unroll
-            for (int t = 0; t < kNepMaxH / 4; ++t) {
+            for (int t = 0; t < kNepMaxH / 4; t += 2) {
                 if (t >= nt) break;
-                v = fma(gmu[t], w[4 * t], v);
+                const double2 ww = w[t >> 1];
+                v = fma(gmu[t], ww.x, v);
+                v2 = fma(gmu[t + 1], ww.y, v2);
             }
-            v = quad_sum(v);
+            v = quad_sum(v + v2);
             if (q == (dsc & 3)) sq[dsc] = v;
         }
         __syncwarp();
-        for (int n = q; n < sp.nr; n += 4)
-            if (valid) qscr[(size_t)n * d.Npad] = sq[n];
+        // the radial descriptors act on the forces through w_i[J][k] = sum_n dU/dq_n cR[I][J][n][k] alone
+        // (nep_radial_pair_kernel): the quad forms the T KR of them, zero beyond k_r
+        if (valid) {
+            const int KR = d.nep_kr_pad;
+            const double *cR = d.dn_w + nNet + (size_t)I * sp.T * sp.nr * sp.kr;  // [J][n][k]
+            double *wv = d.nep_w + ((size_t)slot * d.Npad + ic) * (sp.T * KR);
+            for (int t = q; t < sp.T * KR; t += 4) {
+                const int J = t / KR, k = t % KR;
+                double w = 0.0;
+                if (k < sp.kr)
+                    for (int n = 0; n < sp.nr; ++n) w = fma(sq[n], cR[(J * sp.nr + n) * sp.kr + k], w);
+                wv[t] = w;
+            }
+        }
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh)
 #pragma unroll
@@ -472,14 +488,14 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
             double x = 0.0, y = 0.0, z = 0.0, inv = 0.0, g4[4] = {0.0, 0.0, 0.0, 0.0}, dg4[4] = {0.0, 0.0, 0.0, 0.0};
             double px = 0.0, py = 0.0, pz = 0.0;
             if (r2 < rca2) {
-                inv = rsqrt(r2);
+                inv = rsqrt_nr(r2);
                 const double r = r2 * inv;
                 x = dx * inv; y = dy * inv; z = dz * inv;
                 double f[KMAX], df[KMAX];
                 nep_basis<KMAX>(r * irca, irca, sp.ka, f, df);
 #pragma unroll
-                for (int c4 = 0; c4 < 4; ++c4) {
-                    const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + c4) * KMAX;
+                for (int c4 = 0; c4 < 4; ++c4) {  // g4[t], dg4[t]: the channel of lane q - t (walk 1)
+                    const double *c = cAb + ((size_t)J * kNepMaxN + 4 * pass + ((q - c4) & 3)) * KMAX;
                     double g = 0.0, dg = 0.0;
 #pragma unroll
                     for (int b = 0; b < KMAX; ++b) { g += c[b] * f[b]; dg += c[b] * df[b]; }
@@ -491,8 +507,8 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
 #pragma unroll
             for (int t = 0; t < 4; ++t) {
                 const int src = (q + t) & 3;
-                const double gs = t == 0 ? sel4(g4, q) : shf(sel4(g4, (q - t) & 3), src);
-                const double dgs = t == 0 ? sel4(dg4, q) : shf(sel4(dg4, (q - t) & 3), src);
+                const double gs = t == 0 ? g4[0] : shf(g4[t], src);
+                const double dgs = t == 0 ? dg4[0] : shf(dg4[t], src);
                 const double xs = t == 0 ? x : shf(x, src), ys = t == 0 ? y : shf(y, src), zs = t == 0 ? z : shf(z, src);
                 const double is = t == 0 ? inv : shf(inv, src), as = t == 0 ? inA : shf(inA, src);
                 double cx = 0.0, cy = 0.0, cz = 0.0;
@@ -537,6 +553,7 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
 }
 
 int nep_weight_count(const double *pot) { return nep_weights_size(nep_shape(pot)); }
+int nep_kr_padded(const double *pot) { const int kr = (int)pot[4]; return kr <= 4 ? 4 : kr <= 8 ? 8 : 12; }
 
 // The weight stream of include/cfneb.h (SplitMix64 from the seed), in the layout of Dev::dn_w.  Host.
 void nep_fill_weights(const double *pot, double *w) {
@@ -566,16 +583,17 @@ template <int KMAX>
 static void launch_nep_radial(const Dev &d, int p_lo, dim3 grid, bool force, cudaStream_t st) {
     const int nt = (int)d.pot[8];
     if (force) {
-        if (nt <= 1) nep_radial_force_kernel<KMAX, 1><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
-        else nep_radial_force_kernel<KMAX, 2><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
+        if (nt <= 1) nep_radial_pair_kernel<KMAX, 1><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
+        else nep_radial_pair_kernel<KMAX, 2><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
     } else {
         if (nt <= 1) nep_radial_desc_kernel<KMAX, 1><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
         else nep_radial_desc_kernel<KMAX, 2><<<grid, kNepRadialThreads, 0, st>>>(d, p_lo);
     }
 }
 
-// Pass 1 in three launches: radial descriptors (one atom per thread, all live rows), the quad kernel (angular rows,
-// network, angular partial forces), the radial partial forces (one atom per thread); then pass 2 (kernels_sw.cu).
+// Four launches: radial descriptors (one atom per thread, all live rows), the quad kernel (angular rows, network,
+// angular partial forces), the radial forces pair by pair (one atom per thread, all live rows), pass 2 of the angular
+// partial forces over the angular rows (kernels_sw.cu), which adds to F and to the virial partials.
 void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;

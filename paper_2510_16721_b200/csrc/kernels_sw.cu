@@ -178,7 +178,9 @@ __global__ void __launch_bounds__(kThreadsAtom) sw_force_kernel(Dev d, int p_lo)
 // the cut-off (Stillinger-Weber diamond: 4 of 5-16) the unconditional loads cost more than they hide (c5 0.50 ->
 // 0.54 ms), and loading the partial forces in a third round after the range test loses the gain (c6 1.10, c5 0.52):
 // that case keeps sw_force_kernel.
-template <int U>
+// ADD (the NEP-shaped potential): the rows that can lie inside the angular cut-off only, range test against it, and
+// the result is added to F and to the virial partials that nep_radial_pair_kernel wrote before (same grid).
+template <int U, bool ADD>
 __global__ void __launch_bounds__(kThreadsAtom) pair_force_batched_kernel(Dev d, int p_lo) {
     int p;
     if (!image_of(blockIdx.y, p_lo, d.ctl->P, p)) return;
@@ -189,14 +191,15 @@ __global__ void __launch_bounds__(kThreadsAtom) pair_force_batched_kernel(Dev d,
     __syncthreads();
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const bool valid = i < d.N;
-    const double rc2 = d.r_cut * d.r_cut;
+    const double rc2 = ADD ? d.pot[1] * d.pot[1] : d.r_cut * d.r_cut;
     double fx = 0.0, fy = 0.0, fz = 0.0, vxx = 0.0, vyy = 0.0, vzz = 0.0, vxy = 0.0, vxz = 0.0, vyz = 0.0;
     if (valid) {
         const double4 *Rc = d.Rc + (size_t)slot * d.Npad;
         const uint32_t *lists = d.nbr_list + (size_t)slot * d.cap * d.Npad;
         const double *part = d.part + (size_t)slot * d.cap * 3 * d.Npad;
         const double4 ri = Rc[i];
-        const int cnt = live_rows(d, slot, i);  // rows past it cannot be in range and are neither written nor read
+        // rows past it cannot be in range and are neither written nor read
+        const int cnt = ADD ? nep_angular_rows(d, slot, i) : live_rows(d, slot, i);
         const unsigned short *mir = d.nbr_mirror + (size_t)slot * d.cap * d.Npad + i;
         for (int k0 = 0; k0 < cnt; k0 += U) {
             uint32_t e[U];
@@ -235,6 +238,7 @@ __global__ void __launch_bounds__(kThreadsAtom) pair_force_batched_kernel(Dev d,
             }
         }
         double *F = d.F + (size_t)slot * 3 * d.Npad;
+        if (ADD) { fx += F[i]; fy += F[d.Npad + i]; fz += F[2 * (size_t)d.Npad + i]; }
         F[i] = fx; F[d.Npad + i] = fy; F[2 * (size_t)d.Npad + i] = fz;
     }
     double out7[7] = {0.0, -0.5 * vxx, -0.5 * vyy, -0.5 * vzz, -0.5 * vxy, -0.5 * vxz, -0.5 * vyz};
@@ -242,7 +246,7 @@ __global__ void __launch_bounds__(kThreadsAtom) pair_force_batched_kernel(Dev d,
     if (threadIdx.x == 0) {
         double *out = d.part_force + ((size_t)slot * d.nblk_force + blockIdx.x) * kNForcePart;
 #pragma unroll
-        for (int n = 0; n < 7; ++n) out[n] = out7[n];
+        for (int n = 0; n < 7; ++n) out[n] = ADD ? out[n] + out7[n] : out7[n];
         out[8] = 0.0;
     }
 }
@@ -281,7 +285,8 @@ void launch_pair_forces_manybody(const Dev &d, int p_lo, cudaStream_t st) {
     const int nimg = images_in_grid(d.S, p_lo);
     if (nimg <= 0) return;
     dim3 grid(d.nblk_atom, nimg);
-    if (d.potential == CFNEB_POT_DNN || d.potential == CFNEB_POT_NEP) pair_force_batched_kernel<4><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+    if (d.potential == CFNEB_POT_NEP) pair_force_batched_kernel<4, true><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
+    else if (d.potential == CFNEB_POT_DNN) pair_force_batched_kernel<4, false><<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
     else sw_force_kernel<<<grid, kThreadsAtom, 0, st>>>(d, p_lo);
 }
 
