@@ -142,18 +142,18 @@ __global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) ne
     nep_walk_rows(d, d.nbr_list + (size_t)slot * d.cap * d.Npad + i, Rc, ri, sh, live_rows(d, slot, i),
                   [&](int, uint32_t, const double4 &rj, double, double, double, double r2) {
         if (r2 < rcr2) {
-            double f[KMAX], df[KMAX];
-            nep_basis<KMAX>(r2 * rsqrt_nr(r2) * ircr, ircr, sp.kr, f, df);
-            if (NT == 1) {
+            // B[J][k] accumulates fc T_k (f_k = 1/2 (T_k + 1) fc is put together once per atom below); T_k runs to
+            // KMAX with no guard: |x| <= 1 and the entries beyond k_r are never read
+            const double t = r2 * rsqrt_nr(r2) * ircr, fc = 0.5 + 0.5 * cospi01(t);
+            const double x = 2.0 * (t - 1.0) * (t - 1.0) - 1.0, x2 = 2.0 * x;
+            const double m1 = NT > 1 ? rj.w * fc : 0.0, m0 = fc - m1;  // type of the neighbour as a weight
+            double Tm = 1.0, Tk = x;
 #pragma unroll
-                for (int k = 0; k < KMAX; ++k) B[0][k] += f[k];
-            } else {
-                const double m1 = rj.w, m0 = 1.0 - m1;  // type of the neighbour as a weight
-#pragma unroll
-                for (int k = 0; k < KMAX; ++k) {
-                    B[0][k] = fma(m0, f[k], B[0][k]);
-                    B[NT - 1][k] = fma(m1, f[k], B[NT - 1][k]);
-                }
+            for (int k = 0; k < KMAX; ++k) {
+                const double Tv = k == 0 ? 1.0 : Tk;
+                B[0][k] = fma(m0, Tv, B[0][k]);
+                if (NT > 1) B[NT - 1][k] = fma(m1, Tv, B[NT - 1][k]);
+                if (k >= 1) { const double Tn = fma(x2, Tk, -Tm); Tm = Tk; Tk = Tn; }
             }
         }
     });
@@ -166,8 +166,8 @@ __global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) ne
         for (int J = 0; J < NT; ++J)
 #pragma unroll
             for (int k = 0; k < KMAX; ++k)
-                if (k < sp.kr) qn = fma(cR[(J * sp.nr + n) * sp.kr + k], B[J][k], qn);
-        qscr[(size_t)n * d.Npad] = qn;
+                if (k < sp.kr) qn = fma(cR[(J * sp.nr + n) * sp.kr + k], B[J][k] + B[J][0], qn);  // B[J][0] = sum fc
+        qscr[(size_t)n * d.Npad] = 0.5 * qn;
     }
 }
 
@@ -208,17 +208,27 @@ __global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) ne
 #pragma unroll
                 for (int k = 0; k < KMAX / 2; ++k) wjk[k] = wj[k];
                 const double inv = rsqrt_nr(r2);
-                double f[KMAX], df[KMAX];
-                nep_basis<KMAX>(r2 * inv * ircr, ircr, sp.kr, f, df);
                 const double2 *wi = sWi + (NT > 1 ? (int)rj.w : 0) * (KMAX / 2) * kNepRadialThreads + threadIdx.x;
-                double sa = 0.0, sb = 0.0;
+                // sum_k W_k f_k' with W_k = w_i[J][k] + w_j[I][k] and f_k' = 1/2 T_k' x' fc + 1/2 (T_k + 1) fc':
+                //   = 1/2 x' fc sum_k W_k T_k' + 1/2 fc' (sum_k W_k T_k + sum_k W_k); W_k = 0 beyond k_r, no guard
+                const double t = r2 * inv * ircr;
+                double sn, cs;
+                sincospi01(t, sn, cs);
+                const double fc = 0.5 + 0.5 * cs, dfc = -0.5 * sn * (3.14159265358979323846 * ircr);
+                const double x = 2.0 * (t - 1.0) * (t - 1.0) - 1.0, x2 = 2.0 * x, dx_dr = 4.0 * (t - 1.0) * ircr;
+                double Tm = 1.0, Tk = x, dTm = 0.0, dTk = 1.0, sT = 0.0, sdT = 0.0, sW = 0.0;
 #pragma unroll
-                for (int k = 0; k < KMAX / 2; ++k) {
-                    const double2 a = wi[k * kNepRadialThreads];
-                    sa = fma(a.x + wjk[k].x, df[2 * k], sa);
-                    sb = fma(a.y + wjk[k].y, df[2 * k + 1], sb);
+                for (int k = 0; k < KMAX; ++k) {
+                    const double2 a = wi[(k >> 1) * kNepRadialThreads];
+                    const double W = (k & 1) ? a.y + wjk[k >> 1].y : a.x + wjk[k >> 1].x;
+                    sW += W;
+                    if (k == 0) { sT = W; continue; }
+                    sT = fma(W, Tk, sT);
+                    sdT = fma(W, dTk, sdT);
+                    const double Tn = fma(x2, Tk, -Tm), dTn = fma(x2, dTk, fma(2.0, Tk, -dTm));
+                    Tm = Tk; Tk = Tn; dTm = dTk; dTk = dTn;
                 }
-                const double sr = (sa + sb) * inv;
+                const double sr = 0.5 * (dx_dr * fc * sdT + dfc * (sT + sW)) * inv;
                 const double gx = sr * dx, gy = sr * dy, gz = sr * dz;  // f^ij of Eq. 5, radial part
                 fx += gx; fy += gy; fz += gz;
                 vxx = fma(dx, gx, vxx); vyy = fma(dy, gy, vyy); vzz = fma(dz, gz, vzz);  // Eq. 8 (central: symmetric)
