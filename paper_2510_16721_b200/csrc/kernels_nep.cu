@@ -4,7 +4,8 @@
 // two atom types with type-pair expansion coefficients, basis sizes and descriptor counts as parameters, Legendre
 // orders up to 4, one network of up to 64 neurons per type.  Seeded weights (the trained ones are not available):
 // cost and data flow, no physics.  It enters the path through the partial forces p^ij = dU_i/dr^ij of Eq. 5; pass 2
-// (f^ij = p^ij - p^ji, F_i, virial of Eq. 8) is the kernel the other many-body potentials use (kernels_sw.cu).
+// (f^ij = p^ij - p^ji, F_i, virial of Eq. 8) of the angular part is the kernel the other many-body potentials use
+// (kernels_sw.cu), the radial part is formed pair by pair.
 //   f_k(r; rc) = 1/2 [T_k(x) + 1] fc(r; rc),  x = 2 (r/rc - 1)^2 - 1,  fc = 1/2 [1 + cos(pi r/rc)]
 //   g^R_n = sum_k cR[I][J][n][k] f_k(r; rc_r),   g^A_n = sum_k cA[I][J][n][k] f_k(r; rc_a)      (I, J: types of i, j)
 //   q_n    = sum_j g^R_n(r_ij)                                                                  n < n_r
@@ -15,15 +16,23 @@
 // A_l = sum_jk g g (u_j.u_k)^l = |S^(l)|^2 and q_{n1} = A_1, q_{n2} = 3/2 A_2 - 1/2 A_0, q_{n3} = 5/2 A_3 - 3/2 A_1,
 // q_{n4} = (35 A_4 - 30 A_2 + 3 A_0)/8.
 //
-// Work split (round 1's descriptor kernel held all channels of an atom in one thread: 236 registers, 8 warps per
-// multiprocessor).  FOUR LANES PER ATOM: lane q of a quad owns the angular channels n = q, q + 4 and the radial
-// a quarter of the neurons.  The list is walked four rows at a time, ONE ROW PER LANE: a lane forms the pair vector, the
-// two radial bases and the expansions g_n of its row once, then the rows go round the quad by shuffles and every lane
-// adds each row to the 35 moments of its own channel (registers); the moments are parked in a scratch array (one
-// 280-byte column per atom and channel), the quad exchanges descriptors and descriptor gradients by shuffles, and a
-// second walk of the same shape evaluates phi_n(u) = sum_c G_nc u^c and its gradient per channel and hands the three
-// components back to the row's lane, which writes them once.  Network weights and expansion coefficients sit in shared
-// memory.  No per-thread environment array, hence no limit on the atoms inside the cut-offs but the list capacity.
+// Work split: four launches (launch_force_nep).
+//  1. nep_radial_desc_kernel, one atom per thread over all live rows: q_n through the basis sums per neighbour type.
+//  2. nep_partial_kernel, FOUR LANES PER ATOM, over the rows that can lie inside rc_a only (nep_angular_rows): lane q of
+//     a quad owns the angular channels n = q, q + 4 and a quarter of the neurons.  The list is walked four rows at a
+//     time, ONE ROW PER LANE: a lane forms the pair vector, the angular basis and the expansions g_n of its row once,
+//     then the rows go round the quad by shuffles and every lane adds each row to the 35 moments of its own channel
+//     (registers); the moments are parked in a scratch array (one 280-byte column per atom and channel), the network
+//     runs with the quad's descriptors side by side in shared memory, and a second walk of the same shape evaluates
+//     phi_n(u) = sum_c G_nc u^c and its gradient per channel and hands the three components back to the row's lane,
+//     which writes the angular partial force once.  Network weights and angular expansion coefficients sit in shared
+//     memory.  The radial descriptors act on the forces through w_i[J][k] = sum_n dU_i/dq_n cR[I][J][n][k], written
+//     out per atom.
+//  3. nep_radial_pair_kernel, one atom per thread over all live rows: the radial part of Eq. 5 pair by pair from
+//     w_i[J] + w_j[I]; F_i and the virial partials of that part.
+//  4. pass 2 of the angular partial forces over the angular rows (kernels_sw.cu), added to F_i.
+// No per-thread environment array, hence no limit on the atoms inside the cut-offs but the list capacity.  The type of
+// an atom rides in the fourth double of its position sector (positions_kernel).
 #include "cfneb_internal.cuh"
 #include "nep_poly.cuh"
 #include "trig01.cuh"
