@@ -170,6 +170,44 @@ def bain_pair_counts(cells, dims, r_on, r_cut):
     return out
 
 
+def nep_flops_per_atom(pot, n_r_pairs, n_a_pairs):
+    """fp64 operations per atom of K2 for the NEP-shaped potential, as the formulas of kernels_nep.cu / pass 2 are
+    written (FMA = 2, everything else = 1; reciprocal-square-root seed and integer work not counted), for an atom with
+    n_r_pairs neighbours inside rc_r and n_a_pairs inside rc_a.  Terms, with K_r, K_a the basis sizes, T the atom types,
+    n_r / n_a the radial descriptors / angular channels, D descriptors, H neurons (DESIGN.md section 10 item 6):
+      pair vector 8, own rsqrt 8, cos(pi t) 23 (with sin(pi t): 45), cut-off and Chebyshev argument 7-11;
+      radial descriptors, per pair:      50 + 2 T K_r + 2 (K_r - 1)      (T multiply-adds and one recurrence step per k)
+      radial forces pair by pair:        99 + 2 K_r + 10 (K_r - 1)       (T_k, T_k' recurrences, two sums, F and virial)
+      quad kernel walk 1, per pair:      50 + 14 K_a + 101 n_a           (basis, g_n of 4 channels; per channel 31 monomial
+                                                                          products + 35 multiply-adds into the moments)
+      quad kernel walk 2, per pair:      76 + 32 K_a + 205 n_a           (basis with derivative, g_n and g_n'; per channel
+                                                                          16 monomial products, 60 multiply-adds of the
+                                                                          gradient polynomial, Euler sums, the 3 components)
+      pass 2 over the angular pairs:     35
+      per atom: network 4 D H + 35 H, moments -> descriptors and back 225 n_a, radial coefficients 3 T K_r n_r + 2 T K_r n_r."""
+    n_r, n_a, k_r, k_a, L, H, T = (int(pot[i]) for i in (2, 3, 4, 5, 6, 7, 8))
+    D = n_r + n_a * L
+    radial = (50 + 2 * T * k_r + 2 * (k_r - 1)) + (99 + 2 * k_r + 10 * (k_r - 1))
+    angular = (50 + 14 * k_a + 101 * n_a) + (76 + 32 * k_a + 205 * n_a) + 35
+    per_atom = 4 * D * H + 35 * H + 225 * n_a + 5 * T * k_r * n_r
+    return n_r_pairs * radial + n_a_pairs * angular + per_atom
+
+
+def nep_pair_counts(band, images, rc_r, rc_a):
+    """Mean number of neighbours inside rc_r and inside rc_a per atom, counted on the host from the band's own Verlet
+    lists (parity hook) and current positions, for the given images."""
+    pos, cells, _ = band.get_path()
+    out = []
+    for p in images:
+        count, lst, shift = band.get_neighbors(p)
+        mask = np.arange(lst.shape[1])[None, :] < count[:, None]
+        j = np.where(mask, lst, 0)
+        d = pos[p][j] + shift.astype(np.float64) @ cells[p] - pos[p][:, None, :]
+        r = np.sqrt(np.sum(d * d, axis=2))
+        out.append((float(np.sum((r < rc_r) & mask) / len(count)), float(np.sum((r < rc_a) & mask) / len(count))))
+    return out
+
+
 # ------------------------------------------------------------------------------------------------------------
 def host_cores():
     try:
@@ -364,6 +402,22 @@ def main_ours(args):
                           "ncu": {"force_kernel": ncu_pipe("c4", "force_kernel"), "density_kernel": ncu_pipe("c4", "density_kernel"),
                                   "note": "committed ncu capture of configs[4] (profiles/r2_ncu_full_c4.txt): share of the fp64 pipe's and "
                                           "of the issue slots' peak; 2 x fp64 + other instructions = 91 % of the scheduler cycles"}}
+
+    if spec.potential == cf.POT_NEP:
+        sample = sorted({1, P // 2, P - 2})
+        pcs = nep_pair_counts(band, sample, spec.pot[0], spec.pot[1])
+        n_rp, n_ap = float(np.mean([a for a, _ in pcs])), float(np.mean([b for _, b in pcs]))
+        flop = units_per_step * nep_flops_per_atom(spec.pot, n_rp, n_ap)
+        t_force = kms[cf.binding.K_FORCE] * 1e-3
+        roofline_force = {"kernel": "K2 nep_radial_desc_kernel + nep_partial_kernel + nep_radial_pair_kernel + pair_force_batched_kernel",
+                          "bound": "alu", "achieved": flop / t_force / 1e12, "peak": None, "unit": "TFLOP/s", "frac": None,
+                          "algorithmic_flop": flop, "ms": t_force * 1e3,
+                          "pairs_inside_rc_r_per_atom_mean": n_rp, "pairs_inside_rc_a_per_atom_mean": n_ap,
+                          "pair_count_sample": "images %s, from the band's own lists" % sample,
+                          "peak_source": "measured DFMA chain, cfneb_util_fp64_peak (no fp64 figure in MEASURED_PEAKS.json)",
+                          "share_of_step": float(kms[cf.binding.K_FORCE] / kms.sum()),
+                          "ncu": {kn: ncu_pipe(wl, kn) for kn in ("nep_partial_kernel", "nep_radial_pair_kernel",
+                                                                   "nep_radial_desc_kernel", "pair_force_batched_kernel")}}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
