@@ -92,24 +92,29 @@ __device__ __forceinline__ void nep_basis(double t, double irc, int K, double (&
 
 __device__ __forceinline__ const double4 *Rc_of(const Dev &d, int slot) { return d.Rc + (size_t)slot * d.Npad; }
 
-// One atom per thread over all live rows of its list, the loads software-pipelined:
+// One atom per thread over all live rows of its list, the loads software-pipelined with NO register rotation (a
+// move of a register whose load is in flight waits for the load: the rotating version of this walk spent a third
+// of its stall samples on such a move).  The loop is unrolled over the four entry registers: in stage u (row k + u)
+// the sector of row k + u + 1 is requested through the entry that was loaded three stages ago, the entry register of
+// this row is reloaded for row k + u + 4, and the list row twelve ahead is pulled into L2.
 // body(k, j, rj, dx, dy, dz, r2) for the rows k < cnt of this thread (rj.w = type of the neighbour j).
+// (Requesting w_j of the next row a stage ahead in nep_radial_pair_kernel, into registers or into L1, measured slower.)
 template <class Body>
 __device__ __forceinline__ void nep_walk_rows(const Dev &d, const uint32_t *lp, const double4 *Rc, const double4 &ri,
                                               const double *sh, int cnt, Body body) {
     if (cnt <= 0) return;
     const int last = cnt - 1;
-    // entries three rows and sectors two rows ahead of use (row indices clamped to the last row)
-    uint32_t e0 = lp[0], e1 = lp[(size_t)min(1, last) * d.Npad], e2 = lp[(size_t)min(2, last) * d.Npad];
-    double4 r0 = Rc[e0 & kIdxMask], r1 = Rc[e1 & kIdxMask];
-    for (int k = 0; k < cnt; ++k) {
-        const uint32_t code = e0 >> kShiftBits, j = e0 & kIdxMask;
-        const double4 rc = r0;
-        e0 = e1; e1 = e2;
-        e2 = lp[(size_t)min(k + 3, last) * d.Npad];
-        r0 = r1;
-        r1 = Rc[e1 & kIdxMask];
-        double dx = rc.x - ri.x, dy = rc.y - ri.y, dz = rc.z - ri.z;
+    uint32_t e[4];
+    double4 s[2];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) e[u] = lp[(size_t)min(u, last) * d.Npad];
+    s[0] = Rc[e[0] & kIdxMask];
+    auto stage = [&](int k, uint32_t &ecur, uint32_t enext, const double4 &scur, double4 &snext) {
+        snext = Rc[enext & kIdxMask];
+        const uint32_t code = ecur >> kShiftBits, j = ecur & kIdxMask;
+        ecur = lp[(size_t)min(k + 4, last) * d.Npad];
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(lp + (size_t)min(k + 12, last) * d.Npad));
+        double dx = scur.x - ri.x, dy = scur.y - ri.y, dz = scur.z - ri.z;
         if (code != kCodeCenter) {
             const double n0 = (double)((int)(code & 7u) - 4), n1 = (double)((int)((code >> 3) & 7u) - 4),
                          n2 = (double)((int)((code >> 6) & 7u) - 4);
@@ -117,7 +122,16 @@ __device__ __forceinline__ void nep_walk_rows(const Dev &d, const uint32_t *lp, 
             dy += n0 * sh[1] + n1 * sh[4] + n2 * sh[7];
             dz += n0 * sh[2] + n1 * sh[5] + n2 * sh[8];
         }
-        body(k, j, rc, dx, dy, dz, dx * dx + dy * dy + dz * dz);
+        body(k, j, scur, dx, dy, dz, dx * dx + dy * dy + dz * dz);
+    };
+    for (int k = 0; k < cnt; k += 4) {
+        stage(k, e[0], e[1], s[0], s[1]);
+        if (k + 1 >= cnt) break;
+        stage(k + 1, e[1], e[2], s[1], s[0]);
+        if (k + 2 >= cnt) break;
+        stage(k + 2, e[2], e[3], s[0], s[1]);
+        if (k + 3 >= cnt) break;
+        stage(k + 3, e[3], e[0], s[1], s[0]);
     }
 }
 
@@ -212,10 +226,9 @@ __global__ void __launch_bounds__(kNepRadialThreads, CFNEB_NEP_RADIAL_BLOCKS) ne
         nep_walk_rows(d, d.nbr_list + (size_t)slot * d.cap * d.Npad + i, Rc, ri, sh, live_rows(d, slot, i),
                       [&](int, uint32_t j, const double4 &rj, double dx, double dy, double dz, double r2) {
             if (r2 < rcr2) {
-                const double2 *wj = reinterpret_cast<const double2 *>(wv + ((size_t)j * NT + I) * KMAX);
                 double2 wjk[KMAX / 2];
 #pragma unroll
-                for (int k = 0; k < KMAX / 2; ++k) wjk[k] = wj[k];
+                for (int t = 0; t < KMAX / 2; ++t) wjk[t] = reinterpret_cast<const double2 *>(wv + ((size_t)j * NT + I) * KMAX)[t];
                 const double inv = rsqrt_nr(r2);
                 const double2 *wi = sWi + (NT > 1 ? (int)rj.w : 0) * (KMAX / 2) * kNepRadialThreads + threadIdx.x;
                 // sum_k W_k f_k' with W_k = w_i[J][k] + w_j[I][k] and f_k' = 1/2 T_k' x' fc + 1/2 (T_k + 1) fc':
