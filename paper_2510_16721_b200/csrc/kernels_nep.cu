@@ -55,11 +55,14 @@ __host__ __device__ inline NepShape nep_shape(const double *pot) {
     s.D = s.nr + s.na * s.L;
     return s;
 }
-// layout of Dev::dn_w for this potential: per type [W0t D*Hp | b0 Hp | W1 Hp] (first layer transposed to [d][mu], the
-// neurons zero-padded to Hp, a multiple of eight: the quad kernel copies it to shared memory as it is), then
+// layout of Dev::dn_w for this potential: per type [W0t Dp*HS | b0 Hp | W1 Hp] (first layer transposed to [d][mu];
+// neurons and descriptors zero-padded to multiples of eight, Hp and Dp, rows HS = Hp + 4 doubles apart so that the
+// tensor-core fragment loads of the quad kernel fall on distinct banks; copied to shared memory as it is), then
 // cR [T][T][nr][kr], then cA [T][T][na][ka]
 __host__ __device__ inline int nep_hp(const NepShape &s) { return (s.H + 7) & ~7; }
-__host__ __device__ inline int nep_net_size(const NepShape &s) { return s.D * nep_hp(s) + 2 * nep_hp(s); }
+__host__ __device__ inline int nep_dp(const NepShape &s) { return (s.D + 7) & ~7; }
+__host__ __device__ inline int nep_hs(const NepShape &s) { return nep_hp(s) + 4; }
+__host__ __device__ inline int nep_net_size(const NepShape &s) { return nep_dp(s) * nep_hs(s) + 2 * nep_hp(s); }
 __host__ __device__ inline int nep_weights_size(const NepShape &s) {
     return s.T * nep_net_size(s) + s.T * s.T * (s.nr * s.kr + s.na * s.ka);
 }
@@ -88,6 +91,11 @@ __device__ __forceinline__ void nep_basis(double t, double irc, int K, double (&
             df[k] = 0.0;
         }
     }
+}
+
+// D = A B + D on the fp64 tensor cores, m8n8k4: lane l holds A[l >> 2][l & 3], B[l & 3][l >> 2], D[l >> 2][2 (l & 3) + {0, 1}]
+__device__ __forceinline__ void dmma884(double &d0, double &d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
 __device__ __forceinline__ const double4 *Rc_of(const Dev &d, int slot) { return d.Rc + (size_t)slot * d.Npad; }
@@ -303,7 +311,7 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     const double rca = d.pot[1], rca2 = rca * rca, irca = 1.0 / rca;
     const double4 ri = Rc_of(d, slot)[ic];
     const int I = (int)ri.w;
-    const double *W0t = sW + I * netp, *b0 = W0t + sp.D * Hp, *W1 = b0 + Hp;
+    const double *b0 = sW + I * netp + nep_dp(sp) * nep_hs(sp), *W1 = b0 + Hp;  // of this atom's type
     const double *cAb = cAp + (size_t)I * sp.T * kNepMaxN * KMAX;
     const double4 *Rc = Rc_of(d, slot);
     const uint32_t *lp = d.nbr_list + (size_t)slot * d.cap * d.Npad + ic;
@@ -413,35 +421,43 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
             qA[pass][3] = 0.125 * (35.0 * A[4] - 30.0 * A[2] + 3.0 * A[0]);
         }
     }
-    // ---- the network: each lane takes a quarter of the neurons; the radial descriptors come from
-    // nep_radial_desc_kernel (Dev::nep_q), the angular ones from their owners in the quad.  Weights in shared memory
-    // as W0t[d][mu] with the neurons zero-padded to a multiple of eight: a padded neuron has tanh(0) = 0 and W1 = 0 ----
+    // ---- the network, on the fp64 tensor cores: a warp is eight quads = eight atoms = the eight rows of an m8n8k4
+    // fragment.  Forward z[atom][mu] = sum_d q[atom][d] W0[mu][d]: lane q of quad g supplies A[g][q] = q_{k0 + q} of its
+    // atom, loads B[q][g] = W0t[k0 + q][8 t + g], and receives C[g][2 q], C[g][2 q + 1]: the neurons 8 t + 2 q, + 1 of
+    // its own atom, eight per lane.  The weights are per atom type and a warp holds atoms of both: each type's matrix is
+    // applied with the rows of the other type's atoms zeroed, into the same accumulators.  Backward
+    // dU/dq_d = sum_mu g_mu W0[mu][d] the same way with the lane's own neurons as the A operand (k-step (t, h) takes
+    // neuron 8 t + 2 q + h from lane q).  Padded neurons (b0 = W0 = W1 = 0) and padded descriptors contribute nothing. ----
     double ui = 0.0;
     double FdA[2][kNepMaxL] = {};
     {
-        const int nt = Hp >> 2;  // neurons per lane (even): lane q takes mu = q nt .. q nt + nt - 1, read two at a time
-        double zt[kNepMaxH / 4];
+        const int Dp = nep_dp(sp), HS = nep_hs(sp), ntile = Hp >> 3, g = (threadIdx.x & 31) >> 2;
+        double zt[kNepMaxH / 4];  // zt[2 t + c]: neuron 8 t + 2 q + c
 #pragma unroll
-        for (int t = 0; t < kNepMaxH / 4; ++t) zt[t] = t < nt ? -b0[q * nt + t] : 0.0;
-        // the descriptors of the quad's atom, side by side in shared memory (one short loop instead of an unrolled
-        // ladder of shuffles)
+        for (int t = 0; t < kNepMaxH / 8; ++t) {
+            zt[2 * t] = t < ntile ? -b0[8 * t + 2 * q] : 0.0;
+            zt[2 * t + 1] = t < ntile ? -b0[8 * t + 2 * q + 1] : 0.0;
+        }
+        // the descriptors of the quad's atom side by side in shared memory, zero beyond D
         double *sq = sQ + (threadIdx.x >> 2) * (kNepMaxD + 1);  // odd stride: the quads of a warp on distinct banks
-        for (int n = q; n < sp.nr; n += 4) sq[n] = valid ? qscr[(size_t)n * d.Npad] : 0.0;
+        for (int n = q; n < Dp; n += 4) sq[n] = (n < sp.nr && valid) ? qscr[(size_t)n * d.Npad] : 0.0;
+        __syncwarp();
 #pragma unroll
         for (int hh = 0; hh < 2; ++hh)
 #pragma unroll
             for (int ll = 0; ll < kNepMaxL; ++ll)
                 if (q + 4 * hh < sp.na && ll < sp.L) sq[sp.nr + (q + 4 * hh) * sp.L + ll] = qA[hh][ll];
         __syncwarp();
-        for (int dsc = 0; dsc < sp.D; ++dsc) {
-            const double v = sq[dsc];
-            const double2 *w = reinterpret_cast<const double2 *>(W0t + dsc * Hp + q * nt);
+        for (int T2 = 0; T2 < sp.T; ++T2) {
+            const double *Wt = sW + T2 * netp;
+            for (int k0 = 0; k0 < Dp; k0 += 4) {
+                const double a = I == T2 ? sq[k0 + q] : 0.0;
+                const double *brow = Wt + (k0 + q) * HS + g;
 #pragma unroll
-            for (int t = 0; t < kNepMaxH / 4; t += 2) {
-                if (t >= nt) break;
-                const double2 ww = w[t >> 1];
-                zt[t] = fma(ww.x, v, zt[t]);
-                zt[t + 1] = fma(ww.y, v, zt[t + 1]);
+                for (int t = 0; t < kNepMaxH / 8; ++t) {
+                    if (t >= ntile) break;
+                    dmma884(zt[2 * t], zt[2 * t + 1], a, brow[8 * t]);
+                }
             }
         }
         __syncwarp();
@@ -449,26 +465,26 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
 #pragma unroll
         for (int t = 0; t < kNepMaxH / 4; ++t) {
             gmu[t] = 0.0;
-            if (t < nt) {
-                const double th = tanh(zt[t]), w1 = W1[q * nt + t];
+            if ((t >> 1) < ntile) {
+                const double th = tanh(zt[t]), w1 = W1[8 * (t >> 1) + 2 * q + (t & 1)];
                 ui = fma(w1, th, ui);
                 gmu[t] = w1 * (1.0 - th * th);
             }
         }
-        // dU/dq_d = sum_mu gmu W0[mu][d]: partial over this lane's neurons, summed over the quad
-        // (the radial ones go on to nep_radial_pair_kernel as w_i, the angular ones back to their owners)
-        for (int dsc = 0; dsc < sp.D; ++dsc) {
-            const double2 *w = reinterpret_cast<const double2 *>(W0t + dsc * Hp + q * nt);
-            double v = 0.0, v2 = 0.0;
+        // dU/dq_d (the radial ones go on to nep_radial_pair_kernel as w_i, the angular ones back to their owners)
+        for (int n0 = 0; n0 < Dp; n0 += 8) {
+            double c0 = 0.0, c1 = 0.0;
+            for (int T2 = 0; T2 < sp.T; ++T2) {
+                const double *bcol = sW + T2 * netp + (n0 + g) * HS + 2 * q;
 #pragma unroll
-            for (int t = 0; t < kNepMaxH / 4; t += 2) {
-                if (t >= nt) break;
-                const double2 ww = w[t >> 1];
-                v = fma(gmu[t], ww.x, v);
-                v2 = fma(gmu[t + 1], ww.y, v2);
+                for (int t = 0; t < kNepMaxH / 8; ++t) {
+                    if (t >= ntile) break;
+                    dmma884(c0, c1, I == T2 ? gmu[2 * t] : 0.0, bcol[8 * t]);
+                    dmma884(c0, c1, I == T2 ? gmu[2 * t + 1] : 0.0, bcol[8 * t + 1]);
+                }
             }
-            v = quad_sum(v + v2);
-            if (q == (dsc & 3)) sq[dsc] = v;
+            sq[n0 + 2 * q] = c0;
+            sq[n0 + 2 * q + 1] = c1;
         }
         __syncwarp();
         // the radial descriptors act on the forces through w_i[J][k] = sum_n dU/dq_n cR[I][J][n][k] alone
@@ -602,9 +618,10 @@ void nep_fill_weights(const double *pot, double *w) {
     for (int I = 0; I < s.T; ++I) {  // stream order: W0[mu][d], b0[mu], W1[mu]
         double *net = w + (size_t)I * nep_net_size(s);
         for (int t = 0; t < nep_net_size(s); ++t) net[t] = 0.0;
-        for (int t = 0; t < s.H * s.D; ++t) net[(t % s.D) * Hp + t / s.D] = next() * ((t % s.D) < s.nr ? 0.04 : 0.004);
-        for (int t = 0; t < s.H; ++t) net[s.D * Hp + t] = 0.5 * next();
-        for (int t = 0; t < s.H; ++t) net[s.D * Hp + Hp + t] = next();
+        const int HS = nep_hs(s), Dp = nep_dp(s);
+        for (int t = 0; t < s.H * s.D; ++t) net[(t % s.D) * HS + t / s.D] = next() * ((t % s.D) < s.nr ? 0.04 : 0.004);
+        for (int t = 0; t < s.H; ++t) net[Dp * HS + t] = 0.5 * next();
+        for (int t = 0; t < s.H; ++t) net[Dp * HS + Hp + t] = next();
     }
     double *c = w + (size_t)s.T * nep_net_size(s);
     const int nc = s.T * s.T * (s.nr * s.kr + s.na * s.ka);
