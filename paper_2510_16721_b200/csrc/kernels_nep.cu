@@ -294,7 +294,11 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     const int nNet = sp.T * nep_net_size(sp);  // offset of the expansion coefficients in Dev::dn_w
     const int Hp = nep_hp(sp), netp = nep_net_size(sp);
     if (threadIdx.x < 9) sh[threadIdx.x] = d.geom[slot].h[threadIdx.x];
-    for (int t = threadIdx.x; t < nNet; t += blockDim.x) sW[t] = d.dn_w[t];
+    // the network weights are not needed before the first walk is over: asynchronous copy (16 bytes per request;
+    // nNet is even and both sides are 16-byte aligned), waited for in front of the network
+    for (int t = 2 * threadIdx.x; t < nNet; t += 2 * blockDim.x)
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(sW + t)), "l"(d.dn_w + t));
+    asm volatile("cp.async.commit_group;");
     // angular expansion coefficients zero-padded to [T][T][8][KMAX]: the loops over channels and basis functions then
     // run to their compile-time bounds with no guards, and a row of coefficients is KMAX aligned doubles
     double *cAp = sW + ((nNet + 1) & ~1);
@@ -430,6 +434,8 @@ __global__ void __launch_bounds__(kNepThreads, CFNEB_NEP_BLOCKS) nep_partial_ker
     // neuron 8 t + 2 q + h from lane q).  Padded neurons (b0 = W0 = W1 = 0) and padded descriptors contribute nothing. ----
     double ui = 0.0;
     double FdA[2][kNepMaxL] = {};
+    asm volatile("cp.async.wait_all;");
+    __syncthreads();  // the weights of the other threads' requests
     {
         const int Dp = nep_dp(sp), HS = nep_hs(sp), ntile = Hp >> 3, g = (threadIdx.x & 31) >> 2;
         double zt[kNepMaxH / 4];  // zt[2 t + c]: neuron 8 t + 2 q + c
