@@ -162,6 +162,13 @@ __global__ void __launch_bounds__(256) rebuild_list_kernel(Dev d, int p_lo) {
 
 constexpr int kRadialBuckets = kInnerBuckets + kTailBuckets;
 constexpr int kQueue = 32;
+#ifndef CFNEB_K1_DRAIN
+#define CFNEB_K1_DRAIN 4
+#endif
+#ifndef CFNEB_K1_SCAN
+#define CFNEB_K1_SCAN 8
+#endif
+constexpr int kDrain = CFNEB_K1_DRAIN, kScan = CFNEB_K1_SCAN;  // candidates per round of the drain / of the prefilter scan
 constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 #ifndef CFNEB_SEARCH_BLOCKS
 #define CFNEB_SEARCH_BLOCKS 5
@@ -224,13 +231,23 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
 
     auto flush = [&]() {
         const int nq_w = __reduce_max_sync(0xffffffffu, nq);
-        for (int c = 0; c < nq_w; ++c) {
+        // kDrain candidates per round: their queue entries and coordinates are requested together (the walk is
+        // bound by the latency of these two dependent loads, not by their number)
+        for (int c0 = 0; c0 < nq_w; c0 += kDrain) {
+          uint32_t ee[kDrain];
+          double4 cc[kDrain];
+#pragma unroll
+          for (int u = 0; u < kDrain; ++u) ee[u] = queue[min(c0 + u, kQueue - 1) * kThreadsAtom];
+#pragma unroll
+          for (int u = 0; u < kDrain; ++u) cc[u] = binned[c0 + u < nq ? (int)(ee[u] & kIdxMask) : ic];
+#pragma unroll
+          for (int u = 0; u < kDrain; ++u) {
+            const int c = c0 + u;
             if (c >= nq) continue;
-            const uint32_t e = queue[c * kThreadsAtom];
-            const int q = (int)(e & kIdxMask);
+            const uint32_t e = ee[u];
             const int m0 = (int)((e >> kShiftBits) & 7u) - 4, m1 = (int)((e >> (kShiftBits + 3)) & 7u) - 4,
                       m2 = (int)((e >> (kShiftBits + 6)) & 7u) - 4;
-            const double4 c4 = binned[q];
+            const double4 c4 = cc[u];
             const double s0 = c4.x - si.x + (double)m0, s1 = c4.y - si.y + (double)m1, s2 = c4.z - si.z + (double)m2;
             const double rx = s0 * h[0] + s1 * h[3] + s2 * h[6];
             const double ry = s0 * h[1] + s1 * h[4] + s2 * h[7];
@@ -255,6 +272,7 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
                 hist[bk * kThreadsAtom] += 1;
             }
             ++cnt;
+          }
         }
         nq = 0;
     };
@@ -275,12 +293,12 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
                 // own position minus the periodic shift of this stencil cell, fp32
                 const float ox = cix - (float)(m0 * h[0] + m1 * h[3] + m2 * h[6]), oy = ciy - (float)(m0 * h[1] + m1 * h[4] + m2 * h[7]),
                             oz = ciz - (float)(m0 * h[2] + m1 * h[5] + m2 * h[8]);
-                for (int t = 0; t < len_w; t += 4) {
-                    float4 cf[4];
+                for (int t = 0; t < len_w; t += kScan) {
+                    float4 cf[kScan];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) cf[u] = binned_c[min(lo + t + u, max(hi - 1, 0))];
+                    for (int u = 0; u < kScan; ++u) cf[u] = binned_c[min(lo + t + u, max(hi - 1, 0))];
 #pragma unroll
-                    for (int u = 0; u < 4; ++u) {
+                    for (int u = 0; u < kScan; ++u) {
                         const int q = lo + t + u;
                         const float fx = cf[u].x - ox, fy = cf[u].y - oy, fz = cf[u].z - oz;
                         if (q < hi && fx * fx + fy * fy + fz * fz < rl2f) {
@@ -288,7 +306,7 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
                             ++nq;
                         }
                     }
-                    if (__any_sync(0xffffffffu, nq > kQueue - 4)) flush();
+                    if (__any_sync(0xffffffffu, nq > kQueue - kScan)) flush();
                 }
             }
         }
