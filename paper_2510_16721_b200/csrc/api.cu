@@ -138,7 +138,9 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.Rc = c.take<double4>(S * Npad);
     d.Sw = c.take<double4>(S * Npad);
     d.binned = c.take<double4>(S * Npad);
-    d.binned_c = c.take<float4>(S * Npad);
+    // + slack: the prefilter scan reads (masked) past a short bin's end, by at most the longest bin of the warp's
+    // stencil; a bin of the coarsest grid (3 r_list wide on two axes) holds fewer than 4 x cap atoms
+    d.binned_c = c.take<float4>(S * Npad + 4096 + 8 * (size_t)d.cap);
     d.Xc = c.take<double>(2 * S * 9);
     d.vc = c.take<double>(S * 9);
     d.E = c.take<double>(S);
@@ -167,6 +169,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
         d.n_search_blocks = sms * search_blocks_per_sm();
         d.scr_tmp = c.take<uint32_t>((size_t)d.n_search_blocks * d.cap * kThreadsAtom);
         d.scr_bkt = c.take<unsigned char>((size_t)d.n_search_blocks * d.cap * kThreadsAtom);
+        d.scr_queue = c.take<uint32_t>((size_t)d.n_search_blocks * (d.cap + kQueueSlack) * kThreadsAtom);
     }
     d.part = many_body(prm) ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
     d.nbr_mirror = many_body(prm) ? c.take<unsigned short>(S * (size_t)d.cap * Npad) : nullptr;

@@ -35,6 +35,7 @@ constexpr int kMaxAtoms = 1 << 23;
 constexpr int kDnWeights = 8 * 16 + 2 * 8;  // CFNEB_POT_DNN: H <= 8, D <= 16
 constexpr int kInnerBuckets = 56;      // radial buckets of the list sort: uniform in r^2 on [0, r_cut^2)
 constexpr int kTailBuckets = 8;        // ... and on [r_cut^2, r_list^2)
+constexpr int kQueueSlack = 32;        // rows of the K1 candidate queue beyond the list capacity (prefilter margin)
 constexpr int kEdgeRows = 12;          // inner bucket edges from Dev::edge_b0 on whose list offsets are kept (Dev::nbr_edge)
 
 enum { DOT_PP = 0, DOT_MM, DOT_PM, DOT_GP, DOT_GM, DOT_GG, DOT_GV, DOT_PV, DOT_MV, DOT_VV };
@@ -146,6 +147,7 @@ struct Dev {
     int *rebuild_slots;       // [S] compact list of the slots that rebuild this step (K1)
     uint32_t *scr_tmp;        // [n_search_blocks][cap][128] unsorted column of the block's current work item (K1 scratch)
     unsigned char *scr_bkt;   // [n_search_blocks][cap][128] r^2 bucket of each unsorted entry
+    uint32_t *scr_queue;      // [n_search_blocks][cap + kQueueSlack][128] candidates that passed the fp32 prefilter, per atom
     int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
     int *bin_cursor;          // [S][nbins_max]
     int *bin_members;         // [S][Npad]

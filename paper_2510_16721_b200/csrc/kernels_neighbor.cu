@@ -161,7 +161,6 @@ __global__ void __launch_bounds__(256) rebuild_list_kernel(Dev d, int p_lo) {
 }
 
 constexpr int kRadialBuckets = kInnerBuckets + kTailBuckets;
-constexpr int kQueue = 32;
 #ifndef CFNEB_K1_DRAIN
 #define CFNEB_K1_DRAIN 4
 #endif
@@ -171,17 +170,18 @@ constexpr int kQueue = 32;
 constexpr int kDrain = CFNEB_K1_DRAIN, kScan = CFNEB_K1_SCAN;  // candidates per round of the drain / of the prefilter scan
 constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 #ifndef CFNEB_SEARCH_BLOCKS
-#define CFNEB_SEARCH_BLOCKS 5
+#define CFNEB_SEARCH_BLOCKS 6
 #endif
 // Round 2: the grid has a fixed size (CFNEB_SEARCH_BLOCKS blocks per multiprocessor) and takes its work items
 // (rebuilding image, block of 128 atoms) from the compact list of rebuild_list_kernel -- a step in which no list is
-// stale costs one exit per resident block instead of 77 616 -- and the unsorted column / bucket scratch of a block
-// is a region of its own, reused item after item (scr_tmp, scr_bkt: 143 KB per block), instead of two arrays of the
-// size of the list itself (round 1: 11.4 GB of workspace; DRAM writes per rebuild 2.8 -> 2.3 x the list: the 106 MB of
-// scratch of the resident blocks only partly stay in the L2).
+// stale costs one exit per resident block instead of 77 616 -- and the scratch of a block (candidate queue, unsorted
+// column, buckets: scr_queue, scr_tmp, scr_bkt, 274 KB per block at cap 224) is a region of its own, reused item after
+// item, instead of arrays of the size of the list itself (round 1: 11.4 GB of workspace).  The candidates that pass the
+// fp32 prefilter are queued for the whole environment and drained once (see `queue` below): 0.56 -> 0.43 ms per image
+// at c4; with the queue out of shared memory six blocks are resident (0.40) and the scan reads past short bins
+// instead of clamping its index (0.38).
 __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_search_kernel(Dev d) {
     __shared__ unsigned short s_hist[kRadialBuckets * kThreadsAtom];
-    __shared__ uint32_t s_queue[kQueue * kThreadsAtom];
     __shared__ int s_max;
     if (threadIdx.x == 0) s_max = 0;
     const int n_items = d.ctl->n_rebuild * d.nblk_atom;
@@ -193,7 +193,11 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
     int cnt = 0;
     bool bad_shift = false;
     unsigned short *hist = s_hist + threadIdx.x;
-    uint32_t *queue = s_queue + threadIdx.x;
+    // candidates that pass the prefilter wait in a queue long enough for a whole environment (global scratch of the
+    // block, L2-resident): ONE drain per atom.  With a 32-entry queue in shared memory the drain ran whenever any
+    // lane's queue was full, the average lane a third full: 413 rounds per warp for 153 neighbours per atom at c4.
+    const int kQueue = d.cap + kQueueSlack;
+    uint32_t *queue = d.scr_queue + (size_t)blockIdx.x * kQueue * kThreadsAtom + threadIdx.x;
     for (int b = 0; b < kRadialBuckets; ++b) hist[b * kThreadsAtom] = 0;
     const Geom *g = d.geom + slot;
     const int nb0 = g->nb[0], nb1 = g->nb[1], nb2 = g->nb[2];
@@ -296,7 +300,8 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
                 for (int t = 0; t < len_w; t += kScan) {
                     float4 cf[kScan];
 #pragma unroll
-                    for (int u = 0; u < kScan; ++u) cf[u] = binned_c[min(lo + t + u, max(hi - 1, 0))];
+                    // (reads past this lane's bin are masked by q < hi below; they stay inside the array and its slack)
+                    for (int u = 0; u < kScan; ++u) cf[u] = binned_c[lo + t + u];
 #pragma unroll
                     for (int u = 0; u < kScan; ++u) {
                         const int q = lo + t + u;
