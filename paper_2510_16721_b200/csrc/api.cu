@@ -167,7 +167,6 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         d.n_sm = sms;
         d.n_search_blocks = sms * search_blocks_per_sm();
-        d.scr_tmp = c.take<uint32_t>((size_t)d.n_search_blocks * d.cap * kThreadsAtom);
         d.scr_bkt = c.take<unsigned char>((size_t)d.n_search_blocks * d.cap * kThreadsAtom);
         d.scr_queue = c.take<uint32_t>((size_t)d.n_search_blocks * (d.cap + kQueueSlack) * kThreadsAtom);
     }

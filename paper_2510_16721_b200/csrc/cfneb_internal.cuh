@@ -145,9 +145,9 @@ struct Dev {
     unsigned short *nbr_mirror; // [S][cap][Npad] row of the mirror entry (j; i, -n) of each entry (many-body potentials only)
     double *part;             // [S][cap][3][Npad] partial forces p^ij = dU_i/dr^ij per list entry (many-body potentials only)
     int *rebuild_slots;       // [S] compact list of the slots that rebuild this step (K1)
-    uint32_t *scr_tmp;        // [n_search_blocks][cap][128] unsorted column of the block's current work item (K1 scratch)
     unsigned char *scr_bkt;   // [n_search_blocks][cap][128] r^2 bucket of each unsorted entry
-    uint32_t *scr_queue;      // [n_search_blocks][cap + kQueueSlack][128] candidates that passed the fp32 prefilter, per atom
+    uint32_t *scr_queue;      // [n_search_blocks][cap + kQueueSlack][128] candidates that passed the fp32 prefilter, per atom;
+                              // rewritten in place by the drain as the unsorted column of the block's current work item
     int *bin_count;           // [S][nbins_max + 1]  (counts, then exclusive starts)
     int *bin_cursor;          // [S][nbins_max]
     int *bin_members;         // [S][Npad]

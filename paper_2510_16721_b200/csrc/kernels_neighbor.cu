@@ -174,12 +174,12 @@ constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 #endif
 // Round 2: the grid has a fixed size (CFNEB_SEARCH_BLOCKS blocks per multiprocessor) and takes its work items
 // (rebuilding image, block of 128 atoms) from the compact list of rebuild_list_kernel -- a step in which no list is
-// stale costs one exit per resident block instead of 77 616 -- and the scratch of a block (candidate queue, unsorted
-// column, buckets: scr_queue, scr_tmp, scr_bkt, 274 KB per block at cap 224) is a region of its own, reused item after
-// item, instead of arrays of the size of the list itself (round 1: 11.4 GB of workspace).  The candidates that pass the
+// stale costs one exit per resident block instead of 77 616 -- and the scratch of a block (the candidate queue, which
+// the drain rewrites in place as the unsorted column, and the buckets: scr_queue, scr_bkt, 160 KB per block at cap 224)
+// is a region of its own, reused item after item, instead of arrays of the size of the list itself (round 1: 11.4 GB of workspace).  The candidates that pass the
 // fp32 prefilter are queued for the whole environment and drained once (see `queue` below): 0.56 -> 0.43 ms per image
 // at c4; with the queue out of shared memory six blocks are resident (0.40) and the scan reads past short bins
-// instead of clamping its index (0.38).
+// instead of clamping its index (0.38); unsorted column written over the queue (0.355).
 __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_search_kernel(Dev d) {
     __shared__ unsigned short s_hist[kRadialBuckets * kThreadsAtom];
     __shared__ int s_max;
@@ -226,7 +226,7 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
     const float rlf = (float)(d.r_list + 64.0 * 1.2e-7 * 2.0 * Lext * (1.0 + max(re0, max(re1, re2))));
     const float rl2f = rlf * rlf;
     uint32_t *__restrict__ list = d.nbr_list + (size_t)slot * d.cap * d.Npad + ic;
-    uint32_t *__restrict__ tmp = d.scr_tmp + (size_t)blockIdx.x * d.cap * kThreadsAtom + threadIdx.x;
+    uint32_t *tmp = queue;  // the drain writes accepted entry cnt <= c over the queue rows it has already read
     unsigned char *__restrict__ bkt = d.scr_bkt + (size_t)blockIdx.x * d.cap * kThreadsAtom + threadIdx.x;
     // radial buckets: kInnerBuckets uniform in r^2 below r_cut^2, kTailBuckets uniform between r_cut^2 and r_list^2
     const double rl2 = d.r_list * d.r_list, rc2 = d.r_cut * d.r_cut;
