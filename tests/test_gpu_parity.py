@@ -1200,6 +1200,38 @@ def test_nep_shaped_potential_with_the_rest_of_the_path():
     gpu.close()
 
 
+def test_nep_shaped_potential_hosted_step_and_resume():
+    """The four kernels of the NEP-shaped potential under the image-block selector of cfneb_step_hosted (each uploaded
+    block evaluated on its own) and under the list replay of cfneb_set_state: bit-identical to the resident band."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import diamond_strain_band, nep_params, two_sublattice_types
+    pot = nep_params(rc_r=5.6, rc_a=3.9, n_r=4, n_a=3, k_r=6, k_a=5, L=4, H=12, n_types=2, seed=5)
+    pos, cells = diamond_strain_band((2, 2, 3), 5.35, 7, 33, 0.06, ((0.0, 0.04, 0.0), (0.02, -0.03, 0.0), (0.0, 0.01, 0.05)))
+    types = two_sublattice_types(pos.shape[1], 2)
+    fire = dict(dt0=0.05, dtmax=0.1, maxstep=0.01, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+    prm = cf.default_params(potential=cf.POT_NEP, pot=list(pot), k_spring=1.0, climb=1, cell_factor=0.0, skin=0.3,
+                            max_neighbors=256, max_images=7, fire=fire, types=types)
+    a, b = cf.CFNEB(pos, cells, prm), cf.CFNEB(pos, cells, prm)
+    a.step(3)
+    b.step(3)
+    ck = b.get_checkpoint()
+    X, v, fs = np.ascontiguousarray(ck["X"]), np.ascontiguousarray(ck["v"]), ck["fire"]
+    for it in range(3):
+        a.step(1)
+        b.step_hosted(X, v, fs, 3)  # 5 movable images in blocks of 2, 2, 1
+        Xa, va = a.get_state()
+        assert np.array_equal(X, Xa) and np.array_equal(v, va), it
+    ck = a.get_checkpoint()
+    c = cf.CFNEB(pos, cells, prm)
+    c.set_state(ck["X"], ck["v"], ck["X_list"], ck["list_aux"], ck["fire"])
+    a.step(4)
+    c.step(4)
+    assert np.array_equal(a.get_state()[0], c.get_state()[0]) and np.array_equal(a.get_state()[1], c.get_state()[1])
+    for g in (a, b, c):
+        assert g.get_status().error == 0
+        g.close()
+
+
 def test_nep_shaped_potential_parameter_errors():
     """Out-of-range shapes are refused (workspace size 0); a type outside [0, n_types) is refused by cfneb_create."""
     import paper_2510_16721_b200 as cf
