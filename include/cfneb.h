@@ -305,7 +305,10 @@ CFNEB_API int cfneb_set_state(cfneb_t *h, const double *X, const double *v, cons
  * an image needs only its own coordinates for that -- while the later blocks are still on their way; only the
  * reductions, the FIRE scalars and the update wait for the last block ("structural information is always kept and
  * updated on GPU", is the fast path; this is the way to step a band that does not live there).  Synchronises.
- * Errors: CFNEB_EINVAL (null pointers, scalars out of range), CFNEB_ERANGE (4096 images or more).
+ * v == NULL: the velocities stay resident in the handle (an optimizer's internal state) and only the coordinates
+ * travel, half the bytes; fire == NULL: the FIRE scalars stay resident as well.  Still the same arithmetic bit for bit
+ * when X is the handle's own state handed back.
+ * Errors: CFNEB_EINVAL (null h or X, scalars out of range), CFNEB_ERANGE (4096 images or more).
  */
 CFNEB_API int cfneb_step_hosted(cfneb_t *h, double *X, double *v, cfneb_fire_state *fire, int32_t n_blocks);
 

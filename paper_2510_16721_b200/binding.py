@@ -337,12 +337,14 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_set_state")
 
-    def step_hosted(self, X, v, fire, n_blocks=0):
+    def step_hosted(self, X, v=None, fire=None, n_blocks=0):
         """cfneb_step_hosted: one iteration of a band whose state (X, v: C-contiguous float64 arrays, updated in place;
-        fire: FireState, updated in place) lives in host memory."""
-        if not (X.flags.c_contiguous and v.flags.c_contiguous and X.dtype == np.float64 and v.dtype == np.float64):
-            raise ValueError("X and v must be C-contiguous float64 arrays (they are updated in place)")
-        rc = lib().cfneb_step_hosted(self._h, _dptr(X), _dptr(v), ctypes.byref(fire), int(n_blocks))
+        fire: FireState, updated in place) lives in host memory.  v / fire None: that part stays resident in the handle."""
+        for arr in (X, v):
+            if arr is not None and not (arr.flags.c_contiguous and arr.dtype == np.float64):
+                raise ValueError("X and v must be C-contiguous float64 arrays (they are updated in place)")
+        rc = lib().cfneb_step_hosted(self._h, _dptr(X), _dptr(v), ctypes.byref(fire) if fire is not None else None,
+                                     int(n_blocks))
         if rc:
             raise CfnebError(rc, "cfneb_step_hosted")
 

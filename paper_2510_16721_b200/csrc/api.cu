@@ -908,8 +908,8 @@ int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *
 
 int cfneb_step_hosted(cfneb_t *h, double *X, double *v, cfneb_fire_state *fire, int32_t n_blocks) {
     DeviceGuard dev_guard(h);
-    if (!h || !X || !v || !fire || n_blocks < 0) return CFNEB_EINVAL;
-    if (!(fire->dt > 0.0) || !(fire->alpha >= 0.0) || fire->n_pos < 0 || fire->steps < 0) return CFNEB_EINVAL;
+    if (!h || !X || n_blocks < 0) return CFNEB_EINVAL;  // v, fire: optional (nullptr = that part of the state stays resident)
+    if (fire && (!(fire->dt > 0.0) || !(fire->alpha >= 0.0) || fire->n_pos < 0 || fire->steps < 0)) return CFNEB_EINVAL;
     { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
     const Dev &d = h->d;
     cudaStream_t st = h->st;
@@ -928,17 +928,18 @@ int cfneb_step_hosted(cfneb_t *h, double *X, double *v, cfneb_fire_state *fire, 
     // the copy stream starts after everything enqueued on the handle's stream so far (the staging area may be in use)
     CK(cudaEventRecord(h->ev_blocks[n_blocks], st));
     CK(cudaStreamWaitEvent(h->st2, h->ev_blocks[n_blocks], 0));
-    launch_import_aux(d, nullptr, 0, 1, fire->dt, fire->alpha, fire->n_pos, fire->first ? 1 : 0, (unsigned long long)fire->steps, st);
+    if (fire)
+        launch_import_aux(d, nullptr, 0, 1, fire->dt, fire->alpha, fire->n_pos, fire->first ? 1 : 0, (unsigned long long)fire->steps, st);
     h->interior_stale = false;
     for (int b = 0; b < n_blocks; ++b) {
         const int a = (int)((long long)P * b / n_blocks), e = (int)((long long)P * (b + 1) / n_blocks), cnt = e - a;
         if (cnt <= 0) continue;
         CK(cudaMemcpyAsync(dX + a * row, X + a * row, cnt * row * sizeof(double), cudaMemcpyHostToDevice, h->st2));
-        CK(cudaMemcpyAsync(dv + a * row, v + a * row, cnt * row * sizeof(double), cudaMemcpyHostToDevice, h->st2));
+        if (v) CK(cudaMemcpyAsync(dv + a * row, v + a * row, cnt * row * sizeof(double), cudaMemcpyHostToDevice, h->st2));
         CK(cudaEventRecord(h->ev_blocks[b], h->st2));
         CK(cudaStreamWaitEvent(st, h->ev_blocks[b], 0));
         // K0-K2 of an image need only that image's coordinates: the block is evaluated while the next ones arrive
-        launch_import_state(d, dX, dv, 1, a, cnt, st);
+        launch_import_state(d, dX, v ? dv : nullptr, 1, a, cnt, st);
         const int sel = image_block(a, cnt);
         launch_cell_prep(d, sel, MODE_STEP, st);
         launch_neighbor_build(d, sel, st);
@@ -953,18 +954,20 @@ int cfneb_step_hosted(cfneb_t *h, double *X, double *v, cfneb_fire_state *fire, 
     launch_reduce(d, st);
     launch_scalar(d, 0, st);
     launch_update(d, st);
-    launch_export_state(d, dX, dv, st);
+    launch_export_state(d, dX, v ? dv : nullptr, st);
     CK(cudaMemcpyAsync(X, dX, n * sizeof(double), cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(v, dv, n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (v) CK(cudaMemcpyAsync(v, dv, n * sizeof(double), cudaMemcpyDeviceToHost, st));
     Ctl c;
     CK(cudaMemcpyAsync(&c, d.ctl, sizeof c, cudaMemcpyDeviceToHost, st));
     int rc = sync_status(h);
     if (rc) return rc;
-    fire->dt = c.dt;
-    fire->alpha = c.alpha;
-    fire->steps = (int64_t)c.steps;
-    fire->n_pos = c.n_pos;
-    fire->first = c.first;
+    if (fire) {
+        fire->dt = c.dt;
+        fire->alpha = c.alpha;
+        fire->steps = (int64_t)c.steps;
+        fire->n_pos = c.n_pos;
+        fire->first = c.first;
+    }
     return CFNEB_OK;
 }
 

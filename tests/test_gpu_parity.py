@@ -516,6 +516,14 @@ def test_step_hosted_is_bit_identical_to_the_resident_band(k, n_blocks, over):
     with pytest.raises(cf.CfnebError):
         bad = cf.FireState(dt=-1.0, alpha=0.1, steps=0, n_pos=0, first=1)
         b.step_hosted(X, v, bad)
+    # positions only: the velocities and the FIRE scalars stay resident in the handle
+    for it in range(4):
+        a.step(1)
+        b.step_hosted(X, None, None, n_blocks)
+        Xa, va = a.get_state()
+        assert np.array_equal(X, Xa) and np.array_equal(b.get_state()[1], va), it
+    sa, sb = a.get_status(), b.get_status()
+    assert (sb.dt, sb.alpha, sb.n_pos, sb.steps, sb.fmax) == (sa.dt, sa.alpha, sa.n_pos, sa.steps, sa.fmax)
     a.close()
     b.close()
 
