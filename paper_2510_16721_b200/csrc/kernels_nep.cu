@@ -23,7 +23,8 @@
 //     time, ONE ROW PER LANE: a lane forms the pair vector, the angular basis and the expansions g_n of its row once,
 //     then the rows go round the quad by shuffles and every lane adds each row to the 35 moments of its own channel
 //     (registers); the moments are parked in a scratch array (one 280-byte column per atom and channel), the network
-//     runs with the quad's descriptors side by side in shared memory, and a second walk of the same shape evaluates
+//     runs on the fp64 tensor cores (a warp's eight quads are the eight rows of an m8n8k4 fragment; the quad's
+//     descriptors side by side in shared memory are the A operand), and a second walk of the same shape evaluates
 //     phi_n(u) = sum_c G_nc u^c and its gradient per channel and hands the three components back to the row's lane,
 //     which writes the angular partial force once.  Network weights and angular expansion coefficients sit in shared
 //     memory.  The radial descriptors act on the forces through w_i[J][k] = sum_n dU_i/dq_n cR[I][J][n][k], written
