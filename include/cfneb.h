@@ -317,6 +317,50 @@ CFNEB_API int cfneb_step_hosted(cfneb_t *h, double *X, double *v, cfneb_fire_sta
  * for endpoints), energies: P.  Any may be NULL.  Synchronises. */
 CFNEB_API int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, double *energies);
 
+/* Parity hook: the ten K4 dot products of every image at the CURRENT X (Eq. 1; ref [13] via P:20), taken by
+ * the band's own reduction (reduce_kernel + the second stage in scalar_kernel) in a dry evaluation that updates
+ * nothing, and the generalized force they were taken with.  With tau+ = X_{p+1} - X_p, tau- = X_p - X_{p-1}:
+ *   dots  P*10: {tau+.tau+, tau-.tau-, tau+.tau-, G.tau+, G.tau-, G.G, G.v, tau+.v, tau-.v, v.v} per image, all
+ *               (N+3) x 3 components (cell rows included); endpoint rows are zero;
+ *   coef  P*4:  {c1, c2, f.v, f.f} of K5's one-pass algebra, f = G + c1 tau+ + c2 tau- (zero for endpoints);
+ *   G     P*(N+3)*3: generalized force [F D^T ; G_cell] (Eq. 12, 17) in the layout of cfneb_get_state (zero rows for
+ *               endpoints).
+ * Any may be NULL.  Synchronises. */
+CFNEB_API int cfneb_get_dots(cfneb_t *h, double *dots, double *coef, double *G);
+
+/*
+ * The ten dot products of K4 for callers that cannot allocate device memory -- and cannot hand this library a
+ * workspace to carve either: a plug-in inside a host MD / optimiser code that received its arrays and no allocator, a
+ * process whose GPU memory was committed in full at start-up (a caching pool at its cap, a fixed MPS / MIG budget), a
+ * latency-bound loop that may not take the device-wide synchronisation cudaMalloc implies.  The block partials of the
+ * reduction live in a fixed array inside the library's own device image (640 KiB on every GPU that loads the library,
+ * held until the process exits); the call itself performs no cudaMalloc, cudaFree or other allocating call.
+ *   X, G, v: DEVICE pointers, n_images * n_dof doubles each, row-major [image][dof]: generalized coordinates,
+ *       generalized forces and FIRE velocities of the band (the layouts of cfneb_get_state and of cfneb_get_dots' G
+ *       with n_dof = 3 (N + 3); any n_dof >= 1 is accepted).  Read only; rows 0 and n_images-1 of G and v are not read.
+ *   dots: DEVICE pointer, n_images * 10 doubles, written: per image the ten numbers listed at cfneb_get_dots, rows 0
+ *       and n_images-1 zero.  Summation order is fixed: the same inputs give the same bits on every call.
+ *   cuda_stream: the cudaStream_t to enqueue on (NULL = legacy default stream).  Asynchronous: returns once the two
+ *       kernels are enqueued; `dots` is valid when the stream has reached that point.
+ * Limits: 3 <= n_images <= CFNEB_NOALLOC_MAX_IMAGES (the size of the fixed scratch); a longer band is refused with
+ * CFNEB_ERANGE and nothing is launched -- use a cfneb_create handle, whose scratch is sized by the caller's workspace.
+ * The device that owns the pointers and the stream must be the CURRENT device of the calling thread.
+ * First call on each device: the library looks up the device address of its scratch array (cudaGetSymbolAddress,
+ * which may also make the runtime load the library's device code on that GPU).  That is one-time set-up, not part of
+ * the steady state: make this first call before any CUDA stream capture is begun.
+ * Sharing: one scratch array per GPU serves all calls.  A call rewrites every slot it later reads, so it needs no
+ * clearing and is not affected by what the previous call left; but two calls that are in flight on the same GPU at the
+ * same time (two streams, two host threads) write the same slots and corrupt each other.  Issue them on one stream
+ * or order them with events.
+ * Errors: CFNEB_EINVAL (NULL or non-device pointer, pointer of another device, n_images < 3, n_dof < 1), CFNEB_ERANGE
+ * (n_images beyond the maximum), CFNEB_ECUDA; cfneb_band_dots_noalloc_error() returns the text of this thread's last
+ * failure of this call ("" after a success).
+ */
+#define CFNEB_NOALLOC_MAX_IMAGES 128
+CFNEB_API int cfneb_band_dots_noalloc(const double *X, const double *G, const double *v, int32_t n_images, int64_t n_dof,
+                                      double *dots, void *cuda_stream);
+CFNEB_API const char *cfneb_band_dots_noalloc_error(void);
+
 /* Parity hook: neighbour list of one image as built on the device for the current X:
  * count[N], list[N*cap] (entry k of atom i at list[i*cap + k]), shift[N*cap*3]; r^ij = (s_j - s_i + n) h.
  * cap = prm->max_neighbors.  Forces a fresh build of that image.  Synchronises. */

@@ -21,7 +21,7 @@ EXPORTS = (
     "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_adaptive", "cfneb_step_timed",
     "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_reparametrize", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
     "cfneb_get_path",
-    "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_step_hosted", "cfneb_get_forces", "cfneb_get_neighbors", "cfneb_get_status",
+    "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_step_hosted", "cfneb_get_forces", "cfneb_get_dots", "cfneb_band_dots_noalloc", "cfneb_band_dots_noalloc_error", "cfneb_get_neighbors", "cfneb_get_status",
     "cfneb_destroy", "cfneb_strerror", "cfneb_last_cuda_error", "cfneb_util_fp64_peak",
 )
 
@@ -97,7 +97,8 @@ def lib():
         ("cfneb_get_checkpoint", [vp, dp, dp, dp, dp, ctypes.POINTER(FireState)]),
         ("cfneb_set_state", [vp, dp, dp, dp, dp, ctypes.POINTER(FireState)]),
         ("cfneb_step_hosted", [vp, dp, dp, ctypes.POINTER(FireState), i32]),
-        ("cfneb_get_forces", [vp, dp, dp, dp, dp]), ("cfneb_get_neighbors", [vp, i32, ip, ip, ip]),
+        ("cfneb_get_forces", [vp, dp, dp, dp, dp]), ("cfneb_get_dots", [vp, dp, dp, dp]), ("cfneb_get_neighbors", [vp, i32, ip, ip, ip]),
+        ("cfneb_band_dots_noalloc", [vp, vp, vp, i32, ctypes.c_int64, vp, vp]),
         ("cfneb_get_status", [vp, ctypes.POINTER(Status)]), ("cfneb_util_fp64_peak", [vp, dp]),
     ):
         fn = getattr(L, name)
@@ -109,6 +110,8 @@ def lib():
     L.cfneb_strerror.argtypes = [ctypes.c_int]
     L.cfneb_last_cuda_error.restype = ctypes.c_char_p
     L.cfneb_last_cuda_error.argtypes = []
+    L.cfneb_band_dots_noalloc_error.restype = ctypes.c_char_p
+    L.cfneb_band_dots_noalloc_error.argtypes = []
     _lib = L
     return L
 
@@ -159,6 +162,34 @@ def fp64_peak_tflops():
     if rc:
         raise CfnebError(rc, "cfneb_util_fp64_peak")
     return out.value
+
+
+NOALLOC_MAX_IMAGES = 128  # CFNEB_NOALLOC_MAX_IMAGES of include/cfneb.h
+
+
+def band_dots_noalloc(X, G, v, out, stream=None):
+    """cfneb_band_dots_noalloc: the ten K4 dot products per image of a band given as CUDA tensors, for code that may not
+    allocate device memory: the reduction's scratch is a fixed array inside libcfneb.so, and this wrapper allocates
+    nothing either -- `out` is the caller's.  X, G, v: float64, contiguous, [P, ...] with the same number of elements
+    per image; out: float64, contiguous, P * 10 elements, same device; at most NOALLOC_MAX_IMAGES images.  Enqueued on
+    `stream` (default: torch's current stream on that device) and not waited for.  Calls share one scratch per GPU:
+    do not let two of them run concurrently on one device.  The first call on a device does one-time set-up and
+    should precede any stream capture."""
+    import torch
+    P = int(X.shape[0])
+    for name, t in (("X", X), ("G", G), ("v", v), ("out", out)):
+        if not (t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.device == X.device):
+            raise ValueError("%s must be a contiguous float64 CUDA tensor on %s" % (name, X.device))
+    if G.shape != X.shape or v.shape != X.shape or out.numel() != P * 10:
+        raise ValueError("G and v must have X's shape and out P * 10 elements")
+    n_dof = X.numel() // P if P else 0
+    with torch.cuda.device(X.device):
+        st = stream if stream is not None else torch.cuda.current_stream(X.device)
+        rc = lib().cfneb_band_dots_noalloc(ctypes.c_void_p(X.data_ptr()), ctypes.c_void_p(G.data_ptr()), ctypes.c_void_p(v.data_ptr()),
+                                           P, n_dof, ctypes.c_void_p(out.data_ptr()), ctypes.c_void_p(st.cuda_stream))
+    if rc:
+        raise CfnebError(rc, "cfneb_band_dots_noalloc: " + lib().cfneb_band_dots_noalloc_error().decode())
+    return out
 
 
 class CFNEB:
@@ -358,6 +389,16 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_get_forces")
         return F, V, fn, E
+
+    def get_dots(self, gen_force=True):
+        """cfneb_get_dots: (dots[P,10], coef[P,4], G[P,N+3,3]) of a dry evaluation at the current X."""
+        P = self.P
+        dots, coef = np.zeros((P, 10)), np.zeros((P, 4))
+        G = np.zeros((P, self.N + 3, 3)) if gen_force else None
+        rc = lib().cfneb_get_dots(self._h, _dptr(dots), _dptr(coef), _dptr(G))
+        if rc:
+            raise CfnebError(rc, "cfneb_get_dots")
+        return dots, coef, G
 
     def get_neighbors(self, image):
         cap = int(self.params.max_neighbors)

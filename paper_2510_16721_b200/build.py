@@ -13,7 +13,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcfneb.so")
 SOURCES = ["api.cu", "kernels_cell.cu", "kernels_neighbor.cu", "kernels_force.cu", "kernels_neb.cu",
            "kernels_update.cu", "kernels_relax.cu", "kernels_adapt.cu", "kernels_sw.cu", "kernels_dn.cu", "kernels_nep.cu",
-           "util_peak.cu"]
+           "util_peak.cu", "noalloc_dots.cu"]
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
          "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-cudart", "shared"]
 

@@ -995,6 +995,28 @@ int cfneb_get_forces(cfneb_t *h, double *F, double *virial, double *f_neb, doubl
     return sync_status(h);
 }
 
+int cfneb_get_dots(cfneb_t *h, double *dots, double *coef, double *G) {
+    DeviceGuard dev_guard(h);
+    if (!h) return CFNEB_EINVAL;
+    { int rc_m = sync_mirror(h); if (rc_m) return rc_m; }
+    const Dev &d = h->d;
+    const size_t P = h->P;
+    h->interior_stale = false;
+    launch_cell_prep(d, 1, MODE_STEP, h->st);
+    launch_neighbor_build(d, 1, h->st);
+    launch_force(d, 1, h->st);
+    launch_finalize(d, 1, h->st);
+    launch_reduce(d, h->st);
+    launch_scalar(d, 1, h->st);
+    launch_materialize_gen_force(d, h->st);
+    double *dD = static_cast<double *>(d.scratch), *dC = dD + P * kNDots;
+    launch_export_dots(d, dD, dC, h->st);
+    if (dots) CK(cudaMemcpyAsync(dots, dD, P * kNDots * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (coef) CK(cudaMemcpyAsync(coef, dC, P * 4 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    if (G) CK(cudaMemcpyAsync(G, d.fneb, P * (size_t)(d.N + 3) * 3 * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    return sync_status(h);
+}
+
 int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int32_t *list, int32_t *shift) {
     DeviceGuard dev_guard(h);
     if (!h) return CFNEB_EINVAL;

@@ -141,6 +141,44 @@ __global__ void materialize_fneb_kernel(Dev d) {
     }
 }
 
+// Parity hook (cfneb_get_dots): the generalized force G = [F D^T ; G_cell] (Eq. 12, 17) of every image in the
+// external layout [p][(N+3)][3] (zero rows for endpoints), written into the fneb buffer; and the K4 dot products and
+// K5 coefficients of a dry evaluation in path order.
+__global__ void materialize_gen_force_kernel(Dev d) {
+    const int p = blockIdx.y;
+    const int P = d.ctl->P;
+    if (p >= P) return;
+    const int rows = d.N + 3;
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= rows) return;
+    double *out = d.fneb + ((size_t)p * rows + (a < d.N ? d.perm[a] : a)) * 3;
+    if (p == 0 || p == P - 1) {
+        out[0] = out[1] = out[2] = 0.0;
+        return;
+    }
+    const int s0 = d.order[p];
+    if (a < d.N) {
+        const double *D = d.geom[s0].D;
+        const double *F = d.F + (size_t)s0 * 3 * d.Npad;
+        const double Fx = F[a], Fy = F[d.Npad + a], Fz = F[2 * (size_t)d.Npad + a];
+        for (int c = 0; c < 3; ++c) out[c] = Fx * D[3 * c] + Fy * D[3 * c + 1] + Fz * D[3 * c + 2];
+    } else {
+        for (int c = 0; c < 3; ++c) out[c] = d.Gc[s0 * 9 + 3 * (a - d.N) + c];
+    }
+}
+
+__global__ void export_dots_kernel(Dev d, double *dots_out, double *coef_out) {
+    const int P = d.ctl->P;
+    for (int i = threadIdx.x; i < P * kNDots; i += blockDim.x) {
+        const int p = i / kNDots, q = i % kNDots;
+        dots_out[i] = (p == 0 || p == P - 1) ? 0.0 : d.dots[d.order[p] * kNDots + q];
+    }
+    for (int i = threadIdx.x; i < P * 4; i += blockDim.x) {
+        const int p = i / 4, q = i % 4;
+        coef_out[i] = (p == 0 || p == P - 1) ? 0.0 : d.coef[d.order[p] * 4 + q];
+    }
+}
+
 // K7: new image = midpoint of two stored images in generalized coordinates (O9); v = 0; energy unknown.
 __global__ void midpoint_kernel(Dev d, int sa, int sb, int sn) {
     const size_t img = (size_t)3 * d.Npad, buf = (size_t)d.S * img;
@@ -363,6 +401,15 @@ int update_blocks_per_sm() { return 3; }
 void launch_materialize_fneb(const Dev &d, cudaStream_t st) {
     dim3 grid((d.N + 3 + 127) / 128, d.S);
     materialize_fneb_kernel<<<grid, 128, 0, st>>>(d);
+}
+
+void launch_materialize_gen_force(const Dev &d, cudaStream_t st) {
+    dim3 grid((d.N + 3 + 127) / 128, d.S);
+    materialize_gen_force_kernel<<<grid, 128, 0, st>>>(d);
+}
+
+void launch_export_dots(const Dev &d, double *dots_out, double *coef_out, cudaStream_t st) {
+    export_dots_kernel<<<1, 256, 0, st>>>(d, dots_out, coef_out);
 }
 
 void launch_midpoint(const Dev &d, int sa, int sb, int sn, cudaStream_t st) {

@@ -67,6 +67,12 @@ def test_workspace_bytes_and_argument_errors_need_no_device(cf):
     assert L.cfneb_set_state(None, None, None, None, None, None) == -1
     assert L.cfneb_step_hosted(None, None, None, None, 0) == -1 and L.cfneb_reparametrize(None, 1) == -1
     assert ctypes.sizeof(cf.FireState) == 32
+    assert L.cfneb_get_dots(None, None, None, None) == -1
+    # the no-allocation entry point checks its sizes before it touches the device
+    assert L.cfneb_band_dots_noalloc(None, None, None, 2, 10, None, None) == -1
+    assert L.cfneb_band_dots_noalloc(None, None, None, cf.NOALLOC_MAX_IMAGES + 1, 10, None, None) == -7
+    assert b"CFNEB_NOALLOC_MAX_IMAGES = 128" in L.cfneb_band_dots_noalloc_error()
+    assert re.search(r"#define\s+CFNEB_NOALLOC_MAX_IMAGES\s+128\b", open(os.path.join(ROOT, "include", "cfneb.h")).read())
     for code in range(0, -8, -1):
         assert len(L.cfneb_strerror(code)) > 1
     L.cfneb_destroy(None)  # documented no-op
