@@ -273,7 +273,11 @@ CFNEB_API int cfneb_get_state(cfneb_t *h, double *X, double *v);
  *   X_list    P*(N+3)*3: the generalized coordinates at which each image's neighbour list was last built (the
  *             order of a list's entries fixes the summation order of the forces, so a resume replays the builds);
  *   list_aux  P*4: per image {max_i |R~_i - R~_i(build)|^2 at the last cell map, max_i |dR~_i|^2 of the last update,
- *             iterations since the build, 0} -- the staleness accounting that decides the next rebuild;
+ *             iterations since the build, pending} -- the staleness accounting that decides the next rebuild; pending
+ *             is what calls made since the last iteration left for the next cell map: max_i |dR~_i|^2 of a
+ *             cfneb_set_path / cfneb_set_state / cfneb_reparametrize move, or -1 for an image whose list must be
+ *             rebuilt regardless (just inserted; its X_list row is then meaningless and cfneb_set_state ignores it).
+ *             A checkpoint may therefore be taken at any point between two calls, not only after a plain step;
  *   fire      the FIRE scalars and the iteration counter.
  * All HOST, any may be NULL.  Read only; synchronises.
  */

@@ -877,6 +877,13 @@ int cfneb_set_state(cfneb_t *h, const double *X, const double *v, const double *
     int rc;
     if (X_list) {  // replay the list builds: lists at X_list, then the coordinates proper
         CK(cudaMemcpyAsync(dX, X_list, n * sizeof(double), cudaMemcpyHostToDevice, st));
+        // an image whose rebuild was pending at the checkpoint (list_aux[4p+3] < 0: inserted and not yet stepped) has no
+        // build coordinates worth replaying -- an unused slot exports zeros, which are not a cell: its list is built at X
+        // here and, the flag restored below, again by the next K0, exactly as the uninterrupted band does
+        const size_t row = (size_t)(d.N + 3) * 3;
+        for (int p = 0; p < h->P; ++p)
+            if (list_aux[4 * p + 3] < 0.0)
+                CK(cudaMemcpyAsync(dX + p * row, X + p * row, row * sizeof(double), cudaMemcpyHostToDevice, st));
         launch_import_state(d, dX, nullptr, 0, 0, h->P, st);
         CK(cudaStreamSynchronize(st));
         rc = force_rebuild_all(h);

@@ -204,6 +204,7 @@ void launch_reparametrize(const Dev &d, int hold_climbing, cudaStream_t st) {
     int bx = (d.Npad + 255) / 256;
     if (bx > 64) bx = 64;
     dim3 grid(bx, d.S);
+    launch_pending_guard(d, 0, d.S, st);  // an earlier move not yet seen by K0: its displacement adds to this one
     reparam_apply_kernel<<<grid, 256, 0, st>>>(d);
     reparam_commit_kernel<<<592, 256, 0, st>>>(d);
 }

@@ -290,7 +290,10 @@ __global__ void export_state_kernel(Dev d, double *Xo, double *vo) {
 
 // Checkpoint, second half: the generalized coordinates each image's neighbour list was built at (Xb, Xcb) and the
 // staleness accounting {max |R~_i - R~_i(build)|^2 at the last K0, max |dR~_i|^2 of the last update, steps since
-// the build, 0} -- what cfneb_set_state needs to replay the list builds and continue bit for bit.
+// the build, pending} -- what cfneb_set_state needs to replay the list builds and continue bit for bit.  pending is
+// what host-side moves since the last K0 left for the next one: max |dR~_i|^2 of a path replacement / state import /
+// re-parametrisation (dispmax_in), or -1 when the image's list must be rebuilt whatever moved (a new image, whose
+// stored build coordinates mean nothing).
 __global__ void export_list_state_kernel(Dev d, double *Xo, double *aux) {
     const int p = blockIdx.y;
     const int P = d.ctl->P;
@@ -302,13 +305,25 @@ __global__ void export_list_state_kernel(Dev d, double *Xo, double *aux) {
         aux[4 * p + 0] = bits_nonneg(d.disptot[slot]);
         aux[4 * p + 1] = bits_nonneg(d.dispmax[slot]);
         aux[4 * p + 2] = (double)d.geom[slot].since;
-        aux[4 * p + 3] = 0.0;
+        aux[4 * p + 3] = d.geom[slot].force_rebuild ? -1.0 : bits_nonneg(d.dispmax_in[slot]);
     }
     if (a >= rows || !Xo) return;
     const double *Xb = d.Xb + (size_t)slot * 3 * d.Npad;
     const int ao = a < d.N ? d.perm[a] : a;
     for (int c = 0; c < 3; ++c)
         Xo[((size_t)p * rows + ao) * 3 + c] = a < d.N ? Xb[(size_t)c * d.Npad + a] : d.Xcb[slot * 9 + 3 * (a - d.N) + c];
+}
+
+// Host-side moves (state import with tracking, re-parametrisation) record their largest atomic displacement in
+// dispmax_in by atomicMax, which is right for the blocks of ONE move but not across moves: two moves with no K0
+// between them can add up (triangle inequality) while the maximum only keeps the larger.  Run before such a move:
+// an image that still carries an unconsumed displacement gets its list rebuilt by the next K0, whatever the sum is.
+__global__ void pending_guard_kernel(Dev d, int p_first, int count) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int p = p_first + k;
+    if (k >= count || p >= d.ctl->P) return;
+    const int slot = d.order[p];
+    if (d.dispmax_in[slot] != 0ull) d.geom[slot].force_rebuild = 1;
 }
 
 // Inverse of export_state_kernel: X (and v, if given) from the caller's layout into both coordinate buffers.
@@ -363,7 +378,9 @@ __global__ void import_aux_kernel(Dev d, const double *aux, int have_aux, int ha
         const int slot = d.order[p];
         d.disptot[slot] = nonneg_bits(aux[4 * p + 0]);
         d.dispmax[slot] = nonneg_bits(aux[4 * p + 1]);
-        d.dispmax_in[slot] = 0ull;
+        const double pending = aux[4 * p + 3];
+        d.dispmax_in[slot] = pending > 0.0 ? nonneg_bits(pending) : 0ull;
+        if (pending < 0.0) d.geom[slot].force_rebuild = 1;  // the replay built this list at X itself; K0 builds it again
         d.geom[slot].since = (int)aux[4 * p + 2];
     }
     if (p == 0 && have_fire) {
@@ -441,8 +458,14 @@ void launch_export_list_state(const Dev &d, double *Xl_out, double *aux_out, cud
 void launch_import_state(const Dev &d, const double *X_in, const double *v_in, int track, int p_first, int count,
                          cudaStream_t st) {
     if (count <= 0) return;
+    if (track) launch_pending_guard(d, p_first, count, st);
     dim3 grid((d.N + 3 + 127) / 128, count);
     import_state_kernel<<<grid, 128, 0, st>>>(d, X_in, v_in, track, p_first, count);
+}
+
+void launch_pending_guard(const Dev &d, int p_first, int count, cudaStream_t st) {
+    if (count <= 0) return;
+    pending_guard_kernel<<<(count + 127) / 128, 128, 0, st>>>(d, p_first, count);
 }
 
 void launch_import_aux(const Dev &d, const double *aux_in, int have_aux, int have_fire, double dt, double alpha, int n_pos,

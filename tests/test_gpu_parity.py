@@ -567,6 +567,89 @@ def test_hosted_step_and_checkpoint_after_image_control():
         g.close()
 
 
+@pytest.mark.parametrize("route", ["adaptive", "insert", "reparametrize", "set_state"])
+def test_checkpoint_between_calls_carries_the_pending_list_state(route):
+    """A checkpoint taken after a call that leaves work for the next cell map -- an image inserted on the device
+    (cfneb_step_adaptive ending on its control step) or on the host whose list is still to be built (its X_list row is
+    an unused slot's: not a cell), a re-parametrisation or a tracked state import whose displacement the staleness bound
+    has not seen yet -- resumes bit for bit in a new handle: list_aux[:, 3] carries that pending state."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(1)
+    prm = cf.params_for(spec, cell_factor=0.0, max_images=14)
+    a = cf.CFNEB(pos, cells, prm)
+    L0 = float(np.sum(a.get_segment_lengths()))
+    a.step(4)
+    if route == "adaptive":
+        a.step_adaptive(6, 3, L0 / 12.0, L0 / 48.0)          # the sixth iteration is followed by an insertion
+    elif route == "insert":
+        a.insert_image(2)
+    elif route == "reparametrize":
+        a.reparametrize(True)
+    else:
+        X, v = a.get_state()
+        X[1:-1, :-3] += 1e-3 * np.sin(np.arange(X[1:-1, :-3].size)).reshape(X[1:-1, :-3].shape)
+        a.set_state(X, v, None, None, a.get_checkpoint()["fire"])   # lists kept, the move recorded for the next K0
+    ck = a.get_checkpoint()
+    P = a.P
+    pending = ck["list_aux"][:, 3]
+    if route in ("adaptive", "insert"):
+        assert P > 9 and np.sum(pending < 0) == 1            # the new image: rebuild regardless
+    elif route == "reparametrize":
+        assert np.any(pending > 0) and np.all(pending >= 0)  # (an image the re-parametrisation left in place carries 0)
+    else:
+        assert np.all(pending[1:-1] > 0) and np.all(pending >= 0)
+    c = cf.CFNEB(pos, cells, prm)
+    while c.P < P:
+        c.insert_image(0)
+    c.step(2)
+    c.set_state(ck["X"], ck["v"], ck["X_list"], ck["list_aux"], ck["fire"])
+    assert c.get_status().error == 0
+    a.step(6)
+    c.step(6)
+    Xa, va = a.get_state()
+    Xc, vc = c.get_state()
+    assert np.array_equal(Xa, Xc) and np.array_equal(va, vc)
+    sa, sc = a.get_status(), c.get_status()
+    assert (sa.dt, sa.alpha, sa.n_pos, sa.fmax, sa.barrier, sa.steps) == (sc.dt, sc.alpha, sc.n_pos, sc.fmax, sc.barrier, sc.steps)
+    # and the accounting of the movable images continues identically (the restore itself runs one more cell map of
+    # the two endpoints, whose counters play no part in an iteration)
+    assert np.array_equal(a.get_checkpoint()["list_aux"][1:-1], c.get_checkpoint()["list_aux"][1:-1])
+    a.close()
+    c.close()
+
+
+def test_two_tracked_moves_in_a_row_rebuild_the_lists():
+    """Two state imports that keep the lists (cfneb_set_state without X_list), no iteration between them, each inside the
+    skin of the state before it but together outside the skin of the build: the second finds the first one's
+    displacement still pending and asks for a rebuild instead of keeping the larger of the two."""
+    import paper_2510_16721_b200 as cf
+    from cfneb_workloads import splitmix64_normals
+    from oracle import cfneb as oc
+    spec, pos, cells = build_workload(2, 5)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    X, _ = gpu.get_state()
+    kick = splitmix64_normals(92, X[1:-1, :-3].size).reshape(X[1:-1, :-3].shape)
+    kick /= np.max(np.linalg.norm(kick, axis=2))             # largest atomic displacement = 1 (in R~)
+    X1 = X.copy()
+    X1[1:-1, :-3] += 0.08 * kick
+    gpu.set_state(X1)
+    aux = gpu.get_checkpoint()["list_aux"]
+    assert np.all(aux[1:-1, 3] > 0) and np.all(aux[:, 3] >= 0)   # recorded, no rebuild asked for
+    X2 = X1.copy()
+    X2[1:-1, :-3] += 0.08 * kick
+    gpu.set_state(X2)
+    assert np.all(gpu.get_checkpoint()["list_aux"][1:-1, 3] == -1.0)
+    r0 = gpu.get_status().rebuilds
+    F, V, fneb, E = gpu.get_forces()
+    assert gpu.get_status().rebuilds == r0 + 3
+    p2, c2, _ = gpu.get_path()
+    orc = oc.CFNEB(p2, c2, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=spec.climb, cell_factor=0.0,
+                   fire=spec.fire, skin=spec.skin, max_neighbors=spec.max_neighbors)
+    orc.band.forces()
+    assert rel(E, orc.band.E) < TOL_FORCE and rel(F[1:-1], orc.evaluator.last["F"]) < TOL_FORCE
+    gpu.close()
+
+
 def test_reparametrize_edge_cases():
     """P = 3 with the single interior image held (nothing moves), P = 3 not held (the image goes to mid arc length),
     the small c0 box with periodic self-images, and two calls in a row (the second is the identity to round-off)."""
