@@ -162,13 +162,19 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.nbr_tail = c.take<unsigned short>(S * (size_t)kTailBuckets * Npad);
     d.nbr_edge = prm->potential == CFNEB_POT_NEP ? c.take<unsigned short>(S * (size_t)kEdgeRows * Npad) : nullptr;
     d.rebuild_slots = c.take<int>(S);
-    {   // K1 scratch: one region per resident block of the search kernel (sized for the largest device we know)
+    {   // K1 scratch: one region per resident block of the search kernel.  The SIZE is that of a fixed upper bound on
+        // the multiprocessor count (sm_100a parts have 148 or fewer), so that cfneb_workspace_bytes does not depend on
+        // which device -- if any -- is current when it is asked; the GRID uses the device that is current at
+        // cfneb_create, clamped to what the scratch holds.
+        constexpr int kScratchSMs = 160;
         int dev = 0, sms = 148;
         if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        else cudaGetLastError();
         d.n_sm = sms;
-        d.n_search_blocks = sms * search_blocks_per_sm();
-        d.scr_bkt = c.take<unsigned char>((size_t)d.n_search_blocks * d.cap * kThreadsAtom);
-        d.scr_queue = c.take<uint32_t>((size_t)d.n_search_blocks * (d.cap + kQueueSlack) * kThreadsAtom);
+        d.n_search_blocks = (sms < kScratchSMs ? sms : kScratchSMs) * search_blocks_per_sm();
+        const size_t nscr = (size_t)kScratchSMs * search_blocks_per_sm();
+        d.scr_bkt = c.take<unsigned char>(nscr * d.cap * kThreadsAtom);
+        d.scr_queue = c.take<uint32_t>(nscr * (d.cap + kQueueSlack) * kThreadsAtom);
     }
     d.part = many_body(prm) ? c.take<double>(S * (size_t)d.cap * 3 * Npad) : nullptr;
     d.nbr_mirror = many_body(prm) ? c.take<unsigned short>(S * (size_t)d.cap * Npad) : nullptr;
@@ -452,6 +458,7 @@ int cfneb_create(cfneb_t **out, int32_t n_atoms, const double *pos_init, const d
     d.edge_b0 = prm->potential == CFNEB_POT_NEP
                     ? (int)floor(prm->pot[1] * prm->pot[1] / (d.r_cut * d.r_cut) * kInnerBuckets) : 0;
     prepare_potential(d);
+    if (d.potential == CFNEB_POT_NEP) CKC(prepare_nep_kernels());
     if (set_reference_frame(h, cell_init, cell_final) != CFNEB_OK) { cfneb_destroy(h); return CFNEB_EINVAL; }
     h->P = n_images;
     h->order.resize(n_images);

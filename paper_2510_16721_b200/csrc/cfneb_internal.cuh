@@ -232,6 +232,7 @@ void launch_reparametrize(const Dev &d, int hold_climbing, cudaStream_t st);    
 void launch_relax_init(const Dev &d, cudaStream_t st);                                    // endpoint relaxation
 void launch_relax_step(const Dev &d, double fmax_tol, cudaStream_t st);
 void launch_segment_lengths(const Dev &d, double *out_dev, cudaStream_t st);
+cudaError_t prepare_nep_kernels();  // kernels_nep.cu: per-device kernel attributes, from cfneb_create
 void launch_pending_guard(const Dev &d, int p_first, int count, cudaStream_t st);
 void launch_materialize_gen_force(const Dev &d, cudaStream_t st);
 void launch_export_dots(const Dev &d, double *dots_out, double *coef_out, cudaStream_t st);

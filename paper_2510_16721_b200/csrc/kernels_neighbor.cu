@@ -115,18 +115,6 @@ __device__ inline void stencil_axis(int nb, int bi, int dlt, int &bj, int &m) {
     }
 }
 
-// One thread per atom, two phases per warp so that lanes stay converged:
-//   scan   every lane walks the same stencil cell (its own bin range of it) four candidates at a time -- four
-//          independent fp32 loads, a prefilter on fp32 Cartesian coordinates against r_list + margin -- and pushes
-//          the survivors (about one in six) onto a private queue in shared memory ([entry][thread]: bank = lane);
-//   flush  when some lane's queue is nearly full (or the stencil is done) all lanes drain their queues in step:
-//          the exact fp64 test |ds h|^2 < r_list^2, which alone decides membership, and the append of
-//          (j | code << 23) k-major to the atom's column of nbr_tmp with its r^2 bucket.
-// (A per-candidate `if (pass) { fp64 test }` ran the fp64 block in 55 % of the warp iterations for 16 % of the
-// lanes; ncu: 14.6 of 32 lanes active, 84 k warp instructions per warp.)  The column is then counting-sorted into
-// nbr_list (histogram kept in shared memory during the flushes).  Rows cnt..cap-1 are filled with a stand-in
-// entry (the atom itself shifted by -4 cell vectors along axis 0: farther than r_list whenever a list can be
-// built at all), so the force kernels read any row below cap without a bounds test and find it out of range.
 // Compact list of the images (slots) of the selected set whose list is rebuilt this step, in path order.
 __global__ void __launch_bounds__(256) rebuild_list_kernel(Dev d, int p_lo) {
     const int P = d.ctl->P;
@@ -180,10 +168,24 @@ constexpr uint32_t kCodeFar = 0u | (4u << 3) | (4u << 6);
 // fp32 prefilter are queued for the whole environment and drained once (see `queue` below): 0.56 -> 0.43 ms per image
 // at c4; with the queue out of shared memory six blocks are resident (0.40) and the scan reads past short bins
 // instead of clamping its index (0.38); unsorted column written over the queue (0.355).
+//
+// One thread per atom, two phases per warp so that lanes stay converged:
+//   scan   every lane walks the same stencil cell (its own bin range of it) kScan candidates at a time -- independent
+//          fp32 loads, a prefilter on fp32 Cartesian coordinates against r_list + margin -- and appends the survivors
+//          (about one in six) to its column of the block's candidate queue in global scratch ([row][thread]);
+//   drain  once per atom, after the whole stencil (earlier only if a lane's column is about to run out of rows, which
+//          takes more candidates than the list has capacity): all lanes in step, kDrain candidates per round, the exact
+//          fp64 test |ds h|^2 < r_list^2, which alone decides membership, and the accepted (j | code << 23) with its
+//          r^2 bucket written over the queue rows already read (the unsorted column) and to scr_bkt; histogram of the
+//          buckets in shared memory.
+// The column is then counting-sorted into nbr_list.  Rows cnt..cap-1 are filled with a stand-in entry (the atom itself
+// shifted by -4 cell vectors along axis 0: farther than r_list whenever a list can be built at all), so the force
+// kernels read any row below cap without a bounds test and find it out of range.
 __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_search_kernel(Dev d) {
     __shared__ unsigned short s_hist[kRadialBuckets * kThreadsAtom];
     __shared__ int s_max;
     if (threadIdx.x == 0) s_max = 0;
+    __syncthreads();  // before any thread's atomicMax on it
     const int n_items = d.ctl->n_rebuild * d.nblk_atom;
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {
     const int slot = d.rebuild_slots[item / d.nblk_atom];
@@ -226,28 +228,33 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
     const float rlf = (float)(d.r_list + 64.0 * 1.2e-7 * 2.0 * Lext * (1.0 + max(re0, max(re1, re2))));
     const float rl2f = rlf * rlf;
     uint32_t *__restrict__ list = d.nbr_list + (size_t)slot * d.cap * d.Npad + ic;
-    uint32_t *tmp = queue;  // the drain writes accepted entry cnt <= c over the queue rows it has already read
+    // The drain writes its accepted entries over the queue rows it has already read: the unsorted column is rows
+    // 0..cnt-1 of the queue.  Waiting candidates occupy rows q0..nq-1; q0 = 0 until a drain has run, then the number of
+    // accepted entries, so that candidates queued after a mid-scan drain land behind the column, not on it, and the
+    // drain's write row (cnt) never passes its read row (q0 + c: at most c entries were accepted since q0 = cnt).
+    uint32_t *tmp = queue;
     unsigned char *__restrict__ bkt = d.scr_bkt + (size_t)blockIdx.x * d.cap * kThreadsAtom + threadIdx.x;
     // radial buckets: kInnerBuckets uniform in r^2 below r_cut^2, kTailBuckets uniform between r_cut^2 and r_list^2
     const double rl2 = d.r_list * d.r_list, rc2 = d.r_cut * d.r_cut;
     const double bscale_in = (double)kInnerBuckets / rc2, bscale_tail = rl2 > rc2 ? (double)kTailBuckets / (rl2 - rc2) : 0.0;
-    int nq = 0;
+    int nq = 0, q0 = 0;
 
     auto flush = [&]() {
-        const int nq_w = __reduce_max_sync(0xffffffffu, nq);
+        const int nw = nq - q0;  // this lane's waiting candidates
+        const int nq_w = __reduce_max_sync(0xffffffffu, nw);
         // kDrain candidates per round: their queue entries and coordinates are requested together (the walk is
         // bound by the latency of these two dependent loads, not by their number)
         for (int c0 = 0; c0 < nq_w; c0 += kDrain) {
           uint32_t ee[kDrain];
           double4 cc[kDrain];
 #pragma unroll
-          for (int u = 0; u < kDrain; ++u) ee[u] = queue[min(c0 + u, kQueue - 1) * kThreadsAtom];
+          for (int u = 0; u < kDrain; ++u) ee[u] = queue[min(q0 + c0 + u, kQueue - 1) * kThreadsAtom];
 #pragma unroll
-          for (int u = 0; u < kDrain; ++u) cc[u] = binned[c0 + u < nq ? (int)(ee[u] & kIdxMask) : ic];
+          for (int u = 0; u < kDrain; ++u) cc[u] = binned[c0 + u < nw ? (int)(ee[u] & kIdxMask) : ic];
 #pragma unroll
           for (int u = 0; u < kDrain; ++u) {
             const int c = c0 + u;
-            if (c >= nq) continue;
+            if (c >= nw) continue;
             const uint32_t e = ee[u];
             const int m0 = (int)((e >> kShiftBits) & 7u) - 4, m1 = (int)((e >> (kShiftBits + 3)) & 7u) - 4,
                       m2 = (int)((e >> (kShiftBits + 6)) & 7u) - 4;
@@ -278,7 +285,7 @@ __global__ void __launch_bounds__(kThreadsAtom, CFNEB_SEARCH_BLOCKS) neighbor_se
             ++cnt;
           }
         }
-        nq = 0;
+        nq = q0 = min(cnt, d.cap);
     };
 
     for (int d0 = -re0; d0 <= re0; ++d0) {

@@ -647,6 +647,17 @@ static void launch_nep_radial(const Dev &d, int p_lo, dim3 grid, bool force, cud
     }
 }
 
+// The quad kernel's dynamic shared memory (network weights + expansion coefficients) passes the 48 KB default at the
+// larger shapes (H = 64, D = 40, two types: 48.6 KB): opt in.  The attribute belongs to the (function, device) pair, so
+// this runs in every cfneb_create with the handle's device current -- not once per process -- and its failure is an
+// error of that call.
+cudaError_t prepare_nep_kernels() {
+    cudaError_t e = cudaFuncSetAttribute(nep_partial_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nep_partial_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(nep_partial_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
+    return e;
+}
+
 // Four launches: radial descriptors (one atom per thread, all live rows), the quad kernel (angular rows, network,
 // angular partial forces), the radial forces pair by pair (one atom per thread, all live rows), pass 2 of the angular
 // partial forces over the angular rows (kernels_sw.cu), which adds to F and to the virial partials.
@@ -657,13 +668,6 @@ void launch_force_nep(const Dev &d, int p_lo, cudaStream_t st) {
     const dim3 grid(d.nblk_force, nimg), grid_r((d.N + kNepRadialThreads - 1) / kNepRadialThreads, nimg);
     const int KR = sp.kr <= 4 ? 4 : sp.kr <= 8 ? 8 : 12, KA = sp.ka <= 4 ? 4 : sp.ka <= 8 ? 8 : 12;
     const size_t smem = ((size_t)((sp.T * nep_net_size(sp) + 1) & ~1) + (size_t)sp.T * sp.T * kNepMaxN * KA) * sizeof(double);
-    static bool attr_set = false;
-    if (!attr_set) {
-        cudaFuncSetAttribute(nep_partial_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        cudaFuncSetAttribute(nep_partial_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        cudaFuncSetAttribute(nep_partial_kernel<12>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        attr_set = true;
-    }
     for (int force = 0; force < 2; ++force) {
         if (KR == 4) launch_nep_radial<4>(d, p_lo, grid_r, force, st);
         else if (KR == 8) launch_nep_radial<8>(d, p_lo, grid_r, force, st);
