@@ -23,11 +23,61 @@ def rel(a, b):
     return float(np.max(np.abs(a - b)) / (s if s > 0 else 1.0))
 
 
-def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_images=None, pressure=0.0, **over):
-    """(oracle band, GPU band) on configs[k] inputs."""
+def record_branches(orc):
+    """Instrument the ORACLE side of a parity pair: orc.branches collects which branch of the FIRE state machine (O7:
+    first / uphill / grow / downhill / clip = the step-length limit A4 was active) and of the improved tangent (O5:
+    up / down / ext+ / ext- / tie / flat) every oracle step takes, so that a test can assert the branches it claims to
+    compare -- a quiet change of a workload cannot un-test one.  Nothing of the CUDA path is read."""
+    orc.branches = set()
+    fire = orc.band.fire
+    inner = fire.step
+
+    def fire_step(f, n_rows):
+        if fire.first:
+            orc.branches.add("first")
+        elif np.sum(f * fire.v) > 0.0:
+            orc.branches.add("uphill")
+            if fire.n_pos > fire.nmin:
+                orc.branches.add("grow")
+        else:
+            orc.branches.add("downhill")
+        delta = inner(f, n_rows)
+        if np.sqrt(np.sum((fire.dt * fire.v) ** 2)) > fire.maxstep * np.sqrt(n_rows):
+            orc.branches.add("clip")
+            orc.clipped_steps = getattr(orc, "clipped_steps", 0) + 1
+        return delta
+
+    fire.step = fire_step
+    band = orc.band
+    inner_forces = band.forces
+
+    def forces():
+        f = inner_forces()
+        for p in range(1, band.P - 1):  # the energies the tangents of this evaluation were chosen from
+            Em, E0, Ep = band.E[p - 1], band.E[p], band.E[p + 1]
+            if Ep > E0 > Em:
+                orc.branches.add("up")
+            elif Ep < E0 < Em:
+                orc.branches.add("down")
+            elif Ep == E0 == Em:
+                orc.branches.add("flat")
+            else:
+                orc.branches.add("ext+" if Ep > Em else "ext-" if Ep < Em else "tie")
+        return f
+
+    band.forces = forces
+    return orc
+
+
+def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_images=None, pressure=0.0, fire=None, **over):
+    """(oracle band, GPU band) on configs[k] inputs; fire: overrides of the config's FIRE constants (both sides)."""
     import paper_2510_16721_b200 as cf
     from oracle import cfneb as oc
     spec, pos, cells = build_workload(k, n_images)
+    if fire:
+        import copy
+        spec = copy.copy(spec)                      # CONFIGS[k] itself is shared between tests
+        spec.fire = dict(spec.fire, **fire)
     climb = spec.climb if climb is None else climb
     orc = oc.CFNEB(pos, cells, spec.potential, spec.pot, spec.r_cut, k_spring=spec.k_spring, climb=climb,
                    cell_mode=cell_mode, cell_factor=cell_factor, fire=spec.fire, skin=spec.skin,
@@ -35,7 +85,7 @@ def make_pair(k, cell_factor=1.0, cell_mode=1, climb=None, n_images=None, max_im
     prm = cf.params_for(spec, cell_factor=cell_factor, cell_mode=cell_mode, climb=int(climb), max_images=max_images,
                         pressure=float(pressure), **over)
     gpu = cf.CFNEB(pos, cells, prm)
-    return spec, orc, gpu
+    return spec, record_branches(orc), gpu
 
 
 def first_step_exact(orc, gpu):
@@ -138,6 +188,14 @@ def test_neb_steps_match_oracle(k, lam, nsteps):
         assert abs(st.fmax - orc.band.fmax) <= 1e-8 * orc.band.fmax
         assert abs(st.dt - orc.band.fire.dt) < 1e-15 and abs(st.alpha - orc.band.fire.alpha) < 1e-15
         assert st.n_pos == orc.band.fire.n_pos
+    # the branches of O5 / O7 these trajectories compare (recorded on the oracle side); the step-length limit and the
+    # equal-energy tangents are not among them: test_step_length_limit_follows_oracle, test_equal_energy_tangents_*
+    want = {"first", "uphill", "downhill", "up", "ext+"}
+    if k != 2:
+        want |= {"down", "ext-"}
+    if nsteps >= 20:
+        want |= {"grow"}
+    assert want <= orc.branches and "clip" not in orc.branches, sorted(orc.branches)
     gpu.close()
 
 
@@ -153,6 +211,72 @@ def test_first_step_is_exact_to_1e9():
         assert rel(Xg - X0, Xo - X0) < TOL_STEP and rel(vg, vo) < TOL_STEP
         assert rel(Xg, Xo) < 1e-13
         gpu.close()
+
+
+@pytest.mark.parametrize("k,maxstep,pattern", [(0, 1e-4, "11111111"), (2, 1e-4, "11111111"), (0, 3e-3, "00111111"),
+                                               (2, 6e-3, "00111000")])
+def test_step_length_limit_follows_oracle(k, maxstep, pattern):
+    """Reading A4 (O7 step 3): the band's displacement is limited to maxstep sqrt((P-2)(N+3)) in the 2-norm.  K5 takes the
+    limit from its one-pass |v_new|^2 and K6 applies it as a factor on dt; the oracle clips the materialised Delta.
+    With maxstep this small the limit is active -- asserted on the oracle's own numbers -- from the first iteration
+    (pattern 1...) or from the third on, after two free ones (the switch-on inside a trajectory; on configs[2] a downhill
+    restart at the sixth iteration switches it off again).  A wrong row count in K5's limit (N for N + 3, P for P - 2)
+    changes the clipped step by percents."""
+    spec, orc, gpu = make_pair(k, cell_factor=0.0, fire=dict(maxstep=maxstep))
+    X0, _ = orc.get_state()
+    for n in range(1, 9):
+        Xb, _ = orc.get_state()
+        clipped_before = getattr(orc, "clipped_steps", 0)
+        orc.step(1)
+        gpu.step(1)
+        clipped = getattr(orc, "clipped_steps", 0) > clipped_before
+        assert clipped == (pattern[n - 1] == "1"), (n, clipped)
+        Xo, vo = orc.get_state()
+        Xg, vg = gpu.get_state()
+        if clipped:  # the oracle's step has exactly the limit's length
+            assert abs(np.linalg.norm(Xo[1:-1] - Xb[1:-1]) / (maxstep * np.sqrt((orc.P - 2) * (orc.N + 3))) - 1.0) < 1e-6
+        growth = 4.0 ** (n - 1) if n < 6 else 1e3
+        assert rel(Xg - X0, Xo - X0) < TOL_STEP * min(growth, 1e3), (n, rel(Xg - X0, Xo - X0))
+        assert rel(vg, vo) < TOL_STEP * min(growth, 1e3), (n, rel(vg, vo))
+        st = gpu.get_status()
+        assert abs(st.dt - orc.band.fire.dt) < 1e-15 and st.n_pos == orc.band.fire.n_pos and st.error == 0
+    assert "clip" in orc.branches and "first" in orc.branches and "uphill" in orc.branches
+    gpu.close()
+
+
+@pytest.mark.parametrize("climb", [True, False])
+def test_equal_energy_tangents_follow_oracle(climb):
+    """The equal-energy branches of the improved tangent (O5; reading A26: three equal energies -> bisector; E_{p+1} =
+    E_{p-1} -> the last branch) compared with the oracle, with energies that tie BITWISE on both sides by construction:
+    in the Eq. 14 coordinates (CELL_D, lam = 1) an image with deformation D R, R a rotation by pi about a cell axis
+    (two columns of D negated), has every pair vector r = ds h0 D R with two components negated exactly, hence the same
+    r^2, the same lists in the same order and the same energy bit for bit as the image with D -- while being a
+    different point of the band (the cell rows differ), so the tangents are not zero.  Images 1, 2, 3 and 5 are such
+    copies of one structure (flat at p = 2, ties at p = 4 with image 4 between them).  The state is an INPUT built from
+    the oracle's X; the ties are asserted on the oracle's own energies, then on the kernel's."""
+    spec, orc, gpu = make_pair(0, cell_factor=1.0, cell_mode=2, climb=climb)
+    X, _ = orc.get_state()
+    assert X.shape[0] == 7
+    Rx, Ry, Rz = np.array([1.0, -1.0, -1.0]), np.array([-1.0, 1.0, -1.0]), np.array([-1.0, -1.0, 1.0])
+    for p, R in ((2, Rz), (3, Rx), (5, Ry)):
+        X[p] = X[1]
+        X[p, -3:, :] = X[1, -3:, :] * R          # columns of D negated: D R
+    for p in range(1, 6):
+        orc.band.X[p] = X[p].copy()
+    gpu.set_state(X)
+    f_or = orc.band.forces()
+    Eo = orc.band.E
+    assert Eo[1] == Eo[2] == Eo[3] == Eo[5] and Eo[4] != Eo[3]
+    assert {"flat", "tie"} <= orc.branches, sorted(orc.branches)
+    F, V, fneb, E = gpu.get_forces()
+    assert E[1] == E[2] == E[3] == E[5] and E[4] != E[3]      # the kernel's K5 sees the ties as well
+    assert rel(E, Eo) < TOL_FORCE
+    for p in range(1, 6):
+        assert rel(fneb[p], f_or[p]) < TOL_STEP, (p, rel(fneb[p], f_or[p]))
+    assert gpu.get_status().climb_index == orc.band.pstar
+    first_step_exact(orc, gpu)
+    assert gpu.get_status().error == 0
+    gpu.close()
 
 
 def test_c0_converged_barrier_matches_oracle():
@@ -949,6 +1073,42 @@ def test_c2_converged_bain_barrier_equals_closed_form_saddle():
     gpu.close()
 
 
+def test_one_pass_projection_algebra_against_the_materialised_force_to_convergence():
+    """K5 never forms f^NEB: it takes f.f and f.v of every image from the ten K4 dot products (f = G + c1 tau+ + c2 tau-).
+    That is a difference of terms of the size of G.G, which stays O(10^2) per image on configs[2] while f.f falls with
+    fmax^2 -- so its ABSOLUTE error is what is bounded (a few ulp of (|G| + |c1||tau+| + |c2||tau-|)^2),
+    and its relative error grows as the band converges.  Compared here, along the whole run to fmax < 1e-6, with the same
+    sums over the materialised f^NEB of cfneb_get_forces ("keep a two-pass ... and compare"):
+    the absolute bound at every check; 1e-4 relative while fmax > 1e-4 (the convergence criteria of BASELINE.json's
+    configs are 1e-3 and 1e-4); and the band totals that drive FIRE stay positive -- K5's clamp of a negative f.f
+    does not fire -- and within 20 % down to fmax = 1e-6."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(2)
+    gpu = cf.CFNEB(pos, cells, cf.params_for(spec, cell_factor=0.0))
+    checks = 0
+    for _ in range(40):
+        gpu.step(100)
+        fmax = gpu.get_status().fmax
+        dots, coef, _ = gpu.get_dots(gen_force=False)
+        _, _, fneb, _ = gpu.get_forces(forces=False)
+        _, v = gpu.get_state()
+        d, c1, c2 = dots[1:-1], np.abs(coef[1:-1, 0]), np.abs(coef[1:-1, 1])
+        ff_mat = np.sum(fneb[1:-1] ** 2, axis=(1, 2))
+        fv_mat = np.sum(fneb[1:-1] * v[1:-1], axis=(1, 2))
+        size = np.sqrt(d[:, 5]) + c1 * np.sqrt(d[:, 0]) + c2 * np.sqrt(d[:, 1])      # |G| + |c1| |tau+| + |c2| |tau-|
+        assert np.all(np.abs(coef[1:-1, 3] - ff_mat) <= 2e-15 * size ** 2)
+        assert np.all(np.abs(coef[1:-1, 2] - fv_mat) <= 2e-15 * size * np.sqrt(d[:, 9]))
+        if fmax > 1e-4:
+            assert np.max(np.abs(coef[1:-1, 3] - ff_mat) / ff_mat) < 1e-4
+        tot1, totm = float(np.sum(coef[1:-1, 3])), float(np.sum(ff_mat))
+        assert tot1 > 0.0 and abs(tot1 - totm) < 0.2 * totm, (fmax, tot1, totm)
+        checks += 1
+        if fmax < 1e-6:
+            break
+    assert gpu.get_status().fmax < 1e-6 and checks >= 10 and float(np.sum(d[:, 5])) > 1e2   # G.G did not shrink with f
+    gpu.close()
+
+
 @pytest.mark.parametrize("k,over", [(0, dict(skin=0.0)), (2, dict(skin=0.0)), (2, dict(rebuild_every=1)),
                                     (2, dict(max_neighbors=144)), (2, dict(max_neighbors=145)),
                                     (0, dict(max_neighbors=97, skin=0.05))])
@@ -1100,6 +1260,27 @@ def test_stillinger_weber_many_body_forces_and_steps(dims, n_images):
     assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
     st = gpu.get_status()
     assert st.error == 0 and abs(st.barrier - orc.band.barrier) < 1e-9 * max(1.0, abs(orc.band.E[0]))
+    gpu.close()
+
+
+def test_stillinger_weber_step_length_limit_follows_oracle():
+    """The step-length limit (A4) on a many-body band: active on every compared iteration (asserted on the oracle)."""
+    import paper_2510_16721_b200 as cf
+    from oracle import cfneb as oc
+    pot, pos, cells = _sw_band((2, 2, 2), 5)
+    fire = dict(dt0=0.05, dtmax=0.5, maxstep=1e-5, nmin=5, finc=1.1, fdec=0.5, astart=0.1, fa=0.99)
+    orc = record_branches(oc.CFNEB(pos, cells, 2, pot, pot[2] * pot[1], k_spring=1.0, climb=True, cell_factor=0.0, fire=fire,
+                                   skin=0.3, max_neighbors=64))
+    gpu = cf.CFNEB(pos, cells, cf.default_params(potential=cf.POT_SW, pot=list(pot), k_spring=1.0, climb=1, cell_factor=0.0,
+                                                 skin=0.3, max_neighbors=64, max_images=5, fire=fire))
+    X0 = first_step_exact(orc, gpu)
+    orc.step(4)
+    gpu.step(4)
+    assert orc.clipped_steps == 5
+    Xo, vo = orc.get_state()
+    Xg, vg = gpu.get_state()
+    assert rel(Xg - X0, Xo - X0) < 1e-7 and rel(vg, vo) < 1e-7
+    assert gpu.get_status().error == 0
     gpu.close()
 
 
