@@ -173,7 +173,7 @@ __device__ __forceinline__ double fs_density(const FSc &c, uint32_t T, double r2
 // sees entries k, k + 1 (shift codes and the neighbours' 32-byte sectors).  Entries are fetched two iterations
 // and sectors one iteration ahead of use; the loop is unrolled over the two pipeline stages so that no register
 // is rotated.  Rows past an atom's count hold a stand-in entry that is out of range by construction
-// (kernels_neighbor.cu), and the list carries 8 rows of slack, so no load is predicated.
+// (kernels_neighbor.cu), and the list carries 16 rows of slack (api.cu carve()), so no load is predicated.
 template <class Body>
 __device__ __forceinline__ void walk_list(const uint32_t *__restrict__ lp, size_t stride, const double4 *Rc, int cnt_w,
                                           Body body) {

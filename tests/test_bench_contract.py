@@ -40,6 +40,11 @@ def test_bench_line_has_the_contract_keys():
     ss = d["steady_state"]
     assert ss["steps"] == 100 and ss["value"] > 0 and ss["unit"] == d["unit"] and "neighbor_rebuilds" in ss
     assert d["gpu_launches"] == 13 * 20                       # thirteen kernel nodes per captured iteration
+    assert 0 <= d["config"]["preroll_steps"] <= 150 and "traffic_source" in r
+    # the timed window is representative: within 5 % of the 100 steps that follow it, and the per-class breakdown
+    # (taken after both) does not exceed the step it is part of by more than that
+    assert abs(d["value"] - ss["value"]) < 0.05 * ss["value"], (d["value"], ss["value"])
+    assert d["kernels"]["force"]["ms_per_step"] <= 1.05 * d["ms_per_step"]
     assert set(("sm_mhz", "sm_max_mhz", "reasons")) <= set(d["clocks"])
 
 
