@@ -140,6 +140,19 @@ typedef struct cfneb_status {
     double path_length;     /* sum_p |X_{p+1} - X_p| at the last evaluation */
 } cfneb_status;
 
+/* One row of the per-iteration record kept on the device (cfneb_get_history): what cfneb_get_status would have
+ * reported had it been called right after that iteration. */
+#define CFNEB_HISTORY_LEN 1024
+typedef struct cfneb_history_entry {
+    int64_t step;           /* status.steps after the iteration (1 = the first iteration of the band) */
+    int64_t rebuilds;       /* neighbour-list rebuilds done so far */
+    int32_t n_images;       /* P during the iteration */
+    int32_t climb_index;    /* p* of the iteration, -1 if none */
+    double fmax;            /* O8: max row norm of the NEB force of the iteration */
+    double barrier;         /* O8: E_{p*} - E_0 at its evaluation */
+    double dt, alpha;       /* FIRE state after it */
+} cfneb_history_entry;
+
 /* The scalar part of a checkpoint: the FIRE state of the band (O7; one state for the whole band, A3) and the
  * iteration counter.  first = 1: the next step skips the power test (A2). */
 typedef struct cfneb_fire_state {
@@ -372,6 +385,19 @@ CFNEB_API int cfneb_get_neighbors(cfneb_t *h, int32_t image, int32_t *count, int
 
 /* Synchronise and report. */
 CFNEB_API int cfneb_get_status(cfneb_t *h, cfneb_status *out);
+
+/*
+ * The convergence record of the last iterations (the paper's convergence and energy-barrier plots, P:144, P:152,
+ * without a host synchronisation per step): K5 files one row per iteration in a ring of CFNEB_HISTORY_LEN rows in the
+ * workspace, whoever launched the iteration (cfneb_step, cfneb_step_adaptive, cfneb_step_timed, cfneb_step_hosted), so
+ * cfneb_step(h, 500) leaves 500 rows and this call is the only one that synchronises.
+ *   out[i], i = 0..n-1: the iteration after which status.steps == first_step + i; bit for bit the fields of a
+ *   cfneb_get_status taken at that point.  HOST, n entries.
+ * Errors: CFNEB_ERANGE if first_step < 1, if first_step + n - 1 exceeds the iterations done, if a requested row has been
+ * overwritten (more than CFNEB_HISTORY_LEN iterations ago) or was never written (the counter was moved by
+ * cfneb_set_state); the sticky device error otherwise.  Synchronises.
+ */
+CFNEB_API int cfneb_get_history(cfneb_t *h, int64_t first_step, int32_t n, cfneb_history_entry *out);
 
 CFNEB_API void cfneb_destroy(cfneb_t *h);
 CFNEB_API const char *cfneb_strerror(int code);

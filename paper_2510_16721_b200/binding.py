@@ -21,7 +21,7 @@ EXPORTS = (
     "cfneb_default_params", "cfneb_workspace_bytes", "cfneb_create", "cfneb_step", "cfneb_step_adaptive", "cfneb_step_timed",
     "cfneb_insert_image", "cfneb_delete_image", "cfneb_adapt", "cfneb_reparametrize", "cfneb_relax_endpoints", "cfneb_get_segment_lengths",
     "cfneb_get_path",
-    "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_step_hosted", "cfneb_get_forces", "cfneb_get_dots", "cfneb_band_dots_noalloc", "cfneb_band_dots_noalloc_error", "cfneb_get_neighbors", "cfneb_get_status",
+    "cfneb_set_path", "cfneb_get_state", "cfneb_get_checkpoint", "cfneb_set_state", "cfneb_step_hosted", "cfneb_get_forces", "cfneb_get_dots", "cfneb_band_dots_noalloc", "cfneb_band_dots_noalloc_error", "cfneb_get_neighbors", "cfneb_get_status", "cfneb_get_history",
     "cfneb_destroy", "cfneb_strerror", "cfneb_last_cuda_error", "cfneb_util_fp64_peak",
 )
 
@@ -58,6 +58,16 @@ class FireState(ctypes.Structure):
     """cfneb_fire_state (include/cfneb.h)."""
     _fields_ = [("dt", ctypes.c_double), ("alpha", ctypes.c_double), ("steps", ctypes.c_int64),
                 ("n_pos", ctypes.c_int32), ("first", ctypes.c_int32)]
+
+
+class HistoryEntry(ctypes.Structure):
+    """cfneb_history_entry (include/cfneb.h)."""
+    _fields_ = [("step", ctypes.c_int64), ("rebuilds", ctypes.c_int64), ("n_images", ctypes.c_int32),
+                ("climb_index", ctypes.c_int32), ("fmax", ctypes.c_double), ("barrier", ctypes.c_double),
+                ("dt", ctypes.c_double), ("alpha", ctypes.c_double)]
+
+
+HISTORY_LEN = 1024  # CFNEB_HISTORY_LEN
 
 
 class CfnebError(RuntimeError):
@@ -100,6 +110,7 @@ def lib():
         ("cfneb_get_forces", [vp, dp, dp, dp, dp]), ("cfneb_get_dots", [vp, dp, dp, dp]), ("cfneb_get_neighbors", [vp, i32, ip, ip, ip]),
         ("cfneb_band_dots_noalloc", [vp, vp, vp, i32, ctypes.c_int64, vp, vp]),
         ("cfneb_get_status", [vp, ctypes.POINTER(Status)]), ("cfneb_util_fp64_peak", [vp, dp]),
+        ("cfneb_get_history", [vp, ctypes.c_int64, i32, ctypes.POINTER(HistoryEntry)]),
     ):
         fn = getattr(L, name)
         fn.restype = ctypes.c_int
@@ -298,6 +309,14 @@ class CFNEB:
         if rc:
             raise CfnebError(rc, "cfneb_get_status")
         return s
+
+    def get_history(self, first_step, n):
+        """cfneb_get_history: list of n HistoryEntry, the iterations first_step .. first_step + n - 1."""
+        out = (HistoryEntry * int(n))()
+        rc = lib().cfneb_get_history(self._h, int(first_step), int(n), out)
+        if rc:
+            raise CfnebError(rc, "cfneb_get_history")
+        return list(out)
 
     @property
     def P(self):

@@ -128,6 +128,7 @@ size_t carve(int32_t N, const cfneb_params *prm, void *base, Dev *out) {
     d.order = c.take<int>(S);
     d.free_stack = c.take<int>(S);
     d.seglen = c.take<double>(2 * S);
+    d.hist = c.take<double>((size_t)kHistLen * kHistFields);
     d.plan_q = c.take<int>(S);
     d.plan_t = c.take<double>(S);
     d.perm = c.take<int>(Npad);
@@ -1077,6 +1078,38 @@ int cfneb_get_status(cfneb_t *h, cfneb_status *out) {
     out->path_length = c.path_length;
     CK(cudaGetLastError());
     return CFNEB_OK;
+}
+
+int cfneb_get_history(cfneb_t *h, int64_t first_step, int32_t n, cfneb_history_entry *out) {
+    DeviceGuard dev_guard(h);
+    if (!h || !out || n < 0) return CFNEB_EINVAL;
+    if (n == 0) return CFNEB_OK;
+    std::vector<double> ring((size_t)kHistLen * kHistFields);
+    Ctl c;
+    CK(cudaMemcpyAsync(ring.data(), h->d.hist, ring.size() * sizeof(double), cudaMemcpyDeviceToHost, h->st));
+    CK(cudaMemcpyAsync(&c, h->d.ctl, sizeof c, cudaMemcpyDeviceToHost, h->st));
+    CK(cudaStreamSynchronize(h->st));
+    const int64_t last = (int64_t)c.steps;
+    if (first_step < 1 || first_step + n - 1 > last || first_step + kHistLen <= last) return CFNEB_ERANGE;
+    for (int32_t i = 0; i < n; ++i) {
+        const int64_t s = first_step + i;  // the iteration after which status.steps == s; its row: index s - 1
+        const double *row = ring.data() + (size_t)((s - 1) % kHistLen) * kHistFields;
+        if (row[0] != (double)s) return CFNEB_ERANGE;  // not recorded (the counter was set by cfneb_set_state) or overwritten
+        double f2 = row[1];
+        if (s == last) {  // K6 of the last iteration left its maximum in the control block; no later K5 has filed it yet
+            const unsigned long long b = c.fmax_bits;
+            memcpy(&f2, &b, sizeof f2);
+        }
+        out[i].step = s;
+        out[i].rebuilds = (int64_t)row[7];
+        out[i].n_images = (int32_t)row[6];
+        out[i].climb_index = (int32_t)row[3];
+        out[i].fmax = sqrt(f2);
+        out[i].barrier = row[2];
+        out[i].dt = row[4];
+        out[i].alpha = row[5];
+    }
+    return c.error;
 }
 
 void cfneb_destroy(cfneb_t *h) {

@@ -26,6 +26,8 @@ constexpr int kThreadsAtom = 128;      // neighbour / position / many-body kerne
 constexpr int kThreadsPair = CFNEB_PAIR_THREADS;  // pair-potential K2 kernels (density, force): 1 atom per thread
 constexpr int kThreadsStream = 256;    // K4 / K6: 2 atoms per thread (double2)
 constexpr int kAtomsPerStreamBlock = kThreadsStream * 2;
+constexpr int kHistLen = CFNEB_HISTORY_LEN;  // iterations kept in the per-step record (ring), cfneb_get_history
+constexpr int kHistFields = 8;          // steps after the iteration, |f|max^2, barrier, p*, dt, alpha, P, rebuilds
 constexpr int kNDots = 10;             // pp, mm, pm, Gp, Gm, GG, Gv, pv, mv, vv
 constexpr int kNForcePart = 10;        // E pair, Vxx, Vyy, Vzz, Vxy, Vxz, Vyz, E site (embedding / many-body), low words of [0], [7]
 constexpr uint32_t kIdxMask = 0x7FFFFFu;
@@ -107,6 +109,7 @@ struct Dev {
     Ctl *ctl;
     int *order;               // [S] path position -> slot
     int *free_stack;          // [S] unused slots (device-side adaptive control)
+    double *hist;             // [kHistLen][kHistFields] per-iteration record written by K5 (row = iteration index mod kHistLen)
     double *seglen;           // [2 S] segment lengths of the last control step; second half: running arc length
     int *plan_q;              // [S] re-parametrisation: image p moves onto segment plan_q[p] ...
     double *plan_t;           // [S] ... at the fraction plan_t[p] (kernels_adapt.cu)

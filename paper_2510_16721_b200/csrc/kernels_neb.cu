@@ -259,6 +259,12 @@ __global__ void __launch_bounds__(1024) scalar_kernel(Dev d, int dry) {
         ctl->barrier = (pb > 0) ? d.E[d.order[pb]] - d.E[d.order[0]] : 0.0;
     }
     if (dry) return;
+    if (ctl->steps > 0ull) {  // per-step record: the previous iteration's max row norm^2, complete now that its K6 has run
+        double f2;
+        const unsigned long long b = ctl->fmax_bits;
+        memcpy(&f2, &b, sizeof f2);
+        d.hist[((ctl->steps - 1ull) % kHistLen) * kHistFields + 1] = f2;
+    }
     ctl->fmax_bits = 0ull;  // K6 of this step takes the max row norm of f (O8)
     // ---- FIRE (O7) ----
     double dt = ctl->dt, alpha = ctl->alpha, cv, cf;
@@ -301,6 +307,18 @@ __global__ void __launch_bounds__(1024) scalar_kernel(Dev d, int dry) {
     ctl->src = ctl->cur;
     ctl->dst = 1 - ctl->cur;
     ctl->cur = 1 - ctl->cur;
+    {   // per-step record (cfneb_get_history): what cfneb_get_status would report after this iteration, except its
+        // fmax, which K6 is about to produce (filed by the next K5, or read from the control block for the last one)
+        double *row = d.hist + (ctl->steps % kHistLen) * kHistFields;
+        row[0] = (double)(ctl->steps + 1ull);
+        row[1] = 0.0;
+        row[2] = ctl->barrier;
+        row[3] = (double)pstar;
+        row[4] = dt;
+        row[5] = alpha;
+        row[6] = (double)P;
+        row[7] = (double)ctl->rebuilds;
+    }
     ctl->steps += 1ull;
 }
 

@@ -808,6 +808,37 @@ def test_reparametrize_edge_cases():
     g.close()
 
 
+def test_history_of_a_long_launch_equals_status_snapshots_step_by_step():
+    """cfneb_get_history after ONE cfneb_step(200) -- no host synchronisation in between -- returns, bit for bit, what
+    cfneb_get_status reports on a twin band stepped one iteration at a time (fmax, barrier, climbing index, dt, alpha,
+    P, rebuild count); the ring keeps the last CFNEB_HISTORY_LEN iterations and refuses what it no longer has."""
+    import paper_2510_16721_b200 as cf
+    spec, pos, cells = build_workload(0)
+    prm = cf.params_for(spec, cell_factor=0.0, rebuild_every=7)
+    a, b = cf.CFNEB(pos, cells, prm), cf.CFNEB(pos, cells, prm)
+    a.step(200)
+    hist = a.get_history(1, 200)
+    for s in range(1, 201):
+        b.step(1)
+        st, e = b.get_status(), hist[s - 1]
+        assert (e.step, e.rebuilds, e.n_images, e.climb_index, e.fmax, e.barrier, e.dt, e.alpha) == (
+            st.steps, st.rebuilds, st.n_images, st.climb_index, st.fmax, st.barrier, st.dt, st.alpha), s
+    assert len({e.dt for e in hist}) > 3 and hist[-1].rebuilds > hist[0].rebuilds and hist[-1].fmax < hist[0].fmax
+    tail = a.get_history(150, 51)
+    assert [e.step for e in tail] == list(range(150, 201)) and tail[-1].fmax == a.get_status().fmax
+    for first, n in ((0, 5), (190, 12), (201, 1)):
+        with pytest.raises(cf.CfnebError) as err:
+            a.get_history(first, n)
+        assert err.value.code == cf.binding.ERANGE
+    a.step(cf.HISTORY_LEN)                                   # the ring wraps: iterations 1 .. 200 are gone
+    with pytest.raises(cf.CfnebError):
+        a.get_history(200, 1)
+    wrapped = a.get_history(201, cf.HISTORY_LEN)
+    assert [e.step for e in wrapped] == list(range(201, 201 + cf.HISTORY_LEN)) and a.get_status().error == 0
+    a.close()
+    b.close()
+
+
 def test_neighbor_list_reuse_equals_fresh_lists():
     """Verlet-list reuse (skin) must not change the result: rebuild_every = 1 forces fresh lists each step."""
     import paper_2510_16721_b200 as cf
